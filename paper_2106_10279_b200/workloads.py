@@ -1,0 +1,99 @@
+"""Seeded, synthetic workload definitions shared by the CUDA path, the oracle, the tests and bench.py.
+
+This module holds INPUTS only — process descriptors, the synthetic gluon PDF table and the initial VEGAS
+grid — and none of the method's arithmetic.  It imports neither the CUDA binding nor the oracle.
+
+The five configurations are BASELINE.json `configs[0..4]` (C0..C4).  They stand in for the
+paper's workloads, pp -> t tbar (+jets) at sqrt(s) = 13 TeV with an LHAPDF set through PDFFlow and
+pT > 30 GeV cuts, which cannot be run here (no LHAPDF grids, no MG5_aMC).
+"""
+from dataclasses import dataclass, replace
+import math
+
+import numpy as np
+
+MF_EE_MUMU, MF_GG_TT, MF_GG_TTG, MF_GG_TTGG = 0, 1, 2, 3
+GEV2_TO_PB = 0.3894e9  # BASELINE.json configs[0]: use this literal everywhere
+N_BINS = 50
+N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18}
+N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4}
+VEGAS_ALPHA = 1.5
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    process: int
+    sqrt_s: float
+    alpha_em: float = 1.0 / 132.507
+    alpha_s: float = 0.118
+    m_top: float = 173.0
+    mu2: float = 173.0 ** 2
+    ptmin: float = 0.0
+    etamax: float = 0.0
+    drmin: float = 0.0
+    gev2_to_pb: float = GEV2_TO_PB
+    n_bins: int = N_BINS
+    n_events: int = 0          # events per iteration
+    n_iterations: int = 0      # total iterations
+    n_adapt: int = 0           # iterations after which the grid is refined (the rest run on a frozen grid)
+    unweight: bool = False     # frozen iterations run mf_unweight
+    seed: int = 0
+
+    @property
+    def n_dims(self):
+        return N_DIMS[self.process]
+
+    @property
+    def n_final(self):
+        return N_FINAL[self.process]
+
+    def scaled(self, n_events, n_iterations=None, n_adapt=None):
+        """Same physics at a reduced size (parity tests run the oracle at sizes it finishes in seconds)."""
+        it = self.n_iterations if n_iterations is None else n_iterations
+        ad = min(self.n_adapt, it) if n_adapt is None else n_adapt
+        return replace(self, n_events=n_events, n_iterations=it, n_adapt=ad)
+
+
+C0 = Workload("C0 e+e- -> mu+mu-", MF_EE_MUMU, sqrt_s=100.0, n_events=1_000_000, n_iterations=5, n_adapt=5)
+C1 = Workload("C1 gg -> ttbar", MF_GG_TT, sqrt_s=13000.0, n_events=2 ** 20, n_iterations=10, n_adapt=10)
+C2 = Workload("C2 gg -> ttbar g", MF_GG_TTG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5, n_events=2 ** 22,
+              n_iterations=10, n_adapt=10)
+C3 = Workload("C3 gg -> ttbar gg", MF_GG_TTGG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5, drmin=0.4,
+              n_events=2 ** 22, n_iterations=10, n_adapt=10)
+C4 = Workload("C4 gg -> ttbar gg + unweighting", MF_GG_TTGG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5, drmin=0.4,
+              n_events=2 ** 26, n_iterations=10, n_adapt=5, unweight=True)
+CONFIGS = [C0, C1, C2, C3, C4]
+
+
+def pdf_table(nx=100, nq=50):
+    """Synthetic gluon table of BASELINE.json configs[1]:
+    x g(x,Q) = 3 x^-0.1 (1-x)^5 (1 + 0.1 ln(Q^2/100 GeV^2)) on nx log-spaced x knots in [1e-9, 1] and
+    nq log-spaced Q^2 knots in [2.72, 1e10] GeV^2.  Returns (lnx[nx], lnq2[nq], xf[nx, nq]) in fp64.
+    The PDF the method uses is the INTERPOLANT of this table, not the formula."""
+    i = np.arange(nx, dtype=np.float64)
+    lnx = math.log(1e-9) * (1.0 - i / (nx - 1))
+    lnx[-1] = 0.0
+    j = np.arange(nq, dtype=np.float64)
+    lnq2 = math.log(2.72) + j * (math.log(1e10) - math.log(2.72)) / (nq - 1)
+    x = np.exp(lnx)
+    x[-1] = 1.0
+    q2 = np.exp(lnq2)
+    xf = 3.0 * x[:, None] ** -0.1 * (1.0 - x[:, None]) ** 5 * (1.0 + 0.1 * np.log(q2[None, :] / 100.0))
+    return np.ascontiguousarray(lnx), np.ascontiguousarray(lnq2), np.ascontiguousarray(xf)
+
+
+def uniform_grid(n_dims, n_bins=N_BINS):
+    """Initial VEGAS grid: edges e_{d,i} = i / n_bins, shape [n_dims, n_bins + 1]."""
+    e = np.arange(n_bins + 1, dtype=np.float64) / n_bins
+    e[-1] = 1.0
+    return np.ascontiguousarray(np.tile(e, (n_dims, 1)))
+
+
+def rambo_test_point(n):
+    """The fixed uniforms of SURVEY.md §8(c) 'golden points': for final particle i,
+    (rho1..rho4) = (0.15+0.2i, 0.35+0.15i, 0.55-0.1i, 0.25+0.1i)."""
+    rho = []
+    for i in range(n):
+        rho += [0.15 + 0.2 * i, 0.35 + 0.15 * i, 0.55 - 0.1 * i, 0.25 + 0.1 * i]
+    return np.array(rho, dtype=np.float64)
