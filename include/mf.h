@@ -1,0 +1,118 @@
+/* mf.h — C ABI of the B200-native MadFlow leading-order integrand hot path.
+ *
+ * What the library computes ("generation of random numbers, computation of the phase space
+ * kinematics, matrix element evaluation and histogram accumulation"; L27 VEGAS + PDF interpolation;
+ * L65-67 helicity-summed matrix elements from HELAS-style routines; L71-75 RAMBO; L81-83 unweighting;
+ * BASELINE.json north_star fixes the rest): for every event index k in [first_event, first_event+n_events)
+ *
+ *   Philox4x32-10(seed, iteration, k) -> uniforms -> VEGAS map -> (x1, x2) -> phase space (2-body / RAMBO)
+ *   -> lab boost + cuts -> PDF -> |M|^2 (helicity and colour summed) -> weight w
+ *
+ * in ONE fused CUDA pass, then reduces sum w, sum w^2, max|w|, n_pass and the per-dimension VEGAS
+ * histograms of w^2.  Nothing per event touches HBM except the records mf_unweight accepts.
+ * DESIGN.md states every reading of the paper (R1..R15) the arithmetic follows.
+ *
+ * Conventions
+ *  - All functions return int: MF_OK (0) or a negative error code.  No exceptions, no aborts, no printing.
+ *  - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors); pointers named h_* and
+ *    the mf_process_desc fields are HOST pointers.  `stream` is a cudaStream_t passed as void* (NULL = the
+ *    legacy default stream).
+ *  - The library allocates device memory only in mf_create_process and frees it only in
+ *    mf_destroy_process.  The hot calls never allocate, never synchronise the stream and never touch host
+ *    memory: they are asynchronous, results are valid after the caller synchronises `stream`.
+ *  - A handle is used from one stream at a time (it owns per-block partial-sum scratch).
+ *  - There is no CPU fallback: without a CUDA device mf_create_process returns MF_ECUDA.
+ */
+#ifndef MF_H
+#define MF_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mf_process mf_process; /* opaque; owns its device-side constants and scratch */
+
+/* process ids: BASELINE.json configs[0..3] */
+enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3 };
+enum { MF_OK = 0, MF_EINVAL = -1, MF_ECUDA = -2, MF_EOVERFLOW = -3, MF_ERANGE = -4, MF_ENOMEM = -5 };
+
+/* Process descriptor (host memory; copied at create).  Same field order as the oracle's mfo_process_desc. */
+typedef struct {
+  int32_t process;            /* enum above; fixes n_final, D (2/4/14/18), helicities, colour matrix   */
+  double sqrt_s;              /* GeV; hadronic (pp) for processes 1-3, leptonic for 0                   */
+  double alpha_em, alpha_s;   /* couplings: e^2 = 4 pi alpha_em, g_s^2 = 4 pi alpha_s                   */
+  double m_top;               /* GeV; width 0                                                           */
+  double mu2;                 /* mu_F^2 = mu_R^2 in GeV^2 (fixed scale)                                  */
+  double ptmin, etamax, drmin;/* cuts on the final-state gluons; <= 0 disables each                     */
+  double gev2_to_pb;          /* 0.3894e9                                                               */
+  int32_t n_bins;             /* VEGAS bins per dimension, 2..MF_MAX_BINS                               */
+  int32_t pdf_nx, pdf_nq;     /* knots of the PDF table (0, 0 for MF_EE_MUMU)                           */
+  const double *pdf_lnx;      /* [pdf_nx] ln x knots, increasing, last = 0                              */
+  const double *pdf_lnq2;     /* [pdf_nq] ln Q^2 knots, increasing                                      */
+  const double *pdf_xf;       /* [pdf_nx][pdf_nq] x*g(x,Q^2), row-major xf[ix*nq+iq]                    */
+} mf_process_desc;
+#define MF_MAX_BINS 128
+
+/* Per-iteration sums (device memory, written by the finalize kernel of each hot call). */
+typedef struct {
+  double sum_w, sum_w2, max_abs_w; /* signed sum of w, sum of w^2, max |w| over the events of the call  */
+  uint64_t n_pass, n_accept;       /* events passing the cuts; events accepted (mf_unweight only)      */
+} mf_iter_result;
+
+/* Creates a handle.  Errors: NULL / bad enum / n_bins out of range / bad table -> MF_EINVAL;
+ * mu2 outside the Q^2 knots or tau_min below the x knots -> MF_ERANGE; no device or CUDA failure ->
+ * MF_ECUDA; device allocation failure -> MF_ENOMEM.  On error *out is set to NULL. */
+int mf_create_process(const mf_process_desc *desc, mf_process **out);
+int mf_destroy_process(mf_process *p);
+int mf_n_dims(const mf_process *p, int32_t *D);              /* VEGAS dimensions: 2, 4, 14, 18          */
+int mf_n_final(const mf_process *p, int32_t *n);             /* final-state particles: 2, 2, 3, 4       */
+int mf_record_size(const mf_process *p, int32_t *bytes);     /* (n_final+2)*32 + 16                     */
+int mf_debug_row_len(const mf_process *p, int32_t *n_doubles);/* 3*D + 4*(n_final+2) + 9                */
+const char *mf_last_error(const mf_process *p);              /* static or handle-owned string           */
+/* launch geometry of the fused pass (blocks, threads per block), for reporting */
+int mf_launch_config(const mf_process *p, int32_t *blocks, int32_t *threads);
+
+/* One VEGAS iteration (steps a1-a12 of SURVEY.md 8(a)): events
+ * [first_event, first_event+n_events) of Philox stream (seed, iteration), mapped through
+ * d_grid[D][n_bins+1] (edges, row-major).  Writes d_hist[D][n_bins] = sum of w^2 per bin (overwritten) and
+ * *d_result.  d_hist may be NULL.  n_events may be 0 (all outputs zero). */
+int mf_vegas_iterate(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                     uint64_t n_events, double *d_hist, mf_iter_result *d_result, void *stream);
+
+/* VEGAS grid refinement (step a13; Lepage's smoothing + damping r = ((s-1)/ln s)^alpha + rebinning), in
+ * place on d_grid from d_hist.  A dimension whose histogram is all zero is left unchanged. */
+int mf_refine_grid(mf_process *p, double *d_grid, const double *d_hist, double alpha, void *stream);
+
+/* Same pass plus hit-or-miss unweighting (step a14): event k is accepted iff
+ * r_k * w_max < |w_k| with r_k the Philox accept draw; accepted events are appended to d_records
+ * (array of structs of mf_record_size bytes: (n_final+2) lab-frame four-momenta (E,px,py,pz), beams first,
+ * as doubles; signed w as double; event id as uint64).  *d_count is an in/out cursor: every accepted event
+ * advances it, only slots < capacity are written, so *d_count > capacity after synchronising IS the
+ * overflow signal.  Record order is unspecified (sort by event id).  d_hist may be NULL. */
+int mf_unweight(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                uint64_t n_events, double w_max, void *d_records, uint64_t capacity, uint64_t *d_count,
+                double *d_hist, mf_iter_result *d_result, void *stream);
+
+/* Test/diagnostic: per-event rows of mf_debug_row_len doubles, identical to the oracle's layout:
+ * x[D] | (n+2)x(E,px,py,pz) lab, beams first | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D] */
+int mf_debug_eval(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                  uint64_t n_events, double *d_out, void *stream);
+
+/* Test/diagnostic: raw Philox4x32-10 words for blocks (event, iteration, block) of stream `seed`:
+ * d_out[4*n] uint32, block index b of event first_event+k at d_out[4*(k*n_blocks+b)..]. */
+int mf_debug_philox(uint64_t seed, uint32_t iteration, uint64_t first_event, uint64_t n_events, uint32_t n_blocks,
+                    uint32_t *d_out, void *stream);
+/* Test/diagnostic: general 2-D log-bicubic PDF lookup x*g(x, q2) for n points (device arrays). */
+int mf_debug_pdf(mf_process *p, const double *d_x, const double *d_q2, uint64_t n, double *d_out, void *stream);
+/* Test/diagnostic: averaged |M|^2 at n sets of CM-frame momenta d_mom[n][n_final+2][4] (beams first). */
+int mf_debug_me2(mf_process *p, const double *d_mom, uint64_t n, double *d_out, void *stream);
+
+/* Measurement helper: runs a dependent-free DFMA chain on every SM for `iters` iterations and returns the
+ * achieved FP64 rate in flop/s (2 flop per DFMA) in *h_flops.  Synchronous.  Used by bench.py for the
+ * "alu" roofline denominator (FP64 peak is not in MEASURED_PEAKS.json). */
+int mf_measure_fp64_peak(int64_t iters, double *h_flops, double *h_ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

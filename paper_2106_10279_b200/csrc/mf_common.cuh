@@ -1,0 +1,42 @@
+// mf_common.cuh — shared definitions of the CUDA path (product code; shares nothing with oracle/).
+#pragma once
+#include <stdint.h>
+#include <math.h>
+
+#if defined(__CUDACC__)
+#define MF_HD __host__ __device__ __forceinline__
+#define MF_D __device__ __forceinline__
+#else
+#define MF_HD inline
+#define MF_D inline
+#endif
+
+namespace mf {
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+constexpr double kTwoPi = 6.28318530717958647692528676655900577;
+
+// Static description of the four processes (BASELINE.json configs[0..3]).
+//   D      VEGAS dimensions           NF  final-state particles
+//   NG     gluons incl. the two beams NGF final-state gluons (the ones the cuts act on)
+template <int PROC> struct Traits;
+template <> struct Traits<0> { static constexpr int D = 2, NF = 2, NG = 0, NGF = 0; };
+template <> struct Traits<1> { static constexpr int D = 4, NF = 2, NG = 2, NGF = 0; };
+template <> struct Traits<2> { static constexpr int D = 14, NF = 3, NG = 3, NGF = 1; };
+template <> struct Traits<3> { static constexpr int D = 18, NF = 4, NG = 4, NGF = 2; };
+
+// Scalars every kernel needs (passed by value in the launch).
+struct Params {
+  double s;            // (sqrt_s)^2
+  double alpha_em, alpha_s, m_top, mu2;
+  double ptmin, etamax, drmin;
+  double gev2_to_pb;
+  double tau_min, ln_tau_min;
+  double me_norm;      // coupling^n / (spin, colour, identical-particle averaging)
+  int n_bins;
+  int pdf_nx, pdf_nq;
+  int pdf_jq;          // Q^2 cell of mu2 (clamped), fixed per process
+  double pdf_uq;       // (ln mu2 - lnq2[jq]) / (lnq2[jq+1]-lnq2[jq])
+};
+
+}  // namespace mf

@@ -1,0 +1,84 @@
+// Test-only shim: compiles the PRODUCT's __host__ __device__ per-event code for the host so that the
+// `-m "not gpu"` tests can compare its arithmetic with the oracle without a GPU.  It is not part of the
+// product library (libmadflow_b200.so has no host evaluation path) and is loaded only by tests/.
+#include <cstring>
+#include "../../paper_2106_10279_b200/csrc/mf_event.cuh"
+
+using namespace mf;
+
+extern "C" {
+
+// averaged |M|^2 at CM-frame momenta mom[(n+2)][4], beams first (oracle layout)
+double mfh_me2(int process, const double* mom, double m_top, double alpha_s, double alpha_em) {
+  Params P;
+  std::memset(&P, 0, sizeof(P));
+  P.alpha_em = alpha_em; P.alpha_s = alpha_s; P.m_top = m_top;
+  double shat = 4.0 * mom[0] * mom[0];
+  double gs2 = 4.0 * kPi * alpha_s;
+  double k[4][4];
+  int nf = process <= 1 ? 2 : process + 1;
+  for (int i = 0; i < nf; ++i) for (int m = 0; m < 4; ++m) k[i][m] = mom[(2 + i) * 4 + m];
+  switch (process) {
+    case 0: return matrix_element<0>(P, shat, k);
+    case 1: P.me_norm = gs2 * gs2 / 256.0; return matrix_element<1>(P, shat, k);
+    case 2: P.me_norm = gs2 * gs2 * gs2 / 256.0; return matrix_element<2>(P, shat, k);
+    case 3: P.me_norm = gs2 * gs2 * gs2 * gs2 / 512.0; return matrix_element<3>(P, shat, k);
+  }
+  return -1.0;
+}
+
+void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {
+  U4 r = philox_block(seed, iteration, event, block);
+  out[0] = r.x; out[1] = r.y; out[2] = r.z; out[3] = r.w;
+}
+double mfh_uniform52(uint32_t hi, uint32_t lo) { return uniform52(hi, lo); }
+
+double mfh_pdf_2d(const double* lnx, const double* lnq2, const double* xf, int nx, int nq, double x, double q2) {
+  return pdf_xf_2d(lnx, lnq2, xf, nx, nq, x, q2);
+}
+// collapsed-row path used by the fused pass
+double mfh_pdf_row(const double* lnx, const double* lnq2, const double* xf, int nx, int nq, double x, double q2) {
+  double lq = log(q2);
+  int jq = find_cell(lnq2, nq, lq);
+  double uq = (lq - lnq2[jq]) / (lnq2[jq + 1] - lnq2[jq]);
+  double row[512];
+  for (int i = 0; i < nx; ++i) row[i] = pdf_collapse_q2(xf, lnq2, nq, i, jq, uq);
+  return pdf_xf_row(lnx, row, nx, x);
+}
+
+}  // extern "C"
+
+// full per-event chain on the host: writes x1, x2, phi, jac_vegas, jac_parton, pass, me2(if pass), momenta(lab)
+template <int PROC>
+static void event_host(const Params& P, const double* grid, uint64_t seed, uint32_t it, uint64_t e, double* out) {
+  Event<PROC> ev;
+  Bins<PROC> bins;
+  DebugRow dbg = {nullptr, Traits<PROC>::D, Traits<PROC>::NF};
+  generate_event<PROC>(P, grid, seed, it, e, ev, bins, dbg);
+  out[0] = ev.x1; out[1] = ev.x2; out[2] = ev.phi; out[3] = ev.jac_vegas; out[4] = ev.jac_parton;
+  out[5] = ev.pass ? 1.0 : 0.0;
+  out[6] = ev.pass ? matrix_element<PROC>(P, ev.shat, ev.k) : 0.0;
+  out[7] = ev.shat;
+  for (int i = 0; i < Traits<PROC>::NF; ++i) for (int m = 0; m < 4; ++m) out[8 + 4 * i + m] = ev.k[i][m];
+  for (int d = 0; d < Traits<PROC>::D; ++d) out[8 + 16 + d] = (double)bins.get(d);
+}
+extern "C" {
+
+void mfh_event(int process, const double* grid, int n_bins, double sqrt_s, double m_top, double alpha_s,
+               double alpha_em, double ptmin, double etamax, double drmin, double tau_min, uint64_t seed,
+               uint32_t it, uint64_t e, double* out) {
+  Params P;
+  std::memset(&P, 0, sizeof(P));
+  P.s = sqrt_s * sqrt_s; P.alpha_em = alpha_em; P.alpha_s = alpha_s; P.m_top = m_top;
+  P.ptmin = ptmin; P.etamax = etamax; P.drmin = drmin; P.n_bins = n_bins;
+  P.tau_min = tau_min; P.ln_tau_min = tau_min > 0 ? log(tau_min) : 0.0;
+  double gs2 = 4.0 * kPi * alpha_s;
+  switch (process) {
+    case 0: event_host<0>(P, grid, seed, it, e, out); break;
+    case 1: P.me_norm = gs2 * gs2 / 256.0; event_host<1>(P, grid, seed, it, e, out); break;
+    case 2: P.me_norm = gs2 * gs2 * gs2 / 256.0; event_host<2>(P, grid, seed, it, e, out); break;
+    case 3: P.me_norm = gs2 * gs2 * gs2 * gs2 / 512.0; event_host<3>(P, grid, seed, it, e, out); break;
+  }
+}
+
+}  // extern "C"
