@@ -1,0 +1,59 @@
+"""Builds paper_2106_10279_b200/libmadflow_b200.so (the C-ABI library of include/mf.h) in-tree with nvcc for
+sm_100a.  No GPU is needed to build (nvcc cross-compiles).
+
+    python -m paper_2106_10279_b200.build [--force] [--verbose]
+
+Steps: (1) csrc/gen_me.py writes the straight-line matrix-element code (the role of the paper's exporter
+plugin); (2) nvcc compiles csrc/madflow_b200.cu into the shared library.
+"""
+import glob
+import importlib.util
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libmadflow_b200.so")
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+
+
+def _sources():
+    return (glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh")) +
+            glob.glob(os.path.join(CSRC, "*.py")) + [os.path.join(os.path.dirname(HERE), "include", "mf.h")])
+
+
+def generate():
+    spec = importlib.util.spec_from_file_location("_mf_gen_me", os.path.join(CSRC, "gen_me.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return mod.main()
+
+
+def needs_build():
+    if not os.path.exists(LIB):
+        return True
+    t = os.path.getmtime(LIB)
+    return any(os.path.getmtime(f) > t for f in _sources())
+
+
+def build(force=False, verbose=False):
+    if not force and not needs_build():
+        return LIB
+    generate()
+    cmd = [NVCC] + FLAGS + ["-o", LIB, os.path.join(CSRC, "madflow_b200.cu")]
+    r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    log = os.path.join(HERE, "build.log")
+    with open(log, "w") as f:
+        f.write(" ".join(cmd) + "\n" + r.stdout)
+    if verbose or r.returncode != 0:
+        sys.stderr.write(r.stdout)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed (see %s)" % log)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

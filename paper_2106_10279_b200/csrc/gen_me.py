@@ -77,6 +77,24 @@ def colour_matrix(n):
 
 
 # ----------------------------------------------------------------------------------------------------
+# fp64 operations (adds + multiplies as written; an FMA counts 2) of each primitive of mf_me_prims.cuh
+FLOPS = {"rdot": 7, "radd": 4, "rsub": 4, "rscale": 4, "v3_acc": 65, "v4_acc": 49, "slash_col": 42, "slash_row": 42,
+         "spin_acc": 8, "prop_col": 66, "prop_row": 66, "sdot": 32, "bilinear": 72, "cdot_r": 14}
+
+
+def count_flops(line):
+    """static operation count of one emitted source line"""
+    import re
+    n = sum(FLOPS[f] * len(re.findall(r"\b%s\(" % f, line)) for f in FLOPS)
+    if line.lstrip().startswith(("const double Ar", "const double Ai")):
+        n += line.count(" + ") + line.count(" - ")          # amplitude = signed sum of terms
+    if line.lstrip().startswith(("g =", "g +=")):
+        n += 3 + (1 if "+=" in line else 0)                  # Ar*Ar + Ai*Ai (+ accumulate)
+    if "acc +=" in line or "total +=" in line:
+        n += 2 if "*" in line else 1
+    return n
+
+
 class Emitter:
     def __init__(self, n):
         self.n = n
@@ -286,11 +304,17 @@ def generate(n):
                 E.emit("  acc += %.1f * g;" % v)
             E.emit("  total += acc;")
             E.emit("}")
+    pre = sum(count_flops(l) for l in out) + 1 * sum(l.count("1.0 /") for l in out)
+    body = sum(count_flops(l) for l in E.lines)
+    flops = pre + (1 << n) * body
     for l in E.lines:
         w("    " + l)
     w("  }")
     w("  return total * (1.0 / %.1f);" % Cden)
     w("}")
+    w("// static fp64 operation count of the code above (adds + multiplies as written, FMA = 2; divisions = 1):")
+    w("//   per event %d = preamble %d + %d polarisation combinations x %d" % (flops, pre, 1 << n, body))
+    w("constexpr double kFlopsMe2_%dg = %d.0;" % (n - 2, flops))
     return "\n".join(out)
 
 

@@ -1,0 +1,300 @@
+// madflow_b200.cu — the C ABI of include/mf.h over the sm_100a kernels.  Host side only does argument
+// checking, launch geometry and kernel launches; every step of the hot path runs on the device.
+#include <cuda_runtime.h>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/mf.h"
+#include "mf_aux_kernels.cuh"
+
+static_assert(sizeof(mf::IterResult) == sizeof(mf_iter_result), "result layouts must agree");
+static_assert(mf::kMaxBins == MF_MAX_BINS, "bin limits must agree");
+
+struct mf_process {
+  int process = 0, D = 0, NF = 0;
+  mf::Params P;
+  double *d_lnx = nullptr, *d_lnq2 = nullptr, *d_xf = nullptr, *d_row = nullptr;  // PDF table + collapsed row
+  mf::BlockPartial* d_partials = nullptr;
+  double* d_hist_part = nullptr;
+  int blocks = 0, threads = mf::kThreads;
+  int blocks_unw = 0;
+  size_t smem = 0;
+  char err[256] = {0};
+};
+
+namespace {
+
+const char* kNullHandle = "null handle";
+
+int fail(mf_process* p, int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (p) {
+    if (e != cudaSuccess) snprintf(p->err, sizeof(p->err), "%s: %s", what, cudaGetErrorString(e));
+    else snprintf(p->err, sizeof(p->err), "%s", what);
+  }
+  return code;
+}
+
+template <int PROC, bool UNW> const void* pass_fn() { return (const void*)mf::fused_pass_kernel<PROC, UNW>; }
+const void* pass_fn(int proc, bool unw) {
+  switch (proc) {
+    case 0: return unw ? pass_fn<0, true>() : pass_fn<0, false>();
+    case 1: return unw ? pass_fn<1, true>() : pass_fn<1, false>();
+    case 2: return unw ? pass_fn<2, true>() : pass_fn<2, false>();
+    default: return unw ? pass_fn<3, true>() : pass_fn<3, false>();
+  }
+}
+
+void free_all(mf_process* p) {
+  cudaFree(p->d_lnx); cudaFree(p->d_lnq2); cudaFree(p->d_xf); cudaFree(p->d_row);
+  cudaFree(p->d_partials); cudaFree(p->d_hist_part);
+}
+
+// launches the fused pass + finalize on `stream`
+int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+             uint64_t n_events, double w_max, void* d_records, uint64_t capacity, uint64_t* d_count, double* d_hist,
+             mf_iter_result* d_result, void* stream) {
+  if (!p) return MF_EINVAL;
+  if (!d_grid || !d_result) return fail(p, MF_EINVAL, "d_grid and d_result must not be NULL");
+  if (unw && (!d_count || !(w_max > 0.0))) return fail(p, MF_EINVAL, "mf_unweight needs d_count and w_max > 0");
+  if (unw && capacity > 0 && !d_records) return fail(p, MF_EINVAL, "capacity > 0 with d_records == NULL");
+  mf::PassArgs A;
+  A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row;
+  A.seed = seed; A.first_event = first_event; A.n_events = n_events; A.iteration = iteration;
+  A.w_max = w_max; A.records = (char*)d_records; A.capacity = capacity; A.count = (unsigned long long*)d_count;
+  A.partials = p->d_partials; A.hist_part = d_hist ? p->d_hist_part : nullptr;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int blocks = unw ? p->blocks_unw : p->blocks;
+  void* args[2] = {(void*)&p->P, (void*)&A};
+  cudaError_t e = cudaLaunchKernel(pass_fn(p->process, unw), dim3(blocks), dim3(p->threads), args, p->smem, st);
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "fused pass launch", e);
+  const int n_hist = p->D * p->P.n_bins;
+  const int fin_blocks = (n_hist + 255) / 256 + 1;
+  mf::finalize_kernel<<<fin_blocks, 256, 0, st>>>(p->d_partials, p->d_hist_part, blocks, n_hist, d_hist,
+                                                  (mf::IterResult*)d_result);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "finalize launch", e);
+  return MF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mf_create_process(const mf_process_desc* d, mf_process** out) {
+  if (out) *out = nullptr;
+  if (!d || !out) return MF_EINVAL;
+  if (d->process < 0 || d->process > 3 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
+      !(d->gev2_to_pb > 0.0))
+    return MF_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MF_ECUDA; }
+  mf_process* p = new (std::nothrow) mf_process;
+  if (!p) return MF_ENOMEM;
+  static const int Dtab[4] = {2, 4, 14, 18}, nftab[4] = {2, 2, 3, 4};
+  p->process = d->process; p->D = Dtab[d->process]; p->NF = nftab[d->process];
+  mf::Params& P = p->P;
+  std::memset(&P, 0, sizeof(P));
+  P.s = d->sqrt_s * d->sqrt_s;
+  P.alpha_em = d->alpha_em; P.alpha_s = d->alpha_s; P.m_top = d->m_top; P.mu2 = d->mu2;
+  P.ptmin = d->ptmin; P.etamax = d->etamax; P.drmin = d->drmin; P.gev2_to_pb = d->gev2_to_pb;
+  P.n_bins = d->n_bins;
+  const double gs2 = 4.0 * mf::kPi * d->alpha_s;
+  // |M|^2 normalisation: g_s^{2 n_g} / (4 helicity x 64 colour averages x (n_g - 2)! identical gluons)
+  if (d->process == 0) {
+    if (!(d->alpha_em > 0.0)) { delete p; return MF_EINVAL; }
+    P.me_norm = 1.0;
+  } else {
+    if (!(d->alpha_s > 0.0) || !(d->m_top > 0.0) || !(d->mu2 > 0.0)) { delete p; return MF_EINVAL; }
+    if (d->pdf_nx < 4 || d->pdf_nq < 4 || d->pdf_nx > 512 || !d->pdf_lnx || !d->pdf_lnq2 || !d->pdf_xf) {
+      delete p; return MF_EINVAL;
+    }
+    for (int i = 1; i < d->pdf_nx; ++i) if (!(d->pdf_lnx[i] > d->pdf_lnx[i - 1])) { delete p; return MF_EINVAL; }
+    for (int i = 1; i < d->pdf_nq; ++i) if (!(d->pdf_lnq2[i] > d->pdf_lnq2[i - 1])) { delete p; return MF_EINVAL; }
+    const int ng = d->process + 1;
+    P.me_norm = std::pow(gs2, ng) / (256.0 * (ng == 4 ? 2.0 : 1.0));
+    const int ncut = p->NF - 2;
+    const double thr = 2.0 * d->m_top + ncut * (d->ptmin > 0.0 ? d->ptmin : 0.0);
+    P.tau_min = thr * thr / P.s;
+    P.ln_tau_min = std::log(P.tau_min);
+    const double lq = std::log(d->mu2);
+    if (!(lq >= d->pdf_lnq2[0] && lq <= d->pdf_lnq2[d->pdf_nq - 1])) { delete p; return MF_ERANGE; }
+    if (!(P.tau_min < 1.0) || !(P.ln_tau_min >= d->pdf_lnx[0])) { delete p; return MF_ERANGE; }
+    P.pdf_nx = d->pdf_nx; P.pdf_nq = d->pdf_nq;
+    P.pdf_jq = mf::find_cell(d->pdf_lnq2, d->pdf_nq, lq);
+    P.pdf_uq = (lq - d->pdf_lnq2[P.pdf_jq]) / (d->pdf_lnq2[P.pdf_jq + 1] - d->pdf_lnq2[P.pdf_jq]);
+  }
+  // device-side constants
+  cudaError_t e = cudaSuccess;
+  if (d->process != 0) {
+    const size_t nx = d->pdf_nx, nq = d->pdf_nq;
+    if ((e = cudaMalloc(&p->d_lnx, nx * 8)) != cudaSuccess || (e = cudaMalloc(&p->d_lnq2, nq * 8)) != cudaSuccess ||
+        (e = cudaMalloc(&p->d_xf, nx * nq * 8)) != cudaSuccess || (e = cudaMalloc(&p->d_row, nx * 8)) != cudaSuccess) {
+      free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
+    }
+    cudaMemcpy(p->d_lnx, d->pdf_lnx, nx * 8, cudaMemcpyHostToDevice);
+    cudaMemcpy(p->d_lnq2, d->pdf_lnq2, nq * 8, cudaMemcpyHostToDevice);
+    cudaMemcpy(p->d_xf, d->pdf_xf, nx * nq * 8, cudaMemcpyHostToDevice);
+    mf::pdf_collapse_kernel<<<(int)((nx + 127) / 128), 128>>>(p->d_xf, p->d_lnq2, (int)nx, (int)nq, P.pdf_jq, P.pdf_uq,
+                                                             p->d_row);
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
+  }
+  // launch geometry: fill every SM with as many blocks as fit
+  cudaDeviceProp prop;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
+  p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + 2 * P.pdf_nx + 5 * 32) * sizeof(double);
+  int per_sm = 0, per_sm_unw = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pass_fn(p->process, false), p->threads, p->smem);
+  if (e == cudaSuccess)
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_unw, pass_fn(p->process, true), p->threads, p->smem);
+  if (e != cudaSuccess || per_sm < 1 || per_sm_unw < 1) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
+  p->blocks = prop.multiProcessorCount * per_sm;
+  p->blocks_unw = prop.multiProcessorCount * per_sm_unw;
+  const int max_blocks = p->blocks > p->blocks_unw ? p->blocks : p->blocks_unw;
+  if ((e = cudaMalloc(&p->d_partials, (size_t)max_blocks * sizeof(mf::BlockPartial))) != cudaSuccess ||
+      (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {
+    free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
+  }
+  snprintf(p->err, sizeof(p->err), "ok");
+  *out = p;
+  return MF_OK;
+}
+
+int mf_destroy_process(mf_process* p) {
+  if (!p) return MF_EINVAL;
+  free_all(p);
+  delete p;
+  return MF_OK;
+}
+
+int mf_n_dims(const mf_process* p, int32_t* D) { if (!p || !D) return MF_EINVAL; *D = p->D; return MF_OK; }
+int mf_n_final(const mf_process* p, int32_t* n) { if (!p || !n) return MF_EINVAL; *n = p->NF; return MF_OK; }
+int mf_record_size(const mf_process* p, int32_t* b) {
+  if (!p || !b) return MF_EINVAL;
+  *b = (p->NF + 2) * 32 + 16;
+  return MF_OK;
+}
+int mf_debug_row_len(const mf_process* p, int32_t* n) {
+  if (!p || !n) return MF_EINVAL;
+  *n = 3 * p->D + 4 * (p->NF + 2) + 9;
+  return MF_OK;
+}
+const char* mf_last_error(const mf_process* p) { return p ? p->err : kNullHandle; }
+int mf_launch_config(const mf_process* p, int32_t* blocks, int32_t* threads) {
+  if (!p || !blocks || !threads) return MF_EINVAL;
+  *blocks = p->blocks; *threads = p->threads;
+  return MF_OK;
+}
+
+int mf_vegas_iterate(mf_process* p, const double* d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                     uint64_t n_events, double* d_hist, mf_iter_result* d_result, void* stream) {
+  return run_pass(p, false, d_grid, seed, iteration, first_event, n_events, 0.0, nullptr, 0, nullptr, d_hist, d_result,
+                  stream);
+}
+
+int mf_unweight(mf_process* p, const double* d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                uint64_t n_events, double w_max, void* d_records, uint64_t capacity, uint64_t* d_count, double* d_hist,
+                mf_iter_result* d_result, void* stream) {
+  return run_pass(p, true, d_grid, seed, iteration, first_event, n_events, w_max, d_records, capacity, d_count, d_hist,
+                  d_result, stream);
+}
+
+int mf_refine_grid(mf_process* p, double* d_grid, const double* d_hist, double alpha, void* stream) {
+  if (!p) return MF_EINVAL;
+  if (!d_grid || !d_hist || !(alpha >= 0.0)) return fail(p, MF_EINVAL, "mf_refine_grid: bad argument");
+  mf::refine_grid_kernel<<<p->D, 32, 0, (cudaStream_t)stream>>>(d_grid, d_hist, p->P.n_bins, alpha);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "refine launch", e);
+  return MF_OK;
+}
+
+int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                  uint64_t n_events, double* d_out, void* stream) {
+  if (!p) return MF_EINVAL;
+  if (!d_grid || (!d_out && n_events)) return fail(p, MF_EINVAL, "mf_debug_eval: NULL argument");
+  if (n_events == 0) return MF_OK;
+  mf::PassArgs A;
+  std::memset(&A, 0, sizeof(A));
+  A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row;
+  A.seed = seed; A.first_event = first_event; A.n_events = n_events; A.iteration = iteration;
+  cudaStream_t st = (cudaStream_t)stream;
+  const unsigned blocks = (unsigned)((n_events + mf::kThreads - 1) / mf::kThreads);
+  switch (p->process) {
+    case 0: mf::debug_eval_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    case 1: mf::debug_eval_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    case 2: mf::debug_eval_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    default: mf::debug_eval_kernel<3><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "debug_eval launch", e);
+  return MF_OK;
+}
+
+int mf_debug_philox(uint64_t seed, uint32_t iteration, uint64_t first_event, uint64_t n_events, uint32_t n_blocks,
+                    uint32_t* d_out, void* stream) {
+  if (!d_out && n_events * n_blocks) return MF_EINVAL;
+  uint64_t total = n_events * n_blocks;
+  if (total == 0) return MF_OK;
+  mf::debug_philox_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+      seed, iteration, first_event, n_events, n_blocks, d_out);
+  return cudaGetLastError() == cudaSuccess ? MF_OK : MF_ECUDA;
+}
+
+int mf_debug_pdf(mf_process* p, const double* d_x, const double* d_q2, uint64_t n, double* d_out, void* stream) {
+  if (!p) return MF_EINVAL;
+  if (p->process == 0) return fail(p, MF_EINVAL, "process has no PDF");
+  if (n == 0) return MF_OK;
+  if (!d_x || !d_q2 || !d_out) return fail(p, MF_EINVAL, "mf_debug_pdf: NULL argument");
+  mf::debug_pdf_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+      p->d_lnx, p->d_lnq2, p->d_xf, p->P.pdf_nx, p->P.pdf_nq, d_x, d_q2, n, d_out);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "debug_pdf launch", e);
+  return MF_OK;
+}
+
+int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, void* stream) {
+  if (!p) return MF_EINVAL;
+  if (n == 0) return MF_OK;
+  if (!d_mom || !d_out) return fail(p, MF_EINVAL, "mf_debug_me2: NULL argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  const unsigned blocks = (unsigned)((n + mf::kThreads - 1) / mf::kThreads);
+  switch (p->process) {
+    case 0: mf::debug_me2_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    case 1: mf::debug_me2_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    case 2: mf::debug_me2_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    default: mf::debug_me2_kernel<3><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "debug_me2 launch", e);
+  return MF_OK;
+}
+
+int mf_measure_fp64_peak(int64_t iters, double* h_flops, double* h_ms) {
+  if (iters <= 0 || !h_flops) return MF_EINVAL;
+  cudaDeviceProp prop;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return MF_ECUDA;
+  double* sink = nullptr;
+  if (cudaMalloc(&sink, 8) != cudaSuccess) return MF_ENOMEM;
+  const int blocks = prop.multiProcessorCount * 4, threads = 256;
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  mf::dfma_peak_kernel<<<blocks, threads>>>(iters / 8 + 1, 1.0, sink);  // warm-up
+  cudaEventRecord(a);
+  mf::dfma_peak_kernel<<<blocks, threads>>>(iters, 1.0, sink);
+  cudaEventRecord(b);
+  cudaError_t e = cudaEventSynchronize(b);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, a, b);
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
+  if (e != cudaSuccess) return MF_ECUDA;
+  *h_flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads / ((double)ms * 1e-3);
+  if (h_ms) *h_ms = ms;
+  return MF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,229 @@
+// mf_kernels.cuh — the kernels of the fused pass (steps a1-a12, a14 of SURVEY.md 8(a)).
+//
+// Layout of one launch:
+//   * thread = event, grid-stride over the event range; nothing per event touches HBM;
+//   * the VEGAS grid, the collapsed PDF row and its ln x knots, and the block's w^2 histogram live in
+//     shared memory; per-thread running sums (sum w, sum w^2, max|w|, n_pass, n_accept) live in registers;
+//   * at the end: warp shuffle -> shared -> ONE partial record per block in global memory, and the block's
+//     histogram to its own slice of a [blocks][D*nb] scratch; a second tiny kernel adds the partials in a
+//     fixed order (so the sums do not depend on scheduling; only the shared-memory fp64 atomics of the
+//     histogram are order-dependent, at the 1e-16 level).
+#pragma once
+#include "mf_event.cuh"
+
+namespace mf {
+
+struct BlockPartial {
+  double sum_w, sum_w2, max_abs_w;
+  unsigned long long n_pass, n_accept;
+};
+struct IterResult {  // == mf_iter_result
+  double sum_w, sum_w2, max_abs_w;
+  unsigned long long n_pass, n_accept;
+};
+
+// Everything a launch of the fused pass needs besides Params.
+struct PassArgs {
+  const double* grid;      // [D][nb+1] device
+  const double* pdf_lnx;   // [nx] device (nullptr for e+e-)
+  const double* pdf_row;   // [nx] device: table collapsed at mu2
+  uint64_t seed, first_event, n_events;
+  uint32_t iteration;
+  double w_max;            // unweighting only
+  char* records;           // unweighting only
+  uint64_t capacity;
+  unsigned long long* count;
+  BlockPartial* partials;  // [gridDim.x]
+  double* hist_part;       // [gridDim.x][D*nb] or nullptr
+};
+
+// The matrix element is the only large piece of code; keep ONE copy per process per kernel.
+template <int PROC>
+__device__ __noinline__ double me2_call(const Params& P, double shat, const double (*k)[4]) {
+  return matrix_element<PROC>(P, shat, k);
+}
+
+// Luminosity (step a6): F(x1) F(x2) / (x1 x2) with F the interpolant of the collapsed row in shared memory.
+template <int PROC>
+MF_D double luminosity(const Params& P, const double* s_lnx, const double* s_row, double x1, double x2) {
+  if (PROC == 0) return 1.0;
+  double f1 = pdf_xf_row(s_lnx, s_row, P.pdf_nx, x1);
+  double f2 = pdf_xf_row(s_lnx, s_row, P.pdf_nx, x2);
+  return f1 * f2 / (x1 * x2);
+}
+
+// Lab-frame momenta of an event, beams first (record / debug-row layout).
+template <int PROC>
+MF_D void lab_momenta(const Event<PROC>& ev, double out[][4]) {
+  constexpr int NF = Traits<PROC>::NF;
+  Boost b = make_boost(ev.y);
+  double E = 0.5 * sqrt(ev.shat);
+  double p1[4] = {E, 0.0, 0.0, E}, p2[4] = {E, 0.0, 0.0, -E};
+  boost_z(b, p1, out[0]);
+  boost_z(b, p2, out[1]);
+#pragma unroll
+  for (int i = 0; i < NF; ++i) boost_z(b, ev.k[i], out[2 + i]);
+}
+
+MF_D double accept_draw(uint64_t seed, uint32_t iteration, uint64_t event) {
+  U4 r = philox_block(seed, iteration, event, 0xFFFFFFFFu);
+  return uniform52(r.x, r.y);
+}
+
+constexpr int kThreads = 128;
+
+// ---- the fused pass --------------------------------------------------------------------------------------
+template <int PROC, bool UNW>
+__global__ void __launch_bounds__(kThreads) fused_pass_kernel(const Params P, const PassArgs A) {
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  extern __shared__ double smem[];
+  const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx;
+  double* s_grid = smem;                    // D*(nb+1)
+  double* s_hist = s_grid + D * (nb + 1);   // D*nb
+  double* s_lnx = s_hist + D * nb;          // nx
+  double* s_row = s_lnx + nx;               // nx
+  double* s_red = s_row + nx;               // 5 * 32
+  for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
+  for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
+  for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
+  __syncthreads();
+
+  double sum_w = 0.0, sum_w2 = 0.0, max_w = 0.0;
+  unsigned long long n_pass = 0, n_acc = 0;
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  const uint64_t rounds = (A.n_events + stride - 1) / stride;
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (uint64_t rd = 0; rd < rounds; ++rd, idx += stride) {
+    const bool valid = idx < A.n_events;
+    const uint64_t event = A.first_event + idx;
+    double w = 0.0;
+    Bins<PROC> bins;
+    if (valid) {
+      Event<PROC> ev;
+      DebugRow dbg = {nullptr, D, NF};
+      generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
+      if (ev.pass) {
+        ++n_pass;
+        double lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
+        double me2 = me2_call<PROC>(P, ev.shat, ev.k);
+        w = event_weight<PROC>(P, ev, lum, me2);
+      }
+    }
+    const double w2 = w * w;
+    sum_w += w;
+    sum_w2 += w2;
+    max_w = fmax(max_w, fabs(w));
+    if (w != 0.0) {
+#pragma unroll
+      for (int d = 0; d < D; ++d) atomicAdd(&s_hist[d * nb + bins.get(d)], w2);
+    }
+    if (UNW) {
+      // a14: hit-or-miss against w_max; warp-aggregated cursor, one global atomic per warp with survivors
+      bool acc = false;
+      if (valid && w != 0.0) acc = accept_draw(A.seed, A.iteration, event) * A.w_max < fabs(w);
+      unsigned m = __ballot_sync(0xFFFFFFFFu, acc);
+      if (m) {
+        const int lane = threadIdx.x & 31;
+        unsigned long long base = 0;
+        if (lane == __ffs(m) - 1) base = atomicAdd(A.count, (unsigned long long)__popc(m));
+        base = __shfl_sync(0xFFFFFFFFu, base, __ffs(m) - 1);
+        if (acc) {
+          ++n_acc;
+          unsigned long long slot = base + __popc(m & ((1u << lane) - 1u));
+          if (A.records != nullptr && slot < A.capacity) {
+            // accepted events are rare (<1 %): regenerate the kinematics instead of keeping them live
+            Event<PROC> ev;
+            Bins<PROC> b2;
+            DebugRow dbg = {nullptr, D, NF};
+            generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
+            double mom[NF + 2][4];
+            lab_momenta<PROC>(ev, mom);
+            double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16));
+#pragma unroll
+            for (int i = 0; i < NF + 2; ++i)
+#pragma unroll
+              for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
+            rec[4 * (NF + 2)] = w;
+            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
+          }
+        }
+      }
+    }
+  }
+
+  // a11: warp shuffle -> shared -> one partial per block (fixed order)
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sum_w += __shfl_down_sync(0xFFFFFFFFu, sum_w, o);
+    sum_w2 += __shfl_down_sync(0xFFFFFFFFu, sum_w2, o);
+    max_w = fmax(max_w, __shfl_down_sync(0xFFFFFFFFu, max_w, o));
+    n_pass += __shfl_down_sync(0xFFFFFFFFu, n_pass, o);
+    n_acc += __shfl_down_sync(0xFFFFFFFFu, n_acc, o);
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+  if (lane == 0) {
+    s_red[warp] = sum_w;
+    s_red[32 + warp] = sum_w2;
+    s_red[64 + warp] = max_w;
+    s_red[96 + warp] = __longlong_as_double((long long)n_pass);
+    s_red[128 + warp] = __longlong_as_double((long long)n_acc);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    BlockPartial bp = {0.0, 0.0, 0.0, 0ull, 0ull};
+    for (int i = 0; i < nwarp; ++i) {
+      bp.sum_w += s_red[i];
+      bp.sum_w2 += s_red[32 + i];
+      bp.max_abs_w = fmax(bp.max_abs_w, s_red[64 + i]);
+      bp.n_pass += (unsigned long long)__double_as_longlong(s_red[96 + i]);
+      bp.n_accept += (unsigned long long)__double_as_longlong(s_red[128 + i]);
+    }
+    A.partials[blockIdx.x] = bp;
+  }
+  // a12: flush the block histogram to its slice
+  if (A.hist_part != nullptr) {
+    double* dst = A.hist_part + (size_t)blockIdx.x * (D * nb);
+    for (int i = threadIdx.x; i < D * nb; i += blockDim.x) dst[i] = s_hist[i];
+  }
+}
+
+// Adds the per-block partials in block order.  Blocks 0..gridDim.x-2 own histogram bins (one thread per
+// bin, summing over the pass's blocks); the last block reduces the scalar partials.
+__global__ void __launch_bounds__(256) finalize_kernel(const BlockPartial* partials, const double* hist_part,
+                                                        int n_blocks, int n_hist, double* hist, IterResult* result) {
+  if (blockIdx.x + 1 < gridDim.x) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (hist != nullptr && i < n_hist) {
+      double s = 0.0;
+      for (int b = 0; b < n_blocks; ++b) s += hist_part[(size_t)b * n_hist + i];
+      hist[i] = s;
+    }
+    return;
+  }
+  __shared__ double sw[256], sw2[256], mx[256];
+  __shared__ unsigned long long np[256], na[256];
+  double a = 0.0, b2 = 0.0, m = 0.0;
+  unsigned long long p = 0, q = 0;
+  for (int b = threadIdx.x; b < n_blocks; b += blockDim.x) {
+    BlockPartial bp = partials[b];
+    a += bp.sum_w; b2 += bp.sum_w2; m = fmax(m, bp.max_abs_w); p += bp.n_pass; q += bp.n_accept;
+  }
+  sw[threadIdx.x] = a; sw2[threadIdx.x] = b2; mx[threadIdx.x] = m; np[threadIdx.x] = p; na[threadIdx.x] = q;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      sw[threadIdx.x] += sw[threadIdx.x + o];
+      sw2[threadIdx.x] += sw2[threadIdx.x + o];
+      mx[threadIdx.x] = fmax(mx[threadIdx.x], mx[threadIdx.x + o]);
+      np[threadIdx.x] += np[threadIdx.x + o];
+      na[threadIdx.x] += na[threadIdx.x + o];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    result->sum_w = sw[0]; result->sum_w2 = sw2[0]; result->max_abs_w = mx[0];
+    result->n_pass = np[0]; result->n_accept = na[0];
+  }
+}
+
+}  // namespace mf

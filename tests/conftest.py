@@ -24,3 +24,30 @@ def oracle_procs(pdf):
     from oracle import mfo
     from paper_2106_10279_b200 import workloads as W
     return {wl.process: mfo.Process(wl, pdf) for wl in (W.C0, W.C1, W.C2, W.C3)}
+
+
+@pytest.fixture(scope="session")
+def gpu_procs(pdf):
+    """One CUDA-path handle per process id.  Fails loudly (no fallback) if the library or the GPU is missing."""
+    from paper_2106_10279_b200 import api
+    from paper_2106_10279_b200 import workloads as W
+    procs = {wl.process: api.Process(wl, pdf) for wl in (W.C0, W.C1, W.C2, W.C3)}
+    yield procs
+    for p in procs.values():
+        p.close()
+
+
+_ADAPTED = {}
+
+
+def adapted_grid(oracle_proc, wl, n_iter=3):
+    """A non-uniform VEGAS grid made by the ORACLE alone (a few small adapting iterations); cached."""
+    from paper_2106_10279_b200 import workloads as W
+    if wl.process not in _ADAPTED:
+        n_events = {0: 20000, 1: 8192, 2: 4096, 3: 1024}[wl.process]
+        grid = W.uniform_grid(wl.n_dims, wl.n_bins)
+        for k in range(n_iter):
+            hist, _ = oracle_proc.vegas_iterate(grid, 12345, k, 0, n_events)
+            grid = oracle_proc.refine_grid(grid, hist, W.VEGAS_ALPHA)
+        _ADAPTED[wl.process] = grid
+    return _ADAPTED[wl.process].copy()

