@@ -3,7 +3,7 @@ sm_100a.  No GPU is needed to build (nvcc cross-compiles).
 
     python -m paper_2106_10279_b200.build [--force] [--verbose]
 
-Steps: (1) csrc/gen_me.py writes the straight-line matrix-element code (the role of the paper's exporter
+Steps: (1) csrc/gen_me.py and csrc/gen_coop.py write the straight-line matrix-element code (the role of the paper's exporter
 plugin); (2) nvcc compiles csrc/madflow_b200.cu into the shared library.
 """
 import glob
@@ -26,10 +26,18 @@ def _sources():
 
 
 def generate():
-    spec = importlib.util.spec_from_file_location("_mf_gen_me", os.path.join(CSRC, "gen_me.py"))
-    mod = importlib.util.module_from_spec(spec)
-    spec.loader.exec_module(mod)
-    return mod.main()
+    """runs the build-time generators: gen_me.py (straight-line matrix elements) and gen_coop.py (the
+    cooperative g g -> t tbar g g program); both only rewrite their header when its text changes"""
+    out = []
+    if CSRC not in sys.path:
+        sys.path.insert(0, CSRC)          # gen_coop imports gen_me
+    for name in ("gen_me", "gen_coop"):
+        spec = importlib.util.spec_from_file_location(name, os.path.join(CSRC, name + ".py"))
+        mod = importlib.util.module_from_spec(spec)
+        sys.modules[name] = mod
+        spec.loader.exec_module(mod)
+        out.append(mod.main())
+    return out
 
 
 def needs_build():

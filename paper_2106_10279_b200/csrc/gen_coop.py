@@ -480,7 +480,7 @@ def main():
            "#pragma once", '#include "mf_me_prims.cuh"', "",
            "#if defined(__CUDA_ARCH__)", "#define MF_TABLE static __device__ const", "#else",
            "#define MF_TABLE static const", "#endif", "", "namespace mf {", "",
-           "// scratch layout (doubles), component-major: VEC[4][kCoopNV], SPIN[8][kCoopNS], CVEC[8][kCoopNC], SCAL[kCoopNX]",
+           "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | CVEC 8*kCoopNC | SCAL kCoopNX (each region 16-byte aligned)",
            "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopNC = %d, kCoopNX = %d;" % (L.n("V"), L.n("S"), L.n("C"), L.n("X")),
            "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 8 * kCoopNC + kCoopNX;",
            "constexpr double kCoopCden = %.1f;" % Cden,
@@ -507,35 +507,43 @@ def main():
                (s0_flops, staged, s4_flops))
     hdr.append("constexpr double kFlopsMe2Coop_2g = %d.0;" % total)
     hdr.append("")
-    loaders = '''MF_HD rvec coop_ld_vec(const double* V, int i) {
+    loaders = '''// Scratch items are stored as planes of double2 so that consecutive lanes reading consecutive items issue
+// conflict-free 128-bit shared-memory loads: VEC plane p = components (2p, 2p+1); SPIN / CVEC plane c = (re[c], im[c]).
+MF_HD rvec coop_ld_vec(const double* V, int i) {
+  const double2* q = reinterpret_cast<const double2*>(V);
+  const double2 a = q[i], b = q[kCoopNV + i];
   rvec r;
-#pragma unroll
-  for (int c = 0; c < 4; ++c) r.v[c] = V[c * kCoopNV + i];
+  r.v[0] = a.x; r.v[1] = a.y; r.v[2] = b.x; r.v[3] = b.y;
   return r;
 }
 MF_HD void coop_st_vec(double* V, int i, const rvec& r) {
-#pragma unroll
-  for (int c = 0; c < 4; ++c) V[c * kCoopNV + i] = r.v[c];
+  double2* q = reinterpret_cast<double2*>(V);
+  q[i] = make_double2(r.v[0], r.v[1]);
+  q[kCoopNV + i] = make_double2(r.v[2], r.v[3]);
 }
 MF_HD spin coop_ld_spin(const double* S, int i) {
+  const double2* q = reinterpret_cast<const double2*>(S);
   spin r;
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { r.re[c] = S[c * kCoopNS + i]; r.im[c] = S[(4 + c) * kCoopNS + i]; }
+  for (int c = 0; c < 4; ++c) { const double2 t = q[c * kCoopNS + i]; r.re[c] = t.x; r.im[c] = t.y; }
   return r;
 }
 MF_HD void coop_st_spin(double* S, int i, const spin& r) {
+  double2* q = reinterpret_cast<double2*>(S);
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { S[c * kCoopNS + i] = r.re[c]; S[(4 + c) * kCoopNS + i] = r.im[c]; }
+  for (int c = 0; c < 4; ++c) q[c * kCoopNS + i] = make_double2(r.re[c], r.im[c]);
 }
 MF_HD cvec coop_ld_cvec(const double* C, int i) {
+  const double2* q = reinterpret_cast<const double2*>(C);
   cvec r;
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { r.re[c] = C[c * kCoopNC + i]; r.im[c] = C[(4 + c) * kCoopNC + i]; }
+  for (int c = 0; c < 4; ++c) { const double2 t = q[c * kCoopNC + i]; r.re[c] = t.x; r.im[c] = t.y; }
   return r;
 }
 MF_HD void coop_st_cvec(double* C, int i, const cvec& r) {
+  double2* q = reinterpret_cast<double2*>(C);
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { C[c * kCoopNC + i] = r.re[c]; C[(4 + c) * kCoopNC + i] = r.im[c]; }
+  for (int c = 0; c < 4; ++c) q[c * kCoopNC + i] = make_double2(r.re[c], r.im[c]);
 }
 '''
     text = "\n".join(hdr) + "\n" + loaders + "\n" + tables + "\n\n" + s4 + "\n\n}  // namespace mf\n"

@@ -9,6 +9,7 @@
 
 #include "../../include/mf.h"
 #include "mf_aux_kernels.cuh"
+#include "mf_kernels_coop.cuh"
 
 static_assert(sizeof(mf::IterResult) == sizeof(mf_iter_result), "result layouts must agree");
 static_assert(mf::kMaxBins == MF_MAX_BINS, "bin limits must agree");
@@ -43,7 +44,7 @@ const void* pass_fn(int proc, bool unw) {
     case 0: return unw ? pass_fn<0, true>() : pass_fn<0, false>();
     case 1: return unw ? pass_fn<1, true>() : pass_fn<1, false>();
     case 2: return unw ? pass_fn<2, true>() : pass_fn<2, false>();
-    default: return unw ? pass_fn<3, true>() : pass_fn<3, false>();
+    default: return unw ? (const void*)mf::fused_pass_coop_kernel<true> : (const void*)mf::fused_pass_coop_kernel<false>;
   }
 }
 
@@ -146,7 +147,21 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   int dev = 0;
   cudaGetDevice(&dev);
   if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
-  p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + 2 * P.pdf_nx + 5 * 32) * sizeof(double);
+  if (p->process == 3) {
+    // cooperative pass: as many 64-thread teams per block as the SM's shared memory holds, one block per SM
+    int n_teams = mf::kCoopMaxTeams;
+    while (n_teams > 0 &&
+           (size_t)mf::CoopSmem(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
+      --n_teams;
+    if (n_teams < 1) { free_all(p); delete p; return MF_ECUDA; }
+    p->threads = n_teams * mf::kCoopTeam;
+    p->smem = (size_t)mf::CoopSmem(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8;
+    for (int u = 0; u < 2; ++u)
+      if ((e = cudaFuncSetAttribute(pass_fn(3, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem)) !=
+          cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
+  } else {
+    p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + 2 * P.pdf_nx + 5 * 32) * sizeof(double);
+  }
   int per_sm = 0, per_sm_unw = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pass_fn(p->process, false), p->threads, p->smem);
   if (e == cudaSuccess)
@@ -227,7 +242,10 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
     case 0: mf::debug_eval_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 1: mf::debug_eval_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 2: mf::debug_eval_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
-    default: mf::debug_eval_kernel<3><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    default:
+      mf::debug_eval_coop_kernel<<<(unsigned)((n_events + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
+                                   mf::kCoopTeamDoubles * 8, st>>>(p->P, A, d_out);
+      break;
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "debug_eval launch", e);
@@ -266,7 +284,10 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
     case 0: mf::debug_me2_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 1: mf::debug_me2_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 2: mf::debug_me2_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
-    default: mf::debug_me2_kernel<3><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    default:
+      mf::debug_me2_coop_kernel<<<(unsigned)((n + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
+                                  mf::kCoopTeamDoubles * 8, st>>>(p->P, d_mom, n, d_out);
+      break;
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "debug_me2 launch", e);

@@ -13,6 +13,12 @@
 
 namespace mf {
 
+#if !defined(__CUDACC__)
+// host builds (tests/host_shim) have no CUDA vector types
+struct double2 { double x, y; };
+inline double2 make_double2(double x, double y) { return double2{x, y}; }
+#endif
+
 constexpr double kPi = 3.14159265358979323846264338327950288;
 constexpr double kTwoPi = 6.28318530717958647692528676655900577;
 

@@ -72,86 +72,66 @@ MF_D double accept_draw(uint64_t seed, uint32_t iteration, uint64_t event) {
 
 constexpr int kThreads = 128;
 
-// ---- the fused pass --------------------------------------------------------------------------------------
-template <int PROC, bool UNW>
-__global__ void __launch_bounds__(kThreads) fused_pass_kernel(const Params P, const PassArgs A) {
-  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
-  extern __shared__ double smem[];
-  const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx;
-  double* s_grid = smem;                    // D*(nb+1)
-  double* s_hist = s_grid + D * (nb + 1);   // D*nb
-  double* s_lnx = s_hist + D * nb;          // nx
-  double* s_row = s_lnx + nx;               // nx
-  double* s_red = s_row + nx;               // 5 * 32
-  for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
-  for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
-  for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
-  __syncthreads();
-
+// Per-thread running sums of the pass (registers).
+struct Accum {
   double sum_w = 0.0, sum_w2 = 0.0, max_w = 0.0;
   unsigned long long n_pass = 0, n_acc = 0;
-  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-  const uint64_t rounds = (A.n_events + stride - 1) / stride;
-  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  for (uint64_t rd = 0; rd < rounds; ++rd, idx += stride) {
-    const bool valid = idx < A.n_events;
-    const uint64_t event = A.first_event + idx;
-    double w = 0.0;
-    Bins<PROC> bins;
-    if (valid) {
-      Event<PROC> ev;
-      DebugRow dbg = {nullptr, D, NF};
-      generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
-      if (ev.pass) {
-        ++n_pass;
-        double lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
-        double me2 = me2_call<PROC>(P, ev.shat, ev.k);
-        w = event_weight<PROC>(P, ev, lum, me2);
-      }
-    }
-    const double w2 = w * w;
-    sum_w += w;
-    sum_w2 += w2;
-    max_w = fmax(max_w, fabs(w));
-    if (w != 0.0) {
+};
+
+// a11/a12/a14 for one event (called by every thread of a warp, valid or not): running sums, the block's
+// shared-memory w^2 histogram, and hit-or-miss unweighting with a warp-aggregated cursor.
+template <int PROC, bool UNW>
+MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_grid, double* s_hist, bool valid,
+                           uint64_t event, double w, const Bins<PROC>& bins, Accum& acc) {
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  const int nb = P.n_bins;
+  const double w2 = w * w;
+  acc.sum_w += w;
+  acc.sum_w2 += w2;
+  acc.max_w = fmax(acc.max_w, fabs(w));
+  if (w != 0.0) {
 #pragma unroll
-      for (int d = 0; d < D; ++d) atomicAdd(&s_hist[d * nb + bins.get(d)], w2);
-    }
-    if (UNW) {
-      // a14: hit-or-miss against w_max; warp-aggregated cursor, one global atomic per warp with survivors
-      bool acc = false;
-      if (valid && w != 0.0) acc = accept_draw(A.seed, A.iteration, event) * A.w_max < fabs(w);
-      unsigned m = __ballot_sync(0xFFFFFFFFu, acc);
-      if (m) {
-        const int lane = threadIdx.x & 31;
-        unsigned long long base = 0;
-        if (lane == __ffs(m) - 1) base = atomicAdd(A.count, (unsigned long long)__popc(m));
-        base = __shfl_sync(0xFFFFFFFFu, base, __ffs(m) - 1);
-        if (acc) {
-          ++n_acc;
-          unsigned long long slot = base + __popc(m & ((1u << lane) - 1u));
-          if (A.records != nullptr && slot < A.capacity) {
-            // accepted events are rare (<1 %): regenerate the kinematics instead of keeping them live
-            Event<PROC> ev;
-            Bins<PROC> b2;
-            DebugRow dbg = {nullptr, D, NF};
-            generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
-            double mom[NF + 2][4];
-            lab_momenta<PROC>(ev, mom);
-            double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16));
+    for (int d = 0; d < D; ++d) atomicAdd(&s_hist[d * nb + bins.get(d)], w2);
+  }
+  if (UNW) {
+    // a14: hit-or-miss against w_max; one global atomic per warp with survivors
+    bool ok = false;
+    if (valid && w != 0.0) ok = accept_draw(A.seed, A.iteration, event) * A.w_max < fabs(w);
+    unsigned m = __ballot_sync(0xFFFFFFFFu, ok);
+    if (m) {
+      const int lane = threadIdx.x & 31;
+      unsigned long long base = 0;
+      if (lane == __ffs(m) - 1) base = atomicAdd(A.count, (unsigned long long)__popc(m));
+      base = __shfl_sync(0xFFFFFFFFu, base, __ffs(m) - 1);
+      if (ok) {
+        ++acc.n_acc;
+        unsigned long long slot = base + __popc(m & ((1u << lane) - 1u));
+        if (A.records != nullptr && slot < A.capacity) {
+          // accepted events are rare (<1 %): regenerate the kinematics instead of keeping them live
+          Event<PROC> ev;
+          Bins<PROC> b2;
+          DebugRow dbg = {nullptr, D, NF};
+          generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
+          double mom[NF + 2][4];
+          lab_momenta<PROC>(ev, mom);
+          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16));
 #pragma unroll
-            for (int i = 0; i < NF + 2; ++i)
+          for (int i = 0; i < NF + 2; ++i)
 #pragma unroll
-              for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
-            rec[4 * (NF + 2)] = w;
-            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
-          }
+            for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
+          rec[4 * (NF + 2)] = w;
+          reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
         }
       }
     }
   }
+}
 
-  // a11: warp shuffle -> shared -> one partial per block (fixed order)
+// a11 (warp shuffle -> shared -> ONE partial per block, fixed order) and the a12 histogram flush.
+// s_red: 5 * 32 doubles.  Contains a __syncthreads: every thread of the block must call it.
+MF_D void block_finish(const PassArgs& A, Accum acc, double* s_red, const double* s_hist, int n_hist) {
+  double sum_w = acc.sum_w, sum_w2 = acc.sum_w2, max_w = acc.max_w;
+  unsigned long long n_pass = acc.n_pass, n_acc = acc.n_acc;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     sum_w += __shfl_down_sync(0xFFFFFFFFu, sum_w, o);
@@ -180,11 +160,52 @@ __global__ void __launch_bounds__(kThreads) fused_pass_kernel(const Params P, co
     }
     A.partials[blockIdx.x] = bp;
   }
-  // a12: flush the block histogram to its slice
   if (A.hist_part != nullptr) {
-    double* dst = A.hist_part + (size_t)blockIdx.x * (D * nb);
-    for (int i = threadIdx.x; i < D * nb; i += blockDim.x) dst[i] = s_hist[i];
+    double* dst = A.hist_part + (size_t)blockIdx.x * n_hist;
+    for (int i = threadIdx.x; i < n_hist; i += blockDim.x) dst[i] = s_hist[i];
   }
+}
+
+// ---- the fused pass, one thread per event (e+e- -> mu+mu-, gg -> ttbar, gg -> ttbar g) ----------------------
+template <int PROC, bool UNW>
+__global__ void __launch_bounds__(kThreads) fused_pass_kernel(const Params P, const PassArgs A) {
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  extern __shared__ double smem[];
+  const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx;
+  double* s_grid = smem;                    // D*(nb+1)
+  double* s_hist = s_grid + D * (nb + 1);   // D*nb
+  double* s_lnx = s_hist + D * nb;          // nx
+  double* s_row = s_lnx + nx;               // nx
+  double* s_red = s_row + nx;               // 5 * 32
+  for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
+  for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
+  for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
+  __syncthreads();
+
+  Accum acc;
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  const uint64_t rounds = (A.n_events + stride - 1) / stride;
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (uint64_t rd = 0; rd < rounds; ++rd, idx += stride) {
+    const bool valid = idx < A.n_events;
+    const uint64_t event = A.first_event + idx;
+    double w = 0.0;
+    Bins<PROC> bins;
+    bins.clear();
+    if (valid) {
+      Event<PROC> ev;
+      DebugRow dbg = {nullptr, D, NF};
+      generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
+      if (ev.pass) {
+        ++acc.n_pass;
+        double lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
+        double me2 = me2_call<PROC>(P, ev.shat, ev.k);
+        w = event_weight<PROC>(P, ev, lum, me2);
+      }
+    }
+    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc);
+  }
+  block_finish(A, acc, s_red, s_hist, D * nb);
 }
 
 // Adds the per-block partials in block order.  Blocks 0..gridDim.x-2 own histogram bins (one thread per

@@ -1,0 +1,166 @@
+// mf_kernels_coop.cuh — the fused pass for g g -> t tbar g g (BASELINE.json configs[3], [4]): steps a1-a6 and
+// a10-a14 one thread per event exactly as in mf_kernels.cuh, steps a7-a9 (the matrix element, >99 % of the
+// arithmetic) by teams of 64 threads per event over a shared-memory scratch
+// (mf_me_coop.cuh).
+//
+// Block = T teams of 64 threads (T = 5 for 50 bins: 5 x 42.8 kB of scratch + grid + histogram + PDF row fill the
+// 227 kB of one SM; one block per SM).  Per round every thread generates its own event; each team then walks
+// over the events of its 64 threads that passed the cuts: the owner publishes the four final-state momenta,
+// the team computes |M|^2, the owner keeps the result.  Teams never wait for each other inside the event loop
+// (named barriers, one per team); the only block-wide barriers are at start-up and in the final reduction.
+#pragma once
+#include "mf_kernels.cuh"
+#include "mf_me_coop.cuh"
+
+namespace mf {
+
+constexpr int kCoopMaxTeams = 5;
+
+// shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
+struct CoopSmem {
+  int grid, hist, lnx, row, red, teams, total;
+  __host__ __device__ CoopSmem(int D, int nb, int nx, int n_teams) {
+    auto even = [](int v) { return (v + 1) & ~1; };
+    grid = 0;
+    hist = grid + even(D * (nb + 1));
+    lnx = hist + even(D * nb);
+    row = lnx + even(nx);
+    red = row + even(nx);
+    teams = red + 5 * 32;
+    total = teams + n_teams * kCoopTeamDoubles;
+  }
+};
+
+// |M|^2 (with couplings and averaging) of this thread's own event, computed by its team.  Every thread of the
+// team must call it (it contains team barriers); `round` alternates the mask slot so that consecutive calls do
+// not race.  Returns 0 for threads whose event did not pass.
+__device__ __forceinline__ double coop_team_me2(double* tm, int team, int tid, unsigned round, bool pass,
+                                                const double (*k)[4], double shat, const Params& P) {
+  unsigned* s_mask = reinterpret_cast<unsigned*>(tm + kCoopOffMask) + 2 * (round & 1u);
+  const unsigned bal = __ballot_sync(0xFFFFFFFFu, pass);
+  if ((tid & 31) == 0) s_mask[tid >> 5] = bal;
+  coop_team_sync(team);
+  unsigned long long m = (unsigned long long)s_mask[0] | ((unsigned long long)s_mask[1] << 32);
+  double me2 = 0.0;
+  double* in = tm + kCoopOffIn;
+  while (m) {
+    const int i = __ffsll((long long)m) - 1;
+    m &= m - 1;
+    if (tid == i) {
+#pragma unroll
+      for (int f = 0; f < 4; ++f)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) in[4 * f + c] = k[f][c];
+      in[16] = shat;
+    }
+    coop_team_sync(team);
+    const double r = coop_me2_team(tm, team, tid, P.m_top);
+    if (tid == i) me2 = r * P.me_norm;
+  }
+  return me2;
+}
+
+template <bool UNW>
+__global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_kernel(const Params P, const PassArgs A) {
+  constexpr int PROC = 3, D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  extern __shared__ double2 smem2[];
+  double* smem = reinterpret_cast<double*>(smem2);
+  const int nb = P.n_bins, nx = P.pdf_nx;
+  const int n_teams = blockDim.x / kCoopTeam;
+  const CoopSmem L(D, nb, nx, n_teams);
+  double* s_grid = smem + L.grid;
+  double* s_hist = smem + L.hist;
+  double* s_lnx = smem + L.lnx;
+  double* s_row = smem + L.row;
+  double* s_red = smem + L.red;
+  const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam;
+  double* tm = smem + L.teams + team * kCoopTeamDoubles;
+  for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
+  for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
+  for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
+  __syncthreads();
+
+  Accum acc;
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  const uint64_t rounds = (A.n_events + stride - 1) / stride;
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (uint64_t rd = 0; rd < rounds; ++rd, idx += stride) {
+    const bool valid = idx < A.n_events;
+    const uint64_t event = A.first_event + idx;
+    Bins<PROC> bins;
+    bins.clear();
+    Event<PROC> ev;
+    ev.pass = false;
+    double lum = 0.0;
+    if (valid) {
+      DebugRow dbg = {nullptr, D, NF};
+      generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
+      if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
+    }
+    const bool pass = valid && ev.pass;
+    const double me2 = coop_team_me2(tm, team, tid, (unsigned)rd, pass, ev.k, ev.shat, P);
+    double w = 0.0;
+    if (pass) {
+      ++acc.n_pass;
+      w = event_weight<PROC>(P, ev, lum, me2);
+    }
+    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc);
+  }
+  block_finish(A, acc, s_red, s_hist, D * nb);
+}
+
+// Per-event dump for g g -> t tbar g g through the same team program: block = one team, thread = event.
+__global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params P, const PassArgs A, double* out) {
+  constexpr int PROC = 3, D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  extern __shared__ double2 smem2[];
+  double* tm = reinterpret_cast<double*>(smem2);
+  const int row_len = 3 * D + 4 * (NF + 2) + 9;
+  const uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = idx < A.n_events;
+  const uint64_t event = A.first_event + idx;
+  double* row = out + idx * row_len;
+  Event<PROC> ev;
+  ev.pass = false;
+  Bins<PROC> bins;
+  if (valid) {
+    DebugRow dbg = {row, D, NF};
+    generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
+  }
+  const bool pass = valid && ev.pass;
+  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, pass, ev.k, ev.shat, P);
+  if (!valid) return;
+  double mom[NF + 2][4];
+  lab_momenta<PROC>(ev, mom);
+  double* q = row + D;
+  for (int i = 0; i < NF + 2; ++i)
+    for (int c = 0; c < 4; ++c) *q++ = mom[i][c];
+  double lum = 0.0, w = 0.0;
+  if (pass) {
+    lum = luminosity<PROC>(P, A.pdf_lnx, A.pdf_row, ev.x1, ev.x2);
+    w = event_weight<PROC>(P, ev, lum, me2);
+  }
+  q[0] = ev.x1; q[1] = ev.x2; q[2] = lum; q[3] = me2; q[4] = ev.phi; q[5] = ev.jac_vegas; q[6] = w;
+  q[7] = pass ? 1.0 : 0.0;
+  q[8] = accept_draw(A.seed, A.iteration, event);
+}
+
+// |M|^2 at caller-supplied CM-frame momenta mom[n][6][4] (beams first): block = one team, thread = event.
+__global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params P, const double* mom, uint64_t n,
+                                                                    double* out) {
+  extern __shared__ double2 smem2[];
+  double* tm = reinterpret_cast<double*>(smem2);
+  const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = i < n;
+  double k[4][4];
+  double shat = 0.0;
+  if (valid) {
+    const double* m = mom + i * 24;
+    for (int f = 0; f < 4; ++f)
+      for (int c = 0; c < 4; ++c) k[f][c] = m[(2 + f) * 4 + c];
+    shat = 4.0 * m[0] * m[0];
+  }
+  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, valid, k, shat, P);
+  if (valid) out[i] = me2;
+}
+
+}  // namespace mf

@@ -1,0 +1,208 @@
+// mf_me_coop.cuh — steps a7-a9 for g g -> t tbar g g as a COOPERATIVE program: one event per team of 64
+// threads (2 warps), all intermediate currents in a per-team shared-memory scratch (the
+// matrix element loops over helicities and sums; DESIGN.md "Kernels" explains why not one thread per event).
+//
+//   S0   hand written: momentum sums, propagator denominators, polarisation vectors, external spinors
+//   S1-3 table driven (csrc/gen_coop.py): one task = one off-shell current for one polarisation assignment of
+//        the gluons it contains ("helicity recycling"); a warp executes rounds of 32 equal-shaped tasks
+//   S4   generated straight-line code: thread (pols, h, hb) forms its 24 colour-ordered amplitudes and
+//        contracts them with the colour matrix; the 64 partial sums are added in a fixed order
+//
+// Every function is MF_HD and takes the team-thread index explicitly, so tests/host_shim can run the same
+// program on the host (looping over the 64 "threads" stage by stage) and compare it with the oracle.
+#pragma once
+#include "mf_me_prims.cuh"
+#include "mf_me_ttgg_coop_generated.cuh"
+
+namespace mf {
+
+constexpr int kCoopTeam = 64;                     // threads per event
+constexpr int kCoopInDoubles = 18;                // input area: k[4][4] (t, tbar, g, g; CM frame), shat, pad
+constexpr int kCoopRedDoubles = 2;                // one partial per warp
+// per-team shared memory (doubles): scratch | input | reduction | pass masks (2 x 2 x u32)
+constexpr int kCoopOffIn = (kCoopScratchDoubles + 1) & ~1;
+constexpr int kCoopOffRed = kCoopOffIn + kCoopInDoubles;
+constexpr int kCoopOffMask = kCoopOffRed + kCoopRedDoubles;
+constexpr int kCoopTeamDoubles = kCoopOffMask + 2;
+
+MF_HD double* coop_V(double* scr) { return scr; }
+MF_HD double* coop_S(double* scr) { return scr + 4 * kCoopNV; }
+MF_HD double* coop_C(double* scr) { return scr + 4 * kCoopNV + 8 * kCoopNS; }
+MF_HD double* coop_X(double* scr) { return scr + 4 * kCoopNV + 8 * kCoopNS + 8 * kCoopNC; }
+
+// ---- S0: per-event constants --------------------------------------------------------------------------------
+// in[0..15] = k[4][4] (t, tbar, g2, g3 in the partonic CM frame), in[16] = shat.  Gluon labels: 0, 1 = the beams
+// (+z, -z, energy sqrt(shat)/2), 2, 3 = the final gluons entering with -k (all gluon momenta incoming).
+MF_HD rvec coop_gluon_momentum(const double* in, int g) {
+  const double E = 0.5 * sqrt(in[16]);
+  rvec p;
+  if (g == 0) p = {{E, 0.0, 0.0, E}};
+  else if (g == 1) p = {{E, 0.0, 0.0, -E}};
+  else p = {{-in[4 * g + 0], -in[4 * g + 1], -in[4 * g + 2], -in[4 * g + 3]}};
+  return p;
+}
+
+MF_HD void coop_s0(double* scr, const double* in, int tid, double mt) {
+  double* V = coop_V(scr);
+  double* S = coop_S(scr);
+  double* X = coop_X(scr);
+  if (tid >= 1 && tid <= 15) {
+    const int m = tid;
+    rvec P = {{0.0, 0.0, 0.0, 0.0}};
+    int n = 0;
+#pragma unroll
+    for (int g = 0; g < 4; ++g)
+      if ((m >> g) & 1) { P = radd(P, coop_gluon_momentum(in, g)); ++n; }
+    coop_st_vec(V, kCoopP0 + m - 1, P);
+    if (n >= 2) X[kCoopIP2ofMask[m - 1]] = 1.0 / rdot(P, P);
+    const double mt2 = mt * mt;
+    const int ix = kCoopQXofMask[m - 1], iy = kCoopQYofMask[m - 1];
+    if (ix >= 0) {
+      rvec q = {{P.v[0] - in[4], P.v[1] - in[5], P.v[2] - in[6], P.v[3] - in[7]}};   // P - p4
+      coop_st_vec(V, ix, q);
+      X[kCoopIdXofMask[m - 1]] = 1.0 / (rdot(q, q) - mt2);
+    }
+    if (iy >= 0) {
+      rvec q = {{in[0] - P.v[0], in[1] - P.v[1], in[2] - P.v[2], in[3] - P.v[3]}};   // p3 - P
+      coop_st_vec(V, iy, q);
+      X[kCoopIdYofMask[m - 1]] = 1.0 / (rdot(q, q) - mt2);
+    }
+  } else if (tid >= 16 && tid < 24) {
+    const int g = (tid - 16) >> 1, p = (tid - 16) & 1;
+    rvec e;
+    if (g == 0) e = p == 0 ? rvec{{0.0, 1.0, 0.0, 0.0}} : rvec{{0.0, 0.0, 1.0, 0.0}};
+    else if (g == 1) e = p == 0 ? rvec{{0.0, 1.0, 0.0, 0.0}} : rvec{{0.0, 0.0, -1.0, 0.0}};
+    else {
+      rvec e1, e2;
+      pol_vectors(in + 4 * g, e1, e2);
+      e = p == 0 ? e1 : e2;
+    }
+    coop_st_vec(V, kCoopEps0 + 2 * g + p, e);
+  } else if (tid >= 24 && tid < 28) {
+    const int s = tid & 1;
+    if (tid < 26) coop_st_spin(S, kCoopUb0 + s, ubar_row(in, mt, s));
+    else coop_st_spin(S, kCoopV0 + s, v_col(in + 4, mt, s));
+  }
+}
+
+// ---- S1-S3: the task interpreter -----------------------------------------------------------------------------
+// f points at this lane's column of the round's field table: field j is f[32 * j].
+template <int NV3, int NV4>
+MF_HD void coop_task_J(double* scr, const short* f) {
+  const double* V = coop_V(scr);
+  const int signs = f[32 * (2 + 4 * NV3 + 3 * NV4)];
+  rvec acc = {{0.0, 0.0, 0.0, 0.0}};
+#pragma unroll
+  for (int t = 0; t < NV3; ++t) {
+    const short* g = f + 32 * (2 + 4 * t);
+    const rvec J1 = coop_ld_vec(V, g[0]), P1 = coop_ld_vec(V, g[32]);
+    const rvec J2 = coop_ld_vec(V, g[64]), P2 = coop_ld_vec(V, g[96]);
+    v3_acc(acc, ((signs >> t) & 1) ? -1.0 : 1.0, J1, P1, J2, P2);
+  }
+#pragma unroll
+  for (int t = 0; t < NV4; ++t) {
+    const short* g = f + 32 * (2 + 4 * NV3 + 3 * t);
+    const rvec J1 = coop_ld_vec(V, g[0]), J2 = coop_ld_vec(V, g[32]), J3 = coop_ld_vec(V, g[64]);
+    v4_acc(acc, ((signs >> (NV3 + t)) & 1) ? -1.0 : 1.0, J1, J2, J3);
+  }
+  coop_st_vec(coop_V(scr), f[0], rscale(acc, coop_X(scr)[f[32]]));
+}
+
+template <int NT>
+MF_HD void coop_task_X(double* scr, const short* f, double mt) {
+  const double* V = coop_V(scr);
+  const double* S = coop_S(scr);
+  const int signs = f[32 * (3 + 2 * NT)];
+  spin t;
+#pragma unroll
+  for (int i = 0; i < NT; ++i) {
+    const short* g = f + 32 * (3 + 2 * i);
+    const rvec J = rscale(coop_ld_vec(V, g[0]), ((signs >> i) & 1) ? -1.0 : 1.0);
+    const spin x = coop_ld_spin(S, g[32]);
+    if (i == 0) t = slash_col(J, x);
+    else spin_acc(t, slash_col(J, x));
+  }
+  coop_st_spin(coop_S(scr), f[0], prop_col(coop_ld_vec(V, f[32]), mt, coop_X(scr)[f[64]], t));
+}
+
+template <int NT, bool PROP>
+MF_HD void coop_task_Y(double* scr, const short* f, double mt) {
+  const double* V = coop_V(scr);
+  const double* S = coop_S(scr);
+  const int signs = f[32 * (3 + 2 * NT)];
+  spin t;
+#pragma unroll
+  for (int i = 0; i < NT; ++i) {
+    const short* g = f + 32 * (3 + 2 * i);
+    const spin y = coop_ld_spin(S, g[0]);
+    const rvec J = rscale(coop_ld_vec(V, g[32]), ((signs >> i) & 1) ? -1.0 : 1.0);
+    if (i == 0) t = slash_row(y, J);
+    else spin_acc(t, slash_row(y, J));
+  }
+  if (PROP) t = prop_row(t, coop_ld_vec(V, f[32]), mt, coop_X(scr)[f[64]]);
+  coop_st_spin(coop_S(scr), f[0], t);
+}
+
+MF_HD void coop_task_bil(double* scr, const short* f) {
+  const double* S = coop_S(scr);
+  coop_st_cvec(coop_C(scr), f[0], bilinear(coop_ld_spin(S, f[32]), coop_ld_spin(S, f[64])));
+}
+
+// All rounds of (stage, warp) for one lane.  Rounds are uniform per warp (same op and shape for all lanes);
+// a lane whose output index is negative idles.
+MF_HD void coop_run_stage(double* scr, int stage, int warp, int lane, double mt) {
+  const int row = stage * kCoopWarps + warp;
+  const int nr = kCoopNumRounds[row];
+  for (int r = 0; r < nr; ++r) {
+    const CoopRound R = kCoopRounds[row][r];
+    const short* f = kCoopTable + R.offset + lane;
+    if (f[0] < 0) continue;
+    switch (R.op * 16 + R.a * 4 + R.b) {
+      case 0 * 16 + 1 * 4 + 0: coop_task_J<1, 0>(scr, f); break;
+      case 0 * 16 + 2 * 4 + 1: coop_task_J<2, 1>(scr, f); break;
+      case 0 * 16 + 3 * 4 + 3: coop_task_J<3, 3>(scr, f); break;
+      case 1 * 16 + 1 * 4 + 1: coop_task_X<1>(scr, f, mt); break;
+      case 1 * 16 + 2 * 4 + 1: coop_task_X<2>(scr, f, mt); break;
+      case 2 * 16 + 1 * 4 + 1: coop_task_Y<1, true>(scr, f, mt); break;
+      case 2 * 16 + 2 * 4 + 0: coop_task_Y<2, false>(scr, f, mt); break;
+      case 3 * 16: coop_task_bil(scr, f); break;
+      default: break;
+    }
+  }
+}
+
+// S4 for team thread tid = pols | h << 4 | hb << 5: colour-contracted |Ahat|^2 of its helicity combination
+// (colour-matrix numerators; divide the team sum by kCoopCden).
+MF_HD double coop_s4_thread(double* scr, int tid) {
+  return coop_s4(coop_V(scr), coop_S(scr), coop_C(scr), tid & 15, (tid >> 4) & 1, (tid >> 5) & 1);
+}
+
+#if defined(__CUDACC__)
+// ---- device-side team driver ---------------------------------------------------------------------------------
+// Named barrier over the 64 threads of a team (ids 1..15; 0 is __syncthreads).
+__device__ __forceinline__ void coop_team_sync(int team) {
+  asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
+}
+
+// Called by all 64 threads of a team after the owner has written the input area and the team has synchronised.
+// Returns sum_{helicities} Ahat^dagger C Ahat (no couplings, no averaging) on every thread of the team.
+__device__ __forceinline__ double coop_me2_team(double* tm, int team, int tid, double mt) {
+  double* scr = tm;
+  const int warp = tid >> 5, lane = tid & 31;
+  coop_s0(scr, tm + kCoopOffIn, tid, mt);
+  coop_team_sync(team);
+#pragma unroll 1
+  for (int s = 0; s < kCoopStages; ++s) {
+    coop_run_stage(scr, s, warp, lane, mt);
+    coop_team_sync(team);
+  }
+  double acc = coop_s4_thread(scr, tid);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+  if (lane == 0) tm[kCoopOffRed + warp] = acc;
+  coop_team_sync(team);
+  return (tm[kCoopOffRed] + tm[kCoopOffRed + 1]) * (1.0 / kCoopCden);
+}
+#endif
+
+}  // namespace mf

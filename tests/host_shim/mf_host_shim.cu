@@ -3,6 +3,8 @@
 // product library (libmadflow_b200.so has no host evaluation path) and is loaded only by tests/.
 #include <cstring>
 #include "../../paper_2106_10279_b200/csrc/mf_event.cuh"
+#include "../../paper_2106_10279_b200/csrc/mf_me_coop.cuh"
+#include <vector>
 
 using namespace mf;
 
@@ -25,6 +27,23 @@ double mfh_me2(int process, const double* mom, double m_top, double alpha_s, dou
     case 3: P.me_norm = gs2 * gs2 * gs2 * gs2 / 512.0; return matrix_element<3>(P, shat, k);
   }
   return -1.0;
+}
+
+// The cooperative g g -> t tbar g g program of the fused pass (mf_me_coop.cuh), emulated on the host: the 64
+// team threads are looped over stage by stage (a barrier separates the stages on the device).
+double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {
+  std::vector<double> tm(kCoopTeamDoubles, 0.0);
+  double* in = tm.data() + kCoopOffIn;
+  for (int i = 0; i < 4; ++i) for (int m = 0; m < 4; ++m) in[4 * i + m] = mom[(2 + i) * 4 + m];
+  in[16] = 4.0 * mom[0] * mom[0];
+  for (int t = 0; t < kCoopTeam; ++t) coop_s0(tm.data(), in, t, m_top);
+  for (int s = 0; s < kCoopStages; ++s)
+    for (int w = 0; w < kCoopWarps; ++w)
+      for (int l = 0; l < 32; ++l) coop_run_stage(tm.data(), s, w, l, m_top);
+  double sum = 0.0;
+  for (int t = 0; t < kCoopTeam; ++t) sum += coop_s4_thread(tm.data(), t);
+  double gs2 = 4.0 * kPi * alpha_s;
+  return sum / kCoopCden * (gs2 * gs2 * gs2 * gs2 / 512.0);
 }
 
 void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {
