@@ -426,43 +426,49 @@ def emit_s4(L):
 
 
 def emit_tables(L, stages):
+    """Per warp ONE flat list of rounds over all stages (the last round of a stage carries the team-barrier flag).
+    The operand indices of a round are stored lane-major, padded to whole 16-byte vectors of 8 shorts, so that a
+    lane fetches all fields of its task with nvec 128-bit loads - issued one round ahead by the interpreter."""
     o = []
     w = o.append
-    table = []
-    w("struct CoopRound { short op, a, b, nfields; int offset; };")
-    max_rounds = 0
-    sched = []
-    for st in stages:
-        warps, load = schedule(st)
-        sched.append((warps, load))
-        max_rounds = max(max_rounds, max(len(x) for x in warps))
-    w("constexpr int kCoopStages = %d, kCoopWarps = 2, kCoopMaxRounds = %d;" % (len(stages), max_rounds))
+    words = []          # the table as shorts, later grouped into uint4 (8 shorts)
+    w("struct CoopRound { short op, a, b, nvec, stage, sync; int offset; };  // offset in 16-byte vectors")
+    sched = [schedule(st) for st in stages]
+    n_warps = 2
     rows, counts = [], []
-    for si, (warps, load) in enumerate(sched):
-        for wi, rounds in enumerate(warps):
-            counts.append(len(rounds))
-            row = []
-            for key, tasks in rounds:
+    for wi in range(n_warps):
+        row = []
+        for si, (warps, load) in enumerate(sched):
+            rounds = warps[wi]
+            assert rounds, "every warp needs a round in every stage (it carries the barrier)"
+            for ri, (key, tasks) in enumerate(rounds):
                 nf = len(tasks[0]["fields"])
-                off = len(table)
-                for f in range(nf):
-                    for lane in range(32):
-                        if lane < len(tasks):
-                            table.append(tasks[lane]["fields"][f])
-                        else:
-                            table.append(-1 if f == 0 else 0)
-                row.append("{%d, %d, %d, %d, %d}" % (key[0], key[1], key[2], nf, off))
-            while len(row) < max_rounds:
-                row.append("{-1, 0, 0, 0, 0}")
-            rows.append("  {" + ", ".join(row) + "},  // stage %d warp %d: ~%d flop/lane" % (si + 1, wi, load[wi]))
-    w("MF_TABLE CoopRound kCoopRounds[kCoopStages * kCoopWarps][kCoopMaxRounds] = {")
-    o.extend(rows)
+                nvec = 1
+                while nvec * 8 < nf:
+                    nvec *= 2
+                assert nvec <= 4
+                off = len(words) // 8
+                for lane in range(32):
+                    f = list(tasks[lane]["fields"]) if lane < len(tasks) else [-1]
+                    f += [0] * (nvec * 8 - len(f))
+                    words.extend(f)
+                row.append("{%d, %d, %d, %d, %d, %d, %d}" % (key[0], key[1], key[2], nvec, si, 1 if ri == len(rounds) - 1 else 0, off))
+        counts.append(len(row))
+        rows.append(row)
+    max_rounds = max(counts)
+    w("constexpr int kCoopStages = %d, kCoopWarps = %d, kCoopMaxRounds = %d;" % (len(stages), n_warps, max_rounds))
+    w("MF_CONST CoopRound kCoopRounds[kCoopWarps][kCoopMaxRounds] = {")
+    for wi, row in enumerate(rows):
+        row = row + ["{-1, 0, 0, 0, 0, 0, 0}"] * (max_rounds - len(row))
+        w("  {" + ", ".join(row) + "},  // warp %d: ~%s flop/lane per stage" % (wi, "/".join(str(ld[wi]) for _, ld in sched)))
     w("};")
-    w("MF_TABLE int kCoopNumRounds[kCoopStages * kCoopWarps] = {%s};" % ", ".join(map(str, counts)))
-    assert max(table) < 32768
-    w("MF_TABLE short kCoopTable[%d] = {" % len(table))
-    for i in range(0, len(table), 32):
-        w("  " + ", ".join("%d" % v for v in table[i:i + 32]) + ",")
+    w("MF_CONST int kCoopNumRounds[kCoopWarps] = {%s};" % ", ".join(map(str, counts)))
+    assert max(words) < 32768 and len(words) % 8 == 0
+    w("// operand indices: kCoopTable[(offset + lane * nvec + v) * 8 + j] = field 8 v + j of the lane's task (-1 in field 0 = idle)")
+    w("constexpr int kCoopTableVecs = %d;" % (len(words) // 8))
+    w("__align__(16) MF_TABLE short kCoopTable[%d] = {" % len(words))
+    for i in range(0, len(words), 32):
+        w("  " + ", ".join("%d" % v for v in words[i:i + 32]) + ",")
     w("};")
     return "\n".join(o), sched
 
@@ -478,8 +484,10 @@ def main():
     hdr = ["// GENERATED by gen_coop.py — do not edit.  Cooperative (64 threads per event) matrix element of",
            "// g g -> t tbar g g: scratch layout, task tables of stages S1-S3, straight-line stage S4.",
            "#pragma once", '#include "mf_me_prims.cuh"', "",
-           "#if defined(__CUDA_ARCH__)", "#define MF_TABLE static __device__ const", "#else",
-           "#define MF_TABLE static const", "#endif", "", "namespace mf {", "",
+           "#if defined(__CUDA_ARCH__)", "#define MF_TABLE static __device__ const", "#define MF_CONST static __constant__ const",
+           "#else", "#define MF_TABLE static const", "#define MF_CONST static const", "#endif",
+           "#if !defined(__CUDACC__)", "#define __align__(n) alignas(n)", "#endif", "",
+           "namespace mf {", "",
            "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | CVEC 8*kCoopNC | SCAL kCoopNX (each region 16-byte aligned)",
            "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopNC = %d, kCoopNX = %d;" % (L.n("V"), L.n("S"), L.n("C"), L.n("X")),
            "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 8 * kCoopNC + kCoopNX;",

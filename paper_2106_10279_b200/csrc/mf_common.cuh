@@ -17,6 +17,7 @@ namespace mf {
 // host builds (tests/host_shim) have no CUDA vector types
 struct double2 { double x, y; };
 inline double2 make_double2(double x, double y) { return double2{x, y}; }
+struct alignas(16) uint4 { unsigned x, y, z, w; };
 #endif
 
 constexpr double kPi = 3.14159265358979323846264338327950288;

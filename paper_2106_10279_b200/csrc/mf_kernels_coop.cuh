@@ -35,7 +35,7 @@ struct CoopSmem {
 // team must call it (it contains team barriers); `round` alternates the mask slot so that consecutive calls do
 // not race.  Returns 0 for threads whose event did not pass.
 __device__ __forceinline__ double coop_team_me2(double* tm, int team, int tid, unsigned round, bool pass,
-                                                const double (*k)[4], double shat, const Params& P) {
+                                                const double (*k)[4], double shat, const Params& P, CoopCursor& cur) {
   unsigned* s_mask = reinterpret_cast<unsigned*>(tm + kCoopOffMask) + 2 * (round & 1u);
   const unsigned bal = __ballot_sync(0xFFFFFFFFu, pass);
   if ((tid & 31) == 0) s_mask[tid >> 5] = bal;
@@ -54,7 +54,7 @@ __device__ __forceinline__ double coop_team_me2(double* tm, int team, int tid, u
       in[16] = shat;
     }
     coop_team_sync(team);
-    const double r = coop_me2_team(tm, team, tid, P.m_top);
+    const double r = coop_me2_team(tm, team, tid, P.m_top, cur);
     if (tid == i) me2 = r * P.me_norm;
   }
   return me2;
@@ -81,6 +81,7 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
   __syncthreads();
 
   Accum acc;
+  CoopCursor cur = coop_cursor_init(tid);
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   const uint64_t rounds = (A.n_events + stride - 1) / stride;
   uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -98,7 +99,7 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
       if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
     }
     const bool pass = valid && ev.pass;
-    const double me2 = coop_team_me2(tm, team, tid, (unsigned)rd, pass, ev.k, ev.shat, P);
+    const double me2 = coop_team_me2(tm, team, tid, (unsigned)rd, pass, ev.k, ev.shat, P, cur);
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
@@ -127,7 +128,8 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
     generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
   }
   const bool pass = valid && ev.pass;
-  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, pass, ev.k, ev.shat, P);
+  CoopCursor cur = coop_cursor_init(threadIdx.x);
+  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, pass, ev.k, ev.shat, P, cur);
   if (!valid) return;
   double mom[NF + 2][4];
   lab_momenta<PROC>(ev, mom);
@@ -159,7 +161,8 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
       for (int c = 0; c < 4; ++c) k[f][c] = m[(2 + f) * 4 + c];
     shat = 4.0 * m[0] * m[0];
   }
-  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, valid, k, shat, P);
+  CoopCursor cur = coop_cursor_init(threadIdx.x);
+  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, valid, k, shat, P, cur);
   if (valid) out[i] = me2;
 }
 

@@ -86,88 +86,121 @@ MF_HD void coop_s0(double* scr, const double* in, int tid, double mt) {
 }
 
 // ---- S1-S3: the task interpreter -----------------------------------------------------------------------------
-// f points at this lane's column of the round's field table: field j is f[32 * j].
+// The operand indices of one task: up to 32 shorts in four 16-byte vectors (registers).  The interpreter loads
+// the fields of round r+1 before it executes round r, so the table's load latency is off the critical path.
+struct CoopFields { uint4 q[4]; };
+
+MF_HD int coop_fld(const CoopFields& F, int j) {   // j is a compile-time constant after unrolling
+  const uint4& v = F.q[j >> 3];
+  const int k = (j >> 1) & 3;
+  const unsigned w = k == 0 ? v.x : k == 1 ? v.y : k == 2 ? v.z : v.w;
+  return (int)(short)((j & 1) ? (w >> 16) : (w & 0xFFFFu));
+}
+
+MF_HD CoopFields coop_load_fields(const CoopRound& R, int lane) {
+  const uint4* t = reinterpret_cast<const uint4*>(kCoopTable) + R.offset + lane * R.nvec;
+  CoopFields F;
+#pragma unroll
+  for (int v = 0; v < 4; ++v) {
+    if (v < R.nvec) {
+#if defined(__CUDA_ARCH__)
+      F.q[v] = __ldg(t + v);
+#else
+      F.q[v] = t[v];
+#endif
+    } else {
+      F.q[v] = uint4{0u, 0u, 0u, 0u};
+    }
+  }
+  return F;
+}
+
 template <int NV3, int NV4>
-MF_HD void coop_task_J(double* scr, const short* f) {
+MF_HD void coop_task_J(double* scr, const CoopFields& F) {
   const double* V = coop_V(scr);
-  const int signs = f[32 * (2 + 4 * NV3 + 3 * NV4)];
+  const int signs = coop_fld(F, 2 + 4 * NV3 + 3 * NV4);
   rvec acc = {{0.0, 0.0, 0.0, 0.0}};
 #pragma unroll
   for (int t = 0; t < NV3; ++t) {
-    const short* g = f + 32 * (2 + 4 * t);
-    const rvec J1 = coop_ld_vec(V, g[0]), P1 = coop_ld_vec(V, g[32]);
-    const rvec J2 = coop_ld_vec(V, g[64]), P2 = coop_ld_vec(V, g[96]);
+    const int g = 2 + 4 * t;
+    const rvec J1 = coop_ld_vec(V, coop_fld(F, g)), P1 = coop_ld_vec(V, coop_fld(F, g + 1));
+    const rvec J2 = coop_ld_vec(V, coop_fld(F, g + 2)), P2 = coop_ld_vec(V, coop_fld(F, g + 3));
     v3_acc(acc, ((signs >> t) & 1) ? -1.0 : 1.0, J1, P1, J2, P2);
   }
 #pragma unroll
   for (int t = 0; t < NV4; ++t) {
-    const short* g = f + 32 * (2 + 4 * NV3 + 3 * t);
-    const rvec J1 = coop_ld_vec(V, g[0]), J2 = coop_ld_vec(V, g[32]), J3 = coop_ld_vec(V, g[64]);
+    const int g = 2 + 4 * NV3 + 3 * t;
+    const rvec J1 = coop_ld_vec(V, coop_fld(F, g)), J2 = coop_ld_vec(V, coop_fld(F, g + 1));
+    const rvec J3 = coop_ld_vec(V, coop_fld(F, g + 2));
     v4_acc(acc, ((signs >> (NV3 + t)) & 1) ? -1.0 : 1.0, J1, J2, J3);
   }
-  coop_st_vec(coop_V(scr), f[0], rscale(acc, coop_X(scr)[f[32]]));
+  coop_st_vec(coop_V(scr), coop_fld(F, 0), rscale(acc, coop_X(scr)[coop_fld(F, 1)]));
 }
 
 template <int NT>
-MF_HD void coop_task_X(double* scr, const short* f, double mt) {
+MF_HD void coop_task_X(double* scr, const CoopFields& F, double mt) {
   const double* V = coop_V(scr);
   const double* S = coop_S(scr);
-  const int signs = f[32 * (3 + 2 * NT)];
+  const int signs = coop_fld(F, 3 + 2 * NT);
   spin t;
 #pragma unroll
   for (int i = 0; i < NT; ++i) {
-    const short* g = f + 32 * (3 + 2 * i);
-    const rvec J = rscale(coop_ld_vec(V, g[0]), ((signs >> i) & 1) ? -1.0 : 1.0);
-    const spin x = coop_ld_spin(S, g[32]);
+    const int g = 3 + 2 * i;
+    const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g)), ((signs >> i) & 1) ? -1.0 : 1.0);
+    const spin x = coop_ld_spin(S, coop_fld(F, g + 1));
     if (i == 0) t = slash_col(J, x);
     else spin_acc(t, slash_col(J, x));
   }
-  coop_st_spin(coop_S(scr), f[0], prop_col(coop_ld_vec(V, f[32]), mt, coop_X(scr)[f[64]], t));
+  coop_st_spin(coop_S(scr), coop_fld(F, 0),
+               prop_col(coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)], t));
 }
 
 template <int NT, bool PROP>
-MF_HD void coop_task_Y(double* scr, const short* f, double mt) {
+MF_HD void coop_task_Y(double* scr, const CoopFields& F, double mt) {
   const double* V = coop_V(scr);
   const double* S = coop_S(scr);
-  const int signs = f[32 * (3 + 2 * NT)];
+  const int signs = coop_fld(F, 3 + 2 * NT);
   spin t;
 #pragma unroll
   for (int i = 0; i < NT; ++i) {
-    const short* g = f + 32 * (3 + 2 * i);
-    const spin y = coop_ld_spin(S, g[0]);
-    const rvec J = rscale(coop_ld_vec(V, g[32]), ((signs >> i) & 1) ? -1.0 : 1.0);
+    const int g = 3 + 2 * i;
+    const spin y = coop_ld_spin(S, coop_fld(F, g));
+    const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g + 1)), ((signs >> i) & 1) ? -1.0 : 1.0);
     if (i == 0) t = slash_row(y, J);
     else spin_acc(t, slash_row(y, J));
   }
-  if (PROP) t = prop_row(t, coop_ld_vec(V, f[32]), mt, coop_X(scr)[f[64]]);
-  coop_st_spin(coop_S(scr), f[0], t);
+  if (PROP) t = prop_row(t, coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)]);
+  coop_st_spin(coop_S(scr), coop_fld(F, 0), t);
 }
 
-MF_HD void coop_task_bil(double* scr, const short* f) {
+MF_HD void coop_task_bil(double* scr, const CoopFields& F) {
   const double* S = coop_S(scr);
-  coop_st_cvec(coop_C(scr), f[0], bilinear(coop_ld_spin(S, f[32]), coop_ld_spin(S, f[64])));
+  coop_st_cvec(coop_C(scr), coop_fld(F, 0), bilinear(coop_ld_spin(S, coop_fld(F, 1)), coop_ld_spin(S, coop_fld(F, 2))));
 }
 
-// All rounds of (stage, warp) for one lane.  Rounds are uniform per warp (same op and shape for all lanes);
-// a lane whose output index is negative idles.
+// One round for one lane.  Rounds are uniform per warp (same op and shape for all lanes); a lane whose output
+// index is negative idles.
+MF_HD void coop_exec_round(double* scr, const CoopRound& R, const CoopFields& F, double mt) {
+  if (coop_fld(F, 0) < 0) return;
+  switch (R.op * 16 + R.a * 4 + R.b) {
+    case 0 * 16 + 1 * 4 + 0: coop_task_J<1, 0>(scr, F); break;
+    case 0 * 16 + 2 * 4 + 1: coop_task_J<2, 1>(scr, F); break;
+    case 0 * 16 + 3 * 4 + 3: coop_task_J<3, 3>(scr, F); break;
+    case 1 * 16 + 1 * 4 + 1: coop_task_X<1>(scr, F, mt); break;
+    case 1 * 16 + 2 * 4 + 1: coop_task_X<2>(scr, F, mt); break;
+    case 2 * 16 + 1 * 4 + 1: coop_task_Y<1, true>(scr, F, mt); break;
+    case 2 * 16 + 2 * 4 + 0: coop_task_Y<2, false>(scr, F, mt); break;
+    case 3 * 16: coop_task_bil(scr, F); break;
+    default: break;
+  }
+}
+
+// Host emulation helper (tests/host_shim): all rounds of `stage` for one (warp, lane).
 MF_HD void coop_run_stage(double* scr, int stage, int warp, int lane, double mt) {
-  const int row = stage * kCoopWarps + warp;
-  const int nr = kCoopNumRounds[row];
-  for (int r = 0; r < nr; ++r) {
-    const CoopRound R = kCoopRounds[row][r];
-    const short* f = kCoopTable + R.offset + lane;
-    if (f[0] < 0) continue;
-    switch (R.op * 16 + R.a * 4 + R.b) {
-      case 0 * 16 + 1 * 4 + 0: coop_task_J<1, 0>(scr, f); break;
-      case 0 * 16 + 2 * 4 + 1: coop_task_J<2, 1>(scr, f); break;
-      case 0 * 16 + 3 * 4 + 3: coop_task_J<3, 3>(scr, f); break;
-      case 1 * 16 + 1 * 4 + 1: coop_task_X<1>(scr, f, mt); break;
-      case 1 * 16 + 2 * 4 + 1: coop_task_X<2>(scr, f, mt); break;
-      case 2 * 16 + 1 * 4 + 1: coop_task_Y<1, true>(scr, f, mt); break;
-      case 2 * 16 + 2 * 4 + 0: coop_task_Y<2, false>(scr, f, mt); break;
-      case 3 * 16: coop_task_bil(scr, f); break;
-      default: break;
-    }
+  for (int r = 0; r < kCoopNumRounds[warp]; ++r) {
+    const CoopRound R = kCoopRounds[warp][r];
+    if (R.stage != stage) continue;
+    coop_exec_round(scr, R, coop_load_fields(R, lane), mt);
   }
 }
 
@@ -184,17 +217,34 @@ __device__ __forceinline__ void coop_team_sync(int team) {
   asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
 }
 
+// The interpreter state a thread carries from event to event: the header and operand fields of the NEXT round
+// it will execute (already loaded).
+struct CoopCursor { CoopRound R; CoopFields F; };
+
+__device__ __forceinline__ CoopCursor coop_cursor_init(int tid) {
+  CoopCursor c;
+  c.R = kCoopRounds[tid >> 5][0];
+  c.F = coop_load_fields(c.R, tid & 31);
+  return c;
+}
+
 // Called by all 64 threads of a team after the owner has written the input area and the team has synchronised.
 // Returns sum_{helicities} Ahat^dagger C Ahat (no couplings, no averaging) on every thread of the team.
-__device__ __forceinline__ double coop_me2_team(double* tm, int team, int tid, double mt) {
+__device__ __forceinline__ double coop_me2_team(double* tm, int team, int tid, double mt, CoopCursor& cur) {
   double* scr = tm;
   const int warp = tid >> 5, lane = tid & 31;
   coop_s0(scr, tm + kCoopOffIn, tid, mt);
   coop_team_sync(team);
+  const int nr = kCoopNumRounds[warp];
 #pragma unroll 1
-  for (int s = 0; s < kCoopStages; ++s) {
-    coop_run_stage(scr, s, warp, lane, mt);
-    coop_team_sync(team);
+  for (int r = 0; r < nr; ++r) {
+    // fetch round r+1 (wrapping to round 0 of the next event) before executing round r
+    CoopCursor nxt;
+    nxt.R = kCoopRounds[warp][r + 1 < nr ? r + 1 : 0];
+    nxt.F = coop_load_fields(nxt.R, lane);
+    coop_exec_round(scr, cur.R, cur.F, mt);
+    if (cur.R.sync) coop_team_sync(team);
+    cur = nxt;
   }
   double acc = coop_s4_thread(scr, tid);
 #pragma unroll
