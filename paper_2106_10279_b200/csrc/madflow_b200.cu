@@ -244,7 +244,7 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
     case 2: mf::debug_eval_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     default:
       mf::debug_eval_coop_kernel<<<(unsigned)((n_events + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
-                                   mf::kCoopTeamDoubles * 8, st>>>(p->P, A, d_out);
+                                   mf::kCoopTeamDoubles * 8 + 256, st>>>(p->P, A, d_out);
       break;
   }
   cudaError_t e = cudaGetLastError();
@@ -286,7 +286,7 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
     case 2: mf::debug_me2_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     default:
       mf::debug_me2_coop_kernel<<<(unsigned)((n + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
-                                  mf::kCoopTeamDoubles * 8, st>>>(p->P, d_mom, n, d_out);
+                                  mf::kCoopTeamDoubles * 8 + 256, st>>>(p->P, d_mom, n, d_out);
       break;
   }
   cudaError_t e = cudaGetLastError();

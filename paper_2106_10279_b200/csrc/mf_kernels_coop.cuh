@@ -18,7 +18,7 @@ constexpr int kCoopMaxTeams = 5;
 
 // shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
 struct CoopSmem {
-  int grid, hist, lnx, row, red, teams, total;
+  int grid, hist, lnx, row, red, cnt, teams, total;
   __host__ __device__ CoopSmem(int D, int nb, int nx, int n_teams) {
     auto even = [](int v) { return (v + 1) & ~1; };
     grid = 0;
@@ -26,36 +26,50 @@ struct CoopSmem {
     lnx = hist + even(D * nb);
     row = lnx + even(nx);
     red = row + even(nx);
-    teams = red + 5 * 32;
+    cnt = red + 5 * 32;
+    teams = cnt + 32;
     total = teams + n_teams * kCoopTeamDoubles;
   }
 };
 
-// |M|^2 (with couplings and averaging) of this thread's own event, computed by its team.  Every thread of the
-// team must call it (it contains team barriers); `round` alternates the mask slot so that consecutive calls do
-// not race.  Returns 0 for threads whose event did not pass.
-__device__ __forceinline__ double coop_team_me2(double* tm, int team, int tid, unsigned round, bool pass,
-                                                const double (*k)[4], double shat, const Params& P, CoopCursor& cur) {
-  unsigned* s_mask = reinterpret_cast<unsigned*>(tm + kCoopOffMask) + 2 * (round & 1u);
+// |M|^2 (with couplings and averaging) of this thread's own event.  EVERY thread of the block must call it (it
+// contains block barriers).  The events of the block that passed the cuts are ranked (ballot + prefix over the
+// warps); in step s team t computes the event of rank s * n_teams + t: its owner (any thread of the block)
+// writes the momenta into that team's input area and reads the result from the team's reduction slots.
+// s_cnt: 2 x 32 unsigned (double-buffered by `round`).  Returns 0 for threads whose event did not pass.
+__device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, unsigned* s_cnt, unsigned round,
+                                                 bool pass, const double (*k)[4], double shat, const Params& P,
+                                                 CoopCursor& cur) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+  unsigned* cnt = s_cnt + 32 * (round & 1u);
   const unsigned bal = __ballot_sync(0xFFFFFFFFu, pass);
-  if ((tid & 31) == 0) s_mask[tid >> 5] = bal;
-  coop_team_sync(team);
-  unsigned long long m = (unsigned long long)s_mask[0] | ((unsigned long long)s_mask[1] << 32);
+  if (lane == 0) cnt[warp] = __popc(bal);
+  __syncthreads();
+  int base = 0, total = 0;
+  for (int w = 0; w < n_warps; ++w) {
+    const int c = (int)cnt[w];
+    if (w < warp) base += c;
+    total += c;
+  }
+  const int rank = base + __popc(bal & ((1u << lane) - 1u));
+  const int my_step = pass ? rank / n_teams : -1, my_team = rank - (rank / n_teams) * n_teams;
+  const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam;
+  double* tm = teams + team * kCoopTeamDoubles;
+  double* mine = teams + my_team * kCoopTeamDoubles;
+  const int n_steps = (total + n_teams - 1) / n_teams;
   double me2 = 0.0;
-  double* in = tm + kCoopOffIn;
-  while (m) {
-    const int i = __ffsll((long long)m) - 1;
-    m &= m - 1;
-    if (tid == i) {
+  for (int s = 0; s < n_steps; ++s) {
+    if (s == my_step) {
+      double* in = mine + kCoopOffIn;
 #pragma unroll
       for (int f = 0; f < 4; ++f)
 #pragma unroll
         for (int c = 0; c < 4; ++c) in[4 * f + c] = k[f][c];
       in[16] = shat;
     }
-    coop_team_sync(team);
-    const double r = coop_me2_team(tm, team, tid, P.m_top, cur);
-    if (tid == i) me2 = r * P.me_norm;
+    __syncthreads();
+    coop_me2_lockstep(tm, tid, s * n_teams + team < total, P.m_top, cur);
+    if (s == my_step) me2 = (mine[kCoopOffRed] + mine[kCoopOffRed + 1]) * (P.me_norm / kCoopCden);
   }
   return me2;
 }
@@ -73,15 +87,15 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
   double* s_lnx = smem + L.lnx;
   double* s_row = smem + L.row;
   double* s_red = smem + L.red;
-  const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam;
-  double* tm = smem + L.teams + team * kCoopTeamDoubles;
+  unsigned* s_cnt = reinterpret_cast<unsigned*>(smem + L.cnt);
+  double* s_teams = smem + L.teams;
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
   for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
   __syncthreads();
 
   Accum acc;
-  CoopCursor cur = coop_cursor_init(tid);
+  CoopCursor cur = coop_cursor_init(threadIdx.x % kCoopTeam);
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   const uint64_t rounds = (A.n_events + stride - 1) / stride;
   uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -99,7 +113,7 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
       if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
     }
     const bool pass = valid && ev.pass;
-    const double me2 = coop_team_me2(tm, team, tid, (unsigned)rd, pass, ev.k, ev.shat, P, cur);
+    const double me2 = coop_block_me2(s_teams, n_teams, s_cnt, (unsigned)rd, pass, ev.k, ev.shat, P, cur);
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
@@ -115,6 +129,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
   constexpr int PROC = 3, D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   extern __shared__ double2 smem2[];
   double* tm = reinterpret_cast<double*>(smem2);
+  unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
   const int row_len = 3 * D + 4 * (NF + 2) + 9;
   const uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = idx < A.n_events;
@@ -129,7 +144,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
   }
   const bool pass = valid && ev.pass;
   CoopCursor cur = coop_cursor_init(threadIdx.x);
-  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, pass, ev.k, ev.shat, P, cur);
+  const double me2 = coop_block_me2(tm, 1, s_cnt, 0u, pass, ev.k, ev.shat, P, cur);
   if (!valid) return;
   double mom[NF + 2][4];
   lab_momenta<PROC>(ev, mom);
@@ -151,6 +166,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
                                                                     double* out) {
   extern __shared__ double2 smem2[];
   double* tm = reinterpret_cast<double*>(smem2);
+  unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = i < n;
   double k[4][4];
@@ -162,7 +178,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
     shat = 4.0 * m[0] * m[0];
   }
   CoopCursor cur = coop_cursor_init(threadIdx.x);
-  const double me2 = coop_team_me2(tm, 0, threadIdx.x, 0u, valid, k, shat, P, cur);
+  const double me2 = coop_block_me2(tm, 1, s_cnt, 0u, valid, k, shat, P, cur);
   if (valid) out[i] = me2;
 }
 

@@ -211,12 +211,7 @@ MF_HD double coop_s4_thread(double* scr, int tid) {
 }
 
 #if defined(__CUDACC__)
-// ---- device-side team driver ---------------------------------------------------------------------------------
-// Named barrier over the 64 threads of a team (ids 1..15; 0 is __syncthreads).
-__device__ __forceinline__ void coop_team_sync(int team) {
-  asm volatile("bar.sync %0, 64;" ::"r"(team + 1) : "memory");
-}
-
+// ---- device-side driver ---------------------------------------------------------------------------------
 // The interpreter state a thread carries from event to event: the header and operand fields of the NEXT round
 // it will execute (already loaded).
 struct CoopCursor { CoopRound R; CoopFields F; };
@@ -228,13 +223,15 @@ __device__ __forceinline__ CoopCursor coop_cursor_init(int tid) {
   return c;
 }
 
-// Called by all 64 threads of a team after the owner has written the input area and the team has synchronised.
-// Returns sum_{helicities} Ahat^dagger C Ahat (no couplings, no averaging) on every thread of the team.
-__device__ __forceinline__ double coop_me2_team(double* tm, int team, int tid, double mt, CoopCursor& cur) {
+// Called by EVERY thread of the block (all teams run in lock-step so that the SM fetches one instruction stream:
+// the per-event program is larger than the instruction cache) after the owners have written the input areas
+// and the block has synchronised.  Teams with `active` false only keep the barriers.  Leaves
+// sum_{helicities} Ahat^dagger C Ahat * kCoopCden (no couplings, no averaging) in the team's reduction slots.
+__device__ __forceinline__ void coop_me2_lockstep(double* tm, int tid, bool active, double mt, CoopCursor& cur) {
   double* scr = tm;
   const int warp = tid >> 5, lane = tid & 31;
-  coop_s0(scr, tm + kCoopOffIn, tid, mt);
-  coop_team_sync(team);
+  if (active) coop_s0(scr, tm + kCoopOffIn, tid, mt);
+  __syncthreads();
   const int nr = kCoopNumRounds[warp];
 #pragma unroll 1
   for (int r = 0; r < nr; ++r) {
@@ -242,16 +239,17 @@ __device__ __forceinline__ double coop_me2_team(double* tm, int team, int tid, d
     CoopCursor nxt;
     nxt.R = kCoopRounds[warp][r + 1 < nr ? r + 1 : 0];
     nxt.F = coop_load_fields(nxt.R, lane);
-    coop_exec_round(scr, cur.R, cur.F, mt);
-    if (cur.R.sync) coop_team_sync(team);
+    if (active) coop_exec_round(scr, cur.R, cur.F, mt);
+    if (cur.R.sync) __syncthreads();
     cur = nxt;
   }
-  double acc = coop_s4_thread(scr, tid);
+  if (active) {
+    double acc = coop_s4_thread(scr, tid);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
-  if (lane == 0) tm[kCoopOffRed + warp] = acc;
-  coop_team_sync(team);
-  return (tm[kCoopOffRed] + tm[kCoopOffRed + 1]) * (1.0 / kCoopCden);
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+    if (lane == 0) tm[kCoopOffRed + warp] = acc;
+  }
+  __syncthreads();
 }
 #endif
 
