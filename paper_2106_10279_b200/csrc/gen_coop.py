@@ -205,7 +205,7 @@ def task_J(L, seq, pols):
         fields += list(t[:3])
         signs |= (1 if t[3] < 0 else 0) << (len(v3) + i)
     fields.append(signs)
-    flops = 65 * len(v3) + 49 * len(v4) + 4
+    flops = 53 * len(v3) + 49 * len(v4) + 4
     return dict(op=OP_J, a=len(v3), b=len(v4), fields=fields, flops=flops)
 
 
@@ -415,13 +415,16 @@ def emit_s4(L):
         first = True
         for (i, j) in groups[v]:
             a, b = "A%d%d%d%d" % perms[i], "A%d%d%d%d" % perms[j]
-            w("  g %s %sr * %sr + %si * %si;" % ("=" if first else "+=", a, b, a, b))
+            if first:
+                w("  g = fma(%si, %si, %sr * %sr);" % (a, b, a, b))
+            else:
+                w("  g = fma(%si, %si, fma(%sr, %sr, g));" % (a, b, a, b))
             first = False
-        w("  acc += %.1f * g;" % v)
+        w("  acc = fma(%.1f, g, acc);" % v)
     w("  return acc;")
     w("}")
     npairs = sum(len(v) for v in groups.values())
-    flops = 24 * 32 + 48 * 14 + 4 * 2 * 24 + 4 * npairs + 2 * len(groups)
+    flops = 24 * 30 + 48 * 14 + 4 * 2 * 24 + 4 * npairs + len(groups)
     return "\n".join(o), Cden, flops
 
 

@@ -78,8 +78,8 @@ def colour_matrix(n):
 
 # ----------------------------------------------------------------------------------------------------
 # fp64 operations (adds + multiplies as written; an FMA counts 2) of each primitive of mf_me_prims.cuh
-FLOPS = {"rdot": 7, "radd": 4, "rsub": 4, "rscale": 4, "v3_acc": 65, "v4_acc": 49, "slash_col": 42, "slash_row": 42,
-         "spin_acc": 8, "prop_col": 66, "prop_row": 66, "sdot": 32, "bilinear": 72, "cdot_r": 14}
+FLOPS = {"rdot": 7, "radd": 4, "rsub": 4, "rscale": 4, "v3_acc": 53, "v4_acc": 49, "slash_col": 42, "slash_row": 42,
+         "spin_acc": 8, "prop_col": 66, "prop_row": 66, "sdot": 30, "bilinear": 72, "cdot_r": 14}
 
 
 def count_flops(line):

@@ -14,7 +14,7 @@
 
 namespace mf {
 
-constexpr int kCoopMaxTeams = 5;
+constexpr int kCoopMaxTeams = 4;
 
 // shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
 struct CoopSmem {

@@ -149,7 +149,7 @@ MF_HD void coop_task_X(double* scr, const CoopFields& F, double mt) {
     const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g)), ((signs >> i) & 1) ? -1.0 : 1.0);
     const spin x = coop_ld_spin(S, coop_fld(F, g + 1));
     if (i == 0) t = slash_col(J, x);
-    else spin_acc(t, slash_col(J, x));
+    else slash_col_acc(t, J, x);
   }
   coop_st_spin(coop_S(scr), coop_fld(F, 0),
                prop_col(coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)], t));
@@ -167,7 +167,7 @@ MF_HD void coop_task_Y(double* scr, const CoopFields& F, double mt) {
     const spin y = coop_ld_spin(S, coop_fld(F, g));
     const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g + 1)), ((signs >> i) & 1) ? -1.0 : 1.0);
     if (i == 0) t = slash_row(y, J);
-    else spin_acc(t, slash_row(y, J));
+    else slash_row_acc(t, y, J);
   }
   if (PROP) t = prop_row(t, coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)]);
   coop_st_spin(coop_S(scr), coop_fld(F, 0), t);

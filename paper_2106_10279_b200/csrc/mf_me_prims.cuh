@@ -47,22 +47,22 @@ MF_HD rvec rsub(const rvec& a, const rvec& b) {
 // ---- gluon vertices (colour-ordered Feynman rules, all momenta incoming) -----------------------------
 // V3^r(J1,P1; J2,P2) = (J1.J2)(P1-P2)^r + J2^r ((P2-Q).J1) + J1^r ((Q-P1).J2),  Q = -(P1+P2)
 //                    = (J1.J2)(P1-P2)^r + J2^r ((P1+2P2).J1) - J1^r ((2P1+P2).J2)
-// acc += sgn * V3
+//                    = (J1.J2)(P1-P2)^r + 2 (P2.J1) J2^r - 2 (P1.J2) J1^r
+// the last line by current conservation, P.J(P) = 0, which holds for the polarisation vectors (k.eps = 0) and
+// for every off-shell current built from them by this recursion (Berends-Giele).  acc += sgn * V3, sgn = +-1.
 MF_HD void v3_acc(rvec& acc, double sgn, const rvec& J1, const rvec& P1, const rvec& J2, const rvec& P2) {
-  double j12 = rdot(J1, J2);
-  rvec a, b;
-#pragma unroll
-  for (int m = 0; m < 4; ++m) { a.v[m] = P1.v[m] + 2.0 * P2.v[m]; b.v[m] = 2.0 * P1.v[m] + P2.v[m]; }
-  double c1 = rdot(a, J1), c2 = rdot(b, J2);
+  const double s12 = sgn * rdot(J1, J2);
+  const double sgn2 = sgn + sgn;
+  const double s1 = sgn2 * rdot(P2, J1), s2 = -sgn2 * rdot(P1, J2);
 #pragma unroll
   for (int m = 0; m < 4; ++m)
-    acc.v[m] += sgn * (j12 * (P1.v[m] - P2.v[m]) + c1 * J2.v[m] - c2 * J1.v[m]);
+    acc.v[m] = fma(s2, J1.v[m], fma(s1, J2.v[m], fma(s12, P1.v[m] - P2.v[m], acc.v[m])));
 }
-// V4^r(J1,J2,J3) = 2 (J1.J3) J2^r - (J2.J3) J1^r - (J1.J2) J3^r ;  acc += sgn * V4
+// V4^r(J1,J2,J3) = 2 (J1.J3) J2^r - (J2.J3) J1^r - (J1.J2) J3^r ;  acc += sgn * V4, sgn = +-1
 MF_HD void v4_acc(rvec& acc, double sgn, const rvec& J1, const rvec& J2, const rvec& J3) {
-  double j13 = rdot(J1, J3), j23 = rdot(J2, J3), j12 = rdot(J1, J2);
+  const double a2 = (sgn + sgn) * rdot(J1, J3), a1 = -sgn * rdot(J2, J3), a3 = -sgn * rdot(J1, J2);
 #pragma unroll
-  for (int m = 0; m < 4; ++m) acc.v[m] += sgn * (2.0 * j13 * J2.v[m] - j23 * J1.v[m] - j12 * J3.v[m]);
+  for (int m = 0; m < 4; ++m) acc.v[m] = fma(a3, J3.v[m], fma(a1, J1.v[m], fma(a2, J2.v[m], acc.v[m])));
 }
 MF_HD rvec rscale(const rvec& a, double s) {
   rvec o;
@@ -109,6 +109,29 @@ MF_HD spin slash_row(const spin& r, const rvec& a) {
   o.im[3] = -a1 * r.im[0] + a2 * r.re[0] + ap * r.im[1];
   return o;
 }
+// acc += a-slash c  (column) and acc += r a-slash (row), every component as one FMA chain onto acc
+MF_HD void slash_col_acc(spin& o, const rvec& a, const spin& c) {
+  const double am = a.v[0] - a.v[3], ap = a.v[0] + a.v[3], a1 = a.v[1], a2 = a.v[2];
+  o.re[0] = fma(-a2, c.im[3], fma(-a1, c.re[3], fma(am, c.re[2], o.re[0])));
+  o.im[0] = fma(a2, c.re[3], fma(-a1, c.im[3], fma(am, c.im[2], o.im[0])));
+  o.re[1] = fma(ap, c.re[3], fma(a2, c.im[2], fma(-a1, c.re[2], o.re[1])));
+  o.im[1] = fma(ap, c.im[3], fma(-a2, c.re[2], fma(-a1, c.im[2], o.im[1])));
+  o.re[2] = fma(a2, c.im[1], fma(a1, c.re[1], fma(ap, c.re[0], o.re[2])));
+  o.im[2] = fma(-a2, c.re[1], fma(a1, c.im[1], fma(ap, c.im[0], o.im[2])));
+  o.re[3] = fma(am, c.re[1], fma(-a2, c.im[0], fma(a1, c.re[0], o.re[3])));
+  o.im[3] = fma(am, c.im[1], fma(a2, c.re[0], fma(a1, c.im[0], o.im[3])));
+}
+MF_HD void slash_row_acc(spin& o, const spin& r, const rvec& a) {
+  const double am = a.v[0] - a.v[3], ap = a.v[0] + a.v[3], a1 = a.v[1], a2 = a.v[2];
+  o.re[0] = fma(-a2, r.im[3], fma(a1, r.re[3], fma(ap, r.re[2], o.re[0])));
+  o.im[0] = fma(a2, r.re[3], fma(a1, r.im[3], fma(ap, r.im[2], o.im[0])));
+  o.re[1] = fma(am, r.re[3], fma(a2, r.im[2], fma(a1, r.re[2], o.re[1])));
+  o.im[1] = fma(am, r.im[3], fma(-a2, r.re[2], fma(a1, r.im[2], o.im[1])));
+  o.re[2] = fma(a2, r.im[1], fma(-a1, r.re[1], fma(am, r.re[0], o.re[2])));
+  o.im[2] = fma(-a2, r.re[1], fma(-a1, r.im[1], fma(am, r.im[0], o.im[2])));
+  o.re[3] = fma(ap, r.re[1], fma(-a2, r.im[0], fma(-a1, r.re[0], o.re[3])));
+  o.im[3] = fma(ap, r.im[1], fma(a2, r.re[0], fma(-a1, r.im[0], o.im[3])));
+}
 MF_HD void spin_acc(spin& acc, const spin& a) {
 #pragma unroll
   for (int m = 0; m < 4; ++m) { acc.re[m] += a.re[m]; acc.im[m] += a.im[m]; }
@@ -126,13 +149,19 @@ MF_HD spin prop_row(const spin& r, const rvec& q, double m, double idn) {
   for (int k = 0; k < 4; ++k) { o.re[k] = -(t.re[k] + m * r.re[k]) * idn; o.im[k] = -(t.im[k] + m * r.im[k]) * idn; }
   return o;
 }
-// row . column
+// row . column (two FMA chains)
 MF_HD cplx sdot(const spin& r, const spin& c) {
-  cplx o = {0.0, 0.0};
+  cplx o;
+  o.re = r.re[0] * c.re[0];
+  o.im = r.re[0] * c.im[0];
+  o.re = fma(-r.im[0], c.im[0], o.re);
+  o.im = fma(r.im[0], c.re[0], o.im);
 #pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    o.re += r.re[k] * c.re[k] - r.im[k] * c.im[k];
-    o.im += r.re[k] * c.im[k] + r.im[k] * c.re[k];
+  for (int k = 1; k < 4; ++k) {
+    o.re = fma(r.re[k], c.re[k], o.re);
+    o.im = fma(r.re[k], c.im[k], o.im);
+    o.re = fma(-r.im[k], c.im[k], o.re);
+    o.im = fma(r.im[k], c.re[k], o.im);
   }
   return o;
 }
