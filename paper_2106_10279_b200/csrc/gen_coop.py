@@ -300,23 +300,39 @@ def build_stages(L):
     return [s1, s2, s3]
 
 
+# tasks a lane may interleave in one round, by task shape (op, a, b): independent instruction streams hide the
+# FP64 and shared-memory latencies that two warps per scheduler cannot
+MAX_MULT = {(OP_J, 1, 0): 1, (OP_J, 2, 1): 2, (OP_J, 3, 3): 2, (OP_XCOL, 1, 1): 1, (OP_XCOL, 2, 1): 2,
+            (OP_YROW, 1, 1): 1, (OP_YROW, 2, 0): 2, (OP_BIL, 0, 0): 4}
+
+
 def schedule(stage_tasks, n_warps=2):
-    """groups tasks of equal (op, a, b) into warp-rounds of 32 and balances them over the warps (greedy)"""
+    """Splits the tasks of a stage into warp rounds.  A round = up to 32 * m tasks of equal shape; lane l runs tasks
+    l, 32 + l, ... of the round interleaved (m <= MAX_MULT).  Large groups are halved between the two warps, small
+    ones go whole to the less loaded warp."""
     groups = {}
     for t in stage_tasks:
         groups.setdefault((t["op"], t["a"], t["b"]), []).append(t)
-    rounds = []
-    for key in sorted(groups):
-        ts = groups[key]
-        for i in range(0, len(ts), 32):
-            rounds.append((key, ts[i:i + 32]))
-    rounds.sort(key=lambda r: -r[1][0]["flops"])
     warps = [[] for _ in range(n_warps)]
     load = [0] * n_warps
-    for r in rounds:
-        w = load.index(min(load))
-        warps[w].append(r)
-        load[w] += r[1][0]["flops"]
+
+    def add_rounds(w, key, ts):
+        cap = 32 * MAX_MULT[key]
+        for i in range(0, len(ts), cap):
+            chunk = ts[i:i + cap]
+            m = (len(chunk) + 31) // 32
+            warps[w].append((key, m, chunk))
+            load[w] += chunk[0]["flops"] * m
+
+    for key in sorted(groups, key=lambda k: -groups[k][0]["flops"] * len(groups[k])):
+        ts = groups[key]
+        if len(ts) >= 64:
+            half = (len(ts) // 2 + 31) // 32 * 32 if len(ts) % 64 else len(ts) // 2
+            lo = load.index(min(load))          # the less loaded warp takes the larger part
+            add_rounds(lo, key, ts[:half])
+            add_rounds(1 - lo, key, ts[half:])
+        else:
+            add_rounds(load.index(min(load)), key, ts)
     return warps, load
 
 
@@ -429,33 +445,40 @@ def emit_s4(L):
 
 
 def emit_tables(L, stages):
-    """Per warp ONE flat list of rounds over all stages (the last round of a stage carries the team-barrier flag).
-    The operand indices of a round are stored lane-major, padded to whole 16-byte vectors of 8 shorts, so that a
-    lane fetches all fields of its task with nvec 128-bit loads - issued one round ahead by the interpreter."""
+    """Per warp ONE flat list of rounds over all stages (the last round of a stage carries the barrier flag).  The
+    operand indices of a round are stored as 16-byte vectors of 8 shorts, vector (t, v) of all 32 lanes contiguous
+    (t = task slot of the lane, v = vector of the task), so a warp fetches them with conflict-free 128-bit loads."""
     o = []
     w = o.append
     words = []          # the table as shorts, later grouped into uint4 (8 shorts)
-    w("struct CoopRound { short op, a, b, nvec, stage, sync; int offset; };  // offset in 16-byte vectors")
+    w("struct CoopRound { short variant, m, nvec, stage, sync, pad; int offset; };  // offset in 16-byte vectors")
     sched = [schedule(st) for st in stages]
     n_warps = 2
+    variants = []       # (op, a, b, m) in order of first use
     rows, counts = [], []
     for wi in range(n_warps):
         row = []
         for si, (warps, load) in enumerate(sched):
             rounds = warps[wi]
             assert rounds, "every warp needs a round in every stage (it carries the barrier)"
-            for ri, (key, tasks) in enumerate(rounds):
+            for ri, (key, m, tasks) in enumerate(rounds):
                 nf = len(tasks[0]["fields"])
                 nvec = 1
                 while nvec * 8 < nf:
                     nvec *= 2
                 assert nvec <= 4
+                var = key + (m,)
+                if var not in variants:
+                    variants.append(var)
                 off = len(words) // 8
-                for lane in range(32):
-                    f = list(tasks[lane]["fields"]) if lane < len(tasks) else [-1]
-                    f += [0] * (nvec * 8 - len(f))
-                    words.extend(f)
-                row.append("{%d, %d, %d, %d, %d, %d, %d}" % (key[0], key[1], key[2], nvec, si, 1 if ri == len(rounds) - 1 else 0, off))
+                for t in range(m):
+                    for v in range(nvec):
+                        for lane in range(32):
+                            i = t * 32 + lane
+                            f = list(tasks[i]["fields"]) if i < len(tasks) else [-1]
+                            f += [0] * (nvec * 8 - len(f))
+                            words.extend(f[8 * v:8 * v + 8])
+                row.append("{%d, %d, %d, %d, %d, 0, %d}" % (variants.index(var), m, nvec, si, 1 if ri == len(rounds) - 1 else 0, off))
         counts.append(len(row))
         rows.append(row)
     max_rounds = max(counts)
@@ -466,8 +489,22 @@ def emit_tables(L, stages):
         w("  {" + ", ".join(row) + "},  // warp %d: ~%s flop/lane per stage" % (wi, "/".join(str(ld[wi]) for _, ld in sched)))
     w("};")
     w("MF_CONST int kCoopNumRounds[kCoopWarps] = {%s};" % ", ".join(map(str, counts)))
+    names = {OP_J: "CoopTaskJ<%d, %d>", OP_XCOL: "CoopTaskX<%d>", OP_YROW: "CoopTaskY<%d, %s>", OP_BIL: "CoopTaskBil"}
+    w("// the (task shape, tasks per lane) combinations the rounds use: X(variant id, tasks per lane, task type)")
+    w("#define MF_COOP_VARIANTS(X) \\")
+    for i, (op, a, b, m) in enumerate(variants):
+        if op == OP_J:
+            nm = names[op] % (a, b)
+        elif op == OP_XCOL:
+            nm = names[op] % a
+        elif op == OP_YROW:
+            nm = names[op] % (a, "true" if b else "false")
+        else:
+            nm = names[op]
+        w("  X(%d, %d, %s)%s" % (i, m, nm.replace(", ", " MF_COMMA "), " \\" if i + 1 < len(variants) else ""))
     assert max(words) < 32768 and len(words) % 8 == 0
-    w("// operand indices: kCoopTable[(offset + lane * nvec + v) * 8 + j] = field 8 v + j of the lane's task (-1 in field 0 = idle)")
+    w("// operand indices: vector (offset + (t * nvec + v) * 32 + lane) holds fields 8 v .. 8 v + 7 of task slot t of the lane")
+    w("// (-1 in field 0 = idle slot)")
     w("constexpr int kCoopTableVecs = %d;" % (len(words) // 8))
     w("__align__(16) MF_TABLE short kCoopTable[%d] = {" % len(words))
     for i in range(0, len(words), 32):

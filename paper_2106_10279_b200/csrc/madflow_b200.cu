@@ -159,6 +159,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     for (int u = 0; u < 2; ++u)
       if ((e = cudaFuncSetAttribute(pass_fn(3, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem)) !=
           cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
+    if ((e = cudaFuncSetAttribute((const void*)mf::debug_eval_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  mf::kCoopDebugSmemBytes)) != cudaSuccess ||
+        (e = cudaFuncSetAttribute((const void*)mf::debug_me2_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  mf::kCoopDebugSmemBytes)) != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   } else {
     p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + 2 * P.pdf_nx + 5 * 32) * sizeof(double);
   }
@@ -244,7 +248,7 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
     case 2: mf::debug_eval_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     default:
       mf::debug_eval_coop_kernel<<<(unsigned)((n_events + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
-                                   mf::kCoopTeamDoubles * 8 + 256, st>>>(p->P, A, d_out);
+                                   mf::kCoopDebugSmemBytes, st>>>(p->P, A, d_out);
       break;
   }
   cudaError_t e = cudaGetLastError();
@@ -286,7 +290,7 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
     case 2: mf::debug_me2_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     default:
       mf::debug_me2_coop_kernel<<<(unsigned)((n + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
-                                  mf::kCoopTeamDoubles * 8 + 256, st>>>(p->P, d_mom, n, d_out);
+                                  mf::kCoopDebugSmemBytes, st>>>(p->P, d_mom, n, d_out);
       break;
   }
   cudaError_t e = cudaGetLastError();

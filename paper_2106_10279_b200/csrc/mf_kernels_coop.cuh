@@ -18,7 +18,7 @@ constexpr int kCoopMaxTeams = 4;
 
 // shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
 struct CoopSmem {
-  int grid, hist, lnx, row, red, cnt, teams, total;
+  int grid, hist, lnx, row, red, cnt, tab, teams, total;
   __host__ __device__ CoopSmem(int D, int nb, int nx, int n_teams) {
     auto even = [](int v) { return (v + 1) & ~1; };
     grid = 0;
@@ -27,19 +27,29 @@ struct CoopSmem {
     row = lnx + even(nx);
     red = row + even(nx);
     cnt = red + 5 * 32;
-    teams = cnt + 32;
+    tab = cnt + 32;
+    teams = tab + 2 * kCoopTableVecs;
     total = teams + n_teams * kCoopTeamDoubles;
   }
 };
+
+// shared memory of the single-team debug kernels: team | rank counters | operand table
+constexpr int kCoopDebugSmemBytes = (kCoopTeamDoubles + 32 + 2 * kCoopTableVecs) * 8;
+
+// copies the operand table into shared memory (all threads of the block; the caller synchronises)
+__device__ __forceinline__ void coop_load_table(uint4* s_tab) {
+  const uint4* g = reinterpret_cast<const uint4*>(kCoopTable);
+  for (int i = threadIdx.x; i < kCoopTableVecs; i += blockDim.x) s_tab[i] = g[i];
+}
 
 // |M|^2 (with couplings and averaging) of this thread's own event.  EVERY thread of the block must call it (it
 // contains block barriers).  The events of the block that passed the cuts are ranked (ballot + prefix over the
 // warps); in step s team t computes the event of rank s * n_teams + t: its owner (any thread of the block)
 // writes the momenta into that team's input area and reads the result from the team's reduction slots.
 // s_cnt: 2 x 32 unsigned (double-buffered by `round`).  Returns 0 for threads whose event did not pass.
-__device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, unsigned* s_cnt, unsigned round,
-                                                 bool pass, const double (*k)[4], double shat, const Params& P,
-                                                 CoopCursor& cur) {
+__device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, const uint4* tab, unsigned* s_cnt,
+                                                 unsigned round, bool pass, const double (*k)[4], double shat,
+                                                 const Params& P) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   unsigned* cnt = s_cnt + 32 * (round & 1u);
   const unsigned bal = __ballot_sync(0xFFFFFFFFu, pass);
@@ -68,7 +78,7 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, uns
       in[16] = shat;
     }
     __syncthreads();
-    coop_me2_lockstep(tm, tid, s * n_teams + team < total, P.m_top, cur);
+    coop_me2_lockstep(tm, tab, tid, s * n_teams + team < total, P.m_top);
     if (s == my_step) me2 = (mine[kCoopOffRed] + mine[kCoopOffRed + 1]) * (P.me_norm / kCoopCden);
   }
   return me2;
@@ -89,13 +99,14 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
   double* s_red = smem + L.red;
   unsigned* s_cnt = reinterpret_cast<unsigned*>(smem + L.cnt);
   double* s_teams = smem + L.teams;
+  uint4* s_tab = reinterpret_cast<uint4*>(smem + L.tab);
+  coop_load_table(s_tab);
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
   for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
   __syncthreads();
 
   Accum acc;
-  CoopCursor cur = coop_cursor_init(threadIdx.x % kCoopTeam);
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   const uint64_t rounds = (A.n_events + stride - 1) / stride;
   uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -113,7 +124,7 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
       if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
     }
     const bool pass = valid && ev.pass;
-    const double me2 = coop_block_me2(s_teams, n_teams, s_cnt, (unsigned)rd, pass, ev.k, ev.shat, P, cur);
+    const double me2 = coop_block_me2(s_teams, n_teams, s_tab, s_cnt, (unsigned)rd, pass, ev.k, ev.shat, P);
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
@@ -130,6 +141,9 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
   extern __shared__ double2 smem2[];
   double* tm = reinterpret_cast<double*>(smem2);
   unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
+  uint4* s_tab = reinterpret_cast<uint4*>(tm + kCoopTeamDoubles + 32);
+  coop_load_table(s_tab);
+  __syncthreads();
   const int row_len = 3 * D + 4 * (NF + 2) + 9;
   const uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = idx < A.n_events;
@@ -143,8 +157,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
     generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
   }
   const bool pass = valid && ev.pass;
-  CoopCursor cur = coop_cursor_init(threadIdx.x);
-  const double me2 = coop_block_me2(tm, 1, s_cnt, 0u, pass, ev.k, ev.shat, P, cur);
+  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, 0u, pass, ev.k, ev.shat, P);
   if (!valid) return;
   double mom[NF + 2][4];
   lab_momenta<PROC>(ev, mom);
@@ -167,6 +180,9 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
   extern __shared__ double2 smem2[];
   double* tm = reinterpret_cast<double*>(smem2);
   unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
+  uint4* s_tab = reinterpret_cast<uint4*>(tm + kCoopTeamDoubles + 32);
+  coop_load_table(s_tab);
+  __syncthreads();
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = i < n;
   double k[4][4];
@@ -177,8 +193,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
       for (int c = 0; c < 4; ++c) k[f][c] = m[(2 + f) * 4 + c];
     shat = 4.0 * m[0] * m[0];
   }
-  CoopCursor cur = coop_cursor_init(threadIdx.x);
-  const double me2 = coop_block_me2(tm, 1, s_cnt, 0u, valid, k, shat, P, cur);
+  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, 0u, valid, k, shat, P);
   if (valid) out[i] = me2;
 }
 

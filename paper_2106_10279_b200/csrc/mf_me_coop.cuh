@@ -86,121 +86,146 @@ MF_HD void coop_s0(double* scr, const double* in, int tid, double mt) {
 }
 
 // ---- S1-S3: the task interpreter -----------------------------------------------------------------------------
-// The operand indices of one task: up to 32 shorts in four 16-byte vectors (registers).  The interpreter loads
-// the fields of round r+1 before it executes round r, so the table's load latency is off the critical path.
-struct CoopFields { uint4 q[4]; };
+// The operand indices of one task: NVEC 16-byte vectors of 8 shorts (registers).
+template <int NVEC> struct CoopFields { uint4 q[NVEC]; };
 
-MF_HD int coop_fld(const CoopFields& F, int j) {   // j is a compile-time constant after unrolling
+template <int NVEC>
+MF_HD int coop_fld(const CoopFields<NVEC>& F, int j) {   // j is a compile-time constant after unrolling
   const uint4& v = F.q[j >> 3];
   const int k = (j >> 1) & 3;
   const unsigned w = k == 0 ? v.x : k == 1 ? v.y : k == 2 ? v.z : v.w;
   return (int)(short)((j & 1) ? (w >> 16) : (w & 0xFFFFu));
 }
 
-MF_HD CoopFields coop_load_fields(const CoopRound& R, int lane) {
-  const uint4* t = reinterpret_cast<const uint4*>(kCoopTable) + R.offset + lane * R.nvec;
-  CoopFields F;
+// `tab` is the operand table (kCoopTable; a shared-memory copy on the device), t the lane's task slot
+template <int NVEC>
+MF_HD CoopFields<NVEC> coop_load_fields(const uint4* tab, const CoopRound& R, int t, int lane) {
+  CoopFields<NVEC> F;
 #pragma unroll
-  for (int v = 0; v < 4; ++v) {
-    if (v < R.nvec) {
-#if defined(__CUDA_ARCH__)
-      F.q[v] = __ldg(t + v);
-#else
-      F.q[v] = t[v];
-#endif
-    } else {
-      F.q[v] = uint4{0u, 0u, 0u, 0u};
-    }
-  }
+  for (int v = 0; v < NVEC; ++v) F.q[v] = tab[R.offset + (t * NVEC + v) * 32 + lane];
   return F;
 }
 
+// One task type = how many operand vectors it needs, how its result is computed from the scratch (calc: loads
+// and arithmetic only) and where the result goes (store).  Keeping calc free of stores lets the compiler
+// interleave the instruction streams of the tasks a lane runs in one round.
 template <int NV3, int NV4>
-MF_HD void coop_task_J(double* scr, const CoopFields& F) {
-  const double* V = coop_V(scr);
-  const int signs = coop_fld(F, 2 + 4 * NV3 + 3 * NV4);
-  rvec acc = {{0.0, 0.0, 0.0, 0.0}};
+struct CoopTaskJ {   // gluon current: [out, iP2, (J1, P1, J2, P2) x NV3, (J1, J2, J3) x NV4, signs]
+  static constexpr int NVEC = (3 + 4 * NV3 + 3 * NV4 + 7) / 8 == 3 ? 4 : (3 + 4 * NV3 + 3 * NV4 + 7) / 8;
+  typedef rvec Out;
+  MF_HD static rvec calc(const double* scr_c, const CoopFields<NVEC>& F, double) {
+    double* scr = const_cast<double*>(scr_c);
+    const double* V = coop_V(scr);
+    const int signs = coop_fld(F, 2 + 4 * NV3 + 3 * NV4);
+    rvec acc = {{0.0, 0.0, 0.0, 0.0}};
 #pragma unroll
-  for (int t = 0; t < NV3; ++t) {
-    const int g = 2 + 4 * t;
-    const rvec J1 = coop_ld_vec(V, coop_fld(F, g)), P1 = coop_ld_vec(V, coop_fld(F, g + 1));
-    const rvec J2 = coop_ld_vec(V, coop_fld(F, g + 2)), P2 = coop_ld_vec(V, coop_fld(F, g + 3));
-    v3_acc(acc, ((signs >> t) & 1) ? -1.0 : 1.0, J1, P1, J2, P2);
-  }
+    for (int t = 0; t < NV3; ++t) {
+      const int g = 2 + 4 * t;
+      const rvec J1 = coop_ld_vec(V, coop_fld(F, g)), P1 = coop_ld_vec(V, coop_fld(F, g + 1));
+      const rvec J2 = coop_ld_vec(V, coop_fld(F, g + 2)), P2 = coop_ld_vec(V, coop_fld(F, g + 3));
+      v3_acc(acc, ((signs >> t) & 1) ? -1.0 : 1.0, J1, P1, J2, P2);
+    }
 #pragma unroll
-  for (int t = 0; t < NV4; ++t) {
-    const int g = 2 + 4 * NV3 + 3 * t;
-    const rvec J1 = coop_ld_vec(V, coop_fld(F, g)), J2 = coop_ld_vec(V, coop_fld(F, g + 1));
-    const rvec J3 = coop_ld_vec(V, coop_fld(F, g + 2));
-    v4_acc(acc, ((signs >> (NV3 + t)) & 1) ? -1.0 : 1.0, J1, J2, J3);
+    for (int t = 0; t < NV4; ++t) {
+      const int g = 2 + 4 * NV3 + 3 * t;
+      const rvec J1 = coop_ld_vec(V, coop_fld(F, g)), J2 = coop_ld_vec(V, coop_fld(F, g + 1));
+      const rvec J3 = coop_ld_vec(V, coop_fld(F, g + 2));
+      v4_acc(acc, ((signs >> (NV3 + t)) & 1) ? -1.0 : 1.0, J1, J2, J3);
+    }
+    return rscale(acc, coop_X(scr)[coop_fld(F, 1)]);
   }
-  coop_st_vec(coop_V(scr), coop_fld(F, 0), rscale(acc, coop_X(scr)[coop_fld(F, 1)]));
-}
+  MF_HD static void store(double* scr, int out, const rvec& r) { coop_st_vec(coop_V(scr), out, r); }
+};
 
 template <int NT>
-MF_HD void coop_task_X(double* scr, const CoopFields& F, double mt) {
-  const double* V = coop_V(scr);
-  const double* S = coop_S(scr);
-  const int signs = coop_fld(F, 3 + 2 * NT);
-  spin t;
+struct CoopTaskX {   // propagated column quark current: [out, qX, idX, (J, X) x NT, signs]
+  static constexpr int NVEC = 1;
+  typedef spin Out;
+  MF_HD static spin calc(const double* scr_c, const CoopFields<NVEC>& F, double mt) {
+    double* scr = const_cast<double*>(scr_c);
+    const double* V = coop_V(scr);
+    const double* S = coop_S(scr);
+    const int signs = coop_fld(F, 3 + 2 * NT);
+    spin t;
 #pragma unroll
-  for (int i = 0; i < NT; ++i) {
-    const int g = 3 + 2 * i;
-    const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g)), ((signs >> i) & 1) ? -1.0 : 1.0);
-    const spin x = coop_ld_spin(S, coop_fld(F, g + 1));
-    if (i == 0) t = slash_col(J, x);
-    else slash_col_acc(t, J, x);
+    for (int i = 0; i < NT; ++i) {
+      const int g = 3 + 2 * i;
+      const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g)), ((signs >> i) & 1) ? -1.0 : 1.0);
+      const spin x = coop_ld_spin(S, coop_fld(F, g + 1));
+      if (i == 0) t = slash_col(J, x);
+      else slash_col_acc(t, J, x);
+    }
+    return prop_col(coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)], t);
   }
-  coop_st_spin(coop_S(scr), coop_fld(F, 0),
-               prop_col(coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)], t));
-}
+  MF_HD static void store(double* scr, int out, const spin& r) { coop_st_spin(coop_S(scr), out, r); }
+};
 
 template <int NT, bool PROP>
-MF_HD void coop_task_Y(double* scr, const CoopFields& F, double mt) {
-  const double* V = coop_V(scr);
-  const double* S = coop_S(scr);
-  const int signs = coop_fld(F, 3 + 2 * NT);
-  spin t;
+struct CoopTaskY {   // row quark current, propagated or not: [out, qY, idY, (Y, J) x NT, signs]
+  static constexpr int NVEC = 1;
+  typedef spin Out;
+  MF_HD static spin calc(const double* scr_c, const CoopFields<NVEC>& F, double mt) {
+    double* scr = const_cast<double*>(scr_c);
+    const double* V = coop_V(scr);
+    const double* S = coop_S(scr);
+    const int signs = coop_fld(F, 3 + 2 * NT);
+    spin t;
 #pragma unroll
-  for (int i = 0; i < NT; ++i) {
-    const int g = 3 + 2 * i;
-    const spin y = coop_ld_spin(S, coop_fld(F, g));
-    const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g + 1)), ((signs >> i) & 1) ? -1.0 : 1.0);
-    if (i == 0) t = slash_row(y, J);
-    else slash_row_acc(t, y, J);
+    for (int i = 0; i < NT; ++i) {
+      const int g = 3 + 2 * i;
+      const spin y = coop_ld_spin(S, coop_fld(F, g));
+      const rvec J = rscale(coop_ld_vec(V, coop_fld(F, g + 1)), ((signs >> i) & 1) ? -1.0 : 1.0);
+      if (i == 0) t = slash_row(y, J);
+      else slash_row_acc(t, y, J);
+    }
+    if (PROP) t = prop_row(t, coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)]);
+    return t;
   }
-  if (PROP) t = prop_row(t, coop_ld_vec(V, coop_fld(F, 1)), mt, coop_X(scr)[coop_fld(F, 2)]);
-  coop_st_spin(coop_S(scr), coop_fld(F, 0), t);
+  MF_HD static void store(double* scr, int out, const spin& r) { coop_st_spin(coop_S(scr), out, r); }
+};
+
+struct CoopTaskBil {   // fermion bilinear row gamma^mu col: [out, row, col]
+  static constexpr int NVEC = 1;
+  typedef cvec Out;
+  MF_HD static cvec calc(const double* scr_c, const CoopFields<NVEC>& F, double) {
+    const double* S = coop_S(const_cast<double*>(scr_c));
+    return bilinear(coop_ld_spin(S, coop_fld(F, 1)), coop_ld_spin(S, coop_fld(F, 2)));
+  }
+  MF_HD static void store(double* scr, int out, const cvec& r) { coop_st_cvec(coop_C(scr), out, r); }
+};
+
+// One round for one lane: M tasks of type Task, all computed before any result is stored.  Idle slots (output
+// index < 0, operand indices 0) compute on valid but meaningless operands and store nothing.
+template <int M, class Task>
+MF_HD void coop_run_tasks(double* scr, const uint4* tab, const CoopRound& R, int lane, double mt) {
+  typename Task::Out res[M];
+  int out[M];
+#pragma unroll
+  for (int t = 0; t < M; ++t) {
+    const CoopFields<Task::NVEC> F = coop_load_fields<Task::NVEC>(tab, R, t, lane);
+    out[t] = coop_fld(F, 0);
+    res[t] = Task::calc(scr, F, mt);
+  }
+#pragma unroll
+  for (int t = 0; t < M; ++t)
+    if (out[t] >= 0) Task::store(scr, out[t], res[t]);
 }
 
-MF_HD void coop_task_bil(double* scr, const CoopFields& F) {
-  const double* S = coop_S(scr);
-  coop_st_cvec(coop_C(scr), coop_fld(F, 0), bilinear(coop_ld_spin(S, coop_fld(F, 1)), coop_ld_spin(S, coop_fld(F, 2))));
-}
-
-// One round for one lane.  Rounds are uniform per warp (same op and shape for all lanes); a lane whose output
-// index is negative idles.
-MF_HD void coop_exec_round(double* scr, const CoopRound& R, const CoopFields& F, double mt) {
-  if (coop_fld(F, 0) < 0) return;
-  switch (R.op * 16 + R.a * 4 + R.b) {
-    case 0 * 16 + 1 * 4 + 0: coop_task_J<1, 0>(scr, F); break;
-    case 0 * 16 + 2 * 4 + 1: coop_task_J<2, 1>(scr, F); break;
-    case 0 * 16 + 3 * 4 + 3: coop_task_J<3, 3>(scr, F); break;
-    case 1 * 16 + 1 * 4 + 1: coop_task_X<1>(scr, F, mt); break;
-    case 1 * 16 + 2 * 4 + 1: coop_task_X<2>(scr, F, mt); break;
-    case 2 * 16 + 1 * 4 + 1: coop_task_Y<1, true>(scr, F, mt); break;
-    case 2 * 16 + 2 * 4 + 0: coop_task_Y<2, false>(scr, F, mt); break;
-    case 3 * 16: coop_task_bil(scr, F); break;
+#define MF_COMMA ,
+MF_HD void coop_exec_round(double* scr, const uint4* tab, const CoopRound& R, int lane, double mt) {
+  switch (R.variant) {
+#define MF_COOP_CASE(ID, M, TASK) case ID: coop_run_tasks<M, TASK>(scr, tab, R, lane, mt); break;
+    MF_COOP_VARIANTS(MF_COOP_CASE)
+#undef MF_COOP_CASE
     default: break;
   }
 }
 
 // Host emulation helper (tests/host_shim): all rounds of `stage` for one (warp, lane).
-MF_HD void coop_run_stage(double* scr, int stage, int warp, int lane, double mt) {
+MF_HD void coop_run_stage(double* scr, const uint4* tab, int stage, int warp, int lane, double mt) {
   for (int r = 0; r < kCoopNumRounds[warp]; ++r) {
     const CoopRound R = kCoopRounds[warp][r];
-    if (R.stage != stage) continue;
-    coop_exec_round(scr, R, coop_load_fields(R, lane), mt);
+    if (R.stage == stage) coop_exec_round(scr, tab, R, lane, mt);
   }
 }
 
@@ -212,22 +237,11 @@ MF_HD double coop_s4_thread(double* scr, int tid) {
 
 #if defined(__CUDACC__)
 // ---- device-side driver ---------------------------------------------------------------------------------
-// The interpreter state a thread carries from event to event: the header and operand fields of the NEXT round
-// it will execute (already loaded).
-struct CoopCursor { CoopRound R; CoopFields F; };
-
-__device__ __forceinline__ CoopCursor coop_cursor_init(int tid) {
-  CoopCursor c;
-  c.R = kCoopRounds[tid >> 5][0];
-  c.F = coop_load_fields(c.R, tid & 31);
-  return c;
-}
-
 // Called by EVERY thread of the block (all teams run in lock-step so that the SM fetches one instruction stream:
 // the per-event program is larger than the instruction cache) after the owners have written the input areas
 // and the block has synchronised.  Teams with `active` false only keep the barriers.  Leaves
 // sum_{helicities} Ahat^dagger C Ahat * kCoopCden (no couplings, no averaging) in the team's reduction slots.
-__device__ __forceinline__ void coop_me2_lockstep(double* tm, int tid, bool active, double mt, CoopCursor& cur) {
+__device__ __forceinline__ void coop_me2_lockstep(double* tm, const uint4* tab, int tid, bool active, double mt) {
   double* scr = tm;
   const int warp = tid >> 5, lane = tid & 31;
   if (active) coop_s0(scr, tm + kCoopOffIn, tid, mt);
@@ -235,13 +249,9 @@ __device__ __forceinline__ void coop_me2_lockstep(double* tm, int tid, bool acti
   const int nr = kCoopNumRounds[warp];
 #pragma unroll 1
   for (int r = 0; r < nr; ++r) {
-    // fetch round r+1 (wrapping to round 0 of the next event) before executing round r
-    CoopCursor nxt;
-    nxt.R = kCoopRounds[warp][r + 1 < nr ? r + 1 : 0];
-    nxt.F = coop_load_fields(nxt.R, lane);
-    if (active) coop_exec_round(scr, cur.R, cur.F, mt);
-    if (cur.R.sync) __syncthreads();
-    cur = nxt;
+    const CoopRound R = kCoopRounds[warp][r];
+    if (active) coop_exec_round(scr, tab, R, lane, mt);
+    if (R.sync) __syncthreads();
   }
   if (active) {
     double acc = coop_s4_thread(scr, tid);

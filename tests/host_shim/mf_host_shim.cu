@@ -39,7 +39,7 @@ double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {
   for (int t = 0; t < kCoopTeam; ++t) coop_s0(tm.data(), in, t, m_top);
   for (int s = 0; s < kCoopStages; ++s)
     for (int w = 0; w < kCoopWarps; ++w)
-      for (int l = 0; l < 32; ++l) coop_run_stage(tm.data(), s, w, l, m_top);
+      for (int l = 0; l < 32; ++l) coop_run_stage(tm.data(), reinterpret_cast<const uint4*>(kCoopTable), s, w, l, m_top);
   double sum = 0.0;
   for (int t = 0; t < kCoopTeam; ++t) sum += coop_s4_thread(tm.data(), t);
   double gs2 = 4.0 * kPi * alpha_s;
