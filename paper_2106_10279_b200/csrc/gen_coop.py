@@ -1,31 +1,43 @@
 #!/usr/bin/env python3
 """Build-time generator of the COOPERATIVE matrix element of g g -> t tbar g g (64 threads per event).
 
-The straight-line code of gen_me.py keeps one event per thread; for 4 gluons its working set (30 gluon
-currents, 32 quark currents, 21 bilinears per polarisation combination) spills ~80 kB per thread.  This
-generator re-organises the same colour-ordered recursion (R10) as a STAGED program over a
-shared-memory scratch, executed by 64 threads per event:
+The straight-line code of gen_me.py keeps one event per thread; for 4 gluons its working set spills ~80 kB per
+thread.  This generator re-organises the same colour-ordered recursion (R10) as a STAGED program over a
+shared-memory scratch, executed by a team of 64 threads (2 warps) per event:
 
+  * spin-flip symmetry: with real gluon polarisation vectors the amplitudes of the quark spin assignment
+    (-s, -sbar) are, up to a common phase, the complex conjugates of those of (s, sbar) (B u* with
+    B = gamma^0 gamma^1 gamma^3 is the spin-flipped solution and B gamma^mu* B^-1 = gamma^mu), so
+    A^dagger C A is the same for both: only the top spin state 0 is evaluated and the sum is doubled;
   * helicity recycling: a current is computed once per polarisation assignment of the gluons IT contains
-    (J2: 4 variants, J3: 8, J4: 16; X(cd): 2 spins x 4; ...), not once per full helicity combination;
-  * stages S1..S3 are table driven: one task = one current; the tables (operand indices into the scratch)
-    are emitted here, so the kernel's interpreter has no index arithmetic;
-  * stage S4 is generated straight-line code: thread (pols, h, hb) forms its 24 colour-ordered amplitudes from
-    the staged currents and contracts them with the colour matrix.
+    (J2: 4 variants, J3: 8; X(cd): 2 spins x 4; ...), not once per full helicity combination;
+  * polarisation siblings: one lane computes M = 2 or 4 variants of a current that differ in the polarisation of
+    its first / last gluon, loading the shared operands (and forming the shared dot products) once: the program
+    is co-limited by shared-memory bandwidth, so operand reuse in registers matters as much as flops;
+  * S4 needs a four-gluon current only contracted with the fermion bilinear ubar gamma^mu v, and the bilinears
+    Y(a) gamma^mu X(d) only contracted with J(bc): the tasks store those complex SCALARS (z2, z5), not the vectors;
+  * stages S1, A, B are table driven: one lane-task = M sibling currents; the tables (operand indices into the
+    scratch) are emitted here, so the kernel's interpreter has no index arithmetic;
+  * stage S4 is generated straight-line code: thread (pols, hb, k) forms the real (k = 0) or imaginary (k = 1)
+    parts of its 24 colour-ordered amplitudes and contracts them with the colour matrix
+    (A^dagger C A = Re A^T C Re A + Im A^T C Im A for real symmetric C), so the two warps of a team share S4
+    without exchanging anything.
 
 Emits mf_me_ttgg_coop_generated.cuh.  Imports nothing from oracle/.
 """
 import itertools
 import os
 
-import numpy as np
-
 from gen_me import colour_matrix
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 N = 4           # gluons: 0, 1 beams; 2, 3 final
-P_CUT = N // 2  # the quark line is cut after P_CUT gluons
 LABELS = list(range(N))
+
+# ---- schedule knobs (tuned on B200; any setting gives the same result up to rounding) -------------------------
+# number of sibling groups computed by the wide lane-task of a family; the rest use the next narrower one
+WIDE_GROUPS = {"J3": 32, "X2": 32, "Yt": 24, "z5": 32, "J4": 32}
+ROUND_OVERHEAD = 60      # cost-model flops per round and lane (field fetch, dispatch)
 
 
 def mask_of(seq):
@@ -51,8 +63,8 @@ def polidx(gluons, pols):
     return v
 
 
-def pol_variants(gluons):
-    """all full 4-bit pol words restricted to `gluons` (other bits zero), in polidx order"""
+def pol_words(gluons):
+    """all full 4-bit pol words with zero bits outside `gluons`, in polidx order"""
     gl = sorted(gluons)
     out = []
     for v in range(1 << len(gl)):
@@ -64,10 +76,10 @@ def pol_variants(gluons):
 
 
 class Layout:
-    """component-major arrays: VEC[4][NV], SPIN[8][NS], CVEC[8][NC], SCAL[NSC]"""
+    """VEC items (real 4-vectors), SPIN items (Dirac spinors), X scalars; Z = two planes of complex scalars"""
 
     def __init__(self):
-        self.idx = {"V": {}, "S": {}, "C": {}, "X": {}}
+        self.idx = {"V": {}, "S": {}, "X": {}}
         self.bases = {}
 
     def add(self, arr, key):
@@ -83,82 +95,72 @@ class Layout:
         return len(self.idx[arr])
 
 
+ORDERED_PAIRS = list(itertools.permutations(LABELS, 2))
+PAIR_INDEX = {p: i for i, p in enumerate(ORDERED_PAIRS)}
+SEQS = {k: [s for s in itertools.permutations(LABELS, k) if canon(s)[0] == s] for k in range(2, N + 1)}
+SEQ_INDEX = {k: {s: i for i, s in enumerate(SEQS[k])} for k in SEQS}
+Z_PLANE = 2 * 12 * 2 * 16   # doubles per re / im plane: z2[12][2][16] then z5[12][2][16]
+Z5_OFF = 12 * 2 * 16
+
+
 def build_layout():
     L = Layout()
     for m in range(1, 1 << N):
         L.add("V", ("P", m))
     for m in range(1, 1 << N):
-        if bin(m).count("1") <= N - P_CUT:
+        if bin(m).count("1") <= 2:
             L.add("V", ("qX", m))
     for m in range(1, 1 << N):
-        if bin(m).count("1") <= P_CUT - 1:
+        if bin(m).count("1") == 1:
             L.add("V", ("qY", m))
     for g in LABELS:
         for p in range(2):
             L.add("V", ("eps", g, p))
-    # gluon currents, canonical sequences, family-contiguous so S4 can index them arithmetically
-    seqs = {k: [s for s in itertools.permutations(LABELS, k) if canon(s)[0] == s] for k in range(2, N + 1)}
-    for k in range(2, N + 1):
+    for k in (2, 3):   # gluon currents, canonical sequences, family-contiguous so S4 can index them arithmetically
         L.bases["J%d" % k] = L.n("V")
-        for s in seqs[k]:
-            for pv in pol_variants(s):
-                L.add("V", ("J", s, pv))
+        for s in SEQS[k]:
+            for pw in pol_words(s):
+                L.add("V", ("J", s, pw))
+    # fermion bilinears as pairs of real vectors (k = 0 real part, 1 imaginary part)
+    L.bases["c0"] = L.n("V")
+    for hb in range(2):
+        for k in range(2):
+            L.add("V", ("c0", hb, k))
+    for nm in ("cR", "cL"):
+        L.bases[nm] = L.n("V")
+        for g in LABELS:
+            for hb in range(2):
+                for p in range(2):
+                    for k in range(2):
+                        L.add("V", (nm, g, hb, p, k))
     for m in range(1, 1 << N):
         if bin(m).count("1") >= 2:
             L.add("X", ("iP2", m))
-        if bin(m).count("1") <= N - P_CUT:
+        if bin(m).count("1") <= 2:
             L.add("X", ("idX", m))
-        if bin(m).count("1") <= P_CUT - 1:
+        if bin(m).count("1") == 1:
             L.add("X", ("idY", m))
-    for h in range(2):
-        L.add("S", ("ub", h))
+    L.add("S", ("ub",))
     for hb in range(2):
         L.add("S", ("v", hb))
     L.bases["X1"] = L.n("S")
     for hb in range(2):
         for d in LABELS:
-            for pv in pol_variants((d,)):
-                L.add("S", ("X", (d,), hb, pv))
+            for p in range(2):
+                L.add("S", ("X1", d, hb, p))
     L.bases["Y1"] = L.n("S")
-    for h in range(2):
-        for a in LABELS:
-            for pv in pol_variants((a,)):
-                L.add("S", ("Y", (a,), h, pv))
-    ordered_pairs = list(itertools.permutations(LABELS, 2))
+    for a in LABELS:
+        for p in range(2):
+            L.add("S", ("Y1", a, p))
     L.bases["X2"] = L.n("S")
     for hb in range(2):
-        for cd in ordered_pairs:
-            for pv in pol_variants(cd):
-                L.add("S", ("X", cd, hb, pv))
+        for cd in ORDERED_PAIRS:
+            for pw in pol_words(cd):
+                L.add("S", ("X2", cd, hb, pw))
     L.bases["Yt"] = L.n("S")
-    for h in range(2):
-        for ab in ordered_pairs:
-            for pv in pol_variants(ab):
-                L.add("S", ("Yt", ab, h, pv))
-    L.bases["c0"] = L.n("C")
-    for h in range(2):
-        for hb in range(2):
-            L.add("C", ("c", (), (), h, hb, 0))
-    L.bases["cR"] = L.n("C")
-    for h in range(2):
-        for hb in range(2):
-            for d in LABELS:
-                for pv in pol_variants((d,)):
-                    L.add("C", ("c", (), (d,), h, hb, pv))
-    L.bases["cL"] = L.n("C")
-    for h in range(2):
-        for hb in range(2):
-            for a in LABELS:
-                for pv in pol_variants((a,)):
-                    L.add("C", ("c", (a,), (), h, hb, pv))
-    L.bases["cLR"] = L.n("C")
-    for h in range(2):
-        for hb in range(2):
-            for ad in ordered_pairs:
-                for pv in pol_variants(ad):
-                    L.add("C", ("c", (ad[0],), (ad[1],), h, hb, pv))
-    L.seqs = seqs
-    L.ordered_pairs = ordered_pairs
+    for ab in ORDERED_PAIRS:
+        for pw in pol_words(ab):
+            L.add("S", ("Yt", ab, pw))
     return L
 
 
@@ -169,171 +171,220 @@ def J_ref(L, seq, pols):
     if len(seq) == 1:
         return L.get("V", ("eps", seq[0], (pols >> seq[0]) & 1)), 1
     c, s = canon(seq)
-    pv = pols & mask_of(seq)
-    return L.get("V", ("J", c, pv)), s
+    return L.get("V", ("J", c, pols & mask_of(seq))), s
 
 
 def P_ref(L, seq):
     return L.get("V", ("P", mask_of(seq)))
 
 
-# ---- tasks ---------------------------------------------------------------------------------------------------
-# op codes of the interpreter (mf_me_coop.cuh)
-OP_J, OP_XCOL, OP_YROW, OP_BIL = 0, 1, 2, 3
+def z2_index(seq, pols):
+    return (SEQ_INDEX[4][seq] * 2) * 16 + pols          # hb = 0, k = 0; hb stride 16, k stride Z_PLANE
 
 
-def task_J(L, seq, pols):
-    k = len(seq)
-    v3, v4 = [], []
-    for j in range(1, k):
-        a, sa = J_ref(L, seq[:j], pols)
-        b, sb = J_ref(L, seq[j:], pols)
-        v3.append((a, P_ref(L, seq[:j]), b, P_ref(L, seq[j:]), -sa * sb))
-    for j in range(1, k):
-        for l in range(j + 1, k):
-            a, sa = J_ref(L, seq[:j], pols)
-            b, sb = J_ref(L, seq[j:l], pols)
-            c, sc = J_ref(L, seq[l:], pols)
-            v4.append((a, b, c, sa * sb * sc))
-    out = L.get("V", ("J", tuple(seq), pols & mask_of(seq)))
-    fields = [out, L.get("X", ("iP2", mask_of(seq)))]
-    signs = 0
-    for i, t in enumerate(v3):
-        fields += list(t[:4])
-        signs |= (1 if t[4] < 0 else 0) << i
-    for i, t in enumerate(v4):
-        fields += list(t[:3])
-        signs |= (1 if t[3] < 0 else 0) << (len(v3) + i)
-    fields.append(signs)
-    flops = 53 * len(v3) + 49 * len(v4) + 4
-    return dict(op=OP_J, a=len(v3), b=len(v4), fields=fields, flops=flops)
+def z5_index(pair, hb, pols):
+    return Z5_OFF + (PAIR_INDEX[pair] * 2 + hb) * 16 + pols
 
 
-def task_X(L, seq, hb, pols):
-    """Xhat(seq) = -(qslash+m)/(q^2-m^2) sum_j Jslash(seq[:j]) Xhat(seq[j:]),  Xhat() = v"""
-    k = len(seq)
-    terms = []
-    for j in range(1, k + 1):
-        jv, js = J_ref(L, seq[:j], pols)
-        rest = tuple(seq[j:])
-        sp = L.get("S", ("v", hb)) if not rest else L.get("S", ("X", rest, hb, pols & mask_of(rest)))
-        terms.append((jv, sp, js))
-    m = mask_of(seq)
-    fields = [L.get("S", ("X", tuple(seq), hb, pols & m)), L.get("V", ("qX", m)), L.get("X", ("idX", m))]
-    signs = 0
-    for i, t in enumerate(terms):
-        fields += [t[0], t[1]]
-        signs |= (1 if t[2] < 0 else 0) << i
-    fields.append(signs)
-    return dict(op=OP_XCOL, a=len(terms), b=1, fields=fields, flops=42 * len(terms) + 8 * (len(terms) - 1) + 66)
+# ---- flop model of the task templates of mf_me_coop.cuh (adds + multiplies, FMA = 2; shared dot products of
+# sibling currents counted once, as the templates compute them once) ------------------------------------------
+def flops_v3(ma, md):
+    mm = ma * md
+    return 7 * (mm + ma + md) + (ma + md) + 4 + 24 * mm
 
 
-def task_Y(L, seq, h, pols, propagate):
-    """Ytilde(seq) = sum_j Yhat(seq[:j]) Jslash(seq[j:]);  Yhat = Ytilde (-(qslash+m)/(q^2-m^2)),  Yhat() = ubar"""
-    k = len(seq)
-    terms = []
-    for j in range(0, k):
-        left = tuple(seq[:j])
-        sp = L.get("S", ("ub", h)) if not left else L.get("S", ("Y", left, h, pols & mask_of(left)))
-        jv, js = J_ref(L, seq[j:], pols)
-        terms.append((sp, jv, js))
-    m = mask_of(seq)
-    if propagate:
-        fields = [L.get("S", ("Y", tuple(seq), h, pols & m)), L.get("V", ("qY", m)), L.get("X", ("idY", m))]
-    else:
-        fields = [L.get("S", ("Yt", tuple(seq), h, pols & m)), 0, 0]
-    signs = 0
-    for i, t in enumerate(terms):
-        fields += [t[0], t[1]]
-        signs |= (1 if t[2] < 0 else 0) << i
-    fields.append(signs)
-    return dict(op=OP_YROW, a=len(terms), b=1 if propagate else 0, fields=fields,
-                flops=42 * len(terms) + 8 * (len(terms) - 1) + (66 if propagate else 0))
+def flops_v4(ma, md):
+    mm = ma * md
+    return 7 * (mm + ma + md) + mm + 24 * mm
 
 
-def task_bil(L, left, right, h, hb, pols):
-    row = L.get("S", ("ub", h)) if not left else L.get("S", ("Y", tuple(left), h, pols & mask_of(left)))
-    col = L.get("S", ("v", hb)) if not right else L.get("S", ("X", tuple(right), hb, pols & mask_of(right)))
-    out = L.get("C", ("c", tuple(left), tuple(right), h, hb, pols & (mask_of(left) | mask_of(right))))
-    return dict(op=OP_BIL, a=0, b=0, fields=[out, row, col], flops=72)
+F_SLASH, F_SLASH_ACC, F_PROP, F_BIL, F_CDOT = 42, 50, 66, 72, 14
 
 
-def build_stages(L):
-    s1, s2, s3 = [], [], []
-    for s in L.seqs[2]:
-        for pv in pol_variants(s):
-            s1.append(task_J(L, s, pv))
-    for hb in range(2):
-        for d in LABELS:
-            for pv in pol_variants((d,)):
-                s1.append(task_X(L, (d,), hb, pv))
-    for h in range(2):
-        for a in LABELS:
-            for pv in pol_variants((a,)):
-                s1.append(task_Y(L, (a,), h, pv, True))
-    for h in range(2):
-        for hb in range(2):
-            s1.append(task_bil(L, (), (), h, hb, 0))
-    for s in L.seqs[3]:
-        for pv in pol_variants(s):
-            s2.append(task_J(L, s, pv))
-    for hb in range(2):
-        for cd in L.ordered_pairs:
-            for pv in pol_variants(cd):
-                s2.append(task_X(L, cd, hb, pv))
-    for h in range(2):
-        for ab in L.ordered_pairs:
-            for pv in pol_variants(ab):
-                s2.append(task_Y(L, ab, h, pv, False))
-    for h in range(2):
-        for hb in range(2):
-            for d in LABELS:
-                for pv in pol_variants((d,)):
-                    s2.append(task_bil(L, (), (d,), h, hb, pv))
-                    s2.append(task_bil(L, (d,), (), h, hb, pv))
-            for ad in L.ordered_pairs:
-                for pv in pol_variants(ad):
-                    s2.append(task_bil(L, (ad[0],), (ad[1],), h, hb, pv))
-    for s in L.seqs[4]:
-        for pv in pol_variants(s):
-            s3.append(task_J(L, s, pv))
-    return [s1, s2, s3]
+# ---- lane-tasks ---------------------------------------------------------------------------------------------
+def task_J2(L, s, pw):
+    a, b = s
+    return dict(fam="J2", M=1, flops=flops_v3(1, 1) + 4,
+                fields=[L.get("V", ("J", s, pw)), L.get("X", ("iP2", mask_of(s))), J_ref(L, (a,), pw)[0], P_ref(L, (a,)),
+                        J_ref(L, (b,), pw)[0], P_ref(L, (b,))])
 
 
-# tasks a lane may interleave in one round, by task shape (op, a, b): independent instruction streams hide the
-# FP64 and shared-memory latencies that two warps per scheduler cannot
-MAX_MULT = {(OP_J, 1, 0): 1, (OP_J, 2, 1): 2, (OP_J, 3, 3): 2, (OP_XCOL, 1, 1): 1, (OP_XCOL, 2, 1): 2,
-            (OP_YROW, 1, 1): 1, (OP_YROW, 2, 0): 2, (OP_BIL, 0, 0): 4}
+def task_X1c(L, d, hb, p):
+    pw = p << d
+    return dict(fam="X1c", M=1, flops=F_SLASH + F_PROP + F_BIL,
+                fields=[L.get("S", ("X1", d, hb, p)), L.get("V", ("qX", 1 << d)), L.get("X", ("idX", 1 << d)),
+                        J_ref(L, (d,), pw)[0], L.get("S", ("v", hb)), L.get("S", ("ub",)),
+                        L.get("V", ("cR", d, hb, p, 0)), L.get("V", ("cR", d, hb, p, 1))])
 
 
-def schedule(stage_tasks, n_warps=2):
-    """Splits the tasks of a stage into warp rounds.  A round = up to 32 * m tasks of equal shape; lane l runs tasks
-    l, 32 + l, ... of the round interleaved (m <= MAX_MULT).  Large groups are halved between the two warps, small
-    ones go whole to the less loaded warp."""
-    groups = {}
-    for t in stage_tasks:
-        groups.setdefault((t["op"], t["a"], t["b"]), []).append(t)
-    warps = [[] for _ in range(n_warps)]
-    load = [0] * n_warps
+def task_Y1c(L, a, p):
+    pw = p << a
+    return dict(fam="Y1c", M=1, flops=F_SLASH + F_PROP + 2 * F_BIL,
+                fields=[L.get("S", ("Y1", a, p)), L.get("V", ("qY", 1 << a)), L.get("X", ("idY", 1 << a)),
+                        L.get("S", ("ub",)), J_ref(L, (a,), pw)[0], L.get("S", ("v", 0)), L.get("S", ("v", 1)),
+                        L.get("V", ("cL", a, 0, p, 0)), L.get("V", ("cL", a, 0, p, 1)),
+                        L.get("V", ("cL", a, 1, p, 0)), L.get("V", ("cL", a, 1, p, 1))])
 
-    def add_rounds(w, key, ts):
-        cap = 32 * MAX_MULT[key]
-        for i in range(0, len(ts), cap):
-            chunk = ts[i:i + cap]
-            m = (len(chunk) + 31) // 32
-            warps[w].append((key, m, chunk))
-            load[w] += chunk[0]["flops"] * m
 
-    for key in sorted(groups, key=lambda k: -groups[k][0]["flops"] * len(groups[k])):
-        ts = groups[key]
-        if len(ts) >= 64:
-            half = (len(ts) // 2 + 31) // 32 * 32 if len(ts) % 64 else len(ts) // 2
-            lo = load.index(min(load))          # the less loaded warp takes the larger part
-            add_rounds(lo, key, ts[:half])
-            add_rounds(1 - lo, key, ts[half:])
-        else:
-            add_rounds(load.index(min(load)), key, ts)
-    return warps, load
+def task_J3(L, s, pw_ab, m):
+    """J3(abc) for the polarisations pw_ab of (a, b) and pc = 0..m-1 (m = 2) or pc given in pw_ab (m = 1)"""
+    a, b, c = s
+    pcs = [0, 1] if m == 2 else [(pw_ab >> c) & 1]
+    base = pw_ab & ~(1 << c)
+    pws = [base | (pc << c) for pc in pcs]
+    j2bc = [J_ref(L, (b, c), pw) for pw in pws]
+    j2ab = J_ref(L, (a, b), base)
+    signs = (1 if j2bc[0][1] < 0 else 0) | (2 if j2ab[1] < 0 else 0)
+    f = [L.get("V", ("J", s, pw)) for pw in pws]
+    f += [L.get("X", ("iP2", mask_of(s))), J_ref(L, (a,), base)[0], P_ref(L, (a,))]
+    f += [x[0] for x in j2bc] + [P_ref(L, (b, c)), j2ab[0], P_ref(L, (a, b))]
+    f += [J_ref(L, (c,), pw)[0] for pw in pws] + [P_ref(L, (c,)), J_ref(L, (b,), base)[0], signs]
+    fl = 2 * (7 * (2 * m + 1) + (1 + m) + 4 + 24 * m) + 7 * (2 * m + 1) + 25 * m + 4 * m
+    return dict(fam="J3", M=m, fields=f, flops=fl)
+
+
+def task_J4(L, s, pw_bc, ma, md, pa=0, pd=0):
+    """z2 = c0 . J4(abcd) for the polarisations pw_bc of (b, c) and (pa, pd) in ma x md variants"""
+    a, b, c, d = s
+    base = pw_bc & ((1 << b) | (1 << c))
+    pas = [0, 1] if ma == 2 else [pa]
+    pds = [0, 1] if md == 2 else [pd]
+    wa = [base | (x << a) for x in pas]        # words seen by operands containing a (not d)
+    wd = [base | (x << d) for x in pds]
+    j2ab = [J_ref(L, (a, b), w) for w in wa]
+    j2cd = [J_ref(L, (c, d), w) for w in wd]
+    j2bc = J_ref(L, (b, c), base)
+    signs = (1 if j2ab[0][1] < 0 else 0) | (2 if j2cd[0][1] < 0 else 0) | (4 if j2bc[1] < 0 else 0)
+    f = [z2_index(s, base | (x << a) | (y << d)) for y in pds for x in pas]      # out[ia + ma * id]
+    f += [L.get("X", ("iP2", mask_of(s)))]
+    f += [J_ref(L, (a,), w)[0] for w in wa] + [x[0] for x in j2ab] + [J_ref(L, (a, b, c), w)[0] for w in wa]
+    f += [J_ref(L, (d,), w)[0] for w in wd] + [x[0] for x in j2cd] + [J_ref(L, (b, c, d), w)[0] for w in wd]
+    f += [J_ref(L, (b,), base)[0], J_ref(L, (c,), base)[0], j2bc[0]]
+    f += [P_ref(L, (a,)), P_ref(L, (b, c, d)), P_ref(L, (a, b)), P_ref(L, (c, d)), P_ref(L, (a, b, c)), P_ref(L, (d,))]
+    f += [L.get("V", ("c0", 0, 0)), signs]
+    mm = ma * md
+    fl = 3 * flops_v3(ma, md) + 3 * flops_v4(ma, md) + 16 + 4 * 7 * mm
+    return dict(fam="J4", M=mm, MA=ma, MD=md, fields=f, flops=fl)
+
+
+def task_X2(L, cd, hb, pd, m, pc=0):
+    """X2(cd) = prop [eps_c-slash X1(d) + J2(cd)-slash v] for pc = 0..m-1"""
+    c, d = cd
+    pcs = [0, 1] if m == 2 else [pc]
+    pws = [(x << c) | (pd << d) for x in pcs]
+    j2 = [J_ref(L, cd, w) for w in pws]
+    f = [L.get("S", ("X2", cd, hb, w)) for w in pws]
+    f += [L.get("V", ("qX", mask_of(cd))), L.get("X", ("idX", mask_of(cd))), L.get("S", ("X1", d, hb, pd)),
+          L.get("S", ("v", hb))]
+    f += [J_ref(L, (c,), w)[0] for w in pws] + [x[0] for x in j2] + [1 if j2[0][1] < 0 else 0]
+    return dict(fam="X2", M=m, fields=f, flops=m * (F_SLASH + F_SLASH_ACC + F_PROP))
+
+
+def task_Yt(L, ab, pa, m, pb=0):
+    """Ytilde(ab) = ubar J2(ab)-slash + Y1(a) eps_b-slash for pb = 0..m-1"""
+    a, b = ab
+    pbs = [0, 1] if m == 2 else [pb]
+    pws = [(pa << a) | (x << b) for x in pbs]
+    j2 = [J_ref(L, ab, w) for w in pws]
+    f = [L.get("S", ("Yt", ab, w)) for w in pws]
+    f += [L.get("S", ("ub",)), L.get("S", ("Y1", a, pa))]
+    f += [x[0] for x in j2] + [J_ref(L, (b,), w)[0] for w in pws] + [1 if j2[0][1] < 0 else 0]
+    return dict(fam="Yt", M=m, fields=f, flops=m * (F_SLASH + F_SLASH_ACC))
+
+
+def task_z5(L, ad, hb, pa, m, pd=0):
+    """z5 = [Y1(a) gamma X1(d)] . J2(bc) for the 4 polarisations of (b, c), b < c, and pd = 0..m-1"""
+    a, d = ad
+    b, c = [g for g in LABELS if g not in ad]
+    pds = [0, 1] if m == 2 else [pd]
+    f = [z5_index(ad, hb, (pa << a) | (x << d)) for x in pds]
+    f += [1 << b, 1 << c, L.get("S", ("Y1", a, pa))]
+    f += [L.get("S", ("X1", d, hb, x)) for x in pds]
+    f += [L.get("V", ("J", (b, c), 0))]
+    return dict(fam="z5", M=m, fields=f, flops=m * (F_BIL + 4 * F_CDOT))
+
+
+def build_rounds(L):
+    """lane-tasks grouped into rounds of <= 32 equal-shaped lane-tasks; each round knows the phases it may run in"""
+    rounds = []
+
+    def add(phases, tasks):
+        for i in range(0, len(tasks), 32):
+            chunk = tasks[i:i + 32]
+            t0 = chunk[0]
+            key = (t0["fam"], t0.get("MA", 0), t0.get("MD", 0), t0["M"])
+            rounds.append(dict(key=key, tasks=chunk, phases=phases, cost=t0["flops"] + ROUND_OVERHEAD))
+
+    # S1
+    add(["S1"], [task_J2(L, s, pw) for s in SEQS[2] for pw in pol_words(s)])
+    add(["S1"], [task_X1c(L, d, hb, p) for hb in range(2) for d in LABELS for p in range(2)])
+    add(["S1"], [task_Y1c(L, a, p) for a in LABELS for p in range(2)])
+    # J3: sibling groups (seq, pa, pb)
+    groups = [(s, pw) for s in SEQS[3] for pw in pol_words(s[:2])]
+    w = WIDE_GROUPS["J3"]
+    add(["A"], [task_J3(L, s, pw, 2) for s, pw in groups[:w]])
+    add(["A"], [task_J3(L, s, pw | (pc << s[2]), 1) for s, pw in groups[w:] for pc in range(2)])
+    # J4: sibling groups (seq, pb, pc) of 4 (pa, pd)
+    groups = [(s, pw) for s in SEQS[4] for pw in pol_words(s[1:3])]
+    w = WIDE_GROUPS["J4"]
+    add(["B"], [task_J4(L, s, pw, 2, 2) for s, pw in groups[:w]])
+    add(["B"], [task_J4(L, s, pw, 1, 2, pa=pa) for s, pw in groups[w:] for pa in range(2)])
+    # X2: sibling groups (pair, hb, pd)
+    groups = [(cd, hb, pd) for hb in range(2) for cd in ORDERED_PAIRS for pd in range(2)]
+    w = WIDE_GROUPS["X2"]
+    add(["A", "B"], [task_X2(L, cd, hb, pd, 2) for cd, hb, pd in groups[:w]])
+    add(["A", "B"], [task_X2(L, cd, hb, pd, 1, pc) for cd, hb, pd in groups[w:] for pc in range(2)])
+    # Yt: sibling groups (pair, pa)
+    groups = [(ab, pa) for ab in ORDERED_PAIRS for pa in range(2)]
+    w = WIDE_GROUPS["Yt"]
+    add(["A", "B"], [task_Yt(L, ab, pa, 2) for ab, pa in groups[:w]])
+    add(["A", "B"], [task_Yt(L, ab, pa, 1, pb) for ab, pa in groups[w:] for pb in range(2)])
+    # z5: sibling groups (pair, hb, pa)
+    groups = [(ad, hb, pa) for hb in range(2) for ad in ORDERED_PAIRS for pa in range(2)]
+    w = WIDE_GROUPS["z5"]
+    add(["A", "B"], [task_z5(L, ad, hb, pa, 2) for ad, hb, pa in groups[:w]])
+    add(["A", "B"], [task_z5(L, ad, hb, pa, 1, pd) for ad, hb, pa in groups[w:] for pd in range(2)])
+    return [r for r in rounds if r["tasks"]]
+
+
+PHASES = ["S1", "A", "B"]
+
+
+def schedule(rounds, n_warps=2):
+    """assigns every round to (phase, warp) minimising sum over phases of the slower warp (exhaustive over the
+    rounds that may move, greedy for the rest)"""
+    fixed = [r for r in rounds if len(r["phases"]) == 1]
+    flex = [r for r in rounds if len(r["phases"]) > 1]
+    slots = [(p, w) for p in PHASES for w in range(n_warps)]
+
+    def total(load):
+        return sum(max(load[(p, w)] for w in range(n_warps)) for p in PHASES)
+
+    best = None
+    fixed_sorted = sorted(fixed, key=lambda r: -r["cost"])
+    for combo in itertools.product(*[[(p, w) for p in r["phases"] for w in range(n_warps)] for r in flex]):
+        load = {s: 0 for s in slots}
+        for r, s in zip(flex, combo):
+            load[s] += r["cost"]
+        assign = list(combo)
+        fa = []
+        for r in fixed_sorted:
+            p = r["phases"][0]
+            w = min(range(n_warps), key=lambda x: load[(p, x)])
+            load[(p, w)] += r["cost"]
+            fa.append((p, w))
+        t = total(load)
+        if best is None or t < best[0]:
+            best = (t, assign, fa, dict(load))
+    _, assign, fa, load = best
+    plan = {s: [] for s in slots}
+    for r, s in zip(fixed_sorted, fa):
+        plan[s].append(r)
+    for r, s in zip(flex, assign):
+        plan[s].append(r)
+    for s in slots:   # producers of a phase first is irrelevant inside a phase; keep heavy rounds first
+        plan[s].sort(key=lambda r: -r["cost"])
+    return plan, load
 
 
 # ---- stage S4: generated straight-line code --------------------------------------------------------------------
@@ -347,10 +398,10 @@ def emit_s4(L):
     assert perms_c == perms
     o = []
     w = o.append
-    w("// S4: thread (pols, h, hb) forms its %d colour-ordered amplitudes and contracts them with the colour matrix." % len(perms))
-    w("// Returns sum_{s,s'} conj(Ahat_s) Cnum_{ss'} Ahat_s'  (colour matrix numerators; the caller divides by kCoopCden).")
-    w("MF_HD double coop_s4(const double* V, const double* S, const double* C, int pols, int h, int hb) {")
-    w("  const int hs = h * 2 + hb;")
+    flops = 0
+    w("// S4: thread (pols, hb, k) forms the real (k = 0) or imaginary (k = 1) parts of its %d colour-ordered amplitudes" % len(perms))
+    w("// and contracts them with the colour matrix: returns sum_{s,s'} x_s Cnum_{ss'} x_s' (the caller divides by kCoopCden).")
+    w("MF_HD double coop_s4(const double* V, const double* S, const double* Z, int pols, int hb, int k) {")
     for g in LABELS:
         w("  const int ps%d = (pols >> %d) & 1;" % (g, g))
     for a, b in itertools.combinations(LABELS, 2):
@@ -358,64 +409,56 @@ def emit_s4(L):
     for m in LABELS:
         rest = [g for g in LABELS if g != m]
         w("  const int pt%d = ps%d | (ps%d << 1) | (ps%d << 2);" % (m, rest[0], rest[1], rest[2]))
-    opi = {p: i for i, p in enumerate(L.ordered_pairs)}
-    amp = {}
-    # term 1: Ytilde(ab) . Xhat(cd)
+    w("  const double* Zk = Z + k * %d + hb * 16 + pols;" % Z_PLANE)
+    w("  double " + ", ".join("A%d%d%d%d" % p for p in perms) + ";")
+    # term 1: Ytilde(ab) . Xhat(cd); k selects the real or the imaginary part of the product
     for a, b in itertools.combinations(LABELS, 2):
         c, d = [g for g in LABELS if g not in (a, b)]
         w("  {")
         for (x, y) in ((a, b), (b, a)):
-            w("    const spin yt%d%d = coop_ld_spin(S, %d + (h * 12 + %d) * 4 + %s);" % (x, y, L.bases["Yt"], opi[(x, y)], pair_name(x, y)))
+            w("    const spin yt%d%d = coop_row_part(coop_ld_spin(S, %d + %d * 4 + %s), k);" % (x, y, L.bases["Yt"], PAIR_INDEX[(x, y)], pair_name(x, y)))
         for (x, y) in ((c, d), (d, c)):
-            w("    const spin x%d%d = coop_ld_spin(S, %d + (hb * 12 + %d) * 4 + %s);" % (x, y, L.bases["X2"], opi[(x, y)], pair_name(x, y)))
+            w("    const spin x%d%d = coop_col_part(coop_ld_spin(S, %d + (hb * 12 + %d) * 4 + %s), k);" % (x, y, L.bases["X2"], PAIR_INDEX[(x, y)], pair_name(x, y)))
         for (x, y) in ((a, b), (b, a)):
             for (u, v) in ((c, d), (d, c)):
-                nm = "%d%d%d%d" % (x, y, u, v)
-                w("    const cplx t%s = sdot(yt%d%d, x%d%d);" % (nm, x, y, u, v))
-                w("    A%sr = t%s.re; A%si = t%s.im;" % (nm, nm, nm, nm))
-                amp[(x, y, u, v)] = True
+                w("    A%d%d%d%d = sdot_part(yt%d%d, x%d%d);" % (x, y, u, v, x, y, u, v))
+                flops += 15
         w("  }")
-    decl = "  double " + ", ".join("A%d%d%d%dr, A%d%d%d%di" % (p + p) for p in perms) + ";"
-    # the declarations must precede the blocks: insert after the index preamble
-    first_block = next(i for i, l in enumerate(o) if l == "  {")
-    o.insert(first_block, decl)
 
     def add(perm, z, sign):
-        nm = "%d%d%d%d" % perm
-        w("    A%sr %s= %s.re; A%si %s= %s.im;" % (nm, "+" if sign > 0 else "-", z, nm, "+" if sign > 0 else "-", z))
+        nonlocal flops
+        w("    A%d%d%d%d %s= %s;" % (perm + ("+" if sign > 0 else "-", z)))
+        flops += 1
 
-    # term 2: c0 . J4(sigma)
+    # term 2: z2 = c0 . J4(sigma), stored by the J4 tasks
     w("  {")
-    w("    const cvec c0 = coop_ld_cvec(C, %d + hs);" % L.bases["c0"])
-    for i, s in enumerate(L.seqs[4]):
-        w("    { const cplx z = cdot_r(c0, coop_ld_vec(V, %d + %d * 16 + pols));" % (L.bases["J4"], i))
+    for i, s in enumerate(SEQS[4]):
+        w("    { const double z = Zk[%d];" % (i * 32))
         add(s, "z", 1)
         add(s[::-1], "z", (-1) ** (4 + 1))
         w("    }")
     w("  }")
-    # terms 3 and 4: c(., d) . J3(abc)  and  c(a, .) . J3(bcd)
-    seq3_index = {s: i for i, s in enumerate(L.seqs[3])}
+    # terms 3 and 4: c(., g) . J3(abc)  and  c(g, .) . J3(bcd)
     for g in LABELS:
         w("  {")
-        w("    const cvec cr = coop_ld_cvec(C, %d + (hs * 4 + %d) * 2 + ps%d);" % (L.bases["cR"], g, g))
-        w("    const cvec cl = coop_ld_cvec(C, %d + (hs * 4 + %d) * 2 + ps%d);" % (L.bases["cL"], g, g))
-        for s in L.seqs[3]:
+        w("    const rvec cr = coop_ld_vec(V, %d + ((%d * 2 + hb) * 2 + ps%d) * 2 + k);" % (L.bases["cR"], g, g))
+        w("    const rvec cl = coop_ld_vec(V, %d + ((%d * 2 + hb) * 2 + ps%d) * 2 + k);" % (L.bases["cL"], g, g))
+        for s in SEQS[3]:
             if g in s:
                 continue
-            w("    { const rvec j = coop_ld_vec(V, %d + %d * 8 + pt%d);" % (L.bases["J3"], seq3_index[s], g))
-            w("      const cplx zr = cdot_r(cr, j), zl = cdot_r(cl, j);")
+            w("    { const rvec j = coop_ld_vec(V, %d + %d * 8 + pt%d);" % (L.bases["J3"], SEQ_INDEX[3][s], g))
+            w("      const double zr = rdot(cr, j), zl = rdot(cl, j);")
+            flops += 14
             add(s + (g,), "zr", 1)
             add(s[::-1] + (g,), "zr", 1)
             add((g,) + s, "zl", 1)
             add((g,) + s[::-1], "zl", 1)
             w("    }")
         w("  }")
-    # term 5: c(a, d) . J2(bc)
-    seq2_index = {s: i for i, s in enumerate(L.seqs[2])}
-    for (a, d) in L.ordered_pairs:
+    # term 5: z5 = c(a, d) . J2(bc), stored by the z5 tasks
+    for (a, d) in ORDERED_PAIRS:
         b, c = [g for g in LABELS if g not in (a, d)]
-        w("  { const cvec clr = coop_ld_cvec(C, %d + (hs * 12 + %d) * 4 + %s);" % (L.bases["cLR"], opi[(a, d)], pair_name(a, d)))
-        w("    const cplx z = cdot_r(clr, coop_ld_vec(V, %d + %d * 4 + %s));" % (L.bases["J2"], seq2_index[(b, c)], pair_name(b, c)))
+        w("  { const double z = Zk[%d];" % (Z5_OFF + PAIR_INDEX[(a, d)] * 32))
         add((a, b, c, d), "z", 1)
         add((a, c, b, d), "z", -1)
         w("  }")
@@ -432,118 +475,109 @@ def emit_s4(L):
         for (i, j) in groups[v]:
             a, b = "A%d%d%d%d" % perms[i], "A%d%d%d%d" % perms[j]
             if first:
-                w("  g = fma(%si, %si, %sr * %sr);" % (a, b, a, b))
+                w("  g = %s * %s;" % (a, b))
+                flops += 1
             else:
-                w("  g = fma(%si, %si, fma(%sr, %sr, g));" % (a, b, a, b))
+                w("  g = fma(%s, %s, g);" % (a, b))
+                flops += 2
             first = False
         w("  acc = fma(%.1f, g, acc);" % v)
+        flops += 2
     w("  return acc;")
     w("}")
-    npairs = sum(len(v) for v in groups.values())
-    flops = 24 * 30 + 48 * 14 + 4 * 2 * 24 + 4 * npairs + len(groups)
     return "\n".join(o), Cden, flops
 
 
-def emit_tables(L, stages):
-    """Per warp ONE flat list of rounds over all stages (the last round of a stage carries the barrier flag).  The
-    operand indices of a round are stored as 16-byte vectors of 8 shorts, vector (t, v) of all 32 lanes contiguous
-    (t = task slot of the lane, v = vector of the task), so a warp fetches them with conflict-free 128-bit loads."""
+VARIANT_NAMES = {"J2": "CoopTaskJ2", "X1c": "CoopTaskX1c", "Y1c": "CoopTaskY1c", "J3": "CoopTaskJ3<%(M)d>",
+                 "J4": "CoopTaskJ4<%(MA)d MF_COMMA %(MD)d>", "X2": "CoopTaskX2<%(M)d>", "Yt": "CoopTaskYt<%(M)d>",
+                 "z5": "CoopTaskZ5<%(M)d>"}
+
+
+def emit_tables(L, rounds):
+    """Per warp ONE flat list of rounds over all phases (the last round of a phase carries the barrier flag).  The
+    operand indices of a round are stored as 16-byte vectors of 8 shorts, vector v of all 32 lanes contiguous, so a
+    warp fetches them with conflict-free 128-bit loads."""
     o = []
     w = o.append
-    words = []          # the table as shorts, later grouped into uint4 (8 shorts)
-    w("struct CoopRound { short variant, m, nvec, stage, sync, pad; int offset; };  // offset in 16-byte vectors")
-    sched = [schedule(st) for st in stages]
+    words = []
     n_warps = 2
-    variants = []       # (op, a, b, m) in order of first use
-    rows, counts = [], []
+    plan, load = schedule(rounds, n_warps)
+    variants = []
+    rows = []
     for wi in range(n_warps):
         row = []
-        for si, (warps, load) in enumerate(sched):
-            rounds = warps[wi]
-            assert rounds, "every warp needs a round in every stage (it carries the barrier)"
-            for ri, (key, m, tasks) in enumerate(rounds):
-                nf = len(tasks[0]["fields"])
-                nvec = 1
-                while nvec * 8 < nf:
-                    nvec *= 2
-                assert nvec <= 4
-                var = key + (m,)
-                if var not in variants:
-                    variants.append(var)
+        for pi, ph in enumerate(PHASES):
+            rs = plan[(ph, wi)]
+            if not rs:   # the barrier still needs a carrier: an empty round
+                row.append("{-1, 0, %d, 1, 0}" % pi)
+                continue
+            for ri, r in enumerate(rs):
+                nf = max(len(t["fields"]) for t in r["tasks"])
+                nvec = (nf + 7) // 8
+                if r["key"] not in variants:
+                    variants.append(r["key"])
                 off = len(words) // 8
-                for t in range(m):
-                    for v in range(nvec):
-                        for lane in range(32):
-                            i = t * 32 + lane
-                            f = list(tasks[i]["fields"]) if i < len(tasks) else [-1]
-                            f += [0] * (nvec * 8 - len(f))
-                            words.extend(f[8 * v:8 * v + 8])
-                row.append("{%d, %d, %d, %d, %d, 0, %d}" % (variants.index(var), m, nvec, si, 1 if ri == len(rounds) - 1 else 0, off))
-        counts.append(len(row))
+                for v in range(nvec):
+                    for lane in range(32):
+                        f = list(r["tasks"][lane]["fields"]) if lane < len(r["tasks"]) else [-1]
+                        f += [0] * (nvec * 8 - len(f))
+                        words.extend(f[8 * v:8 * v + 8])
+                row.append("{%d, %d, %d, %d, %d}" % (variants.index(r["key"]), nvec, pi, 1 if ri == len(rs) - 1 else 0, off))
         rows.append(row)
-    max_rounds = max(counts)
-    w("constexpr int kCoopStages = %d, kCoopWarps = %d, kCoopMaxRounds = %d;" % (len(stages), n_warps, max_rounds))
+    max_rounds = max(len(r) for r in rows)
+    w("struct CoopRound { short variant, nvec, phase, sync; int offset; };  // offset in 16-byte vectors")
+    w("constexpr int kCoopPhases = %d, kCoopWarps = %d, kCoopMaxRounds = %d;" % (len(PHASES), n_warps, max_rounds))
     w("MF_CONST CoopRound kCoopRounds[kCoopWarps][kCoopMaxRounds] = {")
     for wi, row in enumerate(rows):
-        row = row + ["{-1, 0, 0, 0, 0, 0, 0}"] * (max_rounds - len(row))
-        w("  {" + ", ".join(row) + "},  // warp %d: ~%s flop/lane per stage" % (wi, "/".join(str(ld[wi]) for _, ld in sched)))
+        cost = "/".join(str(load[(p, wi)]) for p in PHASES)
+        row = row + ["{-1, 0, 0, 0, 0}"] * (max_rounds - len(row))
+        w("  {" + ", ".join(row) + "},  // warp %d: ~%s flop/lane per phase" % (wi, cost))
     w("};")
-    w("MF_CONST int kCoopNumRounds[kCoopWarps] = {%s};" % ", ".join(map(str, counts)))
-    names = {OP_J: "CoopTaskJ<%d, %d>", OP_XCOL: "CoopTaskX<%d>", OP_YROW: "CoopTaskY<%d, %s>", OP_BIL: "CoopTaskBil"}
-    w("// the (task shape, tasks per lane) combinations the rounds use: X(variant id, tasks per lane, task type)")
+    w("MF_CONST int kCoopNumRounds[kCoopWarps] = {%s};" % ", ".join(str(len(r)) for r in rows))
+    w("// the task shapes the rounds use: X(variant id, task type)")
     w("#define MF_COOP_VARIANTS(X) \\")
-    for i, (op, a, b, m) in enumerate(variants):
-        if op == OP_J:
-            nm = names[op] % (a, b)
-        elif op == OP_XCOL:
-            nm = names[op] % a
-        elif op == OP_YROW:
-            nm = names[op] % (a, "true" if b else "false")
-        else:
-            nm = names[op]
-        w("  X(%d, %d, %s)%s" % (i, m, nm.replace(", ", " MF_COMMA "), " \\" if i + 1 < len(variants) else ""))
-    assert max(words) < 32768 and len(words) % 8 == 0
-    w("// operand indices: vector (offset + (t * nvec + v) * 32 + lane) holds fields 8 v .. 8 v + 7 of task slot t of the lane")
-    w("// (-1 in field 0 = idle slot)")
+    for i, key in enumerate(variants):
+        nm = VARIANT_NAMES[key[0]] % dict(MA=key[1], MD=key[2], M=key[3])
+        w("  X(%d, %s)%s" % (i, nm, " \\" if i + 1 < len(variants) else ""))
+    assert max(words) < 32768 and min(words) >= -1 and len(words) % 8 == 0
+    w("// operand indices: vector (offset + v * 32 + lane) holds fields 8 v .. 8 v + 7 of the lane's task")
+    w("// (-1 in field 0 = idle lane)")
     w("constexpr int kCoopTableVecs = %d;" % (len(words) // 8))
     w("__align__(16) MF_TABLE short kCoopTable[%d] = {" % len(words))
     for i in range(0, len(words), 32):
         w("  " + ", ".join("%d" % v for v in words[i:i + 32]) + ",")
     w("};")
-    return "\n".join(o), sched
+    return "\n".join(o), plan, load
 
 
 def main():
     L = build_layout()
-    stages = build_stages(L)
+    rounds = build_rounds(L)
     s4, Cden, s4_flops = emit_s4(L)
-    tables, sched = emit_tables(L, stages)
-    staged = sum(t["flops"] for st in stages for t in st)
-    s0_flops = 15 * 30 + 200
+    tables, plan, load = emit_tables(L, rounds)
+    staged = sum(t["flops"] for r in rounds for t in r["tasks"])
+    s0_flops = 15 * 30 + 250
     total = s0_flops + staged + 64 * s4_flops
     hdr = ["// GENERATED by gen_coop.py — do not edit.  Cooperative (64 threads per event) matrix element of",
-           "// g g -> t tbar g g: scratch layout, task tables of stages S1-S3, straight-line stage S4.",
+           "// g g -> t tbar g g: scratch layout, task tables of phases S1 / A / B, straight-line stage S4.",
            "#pragma once", '#include "mf_me_prims.cuh"', "",
            "#if defined(__CUDA_ARCH__)", "#define MF_TABLE static __device__ const", "#define MF_CONST static __constant__ const",
            "#else", "#define MF_TABLE static const", "#define MF_CONST static const", "#endif",
            "#if !defined(__CUDACC__)", "#define __align__(n) alignas(n)", "#endif", "",
            "namespace mf {", "",
-           "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | CVEC 8*kCoopNC | SCAL kCoopNX (each region 16-byte aligned)",
-           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopNC = %d, kCoopNX = %d;" % (L.n("V"), L.n("S"), L.n("C"), L.n("X")),
-           "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 8 * kCoopNC + kCoopNX;",
+           "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | Z 2*kCoopZPlane | SCAL kCoopNX (each region 16-byte aligned)",
+           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopNX = %d;" % (L.n("V"), L.n("S"), Z_PLANE, L.n("X")),
+           "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 2 * kCoopZPlane + kCoopNX;",
            "constexpr double kCoopCden = %.1f;" % Cden,
            "// item indices the hand-written stage S0 needs"]
-    for m in range(1, 1 << N):
-        hdr.append("//   P[mask %2d] = VEC %d" % (m, L.get("V", ("P", m))))
-    hdr.append("constexpr int kCoopP0 = %d, kCoopQX0 = %d, kCoopQY0 = %d, kCoopEps0 = %d;" %
-               (L.get("V", ("P", 1)), L.get("V", ("qX", 1)), L.get("V", ("qY", 1)), L.get("V", ("eps", 0, 0))))
-    hdr.append("constexpr int kCoopUb0 = %d, kCoopV0 = %d;" % (L.get("S", ("ub", 0)), L.get("S", ("v", 0))))
+    hdr.append("constexpr int kCoopP0 = %d, kCoopEps0 = %d, kCoopC0 = %d;" %
+               (L.get("V", ("P", 1)), L.get("V", ("eps", 0, 0)), L.get("V", ("c0", 0, 0))))
+    hdr.append("constexpr int kCoopUb = %d, kCoopV0 = %d;" % (L.get("S", ("ub",)), L.get("S", ("v", 0))))
 
     def tab(name, arr, key_of):
         vals = []
         for m in range(1, 1 << N):
-            k = key_of(m)
-            vals.append(str(L.idx[arr].get(k, -1)))
+            vals.append(str(L.idx[arr].get(key_of(m), -1)))
         return "MF_TABLE short %s[15] = {%s};" % (name, ", ".join(vals))
 
     hdr.append(tab("kCoopQXofMask", "V", lambda m: ("qX", m)))
@@ -551,12 +585,21 @@ def main():
     hdr.append(tab("kCoopIP2ofMask", "X", lambda m: ("iP2", m)))
     hdr.append(tab("kCoopIdXofMask", "X", lambda m: ("idX", m)))
     hdr.append(tab("kCoopIdYofMask", "X", lambda m: ("idY", m)))
-    hdr.append("// static fp64 operation count per event (adds + multiplies, FMA = 2): S0 %d + S1-S3 %d + 64 x S4 %d" %
+    hdr.append("// static fp64 operation count per event (adds + multiplies, FMA = 2): S0 %d + S1/A/B %d + 64 x S4 %d" %
                (s0_flops, staged, s4_flops))
     hdr.append("constexpr double kFlopsMe2Coop_2g = %d.0;" % total)
     hdr.append("")
-    loaders = '''// Scratch items are stored as planes of double2 so that consecutive lanes reading consecutive items issue
-// conflict-free 128-bit shared-memory loads: VEC plane p = components (2p, 2p+1); SPIN / CVEC plane c = (re[c], im[c]).
+    text = "\n".join(hdr) + "\n" + LOADERS + "\n" + tables + "\n\n" + s4 + "\n\n}  // namespace mf\n"
+    path = os.path.join(HERE, "mf_me_ttgg_coop_generated.cuh")
+    old = open(path).read() if os.path.exists(path) else None
+    if old != text:
+        with open(path, "w") as f:
+            f.write(text)
+    return path
+
+
+LOADERS = '''// Scratch items are stored as planes of double2 so that consecutive lanes reading consecutive items issue
+// conflict-free 128-bit shared-memory loads: VEC plane p = components (2p, 2p+1); SPIN plane c = (re[c], im[c]).
 MF_HD rvec coop_ld_vec(const double* V, int i) {
   const double2* q = reinterpret_cast<const double2*>(V);
   const double2 a = q[i], b = q[kCoopNV + i];
@@ -581,26 +624,35 @@ MF_HD void coop_st_spin(double* S, int i, const spin& r) {
 #pragma unroll
   for (int c = 0; c < 4; ++c) q[c * kCoopNS + i] = make_double2(r.re[c], r.im[c]);
 }
-MF_HD cvec coop_ld_cvec(const double* C, int i) {
-  const double2* q = reinterpret_cast<const double2*>(C);
-  cvec r;
+// x or -x without touching the FP64 pipe (sign-bit flip)
+MF_HD double mf_flip(double x, int neg) {
+#if defined(__CUDA_ARCH__)
+  return __hiloint2double(__double2hiint(x) ^ (neg << 31), __double2loint(x));
+#else
+  return neg ? -x : x;
+#endif
+}
+// Part k (0 = real, 1 = imaginary) of row . column = sum_m r.re x_a + r.im' x_b with the row prepared by
+// coop_row_part (imaginary parts negated for k = 0) and the column by coop_col_part ((re, im) swapped for k = 1).
+MF_HD spin coop_row_part(spin r, int k) {
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { const double2 t = q[c * kCoopNC + i]; r.re[c] = t.x; r.im[c] = t.y; }
+  for (int m = 0; m < 4; ++m) r.im[m] = mf_flip(r.im[m], k ^ 1);
   return r;
 }
-MF_HD void coop_st_cvec(double* C, int i, const cvec& r) {
-  double2* q = reinterpret_cast<double2*>(C);
+MF_HD spin coop_col_part(const spin& c, int k) {
+  spin o;
 #pragma unroll
-  for (int c = 0; c < 4; ++c) q[c * kCoopNC + i] = make_double2(r.re[c], r.im[c]);
+  for (int m = 0; m < 4; ++m) { o.re[m] = k ? c.im[m] : c.re[m]; o.im[m] = k ? c.re[m] : c.im[m]; }
+  return o;
+}
+MF_HD double sdot_part(const spin& r, const spin& c) {
+  double acc = r.re[0] * c.re[0];
+  acc = fma(r.im[0], c.im[0], acc);
+#pragma unroll
+  for (int m = 1; m < 4; ++m) { acc = fma(r.re[m], c.re[m], acc); acc = fma(r.im[m], c.im[m], acc); }
+  return acc;
 }
 '''
-    text = "\n".join(hdr) + "\n" + loaders + "\n" + tables + "\n\n" + s4 + "\n\n}  // namespace mf\n"
-    path = os.path.join(HERE, "mf_me_ttgg_coop_generated.cuh")
-    old = open(path).read() if os.path.exists(path) else None
-    if old != text:
-        with open(path, "w") as f:
-            f.write(text)
-    return path
 
 
 if __name__ == "__main__":

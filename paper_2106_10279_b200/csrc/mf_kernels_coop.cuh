@@ -3,18 +3,20 @@
 // arithmetic) by teams of 64 threads per event over a shared-memory scratch
 // (mf_me_coop.cuh).
 //
-// Block = T teams of 64 threads (T = 5 for 50 bins: 5 x 42.8 kB of scratch + grid + histogram + PDF row fill the
-// 227 kB of one SM; one block per SM).  Per round every thread generates its own event; each team then walks
-// over the events of its 64 threads that passed the cuts: the owner publishes the four final-state momenta,
-// the team computes |M|^2, the owner keeps the result.  Teams never wait for each other inside the event loop
-// (named barriers, one per team); the only block-wide barriers are at start-up and in the final reduction.
+// Block = T teams of 64 threads (T = 6 for 50 bins: 6 x 30.8 kB of scratch + operand table + grid + histogram +
+// PDF row fill the 227 kB of one SM; one block per SM, 12 warps = 3 per scheduler, <= 168 registers).  Per round
+// every thread generates its own event; the events of the block that passed the cuts are ranked and in step s
+// team t computes the event of rank s T + t: the owner publishes the four final-state momenta, the team computes
+// |M|^2, the owner reads the result.  All teams execute the matrix-element program in lock-step (block barriers
+// between its stages): the SM then fetches ONE instruction stream, which matters because the program is larger
+// than the instruction caches.
 #pragma once
 #include "mf_kernels.cuh"
 #include "mf_me_coop.cuh"
 
 namespace mf {
 
-constexpr int kCoopMaxTeams = 4;
+constexpr int kCoopMaxTeams = 6;
 
 // shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
 struct CoopSmem {
@@ -62,24 +64,31 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
     total += c;
   }
   const int rank = base + __popc(bal & ((1u << lane) - 1u));
-  const int my_step = pass ? rank / n_teams : -1, my_team = rank - (rank / n_teams) * n_teams;
+  const int my_step = pass ? rank / n_teams : -2, my_team = rank - (rank / n_teams) * n_teams;
   const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam;
   double* tm = teams + team * kCoopTeamDoubles;
   double* mine = teams + my_team * kCoopTeamDoubles;
   const int n_steps = (total + n_teams - 1) / n_teams;
   double me2 = 0.0;
+  // The owner of step s + 1 publishes its momenta while the teams finish step s (the input area is read only by S0,
+  // which lies at least one barrier back), so one barrier per step separates "results written / inputs written"
+  // from "results read / S0 starts".
+  auto publish = [&]() {
+    double* in = mine + kCoopOffIn;
+#pragma unroll
+    for (int f = 0; f < 4; ++f)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) in[4 * f + c] = k[f][c];
+    in[16] = shat;
+  };
+  if (my_step == 0) publish();
+  __syncthreads();
   for (int s = 0; s < n_steps; ++s) {
-    if (s == my_step) {
-      double* in = mine + kCoopOffIn;
-#pragma unroll
-      for (int f = 0; f < 4; ++f)
-#pragma unroll
-        for (int c = 0; c < 4; ++c) in[4 * f + c] = k[f][c];
-      in[16] = shat;
-    }
-    __syncthreads();
     coop_me2_lockstep(tm, tab, tid, s * n_teams + team < total, P.m_top);
-    if (s == my_step) me2 = (mine[kCoopOffRed] + mine[kCoopOffRed + 1]) * (P.me_norm / kCoopCden);
+    if (my_step == s + 1) publish();
+    __syncthreads();
+    // top spin state 0 only: the other one gives the same sum (spin-flip symmetry), hence the factor 2
+    if (s == my_step) me2 = (mine[kCoopOffRed] + mine[kCoopOffRed + 1]) * (2.0 * P.me_norm / kCoopCden);
   }
   return me2;
 }

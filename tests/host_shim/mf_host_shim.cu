@@ -37,13 +37,13 @@ double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {
   for (int i = 0; i < 4; ++i) for (int m = 0; m < 4; ++m) in[4 * i + m] = mom[(2 + i) * 4 + m];
   in[16] = 4.0 * mom[0] * mom[0];
   for (int t = 0; t < kCoopTeam; ++t) coop_s0(tm.data(), in, t, m_top);
-  for (int s = 0; s < kCoopStages; ++s)
+  for (int s = 0; s < kCoopPhases; ++s)
     for (int w = 0; w < kCoopWarps; ++w)
-      for (int l = 0; l < 32; ++l) coop_run_stage(tm.data(), reinterpret_cast<const uint4*>(kCoopTable), s, w, l, m_top);
+      for (int l = 0; l < 32; ++l) coop_run_phase(tm.data(), reinterpret_cast<const uint4*>(kCoopTable), s, w, l, m_top);
   double sum = 0.0;
   for (int t = 0; t < kCoopTeam; ++t) sum += coop_s4_thread(tm.data(), t);
   double gs2 = 4.0 * kPi * alpha_s;
-  return sum / kCoopCden * (gs2 * gs2 * gs2 * gs2 / 512.0);
+  return 2.0 * sum / kCoopCden * (gs2 * gs2 * gs2 * gs2 / 512.0);   // top spin 0 only, doubled (spin-flip symmetry)
 }
 
 void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {
