@@ -99,8 +99,9 @@ ORDERED_PAIRS = list(itertools.permutations(LABELS, 2))
 PAIR_INDEX = {p: i for i, p in enumerate(ORDERED_PAIRS)}
 SEQS = {k: [s for s in itertools.permutations(LABELS, k) if canon(s)[0] == s] for k in range(2, N + 1)}
 SEQ_INDEX = {k: {s: i for i, s in enumerate(SEQS[k])} for k in SEQS}
-Z_PLANE = 2 * 12 * 2 * 16   # doubles per re / im plane: z2[12][2][16] then z5[12][2][16]
-Z5_OFF = 12 * 2 * 16
+Z_ROW = 17                  # row stride of the z arrays (16 polarisation words + 1 pad: spreads the writers' banks)
+Z_PLANE = 2 * 12 * 2 * Z_ROW   # doubles per re / im plane: z2[12 seqs][2 hb][Z_ROW] then z5[12 pairs][2 hb][Z_ROW]
+Z5_OFF = 12 * 2 * Z_ROW
 
 
 def build_layout():
@@ -179,11 +180,11 @@ def P_ref(L, seq):
 
 
 def z2_index(seq, pols):
-    return (SEQ_INDEX[4][seq] * 2) * 16 + pols          # hb = 0, k = 0; hb stride 16, k stride Z_PLANE
+    return (SEQ_INDEX[4][seq] * 2) * Z_ROW + pols       # hb = 0, k = 0; hb stride Z_ROW, k stride Z_PLANE
 
 
 def z5_index(pair, hb, pols):
-    return Z5_OFF + (PAIR_INDEX[pair] * 2 + hb) * 16 + pols
+    return Z5_OFF + (PAIR_INDEX[pair] * 2 + hb) * Z_ROW + pols
 
 
 # ---- flop model of the task templates of mf_me_coop.cuh (adds + multiplies, FMA = 2; shared dot products of
@@ -409,7 +410,7 @@ def emit_s4(L):
     for m in LABELS:
         rest = [g for g in LABELS if g != m]
         w("  const int pt%d = ps%d | (ps%d << 1) | (ps%d << 2);" % (m, rest[0], rest[1], rest[2]))
-    w("  const double* Zk = Z + k * %d + hb * 16 + pols;" % Z_PLANE)
+    w("  const double* Zk = Z + k * %d + hb * %d + pols;" % (Z_PLANE, Z_ROW))
     w("  double " + ", ".join("A%d%d%d%d" % p for p in perms) + ";")
     # term 1: Ytilde(ab) . Xhat(cd); k selects the real or the imaginary part of the product
     for a, b in itertools.combinations(LABELS, 2):
@@ -433,7 +434,7 @@ def emit_s4(L):
     # term 2: z2 = c0 . J4(sigma), stored by the J4 tasks
     w("  {")
     for i, s in enumerate(SEQS[4]):
-        w("    { const double z = Zk[%d];" % (i * 32))
+        w("    { const double z = Zk[%d];" % (i * 2 * Z_ROW))
         add(s, "z", 1)
         add(s[::-1], "z", (-1) ** (4 + 1))
         w("    }")
@@ -458,31 +459,66 @@ def emit_s4(L):
     # term 5: z5 = c(a, d) . J2(bc), stored by the z5 tasks
     for (a, d) in ORDERED_PAIRS:
         b, c = [g for g in LABELS if g not in (a, d)]
-        w("  { const double z = Zk[%d];" % (Z5_OFF + PAIR_INDEX[(a, d)] * 32))
+        w("  { const double z = Zk[%d];" % (Z5_OFF + PAIR_INDEX[(a, d)] * 2 * Z_ROW))
         add((a, b, c, d), "z", 1)
         add((a, c, b, d), "z", -1)
         w("  }")
-    # colour contraction grouped by distinct matrix entry
-    groups = {}
-    for i in range(len(perms)):
-        for j in range(i, len(perms)):
-            v = int(Cnum[i, j]) * (1 if i == j else 2)
-            if v:
-                groups.setdefault(v, []).append((i, j))
-    w("  double acc = 0.0, g;")
-    for v in sorted(groups):
-        first = True
-        for (i, j) in groups[v]:
-            a, b = "A%d%d%d%d" % perms[i], "A%d%d%d%d" % perms[j]
-            if first:
-                w("  g = %s * %s;" % (a, b))
-                flops += 1
-            else:
-                w("  g = fma(%s, %s, g);" % (a, b))
+    # Colour contraction in a symmetry-adapted basis.  The colour matrix is invariant under relabelling the gluons,
+    # C[rho s][rho s'] = C[s][s'], in particular under the Klein four-group V4 = {e, (01)(23), (02)(13), (03)(12)}:
+    # in the basis y(chi, orbit) = sum_{rho in V4} chi(rho) x[rho s] (4 characters x 6 orbits, add/subtract
+    # butterflies only) it is block diagonal, x^T C x = sum_chi y_chi^T M_chi y_chi / 16, and sequence reversal
+    # (which also leaves C invariant and maps every V4 orbit to itself) empties most of the three non-trivial
+    # blocks: 57 products instead of 300.  Exact integer arithmetic here; the /16 is folded into the literals.
+    V4 = [(0, 1, 2, 3), (1, 0, 3, 2), (2, 3, 0, 1), (3, 2, 1, 0)]
+    pidx = {p: i for i, p in enumerate(perms)}
+    seen, orbits = set(), []
+    for sgm in perms:
+        if sgm in seen:
+            continue
+        orb = [tuple(r[x] for x in sgm) for r in V4]
+        orbits.append(orb)
+        seen.update(orb)
+    for r in V4:   # the invariance the transformation relies on
+        for s1 in perms:
+            for s2 in perms:
+                assert Cnum[pidx[tuple(r[x] for x in s1)]][pidx[tuple(r[x] for x in s2)]] == Cnum[pidx[s1]][pidx[s2]]
+    chars = [(1, 1, 1, 1), (1, 1, -1, -1), (1, -1, 1, -1), (1, -1, -1, 1)]
+    T = [[0] * len(perms) for _ in range(len(perms))]
+    for ci, ch in enumerate(chars):
+        for oi, orb in enumerate(orbits):
+            for gi, sgm in enumerate(orb):
+                T[ci * len(orbits) + oi][pidx[sgm]] = ch[gi]
+    nP = len(perms)
+    CT = [[sum(int(Cnum[i][k]) * T[j][k] for k in range(nP)) for j in range(nP)] for i in range(nP)]
+    M = [[sum(T[i][k] * CT[k][j] for k in range(nP)) for j in range(nP)] for i in range(nP)]
+    nO = len(orbits)
+    for i in range(nP):
+        for j in range(nP):
+            assert M[i][j] == M[j][i] and (i // nO == j // nO or M[i][j] == 0)
+    for oi, orb in enumerate(orbits):
+        x = ["A%d%d%d%d" % p for p in orb]
+        w("  const double s%da = %s + %s, d%da = %s - %s, s%db = %s + %s, d%db = %s - %s;" %
+          (oi, x[0], x[1], oi, x[0], x[1], oi, x[2], x[3], oi, x[2], x[3]))
+        w("  const double y0_%d = s%da + s%db, y1_%d = s%da - s%db, y2_%d = d%da + d%db, y3_%d = d%da - d%db;" %
+          (oi, oi, oi, oi, oi, oi, oi, oi, oi, oi, oi, oi))
+        flops += 8
+    w("  double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;")
+    n_acc = 0
+    for ci in range(len(chars)):
+        for i in range(nO):
+            row = ci * nO + i
+            terms = [(j, M[row][ci * nO + j] * (1 if j == i else 2)) for j in range(i, nO) if M[row][ci * nO + j]]
+            assert terms and terms[0][0] == i
+            expr = "%r * y%d_%d" % (terms[0][1] / 16.0, ci, i)
+            flops += 1
+            for j, v in terms[1:]:
+                expr = "fma(%r, y%d_%d, %s)" % (v / 16.0, ci, j, expr)
                 flops += 2
-            first = False
-        w("  acc = fma(%.1f, g, acc);" % v)
-        flops += 2
+            w("  acc%d = fma(y%d_%d, %s, acc%d);" % (n_acc % 4, ci, i, expr, n_acc % 4))
+            flops += 2
+            n_acc += 1
+    w("  const double acc = (acc0 + acc1) + (acc2 + acc3);")
+    flops += 3
     w("  return acc;")
     w("}")
     return "\n".join(o), Cden, flops
@@ -494,51 +530,39 @@ VARIANT_NAMES = {"J2": "CoopTaskJ2", "X1c": "CoopTaskX1c", "Y1c": "CoopTaskY1c",
 
 
 def emit_tables(L, rounds):
-    """Per warp ONE flat list of rounds over all phases (the last round of a phase carries the barrier flag).  The
-    operand indices of a round are stored as 16-byte vectors of 8 shorts, vector v of all 32 lanes contiguous, so a
-    warp fetches them with conflict-free 128-bit loads."""
+    """Per warp a straight-line program of rounds over all phases (macro MF_COOP_WARPn: R(offset, task type) per round,
+    S() at the end of a phase = team barrier).  The operand indices of a round are stored as 16-byte vectors of 8
+    shorts, vector v of all 32 lanes contiguous, so a warp fetches them with conflict-free 128-bit loads."""
     o = []
     w = o.append
     words = []
     n_warps = 2
     plan, load = schedule(rounds, n_warps)
-    variants = []
-    rows = []
+    progs = []
     for wi in range(n_warps):
-        row = []
-        for pi, ph in enumerate(PHASES):
-            rs = plan[(ph, wi)]
-            if not rs:   # the barrier still needs a carrier: an empty round
-                row.append("{-1, 0, %d, 1, 0}" % pi)
-                continue
-            for ri, r in enumerate(rs):
+        prog = []
+        for ph in PHASES:
+            for r in plan[(ph, wi)]:
                 nf = max(len(t["fields"]) for t in r["tasks"])
                 nvec = (nf + 7) // 8
-                if r["key"] not in variants:
-                    variants.append(r["key"])
                 off = len(words) // 8
                 for v in range(nvec):
                     for lane in range(32):
                         f = list(r["tasks"][lane]["fields"]) if lane < len(r["tasks"]) else [-1]
                         f += [0] * (nvec * 8 - len(f))
                         words.extend(f[8 * v:8 * v + 8])
-                row.append("{%d, %d, %d, %d, %d}" % (variants.index(r["key"]), nvec, pi, 1 if ri == len(rs) - 1 else 0, off))
-        rows.append(row)
-    max_rounds = max(len(r) for r in rows)
-    w("struct CoopRound { short variant, nvec, phase, sync; int offset; };  // offset in 16-byte vectors")
-    w("constexpr int kCoopPhases = %d, kCoopWarps = %d, kCoopMaxRounds = %d;" % (len(PHASES), n_warps, max_rounds))
-    w("MF_CONST CoopRound kCoopRounds[kCoopWarps][kCoopMaxRounds] = {")
-    for wi, row in enumerate(rows):
+                key = r["key"]
+                prog.append("R(%d, %s)" % (off, (VARIANT_NAMES[key[0]] % dict(MA=key[1], MD=key[2], M=key[3])).replace(" MF_COMMA", ",")))
+            prog.append("S()")
+        progs.append(prog)
+    w("constexpr int kCoopPhases = %d, kCoopWarps = %d;" % (len(PHASES), n_warps))
+    w("// the program of each warp of a team: R(table offset in 16-byte vectors, task type) = one round of 32 lane-tasks,")
+    w("// S() = end of a phase (barrier of the team's two warps)")
+    for wi, prog in enumerate(progs):
         cost = "/".join(str(load[(p, wi)]) for p in PHASES)
-        row = row + ["{-1, 0, 0, 0, 0}"] * (max_rounds - len(row))
-        w("  {" + ", ".join(row) + "},  // warp %d: ~%s flop/lane per phase" % (wi, cost))
-    w("};")
-    w("MF_CONST int kCoopNumRounds[kCoopWarps] = {%s};" % ", ".join(str(len(r)) for r in rows))
-    w("// the task shapes the rounds use: X(variant id, task type)")
-    w("#define MF_COOP_VARIANTS(X) \\")
-    for i, key in enumerate(variants):
-        nm = VARIANT_NAMES[key[0]] % dict(MA=key[1], MD=key[2], M=key[3])
-        w("  X(%d, %s)%s" % (i, nm, " \\" if i + 1 < len(variants) else ""))
+        w("// warp %d: ~%s flop/lane per phase" % (wi, cost))
+        w("#define MF_COOP_WARP%d(R, S) \\" % wi)
+        w("  " + " \\\n  ".join(prog))
     assert max(words) < 32768 and min(words) >= -1 and len(words) % 8 == 0
     w("// operand indices: vector (offset + v * 32 + lane) holds fields 8 v .. 8 v + 7 of the lane's task")
     w("// (-1 in field 0 = idle lane)")
@@ -566,7 +590,7 @@ def main():
            "#if !defined(__CUDACC__)", "#define __align__(n) alignas(n)", "#endif", "",
            "namespace mf {", "",
            "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | Z 2*kCoopZPlane | SCAL kCoopNX (each region 16-byte aligned)",
-           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopNX = %d;" % (L.n("V"), L.n("S"), Z_PLANE, L.n("X")),
+           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopZRow = %d, kCoopNX = %d;" % (L.n("V"), L.n("S"), Z_PLANE, Z_ROW, L.n("X")),
            "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 2 * kCoopZPlane + kCoopNX;",
            "constexpr double kCoopCden = %.1f;" % Cden,
            "// item indices the hand-written stage S0 needs"]

@@ -19,6 +19,7 @@ struct mf_process {
   mf::Params P;
   double *d_lnx = nullptr, *d_lnq2 = nullptr, *d_xf = nullptr, *d_row = nullptr;  // PDF table + collapsed row
   mf::BlockPartial* d_partials = nullptr;
+  double* d_queue = nullptr;          // cooperative pass: per-block momenta queue
   double* d_hist_part = nullptr;
   int blocks = 0, threads = mf::kThreads;
   int blocks_unw = 0;
@@ -50,7 +51,7 @@ const void* pass_fn(int proc, bool unw) {
 
 void free_all(mf_process* p) {
   cudaFree(p->d_lnx); cudaFree(p->d_lnq2); cudaFree(p->d_xf); cudaFree(p->d_row);
-  cudaFree(p->d_partials); cudaFree(p->d_hist_part);
+  cudaFree(p->d_partials); cudaFree(p->d_hist_part); cudaFree(p->d_queue);
 }
 
 // launches the fused pass + finalize on `stream`
@@ -66,6 +67,7 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   A.seed = seed; A.first_event = first_event; A.n_events = n_events; A.iteration = iteration;
   A.w_max = w_max; A.records = (char*)d_records; A.capacity = capacity; A.count = (unsigned long long*)d_count;
   A.partials = p->d_partials; A.hist_part = d_hist ? p->d_hist_part : nullptr;
+  A.coop_queue = p->d_queue;
   cudaStream_t st = (cudaStream_t)stream;
   const int blocks = unw ? p->blocks_unw : p->blocks;
   void* args[2] = {(void*)&p->P, (void*)&A};
@@ -176,6 +178,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   const int max_blocks = p->blocks > p->blocks_unw ? p->blocks : p->blocks_unw;
   if ((e = cudaMalloc(&p->d_partials, (size_t)max_blocks * sizeof(mf::BlockPartial))) != cudaSuccess ||
       (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {
+    free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
+  }
+  if (p->process == 3 &&
+      (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads * mf::kCoopQueueDoubles * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
   snprintf(p->err, sizeof(p->err), "ok");

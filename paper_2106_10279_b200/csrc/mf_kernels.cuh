@@ -35,6 +35,7 @@ struct PassArgs {
   unsigned long long* count;
   BlockPartial* partials;  // [gridDim.x]
   double* hist_part;       // [gridDim.x][D*nb] or nullptr
+  double* coop_queue;      // g g -> t tbar g g only: [gridDim.x][blockDim.x][18] momenta queue (mf_kernels_coop.cuh)
 };
 
 // The matrix element is the only large piece of code; keep ONE copy per process per kernel.

@@ -5,11 +5,12 @@
 //
 // Block = T teams of 64 threads (T = 6 for 50 bins: 6 x 30.8 kB of scratch + operand table + grid + histogram +
 // PDF row fill the 227 kB of one SM; one block per SM, 12 warps = 3 per scheduler, <= 168 registers).  Per round
-// every thread generates its own event; the events of the block that passed the cuts are ranked and in step s
-// team t computes the event of rank s T + t: the owner publishes the four final-state momenta, the team computes
-// |M|^2, the owner reads the result.  All teams execute the matrix-element program in lock-step (block barriers
-// between its stages): the SM then fetches ONE instruction stream, which matters because the program is larger
-// than the instruction caches.
+// every thread generates its own event; the events of the block that passed the cuts are ranked and their
+// momenta queued (a per-block slice of a small L2-resident buffer); team t then works through ranks t, t + T, ...
+// on its own, synchronising only its two warps (named barriers), and leaves |M|^2 in a per-rank result slot that
+// the owner reads after the round's closing block barrier.  Teams therefore sit in different stages of the
+// program at any time, so the latency-bound stages of one team (S0, barriers, table fetches) overlap the
+// FP64-bound stages of the others.
 #pragma once
 #include "mf_kernels.cuh"
 #include "mf_me_coop.cuh"
@@ -18,9 +19,11 @@ namespace mf {
 
 constexpr int kCoopMaxTeams = 6;
 
+constexpr int kCoopQueueDoubles = kCoopInDoubles;   // queue entry: k[4][4], shat, pad
+
 // shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
 struct CoopSmem {
-  int grid, hist, lnx, row, red, cnt, tab, teams, total;
+  int grid, hist, lnx, row, red, cnt, res, tab, teams, total;
   __host__ __device__ CoopSmem(int D, int nb, int nx, int n_teams) {
     auto even = [](int v) { return (v + 1) & ~1; };
     grid = 0;
@@ -29,14 +32,16 @@ struct CoopSmem {
     row = lnx + even(nx);
     red = row + even(nx);
     cnt = red + 5 * 32;
-    tab = cnt + 32;
+    res = cnt + 32;
+    tab = res + 2 * n_teams * kCoopTeam;
     teams = tab + 2 * kCoopTableVecs;
     total = teams + n_teams * kCoopTeamDoubles;
   }
 };
 
-// shared memory of the single-team debug kernels: team | rank counters | operand table
-constexpr int kCoopDebugSmemBytes = (kCoopTeamDoubles + 32 + 2 * kCoopTableVecs) * 8;
+// shared memory of the single-team debug kernels: team | rank counters | results | queue | operand table
+constexpr int kCoopDebugSmemBytes =
+    (kCoopTeamDoubles + 32 + 2 * kCoopTeam + kCoopTeam * kCoopQueueDoubles + 2 * kCoopTableVecs) * 8;
 
 // copies the operand table into shared memory (all threads of the block; the caller synchronises)
 __device__ __forceinline__ void coop_load_table(uint4* s_tab) {
@@ -44,53 +49,67 @@ __device__ __forceinline__ void coop_load_table(uint4* s_tab) {
   for (int i = threadIdx.x; i < kCoopTableVecs; i += blockDim.x) s_tab[i] = g[i];
 }
 
+// barrier of the two warps of one team (named barrier 1 + team; barrier 0 is __syncthreads)
+__device__ __forceinline__ void coop_team_sync(int team) {
+  asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "r"(kCoopTeam) : "memory");
+}
+
 // |M|^2 (with couplings and averaging) of this thread's own event.  EVERY thread of the block must call it (it
 // contains block barriers).  The events of the block that passed the cuts are ranked (ballot + prefix over the
-// warps); in step s team t computes the event of rank s * n_teams + t: its owner (any thread of the block)
-// writes the momenta into that team's input area and reads the result from the team's reduction slots.
-// s_cnt: 2 x 32 unsigned (double-buffered by `round`).  Returns 0 for threads whose event did not pass.
+// warps) and queued; team t computes ranks t, t + n_teams, ...  `queue` holds blockDim.x entries (global memory
+// in the fused pass, shared memory in the debug kernels), s_res 2 doubles per thread of the block, s_cnt 2 x 32
+// unsigned (double-buffered by `round`).  Returns 0 for threads whose event did not pass.
 __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, const uint4* tab, unsigned* s_cnt,
-                                                 unsigned round, bool pass, const double (*k)[4], double shat,
-                                                 const Params& P) {
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+                                                 double* s_res, double* queue, unsigned round, bool pass,
+                                                 const double (*k)[4], double shat, const Params& P) {
+  const int bwarp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   unsigned* cnt = s_cnt + 32 * (round & 1u);
   const unsigned bal = __ballot_sync(0xFFFFFFFFu, pass);
-  if (lane == 0) cnt[warp] = __popc(bal);
+  if (lane == 0) cnt[bwarp] = __popc(bal);
   __syncthreads();
   int base = 0, total = 0;
   for (int w = 0; w < n_warps; ++w) {
     const int c = (int)cnt[w];
-    if (w < warp) base += c;
+    if (w < bwarp) base += c;
     total += c;
   }
   const int rank = base + __popc(bal & ((1u << lane) - 1u));
-  const int my_step = pass ? rank / n_teams : -2, my_team = rank - (rank / n_teams) * n_teams;
-  const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam;
-  double* tm = teams + team * kCoopTeamDoubles;
-  double* mine = teams + my_team * kCoopTeamDoubles;
-  const int n_steps = (total + n_teams - 1) / n_teams;
-  double me2 = 0.0;
-  // The owner of step s + 1 publishes its momenta while the teams finish step s (the input area is read only by S0,
-  // which lies at least one barrier back), so one barrier per step separates "results written / inputs written"
-  // from "results read / S0 starts".
-  auto publish = [&]() {
-    double* in = mine + kCoopOffIn;
+  if (pass) {
+    double* q = queue + rank * kCoopQueueDoubles;
 #pragma unroll
     for (int f = 0; f < 4; ++f)
 #pragma unroll
-      for (int c = 0; c < 4; ++c) in[4 * f + c] = k[f][c];
-    in[16] = shat;
-  };
-  if (my_step == 0) publish();
-  __syncthreads();
-  for (int s = 0; s < n_steps; ++s) {
-    coop_me2_lockstep(tm, tab, tid, s * n_teams + team < total, P.m_top);
-    if (my_step == s + 1) publish();
-    __syncthreads();
-    // top spin state 0 only: the other one gives the same sum (spin-flip symmetry), hence the factor 2
-    if (s == my_step) me2 = (mine[kCoopOffRed] + mine[kCoopOffRed + 1]) * (2.0 * P.me_norm / kCoopCden);
+      for (int c = 0; c < 4; ++c) q[4 * f + c] = k[f][c];
+    q[16] = shat;
   }
-  return me2;
+  __syncthreads();
+  {
+    const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam, warp = tid >> 5;
+    double* tm = teams + team * kCoopTeamDoubles;
+    double* in = tm + kCoopOffIn;
+    double nxt = 0.0;
+    if (team < total && tid < 17) nxt = queue[team * kCoopQueueDoubles + tid];
+#pragma unroll 1
+    for (int r = team; r < total; r += n_teams) {
+      if (tid < 17) in[tid] = nxt;
+      coop_team_sync(team);
+      if (r + n_teams < total && tid < 17) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // used next turn
+      coop_s0(tm, in, tid, P.m_top);
+      coop_team_sync(team);
+#define MF_R(OFF, ...) coop_run_task<__VA_ARGS__>(tm, tab, OFF, lane, P.m_top);
+#define MF_S() coop_team_sync(team);
+      if (warp == 0) { MF_COOP_WARP0(MF_R, MF_S) } else { MF_COOP_WARP1(MF_R, MF_S) }
+#undef MF_R
+#undef MF_S
+      double acc = coop_s4_thread(tm, tid);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+      if (lane == 0) s_res[2 * r + warp] = acc;
+    }
+  }
+  __syncthreads();
+  // top spin state 0 only: the other one gives the same sum (spin-flip symmetry), hence the factor 2
+  return pass ? (s_res[2 * rank] + s_res[2 * rank + 1]) * (2.0 * P.me_norm / kCoopCden) : 0.0;
 }
 
 template <bool UNW>
@@ -107,8 +126,10 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
   double* s_row = smem + L.row;
   double* s_red = smem + L.red;
   unsigned* s_cnt = reinterpret_cast<unsigned*>(smem + L.cnt);
+  double* s_res = smem + L.res;
   double* s_teams = smem + L.teams;
   uint4* s_tab = reinterpret_cast<uint4*>(smem + L.tab);
+  double* queue = A.coop_queue + (size_t)blockIdx.x * blockDim.x * kCoopQueueDoubles;
   coop_load_table(s_tab);
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
@@ -133,7 +154,7 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
       if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
     }
     const bool pass = valid && ev.pass;
-    const double me2 = coop_block_me2(s_teams, n_teams, s_tab, s_cnt, (unsigned)rd, pass, ev.k, ev.shat, P);
+    const double me2 = coop_block_me2(s_teams, n_teams, s_tab, s_cnt, s_res, queue, (unsigned)rd, pass, ev.k, ev.shat, P);
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
@@ -150,7 +171,9 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
   extern __shared__ double2 smem2[];
   double* tm = reinterpret_cast<double*>(smem2);
   unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
-  uint4* s_tab = reinterpret_cast<uint4*>(tm + kCoopTeamDoubles + 32);
+  double* s_res = tm + kCoopTeamDoubles + 32;
+  double* queue = s_res + 2 * kCoopTeam;
+  uint4* s_tab = reinterpret_cast<uint4*>(queue + kCoopTeam * kCoopQueueDoubles);
   coop_load_table(s_tab);
   __syncthreads();
   const int row_len = 3 * D + 4 * (NF + 2) + 9;
@@ -166,7 +189,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
     generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
   }
   const bool pass = valid && ev.pass;
-  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, 0u, pass, ev.k, ev.shat, P);
+  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, s_res, queue, 0u, pass, ev.k, ev.shat, P);
   if (!valid) return;
   double mom[NF + 2][4];
   lab_momenta<PROC>(ev, mom);
@@ -189,7 +212,9 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
   extern __shared__ double2 smem2[];
   double* tm = reinterpret_cast<double*>(smem2);
   unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
-  uint4* s_tab = reinterpret_cast<uint4*>(tm + kCoopTeamDoubles + 32);
+  double* s_res = tm + kCoopTeamDoubles + 32;
+  double* queue = s_res + 2 * kCoopTeam;
+  uint4* s_tab = reinterpret_cast<uint4*>(queue + kCoopTeam * kCoopQueueDoubles);
   coop_load_table(s_tab);
   __syncthreads();
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -202,7 +227,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
       for (int c = 0; c < 4; ++c) k[f][c] = m[(2 + f) * 4 + c];
     shat = 4.0 * m[0] * m[0];
   }
-  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, 0u, valid, k, shat, P);
+  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, s_res, queue, 0u, valid, k, shat, P);
   if (valid) out[i] = me2;
 }
 

@@ -51,7 +51,7 @@ MF_HD rvec coop_gluon_momentum(const double* in, int g) {
 }
 
 // team threads 0..14 (warp 0): one gluon subset each; 32..33 (warp 1): the polarisation vectors of the final
-// gluons; 34..35: v(hb), ubar and c0(hb) = ubar gamma^mu v(hb); 36..39: the constant beam polarisations
+// gluons; 34..35: v(hb), ubar and c0(hb) = ubar gamma^mu v(hb); 16..19 (warp 0): the constant beam polarisations
 MF_HD void coop_s0(double* scr, const double* in, int tid, double mt) {
   double* V = coop_V(scr);
   double* S = coop_S(scr);
@@ -91,8 +91,8 @@ MF_HD void coop_s0(double* scr, const double* in, int tid, double mt) {
     const cvec c = bilinear(ub, v);
     coop_st_vec(V, kCoopC0 + 2 * hb, rvec{{c.re[0], c.re[1], c.re[2], c.re[3]}});
     coop_st_vec(V, kCoopC0 + 2 * hb + 1, rvec{{c.im[0], c.im[1], c.im[2], c.im[3]}});
-  } else if (tid >= 36 && tid < 40) {
-    const int g = (tid - 36) >> 1, p = (tid - 36) & 1;
+  } else if (tid >= 16 && tid < 20) {
+    const int g = (tid - 16) >> 1, p = (tid - 16) & 1;
     const rvec e = p == 0 ? rvec{{0.0, 1.0, 0.0, 0.0}} : rvec{{0.0, 0.0, g == 0 ? 1.0 : -1.0, 0.0}};
     coop_st_vec(V, kCoopEps0 + 2 * g + p, e);
   }
@@ -110,12 +110,12 @@ MF_HD int coop_fld(const CoopFields<NVEC>& F, int j) {   // j is a compile-time 
   return (int)(short)((j & 1) ? (w >> 16) : (w & 0xFFFFu));
 }
 
-// `tab` is the operand table (kCoopTable; a shared-memory copy on the device)
+// `tab` is the operand table (kCoopTable; a shared-memory copy on the device), `offset` the round's first vector
 template <int NVEC>
-MF_HD CoopFields<NVEC> coop_load_fields(const uint4* tab, const CoopRound& R, int lane) {
+MF_HD CoopFields<NVEC> coop_load_fields(const uint4* tab, int offset, int lane) {
   CoopFields<NVEC> F;
 #pragma unroll
-  for (int v = 0; v < NVEC; ++v) F.q[v] = tab[R.offset + v * 32 + lane];
+  for (int v = 0; v < NVEC; ++v) F.q[v] = tab[offset + v * 32 + lane];
   return F;
 }
 
@@ -280,7 +280,7 @@ template <int MA, int MD> struct CoopTaskJ4 {
     for (int h = 0; h < 4; ++h) {   // h = 2 hb + k
       const rvec c = rscale(coop_ld_vec(V, ic0 + h), ip2);
 #pragma unroll
-      for (int m = 0; m < MM; ++m) Z[coop_fld(F, m) + (h >> 1) * 16 + (h & 1) * kCoopZPlane] = rdot(c, acc[m]);
+      for (int m = 0; m < MM; ++m) Z[coop_fld(F, m) + (h >> 1) * kCoopZRow + (h & 1) * kCoopZPlane] = rdot(c, acc[m]);
     }
   }
 };
@@ -352,27 +352,19 @@ template <int M> struct CoopTaskZ5 {
 
 // One round for one lane: fetch the lane-task's operand indices and run it (idle lanes: field 0 < 0).
 template <class Task>
-MF_HD void coop_run_task(double* scr, const uint4* tab, const CoopRound& R, int lane, double mt) {
-  const CoopFields<Task::NVEC> F = coop_load_fields<Task::NVEC>(tab, R, lane);
+MF_HD void coop_run_task(double* scr, const uint4* tab, int offset, int lane, double mt) {
+  const CoopFields<Task::NVEC> F = coop_load_fields<Task::NVEC>(tab, offset, lane);
   if (coop_fld(F, 0) >= 0) Task::run(scr, F, mt);
 }
 
-#define MF_COMMA ,
-MF_HD void coop_exec_round(double* scr, const uint4* tab, const CoopRound& R, int lane, double mt) {
-  switch (R.variant) {
-#define MF_COOP_CASE(ID, TASK) case ID: coop_run_task<TASK>(scr, tab, R, lane, mt); break;
-    MF_COOP_VARIANTS(MF_COOP_CASE)
-#undef MF_COOP_CASE
-    default: break;
-  }
-}
-
-// Host emulation helper (tests/host_shim): all rounds of `phase` for one (warp, lane).
+// Host emulation helper (tests/host_shim): all rounds of `phase` of the program of `warp`, for one lane.
 MF_HD void coop_run_phase(double* scr, const uint4* tab, int phase, int warp, int lane, double mt) {
-  for (int r = 0; r < kCoopNumRounds[warp]; ++r) {
-    const CoopRound R = kCoopRounds[warp][r];
-    if (R.phase == phase) coop_exec_round(scr, tab, R, lane, mt);
-  }
+  int ph = 0;
+#define MF_R(OFF, ...) if (ph == phase) coop_run_task<__VA_ARGS__>(scr, tab, OFF, lane, mt);
+#define MF_S() ++ph;
+  if (warp == 0) { MF_COOP_WARP0(MF_R, MF_S) } else { MF_COOP_WARP1(MF_R, MF_S) }
+#undef MF_R
+#undef MF_S
 }
 
 // S4 for team thread tid = pols | hb << 4 | k << 5 (k is warp uniform): x^T Cnum x of the real / imaginary parts of
@@ -380,33 +372,5 @@ MF_HD void coop_run_phase(double* scr, const uint4* tab, int phase, int warp, in
 MF_HD double coop_s4_thread(double* scr, int tid) {
   return coop_s4(coop_V(scr), coop_S(scr), coop_Z(scr), tid & 15, (tid >> 4) & 1, (tid >> 5) & 1);
 }
-
-#if defined(__CUDACC__)
-// ---- device-side driver ---------------------------------------------------------------------------------
-// Called by EVERY thread of the block (all teams run in lock-step so that the SM fetches one instruction stream:
-// the per-event program is larger than the instruction cache) after the owners have written the input areas
-// and the block has synchronised.  Teams with `active` false only keep the barriers.  Leaves the two halves of
-// sum_{pols, hb} x^T Cnum x (no couplings, no averaging, top spin 0 only) in the team's reduction slots; the
-// caller synchronises the block before reading them.
-__device__ __forceinline__ void coop_me2_lockstep(double* tm, const uint4* tab, int tid, bool active, double mt) {
-  double* scr = tm;
-  const int warp = tid >> 5, lane = tid & 31;
-  if (active) coop_s0(scr, tm + kCoopOffIn, tid, mt);
-  __syncthreads();
-  const int nr = kCoopNumRounds[warp];
-#pragma unroll 1
-  for (int r = 0; r < nr; ++r) {
-    const CoopRound R = kCoopRounds[warp][r];
-    if (active) coop_exec_round(scr, tab, R, lane, mt);
-    if (R.sync) __syncthreads();
-  }
-  if (active) {
-    double acc = coop_s4_thread(scr, tid);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
-    if (lane == 0) tm[kCoopOffRed + warp] = acc;
-  }
-}
-#endif
 
 }  // namespace mf
