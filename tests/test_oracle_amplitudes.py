@@ -284,6 +284,30 @@ def test_helicity_index_convention_and_average(oracle_procs):
         assert amps.shape == (4 << n, math.factorial(n))
 
 
+@pytest.mark.parametrize("pid,n", [(1, 2), (2, 3), (3, 4)])
+def test_quark_spin_flip_symmetry(oracle_procs, pid, n):
+    """Flipping BOTH quark spins leaves A^dagger C A unchanged once the gluon polarisations are summed (Kramers
+    conjugation: B u* is the spin-flipped spinor, B gamma^mu* B^-1 = gamma^mu).  With real (linear) polarisations
+    it holds polarisation by polarisation, which is what the cooperative CUDA kernel relies on when it evaluates
+    one top spin state and doubles the sum; with circular polarisations all helicities flip together."""
+    P = oracle_procs[pid]
+    C = mfo.colour_matrix(n)
+    rng = np.random.default_rng(23)
+    for _ in range(3):
+        mom = _rambo_event(n, 500.0 + 2500.0 * rng.random(), rng)
+        for basis in (3, 1, 0, 2):            # bit 0: z-spin / helicity spinors, bit 1: linear / circular pols
+            _, amps = P.me2(mom, basis=basis, want_amps=True)
+            q = np.array([(A.conj() @ C @ A).real for A in amps])
+            nh = len(q)
+            flip_quarks = 3 << n                # helicity index: bits (t, tbar, g0, g1, ...), t highest
+            scale = q.max()
+            for h in range(nh):
+                partner = h ^ flip_quarks if basis & 2 else (nh - 1) ^ h
+                assert abs(q[h] - q[partner]) <= 1e-11 * scale
+            # hence: sum over one top spin state, doubled, is the full sum
+            assert 2 * q[: nh // 2].sum() == pytest.approx(q.sum(), rel=1e-12)
+
+
 def test_colour_matrix_closed_forms():
     """O11 pins: diagonal N_c C_F^n; the distinct entries quoted in SURVEY.md; symmetry; rank (the n! orderings
     are linearly dependent only from n >= ... none for n <= 4 in this basis, but C must be positive semidefinite)."""
