@@ -277,8 +277,11 @@ def generate(n):
     for g in range(n):
         w("    const rvec e%d = eps[%d][(gh >> %d) & 1];" % (g, g, g))
     # body
+    # quark spins: only the top spin state 0 (both antitop states); flipping BOTH spins conjugates every colour-ordered
+    # amplitude up to a common phase when the gluon polarisation vectors are real (gen_coop.py), so the other
+    # half of the spin sum equals this one: the result is doubled below
     for hb in range(2):
-        for h in range(2):
+        for h in range(1):
             amps = []
             for s in perms:
                 re, im = E.amplitude(s, h, hb)
@@ -310,7 +313,7 @@ def generate(n):
     for l in E.lines:
         w("    " + l)
     w("  }")
-    w("  return total * (1.0 / %.1f);" % Cden)
+    w("  return total * (2.0 / %.1f);   // x 2: spin-flip symmetry, only top spin 0 was summed" % Cden)
     w("}")
     w("// static fp64 operation count of the code above (adds + multiplies as written, FMA = 2; divisions = 1):")
     w("//   per event %d = preamble %d + %d polarisation combinations x %d" % (flops, pre, 1 << n, body))
