@@ -143,3 +143,40 @@ def run_config(proc, wl=None, capacity=0, stream=None, alpha=W.VEGAS_ALPHA, grid
     if count is not None:
         out.n_records = int(count.item())
     return out
+
+
+def main(argv=None):
+    """python -m paper_2106_10279_b200.integrate [--config C0..C4] [--events N]: runs every iteration of a
+    BASELINE.json configuration on cuda:0 and prints the per-iteration and combined estimates with timings."""
+    import argparse
+    import json
+    import time
+    import torch
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", default="C3")
+    ap.add_argument("--events", type=int, default=0, help="events per iteration (default: the configuration's)")
+    ap.add_argument("--capacity", type=int, default=1 << 20, help="record buffer capacity (unweighting configs)")
+    args = ap.parse_args(argv)
+    wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4}[args.config]
+    if args.events > 0:
+        wl = wl.scaled(args.events)
+    proc = api.Process(wl, W.pdf_table() if wl.process else None)
+    run_config(proc, wl.scaled(min(wl.n_events, 1 << 16)), capacity=args.capacity if wl.unweight else 0)   # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    run = run_config(proc, wl, capacity=args.capacity if wl.unweight else 0)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    for r in run.iterations:
+        print("iteration %2d  I = %.8g +- %.3g pb  max|w| = %.4g  pass %.4f  accepted %d" %
+              (r.iteration, r.integral, r.sigma, r.max_abs_w, r.n_pass / r.n_events, r.n_accept))
+    mean, err, chi2 = run.combined()
+    n_tot = sum(r.n_events for r in run.iterations)
+    print(json.dumps({"config": args.config, "workload": wl.name, "integral_pb": mean, "error_pb": err,
+                      "chi2_per_dof": chi2, "iterations": len(run.iterations), "events_per_iteration": wl.n_events,
+                      "wall_s": dt, "events_per_s": n_tot / dt, "unweighted_events": run.n_records}))
+    proc.close()
+
+
+if __name__ == "__main__":
+    main()
