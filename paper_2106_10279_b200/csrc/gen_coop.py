@@ -598,17 +598,21 @@ def main():
                (L.get("V", ("P", 1)), L.get("V", ("eps", 0, 0)), L.get("V", ("c0", 0, 0))))
     hdr.append("constexpr int kCoopUb = %d, kCoopV0 = %d;" % (L.get("S", ("ub",)), L.get("S", ("v", 0))))
 
-    def tab(name, arr, key_of):
-        vals = []
-        for m in range(1, 1 << N):
-            vals.append(str(L.idx[arr].get(key_of(m), -1)))
-        return "MF_TABLE short %s[15] = {%s};" % (name, ", ".join(vals))
-
-    hdr.append(tab("kCoopQXofMask", "V", lambda m: ("qX", m)))
-    hdr.append(tab("kCoopQYofMask", "V", lambda m: ("qY", m)))
-    hdr.append(tab("kCoopIP2ofMask", "X", lambda m: ("iP2", m)))
-    hdr.append(tab("kCoopIdXofMask", "X", lambda m: ("idX", m)))
-    hdr.append(tab("kCoopIdYofMask", "X", lambda m: ("idY", m)))
+    # S0 lane table: lane l < kCoopS0Lanes computes v = P(mask) (kind 0), P(mask) - p4 (kind 1) or p3 - P(mask) (kind 2),
+    # stores it as VEC item `vec` and, if x >= 0, 1 / (v.v - [kind > 0] m_t^2) as scalar item `x`
+    s0 = []
+    for m in range(1, 1 << N):
+        s0.append((0, m, L.get("V", ("P", m)), L.idx["X"].get(("iP2", m), -1)))
+    for m in range(1, 1 << N):
+        if ("qX", m) in L.idx["V"]:
+            s0.append((1, m, L.get("V", ("qX", m)), L.get("X", ("idX", m))))
+    for m in range(1, 1 << N):
+        if ("qY", m) in L.idx["V"]:
+            s0.append((2, m, L.get("V", ("qY", m)), L.get("X", ("idY", m))))
+    assert len(s0) <= 32
+    hdr.append("constexpr int kCoopS0Lanes = %d;" % len(s0))
+    hdr.append("MF_TABLE short kCoopS0Tab[%d][4] = {%s};   // kind, mask, vec, x" %
+               (len(s0), ", ".join("{%d, %d, %d, %d}" % t for t in s0)))
     hdr.append("// static fp64 operation count per event (adds + multiplies, FMA = 2): S0 %d + S1/A/B %d + 64 x S4 %d" %
                (s0_flops, staged, s4_flops))
     hdr.append("constexpr double kFlopsMe2Coop_2g = %d.0;" % total)

@@ -81,6 +81,7 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
 #pragma unroll
       for (int c = 0; c < 4; ++c) q[4 * f + c] = k[f][c];
     q[16] = shat;
+    q[17] = 0.5 * sqrt(shat);
   }
   __syncthreads();
   {
@@ -88,12 +89,12 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
     double* tm = teams + team * kCoopTeamDoubles;
     double* in = tm + kCoopOffIn;
     double nxt = 0.0;
-    if (team < total && tid < 17) nxt = queue[team * kCoopQueueDoubles + tid];
+    if (team < total && tid < 18) nxt = queue[team * kCoopQueueDoubles + tid];
 #pragma unroll 1
     for (int r = team; r < total; r += n_teams) {
-      if (tid < 17) in[tid] = nxt;
+      if (tid < 18) in[tid] = nxt;
       coop_team_sync(team);
-      if (r + n_teams < total && tid < 17) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // used next turn
+      if (r + n_teams < total && tid < 18) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // used next turn
       coop_s0(tm, in, tid, P.m_top);
       coop_team_sync(team);
 #define MF_R(OFF, ...) coop_run_task<__VA_ARGS__>(tm, tab, OFF, lane, P.m_top);

@@ -39,60 +39,51 @@ MF_HD rvec rflip(const rvec& a, int neg) {
 }
 
 // ---- S0: per-event constants --------------------------------------------------------------------------------
-// in[0..15] = k[4][4] (t, tbar, g2, g3 in the partonic CM frame), in[16] = shat.  Gluon labels: 0, 1 = the beams
-// (+z, -z, energy sqrt(shat)/2), 2, 3 = the final gluons entering with -k (all gluon momenta incoming).
-MF_HD rvec coop_gluon_momentum(const double* in, int g) {
-  const double E = 0.5 * sqrt(in[16]);
-  rvec p;
-  if (g == 0) p = {{E, 0.0, 0.0, E}};
-  else if (g == 1) p = {{E, 0.0, 0.0, -E}};
-  else p = {{-in[4 * g + 0], -in[4 * g + 1], -in[4 * g + 2], -in[4 * g + 3]}};
-  return p;
-}
-
-// team threads 0..14 (warp 0): one gluon subset each; 32..33 (warp 1): the polarisation vectors of the final
-// gluons; 34..35: v(hb), ubar and c0(hb) = ubar gamma^mu v(hb); 16..19 (warp 0): the constant beam polarisations
+// in[0..15] = k[4][4] (t, tbar, g2, g3 in the partonic CM frame), in[16] = shat, in[17] = sqrt(shat) / 2.  Gluon
+// labels: 0, 1 = the beams (+z, -z), 2, 3 = the final gluons entering with -k (all gluon momenta incoming).
+//
+// team threads 0 .. kCoopS0Lanes-1 (warp 0): one momentum sum / propagator momentum and its inverse denominator
+// each (uniform code, one reciprocal per lane; table kCoopS0Tab); 30, 31: v(hb), ubar and c0(hb) = ubar gamma v(hb);
+// 32, 33 (warp 1): the polarisation vectors of the final gluons; 36..39: the constant beam polarisations
 MF_HD void coop_s0(double* scr, const double* in, int tid, double mt) {
   double* V = coop_V(scr);
   double* S = coop_S(scr);
   double* X = coop_X(scr);
-  if (tid < 15) {
-    const int m = tid + 1;
-    rvec P = {{0.0, 0.0, 0.0, 0.0}};
-    int n = 0;
+  if (tid < kCoopS0Lanes) {
+    const int kind = kCoopS0Tab[tid][0], m = kCoopS0Tab[tid][1], iv = kCoopS0Tab[tid][2], ix = kCoopS0Tab[tid][3];
+    const double E = in[17];
+    // sum of the gluon momenta in the mask (beams: (E, 0, 0, +-E); final gluons enter with -k)
+    const double b0 = (m & 1) ? 1.0 : 0.0, b1 = (m & 2) ? 1.0 : 0.0, b2 = (m & 4) ? -1.0 : 0.0, b3 = (m & 8) ? -1.0 : 0.0;
+    rvec P;
+    P.v[0] = fma(b3, in[12], fma(b2, in[8], (b0 + b1) * E));
+    P.v[1] = fma(b3, in[13], b2 * in[9]);
+    P.v[2] = fma(b3, in[14], b2 * in[10]);
+    P.v[3] = fma(b3, in[15], fma(b2, in[11], (b0 - b1) * E));
+    // kind 0: P;  kind 1: P - p4;  kind 2: p3 - P
+    const double sp = kind == 2 ? -1.0 : 1.0;
+    const double* q = kind == 1 ? in + 4 : in;
+    const double sq = kind == 0 ? 0.0 : (kind == 1 ? -1.0 : 1.0);
+    rvec v;
 #pragma unroll
-    for (int g = 0; g < 4; ++g)
-      if ((m >> g) & 1) { P = radd(P, coop_gluon_momentum(in, g)); ++n; }
-    coop_st_vec(V, kCoopP0 + m - 1, P);
-    if (n >= 2) X[kCoopIP2ofMask[m - 1]] = 1.0 / rdot(P, P);
-    const double mt2 = mt * mt;
-    const int ix = kCoopQXofMask[m - 1], iy = kCoopQYofMask[m - 1];
-    if (ix >= 0) {
-      rvec q = {{P.v[0] - in[4], P.v[1] - in[5], P.v[2] - in[6], P.v[3] - in[7]}};   // P - p4
-      coop_st_vec(V, ix, q);
-      X[kCoopIdXofMask[m - 1]] = 1.0 / (rdot(q, q) - mt2);
-    }
-    if (iy >= 0) {
-      rvec q = {{in[0] - P.v[0], in[1] - P.v[1], in[2] - P.v[2], in[3] - P.v[3]}};   // p3 - P
-      coop_st_vec(V, iy, q);
-      X[kCoopIdYofMask[m - 1]] = 1.0 / (rdot(q, q) - mt2);
-    }
-  } else if (tid >= 32 && tid < 34) {
-    const int g = tid - 30;
-    rvec e1, e2;
-    pol_vectors(in + 4 * g, e1, e2);
-    coop_st_vec(V, kCoopEps0 + 2 * g, e1);
-    coop_st_vec(V, kCoopEps0 + 2 * g + 1, e2);
-  } else if (tid >= 34 && tid < 36) {
-    const int hb = tid - 34;
+    for (int c = 0; c < 4; ++c) v.v[c] = fma(sq, q[c], sp * P.v[c]);
+    coop_st_vec(V, iv, v);
+    if (ix >= 0) X[ix] = 1.0 / (rdot(v, v) - (kind == 0 ? 0.0 : mt * mt));
+  } else if (tid >= 30 && tid < 32) {
+    const int hb = tid - 30;
     const spin ub = ubar_row(in, mt, 0), v = v_col(in + 4, mt, hb);
     if (hb == 0) coop_st_spin(S, kCoopUb, ub);
     coop_st_spin(S, kCoopV0 + hb, v);
     const cvec c = bilinear(ub, v);
     coop_st_vec(V, kCoopC0 + 2 * hb, rvec{{c.re[0], c.re[1], c.re[2], c.re[3]}});
     coop_st_vec(V, kCoopC0 + 2 * hb + 1, rvec{{c.im[0], c.im[1], c.im[2], c.im[3]}});
-  } else if (tid >= 16 && tid < 20) {
-    const int g = (tid - 16) >> 1, p = (tid - 16) & 1;
+  } else if (tid >= 32 && tid < 34) {
+    const int g = tid - 30;
+    rvec e1, e2;
+    pol_vectors(in + 4 * g, e1, e2);
+    coop_st_vec(V, kCoopEps0 + 2 * g, e1);
+    coop_st_vec(V, kCoopEps0 + 2 * g + 1, e2);
+  } else if (tid >= 36 && tid < 40) {
+    const int g = (tid - 36) >> 1, p = (tid - 36) & 1;
     const rvec e = p == 0 ? rvec{{0.0, 1.0, 0.0, 0.0}} : rvec{{0.0, 0.0, g == 0 ? 1.0 : -1.0, 0.0}};
     coop_st_vec(V, kCoopEps0 + 2 * g + p, e);
   }
@@ -370,7 +361,8 @@ MF_HD void coop_run_phase(double* scr, const uint4* tab, int phase, int warp, in
 // S4 for team thread tid = pols | hb << 4 | k << 5 (k is warp uniform): x^T Cnum x of the real / imaginary parts of
 // its helicity combination (colour-matrix numerators; the team sum times 2 / kCoopCden is sum_hel A^dagger C A).
 MF_HD double coop_s4_thread(double* scr, int tid) {
-  return coop_s4(coop_V(scr), coop_S(scr), coop_Z(scr), tid & 15, (tid >> 4) & 1, (tid >> 5) & 1);
+  const int pols = tid & 15, hb = (tid >> 4) & 1;
+  return coop_s4(coop_V(scr), coop_S(scr), coop_Z(scr), pols, hb, (tid >> 5) & 1);
 }
 
 }  // namespace mf

@@ -237,7 +237,7 @@ MF_HD spin v_col(const double p[4], double m, int s) {
 // limit is taken towards the x axis): e1 = (0; kx kz/(|k| pT), ky kz/(|k| pT), -pT/|k|), e2 = (0; -ky/pT, kx/pT, 0).
 MF_HD void pol_vectors(const double k[4], rvec& e1, rvec& e2) {
   double pt2 = k[1] * k[1] + k[2] * k[2];
-  double pt = sqrt(pt2), pabs = sqrt(pt2 + k[3] * k[3]);
+  double pt = sqrt(pt2), pabs = k[0];   // massless: |k| = E
   if (pt > 0.0) {
     double ipt = 1.0 / pt, ip = 1.0 / pabs;
     double cx = k[1] * ipt, cy = k[2] * ipt, cz = k[3] * ip, sz = pt * ip;

@@ -36,6 +36,7 @@ double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {
   double* in = tm.data() + kCoopOffIn;
   for (int i = 0; i < 4; ++i) for (int m = 0; m < 4; ++m) in[4 * i + m] = mom[(2 + i) * 4 + m];
   in[16] = 4.0 * mom[0] * mom[0];
+  in[17] = mom[0];
   for (int t = 0; t < kCoopTeam; ++t) coop_s0(tm.data(), in, t, m_top);
   for (int s = 0; s < kCoopPhases; ++s)
     for (int w = 0; w < kCoopWarps; ++w)
