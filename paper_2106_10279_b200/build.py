@@ -51,7 +51,8 @@ def build(force=False, verbose=False):
     if not force and not needs_build():
         return LIB
     generate()
-    cmd = [NVCC] + FLAGS + ["-o", LIB, os.path.join(CSRC, "madflow_b200.cu")]
+    extra = os.environ.get("MF_NVCC_EXTRA", "").split()        # e.g. -DMF_COOP_GROUP=2 (tuning experiments)
+    cmd = [NVCC] + FLAGS + extra + ["-o", LIB, os.path.join(CSRC, "madflow_b200.cu")]
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     log = os.path.join(HERE, "build.log")
     with open(log, "w") as f:

@@ -99,9 +99,36 @@ ORDERED_PAIRS = list(itertools.permutations(LABELS, 2))
 PAIR_INDEX = {p: i for i, p in enumerate(ORDERED_PAIRS)}
 SEQS = {k: [s for s in itertools.permutations(LABELS, k) if canon(s)[0] == s] for k in range(2, N + 1)}
 SEQ_INDEX = {k: {s: i for i, s in enumerate(SEQS[k])} for k in SEQS}
-Z_ROW = 17                  # row stride of the z arrays (16 polarisation words + 1 pad: spreads the writers' banks)
-Z_PLANE = 2 * 12 * 2 * Z_ROW   # doubles per re / im plane: z2[12 seqs][2 hb][Z_ROW] then z5[12 pairs][2 hb][Z_ROW]
+# z arrays: rows of 16 polarisation words, padded, and with the word's bits PERMUTED per row so that the lanes of a
+# producing round (which differ in the sequence / pair and in the polarisations of the inner gluons) store to
+# different banks: z2 row (seq = (a, b, c, d), hb): bit order (b, c, a, d), stride 18; z5 row (pair (a, d), hb),
+# b < c the other two gluons: bit order (a, b, c, d), stride 17.  The reading S4 threads of a half warp cover one
+# whole row, in any order.
+Z_ROW = 18                  # z2 row stride (also the hb stride the J4 tasks use)
+Z5_ROW = 17
 Z5_OFF = 12 * 2 * Z_ROW
+Z_PLANE = Z5_OFF + 12 * 2 * Z5_ROW   # doubles per re / im plane
+SPIN_ROW = 13               # X2 / Ytilde: rows of 12 ordered pairs, padded (bank spread for the S4 readers)
+J2_STRIDE = len([0 for _ in itertools.combinations(LABELS, 2)])   # J2 stored polarisation-major: [4][6 sequences]
+
+
+def permuted_word(order, pols):
+    """bit i of the result = polarisation of gluon order[i]"""
+    v = 0
+    for i, g in enumerate(order):
+        v |= ((pols >> g) & 1) << i
+    return v
+
+
+def z2_order(seq):
+    a, b, c, d = seq
+    return (b, c, a, d)
+
+
+def z5_order(pair):
+    a, d = pair
+    b, c = [g for g in LABELS if g not in pair]
+    return (a, b, c, d)
 
 
 def build_layout():
@@ -117,11 +144,16 @@ def build_layout():
     for g in LABELS:
         for p in range(2):
             L.add("V", ("eps", g, p))
-    for k in (2, 3):   # gluon currents, canonical sequences, family-contiguous so S4 can index them arithmetically
-        L.bases["J%d" % k] = L.n("V")
-        for s in SEQS[k]:
-            for pw in pol_words(s):
-                L.add("V", ("J", s, pw))
+    # gluon currents, canonical sequences, family-contiguous so S4 and the z5 tasks can index them arithmetically:
+    # J2 [polidx][seq] (the z5 tasks read all four variants of one sequence), J3 [seq][polidx]
+    L.bases["J2"] = L.n("V")
+    for v in range(4):
+        for s in SEQS[2]:
+            L.add("V", ("J", s, pol_words(s)[v]))
+    L.bases["J3"] = L.n("V")
+    for s in SEQS[3]:
+        for pw in pol_words(s):
+            L.add("V", ("J", s, pw))
     # fermion bilinears as pairs of real vectors (k = 0 real part, 1 imaginary part)
     L.bases["c0"] = L.n("V")
     for hb in range(2):
@@ -153,15 +185,19 @@ def build_layout():
     for a in LABELS:
         for p in range(2):
             L.add("S", ("Y1", a, p))
-    L.bases["X2"] = L.n("S")
+    L.bases["X2"] = L.n("S")       # [hb][polidx][pair, padded to SPIN_ROW]
     for hb in range(2):
-        for cd in ORDERED_PAIRS:
-            for pw in pol_words(cd):
-                L.add("S", ("X2", cd, hb, pw))
-    L.bases["Yt"] = L.n("S")
-    for ab in ORDERED_PAIRS:
-        for pw in pol_words(ab):
-            L.add("S", ("Yt", ab, pw))
+        for v in range(4):
+            for cd in ORDERED_PAIRS:
+                L.add("S", ("X2", cd, hb, pol_words(cd)[v]))
+            for i in range(SPIN_ROW - len(ORDERED_PAIRS)):
+                L.add("S", ("pad", "X2", hb, v, i))
+    L.bases["Yt"] = L.n("S")       # [polidx][pair, padded]
+    for v in range(4):
+        for ab in ORDERED_PAIRS:
+            L.add("S", ("Yt", ab, pol_words(ab)[v]))
+        for i in range(SPIN_ROW - len(ORDERED_PAIRS)):
+            L.add("S", ("pad", "Yt", v, i))
     return L
 
 
@@ -180,11 +216,11 @@ def P_ref(L, seq):
 
 
 def z2_index(seq, pols):
-    return (SEQ_INDEX[4][seq] * 2) * Z_ROW + pols       # hb = 0, k = 0; hb stride Z_ROW, k stride Z_PLANE
+    return (SEQ_INDEX[4][seq] * 2) * Z_ROW + permuted_word(z2_order(seq), pols)   # hb = 0, k = 0; hb stride Z_ROW
 
 
 def z5_index(pair, hb, pols):
-    return Z5_OFF + (PAIR_INDEX[pair] * 2 + hb) * Z_ROW + pols
+    return Z5_OFF + (PAIR_INDEX[pair] * 2 + hb) * Z5_ROW + permuted_word(z5_order(pair), pols)
 
 
 # ---- flop model of the task templates of mf_me_coop.cuh (adds + multiplies, FMA = 2; shared dot products of
@@ -299,7 +335,7 @@ def task_z5(L, ad, hb, pa, m, pd=0):
     b, c = [g for g in LABELS if g not in ad]
     pds = [0, 1] if m == 2 else [pd]
     f = [z5_index(ad, hb, (pa << a) | (x << d)) for x in pds]
-    f += [1 << b, 1 << c, L.get("S", ("Y1", a, pa))]
+    f += [2, 4, L.get("S", ("Y1", a, pa))]              # bits of pb, pc in the permuted z5 word
     f += [L.get("S", ("X1", d, hb, x)) for x in pds]
     f += [L.get("V", ("J", (b, c), 0))]
     return dict(fam="z5", M=m, fields=f, flops=m * (F_BIL + 4 * F_CDOT))
@@ -331,12 +367,13 @@ def build_rounds(L):
     add(["B"], [task_J4(L, s, pw, 2, 2) for s, pw in groups[:w]])
     add(["B"], [task_J4(L, s, pw, 1, 2, pa=pa) for s, pw in groups[w:] for pa in range(2)])
     # X2: sibling groups (pair, hb, pd)
-    groups = [(cd, hb, pd) for hb in range(2) for cd in ORDERED_PAIRS for pd in range(2)]
+    groups = [(cd, hb, pd) for hb in range(2) for pd in range(2) for cd in ORDERED_PAIRS]   # pair fastest: the lanes'
+    # spinor stores then go to consecutive items
     w = WIDE_GROUPS["X2"]
     add(["A", "B"], [task_X2(L, cd, hb, pd, 2) for cd, hb, pd in groups[:w]])
     add(["A", "B"], [task_X2(L, cd, hb, pd, 1, pc) for cd, hb, pd in groups[w:] for pc in range(2)])
     # Yt: sibling groups (pair, pa)
-    groups = [(ab, pa) for ab in ORDERED_PAIRS for pa in range(2)]
+    groups = [(ab, pa) for pa in range(2) for ab in ORDERED_PAIRS]
     w = WIDE_GROUPS["Yt"]
     add(["A", "B"], [task_Yt(L, ab, pa, 2) for ab, pa in groups[:w]])
     add(["A", "B"], [task_Yt(L, ab, pa, 1, pb) for ab, pa in groups[w:] for pb in range(2)])
@@ -410,16 +447,19 @@ def emit_s4(L):
     for m in LABELS:
         rest = [g for g in LABELS if g != m]
         w("  const int pt%d = ps%d | (ps%d << 1) | (ps%d << 2);" % (m, rest[0], rest[1], rest[2]))
-    w("  const double* Zk = Z + k * %d + hb * %d + pols;" % (Z_PLANE, Z_ROW))
+    w("  const double* Zk = Z + k * %d;" % Z_PLANE)
+
+    def word_expr(order):
+        return " | ".join("ps%d" % g if i == 0 else "(ps%d << %d)" % (g, i) for i, g in enumerate(order))
     w("  double " + ", ".join("A%d%d%d%d" % p for p in perms) + ";")
     # term 1: Ytilde(ab) . Xhat(cd); k selects the real or the imaginary part of the product
     for a, b in itertools.combinations(LABELS, 2):
         c, d = [g for g in LABELS if g not in (a, b)]
         w("  {")
         for (x, y) in ((a, b), (b, a)):
-            w("    const spin yt%d%d = coop_row_part(coop_ld_spin(S, %d + %d * 4 + %s), k);" % (x, y, L.bases["Yt"], PAIR_INDEX[(x, y)], pair_name(x, y)))
+            w("    const spin yt%d%d = coop_row_part(coop_ld_spin(S, %d + %s * %d + %d), k);" % (x, y, L.bases["Yt"], pair_name(x, y), SPIN_ROW, PAIR_INDEX[(x, y)]))
         for (x, y) in ((c, d), (d, c)):
-            w("    const spin x%d%d = coop_col_part(coop_ld_spin(S, %d + (hb * 12 + %d) * 4 + %s), k);" % (x, y, L.bases["X2"], PAIR_INDEX[(x, y)], pair_name(x, y)))
+            w("    const spin x%d%d = coop_col_part(coop_ld_spin(S, %d + (hb * 4 + %s) * %d + %d), k);" % (x, y, L.bases["X2"], pair_name(x, y), SPIN_ROW, PAIR_INDEX[(x, y)]))
         for (x, y) in ((a, b), (b, a)):
             for (u, v) in ((c, d), (d, c)):
                 w("    A%d%d%d%d = sdot_part(yt%d%d, x%d%d);" % (x, y, u, v, x, y, u, v))
@@ -434,7 +474,7 @@ def emit_s4(L):
     # term 2: z2 = c0 . J4(sigma), stored by the J4 tasks
     w("  {")
     for i, s in enumerate(SEQS[4]):
-        w("    { const double z = Zk[%d];" % (i * 2 * Z_ROW))
+        w("    { const double z = Zk[%d + hb * %d + (%s)];" % (i * 2 * Z_ROW, Z_ROW, word_expr(z2_order(s))))
         add(s, "z", 1)
         add(s[::-1], "z", (-1) ** (4 + 1))
         w("    }")
@@ -459,7 +499,7 @@ def emit_s4(L):
     # term 5: z5 = c(a, d) . J2(bc), stored by the z5 tasks
     for (a, d) in ORDERED_PAIRS:
         b, c = [g for g in LABELS if g not in (a, d)]
-        w("  { const double z = Zk[%d];" % (Z5_OFF + PAIR_INDEX[(a, d)] * 2 * Z_ROW))
+        w("  { const double z = Zk[%d + hb * %d + (%s)];" % (Z5_OFF + PAIR_INDEX[(a, d)] * 2 * Z5_ROW, Z5_ROW, word_expr(z5_order((a, d)))))
         add((a, b, c, d), "z", 1)
         add((a, c, b, d), "z", -1)
         w("  }")
@@ -590,7 +630,7 @@ def main():
            "#if !defined(__CUDACC__)", "#define __align__(n) alignas(n)", "#endif", "",
            "namespace mf {", "",
            "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | Z 2*kCoopZPlane | SCAL kCoopNX (each region 16-byte aligned)",
-           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopZRow = %d, kCoopNX = %d;" % (L.n("V"), L.n("S"), Z_PLANE, Z_ROW, L.n("X")),
+           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopZRow = %d, kCoopNX = %d, kCoopJ2Stride = %d;" % (L.n("V"), L.n("S"), Z_PLANE, Z_ROW, L.n("X"), J2_STRIDE),
            "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 2 * kCoopZPlane + kCoopNX;",
            "constexpr double kCoopCden = %.1f;" % Cden,
            "// item indices the hand-written stage S0 needs"]

@@ -155,6 +155,7 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     while (n_teams > 0 &&
            (size_t)mf::CoopSmem(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
       --n_teams;
+    n_teams -= n_teams % mf::kCoopGroup;   // teams run in lock-step groups
     if (n_teams < 1) { free_all(p); delete p; return MF_ECUDA; }
     p->threads = n_teams * mf::kCoopTeam;
     p->smem = (size_t)mf::CoopSmem(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8;

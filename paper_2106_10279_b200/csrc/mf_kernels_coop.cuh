@@ -49,9 +49,50 @@ __device__ __forceinline__ void coop_load_table(uint4* s_tab) {
   for (int i = threadIdx.x; i < kCoopTableVecs; i += blockDim.x) s_tab[i] = g[i];
 }
 
-// barrier of the two warps of one team (named barrier 1 + team; barrier 0 is __syncthreads)
-__device__ __forceinline__ void coop_team_sync(int team) {
-  asm volatile("bar.sync %0, %1;" ::"r"(team + 1), "r"(kCoopTeam) : "memory");
+// Teams are tied into groups of kCoopGroup that run the matrix-element program in lock-step (one named barrier
+// per group: 1 + group; barrier 0 is __syncthreads).  Group size 1 = every team on its own: least barrier wait,
+// but one instruction stream per team, and the program is larger than the instruction caches.
+#ifndef MF_COOP_GROUP
+#define MF_COOP_GROUP 1
+#endif
+constexpr int kCoopGroup = MF_COOP_GROUP;
+template <int G>
+__device__ __forceinline__ void coop_group_sync(int group) {
+  asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(kCoopTeam * G) : "memory");
+}
+
+// The teams' share of a round: team t of group g works through ranks g G + t, g G + t + n_teams, ... of the queue;
+// the G teams of a group step together (a team whose rank is beyond `total` only keeps the barriers).
+template <int G>
+__device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const uint4* tab, double* s_res,
+                                               const double* queue, int total, double mt) {
+  const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam, warp = tid >> 5, lane = tid & 31;
+  const int group = team / G;
+  double* tm = teams + team * kCoopTeamDoubles;
+  double* in = tm + kCoopOffIn;
+  double nxt = 0.0;
+  if (team < total && tid < 18) nxt = queue[team * kCoopQueueDoubles + tid];
+#pragma unroll 1
+  for (int r0 = group * G; r0 < total; r0 += n_teams) {
+    const int r = r0 + (team - group * G);
+    const bool active = r < total;
+    if (tid < 18) in[tid] = nxt;
+    coop_group_sync<G>(group);
+    if (r + n_teams < total && tid < 18) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // used next turn
+    if (active) coop_s0(tm, in, tid, mt);
+    coop_group_sync<G>(group);
+#define MF_R(OFF, ...) if (active) coop_run_task<__VA_ARGS__>(tm, tab, OFF, lane, mt);
+#define MF_S() coop_group_sync<G>(group);
+    if (warp == 0) { MF_COOP_WARP0(MF_R, MF_S) } else { MF_COOP_WARP1(MF_R, MF_S) }
+#undef MF_R
+#undef MF_S
+    if (active) {
+      double acc = coop_s4_thread(tm, tid);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+      if (lane == 0) s_res[2 * r + warp] = acc;
+    }
+  }
 }
 
 // |M|^2 (with couplings and averaging) of this thread's own event.  EVERY thread of the block must call it (it
@@ -59,6 +100,7 @@ __device__ __forceinline__ void coop_team_sync(int team) {
 // warps) and queued; team t computes ranks t, t + n_teams, ...  `queue` holds blockDim.x entries (global memory
 // in the fused pass, shared memory in the debug kernels), s_res 2 doubles per thread of the block, s_cnt 2 x 32
 // unsigned (double-buffered by `round`).  Returns 0 for threads whose event did not pass.
+template <int G>
 __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, const uint4* tab, unsigned* s_cnt,
                                                  double* s_res, double* queue, unsigned round, bool pass,
                                                  const double (*k)[4], double shat, const Params& P) {
@@ -84,30 +126,7 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
     q[17] = 0.5 * sqrt(shat);
   }
   __syncthreads();
-  {
-    const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam, warp = tid >> 5;
-    double* tm = teams + team * kCoopTeamDoubles;
-    double* in = tm + kCoopOffIn;
-    double nxt = 0.0;
-    if (team < total && tid < 18) nxt = queue[team * kCoopQueueDoubles + tid];
-#pragma unroll 1
-    for (int r = team; r < total; r += n_teams) {
-      if (tid < 18) in[tid] = nxt;
-      coop_team_sync(team);
-      if (r + n_teams < total && tid < 18) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // used next turn
-      coop_s0(tm, in, tid, P.m_top);
-      coop_team_sync(team);
-#define MF_R(OFF, ...) coop_run_task<__VA_ARGS__>(tm, tab, OFF, lane, P.m_top);
-#define MF_S() coop_team_sync(team);
-      if (warp == 0) { MF_COOP_WARP0(MF_R, MF_S) } else { MF_COOP_WARP1(MF_R, MF_S) }
-#undef MF_R
-#undef MF_S
-      double acc = coop_s4_thread(tm, tid);
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
-      if (lane == 0) s_res[2 * r + warp] = acc;
-    }
-  }
+  coop_team_loop<G>(teams, n_teams, tab, s_res, queue, total, P.m_top);   // n_teams is a multiple of G
   __syncthreads();
   // top spin state 0 only: the other one gives the same sum (spin-flip symmetry), hence the factor 2
   return pass ? (s_res[2 * rank] + s_res[2 * rank + 1]) * (2.0 * P.me_norm / kCoopCden) : 0.0;
@@ -155,7 +174,7 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
       if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
     }
     const bool pass = valid && ev.pass;
-    const double me2 = coop_block_me2(s_teams, n_teams, s_tab, s_cnt, s_res, queue, (unsigned)rd, pass, ev.k, ev.shat, P);
+    const double me2 = coop_block_me2<kCoopGroup>(s_teams, n_teams, s_tab, s_cnt, s_res, queue, (unsigned)rd, pass, ev.k, ev.shat, P);
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
@@ -190,7 +209,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
     generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
   }
   const bool pass = valid && ev.pass;
-  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, s_res, queue, 0u, pass, ev.k, ev.shat, P);
+  const double me2 = coop_block_me2<1>(tm, 1, s_tab, s_cnt, s_res, queue, 0u, pass, ev.k, ev.shat, P);
   if (!valid) return;
   double mom[NF + 2][4];
   lab_momenta<PROC>(ev, mom);
@@ -228,7 +247,7 @@ __global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params 
       for (int c = 0; c < 4; ++c) k[f][c] = m[(2 + f) * 4 + c];
     shat = 4.0 * m[0] * m[0];
   }
-  const double me2 = coop_block_me2(tm, 1, s_tab, s_cnt, s_res, queue, 0u, valid, k, shat, P);
+  const double me2 = coop_block_me2<1>(tm, 1, s_tab, s_cnt, s_res, queue, 0u, valid, k, shat, P);
   if (valid) out[i] = me2;
 }
 

@@ -315,7 +315,7 @@ template <int M> struct CoopTaskYt {
 };
 
 // z5 = [Y1(a) gamma X1(d)] . J2(bc) for the 4 polarisations of (b, c) and M polarisations of d
-// [out x M, 1 << b, 1 << c, Y1, X1 x M, J2bc (4 consecutive variants)]
+// [out x M, bit of pb, bit of pc in the z5 word, Y1, X1 x M, J2bc (variant 0; variants kCoopJ2Stride apart)]
 template <int M> struct CoopTaskZ5 {
   static constexpr int NF = 2 * M + 4, NVEC = (NF + 7) / 8;
   MF_HD static void run(double* scr, const CoopFields<NVEC>& F, double) {
@@ -329,7 +329,7 @@ template <int M> struct CoopTaskZ5 {
     for (int m = 0; m < M; ++m) c[m] = bilinear(y, coop_ld_spin(S, coop_fld(F, M + 3 + m)));
 #pragma unroll
     for (int p = 0; p < 4; ++p) {
-      const rvec j = coop_ld_vec(V, j2 + p);
+      const rvec j = coop_ld_vec(V, j2 + p * kCoopJ2Stride);
       const int off = (p & 1) * ob + (p >> 1) * oc;
 #pragma unroll
       for (int m = 0; m < M; ++m) {
