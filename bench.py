@@ -42,9 +42,10 @@ def me_flops(process):
     if process == 0:
         return 2500.0
     csrc = os.path.join(ROOT, "paper_2106_10279_b200", "csrc")
-    if process == 3:    # the cooperative program (csrc/gen_coop.py) is what the fused pass runs for gg -> ttbar gg
-        txt = open(os.path.join(csrc, "mf_me_ttgg_coop_generated.cuh")).read()
-        return float(re.search(r"kFlopsMe2Coop_2g = ([0-9.]+);", txt).group(1))
+    if process >= 2:    # the cooperative programs (csrc/gen_coop.py, gen_coop3.py) are what the fused pass runs
+        name = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g")}[process]
+        txt = open(os.path.join(csrc, name[0])).read()
+        return float(re.search(name[1] + r" = ([0-9.]+);", txt).group(1))
     txt = open(os.path.join(csrc, "mf_me_ggtt_generated.cuh")).read()
     return float(re.search(r"kFlopsMe2_%dg = ([0-9.]+);" % (process - 1), txt).group(1))
 
@@ -312,7 +313,7 @@ def main():
         "n_accept_last_step": last.n_accept,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": ("fused_pass_coop_kernel<true>" if wl.process == 3 else "fused_pass_kernel<%d,true>" % wl.process), "kernel_ms": kern,
+                     "traffic": None, "kernel": ("fused_pass_coop_kernel<%d,true>" if wl.process >= 2 else "fused_pass_kernel<%d,true>") % wl.process, "kernel_ms": kern,
                      "flops_per_me": me_flops(wl.process), "peak_source": "mf_measure_fp64_peak (DFMA chains) on this GPU",
                      "nominal_peak": NOMINAL_FP64 / 1e12, "frac_of_nominal": achieved / (NOMINAL_FP64 / 1e12)},
     }

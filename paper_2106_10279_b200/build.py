@@ -3,7 +3,7 @@ sm_100a.  No GPU is needed to build (nvcc cross-compiles).
 
     python -m paper_2106_10279_b200.build [--force] [--verbose]
 
-Steps: (1) csrc/gen_me.py and csrc/gen_coop.py write the straight-line matrix-element code (the role of the paper's exporter
+Steps: (1) csrc/gen_me.py, csrc/gen_coop.py and csrc/gen_coop3.py write the straight-line matrix-element code (the role of the paper's exporter
 plugin); (2) nvcc compiles csrc/madflow_b200.cu into the shared library.
 """
 import glob
@@ -21,7 +21,7 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
 
 
 def _sources():
-    return (glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh")) +
+    return (glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.inc")) +
             glob.glob(os.path.join(CSRC, "*.py")) + [os.path.join(os.path.dirname(HERE), "include", "mf.h")])
 
 
@@ -31,7 +31,7 @@ def generate():
     out = []
     if CSRC not in sys.path:
         sys.path.insert(0, CSRC)          # gen_coop imports gen_me
-    for name in ("gen_me", "gen_coop"):
+    for name in ("gen_me", "gen_coop", "gen_coop3"):
         spec = importlib.util.spec_from_file_location(name, os.path.join(CSRC, name + ".py"))
         mod = importlib.util.module_from_spec(spec)
         sys.modules[name] = mod

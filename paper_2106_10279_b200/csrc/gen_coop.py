@@ -601,7 +601,7 @@ def emit_tables(L, rounds):
     for wi, prog in enumerate(progs):
         cost = "/".join(str(load[(p, wi)]) for p in PHASES)
         w("// warp %d: ~%s flop/lane per phase" % (wi, cost))
-        w("#define MF_COOP_WARP%d(R, S) \\" % wi)
+        w("#define MF_COOP4_WARP%d(R, S) \\" % wi)
         w("  " + " \\\n  ".join(prog))
     assert max(words) < 32768 and min(words) >= -1 and len(words) % 8 == 0
     w("// operand indices: vector (offset + v * 32 + lane) holds fields 8 v .. 8 v + 7 of the lane's task")
@@ -624,11 +624,8 @@ def main():
     total = s0_flops + staged + 64 * s4_flops
     hdr = ["// GENERATED by gen_coop.py — do not edit.  Cooperative (64 threads per event) matrix element of",
            "// g g -> t tbar g g: scratch layout, task tables of phases S1 / A / B, straight-line stage S4.",
-           "#pragma once", '#include "mf_me_prims.cuh"', "",
-           "#if defined(__CUDA_ARCH__)", "#define MF_TABLE static __device__ const", "#define MF_CONST static __constant__ const",
-           "#else", "#define MF_TABLE static const", "#define MF_CONST static const", "#endif",
-           "#if !defined(__CUDACC__)", "#define __align__(n) alignas(n)", "#endif", "",
-           "namespace mf {", "",
+           "// A FRAGMENT: included by mf_me_coop.cuh inside namespace mf::g4 (no include guard, no namespace of its own).",
+           "",
            "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | Z 2*kCoopZPlane | SCAL kCoopNX (each region 16-byte aligned)",
            "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopZRow = %d, kCoopNX = %d, kCoopJ2Stride = %d;" % (L.n("V"), L.n("S"), Z_PLANE, Z_ROW, L.n("X"), J2_STRIDE),
            "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 2 * kCoopZPlane + kCoopNX;",
@@ -650,14 +647,15 @@ def main():
         if ("qY", m) in L.idx["V"]:
             s0.append((2, m, L.get("V", ("qY", m)), L.get("X", ("idY", m))))
     assert len(s0) <= 32
-    hdr.append("constexpr int kCoopS0Lanes = %d;" % len(s0))
+    hdr.append("constexpr int kCoopS0Lanes = %d, kCoopS0Spin0 = 30, kCoopS0Pol0 = 32, kCoopS0Beam0 = 36;   // S0 lane assignment" % len(s0))
+    hdr.append("constexpr int kCoopNGF = 2, kCoopPolBits = 4;     // final-state gluons; polarisation bits of an S4 thread")
     hdr.append("MF_TABLE short kCoopS0Tab[%d][4] = {%s};   // kind, mask, vec, x" %
                (len(s0), ", ".join("{%d, %d, %d, %d}" % t for t in s0)))
     hdr.append("// static fp64 operation count per event (adds + multiplies, FMA = 2): S0 %d + S1/A/B %d + 64 x S4 %d" %
                (s0_flops, staged, s4_flops))
     hdr.append("constexpr double kFlopsMe2Coop_2g = %d.0;" % total)
     hdr.append("")
-    text = "\n".join(hdr) + "\n" + LOADERS + "\n" + tables + "\n\n" + s4 + "\n\n}  // namespace mf\n"
+    text = "\n".join(hdr) + "\n" + LOADERS + "\n" + tables + "\n\n" + s4 + "\n"
     path = os.path.join(HERE, "mf_me_ttgg_coop_generated.cuh")
     old = open(path).read() if os.path.exists(path) else None
     if old != text:

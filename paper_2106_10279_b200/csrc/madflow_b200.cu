@@ -44,9 +44,33 @@ const void* pass_fn(int proc, bool unw) {
   switch (proc) {
     case 0: return unw ? pass_fn<0, true>() : pass_fn<0, false>();
     case 1: return unw ? pass_fn<1, true>() : pass_fn<1, false>();
-    case 2: return unw ? pass_fn<2, true>() : pass_fn<2, false>();
-    default: return unw ? (const void*)mf::fused_pass_coop_kernel<true> : (const void*)mf::fused_pass_coop_kernel<false>;
+    case 2: return unw ? (const void*)mf::fused_pass_coop_kernel<2, true> : (const void*)mf::fused_pass_coop_kernel<2, false>;
+    default: return unw ? (const void*)mf::fused_pass_coop_kernel<3, true> : (const void*)mf::fused_pass_coop_kernel<3, false>;
   }
+}
+
+// launch shape, shared-memory sizes and kernel attributes of the cooperative pass of process PROC
+template <int PROC>
+cudaError_t coop_setup(mf_process* p, const cudaDeviceProp& prop) {
+  typedef typename mf::CoopOf<PROC>::PG PG;
+  const mf::Params& P = p->P;
+  const int group = PG::Team == 32 ? 1 : mf::kCoopGroup;      // teams run in lock-step groups
+  int n_teams = mf::CoopOf<PROC>::MaxTeams;
+  while (n_teams > 0 &&
+         (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
+    --n_teams;
+  n_teams -= n_teams % group;
+  if (n_teams < 1) return cudaErrorInvalidConfiguration;
+  p->threads = n_teams * PG::Team;
+  p->smem = (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8;
+  cudaError_t e;
+  for (int u = 0; u < 2; ++u)
+    if ((e = cudaFuncSetAttribute(pass_fn(PROC, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem)) !=
+        cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute((const void*)mf::debug_eval_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                mf::coop_debug_smem_bytes<PG>())) != cudaSuccess) return e;
+  return cudaFuncSetAttribute((const void*)mf::debug_me2_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              mf::coop_debug_smem_bytes<PG>());
 }
 
 void free_all(mf_process* p) {
@@ -149,23 +173,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   int dev = 0;
   cudaGetDevice(&dev);
   if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
-  if (p->process == 3) {
-    // cooperative pass: as many 64-thread teams per block as the SM's shared memory holds, one block per SM
-    int n_teams = mf::kCoopMaxTeams;
-    while (n_teams > 0 &&
-           (size_t)mf::CoopSmem(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
-      --n_teams;
-    n_teams -= n_teams % mf::kCoopGroup;   // teams run in lock-step groups
-    if (n_teams < 1) { free_all(p); delete p; return MF_ECUDA; }
-    p->threads = n_teams * mf::kCoopTeam;
-    p->smem = (size_t)mf::CoopSmem(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8;
-    for (int u = 0; u < 2; ++u)
-      if ((e = cudaFuncSetAttribute(pass_fn(3, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem)) !=
-          cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
-    if ((e = cudaFuncSetAttribute((const void*)mf::debug_eval_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  mf::kCoopDebugSmemBytes)) != cudaSuccess ||
-        (e = cudaFuncSetAttribute((const void*)mf::debug_me2_coop_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  mf::kCoopDebugSmemBytes)) != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
+  if (p->process >= 2) {
+    // cooperative pass: as many teams per block as the SM's shared memory holds, one block per SM
+    e = p->process == 3 ? coop_setup<3>(p, prop) : coop_setup<2>(p, prop);
+    if (e != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   } else {
     p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + 2 * P.pdf_nx + 5 * 32) * sizeof(double);
   }
@@ -181,7 +192,7 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
       (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
-  if (p->process == 3 &&
+  if (p->process >= 2 &&
       (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads * mf::kCoopQueueDoubles * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
@@ -252,10 +263,13 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
   switch (p->process) {
     case 0: mf::debug_eval_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 1: mf::debug_eval_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
-    case 2: mf::debug_eval_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    case 2:
+      mf::debug_eval_coop_kernel<2><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
+                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, A, d_out);
+      break;
     default:
-      mf::debug_eval_coop_kernel<<<(unsigned)((n_events + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
-                                   mf::kCoopDebugSmemBytes, st>>>(p->P, A, d_out);
+      mf::debug_eval_coop_kernel<3><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
+                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g4::Prog>(), st>>>(p->P, A, d_out);
       break;
   }
   cudaError_t e = cudaGetLastError();
@@ -294,10 +308,13 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
   switch (p->process) {
     case 0: mf::debug_me2_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 1: mf::debug_me2_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
-    case 2: mf::debug_me2_kernel<2><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    case 2:
+      mf::debug_me2_coop_kernel<2><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
+                                     mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, d_mom, n, d_out);
+      break;
     default:
-      mf::debug_me2_coop_kernel<<<(unsigned)((n + mf::kCoopTeam - 1) / mf::kCoopTeam), mf::kCoopTeam,
-                                  mf::kCoopDebugSmemBytes, st>>>(p->P, d_mom, n, d_out);
+      mf::debug_me2_coop_kernel<3><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
+                                     mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g4::Prog>(), st>>>(p->P, d_mom, n, d_out);
       break;
   }
   cudaError_t e = cudaGetLastError();

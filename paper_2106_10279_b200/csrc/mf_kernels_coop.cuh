@@ -1,27 +1,31 @@
-// mf_kernels_coop.cuh — the fused pass for g g -> t tbar g g (BASELINE.json configs[3], [4]): steps a1-a6 and
-// a10-a14 one thread per event exactly as in mf_kernels.cuh, steps a7-a9 (the matrix element, >99 % of the
-// arithmetic) by teams of 64 threads per event over a shared-memory scratch
-// (mf_me_coop.cuh).
+// mf_kernels_coop.cuh — the fused pass for g g -> t tbar g and g g -> t tbar g g (BASELINE.json configs[2..4]):
+// steps a1-a6 and a10-a14 one thread per event exactly as in mf_kernels.cuh, steps a7-a9 (the matrix element,
+// >95 % of the arithmetic) by TEAMS of threads per event over a shared-memory scratch
+// (mf_me_coop.cuh): 64 threads (2 warps) for g g -> t tbar g g, 32 threads (1 warp) for g g -> t tbar g.
 //
-// Block = T teams of 64 threads (T = 6 for 50 bins: 6 x 30.8 kB of scratch + operand table + grid + histogram +
-// PDF row fill the 227 kB of one SM; one block per SM, 12 warps = 3 per scheduler, <= 168 registers).  Per round
-// every thread generates its own event; the events of the block that passed the cuts are ranked and their
-// momenta queued (a per-block slice of a small L2-resident buffer); team t then works through ranks t, t + T, ...
-// on its own, synchronising only its two warps (named barriers), and leaves |M|^2 in a per-rank result slot that
-// the owner reads after the round's closing block barrier.  Teams therefore sit in different stages of the
-// program at any time, so the latency-bound stages of one team (S0, barriers, table fetches) overlap the
-// FP64-bound stages of the others.
+// Block = T teams (g g -> t tbar g g: T = 6, 6 x 31.6 kB of scratch + operand table + grid + histogram + PDF row
+// fill the 227 kB of one SM; 12 warps = 3 per scheduler, <= 168 registers.  g g -> t tbar g: T = 16 warps).
+// Per round every thread generates its own event; the events of the block that passed the cuts are ranked and
+// their momenta queued (a per-block slice of a small L2-resident buffer); team t then works through ranks t,
+// t + T, ... on its own, synchronising only its own warps (named barriers / __syncwarp), and leaves |M|^2 in a
+// per-rank result slot that the owner reads after the round's closing block barrier.  Teams therefore sit in
+// different stages of the program at any time, so the latency-bound stages of one team (S0, barriers, table
+// fetches) overlap the FP64-bound stages of the others.
 #pragma once
 #include "mf_kernels.cuh"
 #include "mf_me_coop.cuh"
 
 namespace mf {
 
-constexpr int kCoopMaxTeams = 6;
+// the cooperative program of a process and its launch shape
+template <int PROC> struct CoopOf { typedef g4::Prog PG; static constexpr int MaxTeams = 6; };   // PROC = 3
+template <> struct CoopOf<2> { typedef g3::Prog PG; static constexpr int MaxTeams = 16; };
 
-constexpr int kCoopQueueDoubles = kCoopInDoubles;   // queue entry: k[4][4], shat, pad
+constexpr int kCoopQueueDoubles = 18;   // queue entry: k[NF][4] (zero padded to 16), shat, sqrt(shat) / 2
+static_assert(g4::Prog::InDoubles == kCoopQueueDoubles && g3::Prog::InDoubles == kCoopQueueDoubles, "queue entry");
 
 // shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
+template <class PG>
 struct CoopSmem {
   int grid, hist, lnx, row, red, cnt, res, tab, teams, total;
   __host__ __device__ CoopSmem(int D, int nb, int nx, int n_teams) {
@@ -33,64 +37,68 @@ struct CoopSmem {
     red = row + even(nx);
     cnt = red + 5 * 32;
     res = cnt + 32;
-    tab = res + 2 * n_teams * kCoopTeam;
-    teams = tab + 2 * kCoopTableVecs;
-    total = teams + n_teams * kCoopTeamDoubles;
+    tab = res + PG::Warps * n_teams * PG::Team;
+    teams = tab + 2 * PG::TableVecs;
+    total = teams + n_teams * PG::TeamDoubles;
   }
 };
 
-// shared memory of the single-team debug kernels: team | rank counters | results | queue | operand table
-constexpr int kCoopDebugSmemBytes =
-    (kCoopTeamDoubles + 32 + 2 * kCoopTeam + kCoopTeam * kCoopQueueDoubles + 2 * kCoopTableVecs) * 8;
-
-// copies the operand table into shared memory (all threads of the block; the caller synchronises)
-__device__ __forceinline__ void coop_load_table(uint4* s_tab) {
-  const uint4* g = reinterpret_cast<const uint4*>(kCoopTable);
-  for (int i = threadIdx.x; i < kCoopTableVecs; i += blockDim.x) s_tab[i] = g[i];
+// the debug kernels run 64 threads per block (one or two teams)
+constexpr int kCoopDebugThreads = 64;
+// their shared memory: teams | rank counters | results | queue | operand table
+template <class PG>
+constexpr int coop_debug_smem_bytes() {
+  return ((kCoopDebugThreads / PG::Team) * PG::TeamDoubles + 32 + PG::Warps * kCoopDebugThreads +
+          kCoopDebugThreads * kCoopQueueDoubles + 2 * PG::TableVecs) * 8;
 }
 
-// Teams are tied into groups of kCoopGroup that run the matrix-element program in lock-step (one named barrier
-// per group: 1 + group; barrier 0 is __syncthreads).  Group size 1 = every team on its own: least barrier wait,
-// but one instruction stream per team, and the program is larger than the instruction caches.
+// copies the operand table into shared memory (all threads of the block; the caller synchronises)
+template <class PG>
+__device__ __forceinline__ void coop_load_table(uint4* s_tab) {
+  const uint4* g = reinterpret_cast<const uint4*>(PG::table());
+  for (int i = threadIdx.x; i < PG::TableVecs; i += blockDim.x) s_tab[i] = g[i];
+}
+
+// Teams are tied into groups of G that run the matrix-element program in lock-step (one named barrier per group:
+// 1 + group; barrier 0 is __syncthreads).  G = 1 = every team on its own: least barrier wait, one instruction
+// stream per team (measured best on B200 within noise of G = 2).  One-warp teams need only __syncwarp.
 #ifndef MF_COOP_GROUP
 #define MF_COOP_GROUP 1
 #endif
 constexpr int kCoopGroup = MF_COOP_GROUP;
-template <int G>
+template <int THREADS>
 __device__ __forceinline__ void coop_group_sync(int group) {
-  asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(kCoopTeam * G) : "memory");
+  if (THREADS == 32) __syncwarp();
+  else asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(THREADS) : "memory");
 }
 
 // The teams' share of a round: team t of group g works through ranks g G + t, g G + t + n_teams, ... of the queue;
 // the G teams of a group step together (a team whose rank is beyond `total` only keeps the barriers).
-template <int G>
+template <class PG, int G>
 __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const uint4* tab, double* s_res,
                                                const double* queue, int total, double mt) {
-  const int team = threadIdx.x / kCoopTeam, tid = threadIdx.x % kCoopTeam, warp = tid >> 5, lane = tid & 31;
+  const int team = threadIdx.x / PG::Team, tid = threadIdx.x % PG::Team, warp = tid >> 5, lane = tid & 31;
   const int group = team / G;
-  double* tm = teams + team * kCoopTeamDoubles;
-  double* in = tm + kCoopOffIn;
+  double* tm = teams + team * PG::TeamDoubles;
+  double* in = tm + PG::OffIn;
+  auto sync = [group]() { coop_group_sync<PG::Team * G>(group); };
   double nxt = 0.0;
-  if (team < total && tid < 18) nxt = queue[team * kCoopQueueDoubles + tid];
+  if (team < total && tid < kCoopQueueDoubles) nxt = queue[team * kCoopQueueDoubles + tid];
 #pragma unroll 1
   for (int r0 = group * G; r0 < total; r0 += n_teams) {
     const int r = r0 + (team - group * G);
     const bool active = r < total;
-    if (tid < 18) in[tid] = nxt;
-    coop_group_sync<G>(group);
-    if (r + n_teams < total && tid < 18) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // used next turn
-    if (active) coop_s0(tm, in, tid, mt);
-    coop_group_sync<G>(group);
-#define MF_R(OFF, ...) if (active) coop_run_task<__VA_ARGS__>(tm, tab, OFF, lane, mt);
-#define MF_S() coop_group_sync<G>(group);
-    if (warp == 0) { MF_COOP_WARP0(MF_R, MF_S) } else { MF_COOP_WARP1(MF_R, MF_S) }
-#undef MF_R
-#undef MF_S
+    if (tid < kCoopQueueDoubles) in[tid] = nxt;
+    sync();
+    if (r + n_teams < total && tid < kCoopQueueDoubles) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // next turn
+    if (active) PG::s0(tm, in, tid, mt);
+    sync();
+    PG::run(tm, tab, warp, lane, mt, active, sync);
     if (active) {
-      double acc = coop_s4_thread(tm, tid);
+      double acc = PG::s4_thread(tm, tid);
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
-      if (lane == 0) s_res[2 * r + warp] = acc;
+      if (lane == 0) s_res[PG::Warps * r + warp] = acc;
     }
   }
 }
@@ -98,9 +106,10 @@ __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const
 // |M|^2 (with couplings and averaging) of this thread's own event.  EVERY thread of the block must call it (it
 // contains block barriers).  The events of the block that passed the cuts are ranked (ballot + prefix over the
 // warps) and queued; team t computes ranks t, t + n_teams, ...  `queue` holds blockDim.x entries (global memory
-// in the fused pass, shared memory in the debug kernels), s_res 2 doubles per thread of the block, s_cnt 2 x 32
-// unsigned (double-buffered by `round`).  Returns 0 for threads whose event did not pass.
-template <int G>
+// in the fused pass, shared memory in the debug kernels), s_res PG::Warps doubles per thread of the block, s_cnt
+// 2 x 32 unsigned (double-buffered by `round`).  k = the NF final-state momenta.  Returns 0 for threads whose event
+// did not pass.
+template <class PG, int G>
 __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, const uint4* tab, unsigned* s_cnt,
                                                  double* s_res, double* queue, unsigned round, bool pass,
                                                  const double (*k)[4], double shat, const Params& P) {
@@ -121,25 +130,33 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
 #pragma unroll
     for (int f = 0; f < 4; ++f)
 #pragma unroll
-      for (int c = 0; c < 4; ++c) q[4 * f + c] = k[f][c];
+      for (int c = 0; c < 4; ++c) q[4 * f + c] = f < PG::NFinal ? k[f < PG::NFinal ? f : 0][c] : 0.0;
     q[16] = shat;
     q[17] = 0.5 * sqrt(shat);
   }
   __syncthreads();
-  coop_team_loop<G>(teams, n_teams, tab, s_res, queue, total, P.m_top);   // n_teams is a multiple of G
+  coop_team_loop<PG, G>(teams, n_teams, tab, s_res, queue, total, P.m_top);   // n_teams is a multiple of G
   __syncthreads();
   // top spin state 0 only: the other one gives the same sum (spin-flip symmetry), hence the factor 2
-  return pass ? (s_res[2 * rank] + s_res[2 * rank + 1]) * (2.0 * P.me_norm / kCoopCden) : 0.0;
+  double sum = 0.0;
+  if (pass) {
+#pragma unroll
+    for (int w = 0; w < PG::Warps; ++w) sum += s_res[PG::Warps * rank + w];
+  }
+  return sum * (2.0 * P.me_norm / PG::Cden);
 }
 
-template <bool UNW>
-__global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_kernel(const Params P, const PassArgs A) {
-  constexpr int PROC = 3, D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+template <int PROC, bool UNW>
+__global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Team, 1)
+    fused_pass_coop_kernel(const Params P, const PassArgs A) {
+  typedef typename CoopOf<PROC>::PG PG;
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  constexpr int G = PG::Team == 32 ? 1 : kCoopGroup;
   extern __shared__ double2 smem2[];
   double* smem = reinterpret_cast<double*>(smem2);
   const int nb = P.n_bins, nx = P.pdf_nx;
-  const int n_teams = blockDim.x / kCoopTeam;
-  const CoopSmem L(D, nb, nx, n_teams);
+  const int n_teams = blockDim.x / PG::Team;
+  const CoopSmem<PG> L(D, nb, nx, n_teams);
   double* s_grid = smem + L.grid;
   double* s_hist = smem + L.hist;
   double* s_lnx = smem + L.lnx;
@@ -150,7 +167,7 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
   double* s_teams = smem + L.teams;
   uint4* s_tab = reinterpret_cast<uint4*>(smem + L.tab);
   double* queue = A.coop_queue + (size_t)blockIdx.x * blockDim.x * kCoopQueueDoubles;
-  coop_load_table(s_tab);
+  coop_load_table<PG>(s_tab);
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
   for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
@@ -174,7 +191,8 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
       if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
     }
     const bool pass = valid && ev.pass;
-    const double me2 = coop_block_me2<kCoopGroup>(s_teams, n_teams, s_tab, s_cnt, s_res, queue, (unsigned)rd, pass, ev.k, ev.shat, P);
+    const double me2 =
+        coop_block_me2<PG, G>(s_teams, n_teams, s_tab, s_cnt, s_res, queue, (unsigned)rd, pass, ev.k, ev.shat, P);
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
@@ -185,16 +203,30 @@ __global__ void __launch_bounds__(kCoopMaxTeams * kCoopTeam, 1) fused_pass_coop_
   block_finish(A, acc, s_red, s_hist, D * nb);
 }
 
-// Per-event dump for g g -> t tbar g g through the same team program: block = one team, thread = event.
-__global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params P, const PassArgs A, double* out) {
-  constexpr int PROC = 3, D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+// carve-up of the debug kernels' shared memory
+template <class PG>
+struct CoopDebugSmem {
+  double *teams, *s_res, *queue;
+  unsigned* s_cnt;
+  uint4* s_tab;
+  __device__ explicit CoopDebugSmem(double* base) {
+    constexpr int n_teams = kCoopDebugThreads / PG::Team;
+    teams = base;
+    s_cnt = reinterpret_cast<unsigned*>(base + n_teams * PG::TeamDoubles);
+    s_res = base + n_teams * PG::TeamDoubles + 32;
+    queue = s_res + PG::Warps * kCoopDebugThreads;
+    s_tab = reinterpret_cast<uint4*>(queue + kCoopDebugThreads * kCoopQueueDoubles);
+  }
+};
+
+// Per-event dump through the same team program: block = 64 threads (one or two teams), thread = event.
+template <int PROC>
+__global__ void __launch_bounds__(kCoopDebugThreads) debug_eval_coop_kernel(const Params P, const PassArgs A, double* out) {
+  typedef typename CoopOf<PROC>::PG PG;
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   extern __shared__ double2 smem2[];
-  double* tm = reinterpret_cast<double*>(smem2);
-  unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
-  double* s_res = tm + kCoopTeamDoubles + 32;
-  double* queue = s_res + 2 * kCoopTeam;
-  uint4* s_tab = reinterpret_cast<uint4*>(queue + kCoopTeam * kCoopQueueDoubles);
-  coop_load_table(s_tab);
+  const CoopDebugSmem<PG> L(reinterpret_cast<double*>(smem2));
+  coop_load_table<PG>(L.s_tab);
   __syncthreads();
   const int row_len = 3 * D + 4 * (NF + 2) + 9;
   const uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -209,7 +241,8 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
     generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
   }
   const bool pass = valid && ev.pass;
-  const double me2 = coop_block_me2<1>(tm, 1, s_tab, s_cnt, s_res, queue, 0u, pass, ev.k, ev.shat, P);
+  const double me2 = coop_block_me2<PG, 1>(L.teams, kCoopDebugThreads / PG::Team, L.s_tab, L.s_cnt, L.s_res, L.queue, 0u,
+                                           pass, ev.k, ev.shat, P);
   if (!valid) return;
   double mom[NF + 2][4];
   lab_momenta<PROC>(ev, mom);
@@ -226,28 +259,28 @@ __global__ void __launch_bounds__(kCoopTeam) debug_eval_coop_kernel(const Params
   q[8] = accept_draw(A.seed, A.iteration, event);
 }
 
-// |M|^2 at caller-supplied CM-frame momenta mom[n][6][4] (beams first): block = one team, thread = event.
-__global__ void __launch_bounds__(kCoopTeam) debug_me2_coop_kernel(const Params P, const double* mom, uint64_t n,
-                                                                    double* out) {
+// |M|^2 at caller-supplied CM-frame momenta mom[n][NF + 2][4] (beams first): block = 64 threads, thread = event.
+template <int PROC>
+__global__ void __launch_bounds__(kCoopDebugThreads) debug_me2_coop_kernel(const Params P, const double* mom, uint64_t n,
+                                                                           double* out) {
+  typedef typename CoopOf<PROC>::PG PG;
+  constexpr int NF = Traits<PROC>::NF;
   extern __shared__ double2 smem2[];
-  double* tm = reinterpret_cast<double*>(smem2);
-  unsigned* s_cnt = reinterpret_cast<unsigned*>(tm + kCoopTeamDoubles);
-  double* s_res = tm + kCoopTeamDoubles + 32;
-  double* queue = s_res + 2 * kCoopTeam;
-  uint4* s_tab = reinterpret_cast<uint4*>(queue + kCoopTeam * kCoopQueueDoubles);
-  coop_load_table(s_tab);
+  const CoopDebugSmem<PG> L(reinterpret_cast<double*>(smem2));
+  coop_load_table<PG>(L.s_tab);
   __syncthreads();
   const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = i < n;
-  double k[4][4];
+  double k[NF][4];
   double shat = 0.0;
   if (valid) {
-    const double* m = mom + i * 24;
-    for (int f = 0; f < 4; ++f)
+    const double* m = mom + i * (NF + 2) * 4;
+    for (int f = 0; f < NF; ++f)
       for (int c = 0; c < 4; ++c) k[f][c] = m[(2 + f) * 4 + c];
     shat = 4.0 * m[0] * m[0];
   }
-  const double me2 = coop_block_me2<1>(tm, 1, s_tab, s_cnt, s_res, queue, 0u, valid, k, shat, P);
+  const double me2 = coop_block_me2<PG, 1>(L.teams, kCoopDebugThreads / PG::Team, L.s_tab, L.s_cnt, L.s_res, L.queue, 0u,
+                                           valid, k, shat, P);
   if (valid) out[i] = me2;
 }
 

@@ -8,6 +8,24 @@
 
 using namespace mf;
 
+// PG = mf::g4::Prog / mf::g3::Prog; mom[(n+2)][4] beams first; norm = couplings / averaging (top spin 0 only is
+// evaluated and doubled: spin-flip symmetry)
+template <class PG>
+static double coop_host_me2(const double* mom, double m_top, double norm) {
+  std::vector<double> tm(PG::TeamDoubles, 0.0);
+  double* in = tm.data() + PG::OffIn;
+  for (int i = 0; i < PG::NFinal; ++i) for (int m = 0; m < 4; ++m) in[4 * i + m] = mom[(2 + i) * 4 + m];
+  in[16] = 4.0 * mom[0] * mom[0];
+  in[17] = mom[0];
+  for (int t = 0; t < PG::Team; ++t) PG::s0(tm.data(), in, t, m_top);
+  for (int s = 0; s < PG::Phases; ++s)
+    for (int w = 0; w < PG::Warps; ++w)
+      for (int l = 0; l < 32; ++l) PG::run_phase(tm.data(), reinterpret_cast<const uint4*>(PG::table()), s, w, l, m_top);
+  double sum = 0.0;
+  for (int t = 0; t < PG::Team; ++t) sum += PG::s4_thread(tm.data(), t);
+  return 2.0 * sum / PG::Cden * norm;
+}
+
 extern "C" {
 
 // averaged |M|^2 at CM-frame momenta mom[(n+2)][4], beams first (oracle layout)
@@ -29,22 +47,15 @@ double mfh_me2(int process, const double* mom, double m_top, double alpha_s, dou
   return -1.0;
 }
 
-// The cooperative g g -> t tbar g g program of the fused pass (mf_me_coop.cuh), emulated on the host: the 64
-// team threads are looped over stage by stage (a barrier separates the stages on the device).
-double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {
-  std::vector<double> tm(kCoopTeamDoubles, 0.0);
-  double* in = tm.data() + kCoopOffIn;
-  for (int i = 0; i < 4; ++i) for (int m = 0; m < 4; ++m) in[4 * i + m] = mom[(2 + i) * 4 + m];
-  in[16] = 4.0 * mom[0] * mom[0];
-  in[17] = mom[0];
-  for (int t = 0; t < kCoopTeam; ++t) coop_s0(tm.data(), in, t, m_top);
-  for (int s = 0; s < kCoopPhases; ++s)
-    for (int w = 0; w < kCoopWarps; ++w)
-      for (int l = 0; l < 32; ++l) coop_run_phase(tm.data(), reinterpret_cast<const uint4*>(kCoopTable), s, w, l, m_top);
-  double sum = 0.0;
-  for (int t = 0; t < kCoopTeam; ++t) sum += coop_s4_thread(tm.data(), t);
+// The cooperative matrix-element programs of the fused pass (mf_me_coop.cuh), emulated on the host: the team
+// threads are looped over stage by stage (a barrier separates the stages on the device).
+double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {   // g g -> t tbar g g
   double gs2 = 4.0 * kPi * alpha_s;
-  return 2.0 * sum / kCoopCden * (gs2 * gs2 * gs2 * gs2 / 512.0);   // top spin 0 only, doubled (spin-flip symmetry)
+  return coop_host_me2<g4::Prog>(mom, m_top, gs2 * gs2 * gs2 * gs2 / 512.0);
+}
+double mfh_me2_coop3(const double* mom, double m_top, double alpha_s) {  // g g -> t tbar g
+  double gs2 = 4.0 * kPi * alpha_s;
+  return coop_host_me2<g3::Prog>(mom, m_top, gs2 * gs2 * gs2 / 256.0);
 }
 
 void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {

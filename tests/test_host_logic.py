@@ -86,8 +86,9 @@ def shim():
     L = C.CDLL(out)
     L.mfh_me2.restype = C.c_double
     L.mfh_me2.argtypes = [C.c_int, dp, C.c_double, C.c_double, C.c_double]
-    L.mfh_me2_coop.restype = C.c_double
-    L.mfh_me2_coop.argtypes = [dp, C.c_double, C.c_double]
+    for f in (L.mfh_me2_coop, L.mfh_me2_coop3):
+        f.restype = C.c_double
+        f.argtypes = [dp, C.c_double, C.c_double]
     L.mfh_event.argtypes = [C.c_int, dp, C.c_int] + [C.c_double] * 8 + [C.c_uint64, C.c_uint32, C.c_uint64, dp]
     L.mfh_philox.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32)]
     L.mfh_uniform52.restype = C.c_double
@@ -151,17 +152,20 @@ def test_shim_event_chain(shim, wl, oracle_procs):
     assert npass > n // 2
 
 
-def test_shim_cooperative_program(shim, oracle_procs):
-    """The cooperative g g -> t tbar g g program of the fused pass (64 team threads emulated stage by stage on the
-    host: S0, the table-driven phases, S4; top spin 0 only, doubled) against the oracle's full helicity sum."""
+@pytest.mark.parametrize("pid,n", [(2, 3), (3, 4)])
+def test_shim_cooperative_program(shim, oracle_procs, pid, n):
+    """The cooperative programs of the fused pass (g g -> t tbar g: one warp per event; g g -> t tbar g g: 64
+    threads; team threads emulated stage by stage on the host: S0, the table-driven phases, S4; top spin 0 only,
+    doubled) against the oracle's full helicity sum."""
     from oracle import mfo
     rng = np.random.default_rng(5)
+    fn = shim.mfh_me2_coop if n == 4 else shim.mfh_me2_coop3
     for i in range(40):
         w = 420.0 + 4000.0 * rng.random() ** 2
-        k, _ = mfo.rambo([173.0, 173.0, 0.0, 0.0], w, rng.random(16))
+        k, _ = mfo.rambo([173.0, 173.0] + [0.0] * (n - 2), w, rng.random(4 * n))
         mom = np.ascontiguousarray(np.vstack([[w / 2, 0, 0, w / 2], [w / 2, 0, 0, -w / 2], k]))
-        ref = oracle_procs[3].me2(mom)
-        got = shim.mfh_me2_coop(mom.ctypes.data_as(dp), 173.0, 0.118)
+        ref = oracle_procs[pid].me2(mom)
+        got = fn(mom.ctypes.data_as(dp), 173.0, 0.118)
         assert abs(got - ref) <= 1e-11 * ref
 
 
