@@ -193,7 +193,8 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
   if (p->process >= 2 &&
-      (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads * mf::kCoopQueueDoubles * 8)) != cudaSuccess) {
+      (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads *
+                                       (p->process == 3 ? mf::g4::Prog::Queue : mf::g3::Prog::Queue) * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
   snprintf(p->err, sizeof(p->err), "ok");

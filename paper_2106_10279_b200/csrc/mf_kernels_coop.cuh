@@ -21,8 +21,7 @@ namespace mf {
 template <int PROC> struct CoopOf { typedef g4::Prog PG; static constexpr int MaxTeams = 6; };   // PROC = 3
 template <> struct CoopOf<2> { typedef g3::Prog PG; static constexpr int MaxTeams = 16; };
 
-constexpr int kCoopQueueDoubles = 18;   // queue entry: k[NF][4] (zero padded to 16), shat, sqrt(shat) / 2
-static_assert(g4::Prog::InDoubles == kCoopQueueDoubles && g3::Prog::InDoubles == kCoopQueueDoubles, "queue entry");
+// queue entry = the event record of mf_me_coop_tasks.inc (momenta, shat, polarisation vectors, spinors, c0): PG::Queue doubles
 
 // shared-memory carve-up of a coop block (doubles; every region starts 16-byte aligned)
 template <class PG>
@@ -49,7 +48,7 @@ constexpr int kCoopDebugThreads = 64;
 template <class PG>
 constexpr int coop_debug_smem_bytes() {
   return ((kCoopDebugThreads / PG::Team) * PG::TeamDoubles + 32 + PG::Warps * kCoopDebugThreads +
-          kCoopDebugThreads * kCoopQueueDoubles + 2 * PG::TableVecs) * 8;
+          kCoopDebugThreads * PG::Queue + 2 * PG::TableVecs) * 8;
 }
 
 // copies the operand table into shared memory (all threads of the block; the caller synchronises)
@@ -82,15 +81,31 @@ __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const
   double* tm = teams + team * PG::TeamDoubles;
   double* in = tm + PG::OffIn;
   auto sync = [group]() { coop_group_sync<PG::Team * G>(group); };
-  double nxt = 0.0;
-  if (team < total && tid < kCoopQueueDoubles) nxt = queue[team * kCoopQueueDoubles + tid];
+  // lane `tid` moves doubles tid, tid + Team, ... of the event record from the queue to their places in the scratch
+  // (registers in between: the next record is fetched while the current event is being computed)
+  constexpr int QPT = (PG::Queue + PG::Team - 1) / PG::Team;
+  int dst[QPT];
+  double nxt[QPT];
+#pragma unroll
+  for (int i = 0; i < QPT; ++i) {
+    const int j = tid + i * PG::Team;
+    dst[i] = j < PG::Queue ? PG::qdest(j) : -1;
+    nxt[i] = 0.0;
+    if (team < total && dst[i] >= 0) nxt[i] = queue[team * PG::Queue + j];
+  }
 #pragma unroll 1
   for (int r0 = group * G; r0 < total; r0 += n_teams) {
     const int r = r0 + (team - group * G);
     const bool active = r < total;
-    if (tid < kCoopQueueDoubles) in[tid] = nxt;
+#pragma unroll
+    for (int i = 0; i < QPT; ++i)
+      if (dst[i] >= 0) tm[dst[i]] = nxt[i];
     sync();
-    if (r + n_teams < total && tid < kCoopQueueDoubles) nxt = queue[(r + n_teams) * kCoopQueueDoubles + tid];   // next turn
+    if (r + n_teams < total) {
+#pragma unroll
+      for (int i = 0; i < QPT; ++i)
+        if (dst[i] >= 0) nxt[i] = queue[(r + n_teams) * PG::Queue + tid + i * PG::Team];   // next turn
+    }
     if (active) PG::s0(tm, in, tid, mt);
     sync();
     PG::run(tm, tab, warp, lane, mt, active, sync);
@@ -125,15 +140,7 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
     total += c;
   }
   const int rank = base + __popc(bal & ((1u << lane) - 1u));
-  if (pass) {
-    double* q = queue + rank * kCoopQueueDoubles;
-#pragma unroll
-    for (int f = 0; f < 4; ++f)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) q[4 * f + c] = f < PG::NFinal ? k[f < PG::NFinal ? f : 0][c] : 0.0;
-    q[16] = shat;
-    q[17] = 0.5 * sqrt(shat);
-  }
+  if (pass) PG::owner_fill(queue + rank * PG::Queue, k, shat, P.m_top);
   __syncthreads();
   coop_team_loop<PG, G>(teams, n_teams, tab, s_res, queue, total, P.m_top);   // n_teams is a multiple of G
   __syncthreads();
@@ -166,7 +173,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
   double* s_res = smem + L.res;
   double* s_teams = smem + L.teams;
   uint4* s_tab = reinterpret_cast<uint4*>(smem + L.tab);
-  double* queue = A.coop_queue + (size_t)blockIdx.x * blockDim.x * kCoopQueueDoubles;
+  double* queue = A.coop_queue + (size_t)blockIdx.x * blockDim.x * PG::Queue;
   coop_load_table<PG>(s_tab);
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
@@ -215,7 +222,7 @@ struct CoopDebugSmem {
     s_cnt = reinterpret_cast<unsigned*>(base + n_teams * PG::TeamDoubles);
     s_res = base + n_teams * PG::TeamDoubles + 32;
     queue = s_res + PG::Warps * kCoopDebugThreads;
-    s_tab = reinterpret_cast<uint4*>(queue + kCoopDebugThreads * kCoopQueueDoubles);
+    s_tab = reinterpret_cast<uint4*>(queue + kCoopDebugThreads * PG::Queue);
   }
 };
 
