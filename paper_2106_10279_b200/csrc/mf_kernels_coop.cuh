@@ -84,6 +84,7 @@ __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const
   // lane `tid` moves doubles tid, tid + Team, ... of the event record from the queue to their places in the scratch
   // (registers in between: the next record is fetched while the current event is being computed)
   constexpr int QPT = (PG::Queue + PG::Team - 1) / PG::Team;
+  const int qcap = blockDim.x;                   // the queue is stored [double][rank]
   int dst[QPT];
   double nxt[QPT];
 #pragma unroll
@@ -91,7 +92,7 @@ __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const
     const int j = tid + i * PG::Team;
     dst[i] = j < PG::Queue ? PG::qdest(j) : -1;
     nxt[i] = 0.0;
-    if (team < total && dst[i] >= 0) nxt[i] = queue[team * PG::Queue + j];
+    if (team < total && dst[i] >= 0) nxt[i] = queue[j * qcap + team];
   }
 #pragma unroll 1
   for (int r0 = group * G; r0 < total; r0 += n_teams) {
@@ -104,7 +105,7 @@ __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const
     if (r + n_teams < total) {
 #pragma unroll
       for (int i = 0; i < QPT; ++i)
-        if (dst[i] >= 0) nxt[i] = queue[(r + n_teams) * PG::Queue + tid + i * PG::Team];   // next turn
+        if (dst[i] >= 0) nxt[i] = queue[(tid + i * PG::Team) * qcap + r + n_teams];   // next turn
     }
     if (active) PG::s0(tm, in, tid, mt);
     sync();
@@ -140,7 +141,7 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
     total += c;
   }
   const int rank = base + __popc(bal & ((1u << lane) - 1u));
-  if (pass) PG::owner_fill(queue + rank * PG::Queue, k, shat, P.m_top);
+  if (pass) PG::owner_fill(queue + rank, blockDim.x, k, shat, P.m_top);
   __syncthreads();
   coop_team_loop<PG, G>(teams, n_teams, tab, s_res, queue, total, P.m_top);   // n_teams is a multiple of G
   __syncthreads();

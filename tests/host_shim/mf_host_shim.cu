@@ -15,7 +15,7 @@ static double coop_host_me2(const double* mom, double m_top, double norm) {
   std::vector<double> tm(PG::TeamDoubles, 0.0), q(PG::Queue, 0.0);
   double k[4][4] = {};
   for (int i = 0; i < PG::NFinal; ++i) for (int m = 0; m < 4; ++m) k[i][m] = mom[(2 + i) * 4 + m];
-  PG::owner_fill(q.data(), k, 4.0 * mom[0] * mom[0], m_top);        // what the event's owner thread does
+  PG::owner_fill(q.data(), 1, k, 4.0 * mom[0] * mom[0], m_top);        // what the event's owner thread does
   for (int j = 0; j < PG::Queue; ++j) tm[PG::qdest(j)] = q[j];      // what the team's lanes do with the record
   double* in = tm.data() + PG::OffIn;
   for (int t = 0; t < PG::Team; ++t) PG::s0(tm.data(), in, t, m_top);
