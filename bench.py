@@ -34,6 +34,9 @@ UNIT = "events/s"
 # static fp64 operation counts per matrix-element evaluation, written by csrc/gen_me.py into
 # mf_me_ggtt_generated.cuh (kFlopsMe2_*); per-event work outside the matrix element (DESIGN.md table)
 OTHER_FLOPS = {0: 300.0, 1: 800.0, 2: 1500.0, 3: 2000.0}
+# dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
+# (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
+MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
 NOMINAL_FP64 = 148 * 64 * 2 * 1.965e9   # SMs x FP64 lanes x 2 flop x max SM clock = 37.2 Tflop/s
 
 
@@ -313,7 +316,8 @@ def main():
         "n_accept_last_step": last.n_accept,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": ("fused_pass_coop_kernel<%d,true>" if wl.process >= 2 else "fused_pass_kernel<%d,true>") % wl.process, "kernel_ms": kern,
+                     "traffic": MEASURED_TRAFFIC.get((wl.process, n)), "traffic_source": "profiles/r1_coop_v4_traffic.md",
+                     "kernel": ("fused_pass_coop_kernel<%d,true>" if wl.process >= 2 else "fused_pass_kernel<%d,true>") % wl.process, "kernel_ms": kern,
                      "flops_per_me": me_flops(wl.process), "peak_source": "mf_measure_fp64_peak (DFMA chains) on this GPU",
                      "nominal_peak": NOMINAL_FP64 / 1e12, "frac_of_nominal": achieved / (NOMINAL_FP64 / 1e12)},
     }
