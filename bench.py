@@ -33,7 +33,14 @@ METRIC = "integrand events/sec (fp64) for gg->ttbar gg"
 UNIT = "events/s"
 # static fp64 operation counts per matrix-element evaluation, written by csrc/gen_me.py into
 # mf_me_ggtt_generated.cuh (kFlopsMe2_*); per-event work outside the matrix element (DESIGN.md table)
-OTHER_FLOPS = {0: 300.0, 1: 800.0, 2: 1500.0, 3: 2000.0}
+# Executed fp64 flop per event OUTSIDE the matrix element (a1-a6, a10-a14 incl. the software sqrt / div / log / sincos
+# sequences and, for the cooperative kernels, the owner-side wavefunctions), from ncu
+# (smsp__sass_thread_inst_executed_op_{dfma x 2, dadd, dmul}_pred_on of one fused-pass launch minus n_pass x the
+# generator's static matrix-element count; profiles/r1_flops_per_event.md).  For the two thread-per-event kernels the
+# compiler folds the constant beam wavefunctions into the matrix element, so the static count overestimates: there
+# the measured TOTAL per event is used (ME_FLOPS_MEASURED) and OTHER_FLOPS is 0.
+OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0}
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0}
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
@@ -42,8 +49,8 @@ NOMINAL_FP64 = 148 * 64 * 2 * 1.965e9   # SMs x FP64 lanes x 2 flop x max SM clo
 
 def me_flops(process):
     import re
-    if process == 0:
-        return 2500.0
+    if process in ME_FLOPS_MEASURED:
+        return ME_FLOPS_MEASURED[process]
     csrc = os.path.join(ROOT, "paper_2106_10279_b200", "csrc")
     if process >= 2:    # the cooperative programs (csrc/gen_coop.py, gen_coop3.py) are what the fused pass runs
         name = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g")}[process]
