@@ -169,7 +169,7 @@ MF_D void block_finish(const PassArgs& A, Accum acc, double* s_red, const double
 
 // ---- the fused pass, one thread per event (e+e- -> mu+mu-, gg -> ttbar, gg -> ttbar g) ----------------------
 template <int PROC, bool UNW>
-__global__ void __launch_bounds__(kThreads) fused_pass_kernel(const Params P, const PassArgs A) {
+__global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel(const Params P, const PassArgs A) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   extern __shared__ double smem[];
   const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx;
