@@ -93,6 +93,18 @@ int mf_unweight(mf_process *p, const double *d_grid, uint64_t seed, uint32_t ite
                 uint64_t n_events, double w_max, void *d_records, uint64_t capacity, uint64_t *d_count,
                 double *d_hist, mf_iter_result *d_result, void *stream);
 
+/* Observable histograms accumulated in the same pass ("histogram accumulation"; L109-119, Fig. 2:
+ * d sigma / d pT,top and d sigma / d eta,top).  Attaches a caller-owned DEVICE buffer d_obs[2][n_bins + 1] of doubles
+ * to the handle; from then on every mf_vegas_iterate / mf_unweight call ADDS (never overwrites; the caller zeroes)
+ * the weights w of its events (pb per event: divide by the number of events for a cross section per bin) into
+ *   d_obs[0][i]  lab-frame pT of the FIRST final-state particle (the top quark; mu- for MF_EE_MUMU) in
+ *                [i, i+1) * pt_max / n_bins;            i = n_bins: pT >= pt_max
+ *   d_obs[1][i]  its pseudorapidity asinh(pz / pT) in -eta_max + [i, i+1) * 2 eta_max / n_bins;  i = n_bins: outside
+ * Events failing the cuts (w = 0) are not entered.  The additions are L2 atomics: per-bin sums are reproducible up
+ * to the rounding of the summation order.  d_obs = NULL detaches.  Errors: n_bins outside 1..4096 or a non-positive
+ * range -> MF_EINVAL.  The buffer must stay valid while attached. */
+int mf_set_observables(mf_process *p, double *d_obs, int32_t n_bins, double pt_max, double eta_max);
+
 /* Test/diagnostic: per-event rows of mf_debug_row_len doubles, identical to the oracle's layout:
  * x[D] | (n+2)x(E,px,py,pz) lab, beams first | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D] */
 int mf_debug_eval(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,

@@ -290,3 +290,29 @@ class Process:
         assert dt.itemsize == self.record_size and nd * 8 + 16 == self.record_size
         a = np.frombuffer(rec.tobytes()[:count * self.record_size], dtype=dt)
         return a["mom"], a["w"], a["id"]
+
+
+def observable_histograms(rows, n_dims, n_final, n_bins, pt_max, eta_max):
+    """ORACLE for the observable histograms of the fused pass ("histogram accumulation"; L109-119, Fig. 2:
+    d sigma / d pT,top and d sigma / d eta,top), written out from their definition on the oracle's own per-event rows
+    (debug_eval): for every event with w != 0 take the lab-frame momentum (E, px, py, pz) of the FIRST final-state
+    particle, pT = sqrt(px^2 + py^2), eta = asinh(pz / pT), and add w to bin floor(pT / pt_max * n_bins) of row 0 and
+    to bin floor((eta + eta_max) / (2 eta_max) * n_bins) of row 1; bin n_bins collects everything outside.
+    Returns obs[2][n_bins + 1]."""
+    rows = np.asarray(rows)
+    o = n_dims + 4 * (n_final + 2)
+    w = rows[:, o + 6]
+    p = rows[:, n_dims + 8:n_dims + 12]                 # particle 2 = first final-state particle
+    obs = np.zeros((2, n_bins + 1))
+    for k in range(len(rows)):
+        if w[k] == 0.0:
+            continue
+        pt = np.sqrt(p[k, 1] * p[k, 1] + p[k, 2] * p[k, 2])
+        eta = np.arcsinh(p[k, 3] / pt)
+        bp = pt / pt_max * n_bins
+        be = (eta + eta_max) / (2.0 * eta_max) * n_bins
+        ip = int(bp) if bp < n_bins else n_bins
+        ie = int(be) if 0.0 <= be < n_bins else n_bins
+        obs[0, ip] += w[k]
+        obs[1, ie] += w[k]
+    return obs

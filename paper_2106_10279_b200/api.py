@@ -27,7 +27,7 @@ c_double_p = C.POINTER(C.c_double)
 # every symbol include/mf.h declares (tests check the library exports each one)
 EXPORTS = ["mf_create_process", "mf_destroy_process", "mf_n_dims", "mf_n_final", "mf_record_size",
            "mf_debug_row_len", "mf_last_error", "mf_launch_config", "mf_vegas_iterate", "mf_refine_grid",
-           "mf_unweight", "mf_debug_eval", "mf_debug_philox", "mf_debug_pdf", "mf_debug_me2",
+           "mf_unweight", "mf_set_observables", "mf_debug_eval", "mf_debug_philox", "mf_debug_pdf", "mf_debug_me2",
            "mf_measure_fp64_peak"]
 
 
@@ -68,6 +68,7 @@ def lib():
         L.mf_vegas_iterate.argtypes = [vp, vp, u64, u32, u64, u64, vp, vp, vp]
         L.mf_refine_grid.argtypes = [vp, vp, vp, C.c_double, vp]
         L.mf_unweight.argtypes = [vp, vp, u64, u32, u64, u64, C.c_double, vp, u64, vp, vp, vp, vp]
+        L.mf_set_observables.argtypes = [vp, vp, C.c_int32, C.c_double, C.c_double]
         L.mf_debug_eval.argtypes = [vp, vp, u64, u32, u64, u64, vp, vp]
         L.mf_debug_philox.argtypes = [u64, u32, u64, u64, u32, vp, vp]
         L.mf_debug_pdf.argtypes = [vp, vp, vp, u64, vp, vp]
@@ -106,6 +107,10 @@ def mf_unweight(h, d_grid, seed, iteration, first_event, n_events, w_max, d_reco
                 d_result, stream=0):
     return lib().mf_unweight(h, d_grid, seed, iteration, first_event, n_events, w_max, d_records, capacity, d_count,
                              d_hist, d_result, stream)
+
+
+def mf_set_observables(h, d_obs, n_bins, pt_max, eta_max):
+    return lib().mf_set_observables(h, d_obs, n_bins, pt_max, eta_max)
 
 
 def mf_debug_eval(h, d_grid, seed, iteration, first_event, n_events, d_out, stream=0):
@@ -225,6 +230,14 @@ class Process:
                            records.data_ptr() if records is not None else None, capacity, count.data_ptr(),
                            hist.data_ptr() if hist is not None else None, result.data_ptr(), _stream_ptr(stream)),
                self.h, "mf_unweight")
+
+    def set_observables(self, obs, n_bins=0, pt_max=0.0, eta_max=0.0):
+        """attach a zeroed float64 CUDA tensor [2, n_bins + 1] (pT and eta of the first final-state particle); None detaches"""
+        if obs is not None:
+            assert obs.is_cuda and obs.dtype == _torch().float64 and obs.numel() == 2 * (n_bins + 1) and obs.is_contiguous()
+        _check(mf_set_observables(self.h, obs.data_ptr() if obs is not None else None, n_bins, pt_max, eta_max), self.h,
+               "mf_set_observables")
+        self._obs = obs          # keep the buffer alive while attached
 
     # -- diagnostics ---------------------------------------------------------------------------------------
     def debug_eval(self, grid, seed, iteration, first_event, n_events):

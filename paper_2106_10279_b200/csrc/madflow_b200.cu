@@ -20,6 +20,9 @@ struct mf_process {
   double *d_lnx = nullptr, *d_lnq2 = nullptr, *d_xf = nullptr, *d_row = nullptr;  // PDF table + collapsed row
   mf::BlockPartial* d_partials = nullptr;
   double* d_queue = nullptr;          // cooperative pass: per-block momenta queue
+  double* d_obs = nullptr;            // caller-owned observable histograms (mf_set_observables) or NULL
+  int obs_nb = 0;
+  double obs_ptmax = 0.0, obs_etamax = 0.0;
   double* d_hist_part = nullptr;
   int blocks = 0, threads = mf::kThreads;
   int blocks_unw = 0;
@@ -92,6 +95,7 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   A.w_max = w_max; A.records = (char*)d_records; A.capacity = capacity; A.count = (unsigned long long*)d_count;
   A.partials = p->d_partials; A.hist_part = d_hist ? p->d_hist_part : nullptr;
   A.coop_queue = p->d_queue;
+  A.obs = p->d_obs; A.obs_nb = p->obs_nb; A.obs_ptmax = p->obs_ptmax; A.obs_etamax = p->obs_etamax;
   cudaStream_t st = (cudaStream_t)stream;
   const int blocks = unw ? p->blocks_unw : p->blocks;
   void* args[2] = {(void*)&p->P, (void*)&A};
@@ -225,6 +229,14 @@ const char* mf_last_error(const mf_process* p) { return p ? p->err : kNullHandle
 int mf_launch_config(const mf_process* p, int32_t* blocks, int32_t* threads) {
   if (!p || !blocks || !threads) return MF_EINVAL;
   *blocks = p->blocks; *threads = p->threads;
+  return MF_OK;
+}
+
+int mf_set_observables(mf_process* p, double* d_obs, int32_t n_bins, double pt_max, double eta_max) {
+  if (!p) return MF_EINVAL;
+  if (!d_obs) { p->d_obs = nullptr; p->obs_nb = 0; return MF_OK; }
+  if (n_bins < 1 || n_bins > 4096 || !(pt_max > 0.0) || !(eta_max > 0.0)) return fail(p, MF_EINVAL, "mf_set_observables: bad argument");
+  p->d_obs = d_obs; p->obs_nb = n_bins; p->obs_ptmax = pt_max; p->obs_etamax = eta_max;
   return MF_OK;
 }
 

@@ -35,7 +35,10 @@ struct PassArgs {
   unsigned long long* count;
   BlockPartial* partials;  // [gridDim.x]
   double* hist_part;       // [gridDim.x][D*nb] or nullptr
-  double* coop_queue;      // g g -> t tbar g g only: [gridDim.x][blockDim.x][18] momenta queue (mf_kernels_coop.cuh)
+  double* obs;             // observable histograms [2][obs_nb + 1] (added to) or nullptr (mf_set_observables)
+  int obs_nb;
+  double obs_ptmax, obs_etamax;
+  double* coop_queue;      // cooperative kernels only: [gridDim.x][blockDim.x][18] momenta queue (mf_kernels_coop.cuh)
 };
 
 // The matrix element is the only large piece of code; keep ONE copy per process per kernel.
@@ -71,6 +74,23 @@ MF_D double accept_draw(uint64_t seed, uint32_t iteration, uint64_t event) {
   return uniform52(r.x, r.y);
 }
 
+// Observable bins of an event ("histogram accumulation"; L109-119: d sigma / d pT,top, d sigma / d eta,top):
+// lab-frame pT and pseudorapidity of the FIRST final-state particle (the top quark; mu- for e+e-).  Returns the pT bin
+// in the low 16 bits and the eta bin in the high 16 bits; bin obs_nb = outside [0, pt_max) resp. [-eta_max, eta_max).
+template <int PROC>
+MF_D int observable_bins(const PassArgs& A, const Event<PROC>& ev) {
+  const Boost b = make_boost(ev.y);
+  double t[4];
+  boost_z(b, ev.k[0], t);
+  const int nb = A.obs_nb;
+  const double pt = sqrt(t[1] * t[1] + t[2] * t[2]);
+  const double eta = asinh(t[3] / pt);
+  const double bp = pt / A.obs_ptmax * nb, be = (eta + A.obs_etamax) / (2.0 * A.obs_etamax) * nb;
+  const int ip = bp < nb ? (int)bp : nb;
+  const int ie = (be >= 0.0 && be < nb) ? (int)be : nb;
+  return ip | (ie << 16);
+}
+
 constexpr int kThreads = 128;
 
 // Per-thread running sums of the pass (registers).
@@ -83,7 +103,7 @@ struct Accum {
 // shared-memory w^2 histogram, and hit-or-miss unweighting with a warp-aggregated cursor.
 template <int PROC, bool UNW>
 MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_grid, double* s_hist, bool valid,
-                           uint64_t event, double w, const Bins<PROC>& bins, Accum& acc) {
+                           uint64_t event, double w, const Bins<PROC>& bins, Accum& acc, int obs_bins) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   const int nb = P.n_bins;
   const double w2 = w * w;
@@ -93,6 +113,10 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
   if (w != 0.0) {
 #pragma unroll
     for (int d = 0; d < D; ++d) atomicAdd(&s_hist[d * nb + bins.get(d)], w2);
+    if (A.obs != nullptr) {   // observable histograms accumulate the weights themselves (global memory, L2 atomics)
+      atomicAdd(A.obs + (obs_bins & 0xFFFF), w);
+      atomicAdd(A.obs + (A.obs_nb + 1) + (obs_bins >> 16), w);
+    }
   }
   if (UNW) {
     // a14: hit-or-miss against w_max; one global atomic per warp with survivors
@@ -193,10 +217,12 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
     double w = 0.0;
     Bins<PROC> bins;
     bins.clear();
+    int obs_bins = 0;
     if (valid) {
       Event<PROC> ev;
       DebugRow dbg = {nullptr, D, NF};
       generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
+      if (ev.pass && A.obs != nullptr) obs_bins = observable_bins<PROC>(A, ev);
       if (ev.pass) {
         ++acc.n_pass;
         double lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
@@ -204,7 +230,7 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
         w = event_weight<PROC>(P, ev, lum, me2);
       }
     }
-    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc);
+    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins);
   }
   block_finish(A, acc, s_red, s_hist, D * nb);
 }

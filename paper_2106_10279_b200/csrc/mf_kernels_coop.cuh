@@ -199,6 +199,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
       if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
     }
     const bool pass = valid && ev.pass;
+    const int obs_bins = (pass && A.obs != nullptr) ? observable_bins<PROC>(A, ev) : 0;
     const double me2 =
         coop_block_me2<PG, G>(s_teams, n_teams, s_tab, s_cnt, s_res, queue, (unsigned)rd, pass, ev.k, ev.shat, P);
     double w = 0.0;
@@ -206,7 +207,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
       ++acc.n_pass;
       w = event_weight<PROC>(P, ev, lum, me2);
     }
-    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc);
+    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins);
   }
   block_finish(A, acc, s_red, s_hist, D * nb);
 }

@@ -156,6 +156,11 @@ def main(argv=None):
     ap.add_argument("--config", default="C3")
     ap.add_argument("--events", type=int, default=0, help="events per iteration (default: the configuration's)")
     ap.add_argument("--capacity", type=int, default=1 << 20, help="record buffer capacity (unweighting configs)")
+    ap.add_argument("--observables", type=int, default=0, metavar="NBINS",
+                    help="also accumulate d sigma / d pT and d sigma / d eta of the first final-state particle "
+                         "(PAPER.md Fig. 2) in NBINS bins over the frozen-grid / last iteration and print them")
+    ap.add_argument("--pt-max", type=float, default=600.0)
+    ap.add_argument("--eta-max", type=float, default=3.0)
     args = ap.parse_args(argv)
     wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4}[args.config]
     if args.events > 0:
@@ -172,6 +177,23 @@ def main(argv=None):
               (r.iteration, r.integral, r.sigma, r.max_abs_w, r.n_pass / r.n_events, r.n_accept))
     mean, err, chi2 = run.combined()
     n_tot = sum(r.n_events for r in run.iterations)
+    if args.observables > 0:
+        # one more iteration on the final grid with the observable histograms attached (mf_set_observables)
+        nb = args.observables
+        obs = torch.zeros((2, nb + 1), dtype=torch.float64, device="cuda")
+        proc.set_observables(obs, nb, args.pt_max, args.eta_max)
+        res = proc.new_result()
+        proc.vegas_iterate(run.grid, wl.seed, wl.n_iterations, 0, wl.n_events, None, res)
+        torch.cuda.synchronize()
+        proc.set_observables(None)
+        h = (obs / wl.n_events).cpu().numpy()
+        dpt, deta = args.pt_max / nb, 2 * args.eta_max / nb
+        print("pT bin [GeV]      d sigma / d pT [pb / GeV]   |   eta bin          d sigma / d eta [pb]")
+        for i in range(nb):
+            print("%7.1f - %-7.1f  %-12.5g               |   %+5.2f - %+5.2f    %-12.5g" %
+                  (i * dpt, (i + 1) * dpt, h[0, i] / dpt, -args.eta_max + i * deta, -args.eta_max + (i + 1) * deta,
+                   h[1, i] / deta))
+        print("outside the ranges: %.5g pb (pT), %.5g pb (eta)" % (h[0, nb], h[1, nb]))
     print(json.dumps({"config": args.config, "workload": wl.name, "integral_pb": mean, "error_pb": err,
                       "chi2_per_dof": chi2, "iterations": len(run.iterations), "events_per_iteration": wl.n_events,
                       "wall_s": dt, "events_per_s": n_tot / dt, "unweighted_events": run.n_records}))

@@ -351,6 +351,47 @@ def test_full_size_sampled(proc, gpu_procs, oracle_procs):
     assert rg.max_abs_w > 0 and rg.n_pass <= n
 
 
+# ---- observable histograms (Fig. 2) -------------------------------------------------------------------
+@pytest.mark.parametrize("proc,n", [(0, 30_011), (1, 20_001), (2, 4_001), (3, 1_003)])
+def test_observable_histograms(proc, n, gpu_procs, oracle_procs):
+    """pT and eta histograms of the first final-state particle, accumulated in the same pass, against the oracle's
+    definition evaluated on its own per-event rows; accumulation across calls (also through mf_unweight); detaching."""
+    from oracle import mfo
+    torch = _torch()
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    grid = adapted_grid(op, wl)
+    nb, pt_max, eta_max = 20, {0: 55.0}.get(proc, 600.0), 3.2
+    rows = op.debug_eval(grid, 4, 2, 7, n)
+    want = mfo.observable_histograms(rows, wl.n_dims, wl.n_final, nb, pt_max, eta_max)
+    obs = torch.zeros((2, nb + 1), dtype=torch.float64, device="cuda")
+    gp.set_observables(obs, nb, pt_max, eta_max)
+    try:
+        hg, rg = _iterate_gpu(gp, grid, 4, 2, 7, n)
+        got = obs.cpu().numpy()
+        scale = np.abs(want).max()
+        # an event within rounding of a bin edge may change bins: compare bin by bin, tolerate none here (none seen)
+        np.testing.assert_allclose(got, want, rtol=1e-9, atol=1e-12 * scale)
+        for h in got:
+            assert abs(h.sum() - rg.sum_w) <= 1e-11 * abs(rg.sum_w)
+        # a second call (through the unweighting entry point) ADDS to the same buffer
+        dgrid = torch.from_numpy(grid).cuda()
+        res = gp.new_result()
+        count = torch.zeros(1, dtype=torch.int64, device="cuda")
+        gp.unweight(dgrid, 4, 2, 7, n, rg.max_abs_w, None, 0, count, None, res)
+        torch.cuda.synchronize()
+        np.testing.assert_allclose(obs.cpu().numpy(), 2 * want, rtol=1e-9, atol=1e-12 * scale)
+    finally:
+        gp.set_observables(None)
+    before = obs.clone()
+    _iterate_gpu(gp, grid, 4, 2, 7, 257)
+    assert torch.equal(obs, before)        # detached: untouched
+    # argument errors
+    from paper_2106_10279_b200 import api
+    assert api.mf_set_observables(gp.h, obs.data_ptr(), 0, 1.0, 1.0) == api.MF_EINVAL
+    assert api.mf_set_observables(gp.h, obs.data_ptr(), 10, -1.0, 1.0) == api.MF_EINVAL
+
+
 # ---- error behaviour ----------------------------------------------------------------------------------------
 def test_error_codes(pdf):
     from dataclasses import replace
