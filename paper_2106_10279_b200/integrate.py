@@ -91,12 +91,14 @@ def combine_across_ranks(hist, result, group=None):
 
 
 def run_config(proc, wl=None, capacity=0, stream=None, alpha=W.VEGAS_ALPHA, grid=None, hists=None, rank=0, world=1,
-               weak=False):
+               weak=False, drain=None):
     """Runs every iteration of `wl` (default: proc.wl) on the GPU.  Returns a RunResult.
     `hists`, if a list, receives a host copy of each iteration's histogram (tests).
     world > 1: this rank processes its shard of each iteration's events (weak=False: wl.n_events split over
     the ranks; weak=True: wl.n_events PER rank) and the per-iteration sums are combined with
-    combine_across_ranks before the (replicated, identical) grid refinement; records stay rank-local."""
+    combine_across_ranks before the (replicated, identical) grid refinement; records stay rank-local.
+    `drain` (lhe.LheDrain): the records of every unweighting iteration are handed to it right after the call (the
+    record buffer is then reused by the next iteration; out.n_records counts all drained events)."""
     import torch
     wl = proc.wl if wl is None else wl
     if world > 1:
@@ -125,8 +127,12 @@ def run_config(proc, wl=None, capacity=0, stream=None, alpha=W.VEGAS_ALPHA, grid
             if not running_max > 0.0:
                 raise api.MfError("unweighting needs a positive w_max from the last adapting iteration")
             w_max_used[k] = running_max
+            if drain is not None:
+                count.zero_()
             proc.unweight(grid, wl.seed, k, first_event, n_local, running_max, out.records, capacity, count, hist,
                           results[k], stream)
+            if drain is not None:
+                out.n_records += drain.push(out.records, count, running_max, capacity, stream)
         else:
             proc.vegas_iterate(grid, wl.seed, k, first_event, n_local, hist, results[k], stream)
         if world > 1:
@@ -140,7 +146,7 @@ def run_config(proc, wl=None, capacity=0, stream=None, alpha=W.VEGAS_ALPHA, grid
         r = api.Process.result_to_host(results[k])
         out.iterations.append(IterationRecord(k, n_total, r.sum_w, r.sum_w2, r.max_abs_w, r.n_pass, r.n_accept,
                                               w_max_used[k]))
-    if count is not None:
+    if count is not None and drain is None:
         out.n_records = int(count.item())
     return out
 
@@ -159,6 +165,8 @@ def main(argv=None):
     ap.add_argument("--observables", type=int, default=0, metavar="NBINS",
                     help="also accumulate d sigma / d pT and d sigma / d eta of the first final-state particle "
                          "(PAPER.md Fig. 2) in NBINS bins over the frozen-grid / last iteration and print them")
+    ap.add_argument("--lhe", default="", metavar="FILE", help="unweighting configs (C4): drain the accepted events of every "
+                    "frozen iteration asynchronously into this LHE 3.0 file (.gz = compressed; PAPER.md L81)")
     ap.add_argument("--pt-max", type=float, default=600.0)
     ap.add_argument("--eta-max", type=float, default=3.0)
     args = ap.parse_args(argv)
@@ -168,10 +176,17 @@ def main(argv=None):
     proc = api.Process(wl, W.pdf_table() if wl.process else None)
     run_config(proc, wl.scaled(min(wl.n_events, 1 << 16)), capacity=args.capacity if wl.unweight else 0)   # warm-up
     torch.cuda.synchronize()
+    drain = None
+    if args.lhe and wl.unweight:
+        from . import lhe
+        drain = lhe.LheDrain(args.lhe, proc)
     t0 = time.perf_counter()
-    run = run_config(proc, wl, capacity=args.capacity if wl.unweight else 0)
+    run = run_config(proc, wl, capacity=args.capacity if wl.unweight else 0, drain=drain)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
+    if drain is not None:
+        mean, err, _ = run.combined()
+        print("LHE: %d events written to %s" % (drain.close(mean, err), args.lhe))
     for r in run.iterations:
         print("iteration %2d  I = %.8g +- %.3g pb  max|w| = %.4g  pass %.4f  accepted %d" %
               (r.iteration, r.integral, r.sigma, r.max_abs_w, r.n_pass / r.n_events, r.n_accept))

@@ -1,0 +1,99 @@
+"""LHE 3.0 output of the unweighted events: the pure formatting functions on CPU,
+the asynchronous drain on the GPU."""
+import gzip
+import re
+
+import numpy as np
+import pytest
+
+from paper_2106_10279_b200 import lhe
+from paper_2106_10279_b200 import workloads as W
+
+
+def _parse(text):
+    events = []
+    for blk in re.findall(r"<event>\n(.*?)</event>", text, re.S):
+        lines = [l for l in blk.strip().split("\n") if not l.startswith("#")]
+        head = lines[0].split()
+        parts = [l.split() for l in lines[1:]]
+        eid = int(re.search(r"# event id (\d+)", blk).group(1))
+        events.append((int(head[0]), float(head[2]), parts, eid))
+    return events
+
+
+def test_colour_flow_is_a_valid_planar_flow():
+    for proc in (1, 2, 3):
+        ids, flow = lhe.PDG[proc], lhe.colour_flow(proc)
+        out_col, out_acol = [], []
+        for i, (pid, (c, a)) in enumerate(zip(ids, flow)):
+            if i < 2:                       # incoming: crossing swaps the roles
+                c, a = a, c
+            if c:
+                out_col.append(c)
+            if a:
+                out_acol.append(a)
+            assert (pid == 21) == (c != 0 and a != 0)
+        assert sorted(out_col) == sorted(out_acol)           # every colour line ends on an anticolour
+        assert len(set(out_col)) == len(out_col)
+
+
+def test_format_events_round_trip():
+    rng = np.random.default_rng(0)
+    rec = np.zeros(5, dtype=lhe.record_dtype(4))
+    rec["mom"] = rng.normal(size=(5, 6, 4)) * 300
+    rec["w"] = [1.0, -0.5, 3.0, 2.0, 0.25]
+    rec["id"] = [7, 3, 2 ** 40 + 1, 11, 5]
+    text = lhe.format_events(rec, 3, 173.0, 173.0, 1 / 132.507, 0.118, w_max=2.0)
+    ev = _parse(text)
+    assert len(ev) == 5 and [e[3] for e in ev] == [7, 3, 2 ** 40 + 1, 11, 5]
+    assert [e[1] for e in ev] == [1.0, -1.0, 1.5, 1.0, 1.0]          # unit weights, sign kept, overweight 3/2
+    for (nup, _, parts, _), r in zip(ev, rec):
+        assert nup == 6 and [int(p[0]) for p in parts] == [21, 21, 6, -6, 21, 21]
+        assert [int(p[1]) for p in parts] == [-1, -1, 1, 1, 1, 1]
+        for p, m in zip(parts, r["mom"]):
+            got = np.array([float(p[9]), float(p[6]), float(p[7]), float(p[8])])     # E px py pz
+            np.testing.assert_allclose(got, m, rtol=2e-10, atol=1e-9)
+        assert [float(p[10]) for p in parts] == [0, 0, 173, 173, 0, 0]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("compress", [False, True])
+def test_lhe_drain_matches_records(tmp_path, compress, pdf):
+    """frozen iterations of gg -> ttbar with unweighting, each drained asynchronously: the file holds exactly the
+    accepted events of every iteration, in event-id order per iteration, momenta to the printed precision"""
+    import torch
+    from paper_2106_10279_b200 import api
+    wl = W.C1.scaled(30000, 4, 2)
+    gp = api.Process(wl, pdf)
+    grid, hist, res = gp.new_grid(), gp.new_hist(), gp.new_result()
+    w_max = 0.0
+    for k in range(2):
+        gp.vegas_iterate(grid, 0, k, 0, wl.n_events, hist, res)
+        gp.refine_grid(grid, hist)
+        w_max = max(w_max, gp.result_to_host(res).max_abs_w)
+    cap = 4096
+    records = torch.zeros(cap * gp.record_size, dtype=torch.uint8, device="cuda")
+    count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    path = str(tmp_path / ("ev.lhe.gz" if compress else "ev.lhe"))
+    drain = lhe.LheDrain(path, gp)
+    want = []
+    for k in range(2, 4):
+        count.zero_()
+        gp.unweight(grid, 0, k, 0, wl.n_events, w_max, records, cap, count, None, res)
+        n = drain.push(records, count, w_max, cap)
+        torch.cuda.synchronize()
+        mom, w, ids = gp.records_view(records, n)
+        order = np.argsort(ids)
+        want += [(int(ids[i]), mom[i].copy(), float(w[i])) for i in order]
+        assert n == gp.result_to_host(res).n_accept > 0
+    n_tot = drain.close(2649.0, 0.4)
+    text = (gzip.open(path, "rt") if compress else open(path)).read()
+    assert text.startswith('<LesHouchesEvents version="3.0">') and text.rstrip().endswith("</LesHouchesEvents>")
+    assert re.search(r"<init>\n2212 2212 6\.5", text)
+    ev = _parse(text)
+    assert len(ev) == n_tot == len(want)
+    for (nup, xw, parts, eid), (wid, wm, ww) in zip(ev, want):
+        assert eid == wid and nup == 4 and xw == (1.0 if ww >= 0 else -1.0) * max(1.0, abs(ww) / w_max)
+        for p, m in zip(parts, wm):
+            np.testing.assert_allclose([float(p[9]), float(p[6]), float(p[7]), float(p[8])], m, rtol=2e-10, atol=1e-8)
+    gp.close()
