@@ -120,6 +120,34 @@ def oracle_sample(wl, seconds=15.0, n_first=64):
     return n / dt, n, dt
 
 
+_ALL_CORES_WORKER = r"""
+import sys, time
+sys.path.insert(0, sys.argv[1])
+from oracle import mfo
+from paper_2106_10279_b200 import workloads as W
+wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4}[sys.argv[2]]
+first, n = int(sys.argv[3]), int(sys.argv[4])
+op = mfo.Process(wl, W.pdf_table())
+grid = W.uniform_grid(wl.n_dims, wl.n_bins)
+t0 = time.perf_counter()
+op.vegas_iterate(grid, wl.seed, 0, first, n)
+print(time.perf_counter() - t0)
+"""
+
+
+def oracle_all_cores(config, per_event_s, seconds=10.0):
+    """The same single-threaded oracle as P independent processes on disjoint event-index ranges (possible because the
+    RNG is counter based), P = the host's logical cores: aggregate events/s."""
+    P = os.cpu_count() or 1
+    n = max(16, int(seconds / per_event_s))
+    t0 = time.perf_counter()
+    procs = [subprocess.Popen([sys.executable, "-c", _ALL_CORES_WORKER, ROOT, config, str(i * n), str(n)],
+                              stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True) for i in range(P)]
+    ok = all(p.wait() == 0 for p in procs)
+    dt = time.perf_counter() - t0
+    return (P * n / dt, P, n, dt) if ok else None
+
+
 def run_reference(args, wl):
     """--impl reference: the oracle on the host cores (one thread), each step a bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -157,12 +185,16 @@ def main():
     ap.add_argument("--config", default="C3")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--seed", type=int, default=None, help="Philox seed (default: the configuration's, 0)")
     ap.add_argument("--events", type=int, default=0,
                     help="events per step per GPU (default: the config's; smaller values are for ncu captures only)")
     args = ap.parse_args()
     wl = config_by_name(args.config)
     if args.events > 0:
         wl = wl.scaled(args.events)
+    if args.seed is not None:
+        from dataclasses import replace
+        wl = replace(wl, seed=args.seed)
     if args.impl == "reference":
         return run_reference(args, wl)
     if args.warmup < 3:
@@ -309,7 +341,7 @@ def main():
     peak = peak_flops / 1e12
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": total_ms / args.steps, "ms_per_step_median": sorted(ms)[len(ms) // 2], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s: BASELINE.json configs[%d], %d events/step/GPU, step = mf_unweight + mf_refine_grid"
                                % (wl.name, wl.process if args.config != "C4" else 4, n),
@@ -333,6 +365,11 @@ def main():
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": "events [0,%d) of iteration 0 of %s on the uniform grid, %.1f s, 1 thread of %d"
                                          % (ns, wl.name, dt, os.cpu_count())}
+        allc = oracle_all_cores(args.config, dt / ns)
+        if allc is not None:    # context only: the same program, one process per logical core (start-up included)
+            out["cpu_baseline_all_cores"] = {"value": allc[0], "unit": UNIT, "cores": allc[1], "kind": "oracle",
+                                             "sample": "%d processes x %d events, disjoint index ranges, %.1f s wall"
+                                                       % (allc[1], allc[2], allc[3])}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
