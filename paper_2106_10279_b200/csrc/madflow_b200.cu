@@ -68,8 +68,10 @@ cudaError_t coop_setup(mf_process* p, const cudaDeviceProp& prop) {
   p->smem = (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8;
   cudaError_t e;
   for (int u = 0; u < 2; ++u)
-    if ((e = cudaFuncSetAttribute(pass_fn(PROC, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smem)) !=
-        cudaSuccess) return e;
+    // the attribute belongs to the kernel, not to the handle: always ask for the device maximum, so that handles with
+    // different bin counts (different shared-memory needs) can coexist
+    if ((e = cudaFuncSetAttribute(pass_fn(PROC, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)prop.sharedMemPerBlockOptin)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute((const void*)mf::debug_eval_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 mf::coop_debug_smem_bytes<PG>())) != cudaSuccess) return e;
   return cudaFuncSetAttribute((const void*)mf::debug_me2_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,

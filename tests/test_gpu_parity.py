@@ -351,6 +351,29 @@ def test_full_size_sampled(proc, gpu_procs, oracle_procs):
     assert rg.max_abs_w > 0 and rg.n_pass <= n
 
 
+# ---- other bin counts (the launch shape of the cooperative kernels depends on the shared memory left) --------------
+@pytest.mark.parametrize("proc,n", [(1, 20_000), (2, 3_000), (3, 700)])
+@pytest.mark.parametrize("nb", [8, 128])
+def test_other_bin_counts(proc, n, nb, pdf):
+    from dataclasses import replace
+    from oracle import mfo
+    from paper_2106_10279_b200 import api
+    torch = _torch()
+    wl = replace(WLS[proc], n_bins=nb)
+    gp, op = api.Process(wl, pdf), mfo.Process(wl, pdf)
+    try:
+        grid = W.uniform_grid(wl.n_dims, nb)
+        h, _ = op.vegas_iterate(grid, 1, 0, 0, n)
+        grid = op.refine_grid(grid, h, W.VEGAS_ALPHA)
+        ho, ro = op.vegas_iterate(grid, 1, 1, 5, n)
+        hist, res = gp.new_hist(), gp.new_result()
+        gp.vegas_iterate(torch.from_numpy(grid).cuda(), 1, 1, 5, n, hist, res)
+        torch.cuda.synchronize()
+        _check_sums(n, hist.cpu().numpy(), gp.result_to_host(res), ho, ro)
+    finally:
+        gp.close()
+
+
 # ---- observable histograms (Fig. 2) -------------------------------------------------------------------
 @pytest.mark.parametrize("proc,n", [(0, 30_011), (1, 20_001), (2, 4_001), (3, 1_003)])
 def test_observable_histograms(proc, n, gpu_procs, oracle_procs):
