@@ -1,17 +1,21 @@
-// mf_me_coop.cuh — steps a7-a9 for g g -> t tbar g g as a COOPERATIVE program: one event per team of 64
-// threads (2 warps), all intermediate currents in a per-team shared-memory scratch (the
-// matrix element loops over helicities and sums; DESIGN.md "Kernels" explains why not one thread per event).
+// mf_me_coop.cuh — steps a7-a9 for g g -> t tbar g g and g g -> t tbar g as COOPERATIVE programs: one event per
+// team of 64 threads (2 warps) resp. 32 threads (1 warp), all intermediate currents in a per-team shared-memory
+// scratch (the matrix element loops over helicities and sums; DESIGN.md "Kernels" explains why
+// not one thread per event).
 //
-//   S0     hand written: momentum sums, propagator denominators, polarisation vectors, external spinors, c0
-//   S1/A/B table driven (csrc/gen_coop.py): one lane-task = M "polarisation sibling" off-shell currents that
-//          share their operands; a warp executes rounds of 32 equal-shaped lane-tasks
-//   S4     generated straight-line code: thread (pols, hb, k) forms the real / imaginary parts of its 24
-//          colour-ordered amplitudes and contracts them with the colour matrix; the 64 partial sums are
-//          added in a fixed order.  Only the top spin state 0 is evaluated (spin-flip symmetry, gen_coop.py):
-//          the caller doubles the sum.
+//   owner  the thread that generated the event evaluates polarisation vectors, external spinors and c0 = ubar gamma v
+//          and queues them with the momenta (event record); the team's lanes copy the record into the scratch
+//   S0     hand written: momentum sums, propagator momenta and inverse denominators (one reciprocal per lane)
+//   S1/A/B table driven (csrc/gen_coop.py, gen_coop3.py): one lane-task = M "polarisation sibling" off-shell currents
+//          that share their operands; a warp executes rounds of <= 32 equal-shaped lane-tasks
+//   S4     generated straight-line code: thread (pols, hb, k) forms the real / imaginary parts of its colour-ordered
+//          amplitudes and contracts them with the colour matrix; the partial sums are added in a fixed order.  Only
+//          the top spin state 0 is evaluated (spin-flip symmetry, gen_coop.py): the caller doubles the sum.
 //
-// Every function is MF_HD and takes the team-thread index explicitly, so tests/host_shim can run the same
-// program on the host (looping over the 64 "threads" stage by stage) and compare it with the oracle.
+// The two programs share the task templates (mf_me_coop_tasks.inc, compiled once per process inside namespaces
+// mf::g4 / mf::g3 after the process' generated fragment).  Every function is MF_HD and takes the team-thread index
+// explicitly, so tests/host_shim can run the same programs on the host (looping over the team's "threads" stage by
+// stage) and compare them with the oracle.
 #pragma once
 #include "mf_me_prims.cuh"
 
