@@ -93,6 +93,13 @@ int mf_unweight(mf_process *p, const double *d_grid, uint64_t seed, uint32_t ite
                 uint64_t n_events, double w_max, void *d_records, uint64_t capacity, uint64_t *d_count,
                 double *d_hist, mf_iter_result *d_result, void *stream);
 
+/* Dynamic scale (R16).  on != 0: every later pass uses, event by event,
+ * mu_F^2 = mu_R^2 = m_t^2 + pT(top)^2, the general 2-D log-bicubic PDF lookup at that scale, and the strong coupling
+ * running at one loop (n_f = 5) from the descriptor's alpha_s at the descriptor's mu2:
+ * alpha_s(mu^2) = alpha_s / (1 + alpha_s (23 / 12 pi) ln(mu^2 / mu2)); |M|^2 is rescaled by (alpha_s(mu^2)/alpha_s)^n_g.
+ * on == 0 restores the fixed scale.  MF_EINVAL for MF_EE_MUMU. */
+int mf_set_dynamic_scale(mf_process *p, int32_t on);
+
 /* Observable histograms accumulated in the same pass ("histogram accumulation"; L109-119, Fig. 2:
  * d sigma / d pT,top and d sigma / d eta,top).  Attaches a caller-owned DEVICE buffer d_obs[2][n_bins + 1] of doubles
  * to the handle; from then on every mf_vegas_iterate / mf_unweight call ADDS (never overwrites; the caller zeroes)

@@ -16,6 +16,7 @@ struct mfo_process {
   mfo_process_desc d;
   PdfTable pdf;
   int D = 0, nfinal = 0, ng = 0;  // ng = gluons including the two beams (0 for ee->mumu)
+  int dyn_scale = 0;              // mfo_set_dynamic_scale (R16)
   double tau_min = 0;
   std::vector<double> C_d;
   std::vector<long double> C_l;
@@ -113,11 +114,23 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   o.w = R(0);
   if (!o.pass) return;
   o.lum = R(1);
+  R mu2 = R(P.d.mu2), as_factor = R(1);
+  if (P.d.process != 0 && P.dyn_scale) {
+    // R16 (dynamic scale): mu_F^2 = mu_R^2 = m_t^2 + pT(top)^2, event by event; the strong coupling
+    // runs at one loop from its value alpha_s at the reference scale mu2 of the descriptor:
+    //   alpha_s(mu^2) = alpha_s / (1 + alpha_s b0 ln(mu^2 / mu2)),  b0 = (33 - 2 n_f) / (12 pi),  n_f = 5;
+    // |M|^2 ~ alpha_s^{n_g}, so it is rescaled by (alpha_s(mu^2) / alpha_s)^{n_g}.
+    R pt2 = cm[2][1] * cm[2][1] + cm[2][2] * cm[2][2];
+    mu2 = R(P.d.m_top) * R(P.d.m_top) + pt2;
+    R b0 = R(23) / (R(12) * r_pi<R>());
+    R ratio = R(1) / (R(1) + R(P.d.alpha_s) * b0 * r_log(mu2 / R(P.d.mu2)));
+    for (int g = 0; g < P.ng; ++g) as_factor = as_factor * ratio;
+  }
   if (P.d.process != 0) {
-    R f1 = pdf_xf<R>(P.pdf, o.x1, R(P.d.mu2)), f2 = pdf_xf<R>(P.pdf, o.x2, R(P.d.mu2));  // O8
+    R f1 = pdf_xf<R>(P.pdf, o.x1, mu2), f2 = pdf_xf<R>(P.pdf, o.x2, mu2);  // O8
     o.lum = f1 * f2 / (o.x1 * o.x2);
   }
-  o.me2 = matrix_element<R>(P, cm, 0, -1, nullptr, nullptr);     // O9-O11
+  o.me2 = matrix_element<R>(P, cm, 0, -1, nullptr, nullptr) * as_factor;     // O9-O11 (x R16 factor)
   // O12: f = lum/(2 shat) |M|^2 Phi J_tau J_y K ; w = f * J_vegas
   R f = o.lum / (R(2) * shat) * o.me2 * o.phi * jac_parton * R(P.d.gev2_to_pb);
   o.w = f * o.jac;
@@ -286,6 +299,11 @@ int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
   return 0;
 }
 int mfo_destroy_process(mfo_process* P) { delete P; return 0; }
+int mfo_set_dynamic_scale(mfo_process* P, int32_t on) {
+  if (!P || P->d.process == 0) return -1;
+  P->dyn_scale = on ? 1 : 0;
+  return 0;
+}
 int mfo_n_dims(const mfo_process* P, int32_t* D) { if (!P || !D) return -1; *D = P->D; return 0; }
 int mfo_n_final(const mfo_process* P, int32_t* n) { if (!P || !n) return -1; *n = P->nfinal; return 0; }
 int mfo_record_size(const mfo_process* P, int32_t* b) { if (!P || !b) return -1; *b = (P->nfinal + 2) * 32 + 16; return 0; }

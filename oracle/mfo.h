@@ -32,6 +32,9 @@ typedef struct {
 
 int mfo_create_process(const mfo_process_desc*, mfo_process** out);
 int mfo_destroy_process(mfo_process*);
+/* R16: on != 0 switches to the dynamic scale mu_F^2 = mu_R^2 = m_t^2 + pT(top)^2 with one-loop running alpha_s
+ * (n_f = 5) from the descriptor's alpha_s at its mu2; not for process 0 (-1) */
+int mfo_set_dynamic_scale(mfo_process*, int32_t on);
 int mfo_n_dims(const mfo_process*, int32_t* D);
 int mfo_n_final(const mfo_process*, int32_t* n);
 int mfo_record_size(const mfo_process*, int32_t* bytes);

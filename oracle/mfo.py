@@ -66,6 +66,7 @@ def lib():
         L.mfo_count_ops_me2.argtypes = [C.c_void_p, c_double_p, c_u64_p]
         L.mfo_count_ops_event.argtypes = [C.c_void_p, c_double_p, C.c_uint64, C.c_uint32, C.c_uint64, c_u64_p]
         L.mfo_colour_matrix.argtypes = [C.c_int, c_double_p]
+        L.mfo_set_dynamic_scale.argtypes = [C.c_void_p, C.c_int32]
     return _lib
 
 
@@ -230,6 +231,9 @@ class Process:
         rc = lib().mfo_debug_eval(self.h, _dp(grid), seed, iteration, first_event, n_events, _dp(out), prec)
         assert rc == 0
         return out
+
+    def set_dynamic_scale(self, on):
+        assert lib().mfo_set_dynamic_scale(self.h, 1 if on else 0) == 0
 
     def pdf_xf(self, x, q2, prec=0):
         return lib().mfo_pdf_xf(self.h, x, q2, prec)

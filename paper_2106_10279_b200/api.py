@@ -27,7 +27,7 @@ c_double_p = C.POINTER(C.c_double)
 # every symbol include/mf.h declares (tests check the library exports each one)
 EXPORTS = ["mf_create_process", "mf_destroy_process", "mf_n_dims", "mf_n_final", "mf_record_size",
            "mf_debug_row_len", "mf_last_error", "mf_launch_config", "mf_vegas_iterate", "mf_refine_grid",
-           "mf_unweight", "mf_set_observables", "mf_debug_eval", "mf_debug_philox", "mf_debug_pdf", "mf_debug_me2",
+           "mf_unweight", "mf_set_dynamic_scale", "mf_set_observables", "mf_debug_eval", "mf_debug_philox", "mf_debug_pdf", "mf_debug_me2",
            "mf_measure_fp64_peak"]
 
 
@@ -69,6 +69,7 @@ def lib():
         L.mf_refine_grid.argtypes = [vp, vp, vp, C.c_double, vp]
         L.mf_unweight.argtypes = [vp, vp, u64, u32, u64, u64, C.c_double, vp, u64, vp, vp, vp, vp]
         L.mf_set_observables.argtypes = [vp, vp, C.c_int32, C.c_double, C.c_double]
+        L.mf_set_dynamic_scale.argtypes = [vp, C.c_int32]
         L.mf_debug_eval.argtypes = [vp, vp, u64, u32, u64, u64, vp, vp]
         L.mf_debug_philox.argtypes = [u64, u32, u64, u64, u32, vp, vp]
         L.mf_debug_pdf.argtypes = [vp, vp, vp, u64, vp, vp]
@@ -230,6 +231,10 @@ class Process:
                            records.data_ptr() if records is not None else None, capacity, count.data_ptr(),
                            hist.data_ptr() if hist is not None else None, result.data_ptr(), _stream_ptr(stream)),
                self.h, "mf_unweight")
+
+    def set_dynamic_scale(self, on):
+        """mu^2 = m_t^2 + pT(top)^2 per event with one-loop running alpha_s (include/mf.h)"""
+        _check(lib().mf_set_dynamic_scale(self.h, 1 if on else 0), self.h, "mf_set_dynamic_scale")
 
     def set_observables(self, obs, n_bins=0, pt_max=0.0, eta_max=0.0):
         """attach a zeroed float64 CUDA tensor [2, n_bins + 1] (pT and eta of the first final-state particle); None detaches"""

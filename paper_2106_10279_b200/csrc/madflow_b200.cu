@@ -92,7 +92,7 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   if (unw && (!d_count || !(w_max > 0.0))) return fail(p, MF_EINVAL, "mf_unweight needs d_count and w_max > 0");
   if (unw && capacity > 0 && !d_records) return fail(p, MF_EINVAL, "capacity > 0 with d_records == NULL");
   mf::PassArgs A;
-  A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row;
+  A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row; A.pdf_lnq2 = p->d_lnq2; A.pdf_xf = p->d_xf;
   A.seed = seed; A.first_event = first_event; A.n_events = n_events; A.iteration = iteration;
   A.w_max = w_max; A.records = (char*)d_records; A.capacity = capacity; A.count = (unsigned long long*)d_count;
   A.partials = p->d_partials; A.hist_part = d_hist ? p->d_hist_part : nullptr;
@@ -234,6 +234,13 @@ int mf_launch_config(const mf_process* p, int32_t* blocks, int32_t* threads) {
   return MF_OK;
 }
 
+int mf_set_dynamic_scale(mf_process* p, int32_t on) {
+  if (!p) return MF_EINVAL;
+  if (p->process == 0) return fail(p, MF_EINVAL, "mf_set_dynamic_scale: the leptonic process has no scale");
+  p->P.dyn_scale = on ? 1 : 0;
+  return MF_OK;
+}
+
 int mf_set_observables(mf_process* p, double* d_obs, int32_t n_bins, double pt_max, double eta_max) {
   if (!p) return MF_EINVAL;
   if (!d_obs) { p->d_obs = nullptr; p->obs_nb = 0; return MF_OK; }
@@ -271,7 +278,7 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
   if (n_events == 0) return MF_OK;
   mf::PassArgs A;
   std::memset(&A, 0, sizeof(A));
-  A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row;
+  A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row; A.pdf_lnq2 = p->d_lnq2; A.pdf_xf = p->d_xf;
   A.seed = seed; A.first_event = first_event; A.n_events = n_events; A.iteration = iteration;
   cudaStream_t st = (cudaStream_t)stream;
   const unsigned blocks = (unsigned)((n_events + mf::kThreads - 1) / mf::kThreads);

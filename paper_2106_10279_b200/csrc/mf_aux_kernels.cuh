@@ -75,8 +75,9 @@ __global__ void __launch_bounds__(kThreads) debug_eval_kernel(const Params P, co
     for (int c = 0; c < 4; ++c) *q++ = mom[i][c];
   double lum = 0.0, me2 = 0.0, w = 0.0;
   if (ev.pass) {
-    lum = luminosity<PROC>(P, A.pdf_lnx, A.pdf_row, ev.x1, ev.x2);
-    me2 = me2_call<PROC>(P, ev.shat, ev.k);
+    double asf;
+    lum = luminosity<PROC>(P, A, A.pdf_lnx, A.pdf_row, ev, asf);
+    me2 = me2_call<PROC>(P, ev.shat, ev.k) * asf;
     w = event_weight<PROC>(P, ev, lum, me2);
   }
   q[0] = ev.x1; q[1] = ev.x2; q[2] = lum; q[3] = me2; q[4] = ev.phi; q[5] = ev.jac_vegas; q[6] = w;

@@ -44,6 +44,7 @@ struct Params {
   int pdf_nx, pdf_nq;
   int pdf_jq;          // Q^2 cell of mu2 (clamped), fixed per process
   double pdf_uq;       // (ln mu2 - lnq2[jq]) / (lnq2[jq+1]-lnq2[jq])
+  int dyn_scale;       // 1: mu^2 = m_t^2 + pT(top)^2 per event, running alpha_s (mf_set_dynamic_scale; R16)
 };
 
 }  // namespace mf

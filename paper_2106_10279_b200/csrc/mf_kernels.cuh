@@ -27,6 +27,8 @@ struct PassArgs {
   const double* grid;      // [D][nb+1] device
   const double* pdf_lnx;   // [nx] device (nullptr for e+e-)
   const double* pdf_row;   // [nx] device: table collapsed at mu2
+  const double* pdf_lnq2;  // [nq] device, and the full table [nx][nq]: the dynamic-scale path only
+  const double* pdf_xf;
   uint64_t seed, first_event, n_events;
   uint32_t iteration;
   double w_max;            // unweighting only
@@ -47,13 +49,28 @@ __device__ __noinline__ double me2_call(const Params& P, double shat, const doub
   return matrix_element<PROC>(P, shat, k);
 }
 
-// Luminosity (step a6): F(x1) F(x2) / (x1 x2) with F the interpolant of the collapsed row in shared memory.
+// Luminosity (step a6): F(x1) F(x2) / (x1 x2) with F the interpolant of the collapsed row in shared memory; and
+// the factor that rescales |M|^2 (1 at the fixed scale).  Dynamic scale (R16; mf_set_dynamic_scale):
+// mu_F^2 = mu_R^2 = m_t^2 + pT(top)^2 per event, F by the general 2-D lookup in the table (global memory / L2),
+// alpha_s running at one loop (n_f = 5) from its value at the descriptor's mu2: |M|^2 ~ alpha_s^{n_g}.
 template <int PROC>
-MF_D double luminosity(const Params& P, const double* s_lnx, const double* s_row, double x1, double x2) {
+MF_D double luminosity(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                       const Event<PROC>& ev, double& as_factor) {
+  as_factor = 1.0;
   if (PROC == 0) return 1.0;
-  double f1 = pdf_xf_row(s_lnx, s_row, P.pdf_nx, x1);
-  double f2 = pdf_xf_row(s_lnx, s_row, P.pdf_nx, x2);
-  return f1 * f2 / (x1 * x2);
+  double f1, f2;
+  if (P.dyn_scale) {
+    const double mu2 = P.m_top * P.m_top + ev.k[0][1] * ev.k[0][1] + ev.k[0][2] * ev.k[0][2];
+    f1 = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf, P.pdf_nx, P.pdf_nq, ev.x1, mu2);
+    f2 = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf, P.pdf_nx, P.pdf_nq, ev.x2, mu2);
+    const double ratio = 1.0 / (1.0 + P.alpha_s * (23.0 / (12.0 * kPi)) * log(mu2 / P.mu2));
+#pragma unroll
+    for (int g = 0; g < Traits<PROC>::NG; ++g) as_factor *= ratio;
+  } else {
+    f1 = pdf_xf_row(s_lnx, s_row, P.pdf_nx, ev.x1);
+    f2 = pdf_xf_row(s_lnx, s_row, P.pdf_nx, ev.x2);
+  }
+  return f1 * f2 / (ev.x1 * ev.x2);
 }
 
 // Lab-frame momenta of an event, beams first (record / debug-row layout).
@@ -225,8 +242,9 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
       if (ev.pass && A.obs != nullptr) obs_bins = observable_bins<PROC>(A, ev);
       if (ev.pass) {
         ++acc.n_pass;
-        double lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
-        double me2 = me2_call<PROC>(P, ev.shat, ev.k);
+        double asf;
+        double lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
+        double me2 = me2_call<PROC>(P, ev.shat, ev.k) * asf;
         w = event_weight<PROC>(P, ev, lum, me2);
       }
     }

@@ -192,11 +192,11 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
     bins.clear();
     Event<PROC> ev;
     ev.pass = false;
-    double lum = 0.0;
+    double lum = 0.0, asf = 1.0;
     if (valid) {
       DebugRow dbg = {nullptr, D, NF};
       generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
-      if (ev.pass) lum = luminosity<PROC>(P, s_lnx, s_row, ev.x1, ev.x2);
+      if (ev.pass) lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
     }
     const bool pass = valid && ev.pass;
     const int obs_bins = (pass && A.obs != nullptr) ? observable_bins<PROC>(A, ev) : 0;
@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
-      w = event_weight<PROC>(P, ev, lum, me2);
+      w = event_weight<PROC>(P, ev, lum, me2 * asf);
     }
     accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins);
   }
@@ -250,8 +250,8 @@ __global__ void __launch_bounds__(kCoopDebugThreads) debug_eval_coop_kernel(cons
     generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
   }
   const bool pass = valid && ev.pass;
-  const double me2 = coop_block_me2<PG, 1>(L.teams, kCoopDebugThreads / PG::Team, L.s_tab, L.s_cnt, L.s_res, L.queue, 0u,
-                                           pass, ev.k, ev.shat, P);
+  double me2 = coop_block_me2<PG, 1>(L.teams, kCoopDebugThreads / PG::Team, L.s_tab, L.s_cnt, L.s_res, L.queue, 0u,
+                                     pass, ev.k, ev.shat, P);
   if (!valid) return;
   double mom[NF + 2][4];
   lab_momenta<PROC>(ev, mom);
@@ -260,7 +260,9 @@ __global__ void __launch_bounds__(kCoopDebugThreads) debug_eval_coop_kernel(cons
     for (int c = 0; c < 4; ++c) *q++ = mom[i][c];
   double lum = 0.0, w = 0.0;
   if (pass) {
-    lum = luminosity<PROC>(P, A.pdf_lnx, A.pdf_row, ev.x1, ev.x2);
+    double asf;
+    lum = luminosity<PROC>(P, A, A.pdf_lnx, A.pdf_row, ev, asf);
+    me2 *= asf;
     w = event_weight<PROC>(P, ev, lum, me2);
   }
   q[0] = ev.x1; q[1] = ev.x2; q[2] = lum; q[3] = me2; q[4] = ev.phi; q[5] = ev.jac_vegas; q[6] = w;

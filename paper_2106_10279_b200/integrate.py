@@ -167,6 +167,8 @@ def main(argv=None):
                          "(PAPER.md Fig. 2) in NBINS bins over the frozen-grid / last iteration and print them")
     ap.add_argument("--lhe", default="", metavar="FILE", help="unweighting configs (C4): drain the accepted events of every "
                     "frozen iteration asynchronously into this LHE 3.0 file (.gz = compressed; PAPER.md L81)")
+    ap.add_argument("--dynamic-scale", action="store_true",
+                    help="mu^2 = m_t^2 + pT(top)^2 per event with one-loop running alpha_s (mf_set_dynamic_scale)")
     ap.add_argument("--pt-max", type=float, default=600.0)
     ap.add_argument("--eta-max", type=float, default=3.0)
     args = ap.parse_args(argv)
@@ -174,6 +176,8 @@ def main(argv=None):
     if args.events > 0:
         wl = wl.scaled(args.events)
     proc = api.Process(wl, W.pdf_table() if wl.process else None)
+    if args.dynamic_scale:
+        proc.set_dynamic_scale(True)
     run_config(proc, wl.scaled(min(wl.n_events, 1 << 16)), capacity=args.capacity if wl.unweight else 0)   # warm-up
     torch.cuda.synchronize()
     drain = None

@@ -374,6 +374,35 @@ def test_other_bin_counts(proc, n, nb, pdf):
         gp.close()
 
 
+# ---- dynamic scale (R16) -----------------------------------------------------------------
+@pytest.mark.parametrize("proc,n", [(1, 6_001), (2, 2_001), (3, 601)])
+def test_dynamic_scale(proc, n, gpu_procs, oracle_procs):
+    """mu^2 = m_t^2 + pT(top)^2 per event, 2-D PDF lookup, running alpha_s: per-event rows and iteration sums against
+    the oracle in the same mode; switching back restores the fixed-scale results exactly."""
+    torch = _torch()
+    wl = WLS[proc]
+    gp, op = gpu_procs[proc], oracle_procs[proc]
+    grid = adapted_grid(op, wl)
+    dgrid = torch.from_numpy(grid).cuda()
+    fixed = gp.debug_eval(dgrid, 6, 1, 11, 300)
+    gp.set_dynamic_scale(True)
+    op.set_dynamic_scale(True)
+    try:
+        g = gp.debug_eval(dgrid, 6, 1, 11, 300)
+        o = op.debug_eval(grid, 6, 1, 11, 300)
+        _compare_rows(wl, g, o)
+        c = _cols(wl)
+        passed = fixed[:, c["pas"]] > 0
+        assert passed.sum() > 50 and np.all(g[passed, c["w"]] != fixed[passed, c["w"]])      # it does change the weights
+        hg, rg = _iterate_gpu(gp, grid, 6, 1, 0, n)
+        ho, ro = op.vegas_iterate(grid, 6, 1, 0, n)
+        _check_sums(n, hg, rg, ho, ro)
+    finally:
+        gp.set_dynamic_scale(False)
+        op.set_dynamic_scale(False)
+    assert np.array_equal(gp.debug_eval(dgrid, 6, 1, 11, 300), fixed)
+
+
 # ---- observable histograms (PAPER.md L61; Fig. 2) -------------------------------------------------------------------
 @pytest.mark.parametrize("proc,n", [(0, 30_011), (1, 20_001), (2, 4_001), (3, 1_003)])
 def test_observable_histograms(proc, n, gpu_procs, oracle_procs):

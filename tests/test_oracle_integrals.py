@@ -188,3 +188,38 @@ def test_multileg_event_rows_are_consistent(oracle_procs, pid):
         # Lorentz invariance ties the CM-frame |M|^2 to the lab-frame momenta stored in the row
         assert P.me2(mom) == pytest.approx(me2, rel=1e-9)
     assert 0.3 * len(rows) < npass < len(rows)
+
+
+# ---- R16: dynamic scale ----------------------------------------------------------------------------
+@pytest.mark.parametrize("wl,n", [(W.C1, 400), (W.C2, 200), (W.C3, 40)], ids=["C1", "C2", "C3"])
+def test_dynamic_scale_factorises(wl, n, pdf):
+    """mu^2 = m_t^2 + pT(top)^2 per event: every weight changes by exactly
+    [F(x1, mu^2) F(x2, mu^2)] / [F(x1, m_t^2) F(x2, m_t^2)] x (alpha_s(mu^2) / alpha_s)^{n_g}, with F the oracle's own
+    (separately pinned) interpolant and the one-loop alpha_s typed out here; everything else in the row is unchanged."""
+    op = mfo.Process(wl, pdf)
+    grid = W.uniform_grid(wl.n_dims)
+    fixed = op.debug_eval(grid, 2, 0, 0, n)
+    op.set_dynamic_scale(True)
+    dyn = op.debug_eval(grid, 2, 0, 0, n)
+    op.set_dynamic_scale(False)
+    assert np.array_equal(op.debug_eval(grid, 2, 0, 0, n), fixed)          # switching back restores the fixed scale
+    D, nf = wl.n_dims, wl.n_final
+    o = D + 4 * (nf + 2)
+    ng = {1: 2, 2: 3, 3: 4}[wl.process]
+    b0 = 23.0 / (12.0 * math.pi)
+    checked = 0
+    for f, d in zip(fixed, dyn):
+        assert np.array_equal(f[:o + 2], d[:o + 2]) and f[o + 7] == d[o + 7]      # kinematics, x1, x2, pass flag
+        if not f[o + 7]:
+            continue
+        top = f[D + 8:D + 12]                         # lab momentum; pT is boost invariant
+        mu2 = wl.m_top ** 2 + top[1] ** 2 + top[2] ** 2
+        x1, x2 = f[o], f[o + 1]
+        lum_ratio = (op.pdf_xf(x1, mu2) * op.pdf_xf(x2, mu2)) / (op.pdf_xf(x1, wl.mu2) * op.pdf_xf(x2, wl.mu2))
+        as_ratio = 1.0 / (1.0 + wl.alpha_s * b0 * math.log(mu2 / wl.mu2))
+        assert d[o + 2] == pytest.approx(f[o + 2] * lum_ratio, rel=1e-12)                  # lum
+        assert d[o + 3] == pytest.approx(f[o + 3] * as_ratio ** ng, rel=1e-12)             # |M|^2
+        assert d[o + 6] == pytest.approx(f[o + 6] * lum_ratio * as_ratio ** ng, rel=1e-11)  # w
+        assert as_ratio < 1.0 + 1e-15                 # mu^2 >= m_t^2: the coupling only decreases
+        checked += 1
+    assert checked > n // 3
