@@ -51,6 +51,19 @@ def _near_cut_edge(wl, row, c, tol=1e-9):
     return False
 
 
+_KNOTS = {}
+
+
+def _knot_scale(x):
+    """largest |x g| among the four ln x knots the Hermite interpolation at x uses, at any Q^2 of the table"""
+    if not _KNOTS:
+        lnx, lnq2, xf = W.pdf_table()
+        _KNOTS["lnx"], _KNOTS["absmax"] = lnx, np.abs(xf).max(axis=1)
+    lnx, am = _KNOTS["lnx"], _KNOTS["absmax"]
+    i = int(np.clip(np.searchsorted(lnx, np.log(x), side="right") - 1, 0, len(lnx) - 2))
+    return am[max(i - 1, 0):i + 3].max()
+
+
 def _compare_rows(wl, g, o):
     """element-by-element comparison of debug rows; returns the number of excluded cut-edge events"""
     c = _cols(wl)
@@ -73,9 +86,21 @@ def _compare_rows(wl, g, o):
             assert _near_cut_edge(wl, o[k], c), "pass flag differs away from a cut edge (event %d)" % k
             excluded += 1
             continue
-        for key in ("lum", "me2", "w"):
-            a, b = g[k, c[key]], o[k, c[key]]
-            assert abs(a - b) <= REL_EVENT * abs(b), (key, k, a, b)
+        # |M|^2: 1e-10 relative (BASELINE.json north_star).  Luminosity and weight: the same, plus the rounding of
+        # the Hermite interpolation where the interpolant of x g passes through ZERO (near x = 0.87 and 0.97 it changes
+        # sign, R8): there F is a difference of terms of the size of the neighbouring knot values, so two
+        # correct evaluation orders differ by a few ulp of THAT size, not of F.  Allowance: 4e-13 x the knot scale.
+        a, b = g[k, c["me2"]], o[k, c["me2"]]
+        assert abs(a - b) <= REL_EVENT * abs(b), ("me2", k, a, b)
+        lum_g, lum_o = g[k, c["lum"]], o[k, c["lum"]]
+        slack = 0.0
+        if wl.process:
+            x1, x2 = o[k, c["x1"]], o[k, c["x2"]]
+            slack = 4e-13 * _knot_scale(x1) * _knot_scale(x2) / (x1 * x2)
+        assert abs(lum_g - lum_o) <= REL_EVENT * abs(lum_o) + slack, ("lum", k, lum_g, lum_o)
+        wg, wo = g[k, c["w"]], o[k, c["w"]]
+        w_slack = abs(wo / lum_o) * slack if lum_o != 0.0 else 0.0
+        assert abs(wg - wo) <= REL_EVENT * abs(wo) + w_slack, ("w", k, wg, wo)
     return excluded
 
 
@@ -372,6 +397,22 @@ def test_other_bin_counts(proc, n, nb, pdf):
         _check_sums(n, hist.cpu().numpy(), gp.result_to_host(res), ho, ro)
     finally:
         gp.close()
+
+
+# ---- events at the zeros of the PDF interpolant ------------------------------------------------------------------------
+def test_rows_near_pdf_zero_crossings(gpu_procs, oracle_procs):
+    """The uniform-grid stream of gg -> ttbar g reaches x > 0.97, where the interpolant of x g changes sign and a
+    relative comparison of the luminosity alone is meaningless (one event of this range differs by 1.3e-10 relative
+    with |F| = 2e-9 against knot values of 1e-3): the rows must agree within 1e-10 relative plus the documented
+    interpolation-rounding allowance, and |M|^2 within 1e-10 relative."""
+    wl = WLS[2]
+    gp, op = gpu_procs[2], oracle_procs[2]
+    grid = W.uniform_grid(wl.n_dims)
+    g = gp.debug_eval(_torch().from_numpy(grid).cuda(), 0, 0, 0, 6000)
+    o = op.debug_eval(grid, 0, 0, 0, 6000)
+    c = _cols(wl)
+    assert (np.maximum(o[:, c["x1"]], o[:, c["x2"]]) > 0.97).sum() >= 3       # the range is reached
+    assert _compare_rows(wl, g, o) <= 1
 
 
 # ---- dynamic scale (SURVEY.md 8(f4); DESIGN.md R16) -----------------------------------------------------------------
