@@ -383,6 +383,50 @@ template <class R> inline std::vector<R> colour_matrix(int n) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// O10 (quark channel, "pp -> ttbar": the q qbar diagram beside the three gg ones).
+// q(p1, colour i) qbar(p2, colour j) -> t(p3, colour k) tbar(p4, colour l), massless q, s-channel gluon only:
+//   iM = [v-bar(p2) (i g T^a_{ji} gamma^mu) u(p1)] (-i g_{mu nu} delta^{ab} / s) [u-bar(p3) (i g T^b_{kl} gamma^nu) v(p4)]
+// Returns (1/4)(1/9) sum over helicities and colours of |M|^2.  The colour sum
+//   sum_{ijkl} | sum_a T^a_{ji} T^a_{kl} |^2
+// is evaluated from the explicit generators, not typed in.
+template <class R>
+inline R me2_qq_ttbar(const R mom[4][4], R mt, R alpha_s, int basis) {
+  R g2 = R(4) * r_pi<R>() * alpha_s;
+  R P[4];
+  for (int m = 0; m < 4; ++m) P[m] = mom[0][m] + mom[1][m];
+  R s = mdot_rr(P, P);
+  R colour = R(0);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j)
+      for (int k = 0; k < 3; ++k)
+        for (int l = 0; l < 3; ++l) {
+          Cx<R> c;
+          for (int a = 0; a < 8; ++a) {
+            Mat3<R> T = su3_generator<R>(a);
+            c += T.m[j][i] * T.m[k][l];
+          }
+          colour = colour + norm2(c);
+        }
+  R total = R(0);
+  for (int l1 = -1; l1 <= 1; l1 += 2)
+    for (int l2 = -1; l2 <= 1; l2 += 2)
+      for (int l3 = -1; l3 <= 1; l3 += 2)
+        for (int l4 = -1; l4 <= 1; l4 += 2) {
+          Spinor<R> u1 = u_spinor(mom[0], R(0), l1, basis), v2b = bar(v_spinor(mom[1], R(0), l2, basis));
+          Spinor<R> u3b = bar(u_spinor(mom[2], mt, l3, basis)), v4 = v_spinor(mom[3], mt, l4, basis);
+          CVec4<R> jq, jt;
+          for (int mu = 0; mu < 4; ++mu) {
+            Mat4<R> g = gamma_matrix<R>(mu);
+            jq.c[mu] = row_times_col(v2b, mat_vec(g, u1));
+            jt.c[mu] = row_times_col(u3b, mat_vec(g, v4));
+          }
+          Cx<R> M = cx_i<R>() * (mdot(jq, jt) * (g2 / s));   // i g * (-i / s) * i g, colour factor apart
+          total = total + norm2(M);
+        }
+  return total * colour / R(36);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Helicity-summed, colour-summed, averaged |M|^2 for g g -> t tbar (ng-2) g   (O10 + O11).
 // mom = [g_a, g_b, t, tbar, g_1.., ] physical momenta (beams incoming, the rest outgoing).
 // |M|^2_avg = 1/(4 * 64 * (ng-2)!) sum_h A_h^dagger C A_h.

@@ -14,7 +14,8 @@ using namespace mfo;
 
 struct mfo_process {
   mfo_process_desc d;
-  PdfTable pdf;
+  PdfTable pdf;                   // the gluon (table 0)
+  std::vector<PdfTable> pdfq;     // process 4: quark and antiquark tables, [2 i] quark i, [2 i + 1] antiquark i
   int D = 0, nfinal = 0, ng = 0;  // ng = gluons including the two beams (0 for ee->mumu)
   int dyn_scale = 0;              // mfo_set_dynamic_scale (R16)
   double tau_min = 0;
@@ -49,6 +50,7 @@ template <class R> struct EventOut {
   R x[24];
   R mom[6][4];  // lab frame, beams first
   R x1, x2, lum, me2, phi, jac, w;
+  R lum_qq, me2_qq;  // process 4: the flavour-summed q qbar luminosity and the q qbar matrix element
   int pass;
 };
 
@@ -82,7 +84,7 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   } else {
     PartonKin<R> k = parton_fractions<R>(o.x[0], o.x[1], R(P.tau_min), s);  // O4
     y = k.y; shat = k.shat; jac_parton = k.jac; o.x1 = k.x1; o.x2 = k.x2;
-    if (P.d.process == 1) {
+    if (P.d.process == 1 || P.d.process == 4) {
       R m4[4][4];
       o.phi = two_body<R>(shat, R(P.d.m_top), o.x[2], o.x[3], m4);  // O5
       for (int i = 0; i < 4; ++i)
@@ -112,6 +114,8 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   o.lum = R(0);
   o.me2 = R(0);
   o.w = R(0);
+  o.lum_qq = R(0);
+  o.me2_qq = R(0);
   if (!o.pass) return;
   o.lum = R(1);
   R mu2 = R(P.d.mu2), as_factor = R(1);
@@ -133,6 +137,30 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   o.me2 = matrix_element<R>(P, cm, 0, -1, nullptr, nullptr) * as_factor;     // O9-O11 (x R16 factor)
   // O12: f = lum/(2 shat) |M|^2 Phi J_tau J_y K ; w = f * J_vegas
   R f = o.lum / (R(2) * shat) * o.me2 * o.phi * jac_parton * R(P.d.gev2_to_pb);
+  if (P.d.process == 4) {
+    // quark channels: for every flavour the quark may come from either beam,
+    //   sum_i [ q_i(x1) qbar_i(x2) |M|^2(q along +z) + qbar_i(x1) q_i(x2) |M|^2(q along -z) ] / (x1 x2),
+    // added to the gg term at the same phase-space point.  Both are O(alpha_s^2): the same R16 factor.
+    R ma[4][4], mb[4][4];
+    for (int i = 0; i < 4; ++i)
+      for (int m = 0; m < 4; ++m) { ma[i][m] = cm[i][m]; mb[i][m] = cm[i][m]; }
+    for (int m = 0; m < 4; ++m) { mb[0][m] = cm[1][m]; mb[1][m] = cm[0][m]; }   // quark from beam 2
+    R Ma = me2_qq_ttbar<R>(ma, R(P.d.m_top), R(P.d.alpha_s), 0) * as_factor;
+    R Mb = me2_qq_ttbar<R>(mb, R(P.d.m_top), R(P.d.alpha_s), 0) * as_factor;
+    R La = R(0), Lb = R(0);
+    for (size_t i = 0; i + 1 < P.pdfq.size(); i += 2) {
+      R q1 = pdf_xf<R>(P.pdfq[i], o.x1, mu2), qb1 = pdf_xf<R>(P.pdfq[i + 1], o.x1, mu2);
+      R q2 = pdf_xf<R>(P.pdfq[i], o.x2, mu2), qb2 = pdf_xf<R>(P.pdfq[i + 1], o.x2, mu2);
+      La = La + q1 * qb2;
+      Lb = Lb + qb1 * q2;
+    }
+    La = La / (o.x1 * o.x2);
+    Lb = Lb / (o.x1 * o.x2);
+    o.lum_qq = La + Lb;
+    R both = La * Ma + Lb * Mb;
+    o.me2_qq = (o.lum_qq != R(0)) ? both / o.lum_qq : Ma;     // the luminosity-weighted mean of the two orientations
+    f = (o.lum * o.me2 + both) / (R(2) * shat) * o.phi * jac_parton * R(P.d.gev2_to_pb);
+  }
   o.w = f * o.jac;
 }
 
@@ -198,7 +226,7 @@ template <class R>
 int debug_eval(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteration, uint64_t first, uint64_t n_events,
                double* out) {
   const int D = P.D, n = P.nfinal;
-  const int rowlen = 3 * D + 4 * (n + 2) + 9;
+  const int rowlen = 3 * D + 4 * (n + 2) + 9 + (P.d.process == 4 ? 2 : 0);
   EventOut<R> o;
   for (uint64_t k = 0; k < n_events; ++k) {
     uint64_t e = first + k;
@@ -219,6 +247,10 @@ int debug_eval(mfo_process& P, const double* grid, uint64_t seed, uint32_t itera
     row[c++] = accept_draw(seed, iteration, e);
     for (int d = 0; d < D; ++d) row[c++] = o.u[d];
     for (int d = 0; d < D; ++d) row[c++] = (double)o.bin[d];
+    if (P.d.process == 4) {
+      row[c++] = r_to_double(o.lum_qq);
+      row[c++] = r_to_double(o.me2_qq);
+    }
   }
   return 0;
 }
@@ -272,10 +304,10 @@ extern "C" {
 
 int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
   if (!d || !out) return -1;
-  if (d->process < 0 || d->process > 3 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
+  if (d->process < 0 || d->process > 4 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
   std::unique_ptr<mfo_process> P(new mfo_process);
   P->d = *d;
-  static const int Dtab[4] = {2, 4, 14, 18}, ntab[4] = {2, 2, 3, 4}, ngtab[4] = {0, 2, 3, 4};
+  static const int Dtab[5] = {2, 4, 14, 18, 4}, ntab[5] = {2, 2, 3, 4, 2}, ngtab[5] = {0, 2, 3, 4, 2};
   P->D = Dtab[d->process];
   P->nfinal = ntab[d->process];
   P->ng = ngtab[d->process];
@@ -286,6 +318,15 @@ int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
     P->pdf.lnx.assign(d->pdf_lnx, d->pdf_lnx + d->pdf_nx);
     P->pdf.lnq2.assign(d->pdf_lnq2, d->pdf_lnq2 + d->pdf_nq);
     P->pdf.xf.assign(d->pdf_xf, d->pdf_xf + (size_t)d->pdf_nx * d->pdf_nq);
+    if (d->process == 4) {
+      if (d->pdf_nfl < 3 || d->pdf_nfl % 2 == 0) return -1;
+      for (int t = 1; t < d->pdf_nfl; ++t) {
+        PdfTable T = P->pdf;
+        const double* src = d->pdf_xf + (size_t)t * d->pdf_nx * d->pdf_nq;
+        T.xf.assign(src, src + (size_t)d->pdf_nx * d->pdf_nq);
+        P->pdfq.push_back(T);
+      }
+    }
     double lq = std::log(d->mu2);
     if (!(lq >= P->pdf.lnq2.front() && lq <= P->pdf.lnq2.back())) return -4;
     int ncut = P->nfinal - 2;
@@ -309,7 +350,7 @@ int mfo_n_final(const mfo_process* P, int32_t* n) { if (!P || !n) return -1; *n 
 int mfo_record_size(const mfo_process* P, int32_t* b) { if (!P || !b) return -1; *b = (P->nfinal + 2) * 32 + 16; return 0; }
 int mfo_debug_row_len(const mfo_process* P, int32_t* n) {
   if (!P || !n) return -1;
-  *n = 3 * P->D + 4 * (P->nfinal + 2) + 9;
+  *n = 3 * P->D + 4 * (P->nfinal + 2) + 9 + (P->d.process == 4 ? 2 : 0);
   return 0;
 }
 
@@ -394,6 +435,27 @@ double mfo_pdf_xf(const mfo_process* P, double x, double q2, int prec) {
   if (prec == 2) return (double)pdf_xf<__float128>(P->pdf, x, q2);
   if (prec == 1) return (double)pdf_xf<long double>(P->pdf, x, q2);
   return pdf_xf<double>(P->pdf, x, q2);
+}
+double mfo_pdf_xf_table(const mfo_process* P, int table, double x, double q2, int prec) {
+  if (table == 0) return mfo_pdf_xf(P, x, q2, prec);
+  if (table < 0 || (size_t)table > P->pdfq.size()) return 0.0;
+  const PdfTable& T = P->pdfq[table - 1];
+  if (prec == 2) return (double)pdf_xf<__float128>(T, x, q2);
+  if (prec == 1) return (double)pdf_xf<long double>(T, x, q2);
+  return pdf_xf<double>(T, x, q2);
+}
+double mfo_me2_qq(const mfo_process* P, const double* mom, int basis, int prec) {
+  if (!P || P->d.process != 4 || !mom) return -1.0;
+  if (prec == 1) {
+    long double m[4][4];
+    for (int i = 0; i < 4; ++i)
+      for (int c = 0; c < 4; ++c) m[i][c] = mom[4 * i + c];
+    return (double)me2_qq_ttbar<long double>(m, P->d.m_top, P->d.alpha_s, basis);
+  }
+  double m[4][4];
+  for (int i = 0; i < 4; ++i)
+    for (int c = 0; c < 4; ++c) m[i][c] = mom[4 * i + c];
+  return me2_qq_ttbar<double>(m, P->d.m_top, P->d.alpha_s, basis);
 }
 int mfo_colour_matrix(int n, double* out) {
   if (n < 1 || n > 5) return -1;

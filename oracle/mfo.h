@@ -13,7 +13,7 @@ typedef struct mfo_process mfo_process;
 
 /* same field order and meaning as mf_process_desc (include/mf.h) */
 typedef struct {
-  int32_t process; /* 0 ee->mumu, 1 gg->tt, 2 gg->ttg, 3 gg->ttgg */
+  int32_t process; /* 0 ee->mumu, 1 gg->tt, 2 gg->ttg, 3 gg->ttgg, 4 pp->tt (gg + q qbar, flavour summed) */
   double sqrt_s;
   double alpha_em, alpha_s;
   double m_top;
@@ -22,7 +22,8 @@ typedef struct {
   double gev2_to_pb;
   int32_t n_bins;
   int32_t pdf_nx, pdf_nq;
-  const double *pdf_lnx, *pdf_lnq2, *pdf_xf;
+  const double *pdf_lnx, *pdf_lnq2, *pdf_xf; /* pdf_xf[max(pdf_nfl,1)][pdf_nx][pdf_nq]: table 0 gluon, 1+2i quark i, 2+2i antiquark i */
+  int32_t pdf_nfl;                           /* parton tables: 0 or 1 = gluon only; process 4 needs 1 + 2 n_f (odd, >= 3)          */
 } mfo_process_desc;
 
 typedef struct {
@@ -49,11 +50,16 @@ int mfo_refine_grid(mfo_process*, double* grid, const double* hist, double alpha
 int mfo_unweight(mfo_process*, const double* grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                  uint64_t n_events, double w_max, void* records, uint64_t capacity, uint64_t* count, double* hist,
                  mfo_iter_result* result, int prec);
-/* per-event rows:  x[D] | (n+2)x(E,px,py,pz) lab | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D] */
+/* per-event rows:  x[D] | (n+2)x(E,px,py,pz) lab | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D]
+ * process 4 appends | lum_qq | me2_qq (lum, me2 = the gg channel; w = the sum of both channels) */
 int mfo_debug_eval(mfo_process*, const double* grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                    uint64_t n_events, double* out, int prec);
 
 /* ---- component entry points for the pins --------------------------------------------------- */
+/* averaged |M|^2 of q(mom[0]) qbar(mom[1]) -> t(mom[2]) tbar(mom[3]) (process 4 only) */
+double mfo_me2_qq(const mfo_process*, const double* mom, int basis, int prec);
+/* x f(x, q2) of parton table `table` (0 gluon, 1+2i quark i, 2+2i antiquark i) */
+double mfo_pdf_xf_table(const mfo_process*, int table, double x, double q2, int prec);
 void mfo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 void mfo_philox_block(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]);
 double mfo_uniform_from_words(uint32_t hi, uint32_t lo);

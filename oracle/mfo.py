@@ -23,7 +23,8 @@ class ProcessDesc(C.Structure):
     _fields_ = [("process", C.c_int32), ("sqrt_s", C.c_double), ("alpha_em", C.c_double), ("alpha_s", C.c_double),
                 ("m_top", C.c_double), ("mu2", C.c_double), ("ptmin", C.c_double), ("etamax", C.c_double),
                 ("drmin", C.c_double), ("gev2_to_pb", C.c_double), ("n_bins", C.c_int32), ("pdf_nx", C.c_int32),
-                ("pdf_nq", C.c_int32), ("pdf_lnx", c_double_p), ("pdf_lnq2", c_double_p), ("pdf_xf", c_double_p)]
+                ("pdf_nq", C.c_int32), ("pdf_lnx", c_double_p), ("pdf_lnq2", c_double_p), ("pdf_xf", c_double_p),
+                ("pdf_nfl", C.c_int32)]
 
 
 class IterResult(C.Structure):
@@ -67,6 +68,10 @@ def lib():
         L.mfo_count_ops_event.argtypes = [C.c_void_p, c_double_p, C.c_uint64, C.c_uint32, C.c_uint64, c_u64_p]
         L.mfo_colour_matrix.argtypes = [C.c_int, c_double_p]
         L.mfo_set_dynamic_scale.argtypes = [C.c_void_p, C.c_int32]
+        L.mfo_me2_qq.restype = C.c_double
+        L.mfo_me2_qq.argtypes = [C.c_void_p, c_double_p, C.c_int, C.c_int]
+        L.mfo_pdf_xf_table.restype = C.c_double
+        L.mfo_pdf_xf_table.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_int]
     return _lib
 
 
@@ -178,6 +183,7 @@ class Process:
             lnx, lnq2, xf = (_f64(a) for a in pdf)
             self._keep = (lnx, lnq2, xf)
             d.pdf_nx, d.pdf_nq = len(lnx), len(lnq2)
+            d.pdf_nfl = xf.shape[0] if xf.ndim == 3 else 1
             d.pdf_lnx, d.pdf_lnq2, d.pdf_xf = _dp(lnx), _dp(lnq2), _dp(xf)
         h = C.c_void_p()
         rc = lib().mfo_create_process(C.byref(d), C.byref(h))
@@ -238,13 +244,21 @@ class Process:
     def pdf_xf(self, x, q2, prec=0):
         return lib().mfo_pdf_xf(self.h, x, q2, prec)
 
+    def pdf_xf_table(self, table, x, q2, prec=0):
+        return lib().mfo_pdf_xf_table(self.h, table, x, q2, prec)
+
+    def me2_qq(self, mom, basis=0, prec=0):
+        """averaged |M|^2 of q(mom[0]) qbar(mom[1]) -> t(mom[2]) tbar(mom[3]); process 4 only"""
+        mom = _f64(mom)
+        return lib().mfo_me2_qq(self.h, _dp(mom), basis, prec)
+
     def me2(self, mom, basis=0, subst_gluon=-1, prec=0, want_amps=False, want_per_hel=False):
         mom = _f64(mom)
         amps = per = None
         ap = pp = None
         if want_amps:
             import math
-            ng = {1: 2, 2: 3, 3: 4}[self.wl.process]
+            ng = {1: 2, 2: 3, 3: 4, 4: 2}[self.wl.process]
             amps = np.zeros(((4 << ng), math.factorial(ng), 2))
             ap = _dp(amps)
         if want_per_hel:

@@ -13,10 +13,12 @@ import math
 import numpy as np
 
 MF_EE_MUMU, MF_GG_TT, MF_GG_TTG, MF_GG_TTGG = 0, 1, 2, 3
+MF_PP_TT = 4               # gg -> ttbar + the q qbar -> ttbar channels of four flavours
 GEV2_TO_PB = 0.3894e9  # BASELINE.json configs[0]: use this literal everywhere
 N_BINS = 50
-N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18}
-N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4}
+N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18, MF_PP_TT: 4}
+N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4, MF_PP_TT: 2}
+N_FLAVOURS = 4             # quark flavours of the multi-flavour table: d, u, s, c (3 gg + 4 q qbar = the 7 diagrams of PAPER.md L101)
 VEGAS_ALPHA = 1.5
 
 
@@ -64,6 +66,10 @@ C3 = Workload("C3 gg -> ttbar gg", MF_GG_TTGG, sqrt_s=13000.0, ptmin=30.0, etama
 C4 = Workload("C4 gg -> ttbar gg + unweighting", MF_GG_TTGG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5, drmin=0.4,
               n_events=2 ** 26, n_iterations=10, n_adapt=5, unweight=True)
 CONFIGS = [C0, C1, C2, C3, C4]
+# beyond BASELINE.json: the flavour-summed pp -> ttbar of PAPER.md L101 ("pp -> ttbar (7 diagrams)":
+# 3 gg + one q qbar diagram for each of 4 flavours), gluon and quark channels in ONE pass over the same points
+C5 = Workload("C5 pp -> ttbar (gg + q qbar)", MF_PP_TT, sqrt_s=13000.0, n_events=2 ** 20, n_iterations=10, n_adapt=10)
+EXTRA_CONFIGS = {"C5": C5}
 
 
 def pdf_table(nx=100, nq=50):
@@ -81,6 +87,36 @@ def pdf_table(nx=100, nq=50):
     q2 = np.exp(lnq2)
     xf = 3.0 * x[:, None] ** -0.1 * (1.0 - x[:, None]) ** 5 * (1.0 + 0.1 * np.log(q2[None, :] / 100.0))
     return np.ascontiguousarray(lnx), np.ascontiguousarray(lnq2), np.ascontiguousarray(xf)
+
+
+def pdf_table_flavours(nx=100, nq=50):
+    """Synthetic multi-flavour table for MF_PP_TT on the knots of pdf_table: xf[1 + 2 N_FLAVOURS][nx][nq] with
+    table 0 the gluon of pdf_table, table 1 + 2 i the quark of flavour i (d, u, s, c) and table 2 + 2 i its
+    antiquark.  With L = ln(Q^2 / 100 GeV^2):
+        sea_i   = c_i x^-0.1 (1-x)^7 (1 + 0.15 L),     c = (0.20, 0.18, 0.10, 0.03)
+        valence = 1.1 x^0.6 (1-x)^4 (1 + 0.05 L) for d,  2.2 x^0.6 (1-x)^3 (1 + 0.05 L) for u,  0 otherwise
+        x qbar_i = sea_i,   x q_i = valence_i + sea_i
+    (shapes of the kind a proton set has: valence peaks, a steep sea; the numbers are this repository's own)."""
+    lnx, lnq2, xg = pdf_table(nx, nq)
+    x = np.exp(lnx)[:, None]
+    x[-1] = 1.0
+    L = np.log(np.exp(lnq2)[None, :] / 100.0)
+    c = (0.20, 0.18, 0.10, 0.03)
+    val = (1.1 * x ** 0.6 * (1.0 - x) ** 4 * (1.0 + 0.05 * L), 2.2 * x ** 0.6 * (1.0 - x) ** 3 * (1.0 + 0.05 * L))
+    xf = np.zeros((1 + 2 * N_FLAVOURS, nx, nq))
+    xf[0] = xg
+    for i in range(N_FLAVOURS):
+        sea = c[i] * x ** -0.1 * (1.0 - x) ** 7 * (1.0 + 0.15 * L)
+        xf[2 + 2 * i] = sea
+        xf[1 + 2 * i] = sea + (val[i] if i < 2 else 0.0)
+    return lnx, lnq2, np.ascontiguousarray(xf)
+
+
+def pdf_for(process, nx=100, nq=50):
+    """the table a process needs: None, the gluon table, or the multi-flavour table"""
+    if process == MF_EE_MUMU:
+        return None
+    return pdf_table_flavours(nx, nq) if process == MF_PP_TT else pdf_table(nx, nq)
 
 
 def uniform_grid(n_dims, n_bins=N_BINS):
