@@ -39,8 +39,8 @@ UNIT = "events/s"
 # generator's static matrix-element count; profiles/r1_flops_per_event.md).  For the two thread-per-event kernels the
 # compiler folds the constant beam wavefunctions into the matrix element, so the static count overestimates: there
 # the measured TOTAL per event is used (ME_FLOPS_MEASURED) and OTHER_FLOPS is 0.
-OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0}
-ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0}
+OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0}
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5200.0}     # 4: estimate until calibrated
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
@@ -62,7 +62,7 @@ def me_flops(process):
 
 def config_by_name(name):
     from paper_2106_10279_b200 import workloads as W
-    return {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4}[name]
+    return {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4, **W.EXTRA_CONFIGS}[name]
 
 
 # ---- clocks ------------------------------------------------------------------------------------------------
@@ -108,7 +108,7 @@ def oracle_sample(wl, seconds=15.0, n_first=64):
     grid; n is sized from a short probe so the sample takes about `seconds`."""
     from oracle import mfo
     from paper_2106_10279_b200 import workloads as W
-    op = mfo.Process(wl, W.pdf_table())
+    op = mfo.Process(wl, W.pdf_for(wl.process))
     grid = W.uniform_grid(wl.n_dims, wl.n_bins)
     t0 = time.perf_counter()
     op.vegas_iterate(grid, wl.seed, 0, 0, n_first)
@@ -125,9 +125,9 @@ import sys, time
 sys.path.insert(0, sys.argv[1])
 from oracle import mfo
 from paper_2106_10279_b200 import workloads as W
-wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4}[sys.argv[2]]
+wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4, **W.EXTRA_CONFIGS}[sys.argv[2]]
 first, n = int(sys.argv[3]), int(sys.argv[4])
-op = mfo.Process(wl, W.pdf_table())
+op = mfo.Process(wl, W.pdf_for(wl.process))
 grid = W.uniform_grid(wl.n_dims, wl.n_bins)
 t0 = time.perf_counter()
 op.vegas_iterate(grid, wl.seed, 0, first, n)
@@ -155,9 +155,9 @@ def run_reference(args, wl):
         return
     from oracle import mfo
     from paper_2106_10279_b200 import workloads as W
-    op = mfo.Process(wl, W.pdf_table())
+    op = mfo.Process(wl, W.pdf_for(wl.process))
     grid = W.uniform_grid(wl.n_dims, wl.n_bins)
-    n = {0: 200000, 1: 40000, 2: 4000, 3: 400}[wl.process]     # ~2 s per step
+    n = {0: 200000, 1: 40000, 2: 4000, 3: 400, 4: 20000}[wl.process]     # ~2 s per step
     times = []
     for k in range(args.warmup + args.steps):
         t0 = time.perf_counter()
@@ -216,7 +216,7 @@ def main():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     build.build()
-    proc = api.Process(wl, W.pdf_table())
+    proc = api.Process(wl, W.pdf_for(wl.process))
     n = wl.n_events                                   # per rank (weak scaling: shards need no exchange until
     first_event = rank * n                            # the per-iteration sums)
     stream = torch.cuda.current_stream()

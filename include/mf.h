@@ -32,13 +32,16 @@ extern "C" {
 
 typedef struct mf_process mf_process; /* opaque; owns its device-side constants and scratch */
 
-/* process ids: BASELINE.json configs[0..3] */
-enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3 };
+/* process ids: 0..3 are BASELINE.json configs[0..3]; MF_PP_TT ("pp -> ttbar (7 diagrams)")
+ * adds to g g -> t tbar, at the same phase-space point and in the same pass, the q qbar -> t tbar channel of every
+ * quark flavour of a multi-flavour PDF table, the quark taken from either beam:
+ *   w ~ L_gg |M_gg|^2 + sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2) |M_qq|^2                                */
+enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3, MF_PP_TT = 4 };
 enum { MF_OK = 0, MF_EINVAL = -1, MF_ECUDA = -2, MF_EOVERFLOW = -3, MF_ERANGE = -4, MF_ENOMEM = -5 };
 
 /* Process descriptor (host memory; copied at create).  Same field order as the oracle's mfo_process_desc. */
 typedef struct {
-  int32_t process;            /* enum above; fixes n_final, D (2/4/14/18), helicities, colour matrix   */
+  int32_t process;            /* enum above; fixes n_final, D (2/4/14/18/4), helicities, colour matrix */
   double sqrt_s;              /* GeV; hadronic (pp) for processes 1-3, leptonic for 0                   */
   double alpha_em, alpha_s;   /* couplings: e^2 = 4 pi alpha_em, g_s^2 = 4 pi alpha_s                   */
   double m_top;               /* GeV; width 0                                                           */
@@ -49,7 +52,9 @@ typedef struct {
   int32_t pdf_nx, pdf_nq;     /* knots of the PDF table (0, 0 for MF_EE_MUMU)                           */
   const double *pdf_lnx;      /* [pdf_nx] ln x knots, increasing, last = 0                              */
   const double *pdf_lnq2;     /* [pdf_nq] ln Q^2 knots, increasing                                      */
-  const double *pdf_xf;       /* [pdf_nx][pdf_nq] x*g(x,Q^2), row-major xf[ix*nq+iq]                    */
+  const double *pdf_xf;       /* [pdf_nx][pdf_nq] x*g(x,Q^2), row-major xf[ix*nq+iq]; MF_PP_TT:         */
+                              /* [pdf_nfl][pdf_nx][pdf_nq], table 0 gluon, 1+2i quark i, 2+2i antiquark i */
+  int32_t pdf_nfl;            /* parton tables; read for MF_PP_TT only: 1 + 2 n_f, n_f = 1..5           */
 } mf_process_desc;
 #define MF_MAX_BINS 128
 
@@ -59,15 +64,15 @@ typedef struct {
   uint64_t n_pass, n_accept;       /* events passing the cuts; events accepted (mf_unweight only)      */
 } mf_iter_result;
 
-/* Creates a handle.  Errors: NULL / bad enum / n_bins out of range / bad table -> MF_EINVAL;
+/* Creates a handle.  Errors: NULL / bad enum / n_bins out of range / bad table or table count -> MF_EINVAL;
  * mu2 outside the Q^2 knots or tau_min below the x knots -> MF_ERANGE; no device or CUDA failure ->
  * MF_ECUDA; device allocation failure -> MF_ENOMEM.  On error *out is set to NULL. */
 int mf_create_process(const mf_process_desc *desc, mf_process **out);
 int mf_destroy_process(mf_process *p);
-int mf_n_dims(const mf_process *p, int32_t *D);              /* VEGAS dimensions: 2, 4, 14, 18          */
-int mf_n_final(const mf_process *p, int32_t *n);             /* final-state particles: 2, 2, 3, 4       */
+int mf_n_dims(const mf_process *p, int32_t *D);              /* VEGAS dimensions: 2, 4, 14, 18, 4       */
+int mf_n_final(const mf_process *p, int32_t *n);             /* final-state particles: 2, 2, 3, 4, 2    */
 int mf_record_size(const mf_process *p, int32_t *bytes);     /* (n_final+2)*32 + 16                     */
-int mf_debug_row_len(const mf_process *p, int32_t *n_doubles);/* 3*D + 4*(n_final+2) + 9                */
+int mf_debug_row_len(const mf_process *p, int32_t *n_doubles);/* 3*D + 4*(n_final+2) + 9 (+2: MF_PP_TT)  */
 const char *mf_last_error(const mf_process *p);              /* static or handle-owned string           */
 /* launch geometry of the fused pass (blocks, threads per block), for reporting */
 int mf_launch_config(const mf_process *p, int32_t *blocks, int32_t *threads);
@@ -113,7 +118,8 @@ int mf_set_dynamic_scale(mf_process *p, int32_t on);
 int mf_set_observables(mf_process *p, double *d_obs, int32_t n_bins, double pt_max, double eta_max);
 
 /* Test/diagnostic: per-event rows of mf_debug_row_len doubles, identical to the oracle's layout:
- * x[D] | (n+2)x(E,px,py,pz) lab, beams first | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D] */
+ * x[D] | (n+2)x(E,px,py,pz) lab, beams first | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D]
+ * MF_PP_TT appends | lum_qq | me2_qq  (lum, me2 are then the gg channel's; w is the sum of both channels) */
 int mf_debug_eval(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                   uint64_t n_events, double *d_out, void *stream);
 
@@ -121,9 +127,10 @@ int mf_debug_eval(mf_process *p, const double *d_grid, uint64_t seed, uint32_t i
  * d_out[4*n] uint32, block index b of event first_event+k at d_out[4*(k*n_blocks+b)..]. */
 int mf_debug_philox(uint64_t seed, uint32_t iteration, uint64_t first_event, uint64_t n_events, uint32_t n_blocks,
                     uint32_t *d_out, void *stream);
-/* Test/diagnostic: general 2-D log-bicubic PDF lookup x*g(x, q2) for n points (device arrays). */
+/* Test/diagnostic: general 2-D log-bicubic PDF lookup x*g(x, q2) (parton table 0) for n points (device arrays). */
 int mf_debug_pdf(mf_process *p, const double *d_x, const double *d_q2, uint64_t n, double *d_out, void *stream);
-/* Test/diagnostic: averaged |M|^2 at n sets of CM-frame momenta d_mom[n][n_final+2][4] (beams first). */
+/* Test/diagnostic: averaged |M|^2 at n sets of CM-frame momenta d_mom[n][n_final+2][4] (beams first) -> d_out[n];
+ * MF_PP_TT: d_out[n][2] = (g g -> t tbar, q qbar -> t tbar). */
 int mf_debug_me2(mf_process *p, const double *d_mom, uint64_t n, double *d_out, void *stream);
 
 /* Measurement helper: runs a dependent-free DFMA chain on every SM for `iters` iterations and returns the

@@ -40,7 +40,8 @@ class ProcessDesc(C.Structure):
     _fields_ = [("process", C.c_int32), ("sqrt_s", C.c_double), ("alpha_em", C.c_double), ("alpha_s", C.c_double),
                 ("m_top", C.c_double), ("mu2", C.c_double), ("ptmin", C.c_double), ("etamax", C.c_double),
                 ("drmin", C.c_double), ("gev2_to_pb", C.c_double), ("n_bins", C.c_int32), ("pdf_nx", C.c_int32),
-                ("pdf_nq", C.c_int32), ("pdf_lnx", c_double_p), ("pdf_lnq2", c_double_p), ("pdf_xf", c_double_p)]
+                ("pdf_nq", C.c_int32), ("pdf_lnx", c_double_p), ("pdf_lnq2", c_double_p), ("pdf_xf", c_double_p),
+                ("pdf_nfl", C.c_int32)]
 
 
 class IterResult(C.Structure):
@@ -148,6 +149,7 @@ def make_desc(wl, pdf=None):
             raise MfError("process %d needs a PDF table" % wl.process)
         keep = tuple(np.ascontiguousarray(a, dtype=np.float64) for a in pdf)
         d.pdf_nx, d.pdf_nq = len(keep[0]), len(keep[1])
+        d.pdf_nfl = keep[2].shape[0] if keep[2].ndim == 3 else 1
         d.pdf_lnx, d.pdf_lnq2, d.pdf_xf = (a.ctypes.data_as(c_double_p) for a in keep)
     return d, keep
 
@@ -264,7 +266,8 @@ class Process:
     def debug_me2(self, mom):
         torch = _torch()
         m = torch.as_tensor(np.ascontiguousarray(mom, dtype=np.float64)).cuda().reshape(-1, self.n_final + 2, 4)
-        out = torch.empty(m.shape[0], dtype=torch.float64, device="cuda")
+        shape = (m.shape[0], 2) if self.wl.process == 4 else (m.shape[0],)     # MF_PP_TT: (gg, q qbar) per point
+        out = torch.empty(shape, dtype=torch.float64, device="cuda")
         _check(mf_debug_me2(self.h, m.data_ptr(), m.shape[0], out.data_ptr(), _stream_ptr(None)), self.h,
                "mf_debug_me2")
         return out.cpu().numpy()

@@ -47,6 +47,7 @@ const void* pass_fn(int proc, bool unw) {
   switch (proc) {
     case 0: return unw ? pass_fn<0, true>() : pass_fn<0, false>();
     case 1: return unw ? pass_fn<1, true>() : pass_fn<1, false>();
+    case 4: return unw ? pass_fn<4, true>() : pass_fn<4, false>();
     case 2: return unw ? (const void*)mf::fused_pass_coop_kernel<2, true> : (const void*)mf::fused_pass_coop_kernel<2, false>;
     default: return unw ? (const void*)mf::fused_pass_coop_kernel<3, true> : (const void*)mf::fused_pass_coop_kernel<3, false>;
   }
@@ -119,14 +120,14 @@ extern "C" {
 int mf_create_process(const mf_process_desc* d, mf_process** out) {
   if (out) *out = nullptr;
   if (!d || !out) return MF_EINVAL;
-  if (d->process < 0 || d->process > 3 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
+  if (d->process < 0 || d->process > 4 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
       !(d->gev2_to_pb > 0.0))
     return MF_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MF_ECUDA; }
   mf_process* p = new (std::nothrow) mf_process;
   if (!p) return MF_ENOMEM;
-  static const int Dtab[4] = {2, 4, 14, 18}, nftab[4] = {2, 2, 3, 4};
+  static const int Dtab[5] = {2, 4, 14, 18, 4}, nftab[5] = {2, 2, 3, 4, 2};
   p->process = d->process; p->D = Dtab[d->process]; p->NF = nftab[d->process];
   mf::Params& P = p->P;
   std::memset(&P, 0, sizeof(P));
@@ -146,7 +147,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     }
     for (int i = 1; i < d->pdf_nx; ++i) if (!(d->pdf_lnx[i] > d->pdf_lnx[i - 1])) { delete p; return MF_EINVAL; }
     for (int i = 1; i < d->pdf_nq; ++i) if (!(d->pdf_lnq2[i] > d->pdf_lnq2[i - 1])) { delete p; return MF_EINVAL; }
-    const int ng = d->process + 1;
+    const int ng = d->process == MF_PP_TT ? 2 : d->process + 1;
+    const int nfl = d->process == MF_PP_TT ? d->pdf_nfl : 1;
+    if (d->process == MF_PP_TT && (nfl < 3 || nfl % 2 == 0 || nfl > mf::kMaxPartonTables)) { delete p; return MF_EINVAL; }
+    P.pdf_nfl = nfl;
     P.me_norm = std::pow(gs2, ng) / (256.0 * (ng == 4 ? 2.0 : 1.0));
     const int ncut = p->NF - 2;
     const double thr = 2.0 * d->m_top + ncut * (d->ptmin > 0.0 ? d->ptmin : 0.0);
@@ -162,16 +166,16 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   // device-side constants
   cudaError_t e = cudaSuccess;
   if (d->process != 0) {
-    const size_t nx = d->pdf_nx, nq = d->pdf_nq;
+    const size_t nx = d->pdf_nx, nq = d->pdf_nq, nt = (size_t)P.pdf_nfl;
     if ((e = cudaMalloc(&p->d_lnx, nx * 8)) != cudaSuccess || (e = cudaMalloc(&p->d_lnq2, nq * 8)) != cudaSuccess ||
-        (e = cudaMalloc(&p->d_xf, nx * nq * 8)) != cudaSuccess || (e = cudaMalloc(&p->d_row, nx * 8)) != cudaSuccess) {
+        (e = cudaMalloc(&p->d_xf, nt * nx * nq * 8)) != cudaSuccess || (e = cudaMalloc(&p->d_row, nt * nx * 8)) != cudaSuccess) {
       free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
     }
     cudaMemcpy(p->d_lnx, d->pdf_lnx, nx * 8, cudaMemcpyHostToDevice);
     cudaMemcpy(p->d_lnq2, d->pdf_lnq2, nq * 8, cudaMemcpyHostToDevice);
-    cudaMemcpy(p->d_xf, d->pdf_xf, nx * nq * 8, cudaMemcpyHostToDevice);
-    mf::pdf_collapse_kernel<<<(int)((nx + 127) / 128), 128>>>(p->d_xf, p->d_lnq2, (int)nx, (int)nq, P.pdf_jq, P.pdf_uq,
-                                                             p->d_row);
+    cudaMemcpy(p->d_xf, d->pdf_xf, nt * nx * nq * 8, cudaMemcpyHostToDevice);
+    mf::pdf_collapse_kernel<<<(int)((nt * nx + 127) / 128), 128>>>(p->d_xf, p->d_lnq2, (int)(nt * nx), (int)nq, P.pdf_jq,
+                                                                  P.pdf_uq, p->d_row);
     if ((e = cudaDeviceSynchronize()) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
   }
   // launch geometry: fill every SM with as many blocks as fit
@@ -179,12 +183,12 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   int dev = 0;
   cudaGetDevice(&dev);
   if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
-  if (p->process >= 2) {
+  if (p->process == 2 || p->process == 3) {
     // cooperative pass: as many teams per block as the SM's shared memory holds, one block per SM
     e = p->process == 3 ? coop_setup<3>(p, prop) : coop_setup<2>(p, prop);
     if (e != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   } else {
-    p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + 2 * P.pdf_nx + 5 * 32) * sizeof(double);
+    p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + (1 + P.pdf_nfl) * P.pdf_nx + 5 * 32) * sizeof(double);
   }
   int per_sm = 0, per_sm_unw = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pass_fn(p->process, false), p->threads, p->smem);
@@ -198,7 +202,7 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
       (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
-  if (p->process >= 2 &&
+  if ((p->process == 2 || p->process == 3) &&
       (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads *
                                        (p->process == 3 ? mf::g4::Prog::Queue : mf::g3::Prog::Queue) * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
@@ -224,7 +228,7 @@ int mf_record_size(const mf_process* p, int32_t* b) {
 }
 int mf_debug_row_len(const mf_process* p, int32_t* n) {
   if (!p || !n) return MF_EINVAL;
-  *n = 3 * p->D + 4 * (p->NF + 2) + 9;
+  *n = 3 * p->D + 4 * (p->NF + 2) + 9 + (p->process == MF_PP_TT ? 2 : 0);
   return MF_OK;
 }
 const char* mf_last_error(const mf_process* p) { return p ? p->err : kNullHandle; }
@@ -285,6 +289,7 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
   switch (p->process) {
     case 0: mf::debug_eval_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 1: mf::debug_eval_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    case 4: mf::debug_eval_kernel<4><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 2:
       mf::debug_eval_coop_kernel<2><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                       mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, A, d_out);
@@ -330,6 +335,7 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
   switch (p->process) {
     case 0: mf::debug_me2_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 1: mf::debug_me2_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    case 4: mf::debug_me2_kernel<4><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 2:
       mf::debug_me2_coop_kernel<2><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, d_mom, n, d_out);

@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(32) refine_grid_kernel(double* grid, const dou
 template <int PROC>
 __global__ void __launch_bounds__(kThreads) debug_eval_kernel(const Params P, const PassArgs A, double* out) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
-  const int row_len = 3 * D + 4 * (NF + 2) + 9;
+  const int row_len = 3 * D + 4 * (NF + 2) + 9 + (PROC == 4 ? 2 : 0);
   uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= A.n_events) return;
   const uint64_t event = A.first_event + idx;
@@ -73,13 +73,10 @@ __global__ void __launch_bounds__(kThreads) debug_eval_kernel(const Params P, co
   double* q = row + D;
   for (int i = 0; i < NF + 2; ++i)
     for (int c = 0; c < 4; ++c) *q++ = mom[i][c];
-  double lum = 0.0, me2 = 0.0, w = 0.0;
-  if (ev.pass) {
-    double asf;
-    lum = luminosity<PROC>(P, A, A.pdf_lnx, A.pdf_row, ev, asf);
-    me2 = me2_call<PROC>(P, ev.shat, ev.k) * asf;
-    w = event_weight<PROC>(P, ev, lum, me2);
-  }
+  double parts[4] = {0.0, 0.0, 0.0, 0.0}, w = 0.0;
+  if (ev.pass) w = weigh_event<PROC>(P, A, A.pdf_lnx, A.pdf_row, ev, parts);
+  const double lum = parts[0], me2 = parts[1];
+  if (PROC == 4) { row[row_len - 2] = parts[2]; row[row_len - 1] = parts[3]; }
   q[0] = ev.x1; q[1] = ev.x2; q[2] = lum; q[3] = me2; q[4] = ev.phi; q[5] = ev.jac_vegas; q[6] = w;
   q[7] = ev.pass ? 1.0 : 0.0;
   q[8] = accept_draw(A.seed, A.iteration, event);
@@ -97,7 +94,12 @@ __global__ void __launch_bounds__(kThreads) debug_me2_kernel(const Params P, con
   for (int f = 0; f < NF; ++f)
     for (int c = 0; c < 4; ++c) k[f][c] = m[(2 + f) * 4 + c];
   double shat = 4.0 * m[0] * m[0];
-  out[i] = me2_call<PROC>(P, shat, k);
+  if (PROC == 4) {   // two channels per point: (gg, q qbar)
+    out[2 * i] = me2_call<PROC>(P, shat, k);
+    out[2 * i + 1] = matrix_element_qq(P, shat, k);
+  } else {
+    out[i] = me2_call<PROC>(P, shat, k);
+  }
 }
 
 __global__ void debug_philox_kernel(uint64_t seed, uint32_t iteration, uint64_t first, uint64_t n, uint32_t n_blocks,
@@ -116,11 +118,12 @@ __global__ void debug_pdf_kernel(const double* lnx, const double* lnq2, const do
   if (i < n) out[i] = pdf_xf_2d(lnx, lnq2, xf, nx, nq, x[i], q2[i]);
 }
 
-// collapses the table at the process' fixed mu2 (one thread per x knot)
-__global__ void pdf_collapse_kernel(const double* xf, const double* lnq2, int nx, int nq, int jq, double uq,
+// collapses every parton table at the process' fixed mu2 (one thread per table and x knot: the tables are contiguous
+// [n_tables][nx][nq], so (table, knot) is one flat row index)
+__global__ void pdf_collapse_kernel(const double* xf, const double* lnq2, int n_rows, int nq, int jq, double uq,
                                     double* row) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < nx) row[i] = pdf_collapse_q2(xf, lnq2, nq, i, jq, uq);
+  if (i < n_rows) row[i] = pdf_collapse_q2(xf, lnq2, nq, i, jq, uq);
 }
 
 // FP64 peak probe: 8 independent DFMA chains per thread, enough warps to fill the FP64 pipe.

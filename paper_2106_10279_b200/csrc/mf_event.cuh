@@ -7,6 +7,7 @@
 #include "mf_pdf.cuh"
 #include "mf_me_prims.cuh"
 #include "mf_me_eemumu.cuh"
+#include "mf_me_qqtt.cuh"
 #include "mf_me_ggtt_generated.cuh"
 
 namespace mf {
@@ -69,7 +70,7 @@ MF_HD void generate_event(const Params& P, const double* grid, uint64_t seed, ui
   } else {
     Parton pk = parton_fractions(x0, x1, P.ln_tau_min, P.s);
     ev.shat = pk.shat; ev.y = pk.y; ev.x1 = pk.x1; ev.x2 = pk.x2; ev.jac_parton = pk.jac;
-    if (PROC == 1) {
+    if (PROC == 1 || PROC == 4) {
       U4 r = philox_block(seed, iteration, event, 1u);
       double u2 = uniform52(r.x, r.y), u3 = uniform52(r.z, r.w);
       int b2, b3;
@@ -139,11 +140,18 @@ MF_HD double matrix_element(const Params& P, double shat, const double k[][4]) {
     for (int s = 0; s < 2; ++s) { ub[s] = ubar_row(k[0], P.m_top, s); vv[s] = v_col(k[1], P.m_top, s); }
     rvec p3 = {{k[0][0], k[0][1], k[0][2], k[0][3]}}, p4 = {{k[1][0], k[1][1], k[1][2], k[1][3]}};
     double sum;
-    if (PROC == 1) sum = me2_ggtt_0g(Pg, eps, ub, vv, p3, p4, P.m_top);
+    if (PROC == 1 || PROC == 4) sum = me2_ggtt_0g(Pg, eps, ub, vv, p3, p4, P.m_top);
     else if (PROC == 2) sum = me2_ggtt_1g(Pg, eps, ub, vv, p3, p4, P.m_top);
     else sum = me2_ggtt_2g(Pg, eps, ub, vv, p3, p4, P.m_top);
     return sum * P.me_norm;
   }
+}
+
+// a7-a9 for the quark channel of process 4: averaged |M|^2 of q qbar -> t tbar at the same CM-frame point
+MF_HD double matrix_element_qq(const Params& P, double shat, const double k[][4]) {
+  double E = 0.5 * sqrt(shat);
+  double p1[4] = {E, 0.0, 0.0, E}, p2[4] = {E, 0.0, 0.0, -E};
+  return me2_qq_tt(p1, p2, k[0], k[1], P.m_top, 4.0 * kPi * P.alpha_s);
 }
 
 // a10: event weight (R12): w = lum/(2 shat) |M|^2 Phi J_parton K J_vegas.

@@ -26,8 +26,8 @@ struct IterResult {  // == mf_iter_result
 struct PassArgs {
   const double* grid;      // [D][nb+1] device
   const double* pdf_lnx;   // [nx] device (nullptr for e+e-)
-  const double* pdf_row;   // [nx] device: table collapsed at mu2
-  const double* pdf_lnq2;  // [nq] device, and the full table [nx][nq]: the dynamic-scale path only
+  const double* pdf_row;   // [nfl][nx] device: every parton table collapsed at mu2
+  const double* pdf_lnq2;  // [nq] device, and the full tables [nfl][nx][nq]: the dynamic-scale path only
   const double* pdf_xf;
   uint64_t seed, first_event, n_events;
   uint32_t iteration;
@@ -71,6 +71,60 @@ MF_D double luminosity(const Params& P, const PassArgs& A, const double* s_lnx, 
     f2 = pdf_xf_row(s_lnx, s_row, P.pdf_nx, ev.x2);
   }
   return f1 * f2 / (ev.x1 * ev.x2);
+}
+
+// Process 4 (gg + q qbar channels): the gluon-gluon luminosity (returned) and the flavour-summed
+// quark luminosity  lum_qq = sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2);  rows / tables are ordered
+// gluon, q_0, qbar_0, q_1, qbar_1, ...  One logarithm and one cell search per beam serve all tables.
+MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                          const Event<4>& ev, double& as_factor, double& lum_qq) {
+  as_factor = 1.0;
+  double f1[kMaxPartonTables], f2[kMaxPartonTables];
+  const int nt = P.pdf_nfl;
+  if (P.dyn_scale) {
+    const double mu2 = P.m_top * P.m_top + ev.k[0][1] * ev.k[0][1] + ev.k[0][2] * ev.k[0][2];
+    const size_t tab = (size_t)P.pdf_nx * P.pdf_nq;
+    for (int t = 0; t < nt; ++t) {
+      f1[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x1, mu2);
+      f2[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x2, mu2);
+    }
+    const double ratio = 1.0 / (1.0 + P.alpha_s * (23.0 / (12.0 * kPi)) * log(mu2 / P.mu2));
+    as_factor = ratio * ratio;
+  } else {
+    pdf_xf_rows<kMaxPartonTables>(s_lnx, s_row, P.pdf_nx, nt, ev.x1, f1);
+    pdf_xf_rows<kMaxPartonTables>(s_lnx, s_row, P.pdf_nx, nt, ev.x2, f2);
+  }
+  const double inv = 1.0 / (ev.x1 * ev.x2);
+  double a = 0.0, b = 0.0;
+#pragma unroll
+  for (int t = 1; t + 1 < kMaxPartonTables; t += 2)
+    if (t + 1 < nt) {
+      a = fma(f1[t], f2[t + 1], a);
+      b = fma(f1[t + 1], f2[t], b);
+    }
+  lum_qq = (a + b) * inv;
+  return f1[0] * f2[0] * inv;
+}
+
+// a6-a10 of one event that passed the cuts (thread-per-event kernels): luminosity, |M|^2, weight.
+// parts (optional): lum, me2 [, lum_qq, me2_qq for process 4] for the debug rows.
+template <int PROC>
+MF_D double weigh_event(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                        const Event<PROC>& ev, double* parts) {
+  double asf;
+  if constexpr (PROC == 4) {
+    double lum_qq;
+    const double lum = luminosity_pp(P, A, s_lnx, s_row, ev, asf, lum_qq);
+    const double me_gg = me2_call<PROC>(P, ev.shat, ev.k) * asf;
+    const double me_qq = matrix_element_qq(P, ev.shat, ev.k) * asf;
+    if (parts) { parts[0] = lum; parts[1] = me_gg; parts[2] = lum_qq; parts[3] = me_qq; }
+    return event_weight<PROC>(P, ev, 1.0, fma(lum, me_gg, lum_qq * me_qq));
+  } else {
+    const double lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
+    const double me2 = me2_call<PROC>(P, ev.shat, ev.k) * asf;
+    if (parts) { parts[0] = lum; parts[1] = me2; }
+    return event_weight<PROC>(P, ev, lum, me2);
+  }
 }
 
 // Lab-frame momenta of an event, beams first (record / debug-row layout).
@@ -208,20 +262,21 @@ MF_D void block_finish(const PassArgs& A, Accum acc, double* s_red, const double
   }
 }
 
-// ---- the fused pass, one thread per event (e+e- -> mu+mu-, gg -> ttbar, gg -> ttbar g) ----------------------
+// ---- the fused pass, one thread per event (e+e- -> mu+mu-, gg -> ttbar, pp -> ttbar) ----------------------
 template <int PROC, bool UNW>
-__global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel(const Params P, const PassArgs A) {
+__global__ void __launch_bounds__(kThreads, (PROC == 1 || PROC == 4) ? 4 : 2) fused_pass_kernel(const Params P, const PassArgs A) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   extern __shared__ double smem[];
-  const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx;
+  const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx, nrow = PROC == 4 ? nx * P.pdf_nfl : nx;
   double* s_grid = smem;                    // D*(nb+1)
   double* s_hist = s_grid + D * (nb + 1);   // D*nb
   double* s_lnx = s_hist + D * nb;          // nx
-  double* s_row = s_lnx + nx;               // nx
-  double* s_red = s_row + nx;               // 5 * 32
+  double* s_row = s_lnx + nx;               // nx (process 4: one row per parton table)
+  double* s_red = s_row + nrow;             // 5 * 32
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
-  for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
+  for (int i = threadIdx.x; i < nx; i += blockDim.x) s_lnx[i] = A.pdf_lnx[i];
+  for (int i = threadIdx.x; i < nrow; i += blockDim.x) s_row[i] = A.pdf_row[i];
   __syncthreads();
 
   Accum acc;
@@ -242,10 +297,7 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
       if (ev.pass && A.obs != nullptr) obs_bins = observable_bins<PROC>(A, ev);
       if (ev.pass) {
         ++acc.n_pass;
-        double asf;
-        double lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
-        double me2 = me2_call<PROC>(P, ev.shat, ev.k) * asf;
-        w = event_weight<PROC>(P, ev, lum, me2);
+        w = weigh_event<PROC>(P, A, s_lnx, s_row, ev, nullptr);
       }
     }
     accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins);

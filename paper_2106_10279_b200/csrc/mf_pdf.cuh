@@ -56,6 +56,22 @@ MF_HD double pdf_xf_row(const double* lnx, const double* row, int nx, double x) 
   return hermite_cell(lnx, nx, i, t, fm, row[i], row[i + 1], f2);
 }
 
+// The same on NT collapsed rows rows[t * nx + i] at once (multi-flavour table): one logarithm and one cell search.
+template <int NT>
+MF_HD void pdf_xf_rows(const double* lnx, const double* rows, int nx, int nt, double x, double* out) {
+  double lx = log(x);
+  int i = find_cell(lnx, nx, lx);
+  double h = lnx[i + 1] - lnx[i];
+  double t = (lx - lnx[i]) / h;
+#pragma unroll
+  for (int k = 0; k < NT; ++k)
+    if (k < nt) {
+      const double* row = rows + k * nx;
+      double fm = i > 0 ? row[i - 1] : 0.0, f2 = i + 2 < nx ? row[i + 2] : 0.0;
+      out[k] = hermite_cell(lnx, nx, i, t, fm, row[i], row[i + 1], f2);
+    }
+}
+
 // General 2-D lookup: Hermite in ln x on the rows jq-1..jq+2 that exist, then Hermite in ln Q^2.
 MF_HD double pdf_xf_2d(const double* lnx, const double* lnq2, const double* xf, int nx, int nq, double x, double q2) {
   double lx = log(x), lq = log(q2);

@@ -172,10 +172,10 @@ def main(argv=None):
     ap.add_argument("--pt-max", type=float, default=600.0)
     ap.add_argument("--eta-max", type=float, default=3.0)
     args = ap.parse_args(argv)
-    wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4}[args.config]
+    wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4, **W.EXTRA_CONFIGS}[args.config]
     if args.events > 0:
         wl = wl.scaled(args.events)
-    proc = api.Process(wl, W.pdf_table() if wl.process else None)
+    proc = api.Process(wl, W.pdf_for(wl.process))
     if args.dynamic_scale:
         proc.set_dynamic_scale(True)
     run_config(proc, wl.scaled(min(wl.n_events, 1 << 16)), capacity=args.capacity if wl.unweight else 0)   # warm-up

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 
 REL_EVENT = 1e-10
 REL_ITER = 1e-9
-WLS = {0: W.C0, 1: W.C1, 2: W.C2, 3: W.C3}
+WLS = {0: W.C0, 1: W.C1, 2: W.C2, 3: W.C3, 4: W.C5}
 
 
 def _torch():
@@ -26,8 +26,11 @@ def _torch():
 def _cols(wl):
     D, n = wl.n_dims, wl.n_final
     o = D + 4 * (n + 2)
-    return dict(x=slice(0, D), mom=slice(D, o), x1=o, x2=o + 1, lum=o + 2, me2=o + 3, phi=o + 4, jac=o + 5, w=o + 6,
-                pas=o + 7, r=o + 8, u=slice(o + 9, o + 9 + D), bin=slice(o + 9 + D, o + 9 + 2 * D))
+    c = dict(x=slice(0, D), mom=slice(D, o), x1=o, x2=o + 1, lum=o + 2, me2=o + 3, phi=o + 4, jac=o + 5, w=o + 6,
+             pas=o + 7, r=o + 8, u=slice(o + 9, o + 9 + D), bin=slice(o + 9 + D, o + 9 + 2 * D))
+    if wl.process == W.MF_PP_TT:       # the quark channel's flavour-summed luminosity and matrix element
+        c["lum_qq"], c["me2_qq"] = o + 9 + 2 * D, o + 10 + 2 * D
+    return c
 
 
 def _near_cut_edge(wl, row, c, tol=1e-9):
@@ -54,12 +57,14 @@ def _near_cut_edge(wl, row, c, tol=1e-9):
 _KNOTS = {}
 
 
-def _knot_scale(x):
-    """largest |x g| among the four ln x knots the Hermite interpolation at x uses, at any Q^2 of the table"""
+def _knot_scale(x, quarks=False):
+    """largest |x f| among the four ln x knots the Hermite interpolation at x uses, at any Q^2 of the table
+    (quarks: the largest over the quark and antiquark tables of the multi-flavour set)"""
     if not _KNOTS:
-        lnx, lnq2, xf = W.pdf_table()
-        _KNOTS["lnx"], _KNOTS["absmax"] = lnx, np.abs(xf).max(axis=1)
-    lnx, am = _KNOTS["lnx"], _KNOTS["absmax"]
+        lnx, lnq2, xf = W.pdf_table_flavours()
+        _KNOTS["lnx"], _KNOTS[False] = lnx, np.abs(xf[0]).max(axis=1)
+        _KNOTS[True] = np.abs(xf[1:]).max(axis=(0, 2))
+    lnx, am = _KNOTS["lnx"], _KNOTS[quarks]
     i = int(np.clip(np.searchsorted(lnx, np.log(x), side="right") - 1, 0, len(lnx) - 2))
     return am[max(i - 1, 0):i + 3].max()
 
@@ -100,6 +105,15 @@ def _compare_rows(wl, g, o):
         assert abs(lum_g - lum_o) <= REL_EVENT * abs(lum_o) + slack, ("lum", k, lum_g, lum_o)
         wg, wo = g[k, c["w"]], o[k, c["w"]]
         w_slack = abs(wo / lum_o) * slack if lum_o != 0.0 else 0.0
+        if wl.process == W.MF_PP_TT:
+            # two channels: w = common x (lum me2 + lum_qq me2_qq); each product is compared on its own
+            a, b = g[k, c["me2_qq"]], o[k, c["me2_qq"]]
+            assert abs(a - b) <= REL_EVENT * abs(b), ("me2_qq", k, a, b)
+            lq_g, lq_o = g[k, c["lum_qq"]], o[k, c["lum_qq"]]
+            slack_q = 2 * W.N_FLAVOURS * 4e-13 * _knot_scale(x1, True) * _knot_scale(x2, True) / (x1 * x2)
+            assert abs(lq_g - lq_o) <= REL_EVENT * abs(lq_o) + slack_q, ("lum_qq", k, lq_g, lq_o)
+            total = lum_o * o[k, c["me2"]] + lq_o * b
+            w_slack = abs(wo / total) * (slack * o[k, c["me2"]] + slack_q * b) if total != 0.0 else 0.0
         assert abs(wg - wo) <= REL_EVENT * abs(wo) + w_slack, ("w", k, wg, wo)
     return excluded
 
@@ -116,12 +130,12 @@ def test_philox_words_bit_exact():
 
 
 # ---- a1-a10 per event ------------------------------------------------------------------------------------
-@pytest.mark.parametrize("proc", [0, 1, 2, 3])
+@pytest.mark.parametrize("proc", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("grid_kind", ["uniform", "adapted"])
 def test_per_event_rows(proc, grid_kind, gpu_procs, oracle_procs):
     wl = WLS[proc]
     gp, op = gpu_procs[proc], oracle_procs[proc]
-    n = {0: 3000, 1: 3000, 2: 1500, 3: 400}[proc]   # several blocks of 128 and a ragged tail
+    n = {0: 3000, 1: 3000, 2: 1500, 3: 400, 4: 3000}[proc]   # several blocks of 128 and a ragged tail
     grid = W.uniform_grid(wl.n_dims) if grid_kind == "uniform" else adapted_grid(op, wl)
     dgrid = _torch().from_numpy(grid).cuda()
     for seed, it, first in [(0, 0, 0), (3, 5, (1 << 33) + 11)]:
@@ -130,7 +144,7 @@ def test_per_event_rows(proc, grid_kind, gpu_procs, oracle_procs):
         excluded = _compare_rows(wl, g, o)
         assert excluded <= 1
         c = _cols(wl)
-        if proc >= 2:
+        if proc in (2, 3):
             frac = o[:, c["pas"]].mean()
             assert 0.3 < frac < 1.0   # the cuts bite but most events survive
 
@@ -162,6 +176,27 @@ def test_me2_golden_points(gpu_procs, oracle_procs):
         assert abs(g / oracle_procs[proc].me2(mom) - 1) < REL_EVENT
 
 
+def test_me2_quark_channel(gpu_procs, oracle_procs):
+    """q qbar -> t tbar and g g -> t tbar at caller-supplied points (process 4 returns both channels)"""
+    rng = np.random.default_rng(8)
+    mt = W.C5.m_top
+    pts = []
+    for _ in range(300):       # two blocks of 128 and a tail; threshold to 50 x threshold, all angles
+        E = mt * (1.0 + 10 ** rng.uniform(-4, 1.7))
+        p = np.sqrt(E * E - mt * mt)
+        ct, ph = rng.uniform(-1, 1), rng.uniform(0, 2 * np.pi)
+        st = np.sqrt(1 - ct * ct)
+        k = np.array([E, p * st * np.cos(ph), p * st * np.sin(ph), p * ct])
+        pts.append([[E, 0, 0, E], [E, 0, 0, -E], k, [E, -k[1], -k[2], -k[3]]])
+    pts = np.array(pts)
+    g = gpu_procs[4].debug_me2(pts)
+    assert g.shape == (300, 2)
+    for i in range(300):
+        assert abs(g[i, 0] / oracle_procs[4].me2(pts[i]) - 1) < REL_EVENT
+        assert abs(g[i, 1] / oracle_procs[4].me2_qq(pts[i]) - 1) < REL_EVENT
+    np.testing.assert_allclose(g[:, 0], gpu_procs[1].debug_me2(pts), rtol=1e-13)
+
+
 # ---- a11/a12: iteration sums -------------------------------------------------------------------------------
 def _iterate_gpu(gp, grid, seed, it, first, n, want_hist=True):
     torch = _torch()
@@ -190,7 +225,7 @@ def _check_sums(n, hg, rg, ho, ro):
         assert np.array_equal(hg == 0, ho == 0)
 
 
-@pytest.mark.parametrize("proc,n", [(0, 200_003), (1, 100_001), (2, 12_011), (3, 1_501)])
+@pytest.mark.parametrize("proc,n", [(0, 200_003), (1, 100_001), (2, 12_011), (3, 1_501), (4, 60_001)])
 def test_iteration_sums(proc, n, gpu_procs, oracle_procs):
     wl = WLS[proc]
     gp, op = gpu_procs[proc], oracle_procs[proc]
@@ -200,7 +235,7 @@ def test_iteration_sums(proc, n, gpu_procs, oracle_procs):
         _check_sums(n, hg, rg, ho, ro)
 
 
-@pytest.mark.parametrize("proc", [0, 2, 3])
+@pytest.mark.parametrize("proc", [0, 2, 3, 4])
 def test_edge_sizes(proc, gpu_procs, oracle_procs):
     wl = WLS[proc]
     gp, op = gpu_procs[proc], oracle_procs[proc]
@@ -219,14 +254,14 @@ def test_edge_sizes(proc, gpu_procs, oracle_procs):
 
 
 # ---- a13: grid refinement ----------------------------------------------------------------------------------
-@pytest.mark.parametrize("proc", [0, 1, 2, 3])
+@pytest.mark.parametrize("proc", [0, 1, 2, 3, 4])
 def test_refine_grid(proc, gpu_procs, oracle_procs):
     torch = _torch()
     wl = WLS[proc]
     gp, op = gpu_procs[proc], oracle_procs[proc]
     grid = W.uniform_grid(wl.n_dims)
     for k in range(3):
-        hist, _ = op.vegas_iterate(grid, 0, k, 0, {0: 50000, 1: 8192, 2: 4096, 3: 1024}[proc])
+        hist, _ = op.vegas_iterate(grid, 0, k, 0, {0: 50000, 1: 8192, 2: 4096, 3: 1024, 4: 8192}[proc])
         if k == 1:
             hist[0, :] = 0.0  # an empty dimension must be left unchanged
         dgrid = torch.from_numpy(grid.copy()).cuda()
@@ -241,7 +276,8 @@ def test_refine_grid(proc, gpu_procs, oracle_procs):
 
 
 # ---- whole pipelines at reduced N ---------------------------------------------------------------------------
-@pytest.mark.parametrize("proc,n,n_it", [(0, 100_000, 5), (1, 1 << 16, 5), (2, 1 << 13, 3), (3, 1 << 10, 3)])
+@pytest.mark.parametrize("proc,n,n_it", [(0, 100_000, 5), (1, 1 << 16, 5), (2, 1 << 13, 3), (3, 1 << 10, 3),
+                                          (4, 1 << 15, 4)])
 def test_pipeline_reduced_n(proc, n, n_it, gpu_procs, oracle_procs):
     """Every iteration with each side refining its OWN grid: integrals, errors, histograms, final grid."""
     from paper_2106_10279_b200 import integrate
@@ -274,7 +310,7 @@ def test_c0_closed_form(gpu_procs):
 
 
 # ---- a14: unweighting ---------------------------------------------------------------------------------------
-@pytest.mark.parametrize("proc,n", [(1, 50_001), (2, 9_001), (3, 1_200)])
+@pytest.mark.parametrize("proc,n", [(1, 50_001), (2, 9_001), (3, 1_200), (4, 30_001)])
 def test_unweight(proc, n, gpu_procs, oracle_procs):
     torch = _torch()
     wl = WLS[proc]
@@ -340,7 +376,7 @@ def test_unweight_expected_acceptance(gpu_procs, oracle_procs):
 
 
 # ---- full-size launches (bench configuration) ------------------------------------------------------------------
-@pytest.mark.parametrize("proc", [1, 2, 3])
+@pytest.mark.parametrize("proc", [1, 2, 3, 4])
 def test_full_size_sampled(proc, gpu_procs, oracle_procs):
     """BASELINE.json sizes in the launch configuration bench.py times: (i) additivity over index ranges,
     (ii) oracle parity on sampled windows of the same stream, (iii) determinism."""
@@ -362,7 +398,7 @@ def test_full_size_sampled(proc, gpu_procs, oracle_procs):
     np.testing.assert_allclose(ha + hb, hg, rtol=1e-9, atol=1e-12 * hg.max())
     # sampled windows against the oracle
     rng = np.random.default_rng(proc)
-    wn = {1: 512, 2: 256, 3: 64}[proc]
+    wn = {1: 512, 2: 256, 3: 64, 4: 512}[proc]
     dgrid = _torch().from_numpy(grid).cuda()
     for first in rng.integers(0, n - wn, 6):
         first = int(first)
@@ -416,7 +452,7 @@ def test_rows_near_pdf_zero_crossings(gpu_procs, oracle_procs):
 
 
 # ---- dynamic scale (R16) -----------------------------------------------------------------
-@pytest.mark.parametrize("proc,n", [(1, 6_001), (2, 2_001), (3, 601)])
+@pytest.mark.parametrize("proc,n", [(1, 6_001), (2, 2_001), (3, 601), (4, 4_001)])
 def test_dynamic_scale(proc, n, gpu_procs, oracle_procs):
     """mu^2 = m_t^2 + pT(top)^2 per event, 2-D PDF lookup, running alpha_s: per-event rows and iteration sums against
     the oracle in the same mode; switching back restores the fixed-scale results exactly."""
@@ -445,7 +481,7 @@ def test_dynamic_scale(proc, n, gpu_procs, oracle_procs):
 
 
 # ---- observable histograms (Fig. 2) -------------------------------------------------------------------
-@pytest.mark.parametrize("proc,n", [(0, 30_011), (1, 20_001), (2, 4_001), (3, 1_003)])
+@pytest.mark.parametrize("proc,n", [(0, 30_011), (1, 20_001), (2, 4_001), (3, 1_003), (4, 12_001)])
 def test_observable_histograms(proc, n, gpu_procs, oracle_procs):
     """pT and eta histograms of the first final-state particle, accumulated in the same pass, against the oracle's
     definition evaluated on its own per-event rows; accumulation across calls (also through mf_unweight); detaching."""
@@ -496,6 +532,10 @@ def test_error_codes(pdf):
     assert api.mf_create_process(d)[0] == api.MF_ERANGE
     d, keep = api.make_desc(replace(W.C1, n_bins=1000), pdf)
     assert api.mf_create_process(d)[0] == api.MF_EINVAL
+    for bad in (1, 4, 13):            # MF_PP_TT needs 1 + 2 n_f tables, n_f = 1..5
+        d, keep = api.make_desc(W.C5, W.pdf_table_flavours())
+        d.pdf_nfl = bad
+        assert api.mf_create_process(d)[0] == api.MF_EINVAL
     d, keep = api.make_desc(W.C1, pdf)
     d.pdf_xf = None
     assert api.mf_create_process(d)[0] == api.MF_EINVAL

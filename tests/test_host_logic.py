@@ -37,7 +37,8 @@ def test_library_exports_every_declared_symbol(libpath):
 def test_struct_layouts_match_header():
     from paper_2106_10279_b200 import api
     assert C.sizeof(api.IterResult) == 40
-    assert C.sizeof(api.ProcessDesc) == 8 + 9 * 8 + 4 + 4 + 4 + 4 + 3 * 8  # int32 + pad, 9 doubles, 3 int32 + pad, 3 ptrs
+    # int32 + pad, 9 doubles, 3 int32 + pad, 3 ptrs, int32 (pdf_nfl) + pad
+    assert C.sizeof(api.ProcessDesc) == 8 + 9 * 8 + 4 + 4 + 4 + 4 + 3 * 8 + 8
     from oracle import mfo
     assert C.sizeof(mfo.ProcessDesc) == C.sizeof(api.ProcessDesc)
     assert [f[0] for f in mfo.ProcessDesc._fields_] == [f[0] for f in api.ProcessDesc._fields_]
