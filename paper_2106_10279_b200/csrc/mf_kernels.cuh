@@ -49,6 +49,12 @@ __device__ __noinline__ double me2_call(const Params& P, double shat, const doub
   return matrix_element<PROC>(P, shat, k);
 }
 
+// process 4: both channels in ONE out-of-line call, so that the top-quark spinors are formed once
+__device__ __noinline__ double me2_pp_call(const Params& P, double shat, const double (*k)[4], double& me_qq) {
+  me_qq = matrix_element_qq(P, shat, k);
+  return matrix_element<4>(P, shat, k);
+}
+
 // Luminosity (step a6): F(x1) F(x2) / (x1 x2) with F the interpolant of the collapsed row in shared memory; and
 // the factor that rescales |M|^2 (1 at the fixed scale).  Dynamic scale (R16; mf_set_dynamic_scale):
 // mu_F^2 = mu_R^2 = m_t^2 + pT(top)^2 per event, F by the general 2-D lookup in the table (global memory / L2),
@@ -91,8 +97,13 @@ MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_ln
     const double ratio = 1.0 / (1.0 + P.alpha_s * (23.0 / (12.0 * kPi)) * log(mu2 / P.mu2));
     as_factor = ratio * ratio;
   } else {
-    pdf_xf_rows<kMaxPartonTables>(s_lnx, s_row, P.pdf_nx, nt, ev.x1, f1);
-    pdf_xf_rows<kMaxPartonTables>(s_lnx, s_row, P.pdf_nx, nt, ev.x2, f2);
+    const HermiteWeights W1 = hermite_weights(s_lnx, P.pdf_nx, ev.x1), W2 = hermite_weights(s_lnx, P.pdf_nx, ev.x2);
+#pragma unroll
+    for (int t = 0; t < kMaxPartonTables; ++t)
+      if (t < nt) {
+        f1[t] = hermite_apply(W1, s_row + t * P.pdf_nx, P.pdf_nx);
+        f2[t] = hermite_apply(W2, s_row + t * P.pdf_nx, P.pdf_nx);
+      }
   }
   const double inv = 1.0 / (ev.x1 * ev.x2);
   double a = 0.0, b = 0.0;
@@ -115,8 +126,9 @@ MF_D double weigh_event(const Params& P, const PassArgs& A, const double* s_lnx,
   if constexpr (PROC == 4) {
     double lum_qq;
     const double lum = luminosity_pp(P, A, s_lnx, s_row, ev, asf, lum_qq);
-    const double me_gg = me2_call<PROC>(P, ev.shat, ev.k) * asf;
-    const double me_qq = matrix_element_qq(P, ev.shat, ev.k) * asf;
+    double me_qq;
+    const double me_gg = me2_pp_call(P, ev.shat, ev.k, me_qq) * asf;
+    me_qq *= asf;
     if (parts) { parts[0] = lum; parts[1] = me_gg; parts[2] = lum_qq; parts[3] = me_qq; }
     return event_weight<PROC>(P, ev, 1.0, fma(lum, me_gg, lum_qq * me_qq));
   } else {

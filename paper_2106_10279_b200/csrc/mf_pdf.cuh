@@ -56,20 +56,36 @@ MF_HD double pdf_xf_row(const double* lnx, const double* row, int nx, double x) 
   return hermite_cell(lnx, nx, i, t, fm, row[i], row[i + 1], f2);
 }
 
-// The same on NT collapsed rows rows[t * nx + i] at once (multi-flavour table): one logarithm and one cell search.
-template <int NT>
-MF_HD void pdf_xf_rows(const double* lnx, const double* rows, int nx, int nt, double x, double* out) {
-  double lx = log(x);
-  int i = find_cell(lnx, nx, lx);
-  double h = lnx[i + 1] - lnx[i];
-  double t = (lx - lnx[i]) / h;
-#pragma unroll
-  for (int k = 0; k < NT; ++k)
-    if (k < nt) {
-      const double* row = rows + k * nx;
-      double fm = i > 0 ? row[i - 1] : 0.0, f2 = i + 2 < nx ? row[i + 2] : 0.0;
-      out[k] = hermite_cell(lnx, nx, i, t, fm, row[i], row[i + 1], f2);
-    }
+// The same on NT collapsed rows rows[t * nx + i] at once (multi-flavour table).  The Hermite interpolant is linear in
+// the four knot values f(i-1), f(i), f(i+1), f(i+2) it uses, so the cell search, the logarithm, the basis polynomials
+// and the knot-derivative coefficients (all the divisions) are done ONCE per x and every table costs four FMAs:
+//   F = h00 f0 + a d0 + h01 f1 + b d1,   a = h10 h,  b = h11 h,
+//   d0 = al (f0 - fm) + be0 (f1 - f0),   d1 = be1 (f1 - f0) + ga (f2 - f1)
+// with (al, be0) = (1/2hl, 1/2h) inside and (0, 1/h) at the first cell, (be1, ga) = (1/2h, 1/2hr) inside and (1/h, 0)
+// at the last cell (the one-sided differences of R8).
+struct HermiteWeights { int i; double wm, w0, w1, w2; };
+MF_HD HermiteWeights hermite_weights(const double* lnx, int nx, double x) {
+  HermiteWeights W;
+  const double lx = log(x);
+  const int i = find_cell(lnx, nx, lx);
+  const double h = lnx[i + 1] - lnx[i], rh = 1.0 / h;
+  const double t = (lx - lnx[i]) * rh, t2 = t * t, t3 = t2 * t;
+  const double h00 = 2.0 * t3 - 3.0 * t2 + 1.0, h01 = 3.0 * t2 - 2.0 * t3;
+  const double a = (t3 - 2.0 * t2 + t) * h, b = (t3 - t2) * h;
+  double al = 0.0, be0 = rh, be1 = rh, ga = 0.0;
+  if (i > 0) { al = 0.5 / (lnx[i] - lnx[i - 1]); be0 = 0.5 * rh; }
+  if (i + 2 < nx) { ga = 0.5 / (lnx[i + 2] - lnx[i + 1]); be1 = 0.5 * rh; }
+  W.i = i;
+  W.wm = -a * al;
+  W.w0 = h00 + a * (al - be0) - b * be1;
+  W.w1 = h01 + a * be0 + b * (be1 - ga);
+  W.w2 = b * ga;
+  return W;
+}
+MF_HD double hermite_apply(const HermiteWeights& W, const double* row, int nx) {
+  const int i = W.i;
+  const double fm = i > 0 ? row[i - 1] : 0.0, f2 = i + 2 < nx ? row[i + 2] : 0.0;
+  return fma(W.wm, fm, fma(W.w2, f2, fma(W.w0, row[i], W.w1 * row[i + 1])));
 }
 
 // General 2-D lookup: Hermite in ln x on the rows jq-1..jq+2 that exist, then Hermite in ln Q^2.

@@ -37,13 +37,14 @@ double mfh_me2(int process, const double* mom, double m_top, double alpha_s, dou
   double shat = 4.0 * mom[0] * mom[0];
   double gs2 = 4.0 * kPi * alpha_s;
   double k[4][4];
-  int nf = process <= 1 ? 2 : process + 1;
+  int nf = (process <= 1 || process == 4) ? 2 : process + 1;
   for (int i = 0; i < nf; ++i) for (int m = 0; m < 4; ++m) k[i][m] = mom[(2 + i) * 4 + m];
   switch (process) {
     case 0: return matrix_element<0>(P, shat, k);
     case 1: P.me_norm = gs2 * gs2 / 256.0; return matrix_element<1>(P, shat, k);
     case 2: P.me_norm = gs2 * gs2 * gs2 / 256.0; return matrix_element<2>(P, shat, k);
     case 3: P.me_norm = gs2 * gs2 * gs2 * gs2 / 512.0; return matrix_element<3>(P, shat, k);
+    case 4: return matrix_element_qq(P, shat, k);      // the quark channel of MF_PP_TT
   }
   return -1.0;
 }
@@ -76,6 +77,16 @@ double mfh_pdf_row(const double* lnx, const double* lnq2, const double* xf, int 
   double row[512];
   for (int i = 0; i < nx; ++i) row[i] = pdf_collapse_q2(xf, lnq2, nq, i, jq, uq);
   return pdf_xf_row(lnx, row, nx, x);
+}
+// the multi-table variant of it (weights once per x, four FMAs per table)
+double mfh_pdf_row_weights(const double* lnx, const double* lnq2, const double* xf, int nx, int nq, double x, double q2) {
+  double lq = log(q2);
+  int jq = find_cell(lnq2, nq, lq);
+  double uq = (lq - lnq2[jq]) / (lnq2[jq + 1] - lnq2[jq]);
+  double row[512];
+  for (int i = 0; i < nx; ++i) row[i] = pdf_collapse_q2(xf, lnq2, nq, i, jq, uq);
+  HermiteWeights W = hermite_weights(lnx, nx, x);
+  return hermite_apply(W, row, nx);
 }
 
 }  // extern "C"

@@ -94,7 +94,7 @@ def shim():
     L.mfh_philox.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32)]
     L.mfh_uniform52.restype = C.c_double
     L.mfh_uniform52.argtypes = [C.c_uint32, C.c_uint32]
-    for f in (L.mfh_pdf_2d, L.mfh_pdf_row):
+    for f in (L.mfh_pdf_2d, L.mfh_pdf_row, L.mfh_pdf_row_weights):
         f.restype = C.c_double
         f.argtypes = [dp, dp, dp, C.c_int, C.c_int, C.c_double, C.c_double]
     return L
@@ -123,6 +123,37 @@ def test_shim_pdf_paths(shim, pdf, oracle_procs):
         assert abs(shim.mfh_pdf_2d(*args, x, q2) - o) <= 1e-12 * abs(o) + 1e-15
         # the collapsed-row path of the fused pass (Q^2 step applied to the knots first) is the same interpolant
         assert abs(shim.mfh_pdf_row(*args, x, q2) - o) <= 1e-11 * abs(o) + 1e-14
+    # the multi-flavour pass forms the Hermite weights once per x: every table of the flavour set, ends included
+    lnx, lnq2, xf = W.pdf_table_flavours()
+    from oracle import mfo
+    op = mfo.Process(W.C5, (lnx, lnq2, xf))
+    xs = [1e-9, 1.0, float(np.exp(lnx[1])), float(np.exp(lnx[-2])), 0.999] + list(np.exp(rng.uniform(np.log(1e-8), 0, 200)))
+    for t in range(xf.shape[0]):
+        tab = np.ascontiguousarray(xf[t])
+        args = (lnx.ctypes.data_as(dp), lnq2.ctypes.data_as(dp), tab.ctypes.data_as(dp), len(lnx), len(lnq2))
+        scale = np.abs(tab).max(axis=1)
+        for x in xs[:5] + xs[5 + 20 * t:25 + 20 * t]:
+            q2 = float(np.exp(rng.uniform(np.log(3.0), np.log(9e9))))
+            o = op.pdf_xf_table(t, x, q2)
+            i = int(np.clip(np.searchsorted(lnx, np.log(x), side="right") - 1, 0, len(lnx) - 2))
+            assert abs(shim.mfh_pdf_row_weights(*args, x, q2) - o) <= 1e-11 * abs(o) + 4e-15 * scale[max(i - 1, 0):i + 3].max()
+
+
+def test_shim_quark_channel_me(shim):
+    """q qbar -> t tbar of the CUDA path's source (chiral two-component spinors) against the oracle (Dirac matrices)"""
+    from oracle import mfo
+    op = mfo.Process(W.C5, W.pdf_table_flavours())
+    rng = np.random.default_rng(4)
+    mt = W.C5.m_top
+    for _ in range(200):
+        E = mt * (1.0 + 10 ** rng.uniform(-4, 1.7))
+        p = np.sqrt(E * E - mt * mt)
+        ct, ph = rng.uniform(-1, 1), rng.uniform(0, 2 * np.pi)
+        st = np.sqrt(1 - ct * ct)
+        k = np.array([E, p * st * np.cos(ph), p * st * np.sin(ph), p * ct])
+        mom = np.ascontiguousarray([[E, 0, 0, E], [E, 0, 0, -E], k, [E, -k[1], -k[2], -k[3]]])
+        g = shim.mfh_me2(4, mom.ctypes.data_as(dp), mt, W.C5.alpha_s, W.C5.alpha_em)
+        assert abs(g / op.me2_qq(mom) - 1) < 1e-11
 
 
 @pytest.mark.parametrize("wl", [W.C0, W.C1, W.C2, W.C3], ids=["C0", "C1", "C2", "C3"])
