@@ -71,7 +71,7 @@ int mf_create_process(const mf_process_desc *desc, mf_process **out);
 int mf_destroy_process(mf_process *p);
 int mf_n_dims(const mf_process *p, int32_t *D);              /* VEGAS dimensions: 2, 4, 14, 18, 4       */
 int mf_n_final(const mf_process *p, int32_t *n);             /* final-state particles: 2, 2, 3, 4, 2    */
-int mf_record_size(const mf_process *p, int32_t *bytes);     /* (n_final+2)*32 + 16                     */
+int mf_record_size(const mf_process *p, int32_t *bytes);     /* (n_final+2)*32 + 16 (+8: MF_PP_TT)      */
 int mf_debug_row_len(const mf_process *p, int32_t *n_doubles);/* 3*D + 4*(n_final+2) + 9 (+2: MF_PP_TT)  */
 const char *mf_last_error(const mf_process *p);              /* static or handle-owned string           */
 /* launch geometry of the fused pass (blocks, threads per block), for reporting */
@@ -93,7 +93,10 @@ int mf_refine_grid(mf_process *p, double *d_grid, const double *d_hist, double a
  * (array of structs of mf_record_size bytes: (n_final+2) lab-frame four-momenta (E,px,py,pz), beams first,
  * as doubles; signed w as double; event id as uint64).  *d_count is an in/out cursor: every accepted event
  * advances it, only slots < capacity are written, so *d_count > capacity after synchronising IS the
- * overflow signal.  Record order is unspecified (sort by event id).  d_hist may be NULL. */
+ * overflow signal.  Record order is unspecified (sort by event id).  d_hist may be NULL.
+ * MF_PP_TT appends one more uint64 to each record: the partonic channel of the event (0 = g g; 1 + 2 i = quark i from
+ * beam 1 and its antiquark from beam 2; 2 + 2 i = the other way round), drawn in proportion to |luminosity x |M|^2| of
+ * the channels, in that order, with the second uniform of the accept block (R18). */
 int mf_unweight(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                 uint64_t n_events, double w_max, void *d_records, uint64_t capacity, uint64_t *d_count,
                 double *d_hist, mf_iter_result *d_result, void *stream);

@@ -61,6 +61,12 @@ inline double accept_draw(uint64_t seed, uint32_t iteration, uint64_t event) {
   philox_block(seed, iteration, event, 0xFFFFFFFFu, w);
   return uniform_from_words(w[0], w[1]);
 }
+// the second uniform of the same block: picks the partonic channel of an accepted event (process 4, reading R18)
+inline double channel_draw(uint64_t seed, uint32_t iteration, uint64_t event) {
+  uint32_t w[4];
+  philox_block(seed, iteration, event, 0xFFFFFFFFu, w);
+  return uniform_from_words(w[2], w[3]);
+}
 
 // ---------------------------------------------------------------------------------------------
 // O3. VEGAS importance-sampling map (Lepage 1978; PAPER.md L27, L61 by citation to VegasFlow).

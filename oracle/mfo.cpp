@@ -51,6 +51,8 @@ template <class R> struct EventOut {
   R mom[6][4];  // lab frame, beams first
   R x1, x2, lum, me2, phi, jac, w;
   R lum_qq, me2_qq;  // process 4: the flavour-summed q qbar luminosity and the q qbar matrix element
+  R chan[12];        // process 4: luminosity x |M|^2 of every partonic channel (0 gg; 1+2i q_i from beam 1; 2+2i from beam 2)
+  int n_chan;
   int pass;
 };
 
@@ -116,6 +118,7 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   o.w = R(0);
   o.lum_qq = R(0);
   o.me2_qq = R(0);
+  o.n_chan = 0;
   if (!o.pass) return;
   o.lum = R(1);
   R mu2 = R(P.d.mu2), as_factor = R(1);
@@ -153,7 +156,11 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
       R q2 = pdf_xf<R>(P.pdfq[i], o.x2, mu2), qb2 = pdf_xf<R>(P.pdfq[i + 1], o.x2, mu2);
       La = La + q1 * qb2;
       Lb = Lb + qb1 * q2;
+      o.chan[1 + i] = q1 * qb2 / (o.x1 * o.x2) * Ma;
+      o.chan[2 + i] = qb1 * q2 / (o.x1 * o.x2) * Mb;
     }
+    o.chan[0] = o.lum * o.me2;
+    o.n_chan = 1 + (int)P.pdfq.size();
     La = La / (o.x1 * o.x2);
     Lb = Lb / (o.x1 * o.x2);
     o.lum_qq = La + Lb;
@@ -181,7 +188,7 @@ int iterate(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteratio
   S sw = S(0), sw2 = S(0);
   double maxw = 0;
   uint64_t npass = 0, nacc = 0;
-  int recsize = (P.nfinal + 2) * 32 + 16;
+  int recsize = (P.nfinal + 2) * 32 + 16 + (P.d.process == 4 ? 8 : 0);
   EventOut<R> o;
   for (uint64_t e = first; e < first + n_events; ++e) {
     eval_event<R>(P, grid, seed, iteration, e, o);
@@ -206,6 +213,19 @@ int iterate(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteratio
           buf[(P.nfinal + 2) * 4] = w;
           std::memcpy(rec, buf, ((P.nfinal + 2) * 4 + 1) * sizeof(double));
           std::memcpy(rec + ((P.nfinal + 2) * 4 + 1) * sizeof(double), &e, sizeof(uint64_t));
+          if (P.d.process == 4) {
+            // R18: the partonic channel of an accepted event is drawn in proportion to |luminosity x |M|^2| of the
+            // channels, in channel order: the first c with  sum_{c' <= c} |a_c'| > v * sum |a|,  v the channel draw
+            double a[12], total = 0.0;
+            for (int c = 0; c < o.n_chan; ++c) { a[c] = std::fabs(r_to_double(o.chan[c])); total += a[c]; }
+            double v = channel_draw(seed, iteration, e) * total, cum = 0.0;
+            uint64_t pick = (uint64_t)(o.n_chan - 1);
+            for (int c = 0; c < o.n_chan; ++c) {
+              cum += a[c];
+              if (cum > v) { pick = (uint64_t)c; break; }
+            }
+            std::memcpy(rec + ((P.nfinal + 2) * 4 + 2) * sizeof(double), &pick, sizeof(uint64_t));
+          }
         }
       }
     }
@@ -347,7 +367,11 @@ int mfo_set_dynamic_scale(mfo_process* P, int32_t on) {
 }
 int mfo_n_dims(const mfo_process* P, int32_t* D) { if (!P || !D) return -1; *D = P->D; return 0; }
 int mfo_n_final(const mfo_process* P, int32_t* n) { if (!P || !n) return -1; *n = P->nfinal; return 0; }
-int mfo_record_size(const mfo_process* P, int32_t* b) { if (!P || !b) return -1; *b = (P->nfinal + 2) * 32 + 16; return 0; }
+int mfo_record_size(const mfo_process* P, int32_t* b) {
+  if (!P || !b) return -1;
+  *b = (P->nfinal + 2) * 32 + 16 + (P->d.process == 4 ? 8 : 0);   // process 4 appends the u64 channel code
+  return 0;
+}
 int mfo_debug_row_len(const mfo_process* P, int32_t* n) {
   if (!P || !n) return -1;
   *n = 3 * P->D + 4 * (P->nfinal + 2) + 9 + (P->d.process == 4 ? 2 : 0);

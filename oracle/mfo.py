@@ -303,10 +303,14 @@ class Process:
 
     def records_view(self, rec, count):
         """Decode `count` AoS records into (momenta[count, n+2, 4], w[count], event_id[count])."""
-        nd = (self.n_final + 2) * 4
-        dt = np.dtype([("mom", np.float64, (self.n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)])
-        assert dt.itemsize == self.record_size and nd * 8 + 16 == self.record_size
+        fields = [("mom", np.float64, (self.n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)]
+        if self.wl.process == 4:
+            fields.append(("channel", np.uint64))
+        dt = np.dtype(fields)
+        assert dt.itemsize == self.record_size
         a = np.frombuffer(rec.tobytes()[:count * self.record_size], dtype=dt)
+        if self.wl.process == 4:
+            self.last_channels = a["channel"]
         return a["mom"], a["w"], a["id"]
 
 

@@ -274,10 +274,13 @@ class Process:
 
     def records_view(self, records, count):
         """Decode `count` AoS records (uint8 tensor) into (momenta[count, n+2, 4], w[count], id[count])."""
-        dt = np.dtype([("mom", np.float64, (self.n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)])
+        from .lhe import record_dtype
+        dt = record_dtype(self.n_final, self.wl.process)
         assert dt.itemsize == self.record_size
         raw = records[:count * self.record_size].cpu().numpy().tobytes()
         a = np.frombuffer(raw, dtype=dt)
+        if "channel" in dt.names:
+            self.last_channels = a["channel"]       # MF_PP_TT: the partonic channel codes of the decoded records
         return a["mom"], a["w"], a["id"]
 
 

@@ -79,21 +79,21 @@ MF_D double luminosity(const Params& P, const PassArgs& A, const double* s_lnx, 
   return f1 * f2 / (ev.x1 * ev.x2);
 }
 
-// Process 4 (gg + q qbar channels): the gluon-gluon luminosity (returned) and the flavour-summed
-// quark luminosity  lum_qq = sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2);  rows / tables are ordered
-// gluon, q_0, qbar_0, q_1, qbar_1, ...  One logarithm and one cell search per beam serve all tables.
-MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
-                          const Event<4>& ev, double& as_factor, double& lum_qq) {
+// Process 4 (gg + q qbar channels; R17): x f(x) of every parton table at both beams; rows /
+// tables are ordered gluon, q_0, qbar_0, q_1, qbar_1, ...  One logarithm and one cell search per beam serve all tables.
+MF_D void parton_densities(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                           const Event<4>& ev, double* f1, double* f2, double& as_factor) {
   as_factor = 1.0;
-  double f1[kMaxPartonTables], f2[kMaxPartonTables];
   const int nt = P.pdf_nfl;
   if (P.dyn_scale) {
     const double mu2 = P.m_top * P.m_top + ev.k[0][1] * ev.k[0][1] + ev.k[0][2] * ev.k[0][2];
     const size_t tab = (size_t)P.pdf_nx * P.pdf_nq;
-    for (int t = 0; t < nt; ++t) {
-      f1[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x1, mu2);
-      f2[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x2, mu2);
-    }
+#pragma unroll
+    for (int t = 0; t < kMaxPartonTables; ++t)
+      if (t < nt) {
+        f1[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x1, mu2);
+        f2[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x2, mu2);
+      }
     const double ratio = 1.0 / (1.0 + P.alpha_s * (23.0 / (12.0 * kPi)) * log(mu2 / P.mu2));
     as_factor = ratio * ratio;
   } else {
@@ -105,6 +105,15 @@ MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_ln
         f2[t] = hermite_apply(W2, s_row + t * P.pdf_nx, P.pdf_nx);
       }
   }
+}
+
+// the gluon-gluon luminosity (returned) and the flavour-summed quark luminosity
+//   lum_qq = sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2)
+MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                          const Event<4>& ev, double& as_factor, double& lum_qq) {
+  double f1[kMaxPartonTables], f2[kMaxPartonTables];
+  parton_densities(P, A, s_lnx, s_row, ev, f1, f2, as_factor);
+  const int nt = P.pdf_nfl;
   const double inv = 1.0 / (ev.x1 * ev.x2);
   double a = 0.0, b = 0.0;
 #pragma unroll
@@ -115,6 +124,34 @@ MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_ln
     }
   lum_qq = (a + b) * inv;
   return f1[0] * f2[0] * inv;
+}
+
+// Partonic channel of an ACCEPTED event of process 4 (R18): drawn in proportion to |luminosity x |M|^2| of
+// the channels, in channel order (0 gg; 1 + 2 i quark i from beam 1; 2 + 2 i quark i from beam 2): the first c with
+// sum_{c' <= c} |a_c'| > v sum |a|, v = the second uniform of the event's accept block.  Rare path: nothing is kept
+// from the weight computation, everything is formed again.
+__device__ __noinline__ unsigned long long select_channel(const Params& P, const PassArgs& A, const double* s_lnx,
+                                                          const double* s_row, const Event<4>& ev, uint64_t event) {
+  double f1[kMaxPartonTables], f2[kMaxPartonTables], asf, me_qq;
+  parton_densities(P, A, s_lnx, s_row, ev, f1, f2, asf);
+  const double me_gg = me2_pp_call(P, ev.shat, ev.k, me_qq);
+  const int nt = P.pdf_nfl;
+  const double inv = 1.0 / (ev.x1 * ev.x2);
+  double a[kMaxPartonTables], total = 0.0;
+  a[0] = fabs(f1[0] * f2[0] * inv * (me_gg * asf));
+  for (int t = 1; t + 1 < nt; t += 2) {
+    a[t] = fabs(f1[t] * f2[t + 1] * inv * (me_qq * asf));
+    a[t + 1] = fabs(f1[t + 1] * f2[t] * inv * (me_qq * asf));
+  }
+  for (int c = 0; c < nt; ++c) total += a[c];
+  const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);
+  const double v = uniform52(r.z, r.w) * total;
+  double cum = 0.0;
+  for (int c = 0; c < nt; ++c) {
+    cum += a[c];
+    if (cum > v) return (unsigned long long)c;
+  }
+  return (unsigned long long)(nt - 1);
 }
 
 // a6-a10 of one event that passed the cuts (thread-per-event kernels): luminosity, |M|^2, weight.
@@ -186,7 +223,8 @@ struct Accum {
 // shared-memory w^2 histogram, and hit-or-miss unweighting with a warp-aggregated cursor.
 template <int PROC, bool UNW>
 MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_grid, double* s_hist, bool valid,
-                           uint64_t event, double w, const Bins<PROC>& bins, Accum& acc, int obs_bins) {
+                           uint64_t event, double w, const Bins<PROC>& bins, Accum& acc, int obs_bins,
+                           const double* s_lnx = nullptr, const double* s_row = nullptr) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   const int nb = P.n_bins;
   const double w2 = w * w;
@@ -222,13 +260,15 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
           generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
           double mom[NF + 2][4];
           lab_momenta<PROC>(ev, mom);
-          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16));
+          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16 + (PROC == 4 ? 8 : 0)));
 #pragma unroll
           for (int i = 0; i < NF + 2; ++i)
 #pragma unroll
             for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
           rec[4 * (NF + 2)] = w;
           reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
+          if constexpr (PROC == 4)
+            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = select_channel(P, A, s_lnx, s_row, ev, event);
         }
       }
     }
@@ -312,7 +352,7 @@ __global__ void __launch_bounds__(kThreads, (PROC == 1 || PROC == 4) ? 4 : 2) fu
         w = weigh_event<PROC>(P, A, s_lnx, s_row, ev, nullptr);
       }
     }
-    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins);
+    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins, s_lnx, s_row);
   }
   block_finish(A, acc, s_red, s_hist, D * nb);
 }

@@ -26,8 +26,26 @@ import numpy as np
 PDG = {0: (11, -11, 13, -13), 1: (21, 21, 6, -6), 2: (21, 21, 6, -6, 21), 3: (21, 21, 6, -6, 21, 21)}
 
 
-def record_dtype(n_final):
-    return np.dtype([("mom", np.float64, (n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)])
+QUARK_PDG = (1, 2, 3, 4, 5)          # flavour index of the multi-flavour table -> PDG id (d, u, s, c, b)
+
+
+def record_dtype(n_final, process=None):
+    fields = [("mom", np.float64, (n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)]
+    if process == 4:                  # MF_PP_TT records carry the partonic channel (include/mf.h)
+        fields.append(("channel", np.uint64))
+    return np.dtype(fields)
+
+
+def channel_ids(channel):
+    """PDG ids (beam 1, beam 2, t, tbar) and colour flow of an MF_PP_TT record's channel code"""
+    c = int(channel)
+    if c == 0:
+        return PDG[1], colour_flow(1)
+    q = QUARK_PDG[(c - 1) // 2]
+    # q qbar -> g* -> t tbar: the quark's colour goes to the top, the antiquark's anticolour to the antitop
+    if c % 2 == 1:
+        return (q, -q, 6, -6), [(501, 0), (0, 502), (501, 0), (0, 502)]
+    return (-q, q, 6, -6), [(0, 502), (501, 0), (501, 0), (0, 502)]
 
 
 def colour_flow(process):
@@ -50,12 +68,16 @@ def colour_flow(process):
 
 def format_events(rec, process, m_top, scale, alpha_em, alpha_s, w_max):
     """LHE <event> blocks for a structured record array (pure function: also used by the tests)"""
-    ids = PDG[process]
-    flow = colour_flow(process)
-    n = len(ids)
-    mass = [m_top if abs(p) == 6 else 0.0 for p in ids]
+    per_event = process == 4
+    if not per_event:
+        ids = PDG[process]
+        flow = colour_flow(process)
+    n = 4 if per_event else len(ids)
     out = io.StringIO()
     for r in rec:
+        if per_event:
+            ids, flow = channel_ids(r["channel"])
+        mass = [m_top if abs(p) == 6 else 0.0 for p in ids]
         w = float(r["w"])
         xw = (1.0 if w >= 0 else -1.0) * max(1.0, abs(w) / w_max)
         out.write("<event>\n%2d %d %+.10e %.10e %.10e %.10e\n" % (n, 1, xw, scale, alpha_em, alpha_s))
@@ -76,7 +98,7 @@ class LheDrain:
         self.proc = proc
         self.wl = proc.wl
         self.compress = path.endswith(".gz") if compress is None else compress
-        self.dtype = record_dtype(proc.n_final)
+        self.dtype = record_dtype(proc.n_final, proc.wl.process)
         assert self.dtype.itemsize == proc.record_size
         self.side = torch.cuda.Stream()
         self.jobs = queue.Queue()
@@ -147,7 +169,7 @@ class LheDrain:
             f.write('<LesHouchesEvents version="3.0">\n<header>\n<!--\n')
             f.write("madflow-b200: %s, %d unweighted events (hit-or-miss against the running maximum weight)\n" %
                     (wl.name, self.n_written))
-            f.write("colour flow: ONE fixed planar flow per process (the event weights are colour summed)\n-->\n</header>\n")
+            f.write("colour flow: ONE fixed planar flow per partonic channel (the event weights are colour summed)\n-->\n</header>\n")
             f.write("<init>\n%d %d %.8e %.8e 0 0 0 0 3 1\n%.10e %.10e 1.0 1\n</init>\n" %
                     (beam[0], beam[1], wl.sqrt_s / 2, wl.sqrt_s / 2, xsec_pb, xerr_pb))
             with opener(self.body_path, "r") as b:

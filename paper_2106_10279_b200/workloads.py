@@ -68,7 +68,8 @@ C4 = Workload("C4 gg -> ttbar gg + unweighting", MF_GG_TTGG, sqrt_s=13000.0, ptm
 CONFIGS = [C0, C1, C2, C3, C4]
 # beyond BASELINE.json: the flavour-summed pp -> ttbar of PAPER.md L101 ("pp -> ttbar (7 diagrams)":
 # 3 gg + one q qbar diagram for each of 4 flavours), gluon and quark channels in ONE pass over the same points
-C5 = Workload("C5 pp -> ttbar (gg + q qbar)", MF_PP_TT, sqrt_s=13000.0, n_events=2 ** 20, n_iterations=10, n_adapt=10)
+C5 = Workload("C5 pp -> ttbar (gg + q qbar)", MF_PP_TT, sqrt_s=13000.0, n_events=2 ** 20, n_iterations=10, n_adapt=5,
+              unweight=True)
 EXTRA_CONFIGS = {"C5": C5}
 
 

@@ -56,6 +56,56 @@ def test_format_events_round_trip():
         assert [float(p[10]) for p in parts] == [0, 0, 173, 173, 0, 0]
 
 
+def test_flavour_summed_records_carry_their_partons():
+    """MF_PP_TT: PDG ids and colour flow follow the channel code of each record (include/mf.h)"""
+    rec = np.zeros(4, dtype=lhe.record_dtype(2, 4))
+    assert rec.dtype.itemsize == 4 * 32 + 24
+    rec["channel"] = [0, 1, 4, 7]
+    rec["w"] = 1.0
+    ev = _parse(lhe.format_events(rec, 4, 173.0, 173.0, 1 / 132.507, 0.118, w_max=1.0))
+    assert [[int(p[0]) for p in e[2]] for e in ev] == [[21, 21, 6, -6], [1, -1, 6, -6], [-2, 2, 6, -6], [4, -4, 6, -6]]
+    for _, _, parts, _ in ev:
+        col_in = sorted(int(p[4]) for p in parts[:2] if int(p[4]))
+        acol_in = sorted(int(p[5]) for p in parts[:2] if int(p[5]))
+        col_out = sorted(int(p[4]) for p in parts[2:] if int(p[4]))
+        acol_out = sorted(int(p[5]) for p in parts[2:] if int(p[5]))
+        for p in parts:             # quarks carry a colour, antiquarks an anticolour, gluons both
+            pid, c, a = int(p[0]), int(p[4]), int(p[5])
+            assert (c != 0) == (pid == 21 or pid > 0) and (a != 0) == (pid == 21 or pid < 0)
+        # colour is conserved: what flows in and does not annihilate flows out
+        assert sorted(set(col_in) - set(acol_in)) == col_out and sorted(set(acol_in) - set(col_in)) == acol_out
+
+
+@pytest.mark.gpu
+def test_lhe_drain_flavour_summed(tmp_path):
+    """the drain on MF_PP_TT records: every event of the file has the partons of its record's channel"""
+    import torch
+    from paper_2106_10279_b200 import api
+    wl = W.C5.scaled(30000, 2, 1)
+    gp = api.Process(wl, W.pdf_table_flavours())
+    grid, hist, res = gp.new_grid(), gp.new_hist(), gp.new_result()
+    gp.vegas_iterate(grid, 0, 0, 0, wl.n_events, hist, res)
+    gp.refine_grid(grid, hist)
+    w_max = gp.result_to_host(res).max_abs_w / 30
+    cap = 30000
+    records = torch.zeros(cap * gp.record_size, dtype=torch.uint8, device="cuda")
+    count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    path = str(tmp_path / "pp.lhe")
+    drain = lhe.LheDrain(path, gp)
+    gp.unweight(grid, 0, 1, 0, wl.n_events, w_max, records, cap, count, None, res)
+    n = drain.push(records, count, w_max, cap)
+    torch.cuda.synchronize()
+    mom, w, ids = gp.records_view(records, n)
+    chan = gp.last_channels[np.argsort(ids)]
+    assert drain.close(2760.0, 0.4) == n and n > 100 and (chan > 0).sum() > 5
+    ev = _parse(open(path).read())
+    assert len(ev) == n
+    for (nup, _, parts, _), c in zip(ev, chan):
+        want, _ = lhe.channel_ids(c)
+        assert nup == 4 and tuple(int(p[0]) for p in parts) == tuple(want)
+    gp.close()
+
+
 @pytest.mark.gpu
 @pytest.mark.parametrize("compress", [False, True])
 def test_lhe_drain_matches_records(tmp_path, compress, pdf):

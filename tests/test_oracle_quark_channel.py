@@ -197,3 +197,43 @@ def test_vegas_quark_part_agrees_with_quadrature(P4, oracle_procs, qq_quadrature
     assert sc / Ic < 1e-2
     assert abs(Ic - qq_quadrature) < 4 * sc
     assert 100.0 < qq_quadrature < 1000.0          # about a tenth of the gg channel with this synthetic table
+
+
+def test_channel_of_accepted_events(P4):
+    """R18: the channel code of an accepted event, recomputed here from single-table lookups, the closed-form matrix
+    elements and the raw Philox words; and its frequencies against their expectation."""
+    from test_oracle_amplitudes import esw_gg_ttbar
+    n = 6000
+    grid = W.uniform_grid(4)
+    rows = P4.debug_eval(grid, 2, 4, 100, n)
+    w = rows[:, 26]
+    w_max = float(np.quantile(np.abs(w), 0.7))
+    rec, cnt, _, res = P4.unweight(grid, 2, 4, 100, n, w_max, n)
+    mom, wr, ids = P4.records_view(rec, cnt)
+    chan = P4.last_channels
+    assert cnt == res.n_accept and cnt > 1500 and len(chan) == cnt
+    mu2 = MT ** 2
+    expect = np.zeros(1 + 2 * W.N_FLAVOURS)
+    for k in range(n):                         # expected channel counts: P(accept) x channel share, event by event
+        r = rows[k]
+        x1, x2, lum = r[20], r[21], r[22]
+        a = [abs(lum * r[23])]
+        for i in range(W.N_FLAVOURS):
+            q1, qb1 = P4.pdf_xf_table(1 + 2 * i, x1, mu2), P4.pdf_xf_table(2 + 2 * i, x1, mu2)
+            q2, qb2 = P4.pdf_xf_table(1 + 2 * i, x2, mu2), P4.pdf_xf_table(2 + 2 * i, x2, mu2)
+            a += [abs(q1 * qb2 / (x1 * x2) * r[-1]), abs(qb1 * q2 / (x1 * x2) * r[-1])]
+        a = np.array(a)
+        expect += min(1.0, abs(w[k]) / w_max) * a / a.sum()
+        hit = np.nonzero(ids == 100 + k)[0]
+        if len(hit):                           # this event was accepted: its channel from the raw words
+            words = mfo.philox_block(2, 4, 100 + k, 0xFFFFFFFF)
+            v = mfo.uniform_from_words(words[2], words[3]) * a.sum()
+            cum = np.cumsum(a)
+            if np.min(np.abs(cum - v)) > 1e-9 * a.sum():
+                assert chan[hit[0]] == int(np.argmax(cum > v)), k
+    assert abs(expect.sum() - cnt) < 5 * math.sqrt(cnt)
+    got = np.bincount(chan.astype(int), minlength=len(expect))
+    for c in range(len(expect)):
+        assert abs(got[c] - expect[c]) < 5 * math.sqrt(expect[c] + 1), (c, got[c], expect[c])
+    assert got[0] > 0.8 * cnt and got[1:].sum() > 30          # mostly gg; the quark channels do occur
+    assert got[3] + got[4] > 2 * (got[7] + got[8])             # u ubar (valence + a large sea) against c cbar (a small sea)
