@@ -170,9 +170,9 @@ def qq_quadrature(P4):
                 L += P4.pdf_xf_table(1 + 2 * i, x1, mu2) * P4.pdf_xf_table(2 + 2 * i, x2, mu2)
                 L += P4.pdf_xf_table(2 + 2 * i, x1, mu2) * P4.pdf_xf_table(1 + 2 * i, x2, mu2)
             return L / (x1 * x2)
-        val, _ = integrate.quad(lum, -ymax, ymax, epsabs=0, epsrel=1e-8, limit=400)
+        val, _ = integrate.quad(lum, -ymax, ymax, epsabs=0, epsrel=1e-6, limit=400)
         return val * tau * sigma_hat_qq(tau * S)
-    val, _ = integrate.quad(inner, math.log(tau_min), 0, epsabs=0, epsrel=1e-7, limit=400)
+    val, _ = integrate.quad(inner, math.log(tau_min), 0, epsabs=0, epsrel=1e-5, limit=400)
     return val * 0.3894e9
 
 
