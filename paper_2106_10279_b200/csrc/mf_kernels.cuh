@@ -80,20 +80,29 @@ MF_D double luminosity(const Params& P, const PassArgs& A, const double* s_lnx, 
 }
 
 // Process 4 (gg + q qbar channels; R17): x f(x) of every parton table at both beams; rows /
-// tables are ordered gluon, q_0, qbar_0, q_1, qbar_1, ...  One logarithm and one cell search per beam serve all tables.
+// tables are ordered gluon, q_0, qbar_0, q_1, qbar_1, ...
+// Dynamic scale (rare, large code): out of line and rolled, through memory.
+__device__ __noinline__ void parton_densities_dyn(const Params& P, const PassArgs& A, double x1, double x2, double mu2,
+                                                  double* f1, double* f2) {
+  const size_t tab = (size_t)P.pdf_nx * P.pdf_nq;
+#pragma unroll 1
+  for (int t = 0; t < P.pdf_nfl; ++t) {
+    f1[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, x1, mu2);
+    f2[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, x2, mu2);
+  }
+}
+// Fixed scale (the hot path): one logarithm and one cell search per beam serve all rows; everything in registers.
 MF_D void parton_densities(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
                            const Event<4>& ev, double* f1, double* f2, double& as_factor) {
   as_factor = 1.0;
   const int nt = P.pdf_nfl;
   if (P.dyn_scale) {
     const double mu2 = P.m_top * P.m_top + ev.k[0][1] * ev.k[0][1] + ev.k[0][2] * ev.k[0][2];
-    const size_t tab = (size_t)P.pdf_nx * P.pdf_nq;
+    double g1[kMaxPartonTables], g2[kMaxPartonTables];
+    parton_densities_dyn(P, A, ev.x1, ev.x2, mu2, g1, g2);
 #pragma unroll
     for (int t = 0; t < kMaxPartonTables; ++t)
-      if (t < nt) {
-        f1[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x1, mu2);
-        f2[t] = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf + t * tab, P.pdf_nx, P.pdf_nq, ev.x2, mu2);
-      }
+      if (t < nt) { f1[t] = g1[t]; f2[t] = g2[t]; }
     const double ratio = 1.0 / (1.0 + P.alpha_s * (23.0 / (12.0 * kPi)) * log(mu2 / P.mu2));
     as_factor = ratio * ratio;
   } else {
@@ -110,8 +119,7 @@ MF_D void parton_densities(const Params& P, const PassArgs& A, const double* s_l
 // the gluon-gluon luminosity (returned) and the flavour-summed quark luminosity
 //   lum_qq = sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2)
 MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
-                          const Event<4>& ev, double& as_factor, double& lum_qq) {
-  double f1[kMaxPartonTables], f2[kMaxPartonTables];
+                          const Event<4>& ev, double& as_factor, double& lum_qq, double* f1, double* f2) {
   parton_densities(P, A, s_lnx, s_row, ev, f1, f2, as_factor);
   const int nt = P.pdf_nfl;
   const double inv = 1.0 / (ev.x1 * ev.x2);
@@ -126,47 +134,48 @@ MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_ln
   return f1[0] * f2[0] * inv;
 }
 
-// Partonic channel of an ACCEPTED event of process 4 (R18): drawn in proportion to |luminosity x |M|^2| of
-// the channels, in channel order (0 gg; 1 + 2 i quark i from beam 1; 2 + 2 i quark i from beam 2): the first c with
-// sum_{c' <= c} |a_c'| > v sum |a|, v = the second uniform of the event's accept block.  Rare path: nothing is kept
-// from the weight computation, everything is formed again.
-__device__ __noinline__ unsigned long long select_channel(const Params& P, const PassArgs& A, const double* s_lnx,
-                                                          const double* s_row, const Event<4>& ev, uint64_t event) {
-  double f1[kMaxPartonTables], f2[kMaxPartonTables], asf, me_qq;
-  parton_densities(P, A, s_lnx, s_row, ev, f1, f2, asf);
-  const double me_gg = me2_pp_call(P, ev.shat, ev.k, me_qq);
-  const int nt = P.pdf_nfl;
-  const double inv = 1.0 / (ev.x1 * ev.x2);
-  double a[kMaxPartonTables], total = 0.0;
-  a[0] = fabs(f1[0] * f2[0] * inv * (me_gg * asf));
-  for (int t = 1; t + 1 < nt; t += 2) {
-    a[t] = fabs(f1[t] * f2[t + 1] * inv * (me_qq * asf));
-    a[t + 1] = fabs(f1[t + 1] * f2[t] * inv * (me_qq * asf));
-  }
-  for (int c = 0; c < nt; ++c) total += a[c];
-  const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);
-  const double v = uniform52(r.z, r.w) * total;
-  double cum = 0.0;
-  for (int c = 0; c < nt; ++c) {
-    cum += a[c];
-    if (cum > v) return (unsigned long long)c;
-  }
-  return (unsigned long long)(nt - 1);
-}
-
 // a6-a10 of one event that passed the cuts (thread-per-event kernels): luminosity, |M|^2, weight.
 // parts (optional): lum, me2 [, lum_qq, me2_qq for process 4] for the debug rows.
+// channel (optional, process 4; R18): the partonic channel this event gets IF it is accepted, drawn in
+// proportion to |luminosity x |M|^2| of the channels, in channel order (0 gg; 1 + 2 i quark i from beam 1; 2 + 2 i quark
+// i from beam 2): the first c with sum_{c' <= c} |a_c'| > v sum |a|, v = the second uniform of the accept block.  It
+// is formed here, where the densities are in registers (a few dozen flop), not again for the accepted events.
 template <int PROC>
 MF_D double weigh_event(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
-                        const Event<PROC>& ev, double* parts) {
+                        const Event<PROC>& ev, double* parts, double v = 0.0, unsigned* channel = nullptr) {
   double asf;
   if constexpr (PROC == 4) {
-    double lum_qq;
-    const double lum = luminosity_pp(P, A, s_lnx, s_row, ev, asf, lum_qq);
+    double lum_qq, f1[kMaxPartonTables], f2[kMaxPartonTables];
+    const double lum = luminosity_pp(P, A, s_lnx, s_row, ev, asf, lum_qq, f1, f2);
     double me_qq;
     const double me_gg = me2_pp_call(P, ev.shat, ev.k, me_qq) * asf;
     me_qq *= asf;
     if (parts) { parts[0] = lum; parts[1] = me_gg; parts[2] = lum_qq; parts[3] = me_qq; }
+    if (channel) {
+      const int nt = P.pdf_nfl;
+      const double inv = 1.0 / (ev.x1 * ev.x2);
+      double a[kMaxPartonTables], total;
+      a[0] = total = fabs(lum * me_gg);
+#pragma unroll
+      for (int t = 1; t + 1 < kMaxPartonTables; t += 2)
+        if (t + 1 < nt) {
+          a[t] = fabs(f1[t] * f2[t + 1] * inv * me_qq);
+          a[t + 1] = fabs(f1[t + 1] * f2[t] * inv * me_qq);
+          total += a[t];
+          total += a[t + 1];
+        }
+      const double vt = v * total;
+      double cum = 0.0;
+      unsigned pick = (unsigned)(nt - 1);
+      bool found = false;
+#pragma unroll
+      for (int c = 0; c < kMaxPartonTables; ++c)
+        if (c < nt) {
+          cum += a[c];
+          if (!found && cum > vt) { pick = (unsigned)c; found = true; }
+        }
+      *channel = pick;
+    }
     return event_weight<PROC>(P, ev, 1.0, fma(lum, me_gg, lum_qq * me_qq));
   } else {
     const double lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
@@ -224,7 +233,7 @@ struct Accum {
 template <int PROC, bool UNW>
 MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_grid, double* s_hist, bool valid,
                            uint64_t event, double w, const Bins<PROC>& bins, Accum& acc, int obs_bins,
-                           const double* s_lnx = nullptr, const double* s_row = nullptr) {
+                           unsigned channel = 0u, const Event<PROC>* ev_live = nullptr) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   const int nb = P.n_bins;
   const double w2 = w * w;
@@ -253,11 +262,16 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
         ++acc.n_acc;
         unsigned long long slot = base + __popc(m & ((1u << lane) - 1u));
         if (A.records != nullptr && slot < A.capacity) {
-          // accepted events are rare (<1 %): regenerate the kinematics instead of keeping them live
+          // cooperative kernels (accepted events are rare, < 1 %, registers are not): regenerate the kinematics instead
+          // of keeping them live; the thread-per-event kernels pass the event they still hold
           Event<PROC> ev;
-          Bins<PROC> b2;
-          DebugRow dbg = {nullptr, D, NF};
-          generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
+          if (ev_live != nullptr) {
+            ev = *ev_live;
+          } else {
+            Bins<PROC> b2;
+            DebugRow dbg = {nullptr, D, NF};
+            generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
+          }
           double mom[NF + 2][4];
           lab_momenta<PROC>(ev, mom);
           double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16 + (PROC == 4 ? 8 : 0)));
@@ -267,8 +281,7 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
             for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
           rec[4 * (NF + 2)] = w;
           reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
-          if constexpr (PROC == 4)
-            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = select_channel(P, A, s_lnx, s_row, ev, event);
+          if (PROC == 4) reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = channel;
         }
       }
     }
@@ -316,7 +329,7 @@ MF_D void block_finish(const PassArgs& A, Accum acc, double* s_red, const double
 
 // ---- the fused pass, one thread per event (e+e- -> mu+mu-, gg -> ttbar, pp -> ttbar) ----------------------
 template <int PROC, bool UNW>
-__global__ void __launch_bounds__(kThreads, (PROC == 1 || PROC == 4) ? 4 : 2) fused_pass_kernel(const Params P, const PassArgs A) {
+__global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel(const Params P, const PassArgs A) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   extern __shared__ double smem[];
   const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx, nrow = PROC == 4 ? nx * P.pdf_nfl : nx;
@@ -342,17 +355,23 @@ __global__ void __launch_bounds__(kThreads, (PROC == 1 || PROC == 4) ? 4 : 2) fu
     Bins<PROC> bins;
     bins.clear();
     int obs_bins = 0;
+    unsigned channel = 0u;
+    Event<PROC> ev;
     if (valid) {
-      Event<PROC> ev;
       DebugRow dbg = {nullptr, D, NF};
       generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
       if (ev.pass && A.obs != nullptr) obs_bins = observable_bins<PROC>(A, ev);
       if (ev.pass) {
         ++acc.n_pass;
-        w = weigh_event<PROC>(P, A, s_lnx, s_row, ev, nullptr);
+        if (PROC == 4 && UNW) {
+          const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);      // words z, w: the channel draw
+          w = weigh_event<PROC>(P, A, s_lnx, s_row, ev, nullptr, uniform52(r.z, r.w), &channel);
+        } else {
+          w = weigh_event<PROC>(P, A, s_lnx, s_row, ev, nullptr);
+        }
       }
     }
-    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins, s_lnx, s_row);
+    accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins, channel, PROC == 0 ? nullptr : &ev);
   }
   block_finish(A, acc, s_red, s_hist, D * nb);
 }
