@@ -59,6 +59,13 @@ __device__ __noinline__ double me2_pp_call(const Params& P, double shat, const d
 // the factor that rescales |M|^2 (1 at the fixed scale).  Dynamic scale (R16; mf_set_dynamic_scale):
 // mu_F^2 = mu_R^2 = m_t^2 + pT(top)^2 per event, F by the general 2-D lookup in the table (global memory / L2),
 // alpha_s running at one loop (n_f = 5) from its value at the descriptor's mu2: |M|^2 ~ alpha_s^{n_g}.
+// (the two general 2-D lookups of the rarely used dynamic scale are kept out of line: the fused kernels are
+// instruction-cache sensitive)
+__device__ __noinline__ double pdf_pair_2d(const Params& P, const PassArgs& A, double x1, double x2, double mu2,
+                                           double& f2) {
+  f2 = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf, P.pdf_nx, P.pdf_nq, x2, mu2);
+  return pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf, P.pdf_nx, P.pdf_nq, x1, mu2);
+}
 template <int PROC>
 MF_D double luminosity(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
                        const Event<PROC>& ev, double& as_factor) {
@@ -67,8 +74,7 @@ MF_D double luminosity(const Params& P, const PassArgs& A, const double* s_lnx, 
   double f1, f2;
   if (P.dyn_scale) {
     const double mu2 = P.m_top * P.m_top + ev.k[0][1] * ev.k[0][1] + ev.k[0][2] * ev.k[0][2];
-    f1 = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf, P.pdf_nx, P.pdf_nq, ev.x1, mu2);
-    f2 = pdf_xf_2d(A.pdf_lnx, A.pdf_lnq2, A.pdf_xf, P.pdf_nx, P.pdf_nq, ev.x2, mu2);
+    f1 = pdf_pair_2d(P, A, ev.x1, ev.x2, mu2, f2);
     const double ratio = 1.0 / (1.0 + P.alpha_s * (23.0 / (12.0 * kPi)) * log(mu2 / P.mu2));
 #pragma unroll
     for (int g = 0; g < Traits<PROC>::NG; ++g) as_factor *= ratio;
