@@ -301,16 +301,18 @@ class Process:
         lib().mfo_count_ops_event(self.h, _dp(grid), seed, iteration, event, out)
         return dict(zip(["add", "mul", "div", "sqrt", "trans", "cmp"], list(out)))
 
-    def records_view(self, rec, count):
-        """Decode `count` AoS records into (momenta[count, n+2, 4], w[count], event_id[count])."""
+    def records_array(self, rec, count):
+        """Decode `count` AoS records into a structured array: mom[n+2][4], w, id and, for process 4, channel."""
         fields = [("mom", np.float64, (self.n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)]
         if self.wl.process == 4:
             fields.append(("channel", np.uint64))
         dt = np.dtype(fields)
         assert dt.itemsize == self.record_size
-        a = np.frombuffer(rec.tobytes()[:count * self.record_size], dtype=dt)
-        if self.wl.process == 4:
-            self.last_channels = a["channel"]
+        return np.frombuffer(rec.tobytes()[:count * self.record_size], dtype=dt)
+
+    def records_view(self, rec, count):
+        """(momenta[count, n+2, 4], w[count], event_id[count])"""
+        a = self.records_array(rec, count)
         return a["mom"], a["w"], a["id"]
 
 

@@ -272,15 +272,18 @@ class Process:
                "mf_debug_me2")
         return out.cpu().numpy()
 
-    def records_view(self, records, count):
-        """Decode `count` AoS records (uint8 tensor) into (momenta[count, n+2, 4], w[count], id[count])."""
+    def records_array(self, records, count):
+        """Decode `count` AoS records (uint8 tensor) into a numpy structured array with fields mom[n+2][4], w, id and,
+        for MF_PP_TT, channel (include/mf.h)."""
         from .lhe import record_dtype
         dt = record_dtype(self.n_final, self.wl.process)
         assert dt.itemsize == self.record_size
         raw = records[:count * self.record_size].cpu().numpy().tobytes()
-        a = np.frombuffer(raw, dtype=dt)
-        if "channel" in dt.names:
-            self.last_channels = a["channel"]       # MF_PP_TT: the partonic channel codes of the decoded records
+        return np.frombuffer(raw, dtype=dt)
+
+    def records_view(self, records, count):
+        """(momenta[count, n+2, 4], w[count], id[count]) of `count` records"""
+        a = self.records_array(records, count)
         return a["mom"], a["w"], a["id"]
 
 

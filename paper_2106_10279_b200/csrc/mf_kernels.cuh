@@ -43,14 +43,17 @@ struct PassArgs {
   double* coop_queue;      // cooperative kernels only: [gridDim.x][blockDim.x][18] momenta queue (mf_kernels_coop.cuh)
 };
 
-// The matrix element is the only large piece of code; keep ONE copy per process per kernel.
+#define MF_ME_CALL __device__ __forceinline__
+// The matrix element is the only large piece of code, with ONE call site per thread-per-event kernel: inlined, so that
+// the momenta stay in registers (an out-of-line call passes them through local memory: +4 % / +9 % time for gg -> ttbar /
+// e+e- -> mu+mu-).
 template <int PROC>
-__device__ __noinline__ double me2_call(const Params& P, double shat, const double (*k)[4]) {
+MF_ME_CALL double me2_call(const Params& P, double shat, const double (*k)[4]) {
   return matrix_element<PROC>(P, shat, k);
 }
 
 // process 4: both channels in ONE out-of-line call, so that the top-quark spinors are formed once
-__device__ __noinline__ double me2_pp_call(const Params& P, double shat, const double (*k)[4], double& me_qq) {
+MF_ME_CALL double me2_pp_call(const Params& P, double shat, const double (*k)[4], double& me_qq) {
   me_qq = matrix_element_qq(P, shat, k);
   return matrix_element<4>(P, shat, k);
 }

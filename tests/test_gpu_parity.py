@@ -351,7 +351,8 @@ def test_unweight(proc, n, gpu_procs, oracle_procs):
             if proc == 4:
                 # the partonic channel drawn for every accepted event (R18): an integer decided by floating point; both
                 # sides decide in fp64, and no event of this stream sits within rounding of a channel boundary
-                ch_g, ch_o = gp.last_channels[order], op.last_channels
+                ch_g = gp.records_array(records[start * gp.record_size:], n_written)["channel"][order]
+                ch_o = op.records_array(rec_o, cnt_o)["channel"]
                 assert np.array_equal(ch_g, ch_o)
                 assert (ch_o == 0).sum() > 0.8 * cnt_o and (ch_o > 0).sum() > 10 and ch_o.max() <= 2 * W.N_FLAVOURS
         else:

@@ -96,7 +96,7 @@ def test_lhe_drain_flavour_summed(tmp_path):
     n = drain.push(records, count, w_max, cap)
     torch.cuda.synchronize()
     mom, w, ids = gp.records_view(records, n)
-    chan = gp.last_channels[np.argsort(ids)]
+    chan = gp.records_array(records, n)["channel"][np.argsort(ids)]
     assert drain.close(2760.0, 0.4) == n and n > 100 and (chan > 0).sum() > 5
     ev = _parse(open(path).read())
     assert len(ev) == n

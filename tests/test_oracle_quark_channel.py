@@ -210,7 +210,7 @@ def test_channel_of_accepted_events(P4):
     w_max = float(np.quantile(np.abs(w), 0.7))
     rec, cnt, _, res = P4.unweight(grid, 2, 4, 100, n, w_max, n)
     mom, wr, ids = P4.records_view(rec, cnt)
-    chan = P4.last_channels
+    chan = P4.records_array(rec, cnt)["channel"]
     assert cnt == res.n_accept and cnt > 1500 and len(chan) == cnt
     mu2 = MT ** 2
     expect = np.zeros(1 + 2 * W.N_FLAVOURS)
