@@ -29,7 +29,13 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-METRIC = "integrand events/sec (fp64) for gg->ttbar gg"
+METRIC = "integrand events/sec (fp64) for gg->ttbar gg"      # BASELINE.json metric (C3, C4)
+PROCESS_LABEL = {0: "e+e- -> mu+mu-", 1: "gg->ttbar", 2: "gg->ttbar g", 3: "gg->ttbar gg", 4: "pp->ttbar (gg + q qbar)"}
+
+
+def metric_for(wl):
+    """the BASELINE.json metric for the headline process; the same quantity, named after its process, for --config"""
+    return METRIC if wl.process == 3 else "integrand events/sec (fp64) for " + PROCESS_LABEL[wl.process]
 UNIT = "events/s"
 # static fp64 operation counts per matrix-element evaluation, written by csrc/gen_me.py into
 # mf_me_ggtt_generated.cuh (kFlopsMe2_*); per-event work outside the matrix element (DESIGN.md table)
@@ -168,7 +174,7 @@ def run_reference(args, wl):
     tot = sum(times)
     val = n * len(times) / tot
     sample = "%d events/step of %s (iteration k on the oracle's own adapting grid), 1 thread" % (n, wl.name)
-    print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+    print(json.dumps({"impl": "reference", "metric": metric_for(wl), "value": val, "unit": UNIT, "n_gpus": args.gpus,
                       "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
                       "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                       "data": "synthetic", "config": {"workload": wl.name, "events_per_step": n},
@@ -340,7 +346,7 @@ def main():
     peak_flops, _ = api.mf_measure_fp64_peak(1 << 17)
     peak = peak_flops / 1e12
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": metric_for(wl), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "ms_per_step_median": sorted(ms)[len(ms) // 2], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s: BASELINE.json configs[%d], %d events/step/GPU, step = mf_unweight + mf_refine_grid"
