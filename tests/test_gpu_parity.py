@@ -420,7 +420,7 @@ def test_full_size_sampled(proc, gpu_procs, oracle_procs):
 
 
 # ---- other bin counts (the launch shape of the cooperative kernels depends on the shared memory left) --------------
-@pytest.mark.parametrize("proc,n", [(1, 20_000), (2, 3_000), (3, 700)])
+@pytest.mark.parametrize("proc,n", [(1, 20_000), (2, 3_000), (3, 700), (4, 12_000)])
 @pytest.mark.parametrize("nb", [8, 128])
 def test_other_bin_counts(proc, n, nb, pdf):
     from dataclasses import replace
@@ -428,6 +428,8 @@ def test_other_bin_counts(proc, n, nb, pdf):
     from paper_2106_10279_b200 import api
     torch = _torch()
     wl = replace(WLS[proc], n_bins=nb)
+    if proc == W.MF_PP_TT:
+        pdf = W.pdf_table_flavours()
     gp, op = api.Process(wl, pdf), mfo.Process(wl, pdf)
     try:
         grid = W.uniform_grid(wl.n_dims, nb)
@@ -438,6 +440,45 @@ def test_other_bin_counts(proc, n, nb, pdf):
         gp.vegas_iterate(torch.from_numpy(grid).cuda(), 1, 1, 5, n, hist, res)
         torch.cuda.synchronize()
         _check_sums(n, hist.cpu().numpy(), gp.result_to_host(res), ho, ro)
+    finally:
+        gp.close()
+
+
+# ---- other flavour counts of the multi-flavour table (1, 2 and 5 quark flavours) ----------------------------------------
+@pytest.mark.parametrize("n_tables", [3, 5, 11])
+def test_other_flavour_counts(n_tables):
+    from oracle import mfo
+    from paper_2106_10279_b200 import api
+    torch = _torch()
+    lnx, lnq2, xf = W.pdf_table_flavours()
+    if n_tables <= xf.shape[0]:
+        xf = np.ascontiguousarray(xf[:n_tables])
+    else:                                  # a fifth flavour: half the charm sea
+        xf = np.ascontiguousarray(np.concatenate([xf, 0.5 * xf[7:9]]))
+    assert xf.shape[0] == n_tables
+    wl = W.C5
+    gp, op = api.Process(wl, (lnx, lnq2, xf)), mfo.Process(wl, (lnx, lnq2, xf))
+    try:
+        grid = adapted_grid(op, wl)
+        dgrid = torch.from_numpy(grid).cuda()
+        n = 2000
+        g, o = gp.debug_eval(dgrid, 1, 2, 3, n), op.debug_eval(grid, 1, 2, 3, n)
+        _compare_rows(wl, g, o)
+        c = _cols(wl)
+        w_max = float(np.quantile(np.abs(o[:, c["w"]]), 0.8))
+        rec_o, cnt_o, hist_o, res_o = op.unweight(grid, 1, 2, 3, n, w_max, n)
+        records = torch.zeros(n * gp.record_size, dtype=torch.uint8, device="cuda")
+        count = torch.zeros(1, dtype=torch.int64, device="cuda")
+        hist, res = gp.new_hist(), gp.new_result()
+        gp.unweight(dgrid, 1, 2, 3, n, w_max, records, n, count, hist, res)
+        torch.cuda.synchronize()
+        assert int(count.item()) == cnt_o > 300
+        _check_sums(n, hist.cpu().numpy(), gp.result_to_host(res), hist_o, res_o)
+        a_g, a_o = gp.records_array(records, cnt_o), op.records_array(rec_o, cnt_o)
+        order = np.argsort(a_g["id"])
+        assert np.array_equal(a_g["id"][order], a_o["id"])
+        assert np.array_equal(a_g["channel"][order], a_o["channel"])
+        assert a_o["channel"].max() <= n_tables - 1 and (a_o["channel"] > 0).any()
     finally:
         gp.close()
 
