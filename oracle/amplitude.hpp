@@ -649,4 +649,149 @@ template <class R> inline void dressed_init(DressedContext<R>& d) {
       }
 }
 
+// ---------------------------------------------------------------------------------------------
+// O10 (quark channels with one gluon, "pp -> ttbar g (36 diagrams)": 16 gg + 5 for each
+// of q qbar -> ttbar g, q g -> ttbar q, ...).  GROUNDWORK: no kernel evaluates these yet.
+//
+// One massless quark line, the top line and one external gluon; the five tree diagrams written out from the Feynman
+// rules (quark-gluon vertex i g gamma^mu T^a, fermion propagator i (pslash + m)/(p^2 - m^2), gluon propagator
+// -i g_{mu nu} delta^{ab}/q^2, three-gluon vertex g f^{abc} [g^{mu nu}(k1-k2)^rho + g^{nu rho}(k2-k3)^mu +
+// g^{rho mu}(k3-k1)^nu], all momenta incoming), for explicit colours.
+// The light line is given by its column spinor C with fermion-flow momentum pc INTO the line and its row spinor Rw with
+// flow momentum pr OUT of it; the gluon by its wavefunction E and OUTGOING momentum kg:
+//   q(p1) qbar(p2) -> t tbar g(k5):  C = u(p1), pc = p1;  Rw = vbar(p2), pr = -p2;  E = eps*(k5), kg = k5
+//   q(p1) g(p2) -> t tbar q(p5):     C = u(p1), pc = p1;  Rw = ubar(p5), pr = p5;   E = eps(p2),   kg = -p2
+// kin[0..4] = the colour-stripped amplitudes of the diagrams (gluon from the light line before / after the virtual
+// gluon, from the top, from the antitop, three-gluon vertex), with all factors of i and g included.
+template <class R> inline Mat4<R> slash_plus_mass(const R p[4], R m) {
+  Mat4<R> M = slash(cvec_from_real(p));
+  for (int i = 0; i < 4; ++i) M.m[i][i] += Cx<R>(m);
+  return M;
+}
+template <class R> inline Spinor<R> row_times_mat(const Spinor<R>& row, const Mat4<R>& M) {
+  Spinor<R> o;
+  for (int j = 0; j < 4; ++j)
+    for (int i = 0; i < 4; ++i) o.c[j] += row.c[i] * M.m[i][j];
+  return o;
+}
+template <class R>
+inline void light_line_ttbar_g_diagrams(const Spinor<R>& Rw, const R pr[4], const Spinor<R>& C, const R pc[4],
+                                        const Spinor<R>& ub3, const R p3[4], const Spinor<R>& v4, const R p4[4],
+                                        const CVec4<R>& E, const R kg[4], R mt, R g, Cx<R> kin[5]) {
+  const Cx<R> I = cx_i<R>();
+  R ql[4], qt[4], a1[4], a2[4], t1[4], t2[4];
+  for (int m = 0; m < 4; ++m) {
+    ql[m] = pc[m] - pr[m];            // virtual gluon leaving the light line when the gluon is not emitted from it
+    qt[m] = p3[m] + p4[m];            // virtual gluon entering the top line when the gluon is not emitted from it
+    a1[m] = pc[m] - kg[m];            // light-line propagator, emission on the incoming side
+    a2[m] = pr[m] + kg[m];            // light-line propagator, emission on the outgoing side
+    t1[m] = p3[m] + kg[m];            // top propagator, emission from the top
+    t2[m] = -p4[m] - kg[m];           // top propagator, emission from the antitop
+  }
+  const R sl = mdot_rr(ql, ql), st = mdot_rr(qt, qt);
+  const Mat4<R> Es = slash(E);
+  const Cx<R> vert3 = (I * g) * (I * g) * (I * g);      // three quark-gluon vertices
+  const Cx<R> fprop = I, gprop = -I;
+  // currents with an open Lorentz index
+  CVec4<R> jl, jt, jlA, jlB, jtC, jtD;
+  const Spinor<R> lineA = mat_vec(slash_plus_mass(a1, R(0)), mat_vec(Es, C));        // (a1-slash) E-slash C
+  const Spinor<R> rowB = row_times_mat(row_times_mat(Rw, Es), slash_plus_mass(a2, R(0)));
+  const Spinor<R> rowC = row_times_mat(row_times_mat(ub3, Es), slash_plus_mass(t1, mt));
+  const Spinor<R> colD = mat_vec(slash_plus_mass(t2, mt), mat_vec(Es, v4));
+  for (int mu = 0; mu < 4; ++mu) {
+    const Mat4<R> gm = gamma_matrix<R>(mu);
+    jl.c[mu] = row_times_col(Rw, mat_vec(gm, C));
+    jt.c[mu] = row_times_col(ub3, mat_vec(gm, v4));
+    jlA.c[mu] = row_times_col(Rw, mat_vec(gm, lineA));
+    jlB.c[mu] = row_times_col(rowB, mat_vec(gm, C));
+    jtC.c[mu] = row_times_col(rowC, mat_vec(gm, v4));
+    jtD.c[mu] = row_times_col(ub3, mat_vec(gm, colD));
+  }
+  const R dA = mdot_rr(a1, a1), dB = mdot_rr(a2, a2), dC = mdot_rr(t1, t1) - mt * mt, dD = mdot_rr(t2, t2) - mt * mt;
+  kin[0] = vert3 * fprop * gprop * mdot(jlA, jt) / (dA * st);
+  kin[1] = vert3 * fprop * gprop * mdot(jlB, jt) / (dB * st);
+  kin[2] = vert3 * fprop * gprop * mdot(jl, jtC) / (dC * sl);
+  kin[3] = vert3 * fprop * gprop * mdot(jl, jtD) / (dD * sl);
+  // three-gluon vertex with incoming momenta k1 = ql (index mu, from the light line), k2 = -qt (index nu, to the top
+  // line), k3 = -kg (index rho, the external gluon):  jl_mu jt_nu E_rho V^{mu nu rho}
+  CVec4<R> k12, k23, k31;
+  for (int m = 0; m < 4; ++m) {
+    k12.c[m] = Cx<R>(ql[m] + qt[m]);
+    k23.c[m] = Cx<R>(-qt[m] + kg[m]);
+    k31.c[m] = Cx<R>(-kg[m] - ql[m]);
+  }
+  const Cx<R> V = mdot(jl, jt) * mdot(k12, E) + mdot(jt, E) * mdot(k23, jl) + mdot(E, jl) * mdot(k31, jt);
+  kin[4] = (I * g) * (I * g) * Cx<R>(g) * gprop * gprop * V / (sl * st);
+}
+
+// colour tensors of the five diagrams, contracted over all colours: CC[d][e] = sum_{i j k l a} conj(C_d) C_e with
+//   C_0 = (T^b T^a)_{ji} T^b_{kl},  C_1 = (T^a T^b)_{ji} T^b_{kl},  C_2 = T^b_{ji} (T^a T^b)_{kl},
+//   C_3 = T^b_{ji} (T^b T^a)_{kl},  C_4 = f^{bca} T^b_{ji} T^c_{kl}
+// (j, i = colours of the light line's row and column spinor, k, l = of the top's; a = the external gluon), brute force.
+template <class R> inline void light_line_colour_matrix(Cx<R> CC[5][5]) {
+  Mat3<R> T[8];
+  for (int a = 0; a < 8; ++a) T[a] = su3_generator<R>(a);
+  for (int d = 0; d < 5; ++d)
+    for (int e = 0; e < 5; ++e) CC[d][e] = Cx<R>();
+  for (int a = 0; a < 8; ++a) {
+    Mat3<R> TbTa[8], TaTb[8];
+    for (int b = 0; b < 8; ++b) { TbTa[b] = mat3_mul(T[b], T[a]); TaTb[b] = mat3_mul(T[a], T[b]); }
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j)
+        for (int k = 0; k < 3; ++k)
+          for (int l = 0; l < 3; ++l) {
+            Cx<R> c[5];
+            for (int b = 0; b < 8; ++b) {
+              c[0] += TbTa[b].m[j][i] * T[b].m[k][l];
+              c[1] += TaTb[b].m[j][i] * T[b].m[k][l];
+              c[2] += T[b].m[j][i] * TaTb[b].m[k][l];
+              c[3] += T[b].m[j][i] * TbTa[b].m[k][l];
+              for (int cc = 0; cc < 8; ++cc) {
+                R f = structure_constant<R>(b, cc, a);
+                if (f != R(0)) c[4] += (T[b].m[j][i] * T[cc].m[k][l]) * f;
+              }
+            }
+            for (int d = 0; d < 5; ++d)
+              for (int e = 0; e < 5; ++e) CC[d][e] += conj(c[d]) * c[e];
+          }
+  }
+}
+// Averaged |M|^2.  kind 0: q(mom0) qbar(mom1) -> t(mom2) tbar(mom3) g(mom4), average 1/(4 x 9);
+// kind 1: q(mom0) g(mom1) -> t(mom2) tbar(mom3) q(mom4), average 1/(4 x 24).  subst != 0 replaces the gluon's
+// polarisation vector by its momentum (the Ward identity: the result must vanish).
+template <class R>
+inline R me2_light_line_ttbar_g(int kind, const R mom[5][4], R mt, R alpha_s, int basis, int subst) {
+  const R g = r_sqrt(R(4) * r_pi<R>() * alpha_s);
+  const int sb = basis & 1, pb = (basis >> 1) & 1;
+  Cx<R> CC[5][5];
+  light_line_colour_matrix<R>(CC);
+  R pr[4], kg[4];
+  const R* pg = kind == 0 ? mom[4] : mom[1];       // the gluon's physical momentum
+  const R* prow = kind == 0 ? mom[1] : mom[4];     // the particle behind the light line's row spinor
+  for (int m = 0; m < 4; ++m) {
+    pr[m] = kind == 0 ? -prow[m] : prow[m];
+    kg[m] = kind == 0 ? pg[m] : -pg[m];
+  }
+  R total = R(0);
+  for (int l1 = -1; l1 <= 1; l1 += 2)
+    for (int l2 = -1; l2 <= 1; l2 += 2)
+      for (int l3 = -1; l3 <= 1; l3 += 2)
+        for (int l4 = -1; l4 <= 1; l4 += 2)
+          for (int lg = -1; lg <= 1; lg += 2) {
+            const Spinor<R> C = u_spinor(mom[0], R(0), l1, sb);
+            const Spinor<R> Rw = kind == 0 ? bar(v_spinor(prow, R(0), l2, sb)) : bar(u_spinor(prow, R(0), l2, sb));
+            const Spinor<R> ub3 = bar(u_spinor(mom[2], mt, l3, sb)), v4 = v_spinor(mom[3], mt, l4, sb);
+            CVec4<R> E = polarisation(pg, lg, pb);
+            if (kind == 0) E = cconj(E);
+            if (subst) E = cvec_from_real(pg);
+            Cx<R> kin[5];
+            light_line_ttbar_g_diagrams<R>(Rw, pr, C, mom[0], ub3, mom[2], v4, mom[3], E, kg, mt, g, kin);
+            Cx<R> acc;
+            for (int d = 0; d < 5; ++d)
+              for (int e = 0; e < 5; ++e) acc += conj(kin[d]) * CC[d][e] * kin[e];
+            total = total + acc.re;
+          }
+  return total / (kind == 0 ? R(36) : R(96));
+}
+
 }  // namespace mfo

@@ -481,6 +481,20 @@ double mfo_me2_qq(const mfo_process* P, const double* mom, int basis, int prec) 
     for (int c = 0; c < 4; ++c) m[i][c] = mom[4 * i + c];
   return me2_qq_ttbar<double>(m, P->d.m_top, P->d.alpha_s, basis);
 }
+double mfo_me2_light_line_ttbar_g(int kind, const double* mom, double mt, double alpha_s, int basis, int subst,
+                                  int prec) {
+  if (!mom || kind < 0 || kind > 1) return -1.0;
+  if (prec == 1) {
+    long double m[5][4];
+    for (int i = 0; i < 5; ++i)
+      for (int c = 0; c < 4; ++c) m[i][c] = mom[4 * i + c];
+    return (double)me2_light_line_ttbar_g<long double>(kind, m, mt, alpha_s, basis, subst);
+  }
+  double m[5][4];
+  for (int i = 0; i < 5; ++i)
+    for (int c = 0; c < 4; ++c) m[i][c] = mom[4 * i + c];
+  return me2_light_line_ttbar_g<double>(kind, m, mt, alpha_s, basis, subst);
+}
 int mfo_colour_matrix(int n, double* out) {
   if (n < 1 || n > 5) return -1;
   std::vector<double> C = colour_matrix<double>(n);

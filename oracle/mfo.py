@@ -68,6 +68,8 @@ def lib():
         L.mfo_count_ops_event.argtypes = [C.c_void_p, c_double_p, C.c_uint64, C.c_uint32, C.c_uint64, c_u64_p]
         L.mfo_colour_matrix.argtypes = [C.c_int, c_double_p]
         L.mfo_set_dynamic_scale.argtypes = [C.c_void_p, C.c_int32]
+        L.mfo_me2_light_line_ttbar_g.restype = C.c_double
+        L.mfo_me2_light_line_ttbar_g.argtypes = [C.c_int, c_double_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int]
         L.mfo_me2_qq.restype = C.c_double
         L.mfo_me2_qq.argtypes = [C.c_void_p, c_double_p, C.c_int, C.c_int]
         L.mfo_pdf_xf_table.restype = C.c_double
@@ -144,6 +146,12 @@ def boost_z(y, p):
     out = np.empty(4)
     lib().mfo_boost_z(y, _dp(p), _dp(out))
     return out
+
+
+def me2_light_line_ttbar_g(kind, mom, mt, alpha_s, basis=0, subst=0, prec=0):
+    """kind 0: q qbar -> t tbar g; kind 1: q g -> t tbar q (mom: 5 x 4, the two incoming first); oracle/mfo.h"""
+    mom = _f64(mom)
+    return lib().mfo_me2_light_line_ttbar_g(kind, _dp(mom), mt, alpha_s, basis, subst, prec)
 
 
 def colour_matrix(n):

@@ -1,0 +1,115 @@
+"""Pins for the oracle's q qbar -> t tbar g and q g -> t tbar q matrix elements (the quark channels of pp -> ttbar g,
+PAPER.md L101).  GROUNDWORK: no kernel evaluates these yet; the oracle
+is written and pinned first.  CPU only.
+
+The oracle sums the five Feynman diagrams with explicit SU(3) generators and structure constants.  What fixes it:
+  * the Ward identity: with the gluon's polarisation vector replaced by its momentum the colour-summed |M|^2 vanishes
+    (any wrong relative sign, factor of i, propagator momentum or colour order among the five diagrams breaks it);
+  * independence of the spinor and polarisation bases, charge conjugation;
+  * the collinear limits, which fix the overall normalisation against matrix elements pinned elsewhere:
+      k_g || p_q    in q qbar -> ttbar g :  8 pi alpha_s / (2 p.k)  P_qq(z) / z  |M(q qbar -> ttbar)|^2,  P_qq = C_F (1+z^2)/(1-z)
+      p_q' || p_g   in q g -> ttbar q    :  8 pi alpha_s / (2 p.k)  P_qg(z) / z  |M(q qbar -> ttbar)|^2,  P_qg = T_R (z^2+(1-z)^2)
+      p_q' || p_q   in q g -> ttbar q    :  8 pi alpha_s / (2 p.k)  P_gq(z) / z  |M(g g -> ttbar)|^2 after averaging over the
+                                            azimuth of the splitting,                                   P_gq = C_F (1+(1-z)^2)/z
+    (Altarelli-Parisi kernels; z = momentum fraction entering the hard process); the Born matrix elements are the
+    textbook closed forms, typed out in the tests.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import mfo
+from paper_2106_10279_b200 import workloads as W
+from test_oracle_amplitudes import esw_gg_ttbar
+from test_oracle_quark_channel import closed_form_qq, mdot
+
+MT, AS = 173.0, 0.118
+E, Z, CT, PH = 1000.0, 0.6, 0.3, 1.1
+P1, P2 = np.array([E, 0, 0, E]), np.array([E, 0, 0, -E])
+
+
+def boost(p, q):
+    """p from the rest frame of q to the frame in which q is given"""
+    M = math.sqrt(mdot(q, q))
+    b, g = q[1:] / M, q[0] / M
+    bp = float(np.dot(b, p[1:]))
+    return np.concatenate([[g * p[0] + bp], p[1:] + b * (bp / (g + 1) + p[0])])
+
+
+def decay(q, ct=CT, ph=PH):
+    M = math.sqrt(mdot(q, q))
+    En = M / 2
+    pp = math.sqrt(En * En - MT * MT)
+    st = math.sqrt(1 - ct * ct)
+    k = np.array([En, pp * st * math.cos(ph), pp * st * math.sin(ph), pp * ct])
+    return boost(k, q), boost(np.array([En, -k[1], -k[2], -k[3]]), q)
+
+
+def generic_point(seed=0):
+    rng = np.random.default_rng(seed)
+    k, _ = mfo.rambo([MT, MT, 0.0], 900.0 + 400 * rng.random(), rng.random(12))
+    w = k[:, 0].sum() / 2
+    return np.vstack([[w, 0, 0, w], [w, 0, 0, -w], k])
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_ward_identity_bases_and_precision(kind):
+    for seed in range(6):
+        mom = generic_point(seed)
+        v = mfo.me2_light_line_ttbar_g(kind, mom, MT, AS)
+        assert v > 0
+        # eps -> k makes every diagram ~ (k / 1)^2 ~ 1e5 times larger; the sum cancels to rounding
+        assert abs(mfo.me2_light_line_ttbar_g(kind, mom, MT, AS, subst=1)) < 1e-8 * v
+        for basis in (1, 2, 3):
+            assert mfo.me2_light_line_ttbar_g(kind, mom, MT, AS, basis=basis) == pytest.approx(v, rel=1e-12)
+        assert mfo.me2_light_line_ttbar_g(kind, mom, MT, AS, prec=1) == pytest.approx(v, rel=1e-12)
+
+
+def test_charge_conjugation_and_alpha_s_power():
+    mom = generic_point(3)
+    v = mfo.me2_light_line_ttbar_g(0, mom, MT, AS)
+    assert mfo.me2_light_line_ttbar_g(0, mom[[1, 0, 3, 2, 4]], MT, AS) == pytest.approx(v, rel=1e-12)
+    assert mfo.me2_light_line_ttbar_g(0, mom, MT, 2 * AS) == pytest.approx(8 * v, rel=1e-12)
+
+
+def _collinear(direction, th, az):
+    """the massless momentum (1 - Z) E (1, sin th cos az, sin th sin az, +-cos th)"""
+    return (1 - Z) * E * np.array([1, math.sin(th) * math.cos(az), math.sin(th) * math.sin(az), direction * math.cos(th)])
+
+
+def test_collinear_limit_gluon_along_the_quark():
+    born = closed_form_qq(np.array([Z * P1, P2, *decay(Z * P1 + P2)]), MT, AS)
+    P = 4 / 3 * (1 + Z * Z) / (1 - Z)
+    prev = None
+    for th in (1e-3, 1e-4):
+        k5 = _collinear(+1, th, 0.7)
+        v = mfo.me2_light_line_ttbar_g(0, np.array([P1, P2, *decay(P1 + P2 - k5), k5]), MT, AS)
+        ratio = v / (8 * math.pi * AS / (2 * mdot(P1, k5)) * P / Z * born)
+        assert abs(ratio - 1) < 1.5 * th          # approaches 1 linearly in the angle
+        if prev is not None:
+            assert abs(ratio - 1) < 0.2 * abs(prev - 1)
+        prev = ratio
+
+
+def test_collinear_limit_gluon_splits_into_quark_pair():
+    born = closed_form_qq(np.array([P1, Z * P2, *decay(P1 + Z * P2)]), MT, AS)
+    P = 0.5 * (Z * Z + (1 - Z) ** 2)
+    for th in (1e-3, 1e-4):
+        p5 = _collinear(-1, th, 0.7)
+        v = mfo.me2_light_line_ttbar_g(1, np.array([P1, P2, *decay(P1 + P2 - p5), p5]), MT, AS)
+        ratio = v / (8 * math.pi * AS / (2 * mdot(P2, p5)) * P / Z * born)
+        assert abs(ratio - 1) < 1.5 * th
+
+
+def test_collinear_limit_quark_radiates_into_gluon_gluon_channel():
+    born = esw_gg_ttbar(np.array([Z * P1, P2, *decay(Z * P1 + P2)]), MT, AS)
+    P = 4 / 3 * (1 + (1 - Z) ** 2) / Z
+    th = 1e-4
+    vals = []
+    for ia in range(8):                      # the gluon entering g g -> ttbar is linearly polarised: average the azimuth
+        p5 = _collinear(+1, th, 0.3 + ia * 2 * math.pi / 8)
+        vals.append(mfo.me2_light_line_ttbar_g(1, np.array([P1, P2, *decay(P1 + P2 - p5), p5]), MT, AS))
+    pref = 8 * math.pi * AS / (2 * mdot(P1, _collinear(+1, th, 0.0))) * P / Z * born
+    assert np.mean(vals) / pref == pytest.approx(1.0, abs=5e-4)
+    assert max(vals) / min(vals) > 1.02        # and the azimuthal correlation is really there
