@@ -3,6 +3,7 @@
 // product library (libmadflow_b200.so has no host evaluation path) and is loaded only by tests/.
 #include <cstring>
 #include "../../paper_2106_10279_b200/csrc/mf_event.cuh"
+#include "../../paper_2106_10279_b200/csrc/mf_me_qttg.cuh"
 #include "../../paper_2106_10279_b200/csrc/mf_me_coop.cuh"
 #include <vector>
 
@@ -58,6 +59,13 @@ double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {   // g g 
 double mfh_me2_coop3(const double* mom, double m_top, double alpha_s) {  // g g -> t tbar g
   double gs2 = 4.0 * kPi * alpha_s;
   return coop_host_me2<g3::Prog>(mom, m_top, gs2 * gs2 * gs2 / 256.0);
+}
+
+// quark channels of pp -> ttbar g (component; mf_me_qttg.cuh): mom = p1, p2, p3, p4, p5 as in the oracle's entry point
+double mfh_me2_light_line_ttg(int kind, const double* mom, double m_top, double alpha_s) {
+  const double* prow = kind == 0 ? mom + 4 : mom + 16;
+  const double* pg = kind == 0 ? mom + 16 : mom + 4;
+  return me2_light_line_ttg(kind, mom, prow, mom + 8, mom + 12, pg, m_top, 4.0 * kPi * alpha_s);
 }
 
 void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {

@@ -94,6 +94,8 @@ def shim():
     L.mfh_philox.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32)]
     L.mfh_uniform52.restype = C.c_double
     L.mfh_uniform52.argtypes = [C.c_uint32, C.c_uint32]
+    L.mfh_me2_light_line_ttg.restype = C.c_double
+    L.mfh_me2_light_line_ttg.argtypes = [C.c_int, dp, C.c_double, C.c_double]
     for f in (L.mfh_pdf_2d, L.mfh_pdf_row, L.mfh_pdf_row_weights):
         f.restype = C.c_double
         f.argtypes = [dp, dp, dp, C.c_int, C.c_int, C.c_double, C.c_double]
@@ -137,6 +139,21 @@ def test_shim_pdf_paths(shim, pdf, oracle_procs):
             o = op.pdf_xf_table(t, x, q2)
             i = int(np.clip(np.searchsorted(lnx, np.log(x), side="right") - 1, 0, len(lnx) - 2))
             assert abs(shim.mfh_pdf_row_weights(*args, x, q2) - o) <= 1e-11 * abs(o) + 4e-15 * scale[max(i - 1, 0):i + 3].max()
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_shim_quark_gluon_channel_me(shim, kind):
+    """q qbar -> ttbar g / q g -> ttbar q of the CUDA path's source against the oracle's Feynman-diagram sum"""
+    from oracle import mfo
+    rng = np.random.default_rng(10 + kind)
+    mt = W.C2.m_top
+    for _ in range(60):
+        k, _ = mfo.rambo([mt, mt, 0.0], 400.0 + 3000.0 * rng.random(), rng.random(12))
+        w = k[:, 0].sum() / 2
+        mom = np.ascontiguousarray(np.vstack([[w, 0, 0, w], [w, 0, 0, -w], k]))
+        g = shim.mfh_me2_light_line_ttg(kind, mom.ctypes.data_as(dp), mt, W.C2.alpha_s)
+        o = mfo.me2_light_line_ttbar_g(kind, mom, mt, W.C2.alpha_s)
+        assert abs(g / o - 1) < 1e-10, (g, o)
 
 
 def test_shim_quark_channel_me(shim):
