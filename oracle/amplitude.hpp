@@ -757,19 +757,25 @@ template <class R> inline void light_line_colour_matrix(Cx<R> CC[5][5]) {
   }
 }
 // Averaged |M|^2.  kind 0: q(mom0) qbar(mom1) -> t(mom2) tbar(mom3) g(mom4), average 1/(4 x 9);
-// kind 1: q(mom0) g(mom1) -> t(mom2) tbar(mom3) q(mom4), average 1/(4 x 24).  subst != 0 replaces the gluon's
+// kind 1: q(mom0) g(mom1) -> t(mom2) tbar(mom3) q(mom4), average 1/(4 x 24);
+// kind 2: qbar(mom0) g(mom1) -> t(mom2) tbar(mom3) qbar(mom4), average 1/(4 x 24): the light line runs from the outgoing
+// antiquark (column v(mom4), flow momentum -mom4 into the line) to the incoming one (row vbar(mom0), flow -mom0 out).
+// subst != 0 replaces the gluon's
 // polarisation vector by its momentum (the Ward identity: the result must vanish).
 template <class R>
 inline R me2_light_line_ttbar_g(int kind, const R mom[5][4], R mt, R alpha_s, int basis, int subst) {
   const R g = r_sqrt(R(4) * r_pi<R>() * alpha_s);
   const int sb = basis & 1, pb = (basis >> 1) & 1;
-  Cx<R> CC[5][5];
-  light_line_colour_matrix<R>(CC);
-  R pr[4], kg[4];
-  const R* pg = kind == 0 ? mom[4] : mom[1];       // the gluon's physical momentum
-  const R* prow = kind == 0 ? mom[1] : mom[4];     // the particle behind the light line's row spinor
+  static Cx<R> CC[5][5];          // computed once per real type (the oracle is single-threaded)
+  static bool have_cc = false;
+  if (!have_cc) { light_line_colour_matrix<R>(CC); have_cc = true; }
+  R pr[4], pc[4], kg[4];
+  const R* pg = kind == 0 ? mom[4] : mom[1];                       // the gluon's physical momentum
+  const R* prow = kind == 0 ? mom[1] : kind == 1 ? mom[4] : mom[0]; // the particle behind the light line's row spinor
+  const R* pcol = kind == 2 ? mom[4] : mom[0];                     // ... and behind its column spinor
   for (int m = 0; m < 4; ++m) {
-    pr[m] = kind == 0 ? -prow[m] : prow[m];
+    pr[m] = kind == 1 ? prow[m] : -prow[m];
+    pc[m] = kind == 2 ? -pcol[m] : pcol[m];
     kg[m] = kind == 0 ? pg[m] : -pg[m];
   }
   R total = R(0);
@@ -778,14 +784,14 @@ inline R me2_light_line_ttbar_g(int kind, const R mom[5][4], R mt, R alpha_s, in
       for (int l3 = -1; l3 <= 1; l3 += 2)
         for (int l4 = -1; l4 <= 1; l4 += 2)
           for (int lg = -1; lg <= 1; lg += 2) {
-            const Spinor<R> C = u_spinor(mom[0], R(0), l1, sb);
-            const Spinor<R> Rw = kind == 0 ? bar(v_spinor(prow, R(0), l2, sb)) : bar(u_spinor(prow, R(0), l2, sb));
+            const Spinor<R> C = kind == 2 ? v_spinor(pcol, R(0), l1, sb) : u_spinor(pcol, R(0), l1, sb);
+            const Spinor<R> Rw = kind == 1 ? bar(u_spinor(prow, R(0), l2, sb)) : bar(v_spinor(prow, R(0), l2, sb));
             const Spinor<R> ub3 = bar(u_spinor(mom[2], mt, l3, sb)), v4 = v_spinor(mom[3], mt, l4, sb);
             CVec4<R> E = polarisation(pg, lg, pb);
             if (kind == 0) E = cconj(E);
             if (subst) E = cvec_from_real(pg);
             Cx<R> kin[5];
-            light_line_ttbar_g_diagrams<R>(Rw, pr, C, mom[0], ub3, mom[2], v4, mom[3], E, kg, mt, g, kin);
+            light_line_ttbar_g_diagrams<R>(Rw, pr, C, pc, ub3, mom[2], v4, mom[3], E, kg, mt, g, kin);
             Cx<R> acc;
             for (int d = 0; d < 5; ++d)
               for (int e = 0; e < 5; ++e) acc += conj(kin[d]) * CC[d][e] * kin[e];

@@ -53,6 +53,7 @@ template <class R> struct EventOut {
   R lum_qq, me2_qq;  // process 4: the flavour-summed q qbar luminosity and the q qbar matrix element
   R chan[12];        // process 4: luminosity x |M|^2 of every partonic channel (0 gg; 1+2i q_i from beam 1; 2+2i from beam 2)
   int n_chan;
+  R chq[6];          // process 5: luminosity x |M|^2 of the six flavour-summed quark-channel classes
   int pass;
 };
 
@@ -119,6 +120,7 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   o.lum_qq = R(0);
   o.me2_qq = R(0);
   o.n_chan = 0;
+  for (int c = 0; c < 6; ++c) o.chq[c] = R(0);
   if (!o.pass) return;
   o.lum = R(1);
   R mu2 = R(P.d.mu2), as_factor = R(1);
@@ -166,6 +168,35 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
     o.lum_qq = La + Lb;
     R both = La * Ma + Lb * Mb;
     o.me2_qq = (o.lum_qq != R(0)) ? both / o.lum_qq : Ma;     // the luminosity-weighted mean of the two orientations
+    f = (o.lum * o.me2 + both) / (R(2) * shat) * o.phi * jac_parton * R(P.d.gev2_to_pb);
+  }
+  if (P.d.process == 5) {
+    // quark channels of pp -> ttbar g (R19), flavour summed (the quarks are massless, so the
+    // matrix elements do not depend on the flavour), the light parton of the final state being whatever the channel
+    // makes it (the cuts act on it alike):
+    //   q qbar, qbar q -> ttbar g;   q g, g q -> ttbar q;   qbar g, g qbar -> ttbar qbar
+    R Q1 = R(0), Qb1 = R(0), Q2 = R(0), Qb2 = R(0), D12 = R(0), D21 = R(0);
+    for (size_t i = 0; i + 1 < P.pdfq.size(); i += 2) {
+      R q1 = pdf_xf<R>(P.pdfq[i], o.x1, mu2), qb1 = pdf_xf<R>(P.pdfq[i + 1], o.x1, mu2);
+      R q2 = pdf_xf<R>(P.pdfq[i], o.x2, mu2), qb2 = pdf_xf<R>(P.pdfq[i + 1], o.x2, mu2);
+      Q1 = Q1 + q1; Qb1 = Qb1 + qb1; Q2 = Q2 + q2; Qb2 = Qb2 + qb2;
+      D12 = D12 + q1 * qb2;
+      D21 = D21 + qb1 * q2;
+    }
+    R g1 = pdf_xf<R>(P.pdf, o.x1, mu2), g2 = pdf_xf<R>(P.pdf, o.x2, mu2);
+    R lumc[6] = {D12, D21, Q1 * g2, g1 * Q2, Qb1 * g2, g1 * Qb2};
+    const int kind[6] = {0, 0, 1, 1, 2, 2};
+    R both = R(0);
+    for (int c = 0; c < 6; ++c) {
+      R m5[5][4];
+      for (int i = 0; i < 5; ++i)
+        for (int m = 0; m < 4; ++m) m5[i][m] = cm[i][m];
+      if (c & 1)                                     // the (anti)quark comes from beam 2
+        for (int m = 0; m < 4; ++m) { m5[0][m] = cm[1][m]; m5[1][m] = cm[0][m]; }
+      R M = me2_light_line_ttbar_g<R>(kind[c], m5, R(P.d.m_top), R(P.d.alpha_s), 0, 0) * as_factor;
+      o.chq[c] = lumc[c] / (o.x1 * o.x2) * M;
+      both = both + o.chq[c];
+    }
     f = (o.lum * o.me2 + both) / (R(2) * shat) * o.phi * jac_parton * R(P.d.gev2_to_pb);
   }
   o.w = f * o.jac;
@@ -246,7 +277,7 @@ template <class R>
 int debug_eval(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteration, uint64_t first, uint64_t n_events,
                double* out) {
   const int D = P.D, n = P.nfinal;
-  const int rowlen = 3 * D + 4 * (n + 2) + 9 + (P.d.process == 4 ? 2 : 0);
+  const int rowlen = 3 * D + 4 * (n + 2) + 9 + (P.d.process == 4 ? 2 : P.d.process == 5 ? 6 : 0);
   EventOut<R> o;
   for (uint64_t k = 0; k < n_events; ++k) {
     uint64_t e = first + k;
@@ -271,6 +302,8 @@ int debug_eval(mfo_process& P, const double* grid, uint64_t seed, uint32_t itera
       row[c++] = r_to_double(o.lum_qq);
       row[c++] = r_to_double(o.me2_qq);
     }
+    if (P.d.process == 5)
+      for (int q = 0; q < 6; ++q) row[c++] = r_to_double(o.chq[q]);
   }
   return 0;
 }
@@ -324,10 +357,10 @@ extern "C" {
 
 int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
   if (!d || !out) return -1;
-  if (d->process < 0 || d->process > 4 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
+  if (d->process < 0 || d->process > 5 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
   std::unique_ptr<mfo_process> P(new mfo_process);
   P->d = *d;
-  static const int Dtab[5] = {2, 4, 14, 18, 4}, ntab[5] = {2, 2, 3, 4, 2}, ngtab[5] = {0, 2, 3, 4, 2};
+  static const int Dtab[6] = {2, 4, 14, 18, 4, 14}, ntab[6] = {2, 2, 3, 4, 2, 3}, ngtab[6] = {0, 2, 3, 4, 2, 3};
   P->D = Dtab[d->process];
   P->nfinal = ntab[d->process];
   P->ng = ngtab[d->process];
@@ -338,7 +371,7 @@ int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
     P->pdf.lnx.assign(d->pdf_lnx, d->pdf_lnx + d->pdf_nx);
     P->pdf.lnq2.assign(d->pdf_lnq2, d->pdf_lnq2 + d->pdf_nq);
     P->pdf.xf.assign(d->pdf_xf, d->pdf_xf + (size_t)d->pdf_nx * d->pdf_nq);
-    if (d->process == 4) {
+    if (d->process >= 4) {
       if (d->pdf_nfl < 3 || d->pdf_nfl % 2 == 0) return -1;
       for (int t = 1; t < d->pdf_nfl; ++t) {
         PdfTable T = P->pdf;
@@ -374,7 +407,7 @@ int mfo_record_size(const mfo_process* P, int32_t* b) {
 }
 int mfo_debug_row_len(const mfo_process* P, int32_t* n) {
   if (!P || !n) return -1;
-  *n = 3 * P->D + 4 * (P->nfinal + 2) + 9 + (P->d.process == 4 ? 2 : 0);
+  *n = 3 * P->D + 4 * (P->nfinal + 2) + 9 + (P->d.process == 4 ? 2 : P->d.process == 5 ? 6 : 0);
   return 0;
 }
 
@@ -483,7 +516,7 @@ double mfo_me2_qq(const mfo_process* P, const double* mom, int basis, int prec) 
 }
 double mfo_me2_light_line_ttbar_g(int kind, const double* mom, double mt, double alpha_s, int basis, int subst,
                                   int prec) {
-  if (!mom || kind < 0 || kind > 1) return -1.0;
+  if (!mom || kind < 0 || kind > 2) return -1.0;
   if (prec == 1) {
     long double m[5][4];
     for (int i = 0; i < 5; ++i)

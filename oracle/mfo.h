@@ -13,7 +13,7 @@ typedef struct mfo_process mfo_process;
 
 /* same field order and meaning as mf_process_desc (include/mf.h) */
 typedef struct {
-  int32_t process; /* 0 ee->mumu, 1 gg->tt, 2 gg->ttg, 3 gg->ttgg, 4 pp->tt (gg + q qbar, flavour summed) */
+  int32_t process; /* 0 ee->mumu, 1 gg->tt, 2 gg->ttg, 3 gg->ttgg, 4 pp->tt (gg + q qbar, flavour summed), 5 pp->ttg (gg + q qbar, q g, qbar g) */
   double sqrt_s;
   double alpha_em, alpha_s;
   double m_top;
@@ -53,7 +53,8 @@ int mfo_unweight(mfo_process*, const double* grid, uint64_t seed, uint32_t itera
                  uint64_t n_events, double w_max, void* records, uint64_t capacity, uint64_t* count, double* hist,
                  mfo_iter_result* result, int prec);
 /* per-event rows:  x[D] | (n+2)x(E,px,py,pz) lab | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D]
- * process 4 appends | lum_qq | me2_qq (lum, me2 = the gg channel; w = the sum of both channels) */
+ * process 4 appends | lum_qq | me2_qq (lum, me2 = the gg channel; w = the sum of both channels);
+ * process 5 appends luminosity x |M|^2 of the six quark-channel classes q qbar, qbar q, q g, g q, qbar g, g qbar */
 int mfo_debug_eval(mfo_process*, const double* grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                    uint64_t n_events, double* out, int prec);
 

@@ -266,7 +266,7 @@ class Process:
         ap = pp = None
         if want_amps:
             import math
-            ng = {1: 2, 2: 3, 3: 4, 4: 2}[self.wl.process]
+            ng = {1: 2, 2: 3, 3: 4, 4: 2, 5: 3}[self.wl.process]
             amps = np.zeros(((4 << ng), math.factorial(ng), 2))
             ap = _dp(amps)
         if want_per_hel:

@@ -13,11 +13,12 @@ import math
 import numpy as np
 
 MF_EE_MUMU, MF_GG_TT, MF_GG_TTG, MF_GG_TTGG = 0, 1, 2, 3
+MF_PP_TTG = 5              # gg -> ttbar g + the q qbar, q g and qbar g channels (36 diagrams with four flavours)
 MF_PP_TT = 4               # gg -> ttbar + the q qbar -> ttbar channels of four flavours
 GEV2_TO_PB = 0.3894e9  # BASELINE.json configs[0]: use this literal everywhere
 N_BINS = 50
-N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18, MF_PP_TT: 4}
-N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4, MF_PP_TT: 2}
+N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18, MF_PP_TT: 4, MF_PP_TTG: 14}
+N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4, MF_PP_TT: 2, MF_PP_TTG: 3}
 N_FLAVOURS = 4             # quark flavours of the multi-flavour table: d, u, s, c (3 gg + 4 q qbar = the 7 diagrams of PAPER.md L101)
 VEGAS_ALPHA = 1.5
 
@@ -70,7 +71,9 @@ CONFIGS = [C0, C1, C2, C3, C4]
 # 3 gg + one q qbar diagram for each of 4 flavours), gluon and quark channels in ONE pass over the same points
 C5 = Workload("C5 pp -> ttbar (gg + q qbar)", MF_PP_TT, sqrt_s=13000.0, n_events=2 ** 20, n_iterations=10, n_adapt=5,
               unweight=True)
-EXTRA_CONFIGS = {"C5": C5}
+C6 = Workload("C6 pp -> ttbar j (gg + q qbar, q g, qbar g)", MF_PP_TTG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5,
+              n_events=2 ** 22, n_iterations=10, n_adapt=10)
+EXTRA_CONFIGS = {"C5": C5, "C6": C6}
 
 
 def pdf_table(nx=100, nq=50):
@@ -117,7 +120,7 @@ def pdf_for(process, nx=100, nq=50):
     """the table a process needs: None, the gluon table, or the multi-flavour table"""
     if process == MF_EE_MUMU:
         return None
-    return pdf_table_flavours(nx, nq) if process == MF_PP_TT else pdf_table(nx, nq)
+    return pdf_table_flavours(nx, nq) if process in (MF_PP_TT, MF_PP_TTG) else pdf_table(nx, nq)
 
 
 def uniform_grid(n_dims, n_bins=N_BINS):

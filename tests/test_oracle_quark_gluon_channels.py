@@ -113,3 +113,51 @@ def test_collinear_limit_quark_radiates_into_gluon_gluon_channel():
     pref = 8 * math.pi * AS / (2 * mdot(P1, _collinear(+1, th, 0.0))) * P / Z * born
     assert np.mean(vals) / pref == pytest.approx(1.0, abs=5e-4)
     assert max(vals) / min(vals) > 1.02        # and the azimuthal correlation is really there
+
+
+def test_antiquark_gluon_channel_is_the_charge_conjugate():
+    """kind 2 (qbar g -> ttbar qbar, from its own diagrams: the light line runs backwards) = kind 1 with t <-> tbar"""
+    for seed in range(4):
+        mom = generic_point(20 + seed)
+        v2 = mfo.me2_light_line_ttbar_g(2, mom, MT, AS)
+        assert v2 == pytest.approx(mfo.me2_light_line_ttbar_g(1, mom[[0, 1, 3, 2, 4]], MT, AS), rel=1e-12)
+        assert abs(mfo.me2_light_line_ttbar_g(2, mom, MT, AS, subst=1)) < 1e-8 * v2
+        assert v2 != pytest.approx(mfo.me2_light_line_ttbar_g(1, mom, MT, AS), rel=1e-3)     # and differs from q g
+
+
+def test_process_rows_from_parts(oracle_procs):
+    """process 5 (pp -> ttbar j): the gg columns are process 2's; the six quark-channel terms and the weight are
+    reassembled from single-table PDF lookups and matrix-element calls at the row's (lab-frame) momenta"""
+    P5 = mfo.Process(W.C6, W.pdf_table_flavours())
+    grid = W.uniform_grid(14)
+    rows = P5.debug_eval(grid, 5, 2, 40, 120)
+    rows2 = oracle_procs[2].debug_eval(grid, 5, 2, 40, 120)
+    n2 = rows2.shape[1]
+    assert rows.shape[1] == n2 + 6
+    o = 14 + 20
+    keep = [c for c in range(n2) if c != o + 6]
+    assert np.array_equal(rows[:, keep], rows2[:, keep])
+    mu2 = MT ** 2
+    nf = W.N_FLAVOURS
+    n_pass = 0
+    for r, r2 in zip(rows, rows2):
+        x1, x2, lum, me2, phi, jv, w, passed = r[o:o + 8]
+        if not passed:
+            assert w == 0 and not r[-6:].any()
+            continue
+        n_pass += 1
+        mom = r[14:o].reshape(5, 4)
+        f = lambda t, x: P5.pdf_xf_table(t, x, mu2)
+        Q1, Qb1 = sum(f(1 + 2 * i, x1) for i in range(nf)), sum(f(2 + 2 * i, x1) for i in range(nf))
+        Q2, Qb2 = sum(f(1 + 2 * i, x2) for i in range(nf)), sum(f(2 + 2 * i, x2) for i in range(nf))
+        D12 = sum(f(1 + 2 * i, x1) * f(2 + 2 * i, x2) for i in range(nf))
+        D21 = sum(f(2 + 2 * i, x1) * f(1 + 2 * i, x2) for i in range(nf))
+        g1, g2 = f(0, x1), f(0, x2)
+        swapped = mom[[1, 0, 2, 3, 4]]
+        want = [D12 * mfo.me2_light_line_ttbar_g(0, mom, MT, AS), D21 * mfo.me2_light_line_ttbar_g(0, swapped, MT, AS),
+                Q1 * g2 * mfo.me2_light_line_ttbar_g(1, mom, MT, AS), g1 * Q2 * mfo.me2_light_line_ttbar_g(1, swapped, MT, AS),
+                Qb1 * g2 * mfo.me2_light_line_ttbar_g(2, mom, MT, AS), g1 * Qb2 * mfo.me2_light_line_ttbar_g(2, swapped, MT, AS)]
+        np.testing.assert_allclose(r[-6:], np.array(want) / (x1 * x2), rtol=1e-9)
+        # w(5) / w(2) = (gg + quark terms) / gg
+        assert w / r2[o + 6] == pytest.approx((lum * me2 + r[-6:].sum()) / (lum * me2), rel=1e-11)
+    assert n_pass > 60
