@@ -36,7 +36,10 @@ typedef struct mf_process mf_process; /* opaque; owns its device-side constants 
  * adds to g g -> t tbar, at the same phase-space point and in the same pass, the q qbar -> t tbar channel of every
  * quark flavour of a multi-flavour PDF table, the quark taken from either beam:
  *   w ~ L_gg |M_gg|^2 + sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2) |M_qq|^2                                */
-enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3, MF_PP_TT = 4 };
+enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3, MF_PP_TT = 4, MF_PP_TTG = 5 };
+/* MF_PP_TTG ("pp -> ttbar g (36 diagrams)"; R19): at the phase-space point, cuts and stream of MF_GG_TTG the
+ * weight sums g g -> t tbar g and the flavour-summed q qbar -> t tbar g, q g -> t tbar q, qbar g -> t tbar qbar channels (either
+ * beam assignment); the light final-state parton is a jet whatever its flavour.  Same multi-flavour table as MF_PP_TT. */
 enum { MF_OK = 0, MF_EINVAL = -1, MF_ECUDA = -2, MF_EOVERFLOW = -3, MF_ERANGE = -4, MF_ENOMEM = -5 };
 
 /* Process descriptor (host memory; copied at create).  Same field order as the oracle's mfo_process_desc. */
@@ -54,7 +57,7 @@ typedef struct {
   const double *pdf_lnq2;     /* [pdf_nq] ln Q^2 knots, increasing                                      */
   const double *pdf_xf;       /* [pdf_nx][pdf_nq] x*g(x,Q^2), row-major xf[ix*nq+iq]; MF_PP_TT:         */
                               /* [pdf_nfl][pdf_nx][pdf_nq], table 0 gluon, 1+2i quark i, 2+2i antiquark i */
-  int32_t pdf_nfl;            /* parton tables; read for MF_PP_TT only: 1 + 2 n_f, n_f = 1..5           */
+  int32_t pdf_nfl;            /* parton tables; read for MF_PP_TT / MF_PP_TTG: 1 + 2 n_f, n_f = 1..5    */
 } mf_process_desc;
 #define MF_MAX_BINS 128
 
@@ -72,7 +75,7 @@ int mf_destroy_process(mf_process *p);
 int mf_n_dims(const mf_process *p, int32_t *D);              /* VEGAS dimensions: 2, 4, 14, 18, 4       */
 int mf_n_final(const mf_process *p, int32_t *n);             /* final-state particles: 2, 2, 3, 4, 2    */
 int mf_record_size(const mf_process *p, int32_t *bytes);     /* (n_final+2)*32 + 16 (+8: MF_PP_TT)      */
-int mf_debug_row_len(const mf_process *p, int32_t *n_doubles);/* 3*D + 4*(n_final+2) + 9 (+2: MF_PP_TT)  */
+int mf_debug_row_len(const mf_process *p, int32_t *n_doubles);/* 3*D + 4*(n_final+2) + 9 (+2 / +6: MF_PP_TT / _TTG) */
 const char *mf_last_error(const mf_process *p);              /* static or handle-owned string           */
 /* launch geometry of the fused pass (blocks, threads per block), for reporting */
 int mf_launch_config(const mf_process *p, int32_t *blocks, int32_t *threads);
@@ -122,7 +125,8 @@ int mf_set_observables(mf_process *p, double *d_obs, int32_t n_bins, double pt_m
 
 /* Test/diagnostic: per-event rows of mf_debug_row_len doubles, identical to the oracle's layout:
  * x[D] | (n+2)x(E,px,py,pz) lab, beams first | x1 x2 | lum | me2 | phi | jvegas | w | pass | r | u[D] | bin[D]
- * MF_PP_TT appends | lum_qq | me2_qq  (lum, me2 are then the gg channel's; w is the sum of both channels) */
+ * MF_PP_TT appends | lum_qq | me2_qq  (lum, me2 are then the gg channel's; w is the sum of both channels);
+ * MF_PP_TTG appends luminosity x |M|^2 of its six quark-channel classes: q qbar, qbar q, q g, g q, qbar g, g qbar */
 int mf_debug_eval(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                   uint64_t n_events, double *d_out, void *stream);
 
@@ -135,6 +139,11 @@ int mf_debug_pdf(mf_process *p, const double *d_x, const double *d_q2, uint64_t 
 /* Test/diagnostic: averaged |M|^2 at n sets of CM-frame momenta d_mom[n][n_final+2][4] (beams first) -> d_out[n];
  * MF_PP_TT: d_out[n][2] = (g g -> t tbar, q qbar -> t tbar). */
 int mf_debug_me2(mf_process *p, const double *d_mom, uint64_t n, double *d_out, void *stream);
+
+/* Test/diagnostic: averaged |M|^2 of the quark channels of pp -> ttbar g at n sets of momenta d_mom[n][5][4] (the two
+ * incoming first) -> d_out[n].  kind 0: q qbar -> t tbar g; 1: q g -> t tbar q; 2: qbar g -> t tbar qbar. */
+int mf_debug_me2_quark_gluon(int32_t kind, double m_top, double alpha_s, const double *d_mom, uint64_t n, double *d_out,
+                             void *stream);
 
 /* Measurement helper: runs a dependent-free DFMA chain on every SM for `iters` iterations and returns the
  * achieved FP64 rate in flop/s (2 flop per DFMA) in *h_flops.  Synchronous.  Used by bench.py for the

@@ -28,7 +28,7 @@ c_double_p = C.POINTER(C.c_double)
 EXPORTS = ["mf_create_process", "mf_destroy_process", "mf_n_dims", "mf_n_final", "mf_record_size",
            "mf_debug_row_len", "mf_last_error", "mf_launch_config", "mf_vegas_iterate", "mf_refine_grid",
            "mf_unweight", "mf_set_dynamic_scale", "mf_set_observables", "mf_debug_eval", "mf_debug_philox", "mf_debug_pdf", "mf_debug_me2",
-           "mf_measure_fp64_peak"]
+           "mf_debug_me2_quark_gluon", "mf_measure_fp64_peak"]
 
 
 class MfError(RuntimeError):
@@ -75,6 +75,7 @@ def lib():
         L.mf_debug_philox.argtypes = [u64, u32, u64, u64, u32, vp, vp]
         L.mf_debug_pdf.argtypes = [vp, vp, vp, u64, vp, vp]
         L.mf_debug_me2.argtypes = [vp, vp, u64, vp, vp]
+        L.mf_debug_me2_quark_gluon.argtypes = [C.c_int32, C.c_double, C.c_double, vp, u64, vp, vp]
         L.mf_measure_fp64_peak.argtypes = [C.c_int64, c_double_p, c_double_p]
         _lib = L
     return _lib
@@ -285,6 +286,16 @@ class Process:
         """(momenta[count, n+2, 4], w[count], id[count]) of `count` records"""
         a = self.records_array(records, count)
         return a["mom"], a["w"], a["id"]
+
+
+def debug_me2_quark_gluon(kind, m_top, alpha_s, mom):
+    """|M|^2 of q qbar -> ttbar g (kind 0), q g -> ttbar q (1), qbar g -> ttbar qbar (2) at mom[n][5][4]"""
+    torch = _torch()
+    m = torch.as_tensor(np.ascontiguousarray(mom, dtype=np.float64)).cuda().reshape(-1, 5, 4)
+    out = torch.empty(m.shape[0], dtype=torch.float64, device="cuda")
+    _check(lib().mf_debug_me2_quark_gluon(kind, m_top, alpha_s, m.data_ptr(), m.shape[0], out.data_ptr(), _stream_ptr(None)),
+           None, "mf_debug_me2_quark_gluon")
+    return out.cpu().numpy()
 
 
 def debug_philox(seed, iteration, first_event, n_events, n_blocks):

@@ -48,6 +48,7 @@ const void* pass_fn(int proc, bool unw) {
     case 0: return unw ? pass_fn<0, true>() : pass_fn<0, false>();
     case 1: return unw ? pass_fn<1, true>() : pass_fn<1, false>();
     case 4: return unw ? pass_fn<4, true>() : pass_fn<4, false>();
+    case 5: return unw ? pass_fn<5, true>() : pass_fn<5, false>();
     case 2: return unw ? (const void*)mf::fused_pass_coop_kernel<2, true> : (const void*)mf::fused_pass_coop_kernel<2, false>;
     default: return unw ? (const void*)mf::fused_pass_coop_kernel<3, true> : (const void*)mf::fused_pass_coop_kernel<3, false>;
   }
@@ -120,14 +121,14 @@ extern "C" {
 int mf_create_process(const mf_process_desc* d, mf_process** out) {
   if (out) *out = nullptr;
   if (!d || !out) return MF_EINVAL;
-  if (d->process < 0 || d->process > 4 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
+  if (d->process < 0 || d->process > 5 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
       !(d->gev2_to_pb > 0.0))
     return MF_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MF_ECUDA; }
   mf_process* p = new (std::nothrow) mf_process;
   if (!p) return MF_ENOMEM;
-  static const int Dtab[5] = {2, 4, 14, 18, 4}, nftab[5] = {2, 2, 3, 4, 2};
+  static const int Dtab[6] = {2, 4, 14, 18, 4, 14}, nftab[6] = {2, 2, 3, 4, 2, 3};
   p->process = d->process; p->D = Dtab[d->process]; p->NF = nftab[d->process];
   mf::Params& P = p->P;
   std::memset(&P, 0, sizeof(P));
@@ -147,9 +148,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     }
     for (int i = 1; i < d->pdf_nx; ++i) if (!(d->pdf_lnx[i] > d->pdf_lnx[i - 1])) { delete p; return MF_EINVAL; }
     for (int i = 1; i < d->pdf_nq; ++i) if (!(d->pdf_lnq2[i] > d->pdf_lnq2[i - 1])) { delete p; return MF_EINVAL; }
-    const int ng = d->process == MF_PP_TT ? 2 : d->process + 1;
-    const int nfl = d->process == MF_PP_TT ? d->pdf_nfl : 1;
-    if (d->process == MF_PP_TT && (nfl < 3 || nfl % 2 == 0 || nfl > mf::kMaxPartonTables)) { delete p; return MF_EINVAL; }
+    const bool flavoured = d->process == MF_PP_TT || d->process == MF_PP_TTG;
+    const int ng = d->process == MF_PP_TT ? 2 : d->process == MF_PP_TTG ? 3 : d->process + 1;
+    const int nfl = flavoured ? d->pdf_nfl : 1;
+    if (flavoured && (nfl < 3 || nfl % 2 == 0 || nfl > mf::kMaxPartonTables)) { delete p; return MF_EINVAL; }
     P.pdf_nfl = nfl;
     P.me_norm = std::pow(gs2, ng) / (256.0 * (ng == 4 ? 2.0 : 1.0));
     const int ncut = p->NF - 2;
@@ -228,7 +230,7 @@ int mf_record_size(const mf_process* p, int32_t* b) {
 }
 int mf_debug_row_len(const mf_process* p, int32_t* n) {
   if (!p || !n) return MF_EINVAL;
-  *n = 3 * p->D + 4 * (p->NF + 2) + 9 + (p->process == MF_PP_TT ? 2 : 0);
+  *n = 3 * p->D + 4 * (p->NF + 2) + 9 + (p->process == MF_PP_TT ? 2 : p->process == MF_PP_TTG ? 6 : 0);
   return MF_OK;
 }
 const char* mf_last_error(const mf_process* p) { return p ? p->err : kNullHandle; }
@@ -290,6 +292,7 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
     case 0: mf::debug_eval_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 1: mf::debug_eval_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 4: mf::debug_eval_kernel<4><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    case 5: mf::debug_eval_kernel<5><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 2:
       mf::debug_eval_coop_kernel<2><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                       mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, A, d_out);
@@ -336,6 +339,7 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
     case 0: mf::debug_me2_kernel<0><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 1: mf::debug_me2_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 4: mf::debug_me2_kernel<4><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    case 5: mf::debug_me2_kernel<5><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 2:
       mf::debug_me2_coop_kernel<2><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, d_mom, n, d_out);
@@ -348,6 +352,16 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "debug_me2 launch", e);
   return MF_OK;
+}
+
+int mf_debug_me2_quark_gluon(int32_t kind, double m_top, double alpha_s, const double* d_mom, uint64_t n, double* d_out,
+                             void* stream) {
+  if (kind < 0 || kind > 2 || !(m_top > 0.0) || !(alpha_s > 0.0)) return MF_EINVAL;
+  if (n == 0) return MF_OK;
+  if (!d_mom || !d_out) return MF_EINVAL;
+  mf::debug_me2_quark_gluon_kernel<<<(unsigned)((n + mf::kThreads - 1) / mf::kThreads), mf::kThreads, 0,
+                                     (cudaStream_t)stream>>>(kind, m_top, 4.0 * mf::kPi * alpha_s, d_mom, n, d_out);
+  return cudaGetLastError() == cudaSuccess ? MF_OK : MF_ECUDA;
 }
 
 int mf_measure_fp64_peak(int64_t iters, double* h_flops, double* h_ms) {

@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(32) refine_grid_kernel(double* grid, const dou
 template <int PROC>
 __global__ void __launch_bounds__(kThreads) debug_eval_kernel(const Params P, const PassArgs A, double* out) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
-  const int row_len = 3 * D + 4 * (NF + 2) + 9 + (PROC == 4 ? 2 : 0);
+  const int row_len = 3 * D + 4 * (NF + 2) + 9 + (PROC == 4 ? 2 : PROC == 5 ? 6 : 0);
   uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= A.n_events) return;
   const uint64_t event = A.first_event + idx;
@@ -73,10 +73,12 @@ __global__ void __launch_bounds__(kThreads) debug_eval_kernel(const Params P, co
   double* q = row + D;
   for (int i = 0; i < NF + 2; ++i)
     for (int c = 0; c < 4; ++c) *q++ = mom[i][c];
-  double parts[4] = {0.0, 0.0, 0.0, 0.0}, w = 0.0;
+  double parts[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, w = 0.0;
   if (ev.pass) w = weigh_event<PROC>(P, A, A.pdf_lnx, A.pdf_row, ev, parts);
   const double lum = parts[0], me2 = parts[1];
   if (PROC == 4) { row[row_len - 2] = parts[2]; row[row_len - 1] = parts[3]; }
+  if (PROC == 5)
+    for (int c = 0; c < 6; ++c) row[row_len - 6 + c] = parts[2 + c];
   q[0] = ev.x1; q[1] = ev.x2; q[2] = lum; q[3] = me2; q[4] = ev.phi; q[5] = ev.jac_vegas; q[6] = w;
   q[7] = ev.pass ? 1.0 : 0.0;
   q[8] = accept_draw(A.seed, A.iteration, event);
@@ -100,6 +102,17 @@ __global__ void __launch_bounds__(kThreads) debug_me2_kernel(const Params P, con
   } else {
     out[i] = me2_call<PROC>(P, shat, k);
   }
+}
+
+// quark channels of pp -> ttbar g at caller-supplied momenta mom[n][5][4] (the two incoming first), kinds of include/mf.h
+__global__ void __launch_bounds__(kThreads) debug_me2_quark_gluon_kernel(int kind, double m_top, double g2,
+                                                                         const double* mom, uint64_t n, double* out) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double* m = mom + i * 20;
+  if (kind == 0) out[i] = me2_light_line_ttg(0, m, m + 4, m + 8, m + 12, m + 16, m_top, g2);
+  else if (kind == 1) out[i] = me2_light_line_ttg(1, m, m + 16, m + 8, m + 12, m + 4, m_top, g2);
+  else out[i] = me2_light_line_ttg(1, m, m + 16, m + 12, m + 8, m + 4, m_top, g2);   // charge conjugate of kind 1
 }
 
 __global__ void debug_philox_kernel(uint64_t seed, uint32_t iteration, uint64_t first, uint64_t n, uint32_t n_blocks,

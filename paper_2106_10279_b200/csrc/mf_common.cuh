@@ -33,6 +33,8 @@ template <> struct Traits<2> { static constexpr int D = 14, NF = 3, NG = 3, NGF 
 template <> struct Traits<3> { static constexpr int D = 18, NF = 4, NG = 4, NGF = 2; };
 // 4: gg -> ttbar + q qbar -> ttbar (flavour summed): the kinematics and alpha_s power of process 1
 template <> struct Traits<4> { static constexpr int D = 4, NF = 2, NG = 2, NGF = 0; };
+// 5: gg -> ttbar g + the q qbar, q g, qbar g channels (R19): kinematics and cuts of process 2
+template <> struct Traits<5> { static constexpr int D = 14, NF = 3, NG = 3, NGF = 1; };
 constexpr int kMaxPartonTables = 11;   // gluon + up to 5 quark/antiquark pairs
 
 // Scalars every kernel needs (passed by value in the launch).

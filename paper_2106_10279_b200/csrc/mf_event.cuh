@@ -8,6 +8,7 @@
 #include "mf_me_prims.cuh"
 #include "mf_me_eemumu.cuh"
 #include "mf_me_qqtt.cuh"
+#include "mf_me_qttg.cuh"
 #include "mf_me_ggtt_generated.cuh"
 
 namespace mf {
@@ -141,7 +142,7 @@ MF_HD double matrix_element(const Params& P, double shat, const double k[][4]) {
     rvec p3 = {{k[0][0], k[0][1], k[0][2], k[0][3]}}, p4 = {{k[1][0], k[1][1], k[1][2], k[1][3]}};
     double sum;
     if (PROC == 1 || PROC == 4) sum = me2_ggtt_0g(Pg, eps, ub, vv, p3, p4, P.m_top);
-    else if (PROC == 2) sum = me2_ggtt_1g(Pg, eps, ub, vv, p3, p4, P.m_top);
+    else if (PROC == 2 || PROC == 5) sum = me2_ggtt_1g(Pg, eps, ub, vv, p3, p4, P.m_top);
     else sum = me2_ggtt_2g(Pg, eps, ub, vv, p3, p4, P.m_top);
     return sum * P.me_norm;
   }

@@ -58,6 +58,20 @@ MF_ME_CALL double me2_pp_call(const Params& P, double shat, const double (*k)[4]
   return matrix_element<4>(P, shat, k);
 }
 
+// process 5: |M|^2 of quark-channel class c (0 q qbar, 1 qbar q, 2 q g, 3 g q, 4 qbar g, 5 g qbar; first parton from
+// beam 1) at the CM-frame point; the antiquark-gluon classes by charge conjugation (t <-> tbar) of the quark-gluon ones.
+// Inlined ONCE, inside the caller's rolled loop over c (the arguments are selected at run time).
+MF_D double quark_gluon_me2(const Params& P, double shat, const double (*k)[4], int c) {
+  const double E = 0.5 * sqrt(shat);
+  const double pa[4] = {E, 0.0, 0.0, (c & 1) ? -E : E};     // the beam the (anti)quark comes from
+  const double pb[4] = {E, 0.0, 0.0, (c & 1) ? E : -E};     // the other beam
+  const double* prow = c < 2 ? pb : k[2];
+  const double* pg = c < 2 ? k[2] : pb;
+  const double* p3 = c < 4 ? k[0] : k[1];
+  const double* p4 = c < 4 ? k[1] : k[0];
+  return me2_light_line_ttg(c < 2 ? 0 : 1, pa, prow, p3, p4, pg, P.m_top, 4.0 * kPi * P.alpha_s);
+}
+
 // Luminosity (step a6): F(x1) F(x2) / (x1 x2) with F the interpolant of the collapsed row in shared memory; and
 // the factor that rescales |M|^2 (1 at the fixed scale).  Dynamic scale (R16; mf_set_dynamic_scale):
 // mu_F^2 = mu_R^2 = m_t^2 + pT(top)^2 per event, F by the general 2-D lookup in the table (global memory / L2),
@@ -101,8 +115,9 @@ __device__ __noinline__ void parton_densities_dyn(const Params& P, const PassArg
   }
 }
 // Fixed scale (the hot path): one logarithm and one cell search per beam serve all rows; everything in registers.
+template <int PROC>
 MF_D void parton_densities(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
-                           const Event<4>& ev, double* f1, double* f2, double& as_factor) {
+                           const Event<PROC>& ev, double* f1, double* f2, double& as_factor) {
   as_factor = 1.0;
   const int nt = P.pdf_nfl;
   if (P.dyn_scale) {
@@ -113,7 +128,8 @@ MF_D void parton_densities(const Params& P, const PassArgs& A, const double* s_l
     for (int t = 0; t < kMaxPartonTables; ++t)
       if (t < nt) { f1[t] = g1[t]; f2[t] = g2[t]; }
     const double ratio = 1.0 / (1.0 + P.alpha_s * (23.0 / (12.0 * kPi)) * log(mu2 / P.mu2));
-    as_factor = ratio * ratio;
+#pragma unroll
+    for (int g = 0; g < Traits<PROC>::NG; ++g) as_factor *= ratio;
   } else {
     const HermiteWeights W1 = hermite_weights(s_lnx, P.pdf_nx, ev.x1), W2 = hermite_weights(s_lnx, P.pdf_nx, ev.x2);
 #pragma unroll
@@ -129,7 +145,7 @@ MF_D void parton_densities(const Params& P, const PassArgs& A, const double* s_l
 //   lum_qq = sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2)
 MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
                           const Event<4>& ev, double& as_factor, double& lum_qq, double* f1, double* f2) {
-  parton_densities(P, A, s_lnx, s_row, ev, f1, f2, as_factor);
+  parton_densities<4>(P, A, s_lnx, s_row, ev, f1, f2, as_factor);
   const int nt = P.pdf_nfl;
   const double inv = 1.0 / (ev.x1 * ev.x2);
   double a = 0.0, b = 0.0;
@@ -186,6 +202,35 @@ MF_D double weigh_event(const Params& P, const PassArgs& A, const double* s_lnx,
       *channel = pick;
     }
     return event_weight<PROC>(P, ev, 1.0, fma(lum, me_gg, lum_qq * me_qq));
+  } else if constexpr (PROC == 5) {
+    // pp -> ttbar j (R19): the gg channel plus six flavour-summed quark-channel classes at the same point
+    //   0: q qbar   1: qbar q   2: q g   3: g q   4: qbar g   5: g qbar      (first parton from beam 1)
+    double f1[kMaxPartonTables], f2[kMaxPartonTables];
+    parton_densities<5>(P, A, s_lnx, s_row, ev, f1, f2, asf);
+    const int nt = P.pdf_nfl;
+    double Q1 = 0.0, Qb1 = 0.0, Q2 = 0.0, Qb2 = 0.0, D12 = 0.0, D21 = 0.0;
+#pragma unroll
+    for (int t = 1; t + 1 < kMaxPartonTables; t += 2)
+      if (t + 1 < nt) {
+        Q1 += f1[t]; Qb1 += f1[t + 1]; Q2 += f2[t]; Qb2 += f2[t + 1];
+        D12 = fma(f1[t], f2[t + 1], D12);
+        D21 = fma(f1[t + 1], f2[t], D21);
+      }
+    const double inv = 1.0 / (ev.x1 * ev.x2);
+    const double l0 = D12 * inv, l1 = D21 * inv, l2 = Q1 * f2[0] * inv, l3 = f1[0] * Q2 * inv, l4 = Qb1 * f2[0] * inv,
+                 l5 = f1[0] * Qb2 * inv;
+    const double lum = f1[0] * f2[0] * inv;
+    const double me_gg = me2_call<PROC>(P, ev.shat, ev.k) * asf;
+    double sum = lum * me_gg;
+    if (parts) { parts[0] = lum; parts[1] = me_gg; }
+#pragma unroll 1
+    for (int c = 0; c < 6; ++c) {
+      const double lc = c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : c == 3 ? l3 : c == 4 ? l4 : l5;
+      const double term = lc * (quark_gluon_me2(P, ev.shat, ev.k, c) * asf);
+      if (parts) parts[2 + c] = term;
+      sum += term;
+    }
+    return event_weight<PROC>(P, ev, 1.0, sum);
   } else {
     const double lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
     const double me2 = me2_call<PROC>(P, ev.shat, ev.k) * asf;
@@ -341,7 +386,7 @@ template <int PROC, bool UNW>
 __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel(const Params P, const PassArgs A) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   extern __shared__ double smem[];
-  const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx, nrow = PROC == 4 ? nx * P.pdf_nfl : nx;
+  const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx, nrow = (PROC == 4 || PROC == 5) ? nx * P.pdf_nfl : nx;
   double* s_grid = smem;                    // D*(nb+1)
   double* s_hist = s_grid + D * (nb + 1);   // D*nb
   double* s_lnx = s_hist + D * nb;          // nx

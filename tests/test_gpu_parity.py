@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 
 REL_EVENT = 1e-10
 REL_ITER = 1e-9
-WLS = {0: W.C0, 1: W.C1, 2: W.C2, 3: W.C3, 4: W.C5}
+WLS = {0: W.C0, 1: W.C1, 2: W.C2, 3: W.C3, 4: W.C5, 5: W.C6}
 
 
 def _torch():
@@ -30,11 +30,13 @@ def _cols(wl):
              pas=o + 7, r=o + 8, u=slice(o + 9, o + 9 + D), bin=slice(o + 9 + D, o + 9 + 2 * D))
     if wl.process == W.MF_PP_TT:       # the quark channel's flavour-summed luminosity and matrix element
         c["lum_qq"], c["me2_qq"] = o + 9 + 2 * D, o + 10 + 2 * D
+    if wl.process == W.MF_PP_TTG:      # luminosity x |M|^2 of the six quark-channel classes
+        c["chq"] = slice(o + 9 + 2 * D, o + 15 + 2 * D)
     return c
 
 
 def _near_cut_edge(wl, row, c, tol=1e-9):
-    if wl.process < 2:
+    if wl.n_final < 3:
         return False
     mom = row[c["mom"]].reshape(wl.n_final + 2, 4)
     obs = []
@@ -114,6 +116,14 @@ def _compare_rows(wl, g, o):
             assert abs(lq_g - lq_o) <= REL_EVENT * abs(lq_o) + slack_q, ("lum_qq", k, lq_g, lq_o)
             total = lum_o * o[k, c["me2"]] + lq_o * b
             w_slack = abs(wo / total) * (slack * o[k, c["me2"]] + slack_q * b) if total != 0.0 else 0.0
+        if wl.process == W.MF_PP_TTG:
+            # seven channels: each quark-channel term on its own (1e-10 relative, plus 1e-12 of the event's largest term
+            # for the ones that nearly vanish where a density changes sign), then the sum
+            qg, qo = g[k, c["chq"]], o[k, c["chq"]]
+            floor = 1e-12 * max(np.abs(qo).max(), abs(lum_o * b))
+            assert np.all(np.abs(qg - qo) <= REL_EVENT * np.abs(qo) + floor), ("chq", k, qg, qo)
+            total = lum_o * b + qo.sum()
+            w_slack = abs(wo / total) * (slack * abs(b) + 6 * floor) if total != 0.0 else 0.0
         assert abs(wg - wo) <= REL_EVENT * abs(wo) + w_slack, ("w", k, wg, wo)
     return excluded
 
@@ -130,12 +140,12 @@ def test_philox_words_bit_exact():
 
 
 # ---- a1-a10 per event ------------------------------------------------------------------------------------
-@pytest.mark.parametrize("proc", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("proc", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("grid_kind", ["uniform", "adapted"])
 def test_per_event_rows(proc, grid_kind, gpu_procs, oracle_procs):
     wl = WLS[proc]
     gp, op = gpu_procs[proc], oracle_procs[proc]
-    n = {0: 3000, 1: 3000, 2: 1500, 3: 400, 4: 3000}[proc]   # several blocks of 128 and a ragged tail
+    n = {0: 3000, 1: 3000, 2: 1500, 3: 400, 4: 3000, 5: 1500}[proc]   # several blocks of 128 and a ragged tail
     grid = W.uniform_grid(wl.n_dims) if grid_kind == "uniform" else adapted_grid(op, wl)
     dgrid = _torch().from_numpy(grid).cuda()
     for seed, it, first in [(0, 0, 0), (3, 5, (1 << 33) + 11)]:
@@ -144,7 +154,7 @@ def test_per_event_rows(proc, grid_kind, gpu_procs, oracle_procs):
         excluded = _compare_rows(wl, g, o)
         assert excluded <= 1
         c = _cols(wl)
-        if proc in (2, 3):
+        if proc in (2, 3, 5):
             frac = o[:, c["pas"]].mean()
             assert 0.3 < frac < 1.0   # the cuts bite but most events survive
 
@@ -197,6 +207,25 @@ def test_me2_quark_channel(gpu_procs, oracle_procs):
     np.testing.assert_allclose(g[:, 0], gpu_procs[1].debug_me2(pts), rtol=1e-13)
 
 
+@pytest.mark.parametrize("kind", [0, 1, 2])
+def test_me2_quark_gluon_channels(kind):
+    """q qbar -> ttbar g, q g -> ttbar q, qbar g -> ttbar qbar at RAMBO points (5 diagrams; the oracle sums them with explicit
+    colour, the kernel with the contracted colour matrix; kind 2 is the kernel's charge conjugate of kind 1)"""
+    from oracle import mfo
+    from paper_2106_10279_b200 import api
+    rng = np.random.default_rng(30 + kind)
+    mt, a_s = W.C6.m_top, W.C6.alpha_s
+    pts = []
+    for _ in range(300):
+        k, _ = mfo.rambo([mt, mt, 0.0], 400.0 + 4000.0 * rng.random(), rng.random(12))
+        w = k[:, 0].sum() / 2
+        pts.append(np.vstack([[w, 0, 0, w], [w, 0, 0, -w], k]))
+    pts = np.array(pts)
+    g = api.debug_me2_quark_gluon(kind, mt, a_s, pts)
+    for i in range(300):
+        assert abs(g[i] / mfo.me2_light_line_ttbar_g(kind, pts[i], mt, a_s) - 1) < REL_EVENT
+
+
 # ---- a11/a12: iteration sums -------------------------------------------------------------------------------
 def _iterate_gpu(gp, grid, seed, it, first, n, want_hist=True):
     torch = _torch()
@@ -225,7 +254,7 @@ def _check_sums(n, hg, rg, ho, ro):
         assert np.array_equal(hg == 0, ho == 0)
 
 
-@pytest.mark.parametrize("proc,n", [(0, 200_003), (1, 100_001), (2, 12_011), (3, 1_501), (4, 60_001)])
+@pytest.mark.parametrize("proc,n", [(0, 200_003), (1, 100_001), (2, 12_011), (3, 1_501), (4, 60_001), (5, 8_011)])
 def test_iteration_sums(proc, n, gpu_procs, oracle_procs):
     wl = WLS[proc]
     gp, op = gpu_procs[proc], oracle_procs[proc]
@@ -235,7 +264,7 @@ def test_iteration_sums(proc, n, gpu_procs, oracle_procs):
         _check_sums(n, hg, rg, ho, ro)
 
 
-@pytest.mark.parametrize("proc", [0, 2, 3, 4])
+@pytest.mark.parametrize("proc", [0, 2, 3, 4, 5])
 def test_edge_sizes(proc, gpu_procs, oracle_procs):
     wl = WLS[proc]
     gp, op = gpu_procs[proc], oracle_procs[proc]
@@ -277,7 +306,7 @@ def test_refine_grid(proc, gpu_procs, oracle_procs):
 
 # ---- whole pipelines at reduced N ---------------------------------------------------------------------------
 @pytest.mark.parametrize("proc,n,n_it", [(0, 100_000, 5), (1, 1 << 16, 5), (2, 1 << 13, 3), (3, 1 << 10, 3),
-                                          (4, 1 << 15, 4)])
+                                          (4, 1 << 15, 4), (5, 1 << 12, 3)])
 def test_pipeline_reduced_n(proc, n, n_it, gpu_procs, oracle_procs):
     """Every iteration with each side refining its OWN grid: integrals, errors, histograms, final grid."""
     from paper_2106_10279_b200 import integrate
@@ -310,7 +339,7 @@ def test_c0_closed_form(gpu_procs):
 
 
 # ---- a14: unweighting ---------------------------------------------------------------------------------------
-@pytest.mark.parametrize("proc,n", [(1, 50_001), (2, 9_001), (3, 1_200), (4, 30_001)])
+@pytest.mark.parametrize("proc,n", [(1, 50_001), (2, 9_001), (3, 1_200), (4, 30_001), (5, 6_001)])
 def test_unweight(proc, n, gpu_procs, oracle_procs):
     torch = _torch()
     wl = WLS[proc]
@@ -383,7 +412,7 @@ def test_unweight_expected_acceptance(gpu_procs, oracle_procs):
 
 
 # ---- full-size launches (bench configuration) ------------------------------------------------------------------
-@pytest.mark.parametrize("proc", [1, 2, 3, 4])
+@pytest.mark.parametrize("proc", [1, 2, 3, 4, 5])
 def test_full_size_sampled(proc, gpu_procs, oracle_procs):
     """BASELINE.json sizes in the launch configuration bench.py times: (i) additivity over index ranges,
     (ii) oracle parity on sampled windows of the same stream, (iii) determinism."""
@@ -405,7 +434,7 @@ def test_full_size_sampled(proc, gpu_procs, oracle_procs):
     np.testing.assert_allclose(ha + hb, hg, rtol=1e-9, atol=1e-12 * hg.max())
     # sampled windows against the oracle
     rng = np.random.default_rng(proc)
-    wn = {1: 512, 2: 256, 3: 64, 4: 512}[proc]
+    wn = {1: 512, 2: 256, 3: 64, 4: 512, 5: 256}[proc]
     dgrid = _torch().from_numpy(grid).cuda()
     for first in rng.integers(0, n - wn, 6):
         first = int(first)
@@ -500,7 +529,7 @@ def test_rows_near_pdf_zero_crossings(gpu_procs, oracle_procs):
 
 
 # ---- dynamic scale (R16) -----------------------------------------------------------------
-@pytest.mark.parametrize("proc,n", [(1, 6_001), (2, 2_001), (3, 601), (4, 4_001)])
+@pytest.mark.parametrize("proc,n", [(1, 6_001), (2, 2_001), (3, 601), (4, 4_001), (5, 2_001)])
 def test_dynamic_scale(proc, n, gpu_procs, oracle_procs):
     """mu^2 = m_t^2 + pT(top)^2 per event, 2-D PDF lookup, running alpha_s: per-event rows and iteration sums against
     the oracle in the same mode; switching back restores the fixed-scale results exactly."""
@@ -529,7 +558,7 @@ def test_dynamic_scale(proc, n, gpu_procs, oracle_procs):
 
 
 # ---- observable histograms (Fig. 2) -------------------------------------------------------------------
-@pytest.mark.parametrize("proc,n", [(0, 30_011), (1, 20_001), (2, 4_001), (3, 1_003), (4, 12_001)])
+@pytest.mark.parametrize("proc,n", [(0, 30_011), (1, 20_001), (2, 4_001), (3, 1_003), (4, 12_001), (5, 4_001)])
 def test_observable_histograms(proc, n, gpu_procs, oracle_procs):
     """pT and eta histograms of the first final-state particle, accumulated in the same pass, against the oracle's
     definition evaluated on its own per-event rows; accumulation across calls (also through mf_unweight); detaching."""
