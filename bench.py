@@ -30,7 +30,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "integrand events/sec (fp64) for gg->ttbar gg"      # BASELINE.json metric (C3, C4)
-PROCESS_LABEL = {0: "e+e- -> mu+mu-", 1: "gg->ttbar", 2: "gg->ttbar g", 3: "gg->ttbar gg", 4: "pp->ttbar (gg + q qbar)"}
+PROCESS_LABEL = {0: "e+e- -> mu+mu-", 1: "gg->ttbar", 2: "gg->ttbar g", 3: "gg->ttbar gg", 4: "pp->ttbar (gg + q qbar)", 5: "pp->ttbar j (gg + q qbar, q g, qbar g)"}
 
 
 def metric_for(wl):
@@ -45,8 +45,8 @@ UNIT = "events/s"
 # generator's static matrix-element count; profiles/r1_flops_per_event.md).  For the two thread-per-event kernels the
 # compiler folds the constant beam wavefunctions into the matrix element, so the static count overestimates: there
 # the measured TOTAL per event is used (ME_FLOPS_MEASURED) and OTHER_FLOPS is 0.
-OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0}
-ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0}
+OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0}
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 133900.0}    # 5: per event PASSING the cuts (rate 0.8945)
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
@@ -163,7 +163,7 @@ def run_reference(args, wl):
     from paper_2106_10279_b200 import workloads as W
     op = mfo.Process(wl, W.pdf_for(wl.process))
     grid = W.uniform_grid(wl.n_dims, wl.n_bins)
-    n = {0: 200000, 1: 40000, 2: 4000, 3: 400, 4: 20000}[wl.process]     # ~2 s per step
+    n = {0: 200000, 1: 40000, 2: 4000, 3: 400, 4: 20000, 5: 2000}[wl.process]     # ~2 s per step
     times = []
     for k in range(args.warmup + args.steps):
         t0 = time.perf_counter()

@@ -651,7 +651,7 @@ template <class R> inline void dressed_init(DressedContext<R>& d) {
 
 // ---------------------------------------------------------------------------------------------
 // O10 (quark channels with one gluon, "pp -> ttbar g (36 diagrams)": 16 gg + 5 for each
-// of q qbar -> ttbar g, q g -> ttbar q, ...).  GROUNDWORK: no kernel evaluates these yet.
+// of q qbar -> ttbar g, q g -> ttbar q, ...; R19).
 //
 // One massless quark line, the top line and one external gluon; the five tree diagrams written out from the Feynman
 // rules (quark-gluon vertex i g gamma^mu T^a, fermion propagator i (pslash + m)/(p^2 - m^2), gluon propagator

@@ -61,9 +61,8 @@ int mfo_debug_eval(mfo_process*, const double* grid, uint64_t seed, uint32_t ite
 /* ---- component entry points for the pins --------------------------------------------------- */
 /* averaged |M|^2 of q(mom[0]) qbar(mom[1]) -> t(mom[2]) tbar(mom[3]) (process 4 only) */
 double mfo_me2_qq(const mfo_process*, const double* mom, int basis, int prec);
-/* GROUNDWORK for the multi-leg quark channels (no kernel yet): averaged |M|^2 from the five Feynman diagrams with explicit
- * colour.  kind 0: q(mom0) qbar(mom1) -> t(mom2) tbar(mom3) g(mom4); kind 1: q(mom0) g(mom1) -> t(mom2) tbar(mom3) q(mom4).
- * subst != 0: gluon polarisation -> its momentum (Ward identity: 0). */
+/* Quark channels of pp -> ttbar g (R19): averaged |M|^2 from the five Feynman diagrams with explicit colour.  kind 0: q(mom0) qbar(mom1) -> t(mom2) tbar(mom3) g(mom4); kind 1: q(mom0) g(mom1) -> t(mom2) tbar(mom3) q(mom4);
+ * kind 2: qbar(mom0) g(mom1) -> t(mom2) tbar(mom3) qbar(mom4).  subst != 0: gluon polarisation -> its momentum (Ward identity: 0). */
 double mfo_me2_light_line_ttbar_g(int kind, const double* mom, double mt, double alpha_s, int basis, int subst, int prec);
 /* x f(x, q2) of parton table `table` (0 gluon, 1+2i quark i, 2+2i antiquark i) */
 double mfo_pdf_xf_table(const mfo_process*, int table, double x, double q2, int prec);

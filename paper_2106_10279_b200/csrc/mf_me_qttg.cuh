@@ -1,7 +1,6 @@
 // mf_me_qttg.cuh — |M|^2 of the quark channels of pp -> ttbar g ("36 diagrams" = 16 gg + 5
 // for each of q qbar -> ttbar g, q g -> ttbar q, ...): one massless quark line, the top line and one gluon, five diagrams.
-// COMPONENT ONLY: evaluated by mf_debug_me2_quark_gluon (parity against the oracle); no process sums these channels yet
-// (DESIGN.md "what comes next").
+// Used by the fused pass of MF_PP_TTG (mf_kernels.cuh, R19) and by mf_debug_me2_quark_gluon.
 //
 // Conventions of mf_me_prims.cuh (chiral two-component spinors, z-axis spin states, REAL linear gluon polarisations).
 // The light line is described by its column spinor (incoming quark, momentum pc into the line) and its row spinor with

@@ -1,6 +1,5 @@
 """Pins for the oracle's q qbar -> t tbar g and q g -> t tbar q matrix elements (the quark channels of pp -> ttbar g,
-PAPER.md L101).  GROUNDWORK: no kernel evaluates these yet; the oracle
-is written and pinned first.  CPU only.
+PAPER.md L101; R19) and of the process that sums them with g g -> t tbar g.  CPU only.
 
 The oracle sums the five Feynman diagrams with explicit SU(3) generators and structure constants.  What fixes it:
   * the Ward identity: with the gluon's polarisation vector replaced by its momentum the colour-summed |M|^2 vanishes
