@@ -93,6 +93,9 @@ def format_events(rec, process, m_top, scale, alpha_em, alpha_s, w_max):
 class LheDrain:
     def __init__(self, path, proc, compress=None):
         import torch
+        if proc.wl.process not in PDG and proc.wl.process != 4:
+            raise ValueError("LHE output needs the partons of every event: process %d does not record its partonic channel "
+                             "yet (include/mf.h, MF_PP_TTG)" % proc.wl.process)
         self.torch = torch
         self.path = path
         self.proc = proc
