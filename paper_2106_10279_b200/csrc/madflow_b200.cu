@@ -48,7 +48,7 @@ const void* pass_fn(int proc, bool unw) {
     case 0: return unw ? pass_fn<0, true>() : pass_fn<0, false>();
     case 1: return unw ? pass_fn<1, true>() : pass_fn<1, false>();
     case 4: return unw ? pass_fn<4, true>() : pass_fn<4, false>();
-    case 5: return unw ? pass_fn<5, true>() : pass_fn<5, false>();
+    case 5: return unw ? (const void*)mf::fused_pass_coop_kernel<5, true> : (const void*)mf::fused_pass_coop_kernel<5, false>;
     case 2: return unw ? (const void*)mf::fused_pass_coop_kernel<2, true> : (const void*)mf::fused_pass_coop_kernel<2, false>;
     default: return unw ? (const void*)mf::fused_pass_coop_kernel<3, true> : (const void*)mf::fused_pass_coop_kernel<3, false>;
   }
@@ -62,21 +62,22 @@ cudaError_t coop_setup(mf_process* p, const cudaDeviceProp& prop) {
   const int group = PG::Team == 32 ? 1 : mf::kCoopGroup;      // teams run in lock-step groups
   int n_teams = mf::CoopOf<PROC>::MaxTeams;
   while (n_teams > 0 &&
-         (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
+         (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, P.pdf_nx * P.pdf_nfl, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
     --n_teams;
   n_teams -= n_teams % group;
   if (n_teams < 1) return cudaErrorInvalidConfiguration;
   p->threads = n_teams * PG::Team;
-  p->smem = (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, n_teams).total * 8;
+  p->smem = (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, P.pdf_nx * P.pdf_nfl, n_teams).total * 8;
   cudaError_t e;
   for (int u = 0; u < 2; ++u)
     // the attribute belongs to the kernel, not to the handle: always ask for the device maximum, so that handles with
     // different bin counts (different shared-memory needs) can coexist
     if ((e = cudaFuncSetAttribute(pass_fn(PROC, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)prop.sharedMemPerBlockOptin)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute((const void*)mf::debug_eval_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  if constexpr (PROC == 5) return cudaSuccess;   // its debug entry points are the thread-per-event kernels
+  else if ((e = cudaFuncSetAttribute((const void*)mf::debug_eval_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 mf::coop_debug_smem_bytes<PG>())) != cudaSuccess) return e;
-  return cudaFuncSetAttribute((const void*)mf::debug_me2_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  else return cudaFuncSetAttribute((const void*)mf::debug_me2_coop_kernel<PROC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               mf::coop_debug_smem_bytes<PG>());
 }
 
@@ -185,9 +186,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   int dev = 0;
   cudaGetDevice(&dev);
   if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
-  if (p->process == 2 || p->process == 3) {
+  const bool coop = p->process == 2 || p->process == 3 || p->process == 5;
+  if (coop) {
     // cooperative pass: as many teams per block as the SM's shared memory holds, one block per SM
-    e = p->process == 3 ? coop_setup<3>(p, prop) : coop_setup<2>(p, prop);
+    e = p->process == 3 ? coop_setup<3>(p, prop) : p->process == 5 ? coop_setup<5>(p, prop) : coop_setup<2>(p, prop);
     if (e != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   } else {
     p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + (1 + P.pdf_nfl) * P.pdf_nx + 5 * 32) * sizeof(double);
@@ -204,7 +206,7 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
       (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
-  if ((p->process == 2 || p->process == 3) &&
+  if (coop &&
       (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads *
                                        (p->process == 3 ? mf::g4::Prog::Queue : mf::g3::Prog::Queue) * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;

@@ -159,6 +159,38 @@ MF_D double luminosity_pp(const Params& P, const PassArgs& A, const double* s_ln
   return f1[0] * f2[0] * inv;
 }
 
+// pp -> ttbar j (R19): the gluon-gluon luminosity (returned) and the sum over the six flavour-summed
+// quark-channel classes of luminosity x |M|^2 (x the R16 factor):
+//   0: q qbar   1: qbar q   2: q g   3: g q   4: qbar g   5: g qbar      (first parton from beam 1)
+// terms (optional): the six products, for the debug rows.
+MF_D double pp_ttj_terms(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                         const Event<5>& ev, double& asf, double& quark_sum, double* terms) {
+  double f1[kMaxPartonTables], f2[kMaxPartonTables];
+  parton_densities<5>(P, A, s_lnx, s_row, ev, f1, f2, asf);
+  const int nt = P.pdf_nfl;
+  double Q1 = 0.0, Qb1 = 0.0, Q2 = 0.0, Qb2 = 0.0, D12 = 0.0, D21 = 0.0;
+#pragma unroll
+  for (int t = 1; t + 1 < kMaxPartonTables; t += 2)
+    if (t + 1 < nt) {
+      Q1 += f1[t]; Qb1 += f1[t + 1]; Q2 += f2[t]; Qb2 += f2[t + 1];
+      D12 = fma(f1[t], f2[t + 1], D12);
+      D21 = fma(f1[t + 1], f2[t], D21);
+    }
+  const double inv = 1.0 / (ev.x1 * ev.x2);
+  const double l0 = D12 * inv, l1 = D21 * inv, l2 = Q1 * f2[0] * inv, l3 = f1[0] * Q2 * inv, l4 = Qb1 * f2[0] * inv,
+               l5 = f1[0] * Qb2 * inv;
+  double sum = 0.0;
+#pragma unroll 1
+  for (int c = 0; c < 6; ++c) {
+    const double lc = c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : c == 3 ? l3 : c == 4 ? l4 : l5;
+    const double term = lc * (quark_gluon_me2(P, ev.shat, ev.k, c) * asf);
+    if (terms) terms[c] = term;
+    sum += term;
+  }
+  quark_sum = sum;
+  return f1[0] * f2[0] * inv;
+}
+
 // a6-a10 of one event that passed the cuts (thread-per-event kernels): luminosity, |M|^2, weight.
 // parts (optional): lum, me2 [, lum_qq, me2_qq for process 4] for the debug rows.
 // channel (optional, process 4; R18): the partonic channel this event gets IF it is accepted, drawn in
@@ -203,34 +235,11 @@ MF_D double weigh_event(const Params& P, const PassArgs& A, const double* s_lnx,
     }
     return event_weight<PROC>(P, ev, 1.0, fma(lum, me_gg, lum_qq * me_qq));
   } else if constexpr (PROC == 5) {
-    // pp -> ttbar j (R19): the gg channel plus six flavour-summed quark-channel classes at the same point
-    //   0: q qbar   1: qbar q   2: q g   3: g q   4: qbar g   5: g qbar      (first parton from beam 1)
-    double f1[kMaxPartonTables], f2[kMaxPartonTables];
-    parton_densities<5>(P, A, s_lnx, s_row, ev, f1, f2, asf);
-    const int nt = P.pdf_nfl;
-    double Q1 = 0.0, Qb1 = 0.0, Q2 = 0.0, Qb2 = 0.0, D12 = 0.0, D21 = 0.0;
-#pragma unroll
-    for (int t = 1; t + 1 < kMaxPartonTables; t += 2)
-      if (t + 1 < nt) {
-        Q1 += f1[t]; Qb1 += f1[t + 1]; Q2 += f2[t]; Qb2 += f2[t + 1];
-        D12 = fma(f1[t], f2[t + 1], D12);
-        D21 = fma(f1[t + 1], f2[t], D21);
-      }
-    const double inv = 1.0 / (ev.x1 * ev.x2);
-    const double l0 = D12 * inv, l1 = D21 * inv, l2 = Q1 * f2[0] * inv, l3 = f1[0] * Q2 * inv, l4 = Qb1 * f2[0] * inv,
-                 l5 = f1[0] * Qb2 * inv;
-    const double lum = f1[0] * f2[0] * inv;
+    double quark_sum;
+    const double lum = pp_ttj_terms(P, A, s_lnx, s_row, ev, asf, quark_sum, parts ? parts + 2 : nullptr);
     const double me_gg = me2_call<PROC>(P, ev.shat, ev.k) * asf;
-    double sum = lum * me_gg;
     if (parts) { parts[0] = lum; parts[1] = me_gg; }
-#pragma unroll 1
-    for (int c = 0; c < 6; ++c) {
-      const double lc = c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : c == 3 ? l3 : c == 4 ? l4 : l5;
-      const double term = lc * (quark_gluon_me2(P, ev.shat, ev.k, c) * asf);
-      if (parts) parts[2 + c] = term;
-      sum += term;
-    }
-    return event_weight<PROC>(P, ev, 1.0, sum);
+    return event_weight<PROC>(P, ev, 1.0, fma(lum, me_gg, quark_sum));
   } else {
     const double lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
     const double me2 = me2_call<PROC>(P, ev.shat, ev.k) * asf;

@@ -20,6 +20,9 @@ namespace mf {
 // the cooperative program of a process and its launch shape
 template <int PROC> struct CoopOf { typedef g4::Prog PG; static constexpr int MaxTeams = 6; };   // PROC = 3
 template <> struct CoopOf<2> { typedef g3::Prog PG; static constexpr int MaxTeams = 16; };
+// pp -> ttbar j: the gg -> ttbar g program for the gluon channel; the owner threads evaluate the quark-channel classes
+// (register hungry), hence fewer, fatter threads
+template <> struct CoopOf<5> { typedef g3::Prog PG; static constexpr int MaxTeams = 8; };
 
 // queue entry = the event record of mf_me_coop_tasks.inc (momenta, shat, polarisation vectors, spinors, c0): PG::Queue doubles
 
@@ -27,13 +30,13 @@ template <> struct CoopOf<2> { typedef g3::Prog PG; static constexpr int MaxTeam
 template <class PG>
 struct CoopSmem {
   int grid, hist, lnx, row, red, cnt, res, tab, teams, total;
-  __host__ __device__ CoopSmem(int D, int nb, int nx, int n_teams) {
+  __host__ __device__ CoopSmem(int D, int nb, int nx, int nrow, int n_teams) {   // nrow = nx x parton tables
     auto even = [](int v) { return (v + 1) & ~1; };
     grid = 0;
     hist = grid + even(D * (nb + 1));
     lnx = hist + even(D * nb);
     row = lnx + even(nx);
-    red = row + even(nx);
+    red = row + even(nrow);
     cnt = red + 5 * 32;
     res = cnt + 32;
     tab = res + PG::Warps * n_teams * PG::Team;
@@ -162,9 +165,9 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
   constexpr int G = PG::Team == 32 ? 1 : kCoopGroup;
   extern __shared__ double2 smem2[];
   double* smem = reinterpret_cast<double*>(smem2);
-  const int nb = P.n_bins, nx = P.pdf_nx;
+  const int nb = P.n_bins, nx = P.pdf_nx, nrow = PROC == 5 ? nx * P.pdf_nfl : nx;
   const int n_teams = blockDim.x / PG::Team;
-  const CoopSmem<PG> L(D, nb, nx, n_teams);
+  const CoopSmem<PG> L(D, nb, nx, nrow, n_teams);
   double* s_grid = smem + L.grid;
   double* s_hist = smem + L.hist;
   double* s_lnx = smem + L.lnx;
@@ -178,7 +181,8 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
   coop_load_table<PG>(s_tab);
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < D * nb; i += blockDim.x) s_hist[i] = 0.0;
-  for (int i = threadIdx.x; i < nx; i += blockDim.x) { s_lnx[i] = A.pdf_lnx[i]; s_row[i] = A.pdf_row[i]; }
+  for (int i = threadIdx.x; i < nx; i += blockDim.x) s_lnx[i] = A.pdf_lnx[i];
+  for (int i = threadIdx.x; i < nrow; i += blockDim.x) s_row[i] = A.pdf_row[i];
   __syncthreads();
 
   Accum acc;
@@ -192,11 +196,14 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
     bins.clear();
     Event<PROC> ev;
     ev.pass = false;
-    double lum = 0.0, asf = 1.0;
+    double lum = 0.0, asf = 1.0, quark_sum = 0.0;   // quark_sum: the owner's own channels (pp -> ttbar j), else 0
     if (valid) {
       DebugRow dbg = {nullptr, D, NF};
       generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, bins, dbg);
-      if (ev.pass) lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
+      if (ev.pass) {
+        if constexpr (PROC == 5) lum = pp_ttj_terms(P, A, s_lnx, s_row, ev, asf, quark_sum, nullptr);
+        else lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
+      }
     }
     const bool pass = valid && ev.pass;
     const int obs_bins = (pass && A.obs != nullptr) ? observable_bins<PROC>(A, ev) : 0;
@@ -205,7 +212,8 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
-      w = event_weight<PROC>(P, ev, lum, me2 * asf);
+      if (PROC == 5) w = event_weight<PROC>(P, ev, 1.0, fma(lum, me2 * asf, quark_sum));
+      else w = event_weight<PROC>(P, ev, lum, me2 * asf);
     }
     accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins);
   }
