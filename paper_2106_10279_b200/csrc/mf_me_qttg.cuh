@@ -57,33 +57,39 @@ MF_HD double me2_light_line_ttg(int kind, const double p1[4], const double prow[
   double total = 0.0;
   for (int lam = 0; lam < 2; ++lam) {
     const rvec& e = E[lam];
-    cvec jl[4], jlA[4], jlB[4], jt[4], jtC[4], jtD[4];
+    // the top line's three currents for its four spin states (kept in memory), then the light line's, one spin state
+    // at a time (kept in registers)
+    cvec jt[4], jtC[4], jtD[4];
     for (int a = 0; a < 2; ++a)
       for (int b = 0; b < 2; ++b) {
-        const spin col = u_col(p1, 0.0, a);
-        const spin row = kind == 0 ? bar_of(v_col(prow, 0.0, b)) : ubar_row(prow, 0.0, b);
-        jl[2 * a + b] = bilinear(row, col);
-        jlA[2 * a + b] = bilinear(row, slash_col(a1, slash_col(e, col)));
-        jlB[2 * a + b] = bilinear(slash_row(slash_row(row, e), a2), col);
         const spin ub3 = ubar_row(p3, mt, a), v4 = v_col(p4, mt, b);
         jt[2 * a + b] = bilinear(ub3, v4);
         const spin r1 = slash_row(ub3, e), c1 = slash_col(e, v4);
         jtC[2 * a + b] = bilinear(spin_add_scaled(slash_row(r1, t1), mt, r1), v4);
         jtD[2 * a + b] = bilinear(ub3, spin_add_scaled(slash_col(t2, c1), mt, c1));
       }
+    const double k12e = rdot(k12, e);
+#pragma unroll 1
     for (int i = 0; i < 4; ++i) {
-      const cplx el = cdot_r(jl[i], e), k23l = cdot_r(jl[i], k23);
+      const spin col = u_col(p1, 0.0, i >> 1);
+      const spin row = kind == 0 ? bar_of(v_col(prow, 0.0, i & 1)) : ubar_row(prow, 0.0, i & 1);
+      const cvec jl = bilinear(row, col);
+      const cvec jlA = bilinear(row, slash_col(a1, slash_col(e, col)));
+      const cvec jlB = bilinear(slash_row(slash_row(row, e), a2), col);
+      const cplx el = cdot_r(jl, e), k23l = cdot_r(jl, k23);
+#pragma unroll 1
       for (int j = 0; j < 4; ++j) {
         cplx K[5];
-        K[0] = cdot_c(jlA[i], jt[j]);  K[0].re *= wA; K[0].im *= wA;
-        K[1] = cdot_c(jlB[i], jt[j]);  K[1].re *= wB; K[1].im *= wB;
-        K[2] = cdot_c(jl[i], jtC[j]);  K[2].re *= wC; K[2].im *= wC;
-        K[3] = cdot_c(jl[i], jtD[j]);  K[3].re *= wD; K[3].im *= wD;
-        const cplx lt = cdot_c(jl[i], jt[j]), et = cdot_r(jt[j], e), k31t = cdot_r(jt[j], k31);
-        const double k12e = rdot(k12, e);
+        K[0] = cdot_c(jlA, jt[j]);  K[0].re *= wA; K[0].im *= wA;
+        K[1] = cdot_c(jlB, jt[j]);  K[1].re *= wB; K[1].im *= wB;
+        K[2] = cdot_c(jl, jtC[j]);  K[2].re *= wC; K[2].im *= wC;
+        K[3] = cdot_c(jl, jtD[j]);  K[3].re *= wD; K[3].im *= wD;
+        const cplx lt = cdot_c(jl, jt[j]), et = cdot_r(jt[j], e), k31t = cdot_r(jt[j], k31);
         K[4].re = wE * (lt.re * k12e + (et.re * k23l.re - et.im * k23l.im) + (el.re * k31t.re - el.im * k31t.im));
         K[4].im = wE * (lt.im * k12e + (et.re * k23l.im + et.im * k23l.re) + (el.re * k31t.im + el.im * k31t.re));
+#pragma unroll
         for (int d = 0; d < 5; ++d)
+#pragma unroll
           for (int f = 0; f < 5; ++f) total += S[d][f] * re_conj_mul(K[d], K[f]);
       }
     }
