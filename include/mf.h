@@ -10,7 +10,7 @@
  *
  * in ONE fused CUDA pass, then reduces sum w, sum w^2, max|w|, n_pass and the per-dimension VEGAS
  * histograms of w^2.  Nothing per event touches HBM except the records mf_unweight accepts.
- * DESIGN.md states every reading of the paper (R1..R15) the arithmetic follows.
+ * DESIGN.md states every reading of the paper (R1..R19) the arithmetic follows.
  *
  * Conventions
  *  - All functions return int: MF_OK (0) or a negative error code.  No exceptions, no aborts, no printing.
