@@ -52,8 +52,8 @@ MF_HD double me2_light_line_ttg(int kind, const double p1[4], const double prow[
   const double wE = 1.0 / (sl * st);
   rvec E[2];
   pol_vectors(pg, E[0], E[1]);
-  // 3 S (colour matrix in units of 1/3)
-  const double S[5][5] = {{8, -1, 7, -2, 9}, {-1, 8, -2, 7, -9}, {7, -2, 8, -1, 9}, {-2, 7, -1, 8, -9}, {9, -9, 9, -9, 18}};
+  // colour matrix in units of 1/3 (csrc/gen_qttg_colour.py; the fifth tensor taken as i f^{bca} T^b T^c):
+  //   3 S = {{8, -1, 7, -2, 9}, {-1, 8, -2, 7, -9}, {7, -2, 8, -1, 9}, {-2, 7, -1, 8, -9}, {9, -9, 9, -9, 18}}
   double total = 0.0;
   for (int lam = 0; lam < 2; ++lam) {
     const rvec& e = E[lam];
@@ -87,10 +87,13 @@ MF_HD double me2_light_line_ttg(int kind, const double p1[4], const double prow[
         const cplx lt = cdot_c(jl, jt[j]), et = cdot_r(jt[j], e), k31t = cdot_r(jt[j], k31);
         K[4].re = wE * (lt.re * k12e + (et.re * k23l.re - et.im * k23l.im) + (el.re * k31t.re - el.im * k31t.im));
         K[4].im = wE * (lt.im * k12e + (et.re * k23l.im + et.im * k23l.re) + (el.re * k31t.im + el.im * k31t.re));
-#pragma unroll
-        for (int d = 0; d < 5; ++d)
-#pragma unroll
-          for (int f = 0; f < 5; ++f) total += S[d][f] * re_conj_mul(K[d], K[f]);
+        // K^dagger (3 S) K with u = K0 + K2, v = K1 + K3, d = u - v, r = (K0 - K2) + (K1 - K3):
+        //   6 (|u|^2 + |v|^2) + 1.5 |d|^2 + 18 Re(conj(K4) d) + 18 |K4|^2 + 0.5 |r|^2
+        const cplx u = {K[0].re + K[2].re, K[0].im + K[2].im}, v = {K[1].re + K[3].re, K[1].im + K[3].im};
+        const cplx dd = {u.re - v.re, u.im - v.im};
+        const cplx r = {(K[0].re - K[2].re) + (K[1].re - K[3].re), (K[0].im - K[2].im) + (K[1].im - K[3].im)};
+        total += 6.0 * (re_conj_mul(u, u) + re_conj_mul(v, v)) + 1.5 * re_conj_mul(dd, dd) +
+                 18.0 * (re_conj_mul(K[4], dd) + re_conj_mul(K[4], K[4])) + 0.5 * re_conj_mul(r, r);
       }
     }
   }
