@@ -476,6 +476,7 @@ double mfo_rambo(int n, const double* mass, double w, const double* rho, double*
     for (int c = 0; c < 4; ++c) k[i * 4 + c] = (double)kk[i][c];
   return (double)V;
 }
+double mfo_two_pi_power(int n) { return two_pi_power<double>(n); }
 int mfo_cuts(int ng, const double* gl, double ptmin, double etamax, double drmin, double* obs) {
   double g[4][4];
   for (int i = 0; i < ng; ++i)

@@ -76,6 +76,8 @@ void mfo_parton_fractions(double x0, double x1, double tau_min, double s, double
 double mfo_two_body(double shat, double m, double xc, double xphi, double* mom);
 /* k[n][4]; returns the volume V */
 double mfo_rambo(int n, const double* mass, double w, const double* rho, double* k, int prec);
+/* (2 pi)^(4 - 3 n): dPhi_n = (2 pi)^(4 - 3 n) V (O6 step 6) */
+double mfo_two_pi_power(int n);
 /* returns 1 if the gluons pass; obs[ng][3] = pt, eta, phi */
 int mfo_cuts(int ng, const double* gluons_lab, double ptmin, double etamax, double drmin, double* obs);
 void mfo_boost_z(double y, const double in[4], double out[4]);

@@ -41,6 +41,8 @@ def lib():
         L.mfo_vegas_map.restype = C.c_double
         L.mfo_two_body.restype = C.c_double
         L.mfo_rambo.restype = C.c_double
+        L.mfo_two_pi_power.restype = C.c_double
+        L.mfo_two_pi_power.argtypes = [C.c_int]
         L.mfo_pdf_xf.restype = C.c_double
         L.mfo_me2.restype = C.c_double
         L.mfo_pdf_xf.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int]
@@ -132,6 +134,11 @@ def rambo(masses, w, rho, prec=0):
     k = np.empty((n, 4))
     V = lib().mfo_rambo(n, _dp(masses), w, _dp(rho), _dp(k), prec)
     return k, V
+
+
+def two_pi_power(n):
+    """(2 pi)^(4 - 3 n), the oracle's own function (O6 step 6)"""
+    return lib().mfo_two_pi_power(n)
 
 
 def cuts(gluons_lab, ptmin, etamax, drmin):

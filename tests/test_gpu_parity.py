@@ -96,14 +96,18 @@ def _compare_rows(wl, g, o):
         # |M|^2: 1e-10 relative (BASELINE.json north_star).  Luminosity and weight: the same, plus the rounding of
         # the Hermite interpolation where the interpolant of x g passes through ZERO (near x = 0.87 and 0.97 it changes
         # sign, R8): there F is a difference of terms of the size of the neighbouring knot values, so two
-        # correct evaluation orders differ by a few ulp of THAT size, not of F.  Allowance: 4e-13 x the knot scale.
+        # correct evaluation orders differ by a few ulp of THAT size, not of F.  Allowance: 4e-13 x the knot scale, and
+        # only where the cancellation factor knot scale / |lum| exceeds 250 (elsewhere: zero slack, plain 1e-10).
+        # Refereed in quad precision by tests/test_pdf_zero_referee.py: both the fp64 oracle and the kernel sit within
+        # this allowance of the __float128 value; the fp64 oracle's own error there reaches 4e-11 relative.
         a, b = g[k, c["me2"]], o[k, c["me2"]]
         assert abs(a - b) <= REL_EVENT * abs(b), ("me2", k, a, b)
         lum_g, lum_o = g[k, c["lum"]], o[k, c["lum"]]
         slack = 0.0
         if wl.process:
             x1, x2 = o[k, c["x1"]], o[k, c["x2"]]
-            slack = 4e-13 * _knot_scale(x1) * _knot_scale(x2) / (x1 * x2)
+            kscale = _knot_scale(x1) * _knot_scale(x2) / (x1 * x2)
+            slack = 4e-13 * kscale if kscale > 250.0 * abs(lum_o) else 0.0
         assert abs(lum_g - lum_o) <= REL_EVENT * abs(lum_o) + slack, ("lum", k, lum_g, lum_o)
         wg, wo = g[k, c["w"]], o[k, c["w"]]
         w_slack = abs(wo / lum_o) * slack if lum_o != 0.0 else 0.0
@@ -112,7 +116,8 @@ def _compare_rows(wl, g, o):
             a, b = g[k, c["me2_qq"]], o[k, c["me2_qq"]]
             assert abs(a - b) <= REL_EVENT * abs(b), ("me2_qq", k, a, b)
             lq_g, lq_o = g[k, c["lum_qq"]], o[k, c["lum_qq"]]
-            slack_q = 2 * W.N_FLAVOURS * 4e-13 * _knot_scale(x1, True) * _knot_scale(x2, True) / (x1 * x2)
+            scale_q = 2 * W.N_FLAVOURS * _knot_scale(x1, True) * _knot_scale(x2, True) / (x1 * x2)
+            slack_q = 4e-13 * scale_q if scale_q > 250.0 * abs(lq_o) else 0.0
             assert abs(lq_g - lq_o) <= REL_EVENT * abs(lq_o) + slack_q, ("lum_qq", k, lq_g, lq_o)
             total = lum_o * o[k, c["me2"]] + lq_o * b
             w_slack = abs(wo / total) * (slack * o[k, c["me2"]] + slack_q * b) if total != 0.0 else 0.0

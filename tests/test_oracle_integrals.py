@@ -157,12 +157,13 @@ def test_c1_event_weight_formula_from_parts(oracle_procs):
         assert w == pytest.approx(jv * lum / (2 * shat) * me2 * phi * jac * 0.3894e9, rel=1e-12)
 
 
-@pytest.mark.parametrize("pid", [2, 3])
+@pytest.mark.parametrize("pid", [2, 3, 5])
 def test_multileg_event_rows_are_consistent(oracle_procs, pid):
-    """C2/C3 per-event rows: momentum conservation in the lab frame, cuts recomputed from the lab momenta, failed
-    events carry w = 0, and w reassembles from its factors (the integral itself is unpinned)."""
+    """C2/C3/C6 per-event rows: momentum conservation in the lab frame, cuts recomputed from the lab momenta, failed
+    events carry w = 0, the row's Phi is (2 pi)^(4-3n) times the RAMBO volume at the row's own x (the power typed here:
+    PAPER.md L71-75), and w reassembles from its factors (the integral itself is unpinned, O13)."""
     P = oracle_procs[pid]
-    wl = {2: W.C2, 3: W.C3}[pid]
+    wl = {2: W.C2, 3: W.C3, 5: W.C6}[pid]
     D, n = P.n_dims, P.n_final
     rows = P.debug_eval(W.uniform_grid(D), 0, 0, 0, 400)
     s = 13000.0 ** 2
@@ -175,6 +176,10 @@ def test_multileg_event_rows_are_consistent(oracle_procs, pid):
         x1, x2, lum, me2, phi, jv, w, passed = r[D + nm:D + nm + 8]
         assert np.allclose(mom[0] + mom[1], mom[2:].sum(axis=0), atol=1e-9 * 6500)
         assert x1 * x2 >= tau_min * (1 - 1e-12)
+        # O6: Phi = (2 pi)^(4 - 3n) V with V recomputed by the RAMBO component call at the row's own uniforms
+        _, V = mfo.rambo([173.0, 173.0] + [0.0] * (n - 2), math.sqrt(x1 * x2 * s), x[2:])
+        two_pi_pow = {3: 1.0 / (2 * math.pi) ** 5, 4: 1.0 / (2 * math.pi) ** 8}[n]
+        assert phi == pytest.approx(two_pi_pow * V, rel=1e-12)
         ok, _ = mfo.cuts(mom[4:], wl.ptmin, wl.etamax, wl.drmin)
         assert ok == bool(passed)
         if not passed:
@@ -184,10 +189,44 @@ def test_multileg_event_rows_are_consistent(oracle_procs, pid):
         shat = x1 * x2 * s
         L = math.log(tau_min)
         jac = (-x1 * x2 * L) * (-math.log(x1 * x2))
-        assert w == pytest.approx(jv * lum / (2 * shat) * me2 * phi * jac * 0.3894e9, rel=1e-11)
+        if pid == 5:        # gg term + the six quark-channel classes (lum x |M|^2 each, appended to the row)
+            chq = r[3 * D + nm + 9:3 * D + nm + 15]
+            assert w == pytest.approx(jv * (lum * me2 + chq.sum()) / (2 * shat) * phi * jac * 0.3894e9, rel=1e-11)
+        else:
+            assert w == pytest.approx(jv * lum / (2 * shat) * me2 * phi * jac * 0.3894e9, rel=1e-11)
         # Lorentz invariance ties the CM-frame |M|^2 to the lab-frame momenta stored in the row
         assert P.me2(mom) == pytest.approx(me2, rel=1e-9)
     assert 0.3 * len(rows) < npass < len(rows)
+
+
+def test_c1_through_rambo_two_body_gives_the_c1_cross_section(oracle_procs, c1_quadrature):
+    """SURVEY.md O6 chain pin: gg -> ttbar pushed through RAMBO(n = 2) instead of the analytic two-body
+    map must give the C1 cross section (2648.76 pb by quadrature).  Assembled from the oracle's component calls only:
+    VEGAS map on the (tau, y) dimensions of an oracle-adapted C1 grid, O4 parton fractions, RAMBO with two massive
+    particles, the oracle's two_pi_power(2), its gg -> ttbar |M|^2 at the RAMBO momenta, its PDF.  This ties the
+    normalisation of the RAMBO branch (V, the 2 pi power, the weight assembly of O12) to a number fixed without RAMBO."""
+    from conftest import adapted_grid
+    P = oracle_procs[1]
+    grid2 = adapted_grid(P, W.C1)[:2]
+    s = 13000.0 ** 2
+    m = 173.0
+    tau_min = 4 * m * m / s
+    rng = np.random.default_rng(2024)
+    n = 1 << 16
+    w = np.empty(n)
+    tp2 = mfo.two_pi_power(2)
+    for k in range(n):
+        u = rng.random(10)                      # (tau, y) + 4 per RAMBO particle
+        x, jv, _ = mfo.vegas_map(grid2, u[:2])
+        pk = mfo.parton_fractions(x[0], x[1], tau_min, s)
+        rt = math.sqrt(pk["shat"])
+        kf, V = mfo.rambo([m, m], rt, u[2:])
+        mom = np.vstack([[rt / 2, 0, 0, rt / 2], [rt / 2, 0, 0, -rt / 2], kf])
+        lum = P.pdf_xf(pk["x1"], m * m) * P.pdf_xf(pk["x2"], m * m) / (pk["x1"] * pk["x2"])
+        w[k] = jv * lum / (2 * pk["shat"]) * P.me2(mom) * (tp2 * V) * pk["jac"] * 0.3894e9
+    I, err = w.mean(), w.std(ddof=1) / math.sqrt(n)
+    assert err / I < 4e-3
+    assert abs(I - c1_quadrature) < 4 * err
 
 
 # ---- R16: dynamic scale (SURVEY.md 8(f4)) ----------------------------------------------------------------------------

@@ -136,6 +136,31 @@ def test_rambo_three_body_massive_volume_vs_quadrature():
     assert err / vol < 2e-3
 
 
+@pytest.mark.parametrize("n", [2, 3, 4, 5])
+def test_two_pi_power_gives_the_textbook_massless_phase_space(n):
+    """O6 step 6: dPhi_n = (2 pi)^(4-3n) V.  The oracle's OWN two_pi_power(n) times the volume its own
+    RAMBO returns for massless particles must be the textbook integrated n-body phase space
+    Phi_n(s) = s^(n-2) / (2 (4 pi)^(2n-3) (n-1)! (n-2)!): 1/(8 pi), s/(256 pi^3), s^2/(24576 pi^5), s^3/(4718592 pi^7).
+    An exponent that is off by one is a factor 2 pi."""
+    w = 730.0
+    s = w * w
+    literal = {2: 1 / (8 * math.pi), 3: s / (256 * math.pi ** 3), 4: s * s / (24576 * math.pi ** 5),
+               5: s ** 3 / (4718592 * math.pi ** 7)}[n]
+    general = s ** (n - 2) / (2 * (4 * math.pi) ** (2 * n - 3) * math.factorial(n - 1) * math.factorial(n - 2))
+    assert literal == pytest.approx(general, rel=1e-14)
+    rng = np.random.default_rng(40 + n)
+    for _ in range(5):
+        _, V0 = mfo.rambo([0.0] * n, w, rng.random(4 * n))
+        assert mfo.two_pi_power(n) * V0 == pytest.approx(literal, rel=1e-13)
+    # and the massive two-body case against the two-body routine's own weight: beta / (8 pi)
+    m = 173.0
+    _, V = mfo.rambo([m, m], w, rng.random(8))
+    beta = math.sqrt(1 - 4 * m * m / s)
+    assert mfo.two_pi_power(2) * V == pytest.approx(beta / (8 * math.pi), rel=1e-13)
+    _, phi2 = mfo.two_body(s, m, 0.3, 0.6)
+    assert mfo.two_pi_power(2) * V == pytest.approx(phi2, rel=1e-13)
+
+
 def test_rambo_isotropy_and_energy_spectrum():
     """Massless n=2: directions must be isotropic (c = 2 rho1 - 1 is the cosine, phi = 2 pi rho2)."""
     k, _ = mfo.rambo([0, 0], 2.0, [0.75, 0.25, 0.3, 0.6, 0.1, 0.9, 0.5, 0.5])
