@@ -109,20 +109,35 @@ class ClockSampler:
 
 
 # ---- the oracle arm (cpu_baseline and --impl reference) ---------------------------------------------------------
-def oracle_sample(wl, seconds=15.0, n_first=64):
-    """Times the oracle, as it stands, single-threaded, on events [0, n) of iteration 0 of `wl` on the uniform
-    grid; n is sized from a short probe so the sample takes about `seconds`."""
-    from oracle import mfo
-    from paper_2106_10279_b200 import workloads as W
-    op = mfo.Process(wl, W.pdf_for(wl.process))
-    grid = W.uniform_grid(wl.n_dims, wl.n_bins)
-    t0 = time.perf_counter()
-    op.vegas_iterate(grid, wl.seed, 0, 0, n_first)
-    per = (time.perf_counter() - t0) / n_first
-    n = int(max(n_first, min(wl.n_events, seconds / per)))
-    t0 = time.perf_counter()
-    op.vegas_iterate(grid, wl.seed, 0, 0, n)
-    dt = time.perf_counter() - t0
+_SAMPLE_WORKER = r"""
+import sys, time
+sys.path.insert(0, sys.argv[1])
+from oracle import mfo
+from paper_2106_10279_b200 import workloads as W
+wl = {"C0": W.C0, "C1": W.C1, "C2": W.C2, "C3": W.C3, "C4": W.C4, **W.EXTRA_CONFIGS}[sys.argv[2]]
+seconds, n_first = float(sys.argv[3]), int(sys.argv[4])
+op = mfo.Process(wl, W.pdf_for(wl.process))
+grid = W.uniform_grid(wl.n_dims, wl.n_bins)
+t0 = time.perf_counter()
+op.vegas_iterate(grid, wl.seed, 0, 0, n_first)
+per = (time.perf_counter() - t0) / n_first
+n = int(max(n_first, min(wl.n_events, seconds / per)))
+t0 = time.perf_counter()
+op.vegas_iterate(grid, wl.seed, 0, 0, n)
+print(n, time.perf_counter() - t0)
+"""
+
+
+def oracle_sample(config, seconds=15.0, n_first=64):
+    """Times the oracle, as it stands, single-threaded, on events [0, n) of iteration 0 of the config on the uniform
+    grid; n is sized from a short probe so the sample takes about `seconds`.  Runs in a SUBPROCESS: the process that
+    times the CUDA path never loads oracle/libmfo.so."""
+    r = subprocess.run([sys.executable, "-c", _SAMPLE_WORKER, ROOT, config, str(seconds), str(n_first)],
+                       stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("oracle sample failed: " + r.stderr[-2000:])
+    n, dt = r.stdout.split()
+    n, dt = int(n), float(dt)
     return n / dt, n, dt
 
 
@@ -205,6 +220,15 @@ def main():
         return run_reference(args, wl)
     if args.warmup < 3:
         args.warmup = 3
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` on its own: start N ranks (one per GPU) under torch.distributed.run
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
 
     import numpy as np
     import torch
@@ -217,6 +241,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but %d rank(s) were launched (WORLD_SIZE)" % (args.gpus, world))
+    if local_rank >= torch.cuda.device_count():
+        raise SystemExit("bench.py: rank %d has no GPU (%d visible)" % (local_rank, torch.cuda.device_count()))
     torch.cuda.set_device(local_rank)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
@@ -367,7 +395,7 @@ def main():
                      "nominal_peak": NOMINAL_FP64 / 1e12, "frac_of_nominal": achieved / (NOMINAL_FP64 / 1e12)},
     }
     if world == 1 and not args.no_cpu_baseline:
-        v, ns, dt = oracle_sample(wl)
+        v, ns, dt = oracle_sample(args.config)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                "sample": "events [0,%d) of iteration 0 of %s on the uniform grid, %.1f s, 1 thread of %d"
                                          % (ns, wl.name, dt, os.cpu_count())}

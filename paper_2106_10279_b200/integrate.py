@@ -98,8 +98,14 @@ def run_config(proc, wl=None, capacity=0, stream=None, alpha=W.VEGAS_ALPHA, grid
     the ranks; weak=True: wl.n_events PER rank) and the per-iteration sums are combined with
     combine_across_ranks before the (replicated, identical) grid refinement; records stay rank-local.
     `drain` (lhe.LheDrain): the records of every unweighting iteration are handed to it right after the call (the
-    record buffer is then reused by the next iteration; out.n_records counts all drained events)."""
+    record buffer is then reused by the next iteration; out.n_records counts all drained events).
+    `stream` (torch.cuda.Stream or None): every kernel, helper op and host read of the run is issued on it (the body
+    runs with it as torch's current stream, so the small device->host reads of the w_max policy are ordered after the
+    passes they depend on)."""
     import torch
+    if stream is not None and stream != torch.cuda.current_stream():
+        with torch.cuda.stream(stream):
+            return run_config(proc, wl, capacity, None, alpha, grid, hists, rank, world, weak, drain)
     wl = proc.wl if wl is None else wl
     if world > 1:
         n_total = wl.n_events * world if weak else wl.n_events

@@ -42,6 +42,15 @@ def gpu_procs(pdf):
         p.close()
 
 
+@pytest.fixture(scope="session")
+def oracle_pool():
+    """The oracle as one single-threaded process per host core on disjoint index ranges (tests/oracle_pool.py)."""
+    from oracle_pool import OraclePool
+    pool = OraclePool()
+    yield pool
+    pool.close()
+
+
 _ADAPTED = {}
 
 
