@@ -439,9 +439,12 @@ def emit_s4(L):
     flops = 0
     w("// S4: thread (pols, hb, k) forms the real (k = 0) or imaginary (k = 1) parts of its %d colour-ordered amplitudes" % len(perms))
     w("// and contracts them with the colour matrix: returns sum_{s,s'} x_s Cnum_{ss'} x_s' (the caller divides by kCoopCden).")
-    w("MF_HD double coop_s4(const double* V, const double* S, const double* Z, int pols, int hb, int k) {")
-    for g in LABELS:
-        w("  const int ps%d = (pols >> %d) & 1;" % (g, g))
+    w("// Team thread tid: warp = hb, lane = ps2 | ps3 << 1 | k << 2 | ps0 << 3 | ps1 << 4 (the output-fragment layout of")
+    w("// the DMMA blocks of the first pair of gluon pairs; the other two pairs' results are moved to it by lane shuffles).")
+    w("// EVERY lane of the warp must call it (mma.sync / shfl.sync).")
+    w("MF_HD double coop_s4_tid(const double* V, const double* S, const double* Z, int tid) {")
+    w("  const int hb = tid >> 5, lane = tid & 31;")
+    w("  const int ps2 = lane & 1, ps3 = (lane >> 1) & 1, k = (lane >> 2) & 1, ps0 = (lane >> 3) & 1, ps1 = (lane >> 4) & 1;")
     for a, b in itertools.combinations(LABELS, 2):
         w("  const int %s = ps%d | (ps%d << 1);" % (pair_name(a, b), a, b))
     for m in LABELS:
@@ -452,7 +455,45 @@ def emit_s4(L):
     def word_expr(order):
         return " | ".join("ps%d" % g if i == 0 else "(ps%d << %d)" % (g, i) for i, g in enumerate(order))
     w("  double " + ", ".join("A%d%d%d%d" % p for p in perms) + ";")
-    # term 1: Ytilde(ab) . Xhat(cd); k selects the real or the imaginary part of the product
+    # term 1: Ytilde(ab) . Xhat(cd), the real (k = 0) or imaginary (k = 1) part of the product.
+    # Device: per pair of gluon pairs {ab | cd} two complex 8 x 8 x 4 products as DMMA.884 blocks (real 16 x 8 x 8):
+    #   block N: rows Ytilde(ab / ba; pa, pb; part k), columns Xhat(cd / dc; pc, pd)        -> A[(ab)(cd)]
+    #   block T: rows Xhat(ab / ba; pa, pb; part k),  columns Ytilde(cd / dc; pc, pd)       -> A[(cd)(ab)] (transposed, so
+    #            that both blocks leave the helicity (pa, pb, pc, pd) and the part k in the same lane)
+    # fragment lane = t | g << 2 with g = (k, pa, pb), t = (pc, pd); see coop_s4_block.
+    pairs3 = [((0, 1), (2, 3)), ((0, 2), (1, 3)), ((0, 3), (1, 2))]
+    w("#if defined(__CUDA_ARCH__)")
+    w("  {")
+    w("    double c[2][2];")
+    for pi_, ((a, b), (c, d)) in enumerate(pairs3):
+        # lane layout of this pair: bit 0 = ps_c, bit 1 = ps_d, bit 2 = k, bit 3 = ps_a, bit 4 = ps_b
+        names_n = [["A%d%d%d%d" % (x + u) for u in ((c, d), (d, c))] for x in ((a, b), (b, a))]
+        names_t = [["A%d%d%d%d" % (u + x) for u in ((c, d), (d, c))] for x in ((a, b), (b, a))]
+        if pi_ == 0:
+            tgt_n, tgt_t = names_n, names_t
+        else:
+            w("    // lane of this pair's layout that holds this thread's helicity")
+            w("    const int src%d = ps%d | (ps%d << 1) | (k << 2) | (ps%d << 3) | (ps%d << 4);" % (pi_, c, d, a, b))
+        w("    coop_s4_block<%d, %d, %d, %d, %d, %d>(S, lane, 0, hb * %d, c);    // Ytilde(%d%d) x Xhat(%d%d)" %
+          (L.bases["Yt"], L.bases["X2"], PAIR_INDEX[(a, b)], PAIR_INDEX[(b, a)], PAIR_INDEX[(c, d)], PAIR_INDEX[(d, c)], 4 * SPIN_ROW, a, b, c, d))
+        for mt in range(2):
+            for j in range(2):
+                if pi_ == 0:
+                    w("    %s = c[%d][%d];" % (names_n[mt][j], mt, j))
+                else:
+                    w("    %s = __shfl_sync(0xFFFFFFFFu, c[%d][%d], src%d);" % (names_n[mt][j], mt, j, pi_))
+        w("    coop_s4_block<%d, %d, %d, %d, %d, %d>(S, lane, hb * %d, 0, c);    // Xhat(%d%d) x Ytilde(%d%d), transposed" %
+          (L.bases["X2"], L.bases["Yt"], PAIR_INDEX[(a, b)], PAIR_INDEX[(b, a)], PAIR_INDEX[(c, d)], PAIR_INDEX[(d, c)], 4 * SPIN_ROW, a, b, c, d))
+        for mt in range(2):
+            for j in range(2):
+                if pi_ == 0:
+                    w("    %s = c[%d][%d];" % (names_t[mt][j], mt, j))
+                else:
+                    w("    %s = __shfl_sync(0xFFFFFFFFu, c[%d][%d], src%d);" % (names_t[mt][j], mt, j, pi_))
+        flops += 8 * 16
+    w("  }")
+    w("#else   // host emulation (tests/host_shim): the same products thread by thread")
+    flops_dev = flops
     for a, b in itertools.combinations(LABELS, 2):
         c, d = [g for g in LABELS if g not in (a, b)]
         w("  {")
@@ -463,8 +504,8 @@ def emit_s4(L):
         for (x, y) in ((a, b), (b, a)):
             for (u, v) in ((c, d), (d, c)):
                 w("    A%d%d%d%d = sdot_part(yt%d%d, x%d%d);" % (x, y, u, v, x, y, u, v))
-                flops += 15
         w("  }")
+    w("#endif")
 
     def add(perm, z, sign):
         nonlocal flops
@@ -627,7 +668,7 @@ def main():
            "// A FRAGMENT: included by mf_me_coop.cuh inside namespace mf::g4 (no include guard, no namespace of its own).",
            "",
            "// scratch layout (doubles): VEC 4*kCoopNV | SPIN 8*kCoopNS | Z 2*kCoopZPlane | SCAL kCoopNX (each region 16-byte aligned)",
-           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopZRow = %d, kCoopNX = %d, kCoopJ2Stride = %d;" % (L.n("V"), L.n("S"), Z_PLANE, Z_ROW, L.n("X"), J2_STRIDE),
+           "constexpr int kCoopNV = %d, kCoopNS = %d, kCoopZPlane = %d, kCoopZRow = %d, kCoopNX = %d, kCoopJ2Stride = %d, kCoopSpinRow = %d;" % (L.n("V"), L.n("S"), Z_PLANE, Z_ROW, L.n("X"), J2_STRIDE, SPIN_ROW),
            "constexpr int kCoopScratchDoubles = 4 * kCoopNV + 8 * kCoopNS + 2 * kCoopZPlane + kCoopNX;",
            "constexpr double kCoopCden = %.1f;" % Cden,
            "// item indices the hand-written stage S0 needs"]
@@ -718,6 +759,36 @@ MF_HD double sdot_part(const spin& r, const spin& c) {
   for (int m = 1; m < 4; ++m) { acc = fma(r.re[m], c.re[m], acc); acc = fma(r.im[m], c.im[m], acc); }
   return acc;
 }
+#if defined(__CUDA_ARCH__)
+// D = A B + C on the FP64 tensor path (DMMA.884): A 8 x 4 (lane holds A[lane >> 2][lane & 3]), B 4 x 8 (B[lane & 3][lane >> 2]),
+// C / D 8 x 8 (lane holds rows lane >> 2, columns 2 (lane & 3) and 2 (lane & 3) + 1).  Full FP64 rate on B200 (37.0 TFLOP/s
+// measured, profiles/r2_dmma_probe.md) with one instruction per 256 FMAs and the operands read once per fragment.
+__device__ __forceinline__ void coop_dmma(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+// One block of the S4 spinor contraction: rows = the two spinor items (ROWBASE + rowoff + pp kSpinRow + PR0 / PR1) for the
+// polarisations pp = (pa, pb) and the part k of the lane's g = lane >> 2 = (k, pa, pb); columns = the items (COLBASE + coloff
+// + pp' kSpinRow + PC0 / PC1), column n = j + 2 pp'.  The inner index runs over (component c, re / im): K = 8 = two DMMA
+// steps s, c = 2 s + (t & 1), part r = t >> 1, with t = lane & 3:
+//   row element  = r ^ k ? im : re of the row spinor, negated for (k = 0, r = 1)     [Re: yr xr - yi xi;  Im: yi xr + yr xi]
+//   column element = r ? im : re of the column spinor.
+// Result c[m][j]: row item m, column item j, for the helicity (pa, pb) of g and (pc, pd) = t.
+template <int ROWBASE, int COLBASE, int PR0, int PR1, int PC0, int PC1>
+__device__ __forceinline__ void coop_s4_block(const double* S, int lane, int rowoff, int coloff, double (&c)[2][2]) {
+  const int t = lane & 3, kb = (lane >> 2) & 1, pp = lane >> 3, r = t >> 1;
+  const int plane = (t & 1) * kCoopNS;
+  const int row0 = 2 * (plane + ROWBASE + rowoff + pp * kCoopSpinRow) + (r ^ kb);
+  const int col = 2 * (plane + COLBASE + coloff + pp * kCoopSpinRow + (kb ? PC1 : PC0)) + r;
+  const int neg = r & (kb ^ 1);
+  c[0][0] = c[0][1] = c[1][0] = c[1][1] = 0.0;
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    const double b = S[col + 4 * s * kCoopNS];
+    coop_dmma(c[0][0], c[0][1], mf_flip(S[row0 + 2 * PR0 + 4 * s * kCoopNS], neg), b);
+    coop_dmma(c[1][0], c[1][1], mf_flip(S[row0 + 2 * PR1 + 4 * s * kCoopNS], neg), b);
+  }
+}
+#endif
 '''
 
 

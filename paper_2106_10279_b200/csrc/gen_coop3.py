@@ -207,6 +207,10 @@ def emit_s4(L):
     w("  return (acc0 + acc1) + (acc2 + acc3);")
     flops += 3
     w("}")
+    w("// team thread tid = pols | hb << kCoopPolBits | k << (kCoopPolBits + 1)")
+    w("MF_HD double coop_s4_tid(const double* V, const double* S, const double* Z, int tid) {")
+    w("  return coop_s4(V, S, Z, tid & %d, (tid >> %d) & 1, (tid >> %d) & 1);" % ((1 << N) - 1, N, N + 1))
+    w("}")
     return "\n".join(o), Cden, flops
 
 

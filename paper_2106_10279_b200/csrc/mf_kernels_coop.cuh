@@ -62,10 +62,17 @@ __device__ __forceinline__ void coop_load_table(uint4* s_tab) {
 }
 
 // Teams are tied into groups of G that run the matrix-element program in lock-step (one named barrier per group:
-// 1 + group; barrier 0 is __syncthreads).  G = 1 = every team on its own: least barrier wait, one instruction
-// stream per team (measured best on B200 within noise of G = 2).  One-warp teams need only __syncwarp.
+// 1 + group; barrier 0 is __syncthreads).  G = 1 = every team on its own: least barrier wait, but one instruction
+// stream per team: the straight-line round programs are executed once per event, so the instruction cache holds
+// nothing for a warp unless another warp runs the same code at the same time (ncu: 11 % of the stall samples were
+// "no instruction" with G = 1).  Measured on B200, 2^22 events of g g -> t tbar g g (profiles/r2_c3.md): G = 1
+// 38.7 ms, G = 2 38.0 ms, G = 3 35.5 ms, G = 6 37.0 ms, G = 3 with the groups interleaved over the teams 36.0 ms.
+// One-warp teams need only __syncwarp.
 #ifndef MF_COOP_GROUP
-#define MF_COOP_GROUP 1
+#define MF_COOP_GROUP 3
+#endif
+#ifndef MF_COOP_INTERLEAVE
+#define MF_COOP_INTERLEAVE 0
 #endif
 constexpr int kCoopGroup = MF_COOP_GROUP;
 template <int THREADS>
@@ -80,7 +87,11 @@ template <class PG, int G>
 __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const uint4* tab, double* s_res,
                                                const double* queue, int total, double mt) {
   const int team = threadIdx.x / PG::Team, tid = threadIdx.x % PG::Team, warp = tid >> 5, lane = tid & 31;
-  const int group = team / G;
+#if MF_COOP_INTERLEAVE
+  const int n_groups = n_teams / G, group = team % n_groups, member = team / n_groups;   // groups {g, g + n_groups, ...}
+#else
+  const int group = team / G, member = team - group * G;
+#endif
   double* tm = teams + team * PG::TeamDoubles;
   double* in = tm + PG::OffIn;
   auto sync = [group]() { coop_group_sync<PG::Team * G>(group); };
@@ -95,11 +106,11 @@ __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const
     const int j = tid + i * PG::Team;
     dst[i] = j < PG::Queue ? PG::qdest(j) : -1;
     nxt[i] = 0.0;
-    if (team < total && dst[i] >= 0) nxt[i] = queue[j * qcap + team];
+    if (group * G + member < total && dst[i] >= 0) nxt[i] = queue[j * qcap + group * G + member];
   }
 #pragma unroll 1
   for (int r0 = group * G; r0 < total; r0 += n_teams) {
-    const int r = r0 + (team - group * G);
+    const int r = r0 + member;
     const bool active = r < total;
 #pragma unroll
     for (int i = 0; i < QPT; ++i)
