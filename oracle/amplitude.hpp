@@ -354,10 +354,69 @@ template <class R> inline Mat3<R> su3_generator(int a) {  // T^a = lambda^a / 2,
   }
   return t;
 }
+// M(a) = T^{a_0} T^{a_1} .. T^{a_{n-1}} for all 8^n colour assignments a (code = sum_i a_i 8^i)
+template <class R> inline std::vector<Mat3<R>> colour_product_table(int n) {
+  Mat3<R> T[8];
+  for (int a = 0; a < 8; ++a) T[a] = su3_generator<R>(a);
+  int ncol = 1;
+  for (int i = 0; i < n; ++i) ncol *= 8;
+  std::vector<Mat3<R>> M(ncol);
+  for (int code = 0; code < ncol; ++code) {
+    int a[6] = {0, 0, 0, 0, 0, 0}, cc = code;
+    for (int i = 0; i < n; ++i) { a[i] = cc % 8; cc /= 8; }
+    Mat3<R> prod = T[a[0]];
+    for (int i = 1; i < n; ++i) prod = mat3_mul(prod, T[a[i]]);
+    M[code] = prod;
+  }
+  return M;
+}
+// sum_a Tr( M(a o sigma) M(a o tau)^dagger ), (a o sigma)_i = a_{sigma(i)}: the DEFINITION of C_{sigma tau}, with the matrix
+// products looked up in the table (M_sigma(a) = T^{a_sigma(0)} .. T^{a_sigma(n-1)} = M(a o sigma))
+template <class R> inline R colour_sum_with_table(int n, const std::vector<Mat3<R>>& M, const int* sigma, const int* tau) {
+  int ncol = (int)M.size();
+  R total = R(0);
+  for (int code = 0; code < ncol; ++code) {
+    int a[6], cc = code;
+    for (int i = 0; i < n; ++i) { a[i] = cc % 8; cc /= 8; }
+    int cs = 0, ct = 0, pw = 1;
+    for (int i = 0; i < n; ++i) { cs += a[sigma[i]] * pw; ct += a[tau[i]] * pw; pw *= 8; }
+    const Mat3<R>&A = M[cs], &B = M[ct];
+    Cx<R> tr;
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) tr += A.m[i][j] * conj(B.m[i][j]);
+    total = total + tr.re;
+  }
+  return total;
+}
+template <class R> inline R colour_matrix_entry(int n, const int* sigma, const int* tau) {
+  std::vector<Mat3<R>> M = colour_product_table<R>(n);
+  return colour_sum_with_table<R>(n, M, sigma, tau);
+}
 template <class R> inline std::vector<R> colour_matrix(int n) {
   auto perms = permutations(n);
   int np = (int)perms.size();
   std::vector<R> C(np * np, R(0));
+  if (n >= 5) {
+    // 120 x 120 entries over 8^5 colour assignments: the sum over all colour assignments is invariant under relabelling
+    // the summation indices, a -> a o sigma^-1, hence C_{sigma tau} = C_{id, sigma^-1 o tau}: one row from the definition
+    // (colour_sum_with_table), the others by lookup.  tests/ pins this against the definition entry by entry (n <= 4: all
+    // entries against the plain loop below; n = 5: sampled entries against colour_matrix_entry).
+    std::vector<Mat3<R>> M = colour_product_table<R>(n);
+    std::map<std::vector<int>, int> index;
+    for (int s = 0; s < np; ++s) index[perms[s]] = s;
+    std::vector<R> row(np);
+    for (int t = 0; t < np; ++t) row[t] = colour_sum_with_table<R>(n, M, perms[0].data(), perms[t].data());
+    for (int s = 0; s < np; ++s) {
+      std::vector<int> inv(n);
+      for (int i = 0; i < n; ++i) inv[perms[s][i]] = i;
+      for (int t = 0; t < np; ++t) {
+        std::vector<int> rho(n);
+        for (int i = 0; i < n; ++i) rho[i] = inv[perms[t][i]];
+        C[s * np + t] = row[index[rho]];
+      }
+    }
+    return C;
+  }
   Mat3<R> T[8];
   for (int a = 0; a < 8; ++a) T[a] = su3_generator<R>(a);
   int ncol = 1;

@@ -48,7 +48,7 @@ template <class R> struct EventOut {
   double u[24];
   int bin[24];
   R x[24];
-  R mom[6][4];  // lab frame, beams first
+  R mom[7][4];  // lab frame, beams first
   R x1, x2, lum, me2, phi, jac, w;
   R lum_qq, me2_qq;  // process 4: the flavour-summed q qbar luminosity and the q qbar matrix element
   R chan[12];        // process 4: luminosity x |M|^2 of every partonic channel (0 gg; 1+2i q_i from beam 1; 2+2i from beam 2)
@@ -75,7 +75,7 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   uniforms_for_event(seed, iteration, event, D, o.u);           // O1, O2
   o.jac = vegas_map<R>(grid, D, nb, o.u, o.x, o.bin);           // O3
   const R s = R(P.d.sqrt_s) * R(P.d.sqrt_s);
-  R cm[6][4];
+  R cm[7][4];
   R y = R(0), shat = s, jac_parton = R(1);
   o.x1 = R(1);
   o.x2 = R(1);
@@ -94,7 +94,7 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
         for (int m = 0; m < 4; ++m) cm[i][m] = m4[i][m];
     } else {
       R w = r_sqrt(shat);
-      R mass[4] = {R(P.d.m_top), R(P.d.m_top), R(0), R(0)};
+      R mass[5] = {R(P.d.m_top), R(P.d.m_top), R(0), R(0), R(0)};
       R kf[8][4];
       R V = rambo<R>(n, mass, w, o.x + 2, kf);                  // O6
       o.phi = two_pi_power<R>(n) * V;
@@ -238,7 +238,7 @@ int iterate(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteratio
         uint64_t slot = (*count)++;
         if (records && slot < capacity) {
           char* rec = records + slot * (uint64_t)recsize;
-          double buf[6 * 4 + 1];
+          double buf[7 * 4 + 1];
           for (int i = 0; i < P.nfinal + 2; ++i)
             for (int m = 0; m < 4; ++m) buf[i * 4 + m] = r_to_double(o.mom[i][m]);
           buf[(P.nfinal + 2) * 4] = w;
@@ -315,7 +315,7 @@ template <class R> void load_momenta(const mfo_process& P, const double* mom, R 
 
 template <class R>
 double me2_entry(mfo_process& P, const double* mom, int basis, int subst, double* amps, double* per_hel) {
-  R m[6][4];
+  R m[7][4];
   load_momenta<R>(P, mom, m);
   std::vector<R> a, ph(16);
   if (amps && P.ng) {
@@ -357,10 +357,10 @@ extern "C" {
 
 int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
   if (!d || !out) return -1;
-  if (d->process < 0 || d->process > 5 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
+  if (d->process < 0 || d->process > 6 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
   std::unique_ptr<mfo_process> P(new mfo_process);
   P->d = *d;
-  static const int Dtab[6] = {2, 4, 14, 18, 4, 14}, ntab[6] = {2, 2, 3, 4, 2, 3}, ngtab[6] = {0, 2, 3, 4, 2, 3};
+  static const int Dtab[7] = {2, 4, 14, 18, 4, 14, 22}, ntab[7] = {2, 2, 3, 4, 2, 3, 5}, ngtab[7] = {0, 2, 3, 4, 2, 3, 5};
   P->D = Dtab[d->process];
   P->nfinal = ntab[d->process];
   P->ng = ngtab[d->process];
@@ -371,7 +371,7 @@ int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
     P->pdf.lnx.assign(d->pdf_lnx, d->pdf_lnx + d->pdf_nx);
     P->pdf.lnq2.assign(d->pdf_lnq2, d->pdf_lnq2 + d->pdf_nq);
     P->pdf.xf.assign(d->pdf_xf, d->pdf_xf + (size_t)d->pdf_nx * d->pdf_nq);
-    if (d->process >= 4) {
+    if (d->process == 4 || d->process == 5) {
       if (d->pdf_nfl < 3 || d->pdf_nfl % 2 == 0) return -1;
       for (int t = 1; t < d->pdf_nfl; ++t) {
         PdfTable T = P->pdf;
@@ -529,6 +529,12 @@ double mfo_me2_light_line_ttbar_g(int kind, const double* mom, double mt, double
     for (int c = 0; c < 4; ++c) m[i][c] = mom[4 * i + c];
   return me2_light_line_ttbar_g<double>(kind, m, mt, alpha_s, basis, subst);
 }
+double mfo_colour_matrix_entry(int n, const int32_t* sigma, const int32_t* tau) {
+  if (n < 1 || n > 5) return 0.0;
+  int s[5], t[5];
+  for (int i = 0; i < n; ++i) { s[i] = sigma[i]; t[i] = tau[i]; }
+  return colour_matrix_entry<double>(n, s, t);
+}
 int mfo_colour_matrix(int n, double* out) {
   if (n < 1 || n > 5) return -1;
   std::vector<double> C = colour_matrix<double>(n);
@@ -548,7 +554,7 @@ int mfo_dressed_amplitude(const mfo_process* Pc, const double* mom, const int32_
   static DressedContext<R> d;
   static bool init = false;
   if (!init) { dressed_init(d); init = true; }
-  R m[6][4];
+  R m[7][4];
   load_momenta<R>(P, mom, m);
   load_helicities(d, P, m, hel);
   for (int g = 0; g < P.ng; ++g) d.col[g] = col[g];
@@ -563,7 +569,7 @@ int mfo_ordered_amplitude_coloured(const mfo_process* Pc, const double* mom, con
   if (!P.ng) return -1;
   typedef long double R;
   DressedContext<R> d;  // only its AmpContext is used
-  R m[6][4];
+  R m[7][4];
   load_momenta<R>(P, mom, m);
   load_helicities(d, P, m, hel);
   auto perms = permutations(P.ng);
@@ -592,7 +598,7 @@ static void export_counts(uint64_t out[6]) {
 int mfo_count_ops_me2(const mfo_process* Pc, const double* mom, uint64_t out[6]) {
   mfo_process& P = *const_cast<mfo_process*>(Pc);
   colour_of<Counted>(P);
-  Counted m[6][4];
+  Counted m[7][4];
   load_momenta<Counted>(P, mom, m);
   op_counts() = OpCounts();
   matrix_element<Counted>(P, m, 0, -1, nullptr, nullptr);

@@ -13,7 +13,7 @@ typedef struct mfo_process mfo_process;
 
 /* same field order and meaning as mf_process_desc (include/mf.h) */
 typedef struct {
-  int32_t process; /* 0 ee->mumu, 1 gg->tt, 2 gg->ttg, 3 gg->ttgg, 4 pp->tt (gg + q qbar, flavour summed), 5 pp->ttg (gg + q qbar, q g, qbar g) */
+  int32_t process; /* 0 ee->mumu, 1 gg->tt, 2 gg->ttg, 3 gg->ttgg, 4 pp->tt (gg + q qbar, flavour summed), 5 pp->ttg (gg + q qbar, q g, qbar g), 6 gg->ttggg */
   double sqrt_s;
   double alpha_em, alpha_s;
   double m_top;
@@ -84,6 +84,8 @@ void mfo_boost_z(double y, const double in[4], double out[4]);
 double mfo_pdf_xf(const mfo_process*, double x, double q2, int prec);
 /* n! x n! doubles, permutations in lexicographic order */
 int mfo_colour_matrix(int n, double* out);
+/* one entry straight from the definition: sum over all 8^n colour assignments of Tr(T^{a_sigma(0)} .. T^{a_sigma(n-1)} (T^{a_tau(0)} .. )^dagger) */
+double mfo_colour_matrix_entry(int n, const int32_t* sigma, const int32_t* tau);
 /* averaged |M|^2 for the process' particle content at the given momenta [(n+2)][4] (beams first).
  * basis bit0: spinor basis, bit1: polarisation basis; subst_gluon: -1 or the gluon whose polarisation
  * is replaced by its momentum; amps (may be NULL): [n_hel][n_perm][2] ordered amplitudes;

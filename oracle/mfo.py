@@ -69,6 +69,8 @@ def lib():
         L.mfo_count_ops_me2.argtypes = [C.c_void_p, c_double_p, c_u64_p]
         L.mfo_count_ops_event.argtypes = [C.c_void_p, c_double_p, C.c_uint64, C.c_uint32, C.c_uint64, c_u64_p]
         L.mfo_colour_matrix.argtypes = [C.c_int, c_double_p]
+        L.mfo_colour_matrix_entry.restype = C.c_double
+        L.mfo_colour_matrix_entry.argtypes = [C.c_int, c_i32_p, c_i32_p]
         L.mfo_set_dynamic_scale.argtypes = [C.c_void_p, C.c_int32]
         L.mfo_me2_light_line_ttbar_g.restype = C.c_double
         L.mfo_me2_light_line_ttbar_g.argtypes = [C.c_int, c_double_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int]
@@ -168,6 +170,13 @@ def colour_matrix(n):
     rc = lib().mfo_colour_matrix(n, _dp(out))
     assert rc == 0
     return out
+
+
+def colour_matrix_entry(n, sigma, tau):
+    """C_{sigma tau} straight from its definition (sum over all 8^n colour assignments)"""
+    s = np.ascontiguousarray(sigma, dtype=np.int32)
+    t = np.ascontiguousarray(tau, dtype=np.int32)
+    return lib().mfo_colour_matrix_entry(n, s.ctypes.data_as(c_i32_p), t.ctypes.data_as(c_i32_p))
 
 
 def spinor(p, m, lam, basis=0, kind=0):
@@ -273,7 +282,7 @@ class Process:
         ap = pp = None
         if want_amps:
             import math
-            ng = {1: 2, 2: 3, 3: 4, 4: 2, 5: 3}[self.wl.process]
+            ng = {1: 2, 2: 3, 3: 4, 4: 2, 5: 3, 6: 5}[self.wl.process]
             amps = np.zeros(((4 << ng), math.factorial(ng), 2))
             ap = _dp(amps)
         if want_per_hel:

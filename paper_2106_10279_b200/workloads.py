@@ -14,11 +14,12 @@ import numpy as np
 
 MF_EE_MUMU, MF_GG_TT, MF_GG_TTG, MF_GG_TTGG = 0, 1, 2, 3
 MF_PP_TTG = 5              # gg -> ttbar g + the q qbar, q g and qbar g channels (36 diagrams with four flavours)
+MF_GG_TTGGG = 6            # gg -> ttbar ggg: the paper's heaviest process
 MF_PP_TT = 4               # gg -> ttbar + the q qbar -> ttbar channels of four flavours
 GEV2_TO_PB = 0.3894e9  # BASELINE.json configs[0]: use this literal everywhere
 N_BINS = 50
-N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18, MF_PP_TT: 4, MF_PP_TTG: 14}
-N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4, MF_PP_TT: 2, MF_PP_TTG: 3}
+N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18, MF_PP_TT: 4, MF_PP_TTG: 14, MF_GG_TTGGG: 22}
+N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4, MF_PP_TT: 2, MF_PP_TTG: 3, MF_GG_TTGGG: 5}
 N_FLAVOURS = 4             # quark flavours of the multi-flavour table: d, u, s, c (3 gg + 4 q qbar = the 7 diagrams of PAPER.md L101)
 VEGAS_ALPHA = 1.5
 
@@ -73,7 +74,11 @@ C5 = Workload("C5 pp -> ttbar (gg + q qbar)", MF_PP_TT, sqrt_s=13000.0, n_events
               unweight=True)
 C6 = Workload("C6 pp -> ttbar j (gg + q qbar, q g, qbar g)", MF_PP_TTG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5,
               n_events=2 ** 22, n_iterations=10, n_adapt=10)
-EXTRA_CONFIGS = {"C5": C5, "C6": C6}
+# gg -> ttbar ggg (1240 diagrams, 128 helicity states, 120 x 120 colour matrix; RAMBO n = 5, 22-dim VEGAS),
+# cuts as for gg -> ttbar gg on all three gluons; the paper ran its heaviest process at <= 1M events
+C7 = Workload("C7 gg -> ttbar ggg", MF_GG_TTGGG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5, drmin=0.4, n_events=2 ** 18,
+              n_iterations=10, n_adapt=10)
+EXTRA_CONFIGS = {"C5": C5, "C6": C6, "C7": C7}
 
 
 def pdf_table(nx=100, nq=50):

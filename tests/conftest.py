@@ -26,6 +26,7 @@ def oracle_procs(pdf):
     procs = {wl.process: mfo.Process(wl, pdf) for wl in (W.C0, W.C1, W.C2, W.C3)}
     procs[W.MF_PP_TT] = mfo.Process(W.C5, W.pdf_table_flavours())
     procs[W.MF_PP_TTG] = mfo.Process(W.C6, W.pdf_table_flavours())
+    procs[W.MF_GG_TTGGG] = mfo.Process(W.C7, pdf)
     return procs
 
 
@@ -58,7 +59,7 @@ def adapted_grid(oracle_proc, wl, n_iter=3):
     """A non-uniform VEGAS grid made by the ORACLE alone (a few small adapting iterations); cached."""
     from paper_2106_10279_b200 import workloads as W
     if wl.process not in _ADAPTED:
-        n_events = {0: 20000, 1: 8192, 2: 4096, 3: 1024, 4: 8192, 5: 4096}[wl.process]
+        n_events = {0: 20000, 1: 8192, 2: 4096, 3: 1024, 4: 8192, 5: 4096, 6: 96}[wl.process]
         grid = W.uniform_grid(wl.n_dims, wl.n_bins)
         for k in range(n_iter):
             hist, _ = oracle_proc.vegas_iterate(grid, 12345, k, 0, n_events)

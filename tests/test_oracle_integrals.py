@@ -157,15 +157,15 @@ def test_c1_event_weight_formula_from_parts(oracle_procs):
         assert w == pytest.approx(jv * lum / (2 * shat) * me2 * phi * jac * 0.3894e9, rel=1e-12)
 
 
-@pytest.mark.parametrize("pid", [2, 3, 5])
+@pytest.mark.parametrize("pid", [2, 3, 5, 6])
 def test_multileg_event_rows_are_consistent(oracle_procs, pid):
     """C2/C3/C6 per-event rows: momentum conservation in the lab frame, cuts recomputed from the lab momenta, failed
     events carry w = 0, the row's Phi is (2 pi)^(4-3n) times the RAMBO volume at the row's own x (the power typed here:
     PAPER.md L71-75), and w reassembles from its factors (the integral itself is unpinned, O13)."""
     P = oracle_procs[pid]
-    wl = {2: W.C2, 3: W.C3, 5: W.C6}[pid]
+    wl = {2: W.C2, 3: W.C3, 5: W.C6, 6: W.C7}[pid]
     D, n = P.n_dims, P.n_final
-    rows = P.debug_eval(W.uniform_grid(D), 0, 0, 0, 400)
+    rows = P.debug_eval(W.uniform_grid(D), 0, 0, 0, 400 if pid != 6 else 30)      # 6: 80 ms per event
     s = 13000.0 ** 2
     tau_min = (346.0 + 30.0 * (n - 2)) ** 2 / s
     nm = 4 * (n + 2)
@@ -178,7 +178,7 @@ def test_multileg_event_rows_are_consistent(oracle_procs, pid):
         assert x1 * x2 >= tau_min * (1 - 1e-12)
         # O6: Phi = (2 pi)^(4 - 3n) V with V recomputed by the RAMBO component call at the row's own uniforms
         _, V = mfo.rambo([173.0, 173.0] + [0.0] * (n - 2), math.sqrt(x1 * x2 * s), x[2:])
-        two_pi_pow = {3: 1.0 / (2 * math.pi) ** 5, 4: 1.0 / (2 * math.pi) ** 8}[n]
+        two_pi_pow = {3: 1.0 / (2 * math.pi) ** 5, 4: 1.0 / (2 * math.pi) ** 8, 5: 1.0 / (2 * math.pi) ** 11}[n]
         assert phi == pytest.approx(two_pi_pow * V, rel=1e-12)
         ok, _ = mfo.cuts(mom[4:], wl.ptmin, wl.etamax, wl.drmin)
         assert ok == bool(passed)
