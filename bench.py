@@ -30,7 +30,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "integrand events/sec (fp64) for gg->ttbar gg"      # BASELINE.json metric (C3, C4)
-PROCESS_LABEL = {0: "e+e- -> mu+mu-", 1: "gg->ttbar", 2: "gg->ttbar g", 3: "gg->ttbar gg", 4: "pp->ttbar (gg + q qbar)", 5: "pp->ttbar j (gg + q qbar, q g, qbar g)"}
+PROCESS_LABEL = {0: "e+e- -> mu+mu-", 1: "gg->ttbar", 2: "gg->ttbar g", 3: "gg->ttbar gg", 4: "pp->ttbar (gg + q qbar)", 5: "pp->ttbar j (gg + q qbar, q g, qbar g)", 6: "gg->ttbar ggg"}
 
 
 def metric_for(wl):
@@ -45,7 +45,7 @@ UNIT = "events/s"
 # generator's static matrix-element count; profiles/r1_flops_per_event.md).  For the two thread-per-event kernels the
 # compiler folds the constant beam wavefunctions into the matrix element, so the static count overestimates: there
 # the measured TOTAL per event is used (ME_FLOPS_MEASURED) and OTHER_FLOPS is 0.
-OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0}
+OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 6500.0}    # 6: estimate (C3's + one more RAMBO particle)
 ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 115100.0}    # 5: per event PASSING the cuts (rate 0.8945)
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
@@ -59,7 +59,8 @@ def me_flops(process):
         return ME_FLOPS_MEASURED[process]
     csrc = os.path.join(ROOT, "paper_2106_10279_b200", "csrc")
     if process >= 2:    # the cooperative programs (csrc/gen_coop.py, gen_coop3.py) are what the fused pass runs
-        name = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g")}[process]
+        name = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g"),
+                6: ("mf_me_ttggg_tables_generated.cuh", "kFlopsMe2Cta_3g")}[process]
         txt = open(os.path.join(csrc, name[0])).read()
         return float(re.search(name[1] + r" = ([0-9.]+);", txt).group(1))
     txt = open(os.path.join(csrc, "mf_me_ggtt_generated.cuh")).read()
@@ -178,7 +179,7 @@ def run_reference(args, wl):
     from paper_2106_10279_b200 import workloads as W
     op = mfo.Process(wl, W.pdf_for(wl.process))
     grid = W.uniform_grid(wl.n_dims, wl.n_bins)
-    n = {0: 200000, 1: 40000, 2: 4000, 3: 400, 4: 20000, 5: 2000}[wl.process]     # ~2 s per step
+    n = {0: 200000, 1: 40000, 2: 4000, 3: 400, 4: 20000, 5: 2000, 6: 24}[wl.process]     # ~2 s per step
     times = []
     for k in range(args.warmup + args.steps):
         t0 = time.perf_counter()
@@ -390,7 +391,7 @@ def main():
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": MEASURED_TRAFFIC.get((wl.process, n)), "traffic_source": "profiles/r1_coop_v4_traffic.md",
-                     "kernel": ("fused_pass_coop_kernel<%d,true>" if wl.process >= 2 else "fused_pass_kernel<%d,true>") % wl.process, "kernel_ms": kern,
+                     "kernel": "fused_pass_cta_kernel<true>" if wl.process == 6 else ("fused_pass_coop_kernel<%d,true>" if wl.process >= 2 else "fused_pass_kernel<%d,true>") % wl.process, "kernel_ms": kern,
                      "flops_per_me": me_flops(wl.process), "peak_source": "mf_measure_fp64_peak (DFMA chains) on this GPU",
                      "nominal_peak": NOMINAL_FP64 / 1e12, "frac_of_nominal": achieved / (NOMINAL_FP64 / 1e12)},
     }

@@ -36,7 +36,10 @@ typedef struct mf_process mf_process; /* opaque; owns its device-side constants 
  * adds to g g -> t tbar, at the same phase-space point and in the same pass, the q qbar -> t tbar channel of every
  * quark flavour of a multi-flavour PDF table, the quark taken from either beam:
  *   w ~ L_gg |M_gg|^2 + sum_i [ q_i(x1) qbar_i(x2) + qbar_i(x1) q_i(x2) ] / (x1 x2) |M_qq|^2                                */
-enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3, MF_PP_TT = 4, MF_PP_TTG = 5 };
+enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3, MF_PP_TT = 4, MF_PP_TTG = 5, MF_GG_TTGGG = 6 };
+/* MF_GG_TTGGG ("pp -> ttbar ggg", the paper's heaviest process): g g -> t tbar g g g, 1240 diagrams,
+ * 128 helicity states, 120 x 120 colour matrix; RAMBO with five final-state particles, D = 22; the cuts act on the three gluons.
+ * One event per thread block (csrc/mf_me_cta5.cuh); its shared-memory scratch leaves room for n_bins <= 64 (else MF_EINVAL). */
 /* MF_PP_TTG ("pp -> ttbar g (36 diagrams)"; R19): at the phase-space point, cuts and stream of MF_GG_TTG the
  * weight sums g g -> t tbar g and the flavour-summed q qbar -> t tbar g, q g -> t tbar q, qbar g -> t tbar qbar channels (either
  * beam assignment); the light final-state parton is a jet whatever its flavour.  Same multi-flavour table as MF_PP_TT. */

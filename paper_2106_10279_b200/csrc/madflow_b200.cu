@@ -10,6 +10,7 @@
 #include "../../include/mf.h"
 #include "mf_aux_kernels.cuh"
 #include "mf_kernels_coop.cuh"
+#include "mf_kernels_cta.cuh"
 
 static_assert(sizeof(mf::IterResult) == sizeof(mf_iter_result), "result layouts must agree");
 static_assert(mf::kMaxBins == MF_MAX_BINS, "bin limits must agree");
@@ -49,6 +50,7 @@ const void* pass_fn(int proc, bool unw) {
     case 1: return unw ? pass_fn<1, true>() : pass_fn<1, false>();
     case 4: return unw ? pass_fn<4, true>() : pass_fn<4, false>();
     case 5: return unw ? (const void*)mf::fused_pass_coop_kernel<5, true> : (const void*)mf::fused_pass_coop_kernel<5, false>;
+    case 6: return unw ? (const void*)mf::fused_pass_cta_kernel<true> : (const void*)mf::fused_pass_cta_kernel<false>;
     case 2: return unw ? (const void*)mf::fused_pass_coop_kernel<2, true> : (const void*)mf::fused_pass_coop_kernel<2, false>;
     default: return unw ? (const void*)mf::fused_pass_coop_kernel<3, true> : (const void*)mf::fused_pass_coop_kernel<3, false>;
   }
@@ -122,14 +124,14 @@ extern "C" {
 int mf_create_process(const mf_process_desc* d, mf_process** out) {
   if (out) *out = nullptr;
   if (!d || !out) return MF_EINVAL;
-  if (d->process < 0 || d->process > 5 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
+  if (d->process < 0 || d->process > 6 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
       !(d->gev2_to_pb > 0.0))
     return MF_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MF_ECUDA; }
   mf_process* p = new (std::nothrow) mf_process;
   if (!p) return MF_ENOMEM;
-  static const int Dtab[6] = {2, 4, 14, 18, 4, 14}, nftab[6] = {2, 2, 3, 4, 2, 3};
+  static const int Dtab[7] = {2, 4, 14, 18, 4, 14, 22}, nftab[7] = {2, 2, 3, 4, 2, 3, 5};
   p->process = d->process; p->D = Dtab[d->process]; p->NF = nftab[d->process];
   mf::Params& P = p->P;
   std::memset(&P, 0, sizeof(P));
@@ -150,11 +152,11 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     for (int i = 1; i < d->pdf_nx; ++i) if (!(d->pdf_lnx[i] > d->pdf_lnx[i - 1])) { delete p; return MF_EINVAL; }
     for (int i = 1; i < d->pdf_nq; ++i) if (!(d->pdf_lnq2[i] > d->pdf_lnq2[i - 1])) { delete p; return MF_EINVAL; }
     const bool flavoured = d->process == MF_PP_TT || d->process == MF_PP_TTG;
-    const int ng = d->process == MF_PP_TT ? 2 : d->process == MF_PP_TTG ? 3 : d->process + 1;
+    const int ng = d->process == MF_PP_TT ? 2 : d->process == MF_PP_TTG ? 3 : d->process == MF_GG_TTGGG ? 5 : d->process + 1;
     const int nfl = flavoured ? d->pdf_nfl : 1;
     if (flavoured && (nfl < 3 || nfl % 2 == 0 || nfl > mf::kMaxPartonTables)) { delete p; return MF_EINVAL; }
     P.pdf_nfl = nfl;
-    P.me_norm = std::pow(gs2, ng) / (256.0 * (ng == 4 ? 2.0 : 1.0));
+    P.me_norm = std::pow(gs2, ng) / (256.0 * (ng == 4 ? 2.0 : ng == 5 ? 6.0 : 1.0));
     const int ncut = p->NF - 2;
     const double thr = 2.0 * d->m_top + ncut * (d->ptmin > 0.0 ? d->ptmin : 0.0);
     P.tau_min = thr * thr / P.s;
@@ -191,6 +193,21 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     // cooperative pass: as many teams per block as the SM's shared memory holds, one block per SM
     e = p->process == 3 ? coop_setup<3>(p, prop) : p->process == 5 ? coop_setup<5>(p, prop) : coop_setup<2>(p, prop);
     if (e != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
+  } else if (p->process == MF_GG_TTGGG) {
+    // one event per block: the whole block's shared memory is the scratch of the matrix element
+    p->threads = mf::kCtaThreads;
+    p->smem = (size_t)mf::CtaSmem(p->D, P.n_bins, P.pdf_nx, p->threads).total * 8;
+    if (p->smem > (size_t)prop.sharedMemPerBlockOptin) { free_all(p); delete p; return MF_EINVAL; }   // n_bins too large
+    e = cudaSuccess;
+    for (int u = 0; u < 2 && e == cudaSuccess; ++u)
+      e = cudaFuncSetAttribute(pass_fn(6, u != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute((const void*)mf::debug_eval_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               mf::cta_debug_smem_bytes());
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute((const void*)mf::debug_me2_cta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               mf::cta_debug_smem_bytes());
+    if (e != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   } else {
     p->smem = (size_t)(p->D * (2 * P.n_bins + 1) + (1 + P.pdf_nfl) * P.pdf_nx + 5 * 32) * sizeof(double);
   }
@@ -206,9 +223,9 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
       (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
-  if (coop &&
-      (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads *
-                                       (p->process == 3 ? mf::g4::Prog::Queue : mf::g3::Prog::Queue) * 8)) != cudaSuccess) {
+  const int queue_doubles = p->process == MF_GG_TTGGG ? mf::kCtaQueue : p->process == 3 ? mf::g4::Prog::Queue : mf::g3::Prog::Queue;
+  if ((coop || p->process == MF_GG_TTGGG) &&
+      (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads * queue_doubles * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
   snprintf(p->err, sizeof(p->err), "ok");
@@ -295,6 +312,10 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
     case 1: mf::debug_eval_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 4: mf::debug_eval_kernel<4><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
     case 5: mf::debug_eval_kernel<5><<<blocks, mf::kThreads, 0, st>>>(p->P, A, d_out); break;
+    case 6:
+      mf::debug_eval_cta_kernel<<<(unsigned)((n_events + mf::kCtaDebugThreads - 1) / mf::kCtaDebugThreads), mf::kCtaDebugThreads,
+                                  mf::cta_debug_smem_bytes(), st>>>(p->P, A, d_out);
+      break;
     case 2:
       mf::debug_eval_coop_kernel<2><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                       mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, A, d_out);
@@ -342,6 +363,10 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
     case 1: mf::debug_me2_kernel<1><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 4: mf::debug_me2_kernel<4><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
     case 5: mf::debug_me2_kernel<5><<<blocks, mf::kThreads, 0, st>>>(p->P, d_mom, n, d_out); break;
+    case 6:
+      mf::debug_me2_cta_kernel<<<(unsigned)((n + mf::kCtaDebugThreads - 1) / mf::kCtaDebugThreads), mf::kCtaDebugThreads,
+                                 mf::cta_debug_smem_bytes(), st>>>(p->P, d_mom, n, d_out);
+      break;
     case 2:
       mf::debug_me2_coop_kernel<2><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, d_mom, n, d_out);

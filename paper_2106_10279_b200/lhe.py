@@ -23,7 +23,8 @@ import threading
 
 import numpy as np
 
-PDG = {0: (11, -11, 13, -13), 1: (21, 21, 6, -6), 2: (21, 21, 6, -6, 21), 3: (21, 21, 6, -6, 21, 21)}
+PDG = {0: (11, -11, 13, -13), 1: (21, 21, 6, -6), 2: (21, 21, 6, -6, 21), 3: (21, 21, 6, -6, 21, 21),
+       6: (21, 21, 6, -6, 21, 21, 21)}
 
 
 QUARK_PDG = (1, 2, 3, 4, 5)          # flavour index of the multi-flavour table -> PDG id (d, u, s, c, b)

@@ -38,6 +38,7 @@ def gpu_procs(pdf):
     procs = {wl.process: api.Process(wl, pdf) for wl in (W.C0, W.C1, W.C2, W.C3)}
     procs[W.MF_PP_TT] = api.Process(W.C5, W.pdf_table_flavours())
     procs[W.MF_PP_TTG] = api.Process(W.C6, W.pdf_table_flavours())
+    procs[W.MF_GG_TTGGG] = api.Process(W.C7, pdf)
     yield procs
     for p in procs.values():
         p.close()

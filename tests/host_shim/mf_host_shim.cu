@@ -5,6 +5,7 @@
 #include "../../paper_2106_10279_b200/csrc/mf_event.cuh"
 #include "../../paper_2106_10279_b200/csrc/mf_me_qttg.cuh"
 #include "../../paper_2106_10279_b200/csrc/mf_me_coop.cuh"
+#include "../../paper_2106_10279_b200/csrc/mf_me_cta5.cuh"
 #include <vector>
 
 using namespace mf;
@@ -59,6 +60,26 @@ double mfh_me2_coop(const double* mom, double m_top, double alpha_s) {   // g g 
 double mfh_me2_coop3(const double* mom, double m_top, double alpha_s) {  // g g -> t tbar g
   double gs2 = 4.0 * kPi * alpha_s;
   return coop_host_me2<g3::Prog>(mom, m_top, gs2 * gs2 * gs2 / 256.0);
+}
+
+// g g -> t tbar g g g (mf_me_cta5.cuh): the block's work items looped over stage by stage; mom[7][4] beams first
+double mfh_me2_cta5(const double* mom, double m_top, double alpha_s) {
+  using namespace mf::g5;
+  std::vector<double> S(kScratchDoubles, 0.0);
+  for (int i = 0; i < 5; ++i) for (int m = 0; m < 4; ++m) S[kOffIn + 4 * i + m] = mom[(2 + i) * 4 + m];
+  S[kOffIn + 20] = 4.0 * mom[0] * mom[0];
+  for (int i = 0; i < kStage0Items; ++i) stage0_item(S.data(), i, m_top);
+  for (int i = 0; i < kStage1Items; ++i) stage1_item(S.data(), i, m_top);
+  for (int i = 0; i < kStage2Items; ++i) stage2_item(S.data(), i, m_top);
+  for (int i = 0; i < kStage3Items; ++i) gluon_item(S.data(), 4, i);
+  for (int i = 0; i < kStage4Items; ++i) gluon_item(S.data(), 5, i);
+  double tot = 0.0;
+  for (int half = 0; half < 2; ++half) {
+    for (int i = 0; i < kAmpItems; ++i) amp_item(S.data(), half, i);
+    tot += colour_rows_plain(S.data(), 0, 1);
+  }
+  const double gs2 = 4.0 * kPi * alpha_s;
+  return 2.0 * tot / kCden * (gs2 * gs2 * gs2 * gs2 * gs2 / (256.0 * 6.0));
 }
 
 // quark channels of pp -> ttbar g (component; mf_me_qttg.cuh): mom = p1, p2, p3, p4, p5 as in the oracle's entry point

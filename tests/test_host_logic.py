@@ -87,7 +87,7 @@ def shim():
     L = C.CDLL(out)
     L.mfh_me2.restype = C.c_double
     L.mfh_me2.argtypes = [C.c_int, dp, C.c_double, C.c_double, C.c_double]
-    for f in (L.mfh_me2_coop, L.mfh_me2_coop3):
+    for f in (L.mfh_me2_coop, L.mfh_me2_coop3, L.mfh_me2_cta5):
         f.restype = C.c_double
         f.argtypes = [dp, C.c_double, C.c_double]
     L.mfh_event.argtypes = [C.c_int, dp, C.c_int] + [C.c_double] * 8 + [C.c_uint64, C.c_uint32, C.c_uint64, dp]
@@ -216,6 +216,20 @@ def test_shim_cooperative_program(shim, oracle_procs, pid, n):
         ref = oracle_procs[pid].me2(mom)
         got = fn(mom.ctypes.data_as(dp), 173.0, 0.118)
         assert abs(got - ref) <= 1e-11 * ref
+
+
+def test_shim_five_gluon_block_program(shim, oracle_procs):
+    """g g -> t tbar g g g (mf_me_cta5.cuh: one event per thread block, work items looped over stage by stage on the host;
+    meet-in-the-middle amplitudes, top spin 0 doubled, plain colour loop instead of the DMMA tiles) against the oracle."""
+    from oracle import mfo
+    rng = np.random.default_rng(15)
+    for i in range(6):
+        w = 600.0 + 4000.0 * rng.random() ** 2
+        k, _ = mfo.rambo([173.0, 173.0, 0.0, 0.0, 0.0], w, rng.random(20))
+        mom = np.ascontiguousarray(np.vstack([[w / 2, 0, 0, w / 2], [w / 2, 0, 0, -w / 2], k]))
+        ref = oracle_procs[6].me2(mom)
+        got = shim.mfh_me2_cta5(mom.ctypes.data_as(dp), 173.0, 0.118)
+        assert abs(got - ref) <= 1e-11 * ref, (i, got, ref)
 
 
 # ---- multi-rank sharding (gloo, world size 2) ------------------------------------------------------------------
