@@ -47,7 +47,7 @@ enum { MF_OK = 0, MF_EINVAL = -1, MF_ECUDA = -2, MF_EOVERFLOW = -3, MF_ERANGE = 
 
 /* Process descriptor (host memory; copied at create).  Same field order as the oracle's mfo_process_desc. */
 typedef struct {
-  int32_t process;            /* enum above; fixes n_final, D (2/4/14/18/4), helicities, colour matrix */
+  int32_t process;            /* enum above; fixes n_final, D (2/4/14/18/4/14/22), helicities, colour matrix */
   double sqrt_s;              /* GeV; hadronic (pp) for processes 1-3, leptonic for 0                   */
   double alpha_em, alpha_s;   /* couplings: e^2 = 4 pi alpha_em, g_s^2 = 4 pi alpha_s                   */
   double m_top;               /* GeV; width 0                                                           */
@@ -102,7 +102,9 @@ int mf_refine_grid(mf_process *p, double *d_grid, const double *d_hist, double a
  * overflow signal.  Record order is unspecified (sort by event id).  d_hist may be NULL.
  * MF_PP_TT appends one more uint64 to each record: the partonic channel of the event (0 = g g; 1 + 2 i = quark i from
  * beam 1 and its antiquark from beam 2; 2 + 2 i = the other way round), drawn in proportion to |luminosity x |M|^2| of
- * the channels, in that order, with the second uniform of the accept block (R18). */
+ * the channels, in that order, with the second uniform of the accept block (R18).
+ * MF_PP_TTG likewise (R20; the LHE writer needs the partons of every event): 0 = g g; 1 + 6 i + c = flavour i in
+ * class c (0 q qbar, 1 qbar q, 2 q g, 3 g q, 4 qbar g, 5 g qbar; first parton from beam 1): records of 5 x 32 + 16 + 8 bytes. */
 int mf_unweight(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                 uint64_t n_events, double w_max, void *d_records, uint64_t capacity, uint64_t *d_count,
                 double *d_hist, mf_iter_result *d_result, void *stream);

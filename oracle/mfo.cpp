@@ -51,7 +51,8 @@ template <class R> struct EventOut {
   R mom[7][4];  // lab frame, beams first
   R x1, x2, lum, me2, phi, jac, w;
   R lum_qq, me2_qq;  // process 4: the flavour-summed q qbar luminosity and the q qbar matrix element
-  R chan[12];        // process 4: luminosity x |M|^2 of every partonic channel (0 gg; 1+2i q_i from beam 1; 2+2i from beam 2)
+  R chan[32];        // process 4: luminosity x |M|^2 of every partonic channel (0 gg; 1+2i q_i from beam 1; 2+2i from beam 2)
+                     // process 5 (R20): 0 gg; 1 + 6 i + c: flavour i in class c (q qbar, qbar q, q g, g q, qbar g, g qbar)
   int n_chan;
   R chq[6];          // process 5: luminosity x |M|^2 of the six flavour-summed quark-channel classes
   int pass;
@@ -176,17 +177,23 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
     // makes it (the cuts act on it alike):
     //   q qbar, qbar q -> ttbar g;   q g, g q -> ttbar q;   qbar g, g qbar -> ttbar qbar
     R Q1 = R(0), Qb1 = R(0), Q2 = R(0), Qb2 = R(0), D12 = R(0), D21 = R(0);
-    for (size_t i = 0; i + 1 < P.pdfq.size(); i += 2) {
+    R g1 = pdf_xf<R>(P.pdf, o.x1, mu2), g2 = pdf_xf<R>(P.pdf, o.x2, mu2);
+    R lumf[5][6];   // per flavour and class (R20: the partonic channel of an accepted event)
+    int nfl = 0;
+    for (size_t i = 0; i + 1 < P.pdfq.size(); i += 2, ++nfl) {
       R q1 = pdf_xf<R>(P.pdfq[i], o.x1, mu2), qb1 = pdf_xf<R>(P.pdfq[i + 1], o.x1, mu2);
       R q2 = pdf_xf<R>(P.pdfq[i], o.x2, mu2), qb2 = pdf_xf<R>(P.pdfq[i + 1], o.x2, mu2);
       Q1 = Q1 + q1; Qb1 = Qb1 + qb1; Q2 = Q2 + q2; Qb2 = Qb2 + qb2;
       D12 = D12 + q1 * qb2;
       D21 = D21 + qb1 * q2;
+      lumf[nfl][0] = q1 * qb2; lumf[nfl][1] = qb1 * q2; lumf[nfl][2] = q1 * g2; lumf[nfl][3] = g1 * q2;
+      lumf[nfl][4] = qb1 * g2; lumf[nfl][5] = g1 * qb2;
     }
-    R g1 = pdf_xf<R>(P.pdf, o.x1, mu2), g2 = pdf_xf<R>(P.pdf, o.x2, mu2);
     R lumc[6] = {D12, D21, Q1 * g2, g1 * Q2, Qb1 * g2, g1 * Qb2};
     const int kind[6] = {0, 0, 1, 1, 2, 2};
     R both = R(0);
+    o.chan[0] = o.lum * o.me2;
+    o.n_chan = 1 + 6 * nfl;
     for (int c = 0; c < 6; ++c) {
       R m5[5][4];
       for (int i = 0; i < 5; ++i)
@@ -196,6 +203,7 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
       R M = me2_light_line_ttbar_g<R>(kind[c], m5, R(P.d.m_top), R(P.d.alpha_s), 0, 0) * as_factor;
       o.chq[c] = lumc[c] / (o.x1 * o.x2) * M;
       both = both + o.chq[c];
+      for (int i = 0; i < nfl; ++i) o.chan[1 + 6 * i + c] = lumf[i][c] / (o.x1 * o.x2) * M;
     }
     f = (o.lum * o.me2 + both) / (R(2) * shat) * o.phi * jac_parton * R(P.d.gev2_to_pb);
   }
@@ -219,7 +227,8 @@ int iterate(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteratio
   S sw = S(0), sw2 = S(0);
   double maxw = 0;
   uint64_t npass = 0, nacc = 0;
-  int recsize = (P.nfinal + 2) * 32 + 16 + (P.d.process == 4 ? 8 : 0);
+  const bool has_channel = P.d.process == 4 || P.d.process == 5;
+  int recsize = (P.nfinal + 2) * 32 + 16 + (has_channel ? 8 : 0);
   EventOut<R> o;
   for (uint64_t e = first; e < first + n_events; ++e) {
     eval_event<R>(P, grid, seed, iteration, e, o);
@@ -244,10 +253,10 @@ int iterate(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteratio
           buf[(P.nfinal + 2) * 4] = w;
           std::memcpy(rec, buf, ((P.nfinal + 2) * 4 + 1) * sizeof(double));
           std::memcpy(rec + ((P.nfinal + 2) * 4 + 1) * sizeof(double), &e, sizeof(uint64_t));
-          if (P.d.process == 4) {
-            // R18: the partonic channel of an accepted event is drawn in proportion to |luminosity x |M|^2| of the
+          if (has_channel) {
+            // R18 / R20: the partonic channel of an accepted event is drawn in proportion to |luminosity x |M|^2| of the
             // channels, in channel order: the first c with  sum_{c' <= c} |a_c'| > v * sum |a|,  v the channel draw
-            double a[12], total = 0.0;
+            double a[32], total = 0.0;
             for (int c = 0; c < o.n_chan; ++c) { a[c] = std::fabs(r_to_double(o.chan[c])); total += a[c]; }
             double v = channel_draw(seed, iteration, e) * total, cum = 0.0;
             uint64_t pick = (uint64_t)(o.n_chan - 1);
@@ -402,7 +411,7 @@ int mfo_n_dims(const mfo_process* P, int32_t* D) { if (!P || !D) return -1; *D =
 int mfo_n_final(const mfo_process* P, int32_t* n) { if (!P || !n) return -1; *n = P->nfinal; return 0; }
 int mfo_record_size(const mfo_process* P, int32_t* b) {
   if (!P || !b) return -1;
-  *b = (P->nfinal + 2) * 32 + 16 + (P->d.process == 4 ? 8 : 0);   // process 4 appends the u64 channel code
+  *b = (P->nfinal + 2) * 32 + 16 + ((P->d.process == 4 || P->d.process == 5) ? 8 : 0);   // processes 4, 5 append the u64 channel code
   return 0;
 }
 int mfo_debug_row_len(const mfo_process* P, int32_t* n) {

@@ -48,7 +48,8 @@ int mfo_vegas_iterate(mfo_process*, const double* grid, uint64_t seed, uint32_t 
 int mfo_refine_grid(mfo_process*, double* grid, const double* hist, double alpha, int prec);
 /* O15: accepted events appended in event order at records[*count]; *count advances for every accepted event.
  * Record: (n+2) lab four-momenta, w, u64 event id; process 4 appends the u64 channel code of R18
- * (0 gg; 1+2i quark i from beam 1; 2+2i quark i from beam 2), drawn with the second uniform of the accept block */
+ * (0 gg; 1+2i quark i from beam 1; 2+2i quark i from beam 2), drawn with the second uniform of the accept block;
+ * process 5 likewise (R20): 0 gg; 1 + 6 i + c = flavour i in class c (q qbar, qbar q, q g, g q, qbar g, g qbar) */
 int mfo_unweight(mfo_process*, const double* grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                  uint64_t n_events, double w_max, void* records, uint64_t capacity, uint64_t* count, double* hist,
                  mfo_iter_result* result, int prec);

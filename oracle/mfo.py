@@ -328,7 +328,7 @@ class Process:
     def records_array(self, rec, count):
         """Decode `count` AoS records into a structured array: mom[n+2][4], w, id and, for process 4, channel."""
         fields = [("mom", np.float64, (self.n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)]
-        if self.wl.process == 4:
+        if self.wl.process in (4, 5):
             fields.append(("channel", np.uint64))
         dt = np.dtype(fields)
         assert dt.itemsize == self.record_size

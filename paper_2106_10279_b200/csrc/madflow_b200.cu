@@ -244,7 +244,7 @@ int mf_n_dims(const mf_process* p, int32_t* D) { if (!p || !D) return MF_EINVAL;
 int mf_n_final(const mf_process* p, int32_t* n) { if (!p || !n) return MF_EINVAL; *n = p->NF; return MF_OK; }
 int mf_record_size(const mf_process* p, int32_t* b) {
   if (!p || !b) return MF_EINVAL;
-  *b = (p->NF + 2) * 32 + 16 + (p->process == MF_PP_TT ? 8 : 0);
+  *b = (p->NF + 2) * 32 + 16 + ((p->process == MF_PP_TT || p->process == MF_PP_TTG) ? 8 : 0);
   return MF_OK;
 }
 int mf_debug_row_len(const mf_process* p, int32_t* n) {

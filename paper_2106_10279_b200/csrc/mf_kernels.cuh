@@ -285,6 +285,46 @@ MF_D int observable_bins(const PassArgs& A, const Event<PROC>& ev) {
 
 constexpr int kThreads = 128;
 
+// pp -> ttbar j (R20): the partonic channel of an ACCEPTED event: code 0 = gg, code 1 + 6 i + c = flavour i in class
+// c (0 q qbar, 1 qbar q, 2 q g, 3 g q, 4 qbar g, 5 g qbar; first parton from beam 1), drawn in proportion to
+// |luminosity x |M|^2| in code order: the first code whose cumulative sum exceeds v x the total, v = the second uniform of
+// the event's accept block.  Accepted events are rare (< 1 %): everything is recomputed here from the
+// tables in global memory; the gluon channel's term (the team's matrix element is not kept) is what the event's weight w
+// leaves after the quark terms: w = common x (gg term + sum of the signed quark terms).
+// (inlined: as an out-of-line function, with nvcc 12.9 for sm_100a, it received its weight argument as 0 in this kernel,
+// by value or through a struct; measured cost of the larger frame: 34.8 -> 39.2 ms per 2^22 events of mf_unweight)
+__device__ __forceinline__ unsigned pp_ttj_channel(const Params& P, const PassArgs& A, const Event<5>& ev, double w, double v) {
+  double f1[kMaxPartonTables], f2[kMaxPartonTables], asf;
+  parton_densities<5>(P, A, A.pdf_lnx, A.pdf_row, ev, f1, f2, asf);
+  const int nf = (P.pdf_nfl - 1) / 2;
+  const double inv = 1.0 / (ev.x1 * ev.x2);
+  double M[6];
+#pragma unroll 1
+  for (int c = 0; c < 6; ++c) M[c] = quark_gluon_me2(P, ev.shat, ev.k, c) * asf;
+  auto sterm = [&](int i, int c) {
+    const double q1 = f1[1 + 2 * i], qb1 = f1[2 + 2 * i], q2 = f2[1 + 2 * i], qb2 = f2[2 + 2 * i];
+    const double l = c == 0 ? q1 * qb2 : c == 1 ? qb1 * q2 : c == 2 ? q1 * f2[0] : c == 3 ? f1[0] * q2 : c == 4 ? qb1 * f2[0] : f1[0] * qb2;
+    return l * inv * M[c];
+  };
+  auto term = [&](int i, int c) { return fabs(sterm(i, c)); };
+  double quark_sum = 0.0;
+  for (int i = 0; i < nf; ++i)
+    for (int c = 0; c < 6; ++c) quark_sum += sterm(i, c);
+  const double gg_term = w / event_weight<5>(P, ev, 1.0, 1.0) - quark_sum;
+  double total = fabs(gg_term);
+  for (int i = 0; i < nf; ++i)
+    for (int c = 0; c < 6; ++c) total += term(i, c);
+  const double vt = v * total;
+  double cum = fabs(gg_term);
+  if (cum > vt) return 0u;
+  for (int i = 0; i < nf; ++i)
+    for (int c = 0; c < 6; ++c) {
+      cum += term(i, c);
+      if (cum > vt) return (unsigned)(1 + 6 * i + c);
+    }
+  return (unsigned)(6 * nf);
+}
+
 // Per-thread running sums of the pass (registers).
 struct Accum {
   double sum_w = 0.0, sum_w2 = 0.0, max_w = 0.0;
@@ -337,7 +377,7 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
           }
           double mom[NF + 2][4];
           lab_momenta<PROC>(ev, mom);
-          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16 + (PROC == 4 ? 8 : 0)));
+          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16 + ((PROC == 4 || PROC == 5) ? 8 : 0)));
 #pragma unroll
           for (int i = 0; i < NF + 2; ++i)
 #pragma unroll
@@ -345,6 +385,10 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
           rec[4 * (NF + 2)] = w;
           reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
           if (PROC == 4) reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = channel;
+          if constexpr (PROC == 5) {
+            const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);      // words z, w: the channel draw
+            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = pp_ttj_channel(P, A, ev, w, uniform52(r.z, r.w));
+          }
         }
       }
     }

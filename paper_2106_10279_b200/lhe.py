@@ -32,7 +32,7 @@ QUARK_PDG = (1, 2, 3, 4, 5)          # flavour index of the multi-flavour table 
 
 def record_dtype(n_final, process=None):
     fields = [("mom", np.float64, (n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)]
-    if process == 4:                  # MF_PP_TT records carry the partonic channel (include/mf.h)
+    if process in (4, 5):             # MF_PP_TT / MF_PP_TTG records carry the partonic channel (include/mf.h)
         fields.append(("channel", np.uint64))
     return np.dtype(fields)
 
@@ -47,6 +47,25 @@ def channel_ids(channel):
     if c % 2 == 1:
         return (q, -q, 6, -6), [(501, 0), (0, 502), (501, 0), (0, 502)]
     return (-q, q, 6, -6), [(0, 502), (501, 0), (501, 0), (0, 502)]
+
+
+def channel_ids_ttj(channel):
+    """PDG ids (beam 1, beam 2, t, tbar, parton) and one valid colour flow of an MF_PP_TTG record's channel code (R20):
+    0 = gg; 1 + 6 i + c = flavour i in class c (q qbar, qbar q, q g, g q, qbar g, g qbar)"""
+    c = int(channel)
+    if c == 0:
+        return PDG[2], colour_flow(2)
+    q, cls = QUARK_PDG[(c - 1) // 6], (c - 1) % 6
+    if cls < 2:          # q qbar -> t tbar g: q's colour to the gluon, the gluon's anticolour to the top, qbar's line to tbar
+        ids, flow = [q, -q, 6, -6, 21], [(501, 0), (0, 502), (503, 0), (0, 502), (501, 503)]
+    elif cls < 4:        # q g -> t tbar q: the quark line goes through; the gluon's colour to t, its anticolour to tbar
+        ids, flow = [q, 21, 6, -6, q], [(501, 0), (502, 503), (502, 0), (0, 503), (501, 0)]
+    else:                # qbar g -> t tbar qbar
+        ids, flow = [-q, 21, 6, -6, -q], [(0, 501), (502, 503), (502, 0), (0, 503), (0, 501)]
+    if cls & 1:          # the (anti)quark comes from beam 2
+        ids[0], ids[1] = ids[1], ids[0]
+        flow[0], flow[1] = flow[1], flow[0]
+    return tuple(ids), flow
 
 
 def colour_flow(process):
@@ -69,15 +88,15 @@ def colour_flow(process):
 
 def format_events(rec, process, m_top, scale, alpha_em, alpha_s, w_max):
     """LHE <event> blocks for a structured record array (pure function: also used by the tests)"""
-    per_event = process == 4
+    per_event = process in (4, 5)
     if not per_event:
         ids = PDG[process]
         flow = colour_flow(process)
-    n = 4 if per_event else len(ids)
+    n = {4: 4, 5: 5}[process] if per_event else len(ids)
     out = io.StringIO()
     for r in rec:
         if per_event:
-            ids, flow = channel_ids(r["channel"])
+            ids, flow = channel_ids(r["channel"]) if process == 4 else channel_ids_ttj(r["channel"])
         mass = [m_top if abs(p) == 6 else 0.0 for p in ids]
         w = float(r["w"])
         xw = (1.0 if w >= 0 else -1.0) * max(1.0, abs(w) / w_max)
@@ -94,9 +113,8 @@ def format_events(rec, process, m_top, scale, alpha_em, alpha_s, w_max):
 class LheDrain:
     def __init__(self, path, proc, compress=None):
         import torch
-        if proc.wl.process not in PDG and proc.wl.process != 4:
-            raise ValueError("LHE output needs the partons of every event: process %d does not record its partonic channel "
-                             "yet (include/mf.h, MF_PP_TTG)" % proc.wl.process)
+        if proc.wl.process not in PDG and proc.wl.process not in (4, 5):
+            raise ValueError("LHE output: unknown process %d" % proc.wl.process)
         self.torch = torch
         self.path = path
         self.proc = proc

@@ -385,13 +385,14 @@ def test_unweight(proc, n, gpu_procs, oracle_procs):
             np.testing.assert_allclose(w_g[order], w_o, rtol=REL_EVENT)
             scale = np.abs(mom_o).max(axis=(1, 2), keepdims=True)
             assert np.max(np.abs(mom_g[order] - mom_o) / scale) < 1e-11
-            if proc == 4:
-                # the partonic channel drawn for every accepted event (R18): an integer decided by floating point; both
-                # sides decide in fp64, and no event of this stream sits within rounding of a channel boundary
+            if proc in (4, 5):
+                # the partonic channel drawn for every accepted event (R18, R20): an integer decided by floating point;
+                # both sides decide in fp64, and no event of this stream sits within rounding of a channel boundary
                 ch_g = gp.records_array(records[start * gp.record_size:], n_written)["channel"][order]
                 ch_o = op.records_array(rec_o, cnt_o)["channel"]
                 assert np.array_equal(ch_g, ch_o)
-                assert (ch_o == 0).sum() > 0.8 * cnt_o and (ch_o > 0).sum() > 10 and ch_o.max() <= 2 * W.N_FLAVOURS
+                assert (ch_o == 0).sum() > 0.5 * cnt_o and (ch_o > 0).sum() > 10
+                assert ch_o.max() <= (2 if proc == 4 else 6) * W.N_FLAVOURS
         else:
             # overflow: count > capacity is the signal; what was written is a valid subset
             assert int(count.item()) > capacity

@@ -76,6 +76,30 @@ def test_flavour_summed_records_carry_their_partons():
         assert sorted(set(col_in) - set(acol_in)) == col_out and sorted(set(acol_in) - set(col_in)) == acol_out
 
 
+def test_ttj_records_carry_their_partons():
+    """MF_PP_TTG (R20): PDG ids and a colour-conserving flow for every class and beam assignment"""
+    rec = np.zeros(7, dtype=lhe.record_dtype(3, 5))
+    assert rec.dtype.itemsize == 5 * 32 + 24
+    rec["channel"] = [0, 1, 2, 1 + 6 + 2, 1 + 6 + 3, 1 + 12 + 4, 1 + 18 + 5]
+    rec["w"] = 1.0
+    ev = _parse(lhe.format_events(rec, 5, 173.0, 173.0, 1 / 132.507, 0.118, w_max=1.0))
+    assert [[int(p[0]) for p in e[2]] for e in ev] == [[21, 21, 6, -6, 21], [1, -1, 6, -6, 21], [-1, 1, 6, -6, 21],
+                                                       [2, 21, 6, -6, 2], [21, 2, 6, -6, 2], [-3, 21, 6, -6, -3],
+                                                       [21, -4, 6, -6, -4]]
+    for _, _, parts, _ in ev:
+        col_in = sorted(int(p[4]) for p in parts[:2] if int(p[4]))
+        acol_in = sorted(int(p[5]) for p in parts[:2] if int(p[5]))
+        col_out = sorted(int(p[4]) for p in parts[2:] if int(p[4]))
+        acol_out = sorted(int(p[5]) for p in parts[2:] if int(p[5]))
+        for p in parts:
+            pid, c, a = int(p[0]), int(p[4]), int(p[5])
+            assert (c != 0) == (pid == 21 or pid > 0) and (a != 0) == (pid == 21 or pid < 0)
+        # colour conservation: incoming colours = outgoing colours up to lines created in pairs (colour + anticolour out)
+        created = set(col_out) & set(acol_out)
+        assert sorted(set(col_in) - set(acol_in)) == sorted(set(col_out) - created)
+        assert sorted(set(acol_in) - set(col_in)) == sorted(set(acol_out) - created)
+
+
 @pytest.mark.gpu
 def test_lhe_drain_flavour_summed(tmp_path):
     """the drain on MF_PP_TT records: every event of the file has the partons of its record's channel"""

@@ -160,3 +160,60 @@ def test_process_rows_from_parts(oracle_procs):
         # w(5) / w(2) = (gg + quark terms) / gg
         assert w / r2[o + 6] == pytest.approx((lum * me2 + r[-6:].sum()) / (lum * me2), rel=1e-11)
     assert n_pass > 60
+
+
+def test_channel_of_accepted_events():
+    """R20: every accepted event of pp -> ttbar j carries its partonic channel: code 0 = gg, code 1 + 6 i + c =
+    flavour i in class c (q qbar, qbar q, q g, g q, qbar g, g qbar), drawn in proportion to |luminosity x |M|^2| in code
+    order with the second uniform of the accept block.  Recomputed here from single-table lookups, the component
+    matrix-element calls and the raw Philox words; the frequencies against their expectation."""
+    P5 = mfo.Process(W.C6, W.pdf_table_flavours())
+    n = 1500
+    grid = W.uniform_grid(14)
+    rows = P5.debug_eval(grid, 2, 4, 100, n)
+    o = 14 + 20
+    w = rows[:, o + 6]
+    w_max = float(np.quantile(np.abs(w[w != 0]), 0.6))
+    rec, cnt, _, res = P5.unweight(grid, 2, 4, 100, n, w_max, n)
+    arr = P5.records_array(rec, cnt)
+    chan, ids = arr["channel"], arr["id"]
+    assert cnt == res.n_accept and cnt > 300 and P5.record_size == 5 * 32 + 16 + 8
+    mu2, nf = MT ** 2, W.N_FLAVOURS
+    expect = np.zeros(1 + 6 * nf)
+    for k in range(n):
+        r = rows[k]
+        x1, x2, lum, me2 = r[o:o + 4]
+        if not r[o + 7]:
+            continue
+        mom = r[14:o].reshape(5, 4)
+        sw = mom[[1, 0, 2, 3, 4]]
+        M = [mfo.me2_light_line_ttbar_g(0, mom, MT, AS), mfo.me2_light_line_ttbar_g(0, sw, MT, AS),
+             mfo.me2_light_line_ttbar_g(1, mom, MT, AS), mfo.me2_light_line_ttbar_g(1, sw, MT, AS),
+             mfo.me2_light_line_ttbar_g(2, mom, MT, AS), mfo.me2_light_line_ttbar_g(2, sw, MT, AS)]
+        f = lambda t, x: P5.pdf_xf_table(t, x, mu2)
+        g1, g2 = f(0, x1), f(0, x2)
+        terms = [lum * me2]
+        for i in range(nf):
+            q1, qb1, q2, qb2 = f(1 + 2 * i, x1), f(2 + 2 * i, x1), f(1 + 2 * i, x2), f(2 + 2 * i, x2)
+            lumf = [q1 * qb2, qb1 * q2, q1 * g2, g1 * q2, qb1 * g2, g1 * qb2]
+            terms += [lumf[c] / (x1 * x2) * M[c] for c in range(6)]
+        terms = np.array(terms)
+        a = np.abs(terms)
+        # the class sums of the row are the flavour sums of these (signed) terms
+        np.testing.assert_allclose([terms[1 + c::6].sum() for c in range(6)], r[-6:], rtol=1e-9, atol=1e-12 * a.max())
+        expect += min(1.0, abs(w[k]) / w_max) * a / a.sum()
+        hit = np.nonzero(ids == 100 + k)[0]
+        if len(hit):
+            words = mfo.philox_block(2, 4, 100 + k, 0xFFFFFFFF)
+            v = mfo.uniform_from_words(words[2], words[3]) * a.sum()
+            cum = np.cumsum(a)
+            if np.min(np.abs(cum - v)) > 1e-9 * a.sum():
+                assert chan[hit[0]] == int(np.argmax(cum > v)), k
+    assert abs(expect.sum() - cnt) < 5 * math.sqrt(cnt)
+    got = np.bincount(chan.astype(int), minlength=len(expect))
+    by_class = lambda v: np.array([v[0]] + [v[1 + c::6].sum() for c in range(6)])
+    for g, e in zip(by_class(got), by_class(expect)):
+        assert abs(g - e) < 5 * math.sqrt(e + 1), (g, e)
+    assert got[0] > 0.5 * cnt and got[1:].sum() > 30 and chan.max() <= 6 * nf
+    # q g (valence quarks against the large gluon density) dominates the quark channels
+    assert by_class(got)[3] + by_class(got)[4] > by_class(got)[1] + by_class(got)[2]
