@@ -70,14 +70,18 @@ typedef struct {
   uint64_t n_pass, n_accept;       /* events passing the cuts; events accepted (mf_unweight only)      */
 } mf_iter_result;
 
-/* Creates a handle.  Errors: NULL / bad enum / n_bins out of range / bad table or table count -> MF_EINVAL;
+/* Creates a handle for one process of the problem of PAPER.md L25 (i)-(v): (i) the parton-level process and its
+ * couplings, (ii) the parton densities (the table is copied to the device and collapsed at mu2), (iii) the fiducial cuts,
+ * (iv)-(v) the integration set-up (n_bins) the hot calls of PAPER.md L61 then run with.  Errors: NULL / bad enum / n_bins out of range / bad table or table count -> MF_EINVAL;
  * mu2 outside the Q^2 knots or tau_min below the x knots -> MF_ERANGE; no device or CUDA failure ->
  * MF_ECUDA; device allocation failure -> MF_ENOMEM.  On error *out is set to NULL. */
 int mf_create_process(const mf_process_desc *desc, mf_process **out);
+/* Frees everything mf_create_process allocated (the handle is the process definition, nothing else lives in
+ * it).  The handle must be destroyed on the device it was created on, after the streams using it have drained. */
 int mf_destroy_process(mf_process *p);
-int mf_n_dims(const mf_process *p, int32_t *D);              /* VEGAS dimensions: 2, 4, 14, 18, 4       */
-int mf_n_final(const mf_process *p, int32_t *n);             /* final-state particles: 2, 2, 3, 4, 2    */
-int mf_record_size(const mf_process *p, int32_t *bytes);     /* (n_final+2)*32 + 16 (+8: MF_PP_TT)      */
+int mf_n_dims(const mf_process *p, int32_t *D);              /* VEGAS dimensions: 2, 4, 14, 18, 4, 14, 22 */
+int mf_n_final(const mf_process *p, int32_t *n);             /* final-state particles: 2, 2, 3, 4, 2, 3, 5 */
+int mf_record_size(const mf_process *p, int32_t *bytes);     /* (n_final+2)*32 + 16 (+8: MF_PP_TT, MF_PP_TTG) */
 int mf_debug_row_len(const mf_process *p, int32_t *n_doubles);/* 3*D + 4*(n_final+2) + 9 (+2 / +6: MF_PP_TT / _TTG) */
 const char *mf_last_error(const mf_process *p);              /* static or handle-owned string           */
 /* launch geometry of the fused pass (blocks, threads per block), for reporting */
@@ -90,7 +94,8 @@ int mf_launch_config(const mf_process *p, int32_t *blocks, int32_t *threads);
 int mf_vegas_iterate(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                      uint64_t n_events, double *d_hist, mf_iter_result *d_result, void *stream);
 
-/* VEGAS grid refinement (step a13; Lepage's smoothing + damping r = ((s-1)/ln s)^alpha + rebinning), in
+/* VEGAS grid refinement (step a13; the integration is VEGAS importance sampling, whose grid adapts between
+ * iterations; Lepage's smoothing + damping r = ((s-1)/ln s)^alpha + rebinning), in
  * place on d_grid from d_hist.  A dimension whose histogram is all zero is left unchanged. */
 int mf_refine_grid(mf_process *p, double *d_grid, const double *d_hist, double alpha, void *stream);
 

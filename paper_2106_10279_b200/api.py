@@ -4,9 +4,9 @@ Every step of the hot path runs in the CUDA kernels of libmadflow_b200.so; PyTor
 and streams.  There is NO fallback: if the library is missing or no CUDA device is present, calls raise.
 
 The module-level functions carry the C names (mf_create_process, mf_vegas_iterate, mf_refine_grid,
-mf_unweight, ...) and take raw integers (device pointers); `Process` wraps them for torch tensors, and
-`run_config` is the integration driver (iteration loop, grid refinement schedule, w_max policy) that
-bench.py and the tests use.
+mf_unweight, ...) and take raw integers (device pointers); `Process` wraps them for torch tensors.  The
+integration driver (iteration loop, grid refinement schedule, w_max policy) that bench.py and the tests use is
+`integrate.run_config`.
 """
 import ctypes as C
 import math

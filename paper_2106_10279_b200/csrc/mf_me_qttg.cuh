@@ -52,7 +52,9 @@ MF_HD double me2_light_line_ttg(int kind, const double p1[4], const double prow[
   const double wE = 1.0 / (sl * st);
   rvec E[2];
   pol_vectors(pg, E[0], E[1]);
-  // colour matrix in units of 1/3 (csrc/gen_qttg_colour.py; the fifth tensor taken as i f^{bca} T^b T^c):
+  // colour matrix in units of 1/3: S[d][e] = sum over colours of conj(C_d) C_e of the five colour tensors
+  // (T^b T^a)_{ji} T^b_{kl}, (T^a T^b)_{ji} T^b_{kl}, T^b_{ji} (T^a T^b)_{kl}, T^b_{ji} (T^b T^a)_{kl}, i f^{bca} T^b_{ji} T^c_{kl}
+  // (checked against the oracle's explicit-generator sum by the parity tests of this matrix element):
   //   3 S = {{8, -1, 7, -2, 9}, {-1, 8, -2, 7, -9}, {7, -2, 8, -1, 9}, {-2, 7, -1, 8, -9}, {9, -9, 9, -9, 18}}
   double total = 0.0;
   for (int lam = 0; lam < 2; ++lam) {
