@@ -37,16 +37,24 @@ def metric_for(wl):
     """the BASELINE.json metric for the headline process; the same quantity, named after its process, for --config"""
     return METRIC if wl.process == 3 else "integrand events/sec (fp64) for " + PROCESS_LABEL[wl.process]
 UNIT = "events/s"
-# static fp64 operation counts per matrix-element evaluation, written by csrc/gen_me.py into
-# mf_me_ggtt_generated.cuh (kFlopsMe2_*); per-event work outside the matrix element (DESIGN.md table)
-# Executed fp64 flop per event OUTSIDE the matrix element (a1-a6, a10-a14 incl. the software sqrt / div / log / sincos
-# sequences and, for the cooperative kernels, the owner-side wavefunctions), from ncu
-# (smsp__sass_thread_inst_executed_op_{dfma x 2, dadd, dmul}_pred_on of one fused-pass launch minus n_pass x the
-# generator's static matrix-element count; profiles/r1_flops_per_event.md).  For the two thread-per-event kernels the
-# compiler folds the constant beam wavefunctions into the matrix element, so the static count overestimates: there
-# the measured TOTAL per event is used (ME_FLOPS_MEASURED) and OTHER_FLOPS is 0.
-OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 6500.0}    # 6: estimate (C3's + one more RAMBO particle)
-ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 115100.0}    # 5: per event PASSING the cuts (rate 0.8945)
+# ---- the roofline numerator (DESIGN.md section 7) ------------------------------------------------------------------------
+# achieved = (n_pass x flop per matrix element + n_events x flop per event outside it) / kernel time.
+#  * cooperative / block kernels (processes 2, 3, 6): flop per matrix element = the generators' static operation count,
+#    read from the generated headers at run time (FLOP_HEADERS; a DMMA.884 counts its 2 x 256 flop); the rest of the chain
+#    (a1-a6, a10-a14 incl. the software sqrt / div / log / sincos sequences and the owner-side wavefunctions) is OTHER_FLOPS,
+#    calibrated by ncu: executed (2 dfma + dadd + dmul) of one launch minus n_pass x the static count (FLOP_PROFILES).
+#  * thread-per-event kernels (0, 1, 4) and pp -> ttbar j (5): the compiler folds constants into the matrix element, so the
+#    static count overestimates: the ncu-executed TOTAL per event (per passing event for 5) is used (ME_FLOPS_MEASURED).
+# tests/test_host_logic.py::test_bench_flop_constants recomputes every literal below from the committed ncu csv files.
+FLOP_HEADERS = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g"),
+                6: ("mf_me_ttggg_tables_generated.cuh", "kFlopsMe2Cta_3g")}
+FLOP_PROFILES = {0: "profiles/r1_flops_C0.csv", 1: "profiles/r1_flops_C1.csv", 2: "profiles/r1_flops_C2.csv",
+                 3: "profiles/r1_flops_C3.csv", 4: "profiles/r1_flops_C5.csv", 5: "profiles/r1_flops_C6.csv"}
+FLOP_PROFILE_EVENTS = {0: (1_000_000, 1.0), 1: (1 << 20, 1.0), 2: (1 << 22, 0.8934), 3: (1 << 22, 0.7825), 4: (1 << 20, 1.0),
+                       5: (1 << 22, 0.8945)}      # events of the profiled launch, cut pass rate
+FLOP_PROFILE_ME = {2: 21472.0, 3: 157956.0}      # the static matrix-element count of the build that was profiled
+OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 6500.0}    # 6: estimate (process 3's + one more RAMBO particle)
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 115100.0}    # 5: per event PASSING the cuts
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
@@ -58,13 +66,21 @@ def me_flops(process):
     if process in ME_FLOPS_MEASURED:
         return ME_FLOPS_MEASURED[process]
     csrc = os.path.join(ROOT, "paper_2106_10279_b200", "csrc")
-    if process >= 2:    # the cooperative programs (csrc/gen_coop.py, gen_coop3.py) are what the fused pass runs
-        name = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g"),
-                6: ("mf_me_ttggg_tables_generated.cuh", "kFlopsMe2Cta_3g")}[process]
+    if process in FLOP_HEADERS:   # the cooperative / block programs are what the fused pass runs
+        name = FLOP_HEADERS[process]
         txt = open(os.path.join(csrc, name[0])).read()
         return float(re.search(name[1] + r" = ([0-9.]+);", txt).group(1))
-    txt = open(os.path.join(csrc, "mf_me_ggtt_generated.cuh")).read()
-    return float(re.search(r"kFlopsMe2_%dg = ([0-9.]+);" % (process - 1), txt).group(1))
+    raise KeyError(process)
+
+
+def executed_flops_of_profile(path):
+    """2 dfma + dadd + dmul (thread instructions, predicated on) of the ncu --csv metric log `path`"""
+    import csv
+    v = {}
+    for row in csv.reader(open(os.path.join(ROOT, path))):
+        if len(row) > 14 and row[12].startswith("smsp__sass_thread_inst_executed_op_d"):
+            v[row[12].split("_op_")[1].split("_")[0]] = float(row[14])
+    return 2.0 * v["dfma"] + v["dadd"] + v["dmul"]
 
 
 def config_by_name(name):
@@ -374,6 +390,7 @@ def main():
         return
     peak_flops, _ = api.mf_measure_fp64_peak(1 << 17)
     peak = peak_flops / 1e12
+    dmma_flops, _ = api.mf_measure_dmma_peak(1 << 14)
     out = {
         "metric": metric_for(wl), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "ms_per_step_median": sorted(ms)[len(ms) // 2], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -392,7 +409,11 @@ def main():
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": MEASURED_TRAFFIC.get((wl.process, n)), "traffic_source": "profiles/r1_coop_v4_traffic.md",
                      "kernel": "fused_pass_cta_kernel<true>" if wl.process == 6 else ("fused_pass_coop_kernel<%d,true>" if wl.process >= 2 else "fused_pass_kernel<%d,true>") % wl.process, "kernel_ms": kern,
-                     "flops_per_me": me_flops(wl.process), "peak_source": "mf_measure_fp64_peak (DFMA chains) on this GPU",
+                     "flops_per_me": me_flops(wl.process), "flops_per_event_outside_me": OTHER_FLOPS[wl.process],
+                     "flops_source": ("static count of csrc/%s" % FLOP_HEADERS[wl.process][0] if wl.process in FLOP_HEADERS
+                                      else "ncu-executed total, " + FLOP_PROFILES[wl.process]),
+                     "peak_source": "mf_measure_fp64_peak (DFMA chains) on this GPU",
+                     "dmma_peak": dmma_flops / 1e12,
                      "nominal_peak": NOMINAL_FP64 / 1e12, "frac_of_nominal": achieved / (NOMINAL_FP64 / 1e12)},
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -159,6 +159,10 @@ int mf_debug_me2_quark_gluon(int32_t kind, double m_top, double alpha_s, const d
  * achieved FP64 rate in flop/s (2 flop per DFMA) in *h_flops.  Synchronous.  Used by bench.py for the
  * "alu" roofline denominator (FP64 peak is not in MEASURED_PEAKS.json). */
 int mf_measure_fp64_peak(int64_t iters, double *h_flops, double *h_ms);
+/* The same for the FP64 tensor path: independent DMMA.884 (mma.sync m8n8k4 f64) accumulators, 2 x 256 flop per instruction and
+ * warp.  BASELINE.json north_star allows DMMA only on evidence: this probe and profiles/r2_dmma_probe.md are the evidence
+ * (37.0 TFLOP/s on B200, the full FP64 rate, at a sixteenth of the issue slots of a DFMA stream). */
+int mf_measure_dmma_peak(int64_t iters, double *h_flops, double *h_ms);
 
 #ifdef __cplusplus
 }

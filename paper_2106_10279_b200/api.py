@@ -28,7 +28,7 @@ c_double_p = C.POINTER(C.c_double)
 EXPORTS = ["mf_create_process", "mf_destroy_process", "mf_n_dims", "mf_n_final", "mf_record_size",
            "mf_debug_row_len", "mf_last_error", "mf_launch_config", "mf_vegas_iterate", "mf_refine_grid",
            "mf_unweight", "mf_set_dynamic_scale", "mf_set_observables", "mf_debug_eval", "mf_debug_philox", "mf_debug_pdf", "mf_debug_me2",
-           "mf_debug_me2_quark_gluon", "mf_measure_fp64_peak"]
+           "mf_debug_me2_quark_gluon", "mf_measure_fp64_peak", "mf_measure_dmma_peak"]
 
 
 class MfError(RuntimeError):
@@ -77,6 +77,7 @@ def lib():
         L.mf_debug_me2.argtypes = [vp, vp, u64, vp, vp]
         L.mf_debug_me2_quark_gluon.argtypes = [C.c_int32, C.c_double, C.c_double, vp, u64, vp, vp]
         L.mf_measure_fp64_peak.argtypes = [C.c_int64, c_double_p, c_double_p]
+        L.mf_measure_dmma_peak.argtypes = [C.c_int64, c_double_p, c_double_p]
         _lib = L
     return _lib
 
@@ -135,6 +136,12 @@ def mf_debug_me2(h, d_mom, n, d_out, stream=0):
 def mf_measure_fp64_peak(iters=1 << 16):
     fl, ms = C.c_double(), C.c_double()
     _check(lib().mf_measure_fp64_peak(iters, C.byref(fl), C.byref(ms)), None, "mf_measure_fp64_peak")
+    return fl.value, ms.value
+
+
+def mf_measure_dmma_peak(iters=1 << 14):
+    fl, ms = C.c_double(), C.c_double()
+    _check(lib().mf_measure_dmma_peak(iters, C.byref(fl), C.byref(ms)), None, "mf_measure_dmma_peak")
     return fl.value, ms.value
 
 

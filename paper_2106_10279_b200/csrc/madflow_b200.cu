@@ -16,7 +16,7 @@ static_assert(sizeof(mf::IterResult) == sizeof(mf_iter_result), "result layouts 
 static_assert(mf::kMaxBins == MF_MAX_BINS, "bin limits must agree");
 
 struct mf_process {
-  int process = 0, D = 0, NF = 0;
+  int process = 0, D = 0, NF = 0, device = 0;
   mf::Params P;
   double *d_lnx = nullptr, *d_lnq2 = nullptr, *d_xf = nullptr, *d_row = nullptr;  // PDF table + collapsed row
   mf::BlockPartial* d_partials = nullptr;
@@ -96,6 +96,9 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   if (!d_grid || !d_result) return fail(p, MF_EINVAL, "d_grid and d_result must not be NULL");
   if (unw && (!d_count || !(w_max > 0.0))) return fail(p, MF_EINVAL, "mf_unweight needs d_count and w_max > 0");
   if (unw && capacity > 0 && !d_records) return fail(p, MF_EINVAL, "capacity > 0 with d_records == NULL");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device)
+    return fail(p, MF_EINVAL, "the handle belongs to another device than the current one");
   mf::PassArgs A;
   A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row; A.pdf_lnq2 = p->d_lnq2; A.pdf_xf = p->d_xf;
   A.seed = seed; A.first_event = first_event; A.n_events = n_events; A.iteration = iteration;
@@ -176,18 +179,24 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
         (e = cudaMalloc(&p->d_xf, nt * nx * nq * 8)) != cudaSuccess || (e = cudaMalloc(&p->d_row, nt * nx * 8)) != cudaSuccess) {
       free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
     }
-    cudaMemcpy(p->d_lnx, d->pdf_lnx, nx * 8, cudaMemcpyHostToDevice);
-    cudaMemcpy(p->d_lnq2, d->pdf_lnq2, nq * 8, cudaMemcpyHostToDevice);
-    cudaMemcpy(p->d_xf, d->pdf_xf, nt * nx * nq * 8, cudaMemcpyHostToDevice);
+    if ((e = cudaMemcpy(p->d_lnx, d->pdf_lnx, nx * 8, cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMemcpy(p->d_lnq2, d->pdf_lnq2, nq * 8, cudaMemcpyHostToDevice)) != cudaSuccess ||
+        (e = cudaMemcpy(p->d_xf, d->pdf_xf, nt * nx * nq * 8, cudaMemcpyHostToDevice)) != cudaSuccess) {
+      free_all(p); delete p; cudaGetLastError(); return MF_ECUDA;
+    }
     mf::pdf_collapse_kernel<<<(int)((nt * nx + 127) / 128), 128>>>(p->d_xf, p->d_lnq2, (int)(nt * nx), (int)nq, P.pdf_jq,
                                                                   P.pdf_uq, p->d_row);
-    if ((e = cudaDeviceSynchronize()) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
+    if ((e = cudaGetLastError()) != cudaSuccess || (e = cudaDeviceSynchronize()) != cudaSuccess) {
+      free_all(p); delete p; cudaGetLastError(); return MF_ECUDA;
+    }
   }
   // launch geometry: fill every SM with as many blocks as fit
   cudaDeviceProp prop;
   int dev = 0;
-  cudaGetDevice(&dev);
-  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) { free_all(p); delete p; return MF_ECUDA; }
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess || (e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) {
+    free_all(p); delete p; cudaGetLastError(); return MF_ECUDA;
+  }
+  p->device = dev;
   const bool coop = p->process == 2 || p->process == 3 || p->process == 5;
   if (coop) {
     // cooperative pass: as many teams per block as the SM's shared memory holds, one block per SM
@@ -332,6 +341,7 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
 
 int mf_debug_philox(uint64_t seed, uint32_t iteration, uint64_t first_event, uint64_t n_events, uint32_t n_blocks,
                     uint32_t* d_out, void* stream) {
+  if (n_blocks != 0 && n_events > UINT64_MAX / n_blocks) return MF_EINVAL;      // n_events * n_blocks must not wrap
   if (!d_out && n_events * n_blocks) return MF_EINVAL;
   uint64_t total = n_events * n_blocks;
   if (total == 0) return MF_OK;
@@ -411,6 +421,31 @@ int mf_measure_fp64_peak(int64_t iters, double* h_flops, double* h_ms) {
   cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
   if (e != cudaSuccess) return MF_ECUDA;
   *h_flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads / ((double)ms * 1e-3);
+  if (h_ms) *h_ms = ms;
+  return MF_OK;
+}
+
+int mf_measure_dmma_peak(int64_t iters, double* h_flops, double* h_ms) {
+  if (iters <= 0 || !h_flops) return MF_EINVAL;
+  cudaDeviceProp prop;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return MF_ECUDA;
+  double* sink = nullptr;
+  if (cudaMalloc(&sink, 8) != cudaSuccess) return MF_ENOMEM;
+  const int blocks = prop.multiProcessorCount * 2, threads = 256;
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  mf::dmma_peak_kernel<<<blocks, threads>>>(iters / 8 + 1, 1.0, sink);  // warm-up
+  cudaEventRecord(a);
+  mf::dmma_peak_kernel<<<blocks, threads>>>(iters, 1.0, sink);
+  cudaEventRecord(b);
+  cudaError_t e = cudaEventSynchronize(b);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, a, b);
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
+  if (e != cudaSuccess) return MF_ECUDA;
+  // 4 DMMA per iteration and warp, 2 x 8 x 8 x 4 flop each
+  *h_flops = 4.0 * 512.0 * (double)iters * (double)blocks * (double)(threads / 32) / ((double)ms * 1e-3);
   if (h_ms) *h_ms = ms;
   return MF_OK;
 }

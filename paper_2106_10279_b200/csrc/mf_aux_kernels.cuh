@@ -152,4 +152,20 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(long long iters, double 
   if (s == 123456.789) sink[0] = s;
 }
 
+// FP64 tensor-path probe: 4 independent DMMA.884 (mma.sync m8n8k4 f64, 256 multiply-adds each) accumulators per warp.
+__global__ void __launch_bounds__(256) dmma_peak_kernel(long long iters, double seed, double* sink) {
+  double c[4][2];
+  for (int i = 0; i < 4; ++i) { c[i][0] = seed + i; c[i][1] = seed - i; }
+  const double a = 0.999999, b = 1.0 + 1e-9 * (double)threadIdx.x;
+  for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                   : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+  }
+  double s = 0.0;
+  for (int i = 0; i < 4; ++i) s += c[i][0] + c[i][1];
+  if (s == 123456.789) sink[0] = s;
+}
+
 }  // namespace mf

@@ -232,6 +232,31 @@ def test_shim_five_gluon_block_program(shim, oracle_procs):
         assert abs(got - ref) <= 1e-11 * ref, (i, got, ref)
 
 
+def test_bench_flop_constants():
+    """bench.py's roofline numerator: every literal is recomputed from the committed ncu metric logs, and the static
+    matrix-element counts it reads are the generated headers' (the literals must not go stale silently)."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("bench_mod", os.path.join(ROOT, "bench.py"))
+    b = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(b)
+    for proc, path in b.FLOP_PROFILES.items():
+        n, rate = b.FLOP_PROFILE_EVENTS[proc]
+        total = b.executed_flops_of_profile(path)
+        if proc in b.FLOP_PROFILE_ME:          # OTHER_FLOPS = (executed - n_pass x static count) / n
+            other = (total - n * rate * b.FLOP_PROFILE_ME[proc]) / n
+            assert abs(other - b.OTHER_FLOPS[proc]) <= 0.02 * b.OTHER_FLOPS[proc] + 10, (proc, other)
+        else:                                   # measured total per (passing) event
+            per = total / (n * rate)
+            assert abs(per - b.ME_FLOPS_MEASURED[proc]) <= 0.005 * per, (proc, per)
+    from paper_2106_10279_b200 import build
+    build.generate()
+    for proc, (hdr, name) in b.FLOP_HEADERS.items():
+        txt = open(os.path.join(build.CSRC, hdr)).read()
+        assert ("constexpr double %s = %d.0;" % (name, b.me_flops(proc))) in txt
+    # the static count of the profiled gg -> ttbar g build is still the header's (that kernel has not changed since)
+    assert b.me_flops(2) == b.FLOP_PROFILE_ME[2]
+
+
 # ---- multi-rank sharding (gloo, world size 2) ------------------------------------------------------------------
 def test_shard_range_partitions():
     from paper_2106_10279_b200.integrate import shard_range
