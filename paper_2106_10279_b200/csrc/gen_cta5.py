@@ -177,31 +177,31 @@ def main():
       (S_UB, S_V, S_Y1, S_X1, S_Y2, S_X2, N_SPIN))
     w("constexpr int kNSeq2 = %d, kNSeq3 = %d, kNSeq4 = %d, kNSeq5 = %d, kNPerm = %d, kXmStride = %d;" %
       (len(SEQS[2]), len(SEQS[3]), len(SEQS[4]), len(SEQS[5]), len(perms), XM_STRIDE))
-    w("constexpr double kCden = %d.0;" % cden)
+    w("constexpr double kCden = %d.0;         // kColour holds 2 x numerator above the diagonal, 1 x on it: x^T C x = x^T kColour x / kCden" % cden)
     # static operation count (adds + multiplies, FMA = 2) of one matrix element
     q_flops = (2 * N * (FLOPS["slash_row"] + FLOPS["prop_row"]) + 4 * N * (FLOPS["slash_col"] + FLOPS["prop_col"]) +
                80 * (FLOPS["slash_row"] + 50 + FLOPS["prop_row"] + 4) + 160 * (FLOPS["slash_col"] + 50 + FLOPS["prop_col"] + 4))
     amp_flops = len(perms) * 32 * (9 * (48 + 4) + 6 * 32)
-    col_flops = 2 * (2 * 120 * 120 * 64 + 2 * 120 * 64)
+    col_flops = 2 * (2 * 8 * 8 * 4 * 8 * 240 + 2 * 120 * 64)        # 240 (row tile, k-step) pairs x 8 column tiles per half
     s0_flops = 31 * 40 + 200
     total = s0_flops + gl_flops + q_flops + amp_flops + col_flops
     w("// static fp64 operation count per matrix element: S0 %d + gluon currents %d + quark currents %d + amplitudes %d +" %
       (s0_flops, gl_flops, q_flops, amp_flops))
-    w("// colour contraction (DMMA, 2 x 120 x 120 x 64 multiply-adds x 2) %d" % col_flops)
+    w("// colour contraction (DMMA on the upper triangle: 2 halves x 240 x 8 instructions of 512 flop) %d" % col_flops)
     w("constexpr double kFlopsMe2Cta_3g = %d.0;" % total)
     w("")
     w("// canonical gluon sequences of length k = 2..5 (row k - 2): mask, output base, offset into kSplit, n3 | n4 << 8")
-    w("MF_TABLE short kSeqDesc[4][%d][4] = {" % len(SEQS[5]))
+    w("MF_CTABLE short kSeqDesc[4][%d][4] = {" % len(SEQS[5]))
     for k in range(2, N + 1):
         rows = desc[k] + [[0, 0, 0, 0]] * (len(SEQS[5]) - len(desc[k]))
         w("  {" + ", ".join("{%d, %d, %d, %d}" % tuple(r) for r in rows) + "},")
     w("};")
     w("// V3 splits [bL, mL, bR, mR, sign] then V4 splits [bA, mA, bB, mB, bC, mC, sign] of every sequence")
-    w("MF_TABLE short kSplit[%d] = {" % len(split))
+    w("MF_CTABLE short kSplit[%d] = {" % len(split))
     o.extend(fmt_rows(split))
     w("};")
     w("// per ordering: nine blocks (base, mask, sign), entry (j - 3) * 3 + (i - 1) = sigma[i..j]; then sigma")
-    w("MF_TABLE short kAmp[%d][32] = {" % len(amp))
+    w("MF_CTABLE short kAmp[%d][32] = {" % len(amp))
     for r in amp:
         w("  {" + ", ".join("%d" % v for v in r) + "},")
     w("};")
@@ -219,9 +219,12 @@ def main():
     for a in LABELS:
         w("  {" + ", ".join("%d" % (SEQ_INDEX[2][(min(a, b), max(a, b))] if a != b else 0) for b in LABELS) + "},")
     w("};")
-    w("// colour matrix numerators (denominator kCden), orderings in lexicographic order")
+    w("// colour matrix (orderings in lexicographic order), UPPER triangle, numerators over kCden:")
+    w("// (off-diagonal entries doubled, so x^T C x = x^T kColour x), and row tile m of the DMMA contraction only needs the columns >= 8 m")
+    cup = np.triu(2 * cnum, 1) + np.diag(np.diag(cnum))          # doubled: the halved diagonal stays an integer
+    assert (cup + cup.T == 2 * cnum).all()
     w("MF_TABLE double kColour[%d] = {" % (len(perms) ** 2))
-    flat = [int(v) for v in cnum.reshape(-1)]
+    flat = [int(v) for v in cup.reshape(-1)]
     for i in range(0, len(flat), 30):
         w("  " + ", ".join("%d." % v for v in flat[i:i + 30]) + ",")
     w("};")

@@ -61,7 +61,7 @@ template <int PROC>
 cudaError_t coop_setup(mf_process* p, const cudaDeviceProp& prop) {
   typedef typename mf::CoopOf<PROC>::PG PG;
   const mf::Params& P = p->P;
-  const int group = PG::Team == 32 ? 1 : mf::kCoopGroup;      // teams run in lock-step groups
+  const int group = PG::Team == 32 ? mf::kCoopGroupWarp : mf::kCoopGroup;      // teams run in lock-step groups
   int n_teams = mf::CoopOf<PROC>::MaxTeams;
   while (n_teams > 0 &&
          (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, P.pdf_nx * P.pdf_nfl, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)

@@ -74,7 +74,11 @@ __device__ __forceinline__ void coop_load_table(uint4* s_tab) {
 #ifndef MF_COOP_INTERLEAVE
 #define MF_COOP_INTERLEAVE 0
 #endif
-constexpr int kCoopGroup = MF_COOP_GROUP;
+#ifndef MF_COOP_GROUP_WARP
+#define MF_COOP_GROUP_WARP 1
+#endif
+constexpr int kCoopGroup = MF_COOP_GROUP;            // teams of two warps (g g -> t tbar g g)
+constexpr int kCoopGroupWarp = MF_COOP_GROUP_WARP;   // teams of one warp (g g -> t tbar g, pp -> t tbar j)
 template <int THREADS>
 __device__ __forceinline__ void coop_group_sync(int group) {
   if (THREADS == 32) __syncwarp();
@@ -173,7 +177,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
     fused_pass_coop_kernel(const Params P, const PassArgs A) {
   typedef typename CoopOf<PROC>::PG PG;
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
-  constexpr int G = PG::Team == 32 ? 1 : kCoopGroup;
+  constexpr int G = PG::Team == 32 ? kCoopGroupWarp : kCoopGroup;
   extern __shared__ double2 smem2[];
   double* smem = reinterpret_cast<double*>(smem2);
   const int nb = P.n_bins, nx = P.pdf_nx, nrow = PROC == 5 ? nx * P.pdf_nfl : nx;

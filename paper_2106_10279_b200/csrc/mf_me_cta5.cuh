@@ -23,6 +23,13 @@
 #endif
 #endif
 
+// tables every lane of a (half) warp reads at the same index: constant memory on the device
+#if defined(__CUDA_ARCH__)
+#define MF_CTABLE static __constant__ const
+#else
+#define MF_CTABLE static const
+#endif
+
 namespace mf { namespace g5 {
 
 #include "mf_me_ttggg_tables_generated.cuh"
@@ -35,27 +42,29 @@ constexpr int kScratchDoubles = kOffXm + kNPerm * kXmStride;
 constexpr int kStage0Items = 38, kStage1Items = 4 * kNSeq2 + 10 + 20, kStage2Items = 8 * kNSeq3 + 80 + 160;
 constexpr int kStage3Items = 16 * kNSeq4, kStage4Items = 32 * kNSeq5, kAmpItems = 16 * kNPerm;
 
+// VEC items as two planes of double2 (components (0, 1) | (2, 3)), SPIN items as four planes of (re, im): lanes that
+// touch consecutive items issue conflict-free 128-bit accesses
 MF_HD rvec ld_vec(const double* S, int i) {
-  const double2* q = reinterpret_cast<const double2*>(S + 4 * i);
-  const double2 a = q[0], b = q[1];
+  const double2* q = reinterpret_cast<const double2*>(S);
+  const double2 a = q[i], b = q[kNVec + i];
   return rvec{{a.x, a.y, b.x, b.y}};
 }
 MF_HD void st_vec(double* S, int i, const rvec& r) {
-  double2* q = reinterpret_cast<double2*>(S + 4 * i);
-  q[0] = make_double2(r.v[0], r.v[1]);
-  q[1] = make_double2(r.v[2], r.v[3]);
+  double2* q = reinterpret_cast<double2*>(S);
+  q[i] = make_double2(r.v[0], r.v[1]);
+  q[kNVec + i] = make_double2(r.v[2], r.v[3]);
 }
 MF_HD spin ld_spin(const double* S, int i) {
-  const double2* q = reinterpret_cast<const double2*>(S + kOffSpin + 8 * i);
+  const double2* q = reinterpret_cast<const double2*>(S + kOffSpin);
   spin r;
 #pragma unroll
-  for (int c = 0; c < 4; ++c) { const double2 t = q[c]; r.re[c] = t.x; r.im[c] = t.y; }
+  for (int c = 0; c < 4; ++c) { const double2 t = q[c * kNSpin + i]; r.re[c] = t.x; r.im[c] = t.y; }
   return r;
 }
 MF_HD void st_spin(double* S, int i, const spin& r) {
-  double2* q = reinterpret_cast<double2*>(S + kOffSpin + 8 * i);
+  double2* q = reinterpret_cast<double2*>(S + kOffSpin);
 #pragma unroll
-  for (int c = 0; c < 4; ++c) q[c] = make_double2(r.re[c], r.im[c]);
+  for (int c = 0; c < 4; ++c) q[c * kNSpin + i] = make_double2(r.re[c], r.im[c]);
 }
 MF_HD rvec rsigned(const rvec& a, int sgn) { return sgn < 0 ? rvec{{-a.v[0], -a.v[1], -a.v[2], -a.v[3]}} : a; }
 // Jhat of the sub-sequence (base, mask) for the polarisation word pw
@@ -212,47 +221,55 @@ MF_HD double colour_rows_plain(const double* S, int tid, int nthreads) {
   for (int s = tid; s < kNPerm; s += nthreads)
     for (int n = 0; n < 64; ++n) {
       double y = 0.0;
-      for (int u = 0; u < kNPerm; ++u) y = fma(kColour[s * kNPerm + u], xm[u * kXmStride + n], y);
+      for (int u = s; u < kNPerm; ++u) y = fma(kColour[s * kNPerm + u], xm[u * kXmStride + n], y);
       acc = fma(xm[s * kXmStride + n], y, acc);
     }
   return acc;
 }
 #if defined(__CUDACC__)
-// Device: Y = Cnum XM (120 x 120 times 120 x 64) as DMMA.884 tiles; a warp owns the 8 rows of a row tile (15 of them) and all 8
-// column tiles (one C fragment per k-step, reused for the 8 column tiles), then multiplies its Y fragments with the XM
-// entries at the same positions.  The colour matrix is read from global memory (115 kB, the same for every block: L2).
+// Device: Y = kColour XM (upper triangle of 120 x 120 times 120 x 64) as DMMA.884 tiles: row tile m (8 orderings) needs the
+// k-steps 2 m .. 29 only; the 15 row tiles are paired {p, 14 - p} (32 k-steps per pair) and split over the two halves of
+// the 64 columns: 16 equal tasks for 16 warps.  One C fragment per k-step is reused for 4 column tiles; the warp then
+// multiplies its Y fragments with the XM entries at the same positions.  The colour matrix is read from global memory
+// (115 kB, the same for every block: L2).
 __device__ __forceinline__ double colour_half_dmma(const double* S, int warp, int n_warps, int lane) {
   const double* xm = S + kOffXm;
   const int g = lane >> 2, t = lane & 3;
   double acc = 0.0;
+  // task = (pair of row tiles {p, 14 - p}: 30 - 2 p and 2 + 2 p k-steps = 32 in all; tile 7 alone: 16) x half of the columns
 #pragma unroll 1
-  for (int mt = warp; mt < kNPerm / 8; mt += n_warps) {
-    double c[8][2];
+  for (int task = warp; task < 16; task += n_warps) {
+    const int p = task >> 1, nh = task & 1;
+#pragma unroll 1
+    for (int which = 0; which < (p == 7 ? 1 : 2); ++which) {
+      const int mt = which == 0 ? p : 14 - p;
+      double c[4][2];
 #pragma unroll
-    for (int n = 0; n < 8; ++n) c[n][0] = c[n][1] = 0.0;
-    const double* crow = kColour + (8 * mt + g) * kNPerm + t;
-    const double* xcol = xm + t * kXmStride + g;
-#pragma unroll 2
-    for (int ks = 0; ks < kNPerm / 4; ++ks) {
-      const double a = crow[4 * ks];
-      const double* xr = xcol + 4 * ks * kXmStride;
+      for (int n = 0; n < 4; ++n) c[n][0] = c[n][1] = 0.0;
+      const double* crow = kColour + (8 * mt + g) * kNPerm + t;
+      const double* xcol = xm + t * kXmStride + g + 32 * nh;
+#pragma unroll 4
+      for (int ks = 2 * mt; ks < kNPerm / 4; ++ks) {
+        const double a = crow[4 * ks];
+        const double* xr = xcol + 4 * ks * kXmStride;
 #pragma unroll
-      for (int n = 0; n < 8; ++n) {
-        const double b = xr[8 * n];
+        for (int n = 0; n < 4; ++n) {
+          const double b = xr[8 * n];
 #if defined(__CUDA_ARCH__)
-        asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
-            : "+d"(c[n][0]), "+d"(c[n][1]) : "d"(a), "d"(b));
+          asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+              : "+d"(c[n][0]), "+d"(c[n][1]) : "d"(a), "d"(b));
 #else
-        (void)a; (void)b;      // host pass of nvcc: never executed
+          (void)a; (void)b;      // host pass of nvcc: never executed
 #endif
+        }
       }
-    }
-    const double* xo = xm + (8 * mt + g) * kXmStride + 2 * t;
+      const double* xo = xm + (8 * mt + g) * kXmStride + 2 * t + 32 * nh;
 #pragma unroll
-    for (int n = 0; n < 8; ++n) {
-      const double2 x = *reinterpret_cast<const double2*>(xo + 8 * n);
-      acc = fma(x.x, c[n][0], acc);
-      acc = fma(x.y, c[n][1], acc);
+      for (int n = 0; n < 4; ++n) {
+        const double2 x = *reinterpret_cast<const double2*>(xo + 8 * n);
+        acc = fma(x.x, c[n][0], acc);
+        acc = fma(x.y, c[n][1], acc);
+      }
     }
   }
   return acc;
