@@ -43,18 +43,21 @@ UNIT = "events/s"
 #    read from the generated headers at run time (FLOP_HEADERS; a DMMA.884 counts its 2 x 256 flop); the rest of the chain
 #    (a1-a6, a10-a14 incl. the software sqrt / div / log / sincos sequences and the owner-side wavefunctions) is OTHER_FLOPS,
 #    calibrated by ncu: executed (2 dfma + dadd + dmul) of one launch minus n_pass x the static count (FLOP_PROFILES).
-#  * thread-per-event kernels (0, 1, 4) and pp -> ttbar j (5): the compiler folds constants into the matrix element, so the
-#    static count overestimates: the ncu-executed TOTAL per event (per passing event for 5) is used (ME_FLOPS_MEASURED).
+#  * thread-per-event kernels (0, 1, 4), pp -> ttbar j (5) and g g -> ttbar ggg (6): the ncu-executed TOTAL per event (per
+#    passing event for 5 and 6; for 6 plus its 3840 DMMA x 512 flop) is used (ME_FLOPS_MEASURED): for 0, 1, 4 the compiler
+#    folds constants into the matrix element, so the static count overestimates; for 6 the generator's static count
+#    (5.89 M) misses 7 % of the executed operations (sign and scale multiplications).
 # tests/test_host_logic.py::test_bench_flop_constants recomputes every literal below from the committed ncu csv files.
-FLOP_HEADERS = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g"),
-                6: ("mf_me_ttggg_tables_generated.cuh", "kFlopsMe2Cta_3g")}
+FLOP_HEADERS = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g")}
 FLOP_PROFILES = {0: "profiles/r1_flops_C0.csv", 1: "profiles/r1_flops_C1.csv", 2: "profiles/r1_flops_C2.csv",
-                 3: "profiles/r1_flops_C3.csv", 4: "profiles/r1_flops_C5.csv", 5: "profiles/r1_flops_C6.csv"}
+                 3: "profiles/r1_flops_C3.csv", 4: "profiles/r1_flops_C5.csv", 5: "profiles/r1_flops_C6.csv",
+                 6: "profiles/r2_flops_C7.csv"}
 FLOP_PROFILE_EVENTS = {0: (1_000_000, 1.0), 1: (1 << 20, 1.0), 2: (1 << 22, 0.8934), 3: (1 << 22, 0.7825), 4: (1 << 20, 1.0),
-                       5: (1 << 22, 0.8945)}      # events of the profiled launch, cut pass rate
+                       5: (1 << 22, 0.8945), 6: (1 << 18, 0.653)}      # events of the profiled launch, cut pass rate
+FLOP_PROFILE_DMMA = {6: 3840 * 512.0}            # flop per matrix element on the tensor path (not seen by the op_dfma counter)
 FLOP_PROFILE_ME = {2: 21472.0, 3: 157956.0}      # the static matrix-element count of the build that was profiled
-OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 6500.0}    # 6: estimate (process 3's + one more RAMBO particle)
-ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 115100.0}    # 5: per event PASSING the cuts
+OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 0.0}
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 115100.0, 6: 6.31e6}    # 5, 6: per event PASSING the cuts
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
@@ -410,7 +413,7 @@ def main():
                      "traffic": MEASURED_TRAFFIC.get((wl.process, n)), "traffic_source": "profiles/r1_coop_v4_traffic.md",
                      "kernel": "fused_pass_cta_kernel<true>" if wl.process == 6 else ("fused_pass_coop_kernel<%d,true>" if wl.process >= 2 else "fused_pass_kernel<%d,true>") % wl.process, "kernel_ms": kern,
                      "flops_per_me": me_flops(wl.process), "flops_per_event_outside_me": OTHER_FLOPS[wl.process],
-                     "flops_source": ("static count of csrc/%s" % FLOP_HEADERS[wl.process][0] if wl.process in FLOP_HEADERS
+                     "flops_source": ("static count of csrc/%s" % FLOP_HEADERS[wl.process][0] if wl.process in FLOP_HEADERS and wl.process not in ME_FLOPS_MEASURED
                                       else "ncu-executed total, " + FLOP_PROFILES[wl.process]),
                      "peak_source": "mf_measure_fp64_peak (DFMA chains) on this GPU",
                      "dmma_peak": dmma_flops / 1e12,

@@ -245,8 +245,8 @@ def test_bench_flop_constants():
         if proc in b.FLOP_PROFILE_ME:          # OTHER_FLOPS = (executed - n_pass x static count) / n
             other = (total - n * rate * b.FLOP_PROFILE_ME[proc]) / n
             assert abs(other - b.OTHER_FLOPS[proc]) <= 0.02 * b.OTHER_FLOPS[proc] + 10, (proc, other)
-        else:                                   # measured total per (passing) event
-            per = total / (n * rate)
+        else:                                   # measured total per (passing) event (+ the DMMA flop ncu's op counters miss)
+            per = total / (n * rate) + b.FLOP_PROFILE_DMMA.get(proc, 0.0)
             assert abs(per - b.ME_FLOPS_MEASURED[proc]) <= 0.005 * per, (proc, per)
     from paper_2106_10279_b200 import build
     build.generate()
