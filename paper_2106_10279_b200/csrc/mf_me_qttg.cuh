@@ -29,6 +29,25 @@ MF_HD spin spin_add_scaled(const spin& a, double m, const spin& c) {   // a + m 
 }
 MF_HD double re_conj_mul(const cplx& a, const cplx& b) { return a.re * b.re + a.im * b.im; }   // Re(conj(a) b)
 
+// Massless quark: the chirality-c part (c = 0: left, components 0-1; c = 1: right, components 2-3) of u(p) resp. v(p),
+// normalised to psi^dagger psi = 2 E: a helicity eigenstate.  A vector current (an odd number of gamma matrices between
+// row and column) connects equal chiralities only, so the light line has TWO spin states that contribute, not four
+// (the spin-summed |M|^2 does not depend on the basis).  The z-axis spin state that is projected is the one with the
+// larger component along the wanted helicity (no 0/0 for momenta along the z axis: the beams).
+MF_HD spin chiral_col(const double p[4], int c, bool is_v) {
+  const bool up = (c == 0) == (p[3] <= 0.0);          // left part: |(E - p.sigma) xi|^2 = E -+ pz for xi = (1,0) / (0,1)
+  spin u = is_v ? v_col(p, 0.0, up ? 0 : 1) : u_col(p, 0.0, up ? 0 : 1);
+  const double n2 = p[0] + ((c == 0) == up ? -p[3] : p[3]);
+  const double n = sqrt(2.0 * p[0] / n2);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const bool keep = (k >> 1) == c;
+    u.re[k] = keep ? n * u.re[k] : 0.0;
+    u.im[k] = keep ? n * u.im[k] : 0.0;
+  }
+  return u;
+}
+
 MF_HD double me2_light_line_ttg(int kind, const double p1[4], const double prow[4], const double p3[4],
                                 const double p4[4], const double pg[4], double mt, double g2) {
   const double sr = kind == 0 ? -1.0 : 1.0, sk = kind == 0 ? 1.0 : -1.0;
@@ -72,9 +91,9 @@ MF_HD double me2_light_line_ttg(int kind, const double p1[4], const double prow[
       }
     const double k12e = rdot(k12, e);
 #pragma unroll 1
-    for (int i = 0; i < 4; ++i) {
-      const spin col = u_col(p1, 0.0, i >> 1);
-      const spin row = kind == 0 ? bar_of(v_col(prow, 0.0, i & 1)) : ubar_row(prow, 0.0, i & 1);
+    for (int i = 0; i < 2; ++i) {          // the two chiralities of the massless light line
+      const spin col = chiral_col(p1, i, false);
+      const spin row = bar_of(chiral_col(prow, i, kind == 0));
       const cvec jl = bilinear(row, col);
       const cvec jlA = bilinear(row, slash_col(a1, slash_col(e, col)));
       const cvec jlB = bilinear(slash_row(slash_row(row, e), a2), col);
