@@ -124,6 +124,12 @@ class LheDrain:
         assert self.dtype.itemsize == proc.record_size
         self.side = torch.cuda.Stream()
         self.jobs = queue.Queue()
+        # pinned staging buffers are allocated once and reused (cudaHostAlloc is slow and synchronising): the count, and a
+        # ring of two record buffers that grow to the largest batch seen
+        self._h_count = torch.empty(1, dtype=torch.int64).pin_memory()
+        self._ring = [None, None]
+        self._ring_free = [None, None]       # threading.Event: the writer thread has consumed the buffer
+        self._turn = 0
         self.body_path = path + ".body"
         self.n_written = 0
         self.sum_w = 0.0
@@ -138,7 +144,7 @@ class LheDrain:
         main = torch.cuda.current_stream() if stream is None else stream
         ready = torch.cuda.Event()
         ready.record(main)
-        h_count = torch.empty(1, dtype=torch.int64).pin_memory()
+        h_count = self._h_count
         with torch.cuda.stream(self.side):
             self.side.wait_event(ready)
             h_count.copy_(count, non_blocking=True)
@@ -147,14 +153,22 @@ class LheDrain:
         got_count.synchronize()                  # 8 bytes: the size of the next copy depends on it
         n = min(int(h_count.item()), capacity)
         nbytes = n * self.proc.record_size
-        h_rec = torch.empty(max(nbytes, 1), dtype=torch.uint8).pin_memory()
+        slot = self._turn
+        self._turn ^= 1
+        if self._ring_free[slot] is not None:
+            self._ring_free[slot].wait()                      # the writer thread is done with this buffer
+        if self._ring[slot] is None or self._ring[slot].numel() < max(nbytes, 1):
+            self._ring[slot] = torch.empty(max(nbytes, 1 << 20), dtype=torch.uint8).pin_memory()
+        h_rec = self._ring[slot]
+        free = threading.Event()
+        self._ring_free[slot] = free
         done = torch.cuda.Event()
         with torch.cuda.stream(self.side):
             if nbytes:
                 h_rec[:nbytes].copy_(records[:nbytes], non_blocking=True)
             done.record(self.side)
         main.wait_event(done)                    # the buffer may be overwritten once the copy has run
-        self.jobs.put((h_rec, n, done, float(w_max)))
+        self.jobs.put((h_rec, n, done, float(w_max), free))
         return n
 
     # -- writer thread ---------------------------------------------------------------------------------------------
@@ -166,9 +180,10 @@ class LheDrain:
                     job = self.jobs.get()
                     if job is None:
                         break
-                    h_rec, n, done, w_max = job
+                    h_rec, n, done, w_max, free = job
                     done.synchronize()
-                    rec = np.frombuffer(h_rec.numpy()[:n * self.dtype.itemsize].tobytes(), dtype=self.dtype)
+                    rec = np.frombuffer(h_rec.numpy()[:n * self.dtype.itemsize].tobytes(), dtype=self.dtype)   # a copy
+                    free.set()                                # the staging buffer may be reused
                     rec = rec[np.argsort(rec["id"], kind="stable")]          # device order is unspecified
                     wl = self.wl
                     f.write(format_events(rec, wl.process, wl.m_top, np.sqrt(wl.mu2) if wl.process else wl.sqrt_s,
@@ -191,7 +206,8 @@ class LheDrain:
             f.write('<LesHouchesEvents version="3.0">\n<header>\n<!--\n')
             f.write("madflow-b200: %s, %d unweighted events (hit-or-miss against the running maximum weight)\n" %
                     (wl.name, self.n_written))
-            f.write("colour flow: ONE fixed planar flow per partonic channel (the event weights are colour summed)\n-->\n</header>\n")
+            f.write("colour flow: ONE fixed planar flow per partonic channel (the event weights are colour summed)\n")
+            f.write("weights: IDWTUP = 3 with XWGTUP = sign(w); events with |w| > w_max (overweight) carry XWGTUP = sign(w) |w| / w_max > 1\n-->\n</header>\n")
             f.write("<init>\n%d %d %.8e %.8e 0 0 0 0 3 1\n%.10e %.10e 1.0 1\n</init>\n" %
                     (beam[0], beam[1], wl.sqrt_s / 2, wl.sqrt_s / 2, xsec_pb, xerr_pb))
             with opener(self.body_path, "r") as b:

@@ -187,3 +187,48 @@ def test_run_config_on_a_side_stream(gpu_procs):
             assert abs(u - v) <= 1e-11 * abs(u)
     assert a.iterations[0].sum_w == b.iterations[0].sum_w          # same grid in: bit-identical sums
     assert torch.allclose(a.grid, b.grid, rtol=0, atol=1e-12)
+
+
+_NCCL_WORKER = r"""
+import os, sys
+sys.path.insert(0, os.environ["MF_ROOT"])
+import torch, torch.distributed as dist
+from paper_2106_10279_b200 import api, integrate, workloads as W
+rank = int(os.environ["RANK"])
+torch.cuda.set_device(rank)
+dist.init_process_group("nccl", device_id=torch.device("cuda", rank))
+wl = W.C1.scaled(40001, 4, 3)
+gp = api.Process(wl, W.pdf_table())
+run = integrate.run_config(gp, wl, rank=rank, world=dist.get_world_size())
+if rank == 0:
+    ref = integrate.run_config(gp, wl)          # the same events on one rank
+    for a, b in zip(run.iterations, ref.iterations):
+        assert a.n_pass == b.n_pass and a.n_events == b.n_events
+        assert abs(a.sum_w - b.sum_w) <= 1e-11 * abs(b.sum_w) and abs(a.sum_w2 - b.sum_w2) <= 1e-11 * b.sum_w2
+        assert a.max_abs_w == b.max_abs_w or abs(a.max_abs_w - b.max_abs_w) <= 1e-9 * b.max_abs_w
+    assert torch.allclose(run.grid, ref.grid, rtol=0, atol=1e-10)
+# every rank refined identically
+g = [torch.empty_like(run.grid) for _ in range(dist.get_world_size())]
+dist.all_gather(g, run.grid)
+assert all(torch.equal(g[0], x) for x in g)
+dist.destroy_process_group()
+"""
+
+
+def test_run_config_sharded_over_two_gpus_nccl(tmp_path):
+    """events sharded by index range over two ranks, ONE exchange per iteration over NCCL; the combined sums
+    are the single-rank sums and every rank refines the same grid.  Needs two GPUs (this pool has one per box: skipped)."""
+    import os
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    script = tmp_path / "worker.py"
+    script.write_text(_NCCL_WORKER)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, MF_ROOT=root)
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
+                        "127.0.0.1", "--master-port", "29631", str(script)], env=env, stdout=subprocess.PIPE,
+                       stderr=subprocess.STDOUT, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-3000:]
