@@ -58,18 +58,13 @@ MF_ME_CALL double me2_pp_call(const Params& P, double shat, const double (*k)[4]
   return matrix_element<4>(P, shat, k);
 }
 
-// process 5: |M|^2 of quark-channel class c (0 q qbar, 1 qbar q, 2 q g, 3 g q, 4 qbar g, 5 g qbar; first parton from
-// beam 1) at the CM-frame point; the antiquark-gluon classes by charge conjugation (t <-> tbar) of the quark-gluon ones.
-// Inlined ONCE, inside the caller's rolled loop over c (the arguments are selected at run time).
-MF_D double quark_gluon_me2(const Params& P, double shat, const double (*k)[4], int c) {
+// process 5: |M|^2 of the six quark-channel classes (0 q qbar, 1 qbar q, 2 q g, 3 g q, 4 qbar g, 5 g qbar; first parton from
+// beam 1) at the CM-frame point, in one call that shares the top line's currents between the classes with the same gluon
+// (mf_me_qttg.cuh).  Out of line: one copy per kernel.
+__device__ __noinline__ void quark_gluon_me2_all(const Params& P, double shat, const double (*k)[4], double M[6]) {
   const double E = 0.5 * sqrt(shat);
-  const double pa[4] = {E, 0.0, 0.0, (c & 1) ? -E : E};     // the beam the (anti)quark comes from
-  const double pb[4] = {E, 0.0, 0.0, (c & 1) ? E : -E};     // the other beam
-  const double* prow = c < 2 ? pb : k[2];
-  const double* pg = c < 2 ? k[2] : pb;
-  const double* p3 = c < 4 ? k[0] : k[1];
-  const double* p4 = c < 4 ? k[1] : k[0];
-  return me2_light_line_ttg(c < 2 ? 0 : 1, pa, prow, p3, p4, pg, P.m_top, 4.0 * kPi * P.alpha_s);
+  const double b1[4] = {E, 0.0, 0.0, E}, b2[4] = {E, 0.0, 0.0, -E};
+  me2_ttj_quark_classes(b1, b2, k[0], k[1], k[2], P.m_top, 4.0 * kPi * P.alpha_s, M);
 }
 
 // Luminosity (step a6): F(x1) F(x2) / (x1 x2) with F the interpolant of the collapsed row in shared memory; and
@@ -179,11 +174,13 @@ MF_D double pp_ttj_terms(const Params& P, const PassArgs& A, const double* s_lnx
   const double inv = 1.0 / (ev.x1 * ev.x2);
   const double l0 = D12 * inv, l1 = D21 * inv, l2 = Q1 * f2[0] * inv, l3 = f1[0] * Q2 * inv, l4 = Qb1 * f2[0] * inv,
                l5 = f1[0] * Qb2 * inv;
+  double M[6];
+  quark_gluon_me2_all(P, ev.shat, ev.k, M);
   double sum = 0.0;
-#pragma unroll 1
+#pragma unroll
   for (int c = 0; c < 6; ++c) {
     const double lc = c == 0 ? l0 : c == 1 ? l1 : c == 2 ? l2 : c == 3 ? l3 : c == 4 ? l4 : l5;
-    const double term = lc * (quark_gluon_me2(P, ev.shat, ev.k, c) * asf);
+    const double term = lc * (M[c] * asf);
     if (terms) terms[c] = term;
     sum += term;
   }
@@ -299,8 +296,9 @@ __device__ __forceinline__ unsigned pp_ttj_channel(const Params& P, const PassAr
   const int nf = (P.pdf_nfl - 1) / 2;
   const double inv = 1.0 / (ev.x1 * ev.x2);
   double M[6];
-#pragma unroll 1
-  for (int c = 0; c < 6; ++c) M[c] = quark_gluon_me2(P, ev.shat, ev.k, c) * asf;
+  quark_gluon_me2_all(P, ev.shat, ev.k, M);
+#pragma unroll
+  for (int c = 0; c < 6; ++c) M[c] *= asf;
   auto sterm = [&](int i, int c) {
     const double q1 = f1[1 + 2 * i], qb1 = f1[2 + 2 * i], q2 = f2[1 + 2 * i], qb2 = f2[2 + 2 * i];
     const double l = c == 0 ? q1 * qb2 : c == 1 ? qb1 * q2 : c == 2 ? q1 * f2[0] : c == 3 ? f1[0] * q2 : c == 4 ? qb1 * f2[0] : f1[0] * qb2;

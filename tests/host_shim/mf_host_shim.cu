@@ -89,6 +89,11 @@ double mfh_me2_light_line_ttg(int kind, const double* mom, double m_top, double 
   return me2_light_line_ttg(kind, mom, prow, mom + 8, mom + 12, pg, m_top, 4.0 * kPi * alpha_s);
 }
 
+// all six classes at one CM-frame point: mom = b1, b2, t, tbar, parton (mf_me_qttg.cuh: shared top-line currents)
+void mfh_me2_ttj_quark_classes(const double* mom, double m_top, double alpha_s, double out[6]) {
+  me2_ttj_quark_classes(mom, mom + 4, mom + 8, mom + 12, mom + 16, m_top, 4.0 * kPi * alpha_s, out);
+}
+
 void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {
   U4 r = philox_block(seed, iteration, event, block);
   out[0] = r.x; out[1] = r.y; out[2] = r.z; out[3] = r.w;

@@ -94,6 +94,7 @@ def shim():
     L.mfh_philox.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint32)]
     L.mfh_uniform52.restype = C.c_double
     L.mfh_uniform52.argtypes = [C.c_uint32, C.c_uint32]
+    L.mfh_me2_ttj_quark_classes.argtypes = [dp, C.c_double, C.c_double, dp]
     L.mfh_me2_light_line_ttg.restype = C.c_double
     L.mfh_me2_light_line_ttg.argtypes = [C.c_int, dp, C.c_double, C.c_double]
     for f in (L.mfh_pdf_2d, L.mfh_pdf_row, L.mfh_pdf_row_weights):
@@ -154,6 +155,24 @@ def test_shim_quark_gluon_channel_me(shim, kind):
         g = shim.mfh_me2_light_line_ttg(kind, mom.ctypes.data_as(dp), mt, W.C2.alpha_s)
         o = mfo.me2_light_line_ttbar_g(kind, mom, mt, W.C2.alpha_s)
         assert abs(g / o - 1) < 1e-10, (g, o)
+
+
+def test_shim_ttj_quark_classes_at_once(shim):
+    """the six classes with shared top-line currents and native antiquark lines against the oracle's per-class diagram sums"""
+    from oracle import mfo
+    rng = np.random.default_rng(77)
+    mt, a_s = W.C6.m_top, W.C6.alpha_s
+    for _ in range(25):
+        w = 400.0 + 4000.0 * rng.random() ** 2
+        k, _ = mfo.rambo([mt, mt, 0.0], w, rng.random(12))
+        mom = np.ascontiguousarray(np.vstack([[w / 2, 0, 0, w / 2], [w / 2, 0, 0, -w / 2], k]))
+        out = np.zeros(6)
+        shim.mfh_me2_ttj_quark_classes(mom.ctypes.data_as(dp), mt, a_s, out.ctypes.data_as(dp))
+        sw = np.ascontiguousarray(mom[[1, 0, 2, 3, 4]])
+        want = [mfo.me2_light_line_ttbar_g(0, mom, mt, a_s), mfo.me2_light_line_ttbar_g(0, sw, mt, a_s),
+                mfo.me2_light_line_ttbar_g(1, mom, mt, a_s), mfo.me2_light_line_ttbar_g(1, sw, mt, a_s),
+                mfo.me2_light_line_ttbar_g(2, mom, mt, a_s), mfo.me2_light_line_ttbar_g(2, sw, mt, a_s)]
+        np.testing.assert_allclose(out, want, rtol=1e-11)
 
 
 def test_shim_quark_channel_me(shim):
