@@ -50,14 +50,14 @@ UNIT = "events/s"
 # tests/test_host_logic.py::test_bench_flop_constants recomputes every literal below from the committed ncu csv files.
 FLOP_HEADERS = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g")}
 FLOP_PROFILES = {0: "profiles/r1_flops_C0.csv", 1: "profiles/r1_flops_C1.csv", 2: "profiles/r1_flops_C2.csv",
-                 3: "profiles/r1_flops_C3.csv", 4: "profiles/r1_flops_C5.csv", 5: "profiles/r1_flops_C6.csv",
+                 3: "profiles/r1_flops_C3.csv", 4: "profiles/r1_flops_C5.csv", 5: "profiles/r2_flops_C6.csv",
                  6: "profiles/r2_flops_C7.csv"}
 FLOP_PROFILE_EVENTS = {0: (1_000_000, 1.0), 1: (1 << 20, 1.0), 2: (1 << 22, 0.8934), 3: (1 << 22, 0.7825), 4: (1 << 20, 1.0),
                        5: (1 << 22, 0.8945), 6: (1 << 18, 0.653)}      # events of the profiled launch, cut pass rate
 FLOP_PROFILE_DMMA = {6: 3840 * 512.0}            # flop per matrix element on the tensor path (not seen by the op_dfma counter)
 FLOP_PROFILE_ME = {2: 21472.0, 3: 157956.0}      # the static matrix-element count of the build that was profiled
 OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 0.0}
-ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 115100.0, 6: 6.31e6}    # 5, 6: per event PASSING the cuts
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 74090.0, 6: 6.31e6}    # 5, 6: per event PASSING the cuts
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}

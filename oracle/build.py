@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "libmfo.so")
 SOURCES = ["mfo.cpp"]
-HEADERS = ["mfo.h", "real.hpp", "method.hpp", "amplitude.hpp"]
+HEADERS = ["mfo.h", "real.hpp", "method.hpp", "amplitude.hpp", "amplitude_qq.hpp"]
 
 
 def needs_build():

@@ -8,6 +8,7 @@
 #include <memory>
 #include <type_traits>
 #include "amplitude.hpp"
+#include "amplitude_qq.hpp"
 #include "method.hpp"
 
 using namespace mfo;
@@ -143,16 +144,23 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
   o.me2 = matrix_element<R>(P, cm, 0, -1, nullptr, nullptr) * as_factor;     // O9-O11 (x R16 factor)
   // O12: f = lum/(2 shat) |M|^2 Phi J_tau J_y K ; w = f * J_vegas
   R f = o.lum / (R(2) * shat) * o.me2 * o.phi * jac_parton * R(P.d.gev2_to_pb);
-  if (P.d.process == 4) {
+  if (P.d.process == 4 || P.d.process == 7) {
     // quark channels: for every flavour the quark may come from either beam,
     //   sum_i [ q_i(x1) qbar_i(x2) |M|^2(q along +z) + qbar_i(x1) q_i(x2) |M|^2(q along -z) ] / (x1 x2),
-    // added to the gg term at the same phase-space point.  Both are O(alpha_s^2): the same R16 factor.
-    R ma[4][4], mb[4][4];
-    for (int i = 0; i < 4; ++i)
+    // added to the gg term at the same phase-space point.  Both are of the same order in alpha_s: the same R16 factor.
+    // Process 4: q qbar -> ttbar; process 7 (R21): q qbar -> ttbar g g, the 36 diagrams of amplitude_qq.hpp.
+    R ma[6][4], mb[6][4];
+    for (int i = 0; i < n + 2; ++i)
       for (int m = 0; m < 4; ++m) { ma[i][m] = cm[i][m]; mb[i][m] = cm[i][m]; }
     for (int m = 0; m < 4; ++m) { mb[0][m] = cm[1][m]; mb[1][m] = cm[0][m]; }   // quark from beam 2
-    R Ma = me2_qq_ttbar<R>(ma, R(P.d.m_top), R(P.d.alpha_s), 0) * as_factor;
-    R Mb = me2_qq_ttbar<R>(mb, R(P.d.m_top), R(P.d.alpha_s), 0) * as_factor;
+    R Ma, Mb;
+    if (P.d.process == 4) {
+      Ma = me2_qq_ttbar<R>(ma, R(P.d.m_top), R(P.d.alpha_s), 0) * as_factor;
+      Mb = me2_qq_ttbar<R>(mb, R(P.d.m_top), R(P.d.alpha_s), 0) * as_factor;
+    } else {
+      Ma = me2_qq_ttbar_gg<R>(ma, R(P.d.m_top), R(P.d.alpha_s), 0, -1) * as_factor;
+      Mb = me2_qq_ttbar_gg<R>(mb, R(P.d.m_top), R(P.d.alpha_s), 0, -1) * as_factor;
+    }
     R La = R(0), Lb = R(0);
     for (size_t i = 0; i + 1 < P.pdfq.size(); i += 2) {
       R q1 = pdf_xf<R>(P.pdfq[i], o.x1, mu2), qb1 = pdf_xf<R>(P.pdfq[i + 1], o.x1, mu2);
@@ -227,7 +235,7 @@ int iterate(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteratio
   S sw = S(0), sw2 = S(0);
   double maxw = 0;
   uint64_t npass = 0, nacc = 0;
-  const bool has_channel = P.d.process == 4 || P.d.process == 5;
+  const bool has_channel = P.d.process == 4 || P.d.process == 5 || P.d.process == 7;
   int recsize = (P.nfinal + 2) * 32 + 16 + (has_channel ? 8 : 0);
   EventOut<R> o;
   for (uint64_t e = first; e < first + n_events; ++e) {
@@ -286,7 +294,7 @@ template <class R>
 int debug_eval(mfo_process& P, const double* grid, uint64_t seed, uint32_t iteration, uint64_t first, uint64_t n_events,
                double* out) {
   const int D = P.D, n = P.nfinal;
-  const int rowlen = 3 * D + 4 * (n + 2) + 9 + (P.d.process == 4 ? 2 : P.d.process == 5 ? 6 : 0);
+  const int rowlen = 3 * D + 4 * (n + 2) + 9 + ((P.d.process == 4 || P.d.process == 7) ? 2 : P.d.process == 5 ? 6 : 0);
   EventOut<R> o;
   for (uint64_t k = 0; k < n_events; ++k) {
     uint64_t e = first + k;
@@ -307,7 +315,7 @@ int debug_eval(mfo_process& P, const double* grid, uint64_t seed, uint32_t itera
     row[c++] = accept_draw(seed, iteration, e);
     for (int d = 0; d < D; ++d) row[c++] = o.u[d];
     for (int d = 0; d < D; ++d) row[c++] = (double)o.bin[d];
-    if (P.d.process == 4) {
+    if (P.d.process == 4 || P.d.process == 7) {
       row[c++] = r_to_double(o.lum_qq);
       row[c++] = r_to_double(o.me2_qq);
     }
@@ -366,10 +374,10 @@ extern "C" {
 
 int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
   if (!d || !out) return -1;
-  if (d->process < 0 || d->process > 6 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
+  if (d->process < 0 || d->process > 7 || d->n_bins < 2 || !(d->sqrt_s > 0)) return -1;
   std::unique_ptr<mfo_process> P(new mfo_process);
   P->d = *d;
-  static const int Dtab[7] = {2, 4, 14, 18, 4, 14, 22}, ntab[7] = {2, 2, 3, 4, 2, 3, 5}, ngtab[7] = {0, 2, 3, 4, 2, 3, 5};
+  static const int Dtab[8] = {2, 4, 14, 18, 4, 14, 22, 18}, ntab[8] = {2, 2, 3, 4, 2, 3, 5, 4}, ngtab[8] = {0, 2, 3, 4, 2, 3, 5, 4};
   P->D = Dtab[d->process];
   P->nfinal = ntab[d->process];
   P->ng = ngtab[d->process];
@@ -380,7 +388,7 @@ int mfo_create_process(const mfo_process_desc* d, mfo_process** out) {
     P->pdf.lnx.assign(d->pdf_lnx, d->pdf_lnx + d->pdf_nx);
     P->pdf.lnq2.assign(d->pdf_lnq2, d->pdf_lnq2 + d->pdf_nq);
     P->pdf.xf.assign(d->pdf_xf, d->pdf_xf + (size_t)d->pdf_nx * d->pdf_nq);
-    if (d->process == 4 || d->process == 5) {
+    if (d->process == 4 || d->process == 5 || d->process == 7) {
       if (d->pdf_nfl < 3 || d->pdf_nfl % 2 == 0) return -1;
       for (int t = 1; t < d->pdf_nfl; ++t) {
         PdfTable T = P->pdf;
@@ -411,12 +419,12 @@ int mfo_n_dims(const mfo_process* P, int32_t* D) { if (!P || !D) return -1; *D =
 int mfo_n_final(const mfo_process* P, int32_t* n) { if (!P || !n) return -1; *n = P->nfinal; return 0; }
 int mfo_record_size(const mfo_process* P, int32_t* b) {
   if (!P || !b) return -1;
-  *b = (P->nfinal + 2) * 32 + 16 + ((P->d.process == 4 || P->d.process == 5) ? 8 : 0);   // processes 4, 5 append the u64 channel code
+  *b = (P->nfinal + 2) * 32 + 16 + ((P->d.process == 4 || P->d.process == 5 || P->d.process == 7) ? 8 : 0);   // processes 4, 5, 7 append the u64 channel code
   return 0;
 }
 int mfo_debug_row_len(const mfo_process* P, int32_t* n) {
   if (!P || !n) return -1;
-  *n = 3 * P->D + 4 * (P->nfinal + 2) + 9 + (P->d.process == 4 ? 2 : P->d.process == 5 ? 6 : 0);
+  *n = 3 * P->D + 4 * (P->nfinal + 2) + 9 + ((P->d.process == 4 || P->d.process == 7) ? 2 : P->d.process == 5 ? 6 : 0);
   return 0;
 }
 
@@ -523,6 +531,29 @@ double mfo_me2_qq(const mfo_process* P, const double* mom, int basis, int prec) 
   for (int i = 0; i < 4; ++i)
     for (int c = 0; c < 4; ++c) m[i][c] = mom[4 * i + c];
   return me2_qq_ttbar<double>(m, P->d.m_top, P->d.alpha_s, basis);
+}
+double mfo_me2_qq_ttbar_gg(const double* mom, double mt, double alpha_s, int basis, int subst, int prec) {
+  if (prec == 1) {
+    long double m[6][4];
+    for (int i = 0; i < 6; ++i)
+      for (int k = 0; k < 4; ++k) m[i][k] = mom[4 * i + k];
+    return (double)me2_qq_ttbar_gg<long double>(m, mt, alpha_s, basis, subst);
+  }
+  double m[6][4];
+  for (int i = 0; i < 6; ++i)
+    for (int k = 0; k < 4; ++k) m[i][k] = mom[4 * i + k];
+  return me2_qq_ttbar_gg<double>(m, mt, alpha_s, basis, subst);
+}
+void mfo_qq_ttbar_gg_amplitude(const double* mom, double mt, double gs, const int32_t* lam, int basis, const int32_t* col,
+                               double out[4]) {
+  double m[6][4];
+  for (int i = 0; i < 6; ++i)
+    for (int k = 0; k < 4; ++k) m[i][k] = mom[4 * i + k];
+  int l[6];
+  for (int i = 0; i < 6; ++i) l[i] = lam[i];
+  const Cx<double> a = qq_diagram_sum<double>(m, mt, gs, l, basis, col[0], col[1], col[2], col[3], col[4], col[5]);
+  const Cx<double> b = qq_dressed_amplitude<double>(m, mt, gs, l, basis, col[0], col[1], col[2], col[3], col[4], col[5]);
+  out[0] = a.re; out[1] = a.im; out[2] = b.re; out[3] = b.im;
 }
 double mfo_me2_light_line_ttbar_g(int kind, const double* mom, double mt, double alpha_s, int basis, int subst,
                                   int prec) {

@@ -65,6 +65,13 @@ double mfo_me2_qq(const mfo_process*, const double* mom, int basis, int prec);
 /* Quark channels of pp -> ttbar g (R19): averaged |M|^2 from the five Feynman diagrams with explicit colour.  kind 0: q(mom0) qbar(mom1) -> t(mom2) tbar(mom3) g(mom4); kind 1: q(mom0) g(mom1) -> t(mom2) tbar(mom3) q(mom4);
  * kind 2: qbar(mom0) g(mom1) -> t(mom2) tbar(mom3) qbar(mom4).  subst != 0: gluon polarisation -> its momentum (Ward identity: 0). */
 double mfo_me2_light_line_ttbar_g(int kind, const double* mom, double mt, double alpha_s, int basis, int subst, int prec);
+/* q(mom0) qbar(mom1) -> t(mom2) tbar(mom3) g(mom4) g(mom5): averaged |M|^2 from the 36 tree
+ * diagrams with explicit colour tensors.  subst = 0 / 1: that gluon's polarisation -> its momentum (Ward identity: 0), -1: none. */
+double mfo_me2_qq_ttbar_gg(const double* mom, double mt, double alpha_s, int basis, int subst, int prec);
+/* the same amplitude iM for explicit helicities lam[6] in {-1,+1} (q, qbar, t, tbar, g, g) and colours col[6] = (antiquark, quark,
+ * top, antitop in 0..2; gluons in 0..7): out[0..1] = sum over the diagrams, out[2..3] = colour-dressed subset recursion */
+void mfo_qq_ttbar_gg_amplitude(const double* mom, double mt, double gs, const int32_t* lam, int basis, const int32_t* col,
+                               double out[4]);
 /* x f(x, q2) of parton table `table` (0 gluon, 1+2i quark i, 2+2i antiquark i) */
 double mfo_pdf_xf_table(const mfo_process*, int table, double x, double q2, int prec);
 void mfo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);

@@ -72,6 +72,10 @@ def lib():
         L.mfo_colour_matrix_entry.restype = C.c_double
         L.mfo_colour_matrix_entry.argtypes = [C.c_int, c_i32_p, c_i32_p]
         L.mfo_set_dynamic_scale.argtypes = [C.c_void_p, C.c_int32]
+        L.mfo_me2_qq_ttbar_gg.restype = C.c_double
+        L.mfo_me2_qq_ttbar_gg.argtypes = [c_double_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int]
+        L.mfo_qq_ttbar_gg_amplitude.restype = None
+        L.mfo_qq_ttbar_gg_amplitude.argtypes = [c_double_p, C.c_double, C.c_double, c_i32_p, C.c_int, c_i32_p, c_double_p]
         L.mfo_me2_light_line_ttbar_g.restype = C.c_double
         L.mfo_me2_light_line_ttbar_g.argtypes = [C.c_int, c_double_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int]
         L.mfo_me2_qq.restype = C.c_double
@@ -155,6 +159,23 @@ def boost_z(y, p):
     out = np.empty(4)
     lib().mfo_boost_z(y, _dp(p), _dp(out))
     return out
+
+
+def me2_qq_ttbar_gg(mom, mt, alpha_s, basis=0, subst=-1, prec=0):
+    """averaged |M|^2 of q qbar -> t tbar g g at mom[6][4] (36 diagrams, explicit colour tensors)"""
+    mom = np.ascontiguousarray(mom, dtype=np.float64)
+    assert mom.shape == (6, 4)
+    return lib().mfo_me2_qq_ttbar_gg(_dp(mom), mt, alpha_s, basis, subst, prec)
+
+
+def qq_ttbar_gg_amplitude(mom, mt, gs, lam, col, basis=0):
+    """(diagram sum, dressed recursion) of iM for helicities lam[6] and colours col[6] = (qbar, q, t, tbar, g, g)"""
+    mom = np.ascontiguousarray(mom, dtype=np.float64)
+    lam = np.ascontiguousarray(lam, dtype=np.int32)
+    col = np.ascontiguousarray(col, dtype=np.int32)
+    out = np.zeros(4)
+    lib().mfo_qq_ttbar_gg_amplitude(_dp(mom), mt, gs, lam.ctypes.data_as(c_i32_p), basis, col.ctypes.data_as(c_i32_p), _dp(out))
+    return complex(out[0], out[1]), complex(out[2], out[3])
 
 
 def me2_light_line_ttbar_g(kind, mom, mt, alpha_s, basis=0, subst=0, prec=0):
@@ -282,7 +303,7 @@ class Process:
         ap = pp = None
         if want_amps:
             import math
-            ng = {1: 2, 2: 3, 3: 4, 4: 2, 5: 3, 6: 5}[self.wl.process]
+            ng = {1: 2, 2: 3, 3: 4, 4: 2, 5: 3, 6: 5, 7: 4}[self.wl.process]
             amps = np.zeros(((4 << ng), math.factorial(ng), 2))
             ap = _dp(amps)
         if want_per_hel:
@@ -328,7 +349,7 @@ class Process:
     def records_array(self, rec, count):
         """Decode `count` AoS records into a structured array: mom[n+2][4], w, id and, for process 4, channel."""
         fields = [("mom", np.float64, (self.n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)]
-        if self.wl.process in (4, 5):
+        if self.wl.process in (4, 5, 7):
             fields.append(("channel", np.uint64))
         dt = np.dtype(fields)
         assert dt.itemsize == self.record_size

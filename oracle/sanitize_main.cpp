@@ -30,9 +30,9 @@ int main(int argc, char** argv) {
     die("short table");
   std::fclose(f);
 
-  const int n_proc = 7;
-  const int nfinal[n_proc] = {2, 2, 3, 4, 2, 3, 5};
-  const int n_events[n_proc] = {200, 100, 30, 6, 80, 16, 1};
+  const int n_proc = 8;
+  const int nfinal[n_proc] = {2, 2, 3, 4, 2, 3, 5, 4};
+  const int n_events[n_proc] = {200, 100, 30, 6, 80, 16, 1, 2};
   for (int proc = 0; proc < n_proc; ++proc) {
     mfo_process_desc d;
     std::memset(&d, 0, sizeof d);
@@ -49,7 +49,7 @@ int main(int argc, char** argv) {
     if (proc != 0) {
       d.pdf_nx = nx; d.pdf_nq = nq;
       d.pdf_lnx = lnx.data(); d.pdf_lnq2 = lnq2.data(); d.pdf_xf = xf.data();
-      d.pdf_nfl = (proc == 4 || proc == 5) ? nfl : 1;
+      d.pdf_nfl = (proc == 4 || proc == 5 || proc == 7) ? nfl : 1;
     }
     mfo_process* P = nullptr;
     int rc = mfo_create_process(&d, &P);
@@ -82,7 +82,7 @@ int main(int argc, char** argv) {
     std::vector<double> rows((size_t)rl * 4);
     for (int prec = 0; prec < 3; ++prec) {
       const int m = (prec == 0 || proc < 3) ? 4 : 1;
-      if ((proc == 6 && prec != 0) || ((proc == 3 || proc == 5) && prec == 2)) continue;   // minutes under the sanitizers
+      if ((proc >= 6 && prec != 0) || ((proc == 3 || proc == 5) && prec == 2)) continue;   // minutes under the sanitizers
       if (mfo_debug_eval(P, grid.data(), 5, 1, 7, m, rows.data(), prec) != 0) die("debug_eval");
       mfo_vegas_iterate(P, grid.data(), 5, 1, 7, m, hist.data(), &res, prec);
       mfo_refine_grid(P, grid.data(), hist.data(), 1.5, prec);
@@ -166,6 +166,14 @@ int main(int argc, char** argv) {
     mfo_rambo(3, mass, 1000.0, rho, m5 + 8, 0);
     for (int kind = 0; kind < 3; ++kind)
       for (int prec = 0; prec < 2; ++prec) mfo_me2_light_line_ttbar_g(kind, m5, 173.0, 0.118, prec, prec, prec);
+    double m6[6 * 4] = {500, 0, 0, 500, 500, 0, 0, -500};
+    double mass4[4] = {173, 173, 0, 0}, rho4[16] = {0.15, 0.35, 0.55, 0.25, 0.35, 0.5, 0.45, 0.35, 0.55, 0.65, 0.35, 0.45, 0.2, 0.7, 0.4, 0.6};
+    mfo_rambo(4, mass4, 1000.0, rho4, m6 + 8, 0);
+    mfo_me2_qq_ttbar_gg(m6, 173.0, 0.118, 0, -1, 0);
+    mfo_me2_qq_ttbar_gg(m6, 173.0, 0.118, 3, 1, 0);
+    const int32_t lam[6] = {1, -1, 1, 1, -1, 1}, col[6] = {2, 2, 0, 0, 3, 3};
+    double amp[4];
+    mfo_qq_ttbar_gg_amplitude(m6, 173.0, 1.2, lam, 2, col, amp);
   }
   std::puts("sanitize_main: ok");
   return 0;

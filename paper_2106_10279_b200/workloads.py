@@ -15,11 +15,12 @@ import numpy as np
 MF_EE_MUMU, MF_GG_TT, MF_GG_TTG, MF_GG_TTGG = 0, 1, 2, 3
 MF_PP_TTG = 5              # gg -> ttbar g + the q qbar, q g and qbar g channels (36 diagrams with four flavours)
 MF_GG_TTGGG = 6            # gg -> ttbar ggg: the paper's heaviest process
+MF_PP_TTGG = 7             # gg -> ttbar gg + q qbar -> ttbar gg of four flavours: 123 + 4 x 36 = the 267 diagrams of PAPER.md L101, L140
 MF_PP_TT = 4               # gg -> ttbar + the q qbar -> ttbar channels of four flavours
 GEV2_TO_PB = 0.3894e9  # BASELINE.json configs[0]: use this literal everywhere
 N_BINS = 50
-N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18, MF_PP_TT: 4, MF_PP_TTG: 14, MF_GG_TTGGG: 22}
-N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4, MF_PP_TT: 2, MF_PP_TTG: 3, MF_GG_TTGGG: 5}
+N_DIMS = {MF_EE_MUMU: 2, MF_GG_TT: 4, MF_GG_TTG: 14, MF_GG_TTGG: 18, MF_PP_TT: 4, MF_PP_TTG: 14, MF_GG_TTGGG: 22, MF_PP_TTGG: 18}
+N_FINAL = {MF_EE_MUMU: 2, MF_GG_TT: 2, MF_GG_TTG: 3, MF_GG_TTGG: 4, MF_PP_TT: 2, MF_PP_TTG: 3, MF_GG_TTGGG: 5, MF_PP_TTGG: 4}
 N_FLAVOURS = 4             # quark flavours of the multi-flavour table: d, u, s, c (3 gg + 4 q qbar = the 7 diagrams of PAPER.md L101)
 VEGAS_ALPHA = 1.5
 
@@ -78,7 +79,10 @@ C6 = Workload("C6 pp -> ttbar j (gg + q qbar, q g, qbar g)", MF_PP_TTG, sqrt_s=1
 # cuts as for gg -> ttbar gg on all three gluons; the paper ran its heaviest process at <= 1M events
 C7 = Workload("C7 gg -> ttbar ggg", MF_GG_TTGGG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5, drmin=0.4, n_events=2 ** 18,
               n_iterations=10, n_adapt=10)
-EXTRA_CONFIGS = {"C5": C5, "C6": C6, "C7": C7}
+# pp -> ttbar gg (Table 1: the 267-diagram row): C3's sizes and cuts
+C8 = Workload("C8 pp -> ttbar gg (gg + q qbar)", MF_PP_TTGG, sqrt_s=13000.0, ptmin=30.0, etamax=2.5, drmin=0.4,
+              n_events=2 ** 22, n_iterations=10, n_adapt=10)
+EXTRA_CONFIGS = {"C5": C5, "C6": C6, "C7": C7, "C8": C8}
 
 
 def pdf_table(nx=100, nq=50):
@@ -125,7 +129,7 @@ def pdf_for(process, nx=100, nq=50):
     """the table a process needs: None, the gluon table, or the multi-flavour table"""
     if process == MF_EE_MUMU:
         return None
-    return pdf_table_flavours(nx, nq) if process in (MF_PP_TT, MF_PP_TTG) else pdf_table(nx, nq)
+    return pdf_table_flavours(nx, nq) if process in (MF_PP_TT, MF_PP_TTG, MF_PP_TTGG) else pdf_table(nx, nq)
 
 
 def uniform_grid(n_dims, n_bins=N_BINS):

@@ -27,6 +27,7 @@ def oracle_procs(pdf):
     procs[W.MF_PP_TT] = mfo.Process(W.C5, W.pdf_table_flavours())
     procs[W.MF_PP_TTG] = mfo.Process(W.C6, W.pdf_table_flavours())
     procs[W.MF_GG_TTGGG] = mfo.Process(W.C7, pdf)
+    procs[W.MF_PP_TTGG] = mfo.Process(W.C8, W.pdf_table_flavours())
     return procs
 
 
