@@ -30,7 +30,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "integrand events/sec (fp64) for gg->ttbar gg"      # BASELINE.json metric (C3, C4)
-PROCESS_LABEL = {0: "e+e- -> mu+mu-", 1: "gg->ttbar", 2: "gg->ttbar g", 3: "gg->ttbar gg", 4: "pp->ttbar (gg + q qbar)", 5: "pp->ttbar j (gg + q qbar, q g, qbar g)", 6: "gg->ttbar ggg"}
+PROCESS_LABEL = {0: "e+e- -> mu+mu-", 1: "gg->ttbar", 2: "gg->ttbar g", 3: "gg->ttbar gg", 4: "pp->ttbar (gg + q qbar)", 5: "pp->ttbar j (gg + q qbar, q g, qbar g)", 6: "gg->ttbar ggg", 7: "pp->ttbar gg (gg + q qbar)"}
 
 
 def metric_for(wl):
@@ -51,13 +51,13 @@ UNIT = "events/s"
 FLOP_HEADERS = {2: ("mf_me_ttg_coop_generated.cuh", "kFlopsMe2Coop_1g"), 3: ("mf_me_ttgg_coop_generated.cuh", "kFlopsMe2Coop_2g")}
 FLOP_PROFILES = {0: "profiles/r1_flops_C0.csv", 1: "profiles/r1_flops_C1.csv", 2: "profiles/r1_flops_C2.csv",
                  3: "profiles/r1_flops_C3.csv", 4: "profiles/r1_flops_C5.csv", 5: "profiles/r2_flops_C6.csv",
-                 6: "profiles/r2_flops_C7.csv"}
+                 6: "profiles/r2_flops_C7.csv", 7: "profiles/r2_flops_C8.csv"}
 FLOP_PROFILE_EVENTS = {0: (1_000_000, 1.0), 1: (1 << 20, 1.0), 2: (1 << 22, 0.8934), 3: (1 << 22, 0.7825), 4: (1 << 20, 1.0),
                        5: (1 << 22, 0.8945), 6: (1 << 18, 0.653)}      # events of the profiled launch, cut pass rate
 FLOP_PROFILE_DMMA = {6: 3840 * 512.0}            # flop per matrix element on the tensor path (not seen by the op_dfma counter)
 FLOP_PROFILE_ME = {2: 21472.0, 3: 157956.0}      # the static matrix-element count of the build that was profiled
-OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 0.0}
-ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 74090.0, 6: 6.31e6}    # 5, 6: per event PASSING the cuts
+OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 0.0, 7: 0.0}
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 74090.0, 6: 6.31e6, 7: 300000.0}    # 5, 6: per event PASSING the cuts
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
@@ -198,7 +198,7 @@ def run_reference(args, wl):
     from paper_2106_10279_b200 import workloads as W
     op = mfo.Process(wl, W.pdf_for(wl.process))
     grid = W.uniform_grid(wl.n_dims, wl.n_bins)
-    n = {0: 200000, 1: 40000, 2: 4000, 3: 400, 4: 20000, 5: 2000, 6: 24}[wl.process]     # ~2 s per step
+    n = {0: 200000, 1: 40000, 2: 4000, 3: 400, 4: 20000, 5: 2000, 6: 24, 7: 150}[wl.process]     # ~2 s per step
     times = []
     for k in range(args.warmup + args.steps):
         t0 = time.perf_counter()

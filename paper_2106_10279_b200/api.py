@@ -282,7 +282,7 @@ class Process:
 
     def records_array(self, records, count):
         """Decode `count` AoS records (uint8 tensor) into a numpy structured array with fields mom[n+2][4], w, id and,
-        for MF_PP_TT, channel (include/mf.h)."""
+        for MF_PP_TT / MF_PP_TTG / MF_PP_TTGG, channel (include/mf.h)."""
         from .lhe import record_dtype
         dt = record_dtype(self.n_final, self.wl.process)
         assert dt.itemsize == self.record_size
@@ -296,9 +296,10 @@ class Process:
 
 
 def debug_me2_quark_gluon(kind, m_top, alpha_s, mom):
-    """|M|^2 of q qbar -> ttbar g (kind 0), q g -> ttbar q (1), qbar g -> ttbar qbar (2) at mom[n][5][4]"""
+    """|M|^2 of q qbar -> ttbar g (kind 0), q g -> ttbar q (1), qbar g -> ttbar qbar (2) at mom[n][5][4];
+    kind 3: q qbar -> ttbar g g at mom[n][6][4]"""
     torch = _torch()
-    m = torch.as_tensor(np.ascontiguousarray(mom, dtype=np.float64)).cuda().reshape(-1, 5, 4)
+    m = torch.as_tensor(np.ascontiguousarray(mom, dtype=np.float64)).cuda().reshape(-1, 6 if kind == 3 else 5, 4)
     out = torch.empty(m.shape[0], dtype=torch.float64, device="cuda")
     _check(lib().mf_debug_me2_quark_gluon(kind, m_top, alpha_s, m.data_ptr(), m.shape[0], out.data_ptr(), _stream_ptr(None)),
            None, "mf_debug_me2_quark_gluon")

@@ -31,7 +31,7 @@ def generate():
     out = []
     if CSRC not in sys.path:
         sys.path.insert(0, CSRC)          # gen_coop imports gen_me
-    for name in ("gen_me", "gen_coop", "gen_coop3", "gen_cta5"):
+    for name in ("gen_me", "gen_coop", "gen_coop3", "gen_cta5", "gen_qq_colour"):
         spec = importlib.util.spec_from_file_location(name, os.path.join(CSRC, name + ".py"))
         mod = importlib.util.module_from_spec(spec)
         sys.modules[name] = mod

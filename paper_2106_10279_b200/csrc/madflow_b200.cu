@@ -21,12 +21,15 @@ struct mf_process {
   double *d_lnx = nullptr, *d_lnq2 = nullptr, *d_xf = nullptr, *d_row = nullptr;  // PDF table + collapsed row
   mf::BlockPartial* d_partials = nullptr;
   double* d_queue = nullptr;          // cooperative pass: per-block momenta queue
+  double* d_quark = nullptr;          // MF_PP_TTGG: quark-channel term per event of the current launch (grown on demand)
+  uint64_t quark_cap = 0;
   double* d_obs = nullptr;            // caller-owned observable histograms (mf_set_observables) or NULL
   int obs_nb = 0;
   double obs_ptmax = 0.0, obs_etamax = 0.0;
   double* d_hist_part = nullptr;
   int blocks = 0, threads = mf::kThreads;
   int blocks_unw = 0;
+  int prepass_blocks = 0;             // quark_prepass_kernel: resident blocks of the device
   size_t smem = 0;
   char err[256] = {0};
 };
@@ -52,6 +55,7 @@ const void* pass_fn(int proc, bool unw) {
     case 5: return unw ? (const void*)mf::fused_pass_coop_kernel<5, true> : (const void*)mf::fused_pass_coop_kernel<5, false>;
     case 6: return unw ? (const void*)mf::fused_pass_cta_kernel<true> : (const void*)mf::fused_pass_cta_kernel<false>;
     case 2: return unw ? (const void*)mf::fused_pass_coop_kernel<2, true> : (const void*)mf::fused_pass_coop_kernel<2, false>;
+    case 7: return unw ? (const void*)mf::fused_pass_coop_kernel<7, true> : (const void*)mf::fused_pass_coop_kernel<7, false>;
     default: return unw ? (const void*)mf::fused_pass_coop_kernel<3, true> : (const void*)mf::fused_pass_coop_kernel<3, false>;
   }
 }
@@ -64,12 +68,12 @@ cudaError_t coop_setup(mf_process* p, const cudaDeviceProp& prop) {
   const int group = PG::Team == 32 ? mf::kCoopGroupWarp : mf::kCoopGroup;      // teams run in lock-step groups
   int n_teams = mf::CoopOf<PROC>::MaxTeams;
   while (n_teams > 0 &&
-         (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, P.pdf_nx * P.pdf_nfl, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
+         (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, PROC == 5 ? P.pdf_nx * P.pdf_nfl : P.pdf_nx, n_teams).total * 8 > (size_t)prop.sharedMemPerBlockOptin)
     --n_teams;
   n_teams -= n_teams % group;
   if (n_teams < 1) return cudaErrorInvalidConfiguration;
   p->threads = n_teams * PG::Team;
-  p->smem = (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, P.pdf_nx * P.pdf_nfl, n_teams).total * 8;
+  p->smem = (size_t)mf::CoopSmem<PG>(p->D, P.n_bins, P.pdf_nx, PROC == 5 ? P.pdf_nx * P.pdf_nfl : P.pdf_nx, n_teams).total * 8;
   cudaError_t e;
   for (int u = 0; u < 2; ++u)
     // the attribute belongs to the kernel, not to the handle: always ask for the device maximum, so that handles with
@@ -85,7 +89,7 @@ cudaError_t coop_setup(mf_process* p, const cudaDeviceProp& prop) {
 
 void free_all(mf_process* p) {
   cudaFree(p->d_lnx); cudaFree(p->d_lnq2); cudaFree(p->d_xf); cudaFree(p->d_row);
-  cudaFree(p->d_partials); cudaFree(p->d_hist_part); cudaFree(p->d_queue);
+  cudaFree(p->d_partials); cudaFree(p->d_hist_part); cudaFree(p->d_queue); cudaFree(p->d_quark);
 }
 
 // launches the fused pass + finalize on `stream`
@@ -107,6 +111,23 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   A.coop_queue = p->d_queue;
   A.obs = p->d_obs; A.obs_nb = p->obs_nb; A.obs_ptmax = p->obs_ptmax; A.obs_etamax = p->obs_etamax;
   cudaStream_t st = (cudaStream_t)stream;
+  A.quark_terms = nullptr;
+  if (p->process == MF_PP_TTGG && n_events > 0) {
+    // the quark channels of every event of this launch, one thread per event, ahead of the cooperative pass on the same stream
+    if (n_events > p->quark_cap) {
+      cudaFree(p->d_quark);             // synchronises with earlier launches that read the old buffer
+      p->d_quark = nullptr; p->quark_cap = 0;
+      if (cudaMalloc(&p->d_quark, n_events * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(p, MF_ENOMEM, "quark-term buffer"); }
+      p->quark_cap = n_events;
+    }
+    const size_t smem = (size_t)(p->D * (p->P.n_bins + 1) + (1 + p->P.pdf_nfl) * p->P.pdf_nx) * sizeof(double);
+    const uint64_t want = (n_events + mf::kThreads - 1) / mf::kThreads;
+    const unsigned pre_blocks = (unsigned)(want < (uint64_t)p->prepass_blocks ? want : (uint64_t)p->prepass_blocks);
+    mf::quark_prepass_kernel<7><<<pre_blocks, mf::kThreads, smem, st>>>(p->P, A, p->d_quark);
+    cudaError_t pe = cudaGetLastError();
+    if (pe != cudaSuccess) return fail(p, MF_ECUDA, "quark prepass launch", pe);
+    A.quark_terms = p->d_quark;
+  }
   const int blocks = unw ? p->blocks_unw : p->blocks;
   void* args[2] = {(void*)&p->P, (void*)&A};
   cudaError_t e = cudaLaunchKernel(pass_fn(p->process, unw), dim3(blocks), dim3(p->threads), args, p->smem, st);
@@ -127,14 +148,14 @@ extern "C" {
 int mf_create_process(const mf_process_desc* d, mf_process** out) {
   if (out) *out = nullptr;
   if (!d || !out) return MF_EINVAL;
-  if (d->process < 0 || d->process > 6 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
+  if (d->process < 0 || d->process > 7 || d->n_bins < 2 || d->n_bins > MF_MAX_BINS || !(d->sqrt_s > 0.0) ||
       !(d->gev2_to_pb > 0.0))
     return MF_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MF_ECUDA; }
   mf_process* p = new (std::nothrow) mf_process;
   if (!p) return MF_ENOMEM;
-  static const int Dtab[7] = {2, 4, 14, 18, 4, 14, 22}, nftab[7] = {2, 2, 3, 4, 2, 3, 5};
+  static const int Dtab[8] = {2, 4, 14, 18, 4, 14, 22, 18}, nftab[8] = {2, 2, 3, 4, 2, 3, 5, 4};
   p->process = d->process; p->D = Dtab[d->process]; p->NF = nftab[d->process];
   mf::Params& P = p->P;
   std::memset(&P, 0, sizeof(P));
@@ -154,8 +175,8 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     }
     for (int i = 1; i < d->pdf_nx; ++i) if (!(d->pdf_lnx[i] > d->pdf_lnx[i - 1])) { delete p; return MF_EINVAL; }
     for (int i = 1; i < d->pdf_nq; ++i) if (!(d->pdf_lnq2[i] > d->pdf_lnq2[i - 1])) { delete p; return MF_EINVAL; }
-    const bool flavoured = d->process == MF_PP_TT || d->process == MF_PP_TTG;
-    const int ng = d->process == MF_PP_TT ? 2 : d->process == MF_PP_TTG ? 3 : d->process == MF_GG_TTGGG ? 5 : d->process + 1;
+    const bool flavoured = d->process == MF_PP_TT || d->process == MF_PP_TTG || d->process == MF_PP_TTGG;
+    const int ng = d->process == MF_PP_TT ? 2 : d->process == MF_PP_TTG ? 3 : d->process == MF_GG_TTGGG ? 5 : d->process == MF_PP_TTGG ? 4 : d->process + 1;
     const int nfl = flavoured ? d->pdf_nfl : 1;
     if (flavoured && (nfl < 3 || nfl % 2 == 0 || nfl > mf::kMaxPartonTables)) { delete p; return MF_EINVAL; }
     P.pdf_nfl = nfl;
@@ -197,10 +218,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     free_all(p); delete p; cudaGetLastError(); return MF_ECUDA;
   }
   p->device = dev;
-  const bool coop = p->process == 2 || p->process == 3 || p->process == 5;
+  const bool coop = p->process == 2 || p->process == 3 || p->process == 5 || p->process == 7;
   if (coop) {
     // cooperative pass: as many teams per block as the SM's shared memory holds, one block per SM
-    e = p->process == 3 ? coop_setup<3>(p, prop) : p->process == 5 ? coop_setup<5>(p, prop) : coop_setup<2>(p, prop);
+    e = p->process == 3 ? coop_setup<3>(p, prop) : p->process == 5 ? coop_setup<5>(p, prop) : p->process == 7 ? coop_setup<7>(p, prop) : coop_setup<2>(p, prop);
     if (e != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   } else if (p->process == MF_GG_TTGGG) {
     // one event per block: the whole block's shared memory is the scratch of the matrix element
@@ -227,12 +248,13 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   if (e != cudaSuccess || per_sm < 1 || per_sm_unw < 1) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   p->blocks = prop.multiProcessorCount * per_sm;
   p->blocks_unw = prop.multiProcessorCount * per_sm_unw;
+  p->prepass_blocks = prop.multiProcessorCount * MF_PREPASS_BLOCKS;
   const int max_blocks = p->blocks > p->blocks_unw ? p->blocks : p->blocks_unw;
   if ((e = cudaMalloc(&p->d_partials, (size_t)max_blocks * sizeof(mf::BlockPartial))) != cudaSuccess ||
       (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
-  const int queue_doubles = p->process == MF_GG_TTGGG ? mf::kCtaQueue : p->process == 3 ? mf::g4::Prog::Queue : mf::g3::Prog::Queue;
+  const int queue_doubles = p->process == MF_GG_TTGGG ? mf::kCtaQueue : (p->process == 3 || p->process == 7) ? mf::g4::Prog::Queue : mf::g3::Prog::Queue;
   if ((coop || p->process == MF_GG_TTGGG) &&
       (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads * queue_doubles * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
@@ -253,12 +275,12 @@ int mf_n_dims(const mf_process* p, int32_t* D) { if (!p || !D) return MF_EINVAL;
 int mf_n_final(const mf_process* p, int32_t* n) { if (!p || !n) return MF_EINVAL; *n = p->NF; return MF_OK; }
 int mf_record_size(const mf_process* p, int32_t* b) {
   if (!p || !b) return MF_EINVAL;
-  *b = (p->NF + 2) * 32 + 16 + ((p->process == MF_PP_TT || p->process == MF_PP_TTG) ? 8 : 0);
+  *b = (p->NF + 2) * 32 + 16 + ((p->process == MF_PP_TT || p->process == MF_PP_TTG || p->process == MF_PP_TTGG) ? 8 : 0);
   return MF_OK;
 }
 int mf_debug_row_len(const mf_process* p, int32_t* n) {
   if (!p || !n) return MF_EINVAL;
-  *n = 3 * p->D + 4 * (p->NF + 2) + 9 + (p->process == MF_PP_TT ? 2 : p->process == MF_PP_TTG ? 6 : 0);
+  *n = 3 * p->D + 4 * (p->NF + 2) + 9 + ((p->process == MF_PP_TT || p->process == MF_PP_TTGG) ? 2 : p->process == MF_PP_TTG ? 6 : 0);
   return MF_OK;
 }
 const char* mf_last_error(const mf_process* p) { return p ? p->err : kNullHandle; }
@@ -329,6 +351,10 @@ int mf_debug_eval(mf_process* p, const double* d_grid, uint64_t seed, uint32_t i
       mf::debug_eval_coop_kernel<2><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                       mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, A, d_out);
       break;
+    case 7:
+      mf::debug_eval_coop_kernel<7><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
+                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g4::Prog>(), st>>>(p->P, A, d_out);
+      break;
     default:
       mf::debug_eval_coop_kernel<3><<<(unsigned)((n_events + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                       mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g4::Prog>(), st>>>(p->P, A, d_out);
@@ -381,6 +407,10 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
       mf::debug_me2_coop_kernel<2><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g3::Prog>(), st>>>(p->P, d_mom, n, d_out);
       break;
+    case 7:
+      mf::debug_me2_coop_kernel<7><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
+                                     mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g4::Prog>(), st>>>(p->P, d_mom, n, d_out);
+      break;
     default:
       mf::debug_me2_coop_kernel<3><<<(unsigned)((n + mf::kCoopDebugThreads - 1) / mf::kCoopDebugThreads),
                                      mf::kCoopDebugThreads, mf::coop_debug_smem_bytes<mf::g4::Prog>(), st>>>(p->P, d_mom, n, d_out);
@@ -393,7 +423,7 @@ int mf_debug_me2(mf_process* p, const double* d_mom, uint64_t n, double* d_out, 
 
 int mf_debug_me2_quark_gluon(int32_t kind, double m_top, double alpha_s, const double* d_mom, uint64_t n, double* d_out,
                              void* stream) {
-  if (kind < 0 || kind > 2 || !(m_top > 0.0) || !(alpha_s > 0.0)) return MF_EINVAL;
+  if (kind < 0 || kind > 3 || !(m_top > 0.0) || !(alpha_s > 0.0)) return MF_EINVAL;
   if (n == 0) return MF_OK;
   if (!d_mom || !d_out) return MF_EINVAL;
   mf::debug_me2_quark_gluon_kernel<<<(unsigned)((n + mf::kThreads - 1) / mf::kThreads), mf::kThreads, 0,

@@ -109,6 +109,11 @@ __global__ void __launch_bounds__(kThreads) debug_me2_quark_gluon_kernel(int kin
                                                                          const double* mom, uint64_t n, double* out) {
   uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  if (kind == 3) {                      // q qbar -> t tbar g g: mom[n][6][4]
+    const double* m6 = mom + i * 24;
+    out[i] = me2_qq_ttgg(m6, m6 + 4, m6 + 8, m6 + 12, m6 + 16, m6 + 20, m_top, g2);
+    return;
+  }
   const double* m = mom + i * 20;
   if (kind == 0) out[i] = me2_light_line_ttg(0, m, m + 4, m + 8, m + 12, m + 16, m_top, g2);
   else if (kind == 1) out[i] = me2_light_line_ttg(1, m, m + 16, m + 8, m + 12, m + 4, m_top, g2);

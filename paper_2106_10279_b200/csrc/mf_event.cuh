@@ -9,6 +9,7 @@
 #include "mf_me_eemumu.cuh"
 #include "mf_me_qqtt.cuh"
 #include "mf_me_qttg.cuh"
+#include "mf_me_qqttgg.cuh"
 #include "mf_me_ggtt_generated.cuh"
 
 namespace mf {

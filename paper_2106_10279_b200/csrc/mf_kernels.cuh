@@ -40,6 +40,7 @@ struct PassArgs {
   double* obs;             // observable histograms [2][obs_nb + 1] (added to) or nullptr (mf_set_observables)
   int obs_nb;
   double obs_ptmax, obs_etamax;
+  const double* quark_terms;  // pp -> ttbar gg: the quark-channel term of every event (quark_prepass_kernel) or nullptr
   double* coop_queue;      // cooperative kernels only: [gridDim.x][blockDim.x][18] momenta queue (mf_kernels_coop.cuh)
 };
 
@@ -65,6 +66,19 @@ __device__ __noinline__ void quark_gluon_me2_all(const Params& P, double shat, c
   const double E = 0.5 * sqrt(shat);
   const double b1[4] = {E, 0.0, 0.0, E}, b2[4] = {E, 0.0, 0.0, -E};
   me2_ttj_quark_classes(b1, b2, k[0], k[1], k[2], P.m_top, 4.0 * kPi * P.alpha_s, M);
+}
+
+// process 7: |M|^2 of q qbar -> t tbar g g with the quark from beam 1 (Ma) and from beam 2 (Mb) (mf_me_qqttgg.cuh).
+// Out of line: one copy per kernel.
+__device__ __noinline__ void quark_pair_me2_gg(const Params& P, double shat, const double (*k)[4], double M[2]) {
+  const double E = 0.5 * sqrt(shat);
+  const double g2 = 4.0 * kPi * P.alpha_s;
+#pragma unroll 1
+  for (int o = 0; o < 2; ++o) {            // one copy of the code for both assignments
+    const double pz = o == 0 ? E : -E;
+    const double bq[4] = {E, 0.0, 0.0, pz}, bqbar[4] = {E, 0.0, 0.0, -pz};
+    M[o] = me2_qq_ttgg(bq, bqbar, k[0], k[1], k[2], k[3], P.m_top, g2);
+  }
 }
 
 // Luminosity (step a6): F(x1) F(x2) / (x1 x2) with F the interpolant of the collapsed row in shared memory; and
@@ -185,6 +199,35 @@ MF_D double pp_ttj_terms(const Params& P, const PassArgs& A, const double* s_lnx
     sum += term;
   }
   quark_sum = sum;
+  return f1[0] * f2[0] * inv;
+}
+
+// pp -> ttbar gg (R21): the gluon-gluon luminosity (returned) and the flavour-summed quark term
+//   quark_sum = sum_i [ q_i(x1) qbar_i(x2) Ma + qbar_i(x1) q_i(x2) Mb ] / (x1 x2)   (x the R16 factor)
+// parts (optional, debug rows): the flavour-summed q qbar luminosity and the luminosity-weighted mean of Ma, Mb.
+MF_D double pp_ttgg_terms(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                          const Event<7>& ev, double& asf, double& quark_sum, double* parts) {
+  double f1[kMaxPartonTables], f2[kMaxPartonTables];
+  parton_densities<7>(P, A, s_lnx, s_row, ev, f1, f2, asf);
+  const int nt = P.pdf_nfl;
+  double La = 0.0, Lb = 0.0;
+#pragma unroll
+  for (int t = 1; t + 1 < kMaxPartonTables; t += 2)
+    if (t + 1 < nt) {
+      La = fma(f1[t], f2[t + 1], La);
+      Lb = fma(f1[t + 1], f2[t], Lb);
+    }
+  const double inv = 1.0 / (ev.x1 * ev.x2);
+  La *= inv;
+  Lb *= inv;
+  double M[2];
+  quark_pair_me2_gg(P, ev.shat, ev.k, M);
+  const double both = La * (M[0] * asf) + Lb * (M[1] * asf);
+  if (parts) {
+    parts[0] = La + Lb;
+    parts[1] = (La + Lb) != 0.0 ? both / (La + Lb) : M[0] * asf;
+  }
+  quark_sum = both;
   return f1[0] * f2[0] * inv;
 }
 
@@ -323,6 +366,31 @@ __device__ __forceinline__ unsigned pp_ttj_channel(const Params& P, const PassAr
   return (unsigned)(6 * nf);
 }
 
+// pp -> ttbar gg (R21): the partonic channel of an ACCEPTED event, codes as for pp -> ttbar (0 gg; 1 + 2 i quark i
+// from beam 1; 2 + 2 i quark i from beam 2), drawn as in pp_ttj_channel (the gluon channel's term is what w leaves).
+__device__ __forceinline__ unsigned pp_ttgg_channel(const Params& P, const PassArgs& A, const Event<7>& ev, double w, double v) {
+  double f1[kMaxPartonTables], f2[kMaxPartonTables], asf;
+  parton_densities<7>(P, A, A.pdf_lnx, A.pdf_row, ev, f1, f2, asf);
+  const int nt = P.pdf_nfl;
+  const double inv = 1.0 / (ev.x1 * ev.x2);
+  double M[2];
+  quark_pair_me2_gg(P, ev.shat, ev.k, M);
+  auto sterm = [&](int t) { return (t & 1) ? f1[t] * f2[t + 1] * inv * (M[0] * asf) : f1[t] * f2[t - 1] * inv * (M[1] * asf); };
+  double quark_sum = 0.0;
+  for (int t = 1; t < nt; ++t) quark_sum += sterm(t);
+  const double gg_term = w / event_weight<7>(P, ev, 1.0, 1.0) - quark_sum;
+  double total = fabs(gg_term);
+  for (int t = 1; t < nt; ++t) total += fabs(sterm(t));
+  const double vt = v * total;
+  double cum = fabs(gg_term);
+  if (cum > vt) return 0u;
+  for (int t = 1; t < nt; ++t) {
+    cum += fabs(sterm(t));
+    if (cum > vt) return (unsigned)t;
+  }
+  return (unsigned)(nt - 1);
+}
+
 // Per-thread running sums of the pass (registers).
 struct Accum {
   double sum_w = 0.0, sum_w2 = 0.0, max_w = 0.0;
@@ -375,7 +443,7 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
           }
           double mom[NF + 2][4];
           lab_momenta<PROC>(ev, mom);
-          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16 + ((PROC == 4 || PROC == 5) ? 8 : 0)));
+          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16 + ((PROC == 4 || PROC == 5 || PROC == 7) ? 8 : 0)));
 #pragma unroll
           for (int i = 0; i < NF + 2; ++i)
 #pragma unroll
@@ -386,6 +454,10 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
           if constexpr (PROC == 5) {
             const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);      // words z, w: the channel draw
             reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = pp_ttj_channel(P, A, ev, w, uniform52(r.z, r.w));
+          }
+          if constexpr (PROC == 7) {
+            const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);
+            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = pp_ttgg_channel(P, A, ev, w, uniform52(r.z, r.w));
           }
         }
       }
@@ -479,6 +551,42 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
     accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins, channel, PROC == 0 ? nullptr : &ev);
   }
   block_finish(A, acc, s_red, s_hist, D * nb);
+}
+
+// ---- pp -> ttbar gg: the quark channel, one thread per event, BEFORE the cooperative pass ---------------------------------
+// out[i] = sum over the quark channels of luminosity x |M|^2 (x the R16 factor) of event first_event + i (0 if it fails the cuts):
+// the term the cooperative pass adds to  L_gg |M_gg|^2.  The quark matrix elements are thread-per-event code with hundreds of
+// live values; inside the cooperative kernels (168 registers, 231 kB of shared memory, so almost no L1) they ran out of
+// local memory at a fraction of the FP64 rate.  Here: 255 registers, 15 kB of shared memory, the rest of the SM's 256 kB as L1.
+#ifndef MF_PREPASS_BLOCKS
+#define MF_PREPASS_BLOCKS 2
+#endif
+template <int PROC>
+__global__ void __launch_bounds__(kThreads, MF_PREPASS_BLOCKS) quark_prepass_kernel(const Params P, const PassArgs A, double* out) {
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  extern __shared__ double smem[];
+  const int nb = P.n_bins, nx = P.pdf_nx, nrow = nx * P.pdf_nfl;
+  double* s_grid = smem;                    // D*(nb+1)
+  double* s_lnx = s_grid + D * (nb + 1);    // nx
+  double* s_row = s_lnx + nx;               // one row per parton table
+  for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
+  for (int i = threadIdx.x; i < nx; i += blockDim.x) s_lnx[i] = A.pdf_lnx[i];
+  for (int i = threadIdx.x; i < nrow; i += blockDim.x) s_row[i] = A.pdf_row[i];
+  __syncthreads();
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  for (uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < A.n_events; idx += stride) {
+    Bins<PROC> bins;
+    Event<PROC> ev;
+    DebugRow dbg = {nullptr, D, NF};
+    generate_event<PROC>(P, s_grid, A.seed, A.iteration, A.first_event + idx, ev, bins, dbg);
+    double quark_sum = 0.0;
+    if (ev.pass) {
+      double asf;
+      if constexpr (PROC == 5) pp_ttj_terms(P, A, s_lnx, s_row, ev, asf, quark_sum, nullptr);
+      else pp_ttgg_terms(P, A, s_lnx, s_row, ev, asf, quark_sum, nullptr);
+    }
+    out[idx] = quark_sum;
+  }
 }
 
 // Adds the per-block partials in block order.  Blocks 0..gridDim.x-2 own histogram bins (one thread per

@@ -21,8 +21,14 @@ namespace mf {
 template <int PROC> struct CoopOf { typedef g4::Prog PG; static constexpr int MaxTeams = 6; };   // PROC = 3
 template <> struct CoopOf<2> { typedef g3::Prog PG; static constexpr int MaxTeams = 16; };
 // pp -> ttbar j: the gg -> ttbar g program for the gluon channel; the owner threads evaluate the quark-channel classes
-// (register hungry): 12 teams x 168 registers measured best (8 x 255: 39.9 ms, 12: 36.9 ms, 16 x 128: 38.1 ms per 2^22 events)
+// (register hungry): 12 teams x 168 registers measured best (8 x 255: 39.9 ms, 12: 36.9 ms, 16 x 128: 38.1 ms per 2^22 events).
+// Measured and rejected (profiles/r2_c8.md): the quark classes in a thread-per-event kernel of their own ahead of this pass
+// (quark_prepass_kernel, 255 registers) with 16 teams x 128 registers here: 35.3-42.2 ms against 31.1 ms.
 template <> struct CoopOf<5> { typedef g3::Prog PG; static constexpr int MaxTeams = 12; };
+// pp -> ttbar gg: the g g -> t tbar g g program; the quark channel (q qbar -> t tbar g g, two beam assignments: 155 kflop and
+// 4.4 kB of thread-local state per event) comes from quark_prepass_kernel through PassArgs::quark_terms: on the owner threads of
+// this kernel (231 kB of shared memory, so almost no L1) it took 350 ms per 2^22 events, ahead of it 195 ms.
+template <> struct CoopOf<7> { typedef g4::Prog PG; static constexpr int MaxTeams = 6; };
 
 // queue entry = the event record of mf_me_coop_tasks.inc (momenta, shat, polarisation vectors, spinors, c0): PG::Queue doubles
 
@@ -180,7 +186,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
   constexpr int G = PG::Team == 32 ? kCoopGroupWarp : kCoopGroup;
   extern __shared__ double2 smem2[];
   double* smem = reinterpret_cast<double*>(smem2);
-  const int nb = P.n_bins, nx = P.pdf_nx, nrow = PROC == 5 ? nx * P.pdf_nfl : nx;
+  const int nb = P.n_bins, nx = P.pdf_nx, nrow = PROC == 5 ? nx * P.pdf_nfl : nx;   // pp -> ttbar gg: the gluon's row only (the quark rows are the prepass's business)
   const int n_teams = blockDim.x / PG::Team;
   const CoopSmem<PG> L(D, nb, nx, nrow, n_teams);
   double* s_grid = smem + L.grid;
@@ -218,6 +224,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
       if (ev.pass) {
         if constexpr (PROC == 5) lum = pp_ttj_terms(P, A, s_lnx, s_row, ev, asf, quark_sum, nullptr);
         else lum = luminosity<PROC>(P, A, s_lnx, s_row, ev, asf);
+        if constexpr (PROC == 7) quark_sum = A.quark_terms[idx];
       }
     }
     const bool pass = valid && ev.pass;
@@ -227,7 +234,7 @@ __global__ void __launch_bounds__(CoopOf<PROC>::MaxTeams * CoopOf<PROC>::PG::Tea
     double w = 0.0;
     if (pass) {
       ++acc.n_pass;
-      if (PROC == 5) w = event_weight<PROC>(P, ev, 1.0, fma(lum, me2 * asf, quark_sum));
+      if (PROC == 5 || PROC == 7) w = event_weight<PROC>(P, ev, 1.0, fma(lum, me2 * asf, quark_sum));
       else w = event_weight<PROC>(P, ev, lum, me2 * asf);
     }
     accumulate_event<PROC, UNW>(P, A, s_grid, s_hist, valid, event, w, bins, acc, obs_bins);
@@ -260,7 +267,7 @@ __global__ void __launch_bounds__(kCoopDebugThreads) debug_eval_coop_kernel(cons
   const CoopDebugSmem<PG> L(reinterpret_cast<double*>(smem2));
   coop_load_table<PG>(L.s_tab);
   __syncthreads();
-  const int row_len = 3 * D + 4 * (NF + 2) + 9;
+  const int row_len = 3 * D + 4 * (NF + 2) + 9 + (PROC == 7 ? 2 : 0);
   const uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = idx < A.n_events;
   const uint64_t event = A.first_event + idx;
@@ -284,9 +291,21 @@ __global__ void __launch_bounds__(kCoopDebugThreads) debug_eval_coop_kernel(cons
   double lum = 0.0, w = 0.0;
   if (pass) {
     double asf;
-    lum = luminosity<PROC>(P, A, A.pdf_lnx, A.pdf_row, ev, asf);
-    me2 *= asf;
-    w = event_weight<PROC>(P, ev, lum, me2);
+    if constexpr (PROC == 7) {
+      double quark_sum, parts[2];
+      lum = pp_ttgg_terms(P, A, A.pdf_lnx, A.pdf_row, ev, asf, quark_sum, parts);
+      me2 *= asf;
+      w = event_weight<PROC>(P, ev, 1.0, fma(lum, me2, quark_sum));
+      row[3 * D + 4 * (NF + 2) + 9] = parts[0];
+      row[3 * D + 4 * (NF + 2) + 10] = parts[1];
+    } else {
+      lum = luminosity<PROC>(P, A, A.pdf_lnx, A.pdf_row, ev, asf);
+      me2 *= asf;
+      w = event_weight<PROC>(P, ev, lum, me2);
+    }
+  } else if (PROC == 7) {
+    row[3 * D + 4 * (NF + 2) + 9] = 0.0;
+    row[3 * D + 4 * (NF + 2) + 10] = 0.0;
   }
   q[0] = ev.x1; q[1] = ev.x2; q[2] = lum; q[3] = me2; q[4] = ev.phi; q[5] = ev.jac_vegas; q[6] = w;
   q[7] = pass ? 1.0 : 0.0;

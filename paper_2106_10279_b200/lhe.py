@@ -32,7 +32,7 @@ QUARK_PDG = (1, 2, 3, 4, 5)          # flavour index of the multi-flavour table 
 
 def record_dtype(n_final, process=None):
     fields = [("mom", np.float64, (n_final + 2, 4)), ("w", np.float64), ("id", np.uint64)]
-    if process in (4, 5):             # MF_PP_TT / MF_PP_TTG records carry the partonic channel (include/mf.h)
+    if process in (4, 5, 7):          # MF_PP_TT / MF_PP_TTG / MF_PP_TTGG records carry the partonic channel (include/mf.h)
         fields.append(("channel", np.uint64))
     return np.dtype(fields)
 
@@ -68,6 +68,22 @@ def channel_ids_ttj(channel):
     return tuple(ids), flow
 
 
+def channel_ids_ttgg(channel):
+    """PDG ids (beam 1, beam 2, t, tbar, g, g) and one valid colour flow of an MF_PP_TTGG record's channel code (R21): 0 = gg;
+    1 + 2 i = quark i from beam 1 and its antiquark from beam 2; 2 + 2 i = the other way round"""
+    c = int(channel)
+    if c == 0:
+        return PDG[3], colour_flow(3)
+    q = QUARK_PDG[(c - 1) // 2]
+    # the quark's colour leaves on the first gluon, whose anticolour is the second gluon's colour, whose anticolour is the
+    # top's colour; the antiquark's anticolour goes to the antitop
+    ids, flow = [q, -q, 6, -6, 21, 21], [(501, 0), (0, 502), (504, 0), (0, 502), (501, 503), (503, 504)]
+    if c % 2 == 0:
+        ids[0], ids[1] = ids[1], ids[0]
+        flow[0], flow[1] = flow[1], flow[0]
+    return tuple(ids), flow
+
+
 def colour_flow(process):
     """(colour, anticolour) tags per particle for the fixed planar flow; incoming gluons carry the crossed tags"""
     ids = PDG[process]
@@ -88,15 +104,15 @@ def colour_flow(process):
 
 def format_events(rec, process, m_top, scale, alpha_em, alpha_s, w_max):
     """LHE <event> blocks for a structured record array (pure function: also used by the tests)"""
-    per_event = process in (4, 5)
+    per_event = process in (4, 5, 7)
     if not per_event:
         ids = PDG[process]
         flow = colour_flow(process)
-    n = {4: 4, 5: 5}[process] if per_event else len(ids)
+    n = {4: 4, 5: 5, 7: 6}[process] if per_event else len(ids)
     out = io.StringIO()
     for r in rec:
         if per_event:
-            ids, flow = channel_ids(r["channel"]) if process == 4 else channel_ids_ttj(r["channel"])
+            ids, flow = {4: channel_ids, 5: channel_ids_ttj, 7: channel_ids_ttgg}[process](r["channel"])
         mass = [m_top if abs(p) == 6 else 0.0 for p in ids]
         w = float(r["w"])
         xw = (1.0 if w >= 0 else -1.0) * max(1.0, abs(w) / w_max)
@@ -113,7 +129,7 @@ def format_events(rec, process, m_top, scale, alpha_em, alpha_s, w_max):
 class LheDrain:
     def __init__(self, path, proc, compress=None):
         import torch
-        if proc.wl.process not in PDG and proc.wl.process not in (4, 5):
+        if proc.wl.process not in PDG and proc.wl.process not in (4, 5, 7):
             raise ValueError("LHE output: unknown process %d" % proc.wl.process)
         self.torch = torch
         self.path = path

@@ -40,6 +40,7 @@ def gpu_procs(pdf):
     procs[W.MF_PP_TT] = api.Process(W.C5, W.pdf_table_flavours())
     procs[W.MF_PP_TTG] = api.Process(W.C6, W.pdf_table_flavours())
     procs[W.MF_GG_TTGGG] = api.Process(W.C7, pdf)
+    procs[W.MF_PP_TTGG] = api.Process(W.C8, W.pdf_table_flavours())
     yield procs
     for p in procs.values():
         p.close()
@@ -61,7 +62,7 @@ def adapted_grid(oracle_proc, wl, n_iter=3):
     """A non-uniform VEGAS grid made by the ORACLE alone (a few small adapting iterations); cached."""
     from paper_2106_10279_b200 import workloads as W
     if wl.process not in _ADAPTED:
-        n_events = {0: 20000, 1: 8192, 2: 4096, 3: 1024, 4: 8192, 5: 4096, 6: 96}[wl.process]
+        n_events = {0: 20000, 1: 8192, 2: 4096, 3: 1024, 4: 8192, 5: 4096, 6: 96, 7: 384}[wl.process]
         grid = W.uniform_grid(wl.n_dims, wl.n_bins)
         for k in range(n_iter):
             hist, _ = oracle_proc.vegas_iterate(grid, 12345, k, 0, n_events)

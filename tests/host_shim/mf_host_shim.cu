@@ -6,6 +6,7 @@
 #include "../../paper_2106_10279_b200/csrc/mf_me_qttg.cuh"
 #include "../../paper_2106_10279_b200/csrc/mf_me_coop.cuh"
 #include "../../paper_2106_10279_b200/csrc/mf_me_cta5.cuh"
+#include "../../paper_2106_10279_b200/csrc/mf_me_qqttgg.cuh"
 #include <vector>
 
 using namespace mf;
@@ -92,6 +93,11 @@ double mfh_me2_light_line_ttg(int kind, const double* mom, double m_top, double 
 // all six classes at one CM-frame point: mom = b1, b2, t, tbar, parton (mf_me_qttg.cuh: shared top-line currents)
 void mfh_me2_ttj_quark_classes(const double* mom, double m_top, double alpha_s, double out[6]) {
   me2_ttj_quark_classes(mom, mom + 4, mom + 8, mom + 12, mom + 16, m_top, 4.0 * kPi * alpha_s, out);
+}
+
+// q qbar -> t tbar g g at one CM-frame point: mom = q, qbar, t, tbar, g, g (mf_me_qqttgg.cuh)
+double mfh_me2_qq_ttgg(const double* mom, double m_top, double alpha_s) {
+  return me2_qq_ttgg(mom, mom + 4, mom + 8, mom + 12, mom + 16, mom + 20, m_top, 4.0 * kPi * alpha_s);
 }
 
 void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {

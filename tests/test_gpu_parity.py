@@ -30,7 +30,7 @@ def _cols(wl):
     o = D + 4 * (n + 2)
     c = dict(x=slice(0, D), mom=slice(D, o), x1=o, x2=o + 1, lum=o + 2, me2=o + 3, phi=o + 4, jac=o + 5, w=o + 6,
              pas=o + 7, r=o + 8, u=slice(o + 9, o + 9 + D), bin=slice(o + 9 + D, o + 9 + 2 * D))
-    if wl.process == W.MF_PP_TT:       # the quark channel's flavour-summed luminosity and matrix element
+    if wl.process in (W.MF_PP_TT, W.MF_PP_TTGG):       # the quark channel's flavour-summed luminosity and matrix element
         c["lum_qq"], c["me2_qq"] = o + 9 + 2 * D, o + 10 + 2 * D
     if wl.process == W.MF_PP_TTG:      # luminosity x |M|^2 of the six quark-channel classes
         c["chq"] = slice(o + 9 + 2 * D, o + 15 + 2 * D)
@@ -123,6 +123,20 @@ def _compare_rows(wl, g, o):
             assert abs(lq_g - lq_o) <= REL_EVENT * abs(lq_o) + slack_q, ("lum_qq", k, lq_g, lq_o)
             total = lum_o * o[k, c["me2"]] + lq_o * b
             w_slack = abs(wo / total) * (slack * o[k, c["me2"]] + slack_q * b) if total != 0.0 else 0.0
+        if wl.process == W.MF_PP_TTGG:
+            # gg + q qbar (two beam assignments with different matrix elements): me2_qq is their luminosity-weighted mean, so
+            # the product lum_qq x me2_qq (the quark term of the weight) is what is compared where the luminosity cancels
+            lq_g, lq_o = g[k, c["lum_qq"]], o[k, c["lum_qq"]]
+            mq_g, mq_o = g[k, c["me2_qq"]], o[k, c["me2_qq"]]
+            scale_q = 2 * W.N_FLAVOURS * _knot_scale(x1, True) * _knot_scale(x2, True) / (x1 * x2)
+            slack_q = 4e-13 * scale_q if scale_q > 250.0 * abs(lq_o) else 0.0
+            assert abs(lq_g - lq_o) <= REL_EVENT * abs(lq_o) + slack_q, ("lum_qq", k, lq_g, lq_o)
+            if slack_q == 0.0:
+                assert abs(mq_g - mq_o) <= REL_EVENT * abs(mq_o), ("me2_qq", k, mq_g, mq_o)
+            floor = 2 * slack_q * abs(mq_o) + 1e-12 * abs(lum_o * b)
+            assert abs(lq_g * mq_g - lq_o * mq_o) <= REL_EVENT * abs(lq_o * mq_o) + floor, ("quark term", k)
+            total = lum_o * b + lq_o * mq_o
+            w_slack = abs(wo / total) * (slack * abs(b) + floor) if total != 0.0 else 0.0
         if wl.process == W.MF_PP_TTG:
             # seven channels: each quark-channel term on its own (1e-10 relative, plus 1e-12 of the event's largest term
             # for the ones that nearly vanish where a density changes sign), then the sum

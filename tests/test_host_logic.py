@@ -87,7 +87,7 @@ def shim():
     L = C.CDLL(out)
     L.mfh_me2.restype = C.c_double
     L.mfh_me2.argtypes = [C.c_int, dp, C.c_double, C.c_double, C.c_double]
-    for f in (L.mfh_me2_coop, L.mfh_me2_coop3, L.mfh_me2_cta5):
+    for f in (L.mfh_me2_coop, L.mfh_me2_coop3, L.mfh_me2_cta5, L.mfh_me2_qq_ttgg):
         f.restype = C.c_double
         f.argtypes = [dp, C.c_double, C.c_double]
     L.mfh_event.argtypes = [C.c_int, dp, C.c_int] + [C.c_double] * 8 + [C.c_uint64, C.c_uint32, C.c_uint64, dp]
@@ -274,6 +274,22 @@ def test_bench_flop_constants():
         assert ("constexpr double %s = %d.0;" % (name, b.me_flops(proc))) in txt
     # the static count of the profiled gg -> ttbar g build is still the header's (that kernel has not changed since)
     assert b.me_flops(2) == b.FLOP_PROFILE_ME[2]
+
+
+def test_shim_qq_ttgg(shim):
+    """the product's q qbar -> t tbar g g (13 + 13 currents, 20 colour strings, rank-11 colour form, left-handed light line doubled)
+    against the oracle's 36 diagrams with explicit colour tensors at RAMBO points, both beam assignments"""
+    from oracle import mfo
+    rng = np.random.default_rng(21)
+    mt, a_s = 173.0, 0.118
+    for i in range(6):
+        w = 500.0 + 3000.0 * rng.random()
+        k, _ = mfo.rambo([mt, mt, 0.0, 0.0], w, rng.random(16))
+        mom = np.vstack([[w / 2, 0, 0, w / 2], [w / 2, 0, 0, -w / 2], k])
+        if i & 1:
+            mom[[0, 1]] = mom[[1, 0]]
+        g = shim.mfh_me2_qq_ttgg(np.ascontiguousarray(mom).ctypes.data_as(dp), mt, a_s)
+        assert g == pytest.approx(mfo.me2_qq_ttbar_gg(mom, mt, a_s), rel=1e-11)
 
 
 # ---- multi-rank sharding (gloo, world size 2) ------------------------------------------------------------------
