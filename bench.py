@@ -43,8 +43,8 @@ UNIT = "events/s"
 #    read from the generated headers at run time (FLOP_HEADERS; a DMMA.884 counts its 2 x 256 flop); the rest of the chain
 #    (a1-a6, a10-a14 incl. the software sqrt / div / log / sincos sequences and the owner-side wavefunctions) is OTHER_FLOPS,
 #    calibrated by ncu: executed (2 dfma + dadd + dmul) of one launch minus n_pass x the static count (FLOP_PROFILES).
-#  * thread-per-event kernels (0, 1, 4), pp -> ttbar j (5) and g g -> ttbar ggg (6): the ncu-executed TOTAL per event (per
-#    passing event for 5 and 6; for 6 plus its 3840 DMMA x 512 flop) is used (ME_FLOPS_MEASURED): for 0, 1, 4 the compiler
+#  * thread-per-event kernels (0, 1, 4), pp -> ttbar j (5), g g -> ttbar ggg (6) and pp -> ttbar gg (7, prepass + fused pass): the
+#    ncu-executed TOTAL per event (per passing event for 5, 6, 7; for 6 / 7 plus their 3840 / 48 DMMA x 512 flop) is used (ME_FLOPS_MEASURED): for 0, 1, 4 the compiler
 #    folds constants into the matrix element, so the static count overestimates; for 6 the generator's static count
 #    (5.89 M) misses 7 % of the executed operations (sign and scale multiplications).
 # tests/test_host_logic.py::test_bench_flop_constants recomputes every literal below from the committed ncu csv files.
@@ -53,11 +53,11 @@ FLOP_PROFILES = {0: "profiles/r1_flops_C0.csv", 1: "profiles/r1_flops_C1.csv", 2
                  3: "profiles/r1_flops_C3.csv", 4: "profiles/r1_flops_C5.csv", 5: "profiles/r2_flops_C6.csv",
                  6: "profiles/r2_flops_C7.csv", 7: "profiles/r2_flops_C8.csv"}
 FLOP_PROFILE_EVENTS = {0: (1_000_000, 1.0), 1: (1 << 20, 1.0), 2: (1 << 22, 0.8934), 3: (1 << 22, 0.7825), 4: (1 << 20, 1.0),
-                       5: (1 << 22, 0.8945), 6: (1 << 18, 0.653)}      # events of the profiled launch, cut pass rate
-FLOP_PROFILE_DMMA = {6: 3840 * 512.0}            # flop per matrix element on the tensor path (not seen by the op_dfma counter)
+                       5: (1 << 22, 0.8945), 6: (1 << 18, 0.653), 7: (1 << 22, 0.7855)}      # events of the profiled launch, cut pass rate
+FLOP_PROFILE_DMMA = {6: 3840 * 512.0, 7: 48 * 512.0}            # flop per matrix element on the tensor path (not seen by the op_dfma counter)
 FLOP_PROFILE_ME = {2: 21472.0, 3: 157956.0}      # the static matrix-element count of the build that was profiled
 OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 0.0, 7: 0.0}
-ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 74090.0, 6: 6.31e6, 7: 300000.0}    # 5, 6: per event PASSING the cuts
+ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 74090.0, 6: 6.31e6, 7: 318300.0}    # 5, 6: per event PASSING the cuts
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}
@@ -79,10 +79,10 @@ def me_flops(process):
 def executed_flops_of_profile(path):
     """2 dfma + dadd + dmul (thread instructions, predicated on) of the ncu --csv metric log `path`"""
     import csv
-    v = {}
+    v = {"dfma": 0.0, "dadd": 0.0, "dmul": 0.0}            # summed over the profiled launches (C8: prepass + fused pass)
     for row in csv.reader(open(os.path.join(ROOT, path))):
         if len(row) > 14 and row[12].startswith("smsp__sass_thread_inst_executed_op_d"):
-            v[row[12].split("_op_")[1].split("_")[0]] = float(row[14])
+            v[row[12].split("_op_")[1].split("_")[0]] += float(row[14])
     return 2.0 * v["dfma"] + v["dadd"] + v["dmul"]
 
 

@@ -43,7 +43,7 @@ enum { MF_EE_MUMU = 0, MF_GG_TT = 1, MF_GG_TTG = 2, MF_GG_TTGG = 3, MF_PP_TT = 4
 /* MF_PP_TTG ("pp -> ttbar g (36 diagrams)"; R19): at the phase-space point, cuts and stream of MF_GG_TTG the
  * weight sums g g -> t tbar g and the flavour-summed q qbar -> t tbar g, q g -> t tbar q, qbar g -> t tbar qbar channels (either
  * beam assignment); the light final-state parton is a jet whatever its flavour.  Same multi-flavour table as MF_PP_TT. */
-/* MF_PP_TTGG (P:L101 and Table 1, "pp -> ttbar gg (267 diagrams)" = 123 + 4 x 36; R21): at the phase-space point,
+/* MF_PP_TTGG (P:L101 and Table 1, "pp -> ttbar gg (267 diagrams)" = 123 + 4 x 36; R22): at the phase-space point,
  * cuts and stream of MF_GG_TTGG the weight sums g g -> t tbar g g and q qbar -> t tbar g g of every flavour of the multi-flavour
  * table, the quark from either beam (the two assignments have different matrix elements: the charge asymmetry).  Accepted
  * events carry the channel code of MF_PP_TT (0 gg; 1 + 2 i quark i from beam 1; 2 + 2 i from beam 2). */

@@ -148,7 +148,7 @@ void eval_event(mfo_process& P, const double* grid, uint64_t seed, uint32_t iter
     // quark channels: for every flavour the quark may come from either beam,
     //   sum_i [ q_i(x1) qbar_i(x2) |M|^2(q along +z) + qbar_i(x1) q_i(x2) |M|^2(q along -z) ] / (x1 x2),
     // added to the gg term at the same phase-space point.  Both are of the same order in alpha_s: the same R16 factor.
-    // Process 4: q qbar -> ttbar; process 7 (R21): q qbar -> ttbar g g, the 36 diagrams of amplitude_qq.hpp.
+    // Process 4: q qbar -> ttbar; process 7 (R22): q qbar -> ttbar g g, the 36 diagrams of amplitude_qq.hpp.
     R ma[6][4], mb[6][4];
     for (int i = 0; i < n + 2; ++i)
       for (int m = 0; m < 4; ++m) { ma[i][m] = cm[i][m]; mb[i][m] = cm[i][m]; }

@@ -37,7 +37,7 @@ template <> struct Traits<4> { static constexpr int D = 4, NF = 2, NG = 2, NGF =
 template <> struct Traits<5> { static constexpr int D = 14, NF = 3, NG = 3, NGF = 1; };
 // 6: gg -> ttbar ggg: RAMBO n = 5, 22 dimensions, cuts on three gluons
 template <> struct Traits<6> { static constexpr int D = 22, NF = 5, NG = 5, NGF = 3; };
-// 7: gg -> ttbar gg + q qbar -> ttbar gg (R21): kinematics and cuts of process 3
+// 7: gg -> ttbar gg + q qbar -> ttbar gg (R22): kinematics and cuts of process 3
 template <> struct Traits<7> { static constexpr int D = 18, NF = 4, NG = 4, NGF = 2; };
 constexpr int kMaxPartonTables = 11;   // gluon + up to 5 quark/antiquark pairs
 

@@ -202,7 +202,7 @@ MF_D double pp_ttj_terms(const Params& P, const PassArgs& A, const double* s_lnx
   return f1[0] * f2[0] * inv;
 }
 
-// pp -> ttbar gg (R21): the gluon-gluon luminosity (returned) and the flavour-summed quark term
+// pp -> ttbar gg (R22): the gluon-gluon luminosity (returned) and the flavour-summed quark term
 //   quark_sum = sum_i [ q_i(x1) qbar_i(x2) Ma + qbar_i(x1) q_i(x2) Mb ] / (x1 x2)   (x the R16 factor)
 // parts (optional, debug rows): the flavour-summed q qbar luminosity and the luminosity-weighted mean of Ma, Mb.
 MF_D double pp_ttgg_terms(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
@@ -366,7 +366,7 @@ __device__ __forceinline__ unsigned pp_ttj_channel(const Params& P, const PassAr
   return (unsigned)(6 * nf);
 }
 
-// pp -> ttbar gg (R21): the partonic channel of an ACCEPTED event, codes as for pp -> ttbar (0 gg; 1 + 2 i quark i
+// pp -> ttbar gg (R22): the partonic channel of an ACCEPTED event, codes as for pp -> ttbar (0 gg; 1 + 2 i quark i
 // from beam 1; 2 + 2 i quark i from beam 2), drawn as in pp_ttj_channel (the gluon channel's term is what w leaves).
 __device__ __forceinline__ unsigned pp_ttgg_channel(const Params& P, const PassArgs& A, const Event<7>& ev, double w, double v) {
   double f1[kMaxPartonTables], f2[kMaxPartonTables], asf;

@@ -1,6 +1,6 @@
 // mf_me_qqttgg.cuh — |M|^2 of q qbar -> t tbar g g, the quark channel of pp -> ttbar gg (PAPER.md L101 and
 // Table 1: 267 diagrams = 123 of g g -> t tbar g g + 36 for each of four massless flavours).  Used by the fused pass of
-// MF_PP_TTGG (mf_kernels_coop.cuh, R21) and by mf_debug_me2_qq_ttgg.
+// MF_PP_TTGG (mf_kernels_coop.cuh, R22) and by mf_debug_me2_qq_ttgg.
 //
 // Conventions of mf_me_prims.cuh (chiral two-component spinors, z-axis spin states for the top, helicity = chirality states for
 // the massless line, REAL linear gluon polarisations, all factors of i and g pulled out: M = i g^4 sum_s a_s S_s).

@@ -69,7 +69,7 @@ def channel_ids_ttj(channel):
 
 
 def channel_ids_ttgg(channel):
-    """PDG ids (beam 1, beam 2, t, tbar, g, g) and one valid colour flow of an MF_PP_TTGG record's channel code (R21): 0 = gg;
+    """PDG ids (beam 1, beam 2, t, tbar, g, g) and one valid colour flow of an MF_PP_TTGG record's channel code (R22): 0 = gg;
     1 + 2 i = quark i from beam 1 and its antiquark from beam 2; 2 + 2 i = the other way round"""
     c = int(channel)
     if c == 0:

@@ -1,6 +1,6 @@
 """GPU <-> oracle parity for pp -> ttbar gg = g g -> t tbar g g + q qbar -> t tbar g g of four flavours (process 7; SURVEY.md
 8(f2); Table 1: 267 diagrams) through the two C ABIs.  The gluon channel is the cooperative program of
-process 3, the quark channel the current-based csrc/mf_me_qqttgg.cuh on the owner threads; the oracle is the 36 diagrams with
+process 3, the quark channel the current-based csrc/mf_me_qqttgg.cuh in a thread-per-event kernel ahead of it; the oracle is the 36 diagrams with
 explicit colour tensors (oracle/amplitude_qq.hpp, 13 ms per event: it runs through tests/oracle_pool.py).  Tolerances of
 tests/test_gpu_parity.py: uniforms, bins, accept and channel draws bit-exact; |M|^2 and weights 1e-10; iteration sums 1e-9."""
 import math
@@ -101,7 +101,7 @@ def test_iteration_sums_edges_and_unweighting(gpu_procs, oracle_procs, oracle_po
             np.testing.assert_allclose(rec_g["w"][order], rec_o["w"], rtol=1e-10)
             scale = np.abs(rec_o["mom"]).max(axis=(1, 2), keepdims=True)
             assert np.max(np.abs(rec_g["mom"][order] - rec_o["mom"]) / scale) < 1e-11
-            # R21: the partonic channel, an integer decided in fp64 on both sides
+            # R22: the partonic channel, an integer decided in fp64 on both sides
             assert np.array_equal(rec_g["channel"][order], rec_o["channel"])
             ch = rec_o["channel"].astype(np.int64)
             assert ch.max() <= 2 * W.N_FLAVOURS and (ch == 0).any() and (ch > 0).sum() >= 3

@@ -100,6 +100,28 @@ def test_ttj_records_carry_their_partons():
         assert sorted(set(acol_in) - set(col_in)) == sorted(set(acol_out) - created)
 
 
+def test_ttgg_records_carry_their_partons():
+    """MF_PP_TTGG (R22): gg or q qbar of the record's flavour, the quark from either beam, with a colour-conserving flow"""
+    rec = np.zeros(5, dtype=lhe.record_dtype(4, 7))
+    assert rec.dtype.itemsize == 6 * 32 + 24
+    rec["channel"] = [0, 1, 2, 5, 8]
+    rec["w"] = 1.0
+    ev = _parse(lhe.format_events(rec, 7, 173.0, 173.0, 1 / 132.507, 0.118, w_max=1.0))
+    assert [[int(p[0]) for p in e[2]] for e in ev] == [[21, 21, 6, -6, 21, 21], [1, -1, 6, -6, 21, 21], [-1, 1, 6, -6, 21, 21],
+                                                       [3, -3, 6, -6, 21, 21], [-4, 4, 6, -6, 21, 21]]
+    for _, _, parts, _ in ev:
+        col_in = sorted(int(p[4]) for p in parts[:2] if int(p[4]))
+        acol_in = sorted(int(p[5]) for p in parts[:2] if int(p[5]))
+        col_out = sorted(int(p[4]) for p in parts[2:] if int(p[4]))
+        acol_out = sorted(int(p[5]) for p in parts[2:] if int(p[5]))
+        for p in parts:
+            pid, c, a = int(p[0]), int(p[4]), int(p[5])
+            assert (c != 0) == (pid == 21 or pid > 0) and (a != 0) == (pid == 21 or pid < 0)
+        created = set(col_out) & set(acol_out)
+        assert sorted(set(col_in) - set(acol_in)) == sorted(set(col_out) - created)
+        assert sorted(set(acol_in) - set(col_in)) == sorted(set(acol_out) - created)
+
+
 @pytest.mark.gpu
 def test_lhe_drain_flavour_summed(tmp_path):
     """the drain on MF_PP_TT records: every event of the file has the partons of its record's channel"""
