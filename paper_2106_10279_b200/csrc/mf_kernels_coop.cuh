@@ -83,6 +83,13 @@ __device__ __forceinline__ void coop_load_table(uint4* s_tab) {
 #ifndef MF_COOP_GROUP_WARP
 #define MF_COOP_GROUP_WARP 1
 #endif
+// MF_COOP_DECOUPLE = 1: group-level rounds (every lock-step group generates, ranks and queues its own threads' events; no block
+// barrier in the round).  Measured and rejected (profiles/r2_c3.md): g g -> t tbar g g 35.7 -> 41.9 ms, g g -> t tbar g 9.6 -> 11.4 ms,
+// pp -> t tbar j 30.8 -> 44.8 ms: with the groups in different phases the event-generation code and the matrix-element programs
+// compete for the instruction cache all the time.
+#ifndef MF_COOP_DECOUPLE
+#define MF_COOP_DECOUPLE 0
+#endif
 constexpr int kCoopGroup = MF_COOP_GROUP;            // teams of two warps (g g -> t tbar g g)
 constexpr int kCoopGroupWarp = MF_COOP_GROUP_WARP;   // teams of one warp (g g -> t tbar g, pp -> t tbar j)
 template <int THREADS>
@@ -96,11 +103,22 @@ __device__ __forceinline__ void coop_group_sync(int group) {
 template <class PG, int G>
 __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const uint4* tab, double* s_res,
                                                const double* queue, int total, double mt) {
+  (void)n_teams;
   const int team = threadIdx.x / PG::Team, tid = threadIdx.x % PG::Team, warp = tid >> 5, lane = tid & 31;
-#if MF_COOP_INTERLEAVE
+#if MF_COOP_DECOUPLE
+  // every group owns its part of the round (its own events, queue slice and ranks): the teams of a group take ranks
+  // member, member + G, ... of the GROUP's queue
+  const int group = team / G, member = team - group * G;
+  n_teams = G;
+  queue += group * (G * PG::Team);
+  s_res += PG::Warps * group * (G * PG::Team);
+  const int first = 0;
+#elif MF_COOP_INTERLEAVE
   const int n_groups = n_teams / G, group = team % n_groups, member = team / n_groups;   // groups {g, g + n_groups, ...}
+  const int first = group * G;
 #else
   const int group = team / G, member = team - group * G;
+  const int first = group * G;
 #endif
   double* tm = teams + team * PG::TeamDoubles;
   double* in = tm + PG::OffIn;
@@ -116,10 +134,10 @@ __device__ __forceinline__ void coop_team_loop(double* teams, int n_teams, const
     const int j = tid + i * PG::Team;
     dst[i] = j < PG::Queue ? PG::qdest(j) : -1;
     nxt[i] = 0.0;
-    if (group * G + member < total && dst[i] >= 0) nxt[i] = queue[j * qcap + group * G + member];
+    if (first + member < total && dst[i] >= 0) nxt[i] = queue[j * qcap + first + member];
   }
 #pragma unroll 1
-  for (int r0 = group * G; r0 < total; r0 += n_teams) {
+  for (int r0 = first; r0 < total; r0 += n_teams) {
     const int r = r0 + member;
     const bool active = r < total;
 #pragma unroll
@@ -153,11 +171,26 @@ template <class PG, int G>
 __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, const uint4* tab, unsigned* s_cnt,
                                                  double* s_res, double* queue, unsigned round, bool pass,
                                                  const double (*k)[4], double shat, const Params& P) {
+#if MF_COOP_DECOUPLE
+  // group-level rounds: the G teams of a lock-step group rank, queue and work through THEIR threads' events on their own
+  // (named barrier of the group; one-warp teams with G = 1: __syncwarp only), so the groups of a block drift into different
+  // phases: event generation (latency bound, special-function sequences) of one overlaps the matrix elements of the others,
+  // and no warp waits at a block barrier for another group's tail.
+  constexpr int GT = G * PG::Team;
+  const int grp = threadIdx.x / GT, gtid = threadIdx.x % GT, bwarp = gtid >> 5, lane = threadIdx.x & 31;
+  constexpr int n_warps = GT / 32;
+  unsigned* cnt = s_cnt + 32 * (round & 1u) + grp * n_warps;
+  auto gsync = [grp]() { coop_group_sync<GT>(grp); };
+  const int goff = grp * GT;
+#else
   const int bwarp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   unsigned* cnt = s_cnt + 32 * (round & 1u);
+  auto gsync = []() { __syncthreads(); };
+  const int goff = 0;
+#endif
   const unsigned bal = __ballot_sync(0xFFFFFFFFu, pass);
   if (lane == 0) cnt[bwarp] = __popc(bal);
-  __syncthreads();
+  gsync();
   int base = 0, total = 0;
   for (int w = 0; w < n_warps; ++w) {
     const int c = (int)cnt[w];
@@ -165,15 +198,15 @@ __device__ __forceinline__ double coop_block_me2(double* teams, int n_teams, con
     total += c;
   }
   const int rank = base + __popc(bal & ((1u << lane) - 1u));
-  if (pass) PG::owner_fill(queue + rank, blockDim.x, k, shat, P.m_top);
-  __syncthreads();
+  if (pass) PG::owner_fill(queue + goff + rank, blockDim.x, k, shat, P.m_top);
+  gsync();
   coop_team_loop<PG, G>(teams, n_teams, tab, s_res, queue, total, P.m_top);   // n_teams is a multiple of G
-  __syncthreads();
+  gsync();
   // top spin state 0 only: the other one gives the same sum (spin-flip symmetry), hence the factor 2
   double sum = 0.0;
   if (pass) {
 #pragma unroll
-    for (int w = 0; w < PG::Warps; ++w) sum += s_res[PG::Warps * rank + w];
+    for (int w = 0; w < PG::Warps; ++w) sum += s_res[PG::Warps * (goff + rank) + w];
   }
   return sum * (2.0 * P.me_norm / PG::Cden);
 }
