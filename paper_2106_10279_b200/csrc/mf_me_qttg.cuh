@@ -61,7 +61,7 @@ MF_HD void qttg_top_currents(const double p3[4], const double p4[4], const rvec&
       jtD[2 * a + b] = bilinear(ub3, spin_add_scaled(slash_col(t2, c1), mt, c1));
     }
 }
-// sum over the two chiralities of the massless light line and the four top spin states of K^dagger (3 S) K for one gluon
+// sum over the two chiralities of the massless light line (one evaluated, doubled) and the four top spin states of K^dagger (3 S) K for one gluon
 // polarisation e.  The light line runs from the column spinor (pcol, a v spinor if col_v; flow momentum into the line) to
 // the row spinor (prow, a vbar if row_v).  w[5] = the propagator weights of the five diagrams.
 MF_HD double qttg_light_sum(const double pcol[4], bool col_v, const double prow[4], bool row_v, const rvec& e, const rvec& a1,
@@ -73,8 +73,10 @@ MF_HD double qttg_light_sum(const double pcol[4], bool col_v, const double prow[
   //   3 S = {{8, -1, 7, -2, 9}, {-1, 8, -2, 7, -9}, {7, -2, 8, -1, 9}, {-2, 7, -1, 8, -9}, {9, -9, 9, -9, 18}}
   double total = 0.0;
   const double k12e = rdot(k12, e);
-#pragma unroll 1
-  for (int i = 0; i < 2; ++i) {          // the two chiralities of the massless light line
+  // Flipping the spin of every fermion conjugates the amplitudes (real polarisation e, real momenta), and the four top spin
+  // states below are closed under the flip: the right-handed light line gives the same sum as the left-handed one.
+  {
+    const int i = 0;
     const spin col = chiral_col(pcol, i, col_v);
     const spin row = bar_of(chiral_col(prow, i, row_v));
     const cvec jl = bilinear(row, col);
@@ -100,7 +102,7 @@ MF_HD double qttg_light_sum(const double pcol[4], bool col_v, const double prow[
                18.0 * (re_conj_mul(K[4], dd) + re_conj_mul(K[4], K[4])) + 0.5 * re_conj_mul(r, r);
     }
   }
-  return total;
+  return 2.0 * total;
 }
 
 // One class at caller-supplied momenta (mf_debug_me2_quark_gluon, tests/host_shim): kind 0 / 1 as in the header comment.
