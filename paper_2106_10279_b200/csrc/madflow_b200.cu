@@ -120,10 +120,10 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
       if (cudaMalloc(&p->d_quark, n_events * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(p, MF_ENOMEM, "quark-term buffer"); }
       p->quark_cap = n_events;
     }
-    const size_t smem = (size_t)(p->D * (p->P.n_bins + 1) + (1 + p->P.pdf_nfl) * p->P.pdf_nx) * sizeof(double);
-    const uint64_t want = (n_events + mf::kThreads - 1) / mf::kThreads;
+    const size_t smem = (size_t)mf::prepass_smem_doubles(p->D, p->P.n_bins, p->P.pdf_nx, p->P.pdf_nfl) * sizeof(double);
+    const uint64_t want = (n_events + mf::kPrepassThreads - 1) / mf::kPrepassThreads;
     const unsigned pre_blocks = (unsigned)(want < (uint64_t)p->prepass_blocks ? want : (uint64_t)p->prepass_blocks);
-    mf::quark_prepass_kernel<7><<<pre_blocks, mf::kThreads, smem, st>>>(p->P, A, p->d_quark);
+    mf::quark_prepass_kernel<7><<<pre_blocks, mf::kPrepassThreads, smem, st>>>(p->P, A, p->d_quark);
     cudaError_t pe = cudaGetLastError();
     if (pe != cudaSuccess) return fail(p, MF_ECUDA, "quark prepass launch", pe);
     A.quark_terms = p->d_quark;
@@ -248,7 +248,15 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   if (e != cudaSuccess || per_sm < 1 || per_sm_unw < 1) { free_all(p); delete p; cudaGetLastError(); return MF_ECUDA; }
   p->blocks = prop.multiProcessorCount * per_sm;
   p->blocks_unw = prop.multiProcessorCount * per_sm_unw;
-  p->prepass_blocks = prop.multiProcessorCount * MF_PREPASS_BLOCKS;
+  p->prepass_blocks = prop.multiProcessorCount;
+  if (p->process == MF_PP_TTGG) {
+    const int need = mf::prepass_smem_doubles(p->D, P.n_bins, P.pdf_nx, P.pdf_nfl) * (int)sizeof(double);
+    if (need > (int)prop.sharedMemPerBlockOptin) { free_all(p); delete p; return MF_EINVAL; }
+    if (cudaFuncSetAttribute((const void*)mf::quark_prepass_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)prop.sharedMemPerBlockOptin) != cudaSuccess) {
+      free_all(p); delete p; cudaGetLastError(); return MF_ECUDA;
+    }
+  }
   const int max_blocks = p->blocks > p->blocks_unw ? p->blocks : p->blocks_unw;
   if ((e = cudaMalloc(&p->d_partials, (size_t)max_blocks * sizeof(mf::BlockPartial))) != cudaSuccess ||
       (e = cudaMalloc(&p->d_hist_part, (size_t)max_blocks * p->D * P.n_bins * 8)) != cudaSuccess) {

@@ -205,12 +205,13 @@ MF_D double pp_ttj_terms(const Params& P, const PassArgs& A, const double* s_lnx
 // pp -> ttbar gg (R22): the gluon-gluon luminosity (returned) and the flavour-summed quark term
 //   quark_sum = sum_i [ q_i(x1) qbar_i(x2) Ma + qbar_i(x1) q_i(x2) Mb ] / (x1 x2)   (x the R16 factor)
 // parts (optional, debug rows): the flavour-summed q qbar luminosity and the luminosity-weighted mean of Ma, Mb.
-MF_D double pp_ttgg_terms(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
-                          const Event<7>& ev, double& asf, double& quark_sum, double* parts) {
+MF_D double quark_pair_luminosities(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                                    const Event<7>& ev, double& asf, double& La, double& Lb) {
   double f1[kMaxPartonTables], f2[kMaxPartonTables];
   parton_densities<7>(P, A, s_lnx, s_row, ev, f1, f2, asf);
   const int nt = P.pdf_nfl;
-  double La = 0.0, Lb = 0.0;
+  La = 0.0;
+  Lb = 0.0;
 #pragma unroll
   for (int t = 1; t + 1 < kMaxPartonTables; t += 2)
     if (t + 1 < nt) {
@@ -220,6 +221,12 @@ MF_D double pp_ttgg_terms(const Params& P, const PassArgs& A, const double* s_ln
   const double inv = 1.0 / (ev.x1 * ev.x2);
   La *= inv;
   Lb *= inv;
+  return f1[0] * f2[0] * inv;
+}
+MF_D double pp_ttgg_terms(const Params& P, const PassArgs& A, const double* s_lnx, const double* s_row,
+                          const Event<7>& ev, double& asf, double& quark_sum, double* parts) {
+  double La, Lb;
+  const double lum = quark_pair_luminosities(P, A, s_lnx, s_row, ev, asf, La, Lb);
   double M[2];
   quark_pair_me2_gg(P, ev.shat, ev.k, M);
   const double both = La * (M[0] * asf) + Lb * (M[1] * asf);
@@ -228,7 +235,7 @@ MF_D double pp_ttgg_terms(const Params& P, const PassArgs& A, const double* s_ln
     parts[1] = (La + Lb) != 0.0 ? both / (La + Lb) : M[0] * asf;
   }
   quark_sum = both;
-  return f1[0] * f2[0] * inv;
+  return lum;
 }
 
 // a6-a10 of one event that passed the cuts (thread-per-event kernels): luminosity, |M|^2, weight.
@@ -553,39 +560,89 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
   block_finish(A, acc, s_red, s_hist, D * nb);
 }
 
-// ---- pp -> ttbar gg: the quark channel, one thread per event, BEFORE the cooperative pass ---------------------------------
-// out[i] = sum over the quark channels of luminosity x |M|^2 (x the R16 factor) of event first_event + i (0 if it fails the cuts):
-// the term the cooperative pass adds to  L_gg |M_gg|^2.  The quark matrix elements are thread-per-event code with hundreds of
-// live values; inside the cooperative kernels (168 registers, 231 kB of shared memory, so almost no L1) they ran out of
-// local memory at a fraction of the FP64 rate.  Here: 255 registers, 15 kB of shared memory, the rest of the SM's 256 kB as L1.
-#ifndef MF_PREPASS_BLOCKS
-#define MF_PREPASS_BLOCKS 2
-#endif
+// ---- pp -> ttbar gg: the quark channel, BEFORE the cooperative pass ---------------------------------------------------------
+// out[i] = sum over the flavours and the two beam assignments of luminosity x |M(q qbar -> t tbar g g)|^2 (x the R16 factor) of
+// event first_event + i (0 if it fails the cuts): the term the cooperative pass adds to  L_gg |M_gg|^2.
+// Thread = event for a1-a6; the matrix element of every event that passed is then evaluated by a whole WARP
+// (me2_qq_ttgg_warp: lane = beam assignment x polarisation pair x top spin state, the light line's currents shared through
+// 7.4 kB of shared memory per warp, everything else in registers).  As thread-per-event code (~4 kB of thread-local state per
+// event) it ran from local memory: 350 ms per 2^22 events on the owner threads of the cooperative kernel, 103 ms in a
+// thread-per-event kernel of its own (profiles/r2_c8.md).
+// The block's warps step through the block's passing events together (ranked queue in shared memory, one block barrier per
+// step): the matrix element is ~7000 straight-line instructions executed once per event, and without the lock-step the warps
+// of an SM were each waiting for their own instruction fetches (ncu: 5.5 warps per issue stalled on no_instruction).
+constexpr int kPrepassThreads = 256;
+constexpr int kPrepassWarpDoubles = kQQWarpSharedDoubles + 8 * kQQLStride;   // a warp's shared kinematics and light-line currents
+__host__ __device__ inline int prepass_smem_doubles(int D, int nb, int nx, int nfl) {
+  return D * (nb + 1) + nx + nfl * nx + kPrepassThreads * (17 + 2) + 32 + (kPrepassThreads / 32) * kPrepassWarpDoubles;
+}
 template <int PROC>
-__global__ void __launch_bounds__(kThreads, MF_PREPASS_BLOCKS) quark_prepass_kernel(const Params P, const PassArgs A, double* out) {
-  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+__global__ void __launch_bounds__(kPrepassThreads, 1) quark_prepass_kernel(const Params P, const PassArgs A, double* out) {
+  static_assert(PROC == 7, "the prepass serves pp -> ttbar gg");
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF, NW = kPrepassThreads / 32;
   extern __shared__ double smem[];
   const int nb = P.n_bins, nx = P.pdf_nx, nrow = nx * P.pdf_nfl;
   double* s_grid = smem;                    // D*(nb+1)
   double* s_lnx = s_grid + D * (nb + 1);    // nx
   double* s_row = s_lnx + nx;               // one row per parton table
+  double* s_ev = s_row + nrow;              // [rank][17]: momenta and shat of the block's passing events
+  double* s_res = s_ev + kPrepassThreads * 17;                       // [rank][2]
+  unsigned* s_cnt = reinterpret_cast<unsigned*>(s_res + kPrepassThreads * 2);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double* s_warp = reinterpret_cast<double*>(s_cnt) + 32 + warp * kPrepassWarpDoubles;
+  QQWarpShared* s_sh = reinterpret_cast<QQWarpShared*>(s_warp);
+  double* s_L = s_warp + kQQWarpSharedDoubles;
   for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < nx; i += blockDim.x) s_lnx[i] = A.pdf_lnx[i];
   for (int i = threadIdx.x; i < nrow; i += blockDim.x) s_row[i] = A.pdf_row[i];
   __syncthreads();
+  const double g2 = 4.0 * kPi * P.alpha_s;
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-  for (uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < A.n_events; idx += stride) {
-    Bins<PROC> bins;
+  const uint64_t rounds = (A.n_events + stride - 1) / stride;
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (uint64_t rd = 0; rd < rounds; ++rd, idx += stride) {
+    const bool valid = idx < A.n_events;
+    bool pass = false;
+    double La = 0.0, Lb = 0.0, asf = 1.0;
     Event<PROC> ev;
-    DebugRow dbg = {nullptr, D, NF};
-    generate_event<PROC>(P, s_grid, A.seed, A.iteration, A.first_event + idx, ev, bins, dbg);
-    double quark_sum = 0.0;
-    if (ev.pass) {
-      double asf;
-      if constexpr (PROC == 5) pp_ttj_terms(P, A, s_lnx, s_row, ev, asf, quark_sum, nullptr);
-      else pp_ttgg_terms(P, A, s_lnx, s_row, ev, asf, quark_sum, nullptr);
+    if (valid) {
+      Bins<PROC> bins;
+      DebugRow dbg = {nullptr, D, NF};
+      generate_event<PROC>(P, s_grid, A.seed, A.iteration, A.first_event + idx, ev, bins, dbg);
+      pass = ev.pass;
+      if (pass) quark_pair_luminosities(P, A, s_lnx, s_row, ev, asf, La, Lb);
     }
-    out[idx] = quark_sum;
+    // rank the block's passing events (ballot + prefix over the warps) and queue their records
+    const unsigned bal = __ballot_sync(0xFFFFFFFFu, pass);
+    if (lane == 0) s_cnt[warp] = __popc(bal);
+    __syncthreads();
+    int base = 0, total = 0;
+    for (int w = 0; w < NW; ++w) {
+      const int c = (int)s_cnt[w];
+      if (w < warp) base += c;
+      total += c;
+    }
+    const int rank = base + __popc(bal & ((1u << lane) - 1u));
+    if (pass) {
+#pragma unroll
+      for (int f = 0; f < 4; ++f)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) s_ev[17 * rank + 4 * f + c] = ev.k[f][c];
+      s_ev[17 * rank + 16] = ev.shat;
+    }
+#pragma unroll 1
+    for (int r0 = 0; r0 < total; r0 += NW) {
+      __syncthreads();                       // (first turn: the queue is complete) keeps the warps on the same code
+      const int r = r0 + warp;
+      if (r < total) {
+        double m0, m1;
+        me2_qq_ttgg_warp(s_ev + 17 * r, s_sh, s_L, lane, P.m_top, g2, m0, m1);
+        if (lane == 0) { s_res[2 * r] = m0; s_res[2 * r + 1] = m1; }
+      }
+    }
+    __syncthreads();
+    if (valid) out[idx] = pass ? La * (s_res[2 * rank] * asf) + Lb * (s_res[2 * rank + 1] * asf) : 0.0;
+    __syncthreads();                         // the queue and the counters are rewritten in the next round
   }
 }
 

@@ -185,13 +185,17 @@ MF_HD void qq_assemble(const cvec L[13], const spin& row, const spin& col, const
 #include "mf_me_qqttgg_colour_generated.cuh"
 namespace mf {
 
-// Averaged |M|^2 of q(p1) qbar(p2) -> t(p3) tbar(p4) g(k5) g(k6) at CM-frame momenta: 1/(4 x 9) for spins and colours of the
-// initial state, 1/2! for the identical gluons, g2 = 4 pi alpha_s.  Flipping every fermion spin conjugates the amplitude (real
-// polarisations; DESIGN.md), so only the left-handed light line is evaluated and the sum doubled.
-MF_HD double me2_qq_ttgg(const double p1[4], const double p2[4], const double p3[4], const double p4[4], const double k5[4],
-                         const double k6[4], double mt, double g2) {
-  rvec ka, kb, pcl, prl, pct, prt;
+// kinematics of one phase-space point and beam assignment: everything that does not depend on the helicities
+struct QQPoint {
   QQKin q;
+  QQLineKin kl, kt;
+  rvec Ea[2], Eb[2];
+  double isab;
+};
+MF_HD void qq_point(const double p1[4], const double p2[4], const double p3[4], const double p4[4], const double k5[4],
+                    const double k6[4], double mt, QQPoint& pt) {
+  rvec ka, kb, pcl, prl, pct, prt;
+  QQKin& q = pt.q;
 #pragma unroll
   for (int m = 0; m < 4; ++m) {
     ka.v[m] = k5[m]; kb.v[m] = k6[m];
@@ -208,30 +212,119 @@ MF_HD double me2_qq_ttgg(const double p1[4], const double p2[4], const double p3
   q.iB = 1.0 / rdot(PT0, PT0);
   q.iCa = 1.0 / rdot(q.PLa, q.PLa);
   q.iCb = 1.0 / rdot(q.PLb, q.PLb);
-  const double isab = 1.0 / rdot(q.K, q.K);
-  const QQLineKin kl = qq_line_kin(pcl, prl, ka, kb, 0.0), kt = qq_line_kin(pct, prt, ka, kb, mt);
-  rvec Ea[2], Eb[2];
-  pol_vectors(k5, Ea[0], Ea[1]);
-  pol_vectors(k6, Eb[0], Eb[1]);
+  pt.isab = 1.0 / rdot(q.K, q.K);
+  pt.kl = qq_line_kin(pcl, prl, ka, kb, 0.0);
+  pt.kt = qq_line_kin(pct, prt, ka, kb, mt);
+  pol_vectors(k5, pt.Ea[0], pt.Ea[1]);
+  pol_vectors(k6, pt.Eb[0], pt.Eb[1]);
+}
+MF_HD rvec qq_merged(const QQKin& q, double isab, const rvec& ea, const rvec& eb) {   // hatted three-gluon merger of the two gluons
+  rvec G = {{0.0, 0.0, 0.0, 0.0}};
+  v3_acc(G, 1.0, ea, q.mka, eb, q.mkb);
+  return rscale(G, isab);
+}
+
+// Averaged |M|^2 of q(p1) qbar(p2) -> t(p3) tbar(p4) g(k5) g(k6) at CM-frame momenta: 1/(4 x 9) for spins and colours of the
+// initial state, 1/2! for the identical gluons, g2 = 4 pi alpha_s.  Flipping every fermion spin conjugates the amplitude (real
+// polarisations; DESIGN.md), so only the left-handed light line is evaluated and the sum doubled.
+MF_HD double me2_qq_ttgg(const double p1[4], const double p2[4], const double p3[4], const double p4[4], const double k5[4],
+                         const double k6[4], double mt, double g2) {
+  QQPoint pt;
+  qq_point(p1, p2, p3, p4, k5, k6, mt, pt);
   const spin lcol = chiral_col(p1, 0, false), lrow = bar_of(chiral_col(p2, 0, true));
   double total = 0.0;
 #pragma unroll 1
   for (int pol = 0; pol < 4; ++pol) {
-    const rvec ea = Ea[pol & 1], eb = Eb[pol >> 1];
-    rvec G = {{0.0, 0.0, 0.0, 0.0}};
-    v3_acc(G, 1.0, ea, q.mka, eb, q.mkb);
-    G = rscale(G, isab);
+    const rvec ea = pt.Ea[pol & 1], eb = pt.Eb[pol >> 1];
+    const rvec G = qq_merged(pt.q, pt.isab, ea, eb);
     cvec L[13];
-    qq_line_currents(lrow, lcol, kl, ea, eb, G, L);
+    qq_line_currents(lrow, lcol, pt.kl, ea, eb, G, L);
 #pragma unroll 1
     for (int st = 0; st < 4; ++st) {
       cplx a[20];
-      qq_assemble(L, ubar_row(p3, mt, st >> 1), v_col(p4, mt, st & 1), kt, ea, eb, G, q, a);
+      qq_assemble(L, ubar_row(p3, mt, st >> 1), v_col(p4, mt, st & 1), pt.kt, ea, eb, G, pt.q, a);
       total += qq_colour_square(a);
     }
   }
   const double g4 = g2 * g2;
   return 2.0 * total * g4 * g4 / 72.0;
 }
+
+#if defined(__CUDACC__)
+// The same matrix element by ONE WARP per event, both beam assignments at once (quark_prepass_kernel): lane = beam assignment o
+// (bit 4), polarisation pair (bits 2-3), top spin state st (bits 0-1).  The four lanes of an (o, polarisation pair) share its 13
+// light-line currents through shared memory (each stores a quarter of them); every lane then streams its own top-line currents
+// against them, forms its 20 string coefficients and the colour form in registers; the 16 lanes of an assignment are summed by
+// shuffles.
+constexpr int kQQLStride = 106;        // 13 currents x 8 doubles, padded: the 8 groups' broadcast reads fall into different banks
+// what does not depend on the lane, nor on the beam assignment (the top line's and the virtual gluon's kinematics, the
+// polarisation vectors): formed by lane 0, read by all from shared memory when needed (76 doubles that would otherwise sit in
+// every lane's registers)
+struct QQWarpShared {
+  QQKin q;
+  QQLineKin kt;
+  rvec Ea[2], Eb[2];
+  double isab;
+};
+constexpr int kQQWarpSharedDoubles = (sizeof(QQWarpShared) + 7) / 8;
+__device__ __forceinline__ void qq_store(double* dst, const cvec& c) {
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { dst[m] = c.re[m]; dst[4 + m] = c.im[m]; }
+}
+// ev = the event's four final-state momenta and shat (17 doubles), sh and Ls[8 x kQQLStride]: the warp's shared memory
+__device__ __forceinline__ void me2_qq_ttgg_warp(const double* ev, QQWarpShared* sh, double* Ls, int lane, double mt, double g2,
+                                                 double& m0, double& m1) {
+  const int o = lane >> 4, pol = (lane >> 2) & 3, st = lane & 3;
+  const double E = 0.5 * sqrt(ev[16]), pz = o == 0 ? E : -E;
+  const double p1[4] = {E, 0.0, 0.0, pz}, p2[4] = {E, 0.0, 0.0, -pz};
+  if (lane == 0) {
+    QQPoint pt;
+    qq_point(p1, p2, ev, ev + 4, ev + 8, ev + 12, mt, pt);
+    sh->q = pt.q; sh->kt = pt.kt; sh->isab = pt.isab;
+    sh->Ea[0] = pt.Ea[0]; sh->Ea[1] = pt.Ea[1]; sh->Eb[0] = pt.Eb[0]; sh->Eb[1] = pt.Eb[1];
+  }
+  __syncwarp();
+  const rvec ea = sh->Ea[pol & 1], eb = sh->Eb[pol >> 1];
+  const rvec G = qq_merged(sh->q, sh->isab, ea, eb);
+  {
+    // the light line's 13 currents: every lane of an (o, polarisation pair) forms them all (the same instructions for the whole
+    // warp: four different code paths would be executed one after the other) and stores its quarter
+    rvec pcl, prl, ka, kb;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) { pcl.v[m] = p1[m]; prl.v[m] = -p2[m]; ka.v[m] = ev[8 + m]; kb.v[m] = ev[12 + m]; }
+    const QQLineKin k = qq_line_kin(pcl, prl, ka, kb, 0.0);
+    const spin col = chiral_col(p1, 0, false), row = bar_of(chiral_col(p2, 0, true));
+    double* L = Ls + (lane >> 2) * kQQLStride;
+    const spin ca = prop_col(k.qa, k.m, k.ia, slash_col(ea, col)), cb = prop_col(k.qb, k.m, k.ib, slash_col(eb, col));
+    const spin ra = prop_row(slash_row(row, ea), k.ra, k.m, k.ja), rb = prop_row(slash_row(row, eb), k.rb, k.m, k.jb);
+    auto put = [&](int i, const cvec& c) { if ((i & 3) == st) qq_store(L + 8 * i, c); };
+    put(0, bilinear(row, col));
+    put(1, bilinear(row, ca));
+    put(2, bilinear(ra, col));
+    put(3, bilinear(row, cb));
+    put(4, bilinear(rb, col));
+    put(5, bilinear(row, prop_col(k.qab, k.m, k.iab, slash_col(ea, cb))));
+    put(6, bilinear(row, prop_col(k.qab, k.m, k.iab, slash_col(eb, ca))));
+    put(7, bilinear(ra, cb));
+    put(8, bilinear(rb, ca));
+    put(9, bilinear(prop_row(slash_row(ra, eb), k.rab, k.m, k.jab), col));
+    put(10, bilinear(prop_row(slash_row(rb, ea), k.rab, k.m, k.jab), col));
+    put(11, bilinear(row, prop_col(k.qab, k.m, k.iab, slash_col(G, col))));
+    put(12, bilinear(prop_row(slash_row(row, G), k.rab, k.m, k.jab), col));
+  }
+  __syncwarp();
+  cplx a[20];
+  qq_assemble(reinterpret_cast<const cvec*>(Ls + (lane >> 2) * kQQLStride), ubar_row(ev, mt, st >> 1), v_col(ev + 4, mt, st & 1), sh->kt,
+              ea, eb, G, sh->q, a);
+  double v = qq_colour_square(a);
+#pragma unroll
+  for (int d = 1; d < 16; d <<= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, d);
+  const double g4 = g2 * g2;
+  v *= 2.0 * g4 * g4 / 72.0;
+  m0 = __shfl_sync(0xFFFFFFFFu, v, 0);
+  m1 = __shfl_sync(0xFFFFFFFFu, v, 16);
+  __syncwarp();
+}
+#endif
 
 }  // namespace mf

@@ -1,6 +1,6 @@
 """GPU <-> oracle parity for pp -> ttbar gg = g g -> t tbar g g + q qbar -> t tbar g g of four flavours (process 7; SURVEY.md
 8(f2); Table 1: 267 diagrams) through the two C ABIs.  The gluon channel is the cooperative program of
-process 3, the quark channel the current-based csrc/mf_me_qqttgg.cuh in a thread-per-event kernel ahead of it; the oracle is the 36 diagrams with
+process 3, the quark channel the current-based csrc/mf_me_qqttgg.cuh by one warp per event in a kernel ahead of it; the oracle is the 36 diagrams with
 explicit colour tensors (oracle/amplitude_qq.hpp, 13 ms per event: it runs through tests/oracle_pool.py).  Tolerances of
 tests/test_gpu_parity.py: uniforms, bins, accept and channel draws bit-exact; |M|^2 and weights 1e-10; iteration sums 1e-9."""
 import math
