@@ -347,7 +347,10 @@ def test_pipeline_reduced_n(proc, n, n_it, gpu_procs, oracle_procs, oracle_pool)
         assert abs(rec.sigma - so) <= REL_ITER * so, (k, rec.sigma, so)
         np.testing.assert_allclose(hists[k], ho, rtol=1e-8, atol=1e-14 * ho.max())
         grid = op.refine_grid(grid, ho, W.VEGAS_ALPHA)
-    np.testing.assert_allclose(run.grid.cpu().numpy(), grid, rtol=0, atol=1e-11)
+    # the two final grids come from independently refined pipelines whose histograms agree to 1e-9, not bitwise (shared-memory
+    # fp64 atomics: order dependent): DESIGN.md section 3 "Other readings", 5e-10 absolute after five refinements (as in
+    # tests/test_gpu_c4.py); seen: 1.2e-11 for g g -> t tbar g g in a full-suite run, below 1e-11 when the test runs alone
+    np.testing.assert_allclose(run.grid.cpu().numpy(), grid, rtol=0, atol=5e-10)
 
 
 def test_c0_closed_form(gpu_procs):
