@@ -98,6 +98,21 @@ int mf_launch_config(const mf_process *p, int32_t *blocks, int32_t *threads);
 int mf_vegas_iterate(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                      uint64_t n_events, double *d_hist, mf_iter_result *d_result, void *stream);
 
+/* mf_vegas_iterate for callers that must not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * same arguments, same kernels, same results; the per-block partial sums and histogram slices of the launch live in a file-scope
+ * `static __device__` array of MF_STATIC_SCRATCH_BYTES inside the library (held by every GPU that loads it, until exit) instead of
+ * the handle's buffers.  The call itself calls no cudaMalloc / cudaFree or allocating library routine (the handle was created,
+ * and the array's device address looked up, at set-up in mf_create_process).
+ * Limits: MF_EE_MUMU, MF_GG_TT and MF_PP_TT handles only (the cooperative kernels queue events in tens of MB), and
+ *   launch blocks x (40 + 8 D n_bins) bytes <= MF_STATIC_SCRATCH_BYTES  (e.g. MF_GG_TT with 50 bins: 0.97 MB; with 128 bins: refused);
+ * anything else returns MF_EINVAL with the reason in mf_last_error.
+ * Every call on a device shares the one array, from every handle and stream: two calls that overlap on the GPU race (keep
+ * them on one stream, or order them with events).  The array keeps the last call's contents; nothing in it has to start at
+ * zero, every block overwrites its part before it is read. */
+#define MF_STATIC_SCRATCH_BYTES (2 * 1024 * 1024)
+int mf_vegas_iterate_static(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                            uint64_t n_events, double *d_hist, mf_iter_result *d_result, void *stream);
+
 /* VEGAS grid refinement (step a13; the integration is VEGAS importance sampling, whose grid adapts between
  * iterations; Lepage's smoothing + damping r = ((s-1)/ln s)^alpha + rebinning), in
  * place on d_grid from d_hist.  A dimension whose histogram is all zero is left unchanged. */

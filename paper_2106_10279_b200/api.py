@@ -26,7 +26,7 @@ c_double_p = C.POINTER(C.c_double)
 
 # every symbol include/mf.h declares (tests check the library exports each one)
 EXPORTS = ["mf_create_process", "mf_destroy_process", "mf_n_dims", "mf_n_final", "mf_record_size",
-           "mf_debug_row_len", "mf_last_error", "mf_launch_config", "mf_vegas_iterate", "mf_refine_grid",
+           "mf_debug_row_len", "mf_last_error", "mf_launch_config", "mf_vegas_iterate", "mf_vegas_iterate_static", "mf_refine_grid",
            "mf_unweight", "mf_set_dynamic_scale", "mf_set_observables", "mf_debug_eval", "mf_debug_philox", "mf_debug_pdf", "mf_debug_me2",
            "mf_debug_me2_quark_gluon", "mf_measure_fp64_peak", "mf_measure_dmma_peak"]
 
@@ -67,6 +67,7 @@ def lib():
         L.mf_last_error.restype = C.c_char_p
         L.mf_launch_config.argtypes = [vp, i32p, i32p]
         L.mf_vegas_iterate.argtypes = [vp, vp, u64, u32, u64, u64, vp, vp, vp]
+        L.mf_vegas_iterate_static.argtypes = [vp, vp, u64, u32, u64, u64, vp, vp, vp]
         L.mf_refine_grid.argtypes = [vp, vp, vp, C.c_double, vp]
         L.mf_unweight.argtypes = [vp, vp, u64, u32, u64, u64, C.c_double, vp, u64, vp, vp, vp, vp]
         L.mf_set_observables.argtypes = [vp, vp, C.c_int32, C.c_double, C.c_double]
@@ -101,6 +102,10 @@ def mf_destroy_process(h):
 
 def mf_vegas_iterate(h, d_grid, seed, iteration, first_event, n_events, d_hist, d_result, stream=0):
     return lib().mf_vegas_iterate(h, d_grid, seed, iteration, first_event, n_events, d_hist, d_result, stream)
+
+
+def mf_vegas_iterate_static(h, d_grid, seed, iteration, first_event, n_events, d_hist, d_result, stream=0):
+    return lib().mf_vegas_iterate_static(h, d_grid, seed, iteration, first_event, n_events, d_hist, d_result, stream)
 
 
 def mf_refine_grid(h, d_grid, d_hist, alpha, stream=0):
@@ -230,6 +235,12 @@ class Process:
         _check(mf_vegas_iterate(self.h, grid.data_ptr(), seed, iteration, first_event, n_events,
                                 hist.data_ptr() if hist is not None else None, result.data_ptr(),
                                 _stream_ptr(stream)), self.h, "mf_vegas_iterate")
+
+    def vegas_iterate_static(self, grid, seed, iteration, first_event, n_events, hist, result, stream=None):
+        """mf_vegas_iterate with the launch's scratch in the library's static device array: allocates nothing (include/mf.h)"""
+        _check(mf_vegas_iterate_static(self.h, grid.data_ptr(), seed, iteration, first_event, n_events,
+                                       hist.data_ptr() if hist is not None else None, result.data_ptr(),
+                                       _stream_ptr(stream)), self.h, "mf_vegas_iterate_static")
 
     def refine_grid(self, grid, hist, alpha=1.5, stream=None):
         _check(mf_refine_grid(self.h, grid.data_ptr(), hist.data_ptr(), alpha, _stream_ptr(stream)), self.h,

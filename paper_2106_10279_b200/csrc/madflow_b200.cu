@@ -12,6 +12,12 @@
 #include "mf_kernels_coop.cuh"
 #include "mf_kernels_cta.cuh"
 
+// Scratch of mf_vegas_iterate_static (include/mf.h): per-block partial sums and histogram slices of ONE fused-pass launch.
+// File scope, so every GPU that loads the library holds these MF_STATIC_SCRATCH_BYTES until exit.  In host code this name is a
+// host-side stand-in, NOT a device address: the address kernels may use comes from cudaGetSymbolAddress (mf_create_process,
+// once per handle, with the handle's device current).
+static __device__ __align__(256) unsigned char mf_static_scratch[MF_STATIC_SCRATCH_BYTES];
+
 static_assert(sizeof(mf::IterResult) == sizeof(mf_iter_result), "result layouts must agree");
 static_assert(mf::kMaxBins == MF_MAX_BINS, "bin limits must agree");
 
@@ -21,6 +27,7 @@ struct mf_process {
   double *d_lnx = nullptr, *d_lnq2 = nullptr, *d_xf = nullptr, *d_row = nullptr;  // PDF table + collapsed row
   mf::BlockPartial* d_partials = nullptr;
   double* d_queue = nullptr;          // cooperative pass: per-block momenta queue
+  unsigned char* d_static = nullptr;  // device address of mf_static_scratch on the handle's device (cudaGetSymbolAddress)
   double* d_quark = nullptr;          // MF_PP_TTGG: quark-channel term per event of the current launch (grown on demand)
   uint64_t quark_cap = 0;
   double* d_obs = nullptr;            // caller-owned observable histograms (mf_set_observables) or NULL
@@ -218,6 +225,9 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     free_all(p); delete p; cudaGetLastError(); return MF_ECUDA;
   }
   p->device = dev;
+  if ((e = cudaGetSymbolAddress((void**)&p->d_static, mf_static_scratch)) != cudaSuccess || p->d_static == nullptr) {
+    free_all(p); delete p; cudaGetLastError(); return MF_ECUDA;
+  }
   const bool coop = p->process == 2 || p->process == 3 || p->process == 5 || p->process == 7;
   if (coop) {
     // cooperative pass: as many teams per block as the SM's shared memory holds, one block per SM
@@ -317,6 +327,44 @@ int mf_vegas_iterate(mf_process* p, const double* d_grid, uint64_t seed, uint32_
                      uint64_t n_events, double* d_hist, mf_iter_result* d_result, void* stream) {
   return run_pass(p, false, d_grid, seed, iteration, first_event, n_events, 0.0, nullptr, 0, nullptr, d_hist, d_result,
                   stream);
+}
+
+int mf_vegas_iterate_static(mf_process* p, const double* d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
+                            uint64_t n_events, double* d_hist, mf_iter_result* d_result, void* stream) {
+  if (!p) return MF_EINVAL;
+  if (!d_grid || !d_result) return fail(p, MF_EINVAL, "d_grid and d_result must not be NULL");
+  if (p->process != MF_EE_MUMU && p->process != MF_GG_TT && p->process != MF_PP_TT)
+    return fail(p, MF_EINVAL, "mf_vegas_iterate_static: thread-per-event processes only (MF_EE_MUMU, MF_GG_TT, MF_PP_TT); "
+                              "the others queue events in tens of MB of scratch");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device)
+    return fail(p, MF_EINVAL, "the handle belongs to another device than the current one");
+  const int blocks = p->blocks, n_hist = p->D * p->P.n_bins;
+  const size_t off_hist = ((size_t)blocks * sizeof(mf::BlockPartial) + 255) & ~(size_t)255;
+  const size_t need = off_hist + (size_t)blocks * n_hist * sizeof(double);
+  if (need > (size_t)MF_STATIC_SCRATCH_BYTES) {
+    snprintf(p->err, sizeof(p->err), "mf_vegas_iterate_static: %d blocks x %d histogram bins need %zu bytes of scratch, the static "
+             "array holds %d (use fewer bins, or mf_vegas_iterate)", blocks, n_hist, need, (int)MF_STATIC_SCRATCH_BYTES);
+    return MF_EINVAL;
+  }
+  mf::PassArgs A;
+  std::memset(&A, 0, sizeof(A));
+  A.grid = d_grid; A.pdf_lnx = p->d_lnx; A.pdf_row = p->d_row; A.pdf_lnq2 = p->d_lnq2; A.pdf_xf = p->d_xf;
+  A.seed = seed; A.first_event = first_event; A.n_events = n_events; A.iteration = iteration;
+  // nothing in the scratch has to start at zero: every block of the pass overwrites its partial and its whole histogram slice
+  // before finalize_kernel (next on the stream) reads them, so the previous call's contents are never seen
+  A.partials = reinterpret_cast<mf::BlockPartial*>(p->d_static);
+  A.hist_part = d_hist ? reinterpret_cast<double*>(p->d_static + off_hist) : nullptr;
+  A.obs = p->d_obs; A.obs_nb = p->obs_nb; A.obs_ptmax = p->obs_ptmax; A.obs_etamax = p->obs_etamax;
+  cudaStream_t st = (cudaStream_t)stream;
+  void* args[2] = {(void*)&p->P, (void*)&A};
+  cudaError_t e = cudaLaunchKernel(pass_fn(p->process, false), dim3(blocks), dim3(p->threads), args, p->smem, st);
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "fused pass launch", e);
+  mf::finalize_kernel<<<(n_hist + 255) / 256 + 1, 256, 0, st>>>(A.partials, A.hist_part, blocks, n_hist, d_hist,
+                                                               (mf::IterResult*)d_result);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(p, MF_ECUDA, "finalize launch", e);
+  return MF_OK;
 }
 
 int mf_unweight(mf_process* p, const double* d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
