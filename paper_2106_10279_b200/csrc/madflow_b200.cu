@@ -30,6 +30,7 @@ struct mf_process {
   unsigned char* d_static = nullptr;  // device address of mf_static_scratch on the handle's device (cudaGetSymbolAddress)
   double* d_quark = nullptr;          // MF_PP_TTGG: quark-channel term per event of the current launch (grown on demand)
   uint64_t quark_cap = 0;
+  unsigned long long* d_start = nullptr;   // MF_PP_TTG / MF_PP_TTGG: the record cursor before the current mf_unweight launch
   double* d_obs = nullptr;            // caller-owned observable histograms (mf_set_observables) or NULL
   int obs_nb = 0;
   double obs_ptmax = 0.0, obs_etamax = 0.0;
@@ -96,7 +97,7 @@ cudaError_t coop_setup(mf_process* p, const cudaDeviceProp& prop) {
 
 void free_all(mf_process* p) {
   cudaFree(p->d_lnx); cudaFree(p->d_lnq2); cudaFree(p->d_xf); cudaFree(p->d_row);
-  cudaFree(p->d_partials); cudaFree(p->d_hist_part); cudaFree(p->d_queue); cudaFree(p->d_quark);
+  cudaFree(p->d_partials); cudaFree(p->d_hist_part); cudaFree(p->d_queue); cudaFree(p->d_quark); cudaFree(p->d_start);
 }
 
 // launches the fused pass + finalize on `stream`
@@ -137,8 +138,20 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   }
   const int blocks = unw ? p->blocks_unw : p->blocks;
   void* args[2] = {(void*)&p->P, (void*)&A};
-  cudaError_t e = cudaLaunchKernel(pass_fn(p->process, unw), dim3(blocks), dim3(p->threads), args, p->smem, st);
+  // MF_PP_TTG / MF_PP_TTGG: the partonic channel of the records of this launch is drawn by channel_kernel after the pass; it
+  // needs the cursor as it was before
+  const bool draw_channels = unw && d_records && capacity > 0 && n_events > 0 && (p->process == MF_PP_TTG || p->process == MF_PP_TTGG);
+  cudaError_t e;
+  if (draw_channels && (e = cudaMemcpyAsync(p->d_start, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st)) != cudaSuccess)
+    return fail(p, MF_ECUDA, "record cursor snapshot", e);
+  e = cudaLaunchKernel(pass_fn(p->process, unw), dim3(blocks), dim3(p->threads), args, p->smem, st);
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "fused pass launch", e);
+  if (draw_channels) {
+    const int cb = p->prepass_blocks;       // one block per SM: accepted events are few
+    if (p->process == MF_PP_TTG) mf::channel_kernel<5><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start);
+    else mf::channel_kernel<7><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start);
+    if ((e = cudaGetLastError()) != cudaSuccess) return fail(p, MF_ECUDA, "channel kernel launch", e);
+  }
   const int n_hist = p->D * p->P.n_bins;
   const int fin_blocks = (n_hist + 255) / 256 + 1;
   mf::finalize_kernel<<<fin_blocks, 256, 0, st>>>(p->d_partials, p->d_hist_part, blocks, n_hist, d_hist,
@@ -275,6 +288,9 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
   const int queue_doubles = p->process == MF_GG_TTGGG ? mf::kCtaQueue : (p->process == 3 || p->process == 7) ? mf::g4::Prog::Queue : mf::g3::Prog::Queue;
   if ((coop || p->process == MF_GG_TTGGG) &&
       (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads * queue_doubles * 8)) != cudaSuccess) {
+    free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
+  }
+  if ((p->process == MF_PP_TTG || p->process == MF_PP_TTGG) && (e = cudaMalloc(&p->d_start, sizeof(unsigned long long))) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
   snprintf(p->err, sizeof(p->err), "ok");

@@ -338,8 +338,8 @@ constexpr int kThreads = 128;
 // the event's accept block.  Accepted events are rare (< 1 %): everything is recomputed here from the
 // tables in global memory; the gluon channel's term (the team's matrix element is not kept) is what the event's weight w
 // leaves after the quark terms: w = common x (gg term + sum of the signed quark terms).
-// (inlined: as an out-of-line function, with nvcc 12.9 for sm_100a, it received its weight argument as 0 in this kernel,
-// by value or through a struct; measured cost of the larger frame: 34.8 -> 39.2 ms per 2^22 events of mf_unweight)
+// (inlined: as an out-of-line function inside the fused pass, with nvcc 12.9 for sm_100a, it received its weight argument as 0,
+// by value or through a struct; inlined there it cost 12 % of the step, so it now runs in channel_kernel after the pass)
 __device__ __forceinline__ unsigned pp_ttj_channel(const Params& P, const PassArgs& A, const Event<5>& ev, double w, double v) {
   double f1[kMaxPartonTables], f2[kMaxPartonTables], asf;
   parton_densities<5>(P, A, A.pdf_lnx, A.pdf_row, ev, f1, f2, asf);
@@ -458,17 +458,39 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
           rec[4 * (NF + 2)] = w;
           reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
           if (PROC == 4) reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = channel;
-          if constexpr (PROC == 5) {
-            const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);      // words z, w: the channel draw
-            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = pp_ttj_channel(P, A, ev, w, uniform52(r.z, r.w));
-          }
-          if constexpr (PROC == 7) {
-            const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);
-            reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = pp_ttgg_channel(P, A, ev, w, uniform52(r.z, r.w));
-          }
+          // pp -> ttbar j, pp -> ttbar gg: the channel of the record is drawn by channel_kernel, next on the stream (the draw
+          // needs the quark matrix elements again: hundreds of registers of code that does not belong into this loop)
+          if (PROC == 5 || PROC == 7) reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = 0ull;
         }
       }
     }
+  }
+}
+
+// R20 / R22: the partonic channel of the records mf_unweight has just written, slots [*start, min(*A.count, A.capacity)):
+// thread = record; the event is regenerated from its id, the channel drawn from the record's weight and the event's accept
+// block.  Accepted events are rare (< 1 %), so this costs microseconds; inside the fused pass the same code cost 12 % of
+// pp -> ttbar j's step (registers and instruction cache of a loop that almost never runs it).
+template <int PROC>
+__global__ void __launch_bounds__(kThreads) channel_kernel(const Params P, const PassArgs A, const unsigned long long* start) {
+  static_assert(PROC == 5 || PROC == 7, "processes whose channel draw needs the quark matrix elements");
+  constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  const unsigned long long first = *start, cnt = *A.count;
+  const unsigned long long last = cnt < A.capacity ? cnt : A.capacity;
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long slot = first + (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; slot < last; slot += stride) {
+    double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 24));
+    const double w = rec[4 * (NF + 2)];
+    const unsigned long long event = reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1];
+    Event<PROC> ev;
+    Bins<PROC> bins;
+    DebugRow dbg = {nullptr, D, NF};
+    generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
+    const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);      // words z, w: the channel draw
+    unsigned ch;
+    if constexpr (PROC == 5) ch = pp_ttj_channel(P, A, ev, w, uniform52(r.z, r.w));
+    else ch = pp_ttgg_channel(P, A, ev, w, uniform52(r.z, r.w));
+    reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = ch;
   }
 }
 
