@@ -18,7 +18,7 @@ ORACLE = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))
 @pytest.mark.skipif(shutil.which("g++") is None, reason="needs g++")
 def test_oracle_is_clean_under_asan_and_ubsan(tmp_path):
     exe = str(tmp_path / "sanitize_main")
-    cmd = ["g++", "-std=gnu++17", "-O1", "-g", "-fno-omit-frame-pointer", "-ffp-contract=off",
+    cmd = ["g++", "-std=gnu++17", "-O1", "-g1", "-fno-omit-frame-pointer", "-ffp-contract=off",
            "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-o", exe,
            os.path.join(ORACLE, "sanitize_main.cpp"), os.path.join(ORACLE, "mfo.cpp"), "-lquadmath"]
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
