@@ -594,18 +594,18 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
 // step): the matrix element is ~7000 straight-line instructions executed once per event, and without the lock-step the warps
 // of an SM were each waiting for their own instruction fetches (ncu: 5.5 warps per issue stalled on no_instruction).
 constexpr int kPrepassThreads = 256;
-constexpr int kPrepassWarpDoubles = kQQWarpSharedDoubles + 8 * kQQLStride;   // a warp's shared kinematics and light-line currents
+constexpr int kPrepassWarpDoubles = kQQWarpSharedDoubles + kQQWarpSets * kQQLStride;   // a warp's shared kinematics and line currents
 __host__ __device__ inline int prepass_smem_doubles(int D, int nb, int nx, int nfl) {
-  return D * (nb + 1) + nx + nfl * nx + kPrepassThreads * (17 + 2) + 32 + (kPrepassThreads / 32) * kPrepassWarpDoubles;
+  (void)D; (void)nb;      // the grid stays in global memory here (two edges per dimension and event: L1 hits)
+  return nx + nfl * nx + kPrepassThreads * (17 + 2) + 32 + (kPrepassThreads / 32) * kPrepassWarpDoubles;
 }
 template <int PROC>
 __global__ void __launch_bounds__(kPrepassThreads, 1) quark_prepass_kernel(const Params P, const PassArgs A, double* out) {
   static_assert(PROC == 7, "the prepass serves pp -> ttbar gg");
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF, NW = kPrepassThreads / 32;
   extern __shared__ double smem[];
-  const int nb = P.n_bins, nx = P.pdf_nx, nrow = nx * P.pdf_nfl;
-  double* s_grid = smem;                    // D*(nb+1)
-  double* s_lnx = s_grid + D * (nb + 1);    // nx
+  const int nx = P.pdf_nx, nrow = nx * P.pdf_nfl;
+  double* s_lnx = smem;                     // nx
   double* s_row = s_lnx + nx;               // one row per parton table
   double* s_ev = s_row + nrow;              // [rank][17]: momenta and shat of the block's passing events
   double* s_res = s_ev + kPrepassThreads * 17;                       // [rank][2]
@@ -614,7 +614,6 @@ __global__ void __launch_bounds__(kPrepassThreads, 1) quark_prepass_kernel(const
   double* s_warp = reinterpret_cast<double*>(s_cnt) + 32 + warp * kPrepassWarpDoubles;
   QQWarpShared* s_sh = reinterpret_cast<QQWarpShared*>(s_warp);
   double* s_L = s_warp + kQQWarpSharedDoubles;
-  for (int i = threadIdx.x; i < D * (nb + 1); i += blockDim.x) s_grid[i] = A.grid[i];
   for (int i = threadIdx.x; i < nx; i += blockDim.x) s_lnx[i] = A.pdf_lnx[i];
   for (int i = threadIdx.x; i < nrow; i += blockDim.x) s_row[i] = A.pdf_row[i];
   __syncthreads();
@@ -630,7 +629,7 @@ __global__ void __launch_bounds__(kPrepassThreads, 1) quark_prepass_kernel(const
     if (valid) {
       Bins<PROC> bins;
       DebugRow dbg = {nullptr, D, NF};
-      generate_event<PROC>(P, s_grid, A.seed, A.iteration, A.first_event + idx, ev, bins, dbg);
+      generate_event<PROC>(P, A.grid, A.seed, A.iteration, A.first_event + idx, ev, bins, dbg);
       pass = ev.pass;
       if (pass) quark_pair_luminosities(P, A, s_lnx, s_row, ev, asf, La, Lb);
     }

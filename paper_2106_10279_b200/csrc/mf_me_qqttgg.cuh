@@ -250,19 +250,92 @@ MF_HD double me2_qq_ttgg(const double p1[4], const double p2[4], const double p3
   return 2.0 * total * g4 * g4 / 72.0;
 }
 
+// The same 20 coefficients with BOTH lines' currents in memory (the warp kernel below: every current set is formed once per
+// (polarisation pair, spin state) and shared).
+MF_HD void qq_assemble_mem(const cvec* L, const cvec* T, const rvec& ea, const rvec& eb, const rvec& G, const QQKin& q, cplx a[20]) {
+  const cvec L0 = L[0], T0 = T[0];
+  // (I) nothing on the virtual gluon: one term per tensor, plus the merged pair on either line ([T^b, T^a] in its place)
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    a[i] = cscale(cdot_c(L0, T[5 + i]), q.iA);
+    a[6 + i] = cscale(cdot_c(L[5 + i], T0), q.iB);
+  }
+  a[12] = cscale(cdot_c(L[1], T[3]), q.iCa); a[13] = cscale(cdot_c(L[1], T[4]), q.iCa);
+  a[14] = cscale(cdot_c(L[2], T[3]), q.iCa); a[15] = cscale(cdot_c(L[2], T[4]), q.iCa);
+  a[16] = cscale(cdot_c(L[3], T[1]), q.iCb); a[17] = cscale(cdot_c(L[3], T[2]), q.iCb);
+  a[18] = cscale(cdot_c(L[4], T[1]), q.iCb); a[19] = cscale(cdot_c(L[4], T[2]), q.iCb);
+  const cplx m1 = cdot_c(L0, T[11]), m2 = cdot_c(L0, T[12]), m3 = cdot_c(L[11], T0), m4 = cdot_c(L[12], T0);
+  cacc(a[1], q.iA, m1);  cacc(a[0], -q.iA, m1);        // x G   ->  x b a - x a b
+  cacc(a[5], q.iA, m2);  cacc(a[4], -q.iA, m2);        // G x   ->  b a x - a b x
+  cacc(a[7], q.iB, m3);  cacc(a[6], -q.iB, m3);
+  cacc(a[11], q.iB, m4); cacc(a[10], -q.iB, m4);
+  // (II) gluon g on the virtual gluon (T^x -> [T^g, T^x] on the top line), the other one on the top line ...
+  const cvec Wa = v3c_vec(L0, q.PL0, ea, q.mka), Wb = v3c_vec(L0, q.PL0, eb, q.mkb);
+  const double dA = q.iA * q.iCa, dB = q.iA * q.iCb;
+  const cplx t1 = cdot_c(Wa, T[3]), t2 = cdot_c(Wa, T[4]), t3 = cdot_c(Wb, T[1]), t4 = cdot_c(Wb, T[2]);
+  cacc(a[2], dA, t1); cacc(a[0], -dA, t1);             // (x b) -> a x b - x a b
+  cacc(a[5], dA, t2); cacc(a[3], -dA, t2);             // (b x) -> b a x - b x a
+  cacc(a[3], dB, t3); cacc(a[1], -dB, t3);             // (x a) -> b x a - x b a
+  cacc(a[4], dB, t4); cacc(a[2], -dB, t4);             // (a x) -> a b x - a x b
+  // ... or on the light line: top string x -> g x - x g
+  const double eA = q.iCb * q.iB, eB = q.iCa * q.iB;
+  const cplx u1 = cdot_c(v3c_vec(L[3], q.PLb, ea, q.mka), T0), u2 = cdot_c(v3c_vec(L[4], q.PLb, ea, q.mka), T0);
+  const cplx u3 = cdot_c(v3c_vec(L[1], q.PLa, eb, q.mkb), T0), u4 = cdot_c(v3c_vec(L[2], q.PLa, eb, q.mkb), T0);
+  cacc(a[17], eA, u1); cacc(a[16], -eA, u1);
+  cacc(a[19], eA, u2); cacc(a[18], -eA, u2);
+  cacc(a[13], eB, u3); cacc(a[12], -eB, u3);
+  cacc(a[15], eB, u4); cacc(a[14], -eB, u4);
+  // (III) both on the virtual gluon: a then b, b then a, the merged pair, the four-gluon vertex (see qq_assemble)
+  const double d3 = q.iA * q.iB;
+  const cplx l0t0 = cdot_c(L0, T0), lea = cdot_r(L0, ea), leb = cdot_r(L0, eb), tea = cdot_r(T0, ea), teb = cdot_r(T0, eb);
+  const double eab = rdot(ea, eb);
+  const cplx sab = cdot_c(v3c_vec(Wa, q.PLa, eb, q.mkb), T0), sba = cdot_c(v3c_vec(Wb, q.PLb, ea, q.mka), T0);
+  const cplx sG = cdot_c(v3c_vec(L0, q.PL0, G, q.K), T0);
+  const cplx v0 = cmul(leb, tea), v1 = cmul(lea, teb);
+  const cplx A = {d3 * (sab.re * q.iCa + v0.re - eab * l0t0.re), d3 * (sab.im * q.iCa + v0.im - eab * l0t0.im)};
+  const cplx B = {d3 * (sba.re * q.iCb + v1.re - eab * l0t0.re), d3 * (sba.im * q.iCb + v1.im - eab * l0t0.im)};
+  const cplx C = {d3 * (sG.re - (v1.re - v0.re)), d3 * (sG.im - (v1.im - v0.im))};
+  cacc(a[5], 1.0, A); cacc(a[3], -1.0, A); cacc(a[2], -1.0, A); cacc(a[0], 1.0, A);
+  cacc(a[4], 1.0, B); cacc(a[2], -1.0, B); cacc(a[3], -1.0, B); cacc(a[1], 1.0, B);
+  cacc(a[5], 1.0, C); cacc(a[4], -1.0, C); cacc(a[1], -1.0, C); cacc(a[0], 1.0, C);
+}
+
+// thread-per-event evaluation through qq_assemble_mem (tests/host_shim: the arithmetic of the warp kernel, checked on the host)
+MF_HD double me2_qq_ttgg_mem(const double p1[4], const double p2[4], const double p3[4], const double p4[4], const double k5[4],
+                             const double k6[4], double mt, double g2) {
+  QQPoint pt;
+  qq_point(p1, p2, p3, p4, k5, k6, mt, pt);
+  const spin lcol = chiral_col(p1, 0, false), lrow = bar_of(chiral_col(p2, 0, true));
+  double total = 0.0;
+  for (int pol = 0; pol < 4; ++pol) {
+    const rvec ea = pt.Ea[pol & 1], eb = pt.Eb[pol >> 1];
+    const rvec G = qq_merged(pt.q, pt.isab, ea, eb);
+    cvec L[13], T[13];
+    qq_line_currents(lrow, lcol, pt.kl, ea, eb, G, L);
+    for (int st = 0; st < 4; ++st) {
+      qq_line_currents(ubar_row(p3, mt, st >> 1), v_col(p4, mt, st & 1), pt.kt, ea, eb, G, T);
+      cplx a[20];
+      qq_assemble_mem(L, T, ea, eb, G, pt.q, a);
+      total += qq_colour_square(a);
+    }
+  }
+  const double g4 = g2 * g2;
+  return 2.0 * total * g4 * g4 / 72.0;
+}
+
 #if defined(__CUDACC__)
-// The same matrix element by ONE WARP per event, both beam assignments at once (quark_prepass_kernel): lane = beam assignment o
-// (bit 4), polarisation pair (bits 2-3), top spin state st (bits 0-1).  The four lanes of an (o, polarisation pair) share its 13
-// light-line currents through shared memory (each stores a quarter of them); every lane then streams its own top-line currents
-// against them, forms its 20 string coefficients and the colour form in registers; the 16 lanes of an assignment are summed by
-// shuffles.
-constexpr int kQQLStride = 106;        // 13 currents x 8 doubles, padded: the 8 groups' broadcast reads fall into different banks
-// what does not depend on the lane, nor on the beam assignment (the top line's and the virtual gluon's kinematics, the
-// polarisation vectors): formed by lane 0, read by all from shared memory when needed (76 doubles that would otherwise sit in
-// every lane's registers)
+// The same matrix element by ONE WARP per event, both beam assignments at once (quark_prepass_kernel).
+// Stage 1: one set of 13 line currents per lane, the same code for both lines (qq_line_kin + the chains + 13 bilinears with the
+// lane's spinors, momenta and mass): lanes 0-15 the top line for (polarisation pair, spin state) = 16 sets, lanes 16-31 the light
+// line for (beam assignment, polarisation pair) = 8 sets (formed twice, stored once).  All sets go to shared memory.
+// Stage 2: lane = (beam assignment o, polarisation pair, top spin state): the 20 string coefficients from its two sets
+// (qq_assemble_mem), the colour form in registers; the 16 lanes of an assignment are summed by shuffles.
+constexpr int kQQLStride = 106;        // 13 currents x 8 doubles, padded: broadcast reads of different sets fall into different banks
+constexpr int kQQWarpSets = 8 + 16;    // light-line sets, then top-line sets
+// what does not depend on the lane, nor on the beam assignment (the virtual gluon's kinematics, the polarisation vectors):
+// formed by lane 0, read by all from shared memory when needed
 struct QQWarpShared {
   QQKin q;
-  QQLineKin kt;
   rvec Ea[2], Eb[2];
   double isab;
 };
@@ -271,33 +344,50 @@ __device__ __forceinline__ void qq_store(double* dst, const cvec& c) {
 #pragma unroll
   for (int m = 0; m < 4; ++m) { dst[m] = c.re[m]; dst[4 + m] = c.im[m]; }
 }
-// ev = the event's four final-state momenta and shat (17 doubles), sh and Ls[8 x kQQLStride]: the warp's shared memory
-__device__ __forceinline__ void me2_qq_ttgg_warp(const double* ev, QQWarpShared* sh, double* Ls, int lane, double mt, double g2,
+// ev = the event's four final-state momenta and shat (17 doubles), sh and Js[kQQWarpSets x kQQLStride]: the warp's shared memory
+__device__ __forceinline__ void me2_qq_ttgg_warp(const double* ev, QQWarpShared* sh, double* Js, int lane, double mt, double g2,
                                                  double& m0, double& m1) {
-  const int o = lane >> 4, pol = (lane >> 2) & 3, st = lane & 3;
-  const double E = 0.5 * sqrt(ev[16]), pz = o == 0 ? E : -E;
-  const double p1[4] = {E, 0.0, 0.0, pz}, p2[4] = {E, 0.0, 0.0, -pz};
+  const double E = 0.5 * sqrt(ev[16]);
   if (lane == 0) {
+    const double p1[4] = {E, 0.0, 0.0, E}, p2[4] = {E, 0.0, 0.0, -E};
     QQPoint pt;
-    qq_point(p1, p2, ev, ev + 4, ev + 8, ev + 12, mt, pt);
-    sh->q = pt.q; sh->kt = pt.kt; sh->isab = pt.isab;
+    qq_point(p1, p2, ev, ev + 4, ev + 8, ev + 12, mt, pt);      // q, Ea, Eb, isab do not depend on the beam assignment
+    sh->q = pt.q; sh->isab = pt.isab;
     sh->Ea[0] = pt.Ea[0]; sh->Ea[1] = pt.Ea[1]; sh->Eb[0] = pt.Eb[0]; sh->Eb[1] = pt.Eb[1];
   }
   __syncwarp();
-  const rvec ea = sh->Ea[pol & 1], eb = sh->Eb[pol >> 1];
-  const rvec G = qq_merged(sh->q, sh->isab, ea, eb);
   {
-    // the light line's 13 currents: every lane of an (o, polarisation pair) forms them all (the same instructions for the whole
-    // warp: four different code paths would be executed one after the other) and stores its quarter
-    rvec pcl, prl, ka, kb;
+    const bool top = lane < 16;
+    const int c = lane & 15;
+    const int pol1 = top ? (c >> 2) : ((c >> 1) & 3);
+    const rvec ea = sh->Ea[pol1 & 1], eb = sh->Eb[pol1 >> 1];
+    const rvec G = qq_merged(sh->q, sh->isab, ea, eb);
+    spin row, col;
+    rvec pc, pr, ka, kb;
+    double m;
+    if (top) {
+      row = ubar_row(ev, mt, (c >> 1) & 1);
+      col = v_col(ev + 4, mt, c & 1);
+      m = mt;
 #pragma unroll
-    for (int m = 0; m < 4; ++m) { pcl.v[m] = p1[m]; prl.v[m] = -p2[m]; ka.v[m] = ev[8 + m]; kb.v[m] = ev[12 + m]; }
-    const QQLineKin k = qq_line_kin(pcl, prl, ka, kb, 0.0);
-    const spin col = chiral_col(p1, 0, false), row = bar_of(chiral_col(p2, 0, true));
-    double* L = Ls + (lane >> 2) * kQQLStride;
+      for (int i = 0; i < 4; ++i) { pc.v[i] = -ev[4 + i]; pr.v[i] = ev[i]; }
+    } else {
+      const double pz = (c >> 3) == 0 ? E : -E;
+      const double p1[4] = {E, 0.0, 0.0, pz}, p2[4] = {E, 0.0, 0.0, -pz};
+      col = chiral_col(p1, 0, false);
+      row = bar_of(chiral_col(p2, 0, true));
+      m = 0.0;
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { pc.v[i] = p1[i]; pr.v[i] = -p2[i]; }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { ka.v[i] = ev[8 + i]; kb.v[i] = ev[12 + i]; }
+    const QQLineKin k = qq_line_kin(pc, pr, ka, kb, m);
+    double* dst = Js + (top ? 8 + c : (c >> 1)) * kQQLStride;
+    const bool store = top || (c & 1) == 0;
     const spin ca = prop_col(k.qa, k.m, k.ia, slash_col(ea, col)), cb = prop_col(k.qb, k.m, k.ib, slash_col(eb, col));
     const spin ra = prop_row(slash_row(row, ea), k.ra, k.m, k.ja), rb = prop_row(slash_row(row, eb), k.rb, k.m, k.jb);
-    auto put = [&](int i, const cvec& c) { if ((i & 3) == st) qq_store(L + 8 * i, c); };
+    auto put = [&](int i, const cvec& v) { if (store) qq_store(dst + 8 * i, v); };
     put(0, bilinear(row, col));
     put(1, bilinear(row, ca));
     put(2, bilinear(ra, col));
@@ -313,9 +403,12 @@ __device__ __forceinline__ void me2_qq_ttgg_warp(const double* ev, QQWarpShared*
     put(12, bilinear(prop_row(slash_row(row, G), k.rab, k.m, k.jab), col));
   }
   __syncwarp();
+  const int o = lane >> 4, pol = (lane >> 2) & 3, st = lane & 3;
+  const rvec ea = sh->Ea[pol & 1], eb = sh->Eb[pol >> 1];
+  const rvec G = qq_merged(sh->q, sh->isab, ea, eb);
   cplx a[20];
-  qq_assemble(reinterpret_cast<const cvec*>(Ls + (lane >> 2) * kQQLStride), ubar_row(ev, mt, st >> 1), v_col(ev + 4, mt, st & 1), sh->kt,
-              ea, eb, G, sh->q, a);
+  qq_assemble_mem(reinterpret_cast<const cvec*>(Js + (o * 4 + pol) * kQQLStride),
+                  reinterpret_cast<const cvec*>(Js + (8 + pol * 4 + st) * kQQLStride), ea, eb, G, sh->q, a);
   double v = qq_colour_square(a);
 #pragma unroll
   for (int d = 1; d < 16; d <<= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, d);

@@ -100,6 +100,10 @@ double mfh_me2_qq_ttgg(const double* mom, double m_top, double alpha_s) {
   return me2_qq_ttgg(mom, mom + 4, mom + 8, mom + 12, mom + 16, mom + 20, m_top, 4.0 * kPi * alpha_s);
 }
 
+double mfh_me2_qq_ttgg_mem(const double* mom, double m_top, double alpha_s) {
+  return me2_qq_ttgg_mem(mom, mom + 4, mom + 8, mom + 12, mom + 16, mom + 20, m_top, 4.0 * kPi * alpha_s);
+}
+
 void mfh_philox(uint64_t seed, uint32_t iteration, uint64_t event, uint32_t block, uint32_t out[4]) {
   U4 r = philox_block(seed, iteration, event, block);
   out[0] = r.x; out[1] = r.y; out[2] = r.z; out[3] = r.w;

@@ -87,7 +87,7 @@ def shim():
     L = C.CDLL(out)
     L.mfh_me2.restype = C.c_double
     L.mfh_me2.argtypes = [C.c_int, dp, C.c_double, C.c_double, C.c_double]
-    for f in (L.mfh_me2_coop, L.mfh_me2_coop3, L.mfh_me2_cta5, L.mfh_me2_qq_ttgg):
+    for f in (L.mfh_me2_coop, L.mfh_me2_coop3, L.mfh_me2_cta5, L.mfh_me2_qq_ttgg, L.mfh_me2_qq_ttgg_mem):
         f.restype = C.c_double
         f.argtypes = [dp, C.c_double, C.c_double]
     L.mfh_event.argtypes = [C.c_int, dp, C.c_int] + [C.c_double] * 8 + [C.c_uint64, C.c_uint32, C.c_uint64, dp]
@@ -288,8 +288,9 @@ def test_shim_qq_ttgg(shim):
         mom = np.vstack([[w / 2, 0, 0, w / 2], [w / 2, 0, 0, -w / 2], k])
         if i & 1:
             mom[[0, 1]] = mom[[1, 0]]
-        g = shim.mfh_me2_qq_ttgg(np.ascontiguousarray(mom).ctypes.data_as(dp), mt, a_s)
-        assert g == pytest.approx(mfo.me2_qq_ttbar_gg(mom, mt, a_s), rel=1e-11)
+        want = mfo.me2_qq_ttbar_gg(mom, mt, a_s)
+        for f in (shim.mfh_me2_qq_ttgg, shim.mfh_me2_qq_ttgg_mem):      # streamed top line; both lines' currents in memory
+            assert f(np.ascontiguousarray(mom).ctypes.data_as(dp), mt, a_s) == pytest.approx(want, rel=1e-11)
 
 
 # ---- multi-rank sharding (gloo, world size 2) ------------------------------------------------------------------
