@@ -24,11 +24,16 @@ def combine(I, var):
     return Ic, wsum ** -0.5, chi2
 
 
-def run_vegas(P, wl, n_events, n_iter, alpha=W.VEGAS_ALPHA):
+def run_vegas(P, wl, n_events, n_iter, alpha=W.VEGAS_ALPHA, pool=None):
+    """pool: the iterations' events on one single-threaded oracle process per host core (tests/oracle_pool.py; partial sums
+    added in range order: 1e-16 relative against the single process, test_oracle_pool.py)"""
     grid = W.uniform_grid(wl.n_dims)
     I, var = [], []
     for it in range(n_iter):
-        hist, res = P.vegas_iterate(grid, wl.seed, it, 0, n_events)
+        if pool is not None:
+            hist, res, _ = pool.iterate(wl, grid, wl.seed, it, 0, n_events)
+        else:
+            hist, res = P.vegas_iterate(grid, wl.seed, it, 0, n_events)
         Ik = res.sum_w / n_events
         I.append(Ik)
         var.append((res.sum_w2 / n_events - Ik * Ik) / (n_events - 1))
@@ -57,8 +62,8 @@ def test_c0_brute_force_gauss_legendre(oracle_procs):
 
 
 @pytest.fixture(scope="module")
-def c0_full(oracle_procs):
-    return run_vegas(oracle_procs[0], W.C0, W.C0.n_events, W.C0.n_iterations)
+def c0_full(oracle_procs, oracle_pool):
+    return run_vegas(oracle_procs[0], W.C0, W.C0.n_events, W.C0.n_iterations, pool=oracle_pool)
 
 
 def test_c0_full_config_matches_closed_form_and_stream_pins(c0_full):
@@ -117,9 +122,9 @@ def test_c1_quadrature_value(c1_quadrature):
     assert c1_quadrature == pytest.approx(2648.76, abs=0.02)
 
 
-def test_c1_vegas_agrees_with_quadrature(oracle_procs, c1_quadrature):
+def test_c1_vegas_agrees_with_quadrature(oracle_procs, oracle_pool, c1_quadrature):
     """Reduced-N run of the whole chain (Philox -> VEGAS -> tau,y -> 2-body -> PDF -> helicity amplitudes -> w)."""
-    I, var, _ = run_vegas(oracle_procs[1], W.C1, 2 ** 16, 6)
+    I, var, _ = run_vegas(oracle_procs[1], W.C1, 2 ** 16, 6, pool=oracle_pool)
     Ic, sc, chi2 = combine(I[1:], var[1:])
     assert sc / Ic < 2e-3
     assert abs(Ic - c1_quadrature) < 4 * sc
