@@ -123,17 +123,19 @@ def test_ttgg_records_carry_their_partons():
 
 
 @pytest.mark.gpu
-def test_lhe_drain_flavour_summed(tmp_path):
-    """the drain on MF_PP_TT records: every event of the file has the partons of its record's channel"""
+@pytest.mark.parametrize("cfg,n_ev,div,ids_of,nup_want", [("C5", 30000, 30, "channel_ids", 4), ("C6", 30000, 30, "channel_ids_ttj", 5),
+                                                         ("C8", 20000, 300, "channel_ids_ttgg", 6)])
+def test_lhe_drain_flavour_summed(tmp_path, cfg, n_ev, div, ids_of, nup_want):
+    """the drain on MF_PP_TT / MF_PP_TTG / MF_PP_TTGG records: every event of the file has the partons of its record's channel"""
     import torch
     from paper_2106_10279_b200 import api
-    wl = W.C5.scaled(30000, 2, 1)
+    wl = {"C5": W.C5, "C6": W.C6, "C8": W.C8}[cfg].scaled(n_ev, 2, 1)
     gp = api.Process(wl, W.pdf_table_flavours())
     grid, hist, res = gp.new_grid(), gp.new_hist(), gp.new_result()
     gp.vegas_iterate(grid, 0, 0, 0, wl.n_events, hist, res)
     gp.refine_grid(grid, hist)
-    w_max = gp.result_to_host(res).max_abs_w / 30
-    cap = 30000
+    w_max = gp.result_to_host(res).max_abs_w / div
+    cap = n_ev
     records = torch.zeros(cap * gp.record_size, dtype=torch.uint8, device="cuda")
     count = torch.zeros(1, dtype=torch.int64, device="cuda")
     path = str(tmp_path / "pp.lhe")
@@ -147,8 +149,8 @@ def test_lhe_drain_flavour_summed(tmp_path):
     ev = _parse(open(path).read())
     assert len(ev) == n
     for (nup, _, parts, _), c in zip(ev, chan):
-        want, _ = lhe.channel_ids(c)
-        assert nup == 4 and tuple(int(p[0]) for p in parts) == tuple(want)
+        want, _ = getattr(lhe, ids_of)(c)
+        assert nup == nup_want and tuple(int(p[0]) for p in parts) == tuple(want)
     gp.close()
 
 
