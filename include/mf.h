@@ -19,7 +19,9 @@
  *    legacy default stream).
  *  - The library allocates device memory only in mf_create_process and frees it only in
  *    mf_destroy_process.  The hot calls never allocate, never synchronise the stream and never touch host
- *    memory: they are asynchronous, results are valid after the caller synchronises `stream`.
+ *    memory: they are asynchronous, results are valid after the caller synchronises `stream`.  (MF_PP_TTGG keeps one
+ *    double per event between its two kernels in a buffer of 2^22 events made at create; a larger call runs as
+ *    consecutive pieces on the stream whose sums are added in piece order.)
  *  - A handle is used from one stream at a time (it owns per-block partial-sum scratch).
  *  - There is no CPU fallback: without a CUDA device mf_create_process returns MF_ECUDA.
  */

@@ -28,7 +28,7 @@ struct mf_process {
   mf::BlockPartial* d_partials = nullptr;
   double* d_queue = nullptr;          // cooperative pass: per-block momenta queue
   unsigned char* d_static = nullptr;  // device address of mf_static_scratch on the handle's device (cudaGetSymbolAddress)
-  double* d_quark = nullptr;          // MF_PP_TTGG: quark-channel term per event of the current launch (grown on demand)
+  double* d_quark = nullptr;          // MF_PP_TTGG: quark-channel term per event of the current piece (kQuarkChunk events, made at create)
   uint64_t quark_cap = 0;
   unsigned long long* d_start = nullptr;   // MF_PP_TTG / MF_PP_TTGG: the record cursor before the current mf_unweight launch
   double* d_obs = nullptr;            // caller-owned observable histograms (mf_set_observables) or NULL
@@ -43,6 +43,8 @@ struct mf_process {
 };
 
 namespace {
+
+constexpr uint64_t kQuarkChunk = 1ull << 22;     // events per piece of an MF_PP_TTGG call (32 MB of quark terms)
 
 const char* kNullHandle = "null handle";
 
@@ -120,42 +122,50 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   A.obs = p->d_obs; A.obs_nb = p->obs_nb; A.obs_ptmax = p->obs_ptmax; A.obs_etamax = p->obs_etamax;
   cudaStream_t st = (cudaStream_t)stream;
   A.quark_terms = nullptr;
-  if (p->process == MF_PP_TTGG && n_events > 0) {
-    // the quark channels of every event of this launch, one thread per event, ahead of the cooperative pass on the same stream
-    if (n_events > p->quark_cap) {
-      cudaFree(p->d_quark);             // synchronises with earlier launches that read the old buffer
-      p->d_quark = nullptr; p->quark_cap = 0;
-      if (cudaMalloc(&p->d_quark, n_events * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(p, MF_ENOMEM, "quark-term buffer"); }
-      p->quark_cap = n_events;
-    }
-    const size_t smem = (size_t)mf::prepass_smem_doubles(p->D, p->P.n_bins, p->P.pdf_nx, p->P.pdf_nfl) * sizeof(double);
-    const uint64_t want = (n_events + mf::kPrepassThreads - 1) / mf::kPrepassThreads;
-    const unsigned pre_blocks = (unsigned)(want < (uint64_t)p->prepass_blocks ? want : (uint64_t)p->prepass_blocks);
-    mf::quark_prepass_kernel<7><<<pre_blocks, mf::kPrepassThreads, smem, st>>>(p->P, A, p->d_quark);
-    cudaError_t pe = cudaGetLastError();
-    if (pe != cudaSuccess) return fail(p, MF_ECUDA, "quark prepass launch", pe);
-    A.quark_terms = p->d_quark;
-  }
   const int blocks = unw ? p->blocks_unw : p->blocks;
-  void* args[2] = {(void*)&p->P, (void*)&A};
-  // MF_PP_TTG / MF_PP_TTGG: the partonic channel of the records of this launch is drawn by channel_kernel after the pass; it
+  const int n_hist = p->D * p->P.n_bins;
+  const int fin_blocks = (n_hist + 255) / 256 + 1;
+  // MF_PP_TTG / MF_PP_TTGG: the partonic channel of the records of this call is drawn by channel_kernel after the pass; it
   // needs the cursor as it was before
   const bool draw_channels = unw && d_records && capacity > 0 && n_events > 0 && (p->process == MF_PP_TTG || p->process == MF_PP_TTGG);
   cudaError_t e;
   if (draw_channels && (e = cudaMemcpyAsync(p->d_start, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st)) != cudaSuccess)
     return fail(p, MF_ECUDA, "record cursor snapshot", e);
-  e = cudaLaunchKernel(pass_fn(p->process, unw), dim3(blocks), dim3(p->threads), args, p->smem, st);
-  if (e != cudaSuccess) return fail(p, MF_ECUDA, "fused pass launch", e);
+  // MF_PP_TTGG keeps one double per event between its two kernels, in a buffer of kQuarkChunk events made at create: a larger
+  // call runs as consecutive pieces whose results finalize_kernel adds up (in piece order: deterministic)
+  const uint64_t piece_max = p->process == MF_PP_TTGG ? p->quark_cap : n_events;
+  uint64_t done = 0;
+  int piece = 0;
+  do {
+    const uint64_t m = n_events - done < piece_max ? n_events - done : piece_max;
+    A.first_event = first_event + done;
+    A.n_events = m;
+    if (p->process == MF_PP_TTGG && m > 0) {
+      // the quark channel of every event of this piece, ahead of the cooperative pass on the same stream
+      const size_t smem = (size_t)mf::prepass_smem_doubles(p->D, p->P.n_bins, p->P.pdf_nx, p->P.pdf_nfl) * sizeof(double);
+      const uint64_t want = (m + mf::kPrepassThreads - 1) / mf::kPrepassThreads;
+      const unsigned pre_blocks = (unsigned)(want < (uint64_t)p->prepass_blocks ? want : (uint64_t)p->prepass_blocks);
+      mf::quark_prepass_kernel<7><<<pre_blocks, mf::kPrepassThreads, smem, st>>>(p->P, A, p->d_quark);
+      if ((e = cudaGetLastError()) != cudaSuccess) return fail(p, MF_ECUDA, "quark prepass launch", e);
+      A.quark_terms = p->d_quark;
+    }
+    void* args[2] = {(void*)&p->P, (void*)&A};
+    e = cudaLaunchKernel(pass_fn(p->process, unw), dim3(blocks), dim3(p->threads), args, p->smem, st);
+    if (e != cudaSuccess) return fail(p, MF_ECUDA, "fused pass launch", e);
+    mf::finalize_kernel<<<fin_blocks, 256, 0, st>>>(p->d_partials, p->d_hist_part, blocks, n_hist, d_hist,
+                                                    (mf::IterResult*)d_result, piece > 0 ? 1 : 0);
+    if ((e = cudaGetLastError()) != cudaSuccess) return fail(p, MF_ECUDA, "finalize launch", e);
+    done += m;
+    ++piece;
+  } while (done < n_events);
   if (draw_channels) {
+    A.first_event = first_event;
+    A.n_events = n_events;
     const int cb = p->prepass_blocks;       // one block per SM: accepted events are few
     if (p->process == MF_PP_TTG) mf::channel_kernel<5><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start);
     else mf::channel_kernel<7><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start);
     if ((e = cudaGetLastError()) != cudaSuccess) return fail(p, MF_ECUDA, "channel kernel launch", e);
   }
-  const int n_hist = p->D * p->P.n_bins;
-  const int fin_blocks = (n_hist + 255) / 256 + 1;
-  mf::finalize_kernel<<<fin_blocks, 256, 0, st>>>(p->d_partials, p->d_hist_part, blocks, n_hist, d_hist,
-                                                  (mf::IterResult*)d_result);
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "finalize launch", e);
   return MF_OK;
@@ -290,6 +300,10 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
       (e = cudaMalloc(&p->d_queue, (size_t)max_blocks * p->threads * queue_doubles * 8)) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
+  if (p->process == MF_PP_TTGG) {
+    if ((e = cudaMalloc(&p->d_quark, kQuarkChunk * sizeof(double))) != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM; }
+    p->quark_cap = kQuarkChunk;
+  }
   if ((p->process == MF_PP_TTG || p->process == MF_PP_TTGG) && (e = cudaMalloc(&p->d_start, sizeof(unsigned long long))) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
@@ -377,7 +391,7 @@ int mf_vegas_iterate_static(mf_process* p, const double* d_grid, uint64_t seed, 
   cudaError_t e = cudaLaunchKernel(pass_fn(p->process, false), dim3(blocks), dim3(p->threads), args, p->smem, st);
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "fused pass launch", e);
   mf::finalize_kernel<<<(n_hist + 255) / 256 + 1, 256, 0, st>>>(A.partials, A.hist_part, blocks, n_hist, d_hist,
-                                                               (mf::IterResult*)d_result);
+                                                               (mf::IterResult*)d_result, 0);
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "finalize launch", e);
   return MF_OK;

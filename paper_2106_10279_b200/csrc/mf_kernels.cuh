@@ -668,13 +668,15 @@ __global__ void __launch_bounds__(kPrepassThreads, 1) quark_prepass_kernel(const
 }
 
 // Adds the per-block partials in block order.  Blocks 0..gridDim.x-2 own histogram bins (one thread per
-// bin, summing over the pass's blocks); the last block reduces the scalar partials.
+// bin, summing over the pass's blocks); the last block reduces the scalar partials.  accumulate != 0: the outputs already hold
+// the earlier pieces of the same call (MF_PP_TTGG calls larger than its quark-term buffer) and are added to.
 __global__ void __launch_bounds__(256) finalize_kernel(const BlockPartial* partials, const double* hist_part,
-                                                        int n_blocks, int n_hist, double* hist, IterResult* result) {
+                                                        int n_blocks, int n_hist, double* hist, IterResult* result,
+                                                        int accumulate) {
   if (blockIdx.x + 1 < gridDim.x) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (hist != nullptr && i < n_hist) {
-      double s = 0.0;
+      double s = accumulate ? hist[i] : 0.0;
       for (int b = 0; b < n_blocks; ++b) s += hist_part[(size_t)b * n_hist + i];
       hist[i] = s;
     }
@@ -701,8 +703,13 @@ __global__ void __launch_bounds__(256) finalize_kernel(const BlockPartial* parti
     __syncthreads();
   }
   if (threadIdx.x == 0) {
-    result->sum_w = sw[0]; result->sum_w2 = sw2[0]; result->max_abs_w = mx[0];
-    result->n_pass = np[0]; result->n_accept = na[0];
+    if (accumulate) {
+      result->sum_w += sw[0]; result->sum_w2 += sw2[0]; result->max_abs_w = fmax(result->max_abs_w, mx[0]);
+      result->n_pass += np[0]; result->n_accept += na[0];
+    } else {
+      result->sum_w = sw[0]; result->sum_w2 = sw2[0]; result->max_abs_w = mx[0];
+      result->n_pass = np[0]; result->n_accept = na[0];
+    }
   }
 }
 

@@ -160,3 +160,40 @@ def test_full_size_sampled(gpu_procs, oracle_procs, oracle_pool):
         wo = o[:, c["w"]]
         assert rw.n_pass == int(o[:, c["pas"]].sum())
         assert abs(rw.sum_w - math.fsum(wo)) <= 1e-9 * abs(math.fsum(wo))
+
+
+def test_call_larger_than_the_quark_term_buffer(gpu_procs, oracle_procs):
+    """more than 2^22 events in one call: the library runs it as consecutive pieces (its per-event quark terms live in a buffer
+    made at create: the hot calls never allocate) and adds their sums in piece order; records and channels span the pieces"""
+    torch = _torch()
+    gp, op = gpu_procs[PID], oracle_procs[PID]
+    grid = adapted_grid(op, WL)
+    n1 = 1 << 22
+    n = n1 + 100_003
+    hg, rg = _iterate_gpu(gp, grid, 0, 4, 0, n)
+    ha, ra = _iterate_gpu(gp, grid, 0, 4, 0, n1)
+    hb, rb = _iterate_gpu(gp, grid, 0, 4, n1, n - n1)
+    assert rg.n_pass == ra.n_pass + rb.n_pass
+    assert rg.sum_w == ra.sum_w + rb.sum_w and rg.sum_w2 == ra.sum_w2 + rb.sum_w2      # the same two numbers, added once
+    assert rg.max_abs_w == max(ra.max_abs_w, rb.max_abs_w)
+    np.testing.assert_allclose(hg, ha + hb, rtol=1e-12, atol=1e-14 * hg.max())
+    # unweighting through both pieces: one cursor, channels drawn for the records of both
+    dgrid = torch.from_numpy(grid).cuda()
+    w_max = 300.0 * rg.sum_w / n          # 300 x the mean weight: about one event in 300 survives
+    cap = 200_000
+    out = []
+    for first, m in [(0, n), (0, n1), (n1, n - n1)]:
+        records = torch.zeros(cap * gp.record_size, dtype=torch.uint8, device="cuda")
+        count = torch.zeros(1, dtype=torch.int64, device="cuda")
+        res = gp.new_result()
+        gp.unweight(dgrid, 0, 4, first, m, w_max, records, cap, count, None, res)
+        torch.cuda.synchronize()
+        k = int(count.item())
+        assert 0 < k < cap and gp.result_to_host(res).n_accept == k
+        rec = gp.records_array(records, k)
+        out.append(rec[np.argsort(rec["id"])])
+    whole, parts = out[0], np.concatenate(out[1:])
+    assert len(whole) == len(parts) > 100 and (whole["id"] >= n1).any()
+    assert np.array_equal(whole["id"], parts["id"]) and np.array_equal(whole["channel"], parts["channel"])
+    assert np.array_equal(whole["w"], parts["w"]) and np.array_equal(whole["mom"], parts["mom"])
+    assert (whole["channel"] > 0).any()
