@@ -106,12 +106,12 @@ int mf_vegas_iterate(mf_process *p, const double *d_grid, uint64_t seed, uint32_
  * the handle's buffers.  The call itself calls no cudaMalloc / cudaFree or allocating library routine (the handle was created,
  * and the array's device address looked up, at set-up in mf_create_process).
  * Limits: MF_EE_MUMU, MF_GG_TT and MF_PP_TT handles only (the cooperative kernels queue events in tens of MB), and
- *   launch blocks x (40 + 8 D n_bins) bytes <= MF_STATIC_SCRATCH_BYTES  (e.g. MF_GG_TT with 50 bins: 0.97 MB; with 128 bins: refused);
+ *   launch blocks x (40 + 8 D n_bins) bytes <= MF_STATIC_SCRATCH_BYTES  (e.g. MF_GG_TT, 444 blocks on a B200: 0.73 MB with 50 bins; refused with 128 bins);
  * anything else returns MF_EINVAL with the reason in mf_last_error.
  * Every call on a device shares the one array, from every handle and stream: two calls that overlap on the GPU race (keep
  * them on one stream, or order them with events).  The array keeps the last call's contents; nothing in it has to start at
  * zero, every block overwrites its part before it is read. */
-#define MF_STATIC_SCRATCH_BYTES (2 * 1024 * 1024)
+#define MF_STATIC_SCRATCH_BYTES (1024 * 1024)
 int mf_vegas_iterate_static(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                             uint64_t n_events, double *d_hist, mf_iter_result *d_result, void *stream);
 

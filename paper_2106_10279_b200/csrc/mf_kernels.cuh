@@ -534,8 +534,23 @@ MF_D void block_finish(const PassArgs& A, Accum acc, double* s_red, const double
 }
 
 // ---- the fused pass, one thread per event (e+e- -> mu+mu-, gg -> ttbar, pp -> ttbar) ----------------------
+// Lock-step: a block barrier at the top of every grid-stride round keeps the four warps of a block on the same part of the
+// (straight-line, once-per-event) matrix-element code, so one warp's instruction fetches serve all four (ncu on gg -> ttbar:
+// no_instruction 1.19 warps per issue without it).  Measured per 2^20 events (profiles/r2_tpe.md): gg -> ttbar 0.292 -> 0.271 ms,
+// with 3 instead of 4 blocks per SM (168 registers: fewer spills) 0.267 ms; pp -> ttbar 0.429 -> 0.402 ms (3 blocks per SM:
+// 0.437 ms); e+e- -> mu+mu- 0.112 -> 0.118 ms (its code is small: no barrier there).
+#ifndef MF_TPE_BLOCKS1
+#define MF_TPE_BLOCKS1 3
+#endif
+#ifndef MF_TPE_BLOCKS4
+#define MF_TPE_BLOCKS4 2
+#endif
+#ifndef MF_TPE_LOCKSTEP
+#define MF_TPE_LOCKSTEP 1
+#endif
 template <int PROC, bool UNW>
-__global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel(const Params P, const PassArgs A) {
+__global__ void __launch_bounds__(kThreads, PROC == 1 ? MF_TPE_BLOCKS1 : PROC == 4 ? MF_TPE_BLOCKS4 : 2)
+    fused_pass_kernel(const Params P, const PassArgs A) {
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
   extern __shared__ double smem[];
   const int nb = P.n_bins, nx = PROC == 0 ? 0 : P.pdf_nx, nrow = (PROC == 4 || PROC == 5) ? nx * P.pdf_nfl : nx;
@@ -555,6 +570,9 @@ __global__ void __launch_bounds__(kThreads, PROC == 1 ? 4 : 2) fused_pass_kernel
   const uint64_t rounds = (A.n_events + stride - 1) / stride;
   uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   for (uint64_t rd = 0; rd < rounds; ++rd, idx += stride) {
+#if MF_TPE_LOCKSTEP
+    if (PROC != 0) __syncthreads();
+#endif
     const bool valid = idx < A.n_events;
     const uint64_t event = A.first_event + idx;
     double w = 0.0;

@@ -55,7 +55,7 @@ def test_static_scratch_refusals():
     import dataclasses
     import torch
     from paper_2106_10279_b200 import api
-    big = dataclasses.replace(W.C1, n_bins=128)          # 592 blocks x (40 + 8 x 4 x 128) bytes = 2.4 MB > 2 MiB
+    big = dataclasses.replace(W.C1, n_bins=128)          # 444 blocks x (40 + 8 x 4 x 128) bytes = 1.8 MB > 1 MiB
     for wl, word in [(big, "static"), (W.C2, "thread-per-event")]:
         proc = api.Process(wl, W.pdf_for(wl.process))
         try:
