@@ -58,9 +58,9 @@ FLOP_PROFILE_DMMA = {6: 3840 * 512.0, 7: 48 * 512.0}            # flop per matri
 FLOP_PROFILE_ME = {2: 21472.0, 3: 157956.0}      # the static matrix-element count of the build that was profiled
 OTHER_FLOPS = {0: 0.0, 1: 0.0, 2: 2930.0, 3: 5290.0, 4: 0.0, 5: 0.0, 6: 0.0, 7: 0.0}
 ME_FLOPS_MEASURED = {0: 1232.0, 1: 3766.0, 4: 5023.0, 5: 54030.0, 6: 6.31e6, 7: 321600.0}    # 5, 6: per event PASSING the cuts
-# kernels of this library launched per step (mf_unweight + mf_refine_grid): fused pass, finalize, refine; pp -> ttbar j adds the
-# channel kernel of its accepted records, pp -> ttbar gg that and the quark prepass
-LAUNCHES_PER_STEP = {5: 4, 7: 5}
+# kernels of this library launched per step (mf_unweight + mf_refine_grid): fused pass, finalize, refine; g g -> ttbar g and
+# pp -> ttbar j add the record kernel of their accepted events, pp -> ttbar gg that and the quark prepass
+LAUNCHES_PER_STEP = {2: 4, 5: 4, 7: 5}
 # dram__bytes_read + dram__bytes_write per launch of the fused pass from an ncu capture of this very command
 # (profiles/r1_coop_v4_traffic.md), keyed by (process, events per launch); None where no capture was taken
 MEASURED_TRAFFIC = {(3, 1 << 22): 3.86e7}

@@ -131,8 +131,9 @@ int mf_refine_grid(mf_process *p, double *d_grid, const double *d_hist, double a
  * the channels, in that order, with the second uniform of the accept block (R18).
  * MF_PP_TTG likewise (R20; the LHE writer needs the partons of every event): 0 = g g; 1 + 6 i + c = flavour i in
  * class c (0 q qbar, 1 qbar q, 2 q g, 3 g q, 4 qbar g, 5 g qbar; first parton from beam 1): records of 5 x 32 + 16 + 8 bytes.
- * For MF_PP_TTG and MF_PP_TTGG the channel field of the new records is filled by a second kernel that follows the pass on the
- * same stream (complete when the stream has reached the end of the call, like everything else the call writes). */
+ * For MF_GG_TTG, MF_PP_TTG and MF_PP_TTGG the momenta (and channel) of the new records are filled in by a second kernel that
+ * follows the pass on the same stream (complete when the stream has reached the end of the call, like everything else the call
+ * writes). */
 int mf_unweight(mf_process *p, const double *d_grid, uint64_t seed, uint32_t iteration, uint64_t first_event,
                 uint64_t n_events, double w_max, void *d_records, uint64_t capacity, uint64_t *d_count,
                 double *d_hist, mf_iter_result *d_result, void *stream);

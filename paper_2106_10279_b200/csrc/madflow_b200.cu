@@ -30,7 +30,7 @@ struct mf_process {
   unsigned char* d_static = nullptr;  // device address of mf_static_scratch on the handle's device (cudaGetSymbolAddress)
   double* d_quark = nullptr;          // MF_PP_TTGG: quark-channel term per event of the current piece (kQuarkChunk events, made at create)
   uint64_t quark_cap = 0;
-  unsigned long long* d_start = nullptr;   // MF_PP_TTG / MF_PP_TTGG: the record cursor before the current mf_unweight launch
+  unsigned long long* d_start = nullptr;   // cooperative / block processes: the record cursor before the current mf_unweight call
   double* d_obs = nullptr;            // caller-owned observable histograms (mf_set_observables) or NULL
   int obs_nb = 0;
   double obs_ptmax = 0.0, obs_etamax = 0.0;
@@ -125,9 +125,9 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
   const int blocks = unw ? p->blocks_unw : p->blocks;
   const int n_hist = p->D * p->P.n_bins;
   const int fin_blocks = (n_hist + 255) / 256 + 1;
-  // MF_PP_TTG / MF_PP_TTGG: the partonic channel of the records of this call is drawn by channel_kernel after the pass; it
-  // needs the cursor as it was before
-  const bool draw_channels = unw && d_records && capacity > 0 && n_events > 0 && (p->process == MF_PP_TTG || p->process == MF_PP_TTGG);
+  // cooperative / block processes: the records of this call are completed by record_kernel after the pass (momenta, partonic
+  // channel); it needs the cursor as it was before
+  const bool draw_channels = unw && d_records && capacity > 0 && n_events > 0 && mf::defers_record(p->process);
   cudaError_t e;
   if (draw_channels && (e = cudaMemcpyAsync(p->d_start, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st)) != cudaSuccess)
     return fail(p, MF_ECUDA, "record cursor snapshot", e);
@@ -162,9 +162,12 @@ int run_pass(mf_process* p, bool unw, const double* d_grid, uint64_t seed, uint3
     A.first_event = first_event;
     A.n_events = n_events;
     const int cb = p->prepass_blocks;       // one block per SM: accepted events are few
-    if (p->process == MF_PP_TTG) mf::channel_kernel<5><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start);
-    else mf::channel_kernel<7><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start);
-    if ((e = cudaGetLastError()) != cudaSuccess) return fail(p, MF_ECUDA, "channel kernel launch", e);
+    switch (p->process) {
+      case 2: mf::record_kernel<2><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start); break;
+      case 5: mf::record_kernel<5><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start); break;
+      default: mf::record_kernel<7><<<cb, mf::kThreads, 0, st>>>(p->P, A, p->d_start); break;
+    }
+    if ((e = cudaGetLastError()) != cudaSuccess) return fail(p, MF_ECUDA, "record kernel launch", e);
   }
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(p, MF_ECUDA, "finalize launch", e);
@@ -304,7 +307,7 @@ int mf_create_process(const mf_process_desc* d, mf_process** out) {
     if ((e = cudaMalloc(&p->d_quark, kQuarkChunk * sizeof(double))) != cudaSuccess) { free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM; }
     p->quark_cap = kQuarkChunk;
   }
-  if ((p->process == MF_PP_TTG || p->process == MF_PP_TTGG) && (e = cudaMalloc(&p->d_start, sizeof(unsigned long long))) != cudaSuccess) {
+  if (mf::defers_record(p->process) && (e = cudaMalloc(&p->d_start, sizeof(unsigned long long))) != cudaSuccess) {
     free_all(p); delete p; cudaGetLastError(); return MF_ENOMEM;
   }
   snprintf(p->err, sizeof(p->err), "ok");

@@ -339,7 +339,7 @@ constexpr int kThreads = 128;
 // tables in global memory; the gluon channel's term (the team's matrix element is not kept) is what the event's weight w
 // leaves after the quark terms: w = common x (gg term + sum of the signed quark terms).
 // (inlined: as an out-of-line function inside the fused pass, with nvcc 12.9 for sm_100a, it received its weight argument as 0,
-// by value or through a struct; inlined there it cost 12 % of the step, so it now runs in channel_kernel after the pass)
+// by value or through a struct; inlined there it cost 12 % of the step, so it now runs in record_kernel after the pass)
 __device__ __forceinline__ unsigned pp_ttj_channel(const Params& P, const PassArgs& A, const Event<5>& ev, double w, double v) {
   double f1[kMaxPartonTables], f2[kMaxPartonTables], asf;
   parton_densities<5>(P, A, A.pdf_lnx, A.pdf_row, ev, f1, f2, asf);
@@ -398,6 +398,11 @@ __device__ __forceinline__ unsigned pp_ttgg_channel(const Params& P, const PassA
   return (unsigned)(nt - 1);
 }
 
+// processes whose accepted records are completed by record_kernel after the pass: the one-warp-team kernels (g g -> t tbar g:
+// 9.58 -> 9.26 ms per 2^22 events; pp -> ttbar j: 20.3 -> 19.5 ms) and pp -> ttbar gg (its channel draw); g g -> t tbar g g and
+// g g -> t tbar g g g write their records in the pass (no gain from deferring, and one launch fewer per step)
+__host__ __device__ constexpr bool defers_record(int proc) { return proc == 2 || proc == 5 || proc == 7; }
+
 // Per-thread running sums of the pass (registers).
 struct Accum {
   double sum_w = 0.0, sum_w2 = 0.0, max_w = 0.0;
@@ -438,59 +443,72 @@ MF_D void accumulate_event(const Params& P, const PassArgs& A, const double* s_g
         ++acc.n_acc;
         unsigned long long slot = base + __popc(m & ((1u << lane) - 1u));
         if (A.records != nullptr && slot < A.capacity) {
-          // cooperative kernels (accepted events are rare, < 1 %, registers are not): regenerate the kinematics instead
-          // of keeping them live; the thread-per-event kernels pass the event they still hold
-          Event<PROC> ev;
-          if (ev_live != nullptr) {
-            ev = *ev_live;
-          } else {
-            Bins<PROC> b2;
-            DebugRow dbg = {nullptr, D, NF};
-            generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
-          }
-          double mom[NF + 2][4];
-          lab_momenta<PROC>(ev, mom);
-          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 16 + ((PROC == 4 || PROC == 5 || PROC == 7) ? 8 : 0)));
-#pragma unroll
-          for (int i = 0; i < NF + 2; ++i)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
+          constexpr int kRec = (NF + 2) * 32 + 16 + ((PROC == 4 || PROC == 5 || PROC == 7) ? 8 : 0);
+          double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)kRec);
           rec[4 * (NF + 2)] = w;
           reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1] = event;
-          if (PROC == 4) reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = channel;
-          // pp -> ttbar j, pp -> ttbar gg: the channel of the record is drawn by channel_kernel, next on the stream (the draw
-          // needs the quark matrix elements again: hundreds of registers of code that does not belong into this loop)
-          if (PROC == 5 || PROC == 7) reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = 0ull;
+          if constexpr (defers_record(PROC)) {
+            // the thread does not hold the event any more (registers), and accepted events are
+            // rare (< 1 %): record_kernel, next on the stream, regenerates the event from its id and fills in the momenta
+            // (and, for pp -> ttbar j / gg, the partonic channel); here only the weight and the id are written
+          } else {
+            // the thread-per-event kernels pass the event they still hold; the others regenerate it here
+            Event<PROC> ev;
+            if (ev_live != nullptr) {
+              ev = *ev_live;
+            } else {
+              Bins<PROC> b2;
+              DebugRow dbg = {nullptr, D, NF};
+              generate_event<PROC>(P, s_grid, A.seed, A.iteration, event, ev, b2, dbg);
+            }
+            double mom[NF + 2][4];
+            lab_momenta<PROC>(ev, mom);
+#pragma unroll
+            for (int i = 0; i < NF + 2; ++i)
+#pragma unroll
+              for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
+            if (PROC == 4) reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = channel;
+          }
         }
       }
     }
   }
 }
 
-// R20 / R22: the partonic channel of the records mf_unweight has just written, slots [*start, min(*A.count, A.capacity)):
-// thread = record; the event is regenerated from its id, the channel drawn from the record's weight and the event's accept
-// block.  Accepted events are rare (< 1 %), so this costs microseconds; inside the fused pass the same code cost 12 % of
-// pp -> ttbar j's step (registers and instruction cache of a loop that almost never runs it).
+// Completes the records an mf_unweight call of a cooperative / block process has just written (weight and event id), slots
+// [*start, min(*A.count, A.capacity)): thread = record; the event is regenerated from its id, its lab-frame momenta stored and,
+// for pp -> ttbar j / pp -> ttbar gg (R20 / R22), the partonic channel drawn from the record's weight and the event's accept
+// block.  Accepted events are rare (< 1 %), so this costs microseconds; inside the fused pass the same code cost registers
+// and instruction cache in a loop that almost never runs it (pp -> ttbar j: 20 % of the step with the channel draw).
 template <int PROC>
-__global__ void __launch_bounds__(kThreads) channel_kernel(const Params P, const PassArgs A, const unsigned long long* start) {
-  static_assert(PROC == 5 || PROC == 7, "processes whose channel draw needs the quark matrix elements");
+__global__ void __launch_bounds__(kThreads) record_kernel(const Params P, const PassArgs A, const unsigned long long* start) {
+  static_assert(defers_record(PROC), "thread-per-event kernels write their records themselves");
   constexpr int D = Traits<PROC>::D, NF = Traits<PROC>::NF;
+  constexpr int kRec = (NF + 2) * 32 + 16 + ((PROC == 5 || PROC == 7) ? 8 : 0);
   const unsigned long long first = *start, cnt = *A.count;
   const unsigned long long last = cnt < A.capacity ? cnt : A.capacity;
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   for (unsigned long long slot = first + (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; slot < last; slot += stride) {
-    double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)((NF + 2) * 32 + 24));
+    double* rec = reinterpret_cast<double*>(A.records + slot * (uint64_t)kRec);
     const double w = rec[4 * (NF + 2)];
     const unsigned long long event = reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 1];
     Event<PROC> ev;
     Bins<PROC> bins;
     DebugRow dbg = {nullptr, D, NF};
     generate_event<PROC>(P, A.grid, A.seed, A.iteration, event, ev, bins, dbg);
-    const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);      // words z, w: the channel draw
-    unsigned ch;
-    if constexpr (PROC == 5) ch = pp_ttj_channel(P, A, ev, w, uniform52(r.z, r.w));
-    else ch = pp_ttgg_channel(P, A, ev, w, uniform52(r.z, r.w));
-    reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = ch;
+    double mom[NF + 2][4];
+    lab_momenta<PROC>(ev, mom);
+#pragma unroll
+    for (int i = 0; i < NF + 2; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) rec[4 * i + c] = mom[i][c];
+    if constexpr (PROC == 5 || PROC == 7) {
+      const U4 r = philox_block(A.seed, A.iteration, event, 0xFFFFFFFFu);      // words z, w: the channel draw
+      unsigned ch;
+      if constexpr (PROC == 5) ch = pp_ttj_channel(P, A, ev, w, uniform52(r.z, r.w));
+      else ch = pp_ttgg_channel(P, A, ev, w, uniform52(r.z, r.w));
+      reinterpret_cast<unsigned long long*>(rec)[4 * (NF + 2) + 2] = ch;
+    }
   }
 }
 
