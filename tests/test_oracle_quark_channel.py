@@ -176,16 +176,17 @@ def qq_quadrature(P4):
     return val * 0.3894e9
 
 
-def test_vegas_quark_part_agrees_with_quadrature(P4, oracle_procs, qq_quadrature):
-    """whole chain: (process 4 - process 1) event by event on the same stream is the quark channel's integrand"""
+def test_vegas_quark_part_agrees_with_quadrature(P4, oracle_procs, oracle_pool, qq_quadrature):
+    """whole chain: (process 4 - process 1) event by event on the same stream is the quark channel's integrand
+    (the rows come from the multi-process oracle harness: the same single-threaded code on disjoint index ranges)"""
     n = 2 ** 15
     grid = W.uniform_grid(4)
     I, var = [], []
     for it in range(5):
         hist, res = P4.vegas_iterate(grid, 0, it, 0, n)
         if it >= 2:
-            r4 = P4.debug_eval(grid, 0, it, 0, n)
-            r1 = oracle_procs[1].debug_eval(grid, 0, it, 0, n)
+            r4 = oracle_pool.debug_eval(W.C5, grid, 0, it, 0, n)
+            r1 = oracle_pool.debug_eval(W.C1, grid, 0, it, 0, n)
             d = r4[:, 26] - r1[:, 26]
             I.append(d.mean())
             var.append(d.var(ddof=1) / n)
